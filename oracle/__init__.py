@@ -1,0 +1,196 @@
+"""ctypes loader for the fp64 CPU oracle (oracle/glad_oracle.c).
+
+TEST INFRASTRUCTURE, NOT PRODUCT CODE.  Only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference leg may import this package.  It
+shares nothing with paper_2504_01302_b200 (no import in either direction).
+
+`build()` compiles the C file with gcc (-O2, no fast-math, OpenMP over the batch).
+All array arguments are numpy; float32 inputs are the very arrays the CUDA path
+reads (the C code promotes them to double), outputs are float64.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "glad_oracle.c")
+_LIB = os.path.join(_HERE, "libglad_oracle.so")
+_lib = None
+
+NLENS = 26
+NDYN = 4
+FLAG_LENS_INVALID, FLAG_DYN_INVALID, FLAG_BIN_INVALID = 1, 2, 4
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _f32(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _ptr(a, ty):
+    return None if a is None else a.ctypes.data_as(C.POINTER(ty))
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(_LIB)
+        d, i, fp, dp, ip = C.c_double, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_double), C.POINTER(C.c_int32)
+        L.glad_oracle_num_threads.restype = i
+        L.glad_oracle_sersic_bn.restype = d
+        L.glad_oracle_sersic_bn.argtypes = [d]
+        L.glad_oracle_sersic.restype = d
+        L.glad_oracle_sersic.argtypes = [d] * 8
+        L.glad_oracle_epl_alpha.restype = None
+        L.glad_oracle_epl_alpha.argtypes = [d] * 5 + [dp, dp]
+        L.glad_oracle_deflection.restype = None
+        L.glad_oracle_deflection.argtypes = [dp, d, d, dp, dp]
+        L.glad_oracle_lens_image_batch.restype = i
+        L.glad_oracle_lens_image_batch.argtypes = [fp, i, i, i, i, d, d, d, fp, i, fp, fp, dp, dp, ip]
+        L.glad_oracle_jam_sigv2_point.restype = d
+        L.glad_oracle_jam_sigv2_point.argtypes = [d, d, d, i, dp, dp, dp, dp, i, dp, dp, dp, i, dp, dp]
+        L.glad_oracle_jam_vrms_batch.restype = i
+        L.glad_oracle_jam_vrms_batch.argtypes = [fp, i, fp, i, C.c_long, fp, i, C.c_long, fp, i, i, i, fp, fp,
+                                                 ip, i, fp, i, fp, fp, fp, fp, i, dp, dp, dp, dp, ip]
+        L.glad_oracle_kin_bins.restype = i
+        L.glad_oracle_kin_bins.argtypes = [dp, dp, i, i, ip, i, fp, i, fp, fp, dp, dp]
+        L.glad_oracle_joint.restype = None
+        L.glad_oracle_joint.argtypes = [dp, dp, i, dp]
+        L.glad_oracle_bh_theta2.restype = d
+        L.glad_oracle_bh_theta2.argtypes = [d, d, d]
+        _lib = L
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().glad_oracle_num_threads())
+
+
+def sersic_bn(n: float) -> float:
+    return float(lib().glad_oracle_sersic_bn(float(n)))
+
+
+def sersic(dx, dy, Ie, Re, n, q, phi, bn=None) -> float:
+    bn = sersic_bn(n) if bn is None else bn
+    return float(lib().glad_oracle_sersic(dx, dy, Ie, Re, n, q, phi, bn))
+
+
+def epl_alpha(x, y, thetaE, gamma, q):
+    ax, ay = C.c_double(), C.c_double()
+    lib().glad_oracle_epl_alpha(x, y, thetaE, gamma, q, C.byref(ax), C.byref(ay))
+    return ax.value, ay.value
+
+
+def deflection(params, thx, thy):
+    p = np.ascontiguousarray(params, dtype=np.float64)
+    assert p.size == NLENS
+    ax, ay = C.c_double(), C.c_double()
+    lib().glad_oracle_deflection(_ptr(p, C.c_double), thx, thy, C.byref(ax), C.byref(ay))
+    return ax.value, ay.value
+
+
+def bh_theta2(Mbh, Ddt_mpc, zd) -> float:
+    return float(lib().glad_oracle_bh_theta2(float(Mbh), float(Ddt_mpc), float(zd)))
+
+
+def lens_image_batch(lens, grid, psf, data=None, ivar=None, want_images=True):
+    """grid = dict(nx, ny, supersample, pix, x0, y0). Returns dict(images, chi2, flags)."""
+    lens = _f32(lens).reshape(-1, NLENS)
+    B = lens.shape[0]
+    nx, ny = int(grid["nx"]), int(grid["ny"])
+    psf = _f32(psf)
+    k = psf.shape[0]
+    data, ivar = _f32(data), _f32(ivar)
+    images = np.empty((B, ny, nx), np.float64) if want_images else None
+    chi2 = np.empty(B, np.float64)
+    flags = np.zeros(B, np.int32)
+    rc = lib().glad_oracle_lens_image_batch(
+        _ptr(lens, C.c_float), B, nx, ny, int(grid["supersample"]), float(grid["pix"]), float(grid["x0"]),
+        float(grid["y0"]), _ptr(psf, C.c_float), k, _ptr(data, C.c_float), _ptr(ivar, C.c_float),
+        _ptr(images, C.c_double), _ptr(chi2, C.c_double), _ptr(flags, C.c_int32))
+    if rc != 0:
+        raise ValueError("oracle: bad lens arguments")
+    return {"images": images, "chi2": chi2, "flags": flags}
+
+
+def jam_vrms_batch(dyn, lum_mge, mass_mge, beta, kin, want_maps=False):
+    """kin = dict(xs, ys, bin_id, nbins, kernel, vrms_obs, vrms_ivar, u_nodes, u_weights).
+    lum_mge / mass_mge: [n,3] (shared) or [B,n,3] (per vector). beta: [B] or [B,n_lum].
+    Returns dict(vrms, chi2, flags[, v2map, sbmap])."""
+    dyn = _f32(dyn).reshape(-1, NDYN)
+    B = dyn.shape[0]
+    lum, mass, beta = _f32(lum_mge), _f32(mass_mge), _f32(beta)
+    n_lum, n_mass = lum.shape[-2], mass.shape[-2]
+    lum_stride = 0 if lum.ndim == 2 else n_lum * 3
+    mass_stride = 0 if mass.ndim == 2 else n_mass * 3
+    per_g = 1 if beta.ndim == 2 else 0
+    xs, ys = _f32(kin["xs"]), _f32(kin["ys"])
+    nx, ny = xs.size, ys.size
+    bin_id = np.ascontiguousarray(kin["bin_id"], dtype=np.int32)
+    nbins = int(kin["nbins"])
+    kern = _f32(kin["kernel"])
+    vo, vi = _f32(kin.get("vrms_obs")), _f32(kin.get("vrms_ivar"))
+    un, uw = _f32(kin["u_nodes"]), _f32(kin["u_weights"])
+    vrms = np.empty((B, nbins), np.float64)
+    chi2 = np.empty(B, np.float64)
+    flags = np.zeros(B, np.int32)
+    v2map = np.empty((B, ny, nx), np.float64) if want_maps else None
+    sbmap = np.empty((B, ny, nx), np.float64) if want_maps else None
+    rc = lib().glad_oracle_jam_vrms_batch(
+        _ptr(dyn, C.c_float), B, _ptr(lum, C.c_float), n_lum, lum_stride, _ptr(mass, C.c_float), n_mass,
+        mass_stride, _ptr(beta, C.c_float), per_g, nx, ny, _ptr(xs, C.c_float), _ptr(ys, C.c_float),
+        _ptr(bin_id, C.c_int32), nbins, _ptr(kern, C.c_float), kern.shape[0], _ptr(vo, C.c_float),
+        _ptr(vi, C.c_float), _ptr(un, C.c_float), _ptr(uw, C.c_float), un.size, _ptr(vrms, C.c_double),
+        _ptr(chi2, C.c_double), _ptr(v2map, C.c_double), _ptr(sbmap, C.c_double), _ptr(flags, C.c_int32))
+    if rc != 0:
+        raise ValueError("oracle: bad jam arguments")
+    out = {"vrms": vrms, "chi2": chi2, "flags": flags}
+    if want_maps:
+        out["v2map"], out["sbmap"] = v2map, sbmap
+    return out
+
+
+def jam_sigv2_point(xp, yp, inc, sig_k, q_k, nu0_k, b_k, sig_j, q_j, rho0_j, u_nodes, u_weights) -> float:
+    """Raw quadrature at one sky point, all lengths pc, intrinsic (deprojected) tables."""
+    f = lambda a: np.ascontiguousarray(a, dtype=np.float64)
+    sig_k, q_k, nu0_k, b_k, sig_j, q_j, rho0_j, un, uw = map(
+        f, (sig_k, q_k, nu0_k, b_k, sig_j, q_j, rho0_j, u_nodes, u_weights))
+    P = lambda a: _ptr(a, C.c_double)
+    return float(lib().glad_oracle_jam_sigv2_point(
+        xp, yp, inc, sig_k.size, P(sig_k), P(q_k), P(nu0_k), P(b_k), sig_j.size, P(sig_j), P(q_j), P(rho0_j),
+        un.size, P(un), P(uw)))
+
+
+def kin_bins(sv2, sb, bin_id, nbins, kernel, vrms_obs=None, vrms_ivar=None):
+    """Rows a7+a8 on given fp64 maps [ny,nx]. Returns (vrms[nbins], chi2, bad)."""
+    sv2 = np.ascontiguousarray(sv2, dtype=np.float64)
+    sb = np.ascontiguousarray(sb, dtype=np.float64)
+    ny, nx = sv2.shape
+    bin_id = np.ascontiguousarray(bin_id, dtype=np.int32)
+    kern = _f32(kernel)
+    vo, vi = _f32(vrms_obs), _f32(vrms_ivar)
+    vr = np.empty(nbins, np.float64)
+    x2 = C.c_double(0.0)
+    bad = lib().glad_oracle_kin_bins(_ptr(sv2, C.c_double), _ptr(sb, C.c_double), nx, ny, _ptr(bin_id, C.c_int32),
+                                     nbins, _ptr(kern, C.c_float), kern.shape[0], _ptr(vo, C.c_float),
+                                     _ptr(vi, C.c_float), _ptr(vr, C.c_double), C.byref(x2))
+    return vr, x2.value, int(bad)
+
+
+def joint_loglike(chi2_lens, chi2_dyn):
+    a = np.ascontiguousarray(chi2_lens, dtype=np.float64)
+    b = np.ascontiguousarray(chi2_dyn, dtype=np.float64)
+    out = np.empty_like(a)
+    lib().glad_oracle_joint(_ptr(a, C.c_double), _ptr(b, C.c_double), a.size, _ptr(out, C.c_double))
+    return out

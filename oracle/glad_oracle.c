@@ -1,0 +1,488 @@
+/*
+ * glad_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, double-precision CPU statement of what the batched joint
+ * lensing + dynamics log-likelihood computes (arXiv 2504.01302, "GLaD").
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference leg may build, load or call this file.  It shares no code,
+ * header, table or helper with the CUDA path in paper_2504_01302_b200/csrc.
+ *
+ * Citations: "P:n" = /root/reference/PAPER.md line n.  Where the paper prints
+ * no formula the reading taken is listed in DESIGN.md ("Readings").
+ *
+ * No blocking, fusion, symmetry or separability is used anywhere: every ray,
+ * every PSF tap and every (node, mass Gaussian, luminous Gaussian, pixel)
+ * quadrature term is evaluated exactly as the formulas are written, in fp64.
+ * The only parallelism is an OpenMP `parallel for` over batch elements.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"):
+ *   EPL deflection ........ SIE closed form, kappa = div(alpha)/2 by finite
+ *                           differences vs Eq. B.1-B.3, curl = 0, alpha(theta_E)
+ *                           = theta_E at q = 1
+ *   shear, point mass ..... analytic; kappa = 0 by finite differences
+ *   Sersic ................ b_n vs scipy.special.gammaincinv, n = 1/2 Gaussian,
+ *                           total flux closed form
+ *   image / PSF / chi2 .... SIS ring, delta image, flux conservation, chi2 = k^2 N
+ *   JAM second moment ..... brute-force spherical Jeans, brute-force axisymmetric
+ *                           Jeans (anisotropic, inclined), Keplerian point mass,
+ *                           inclination independence, evenness, linearity
+ *   PSF / bins (kin) ...... constant-field invariance, delta kernel
+ *   joint ................. additivity, -inf propagation
+ * Overall numbers: PARITY UNPINNED against any published value -- the paper
+ * prints no model image, v_rms map or likelihood value for any parameter
+ * vector.
+ */
+#include <complex.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_NLENS 26
+#define ORACLE_NDYN 4
+
+/* flag bits (same meaning as include/glad.h, restated, not included) */
+#define FLAG_LENS_INVALID 1
+#define FLAG_DYN_INVALID 2
+#define FLAG_BIN_INVALID 4
+
+static const double PI = 3.14159265358979323846;
+/* G in (km/s)^2 pc / Msun -- paper silent; reading R-D1 */
+static const double G_NEWTON = 0.004301;
+/* BH Gaussian width in arcsec = the paper's central softening scale */
+static const double SIGMA_BH_ARCSEC = 0.01;
+
+int glad_oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------------ */
+/* Sersic b_n: exact root of P(2n, b) = 1/2 (regularised lower incomplete    */
+/* gamma).  DESIGN.md reading R-L7 (paper names Sersic only).         */
+/* ------------------------------------------------------------------------ */
+static double gammainc_P(double a, double x) {
+    if (x <= 0.0) return 0.0;
+    if (x < a + 1.0) { /* series: P = x^a e^-x / Gamma(a+1) * sum x^n / (a+1)...(a+n) */
+        double term = 1.0 / a, sum = term, ap = a;
+        for (int n = 0; n < 100000; ++n) {
+            ap += 1.0;
+            term *= x / ap;
+            sum += term;
+            if (fabs(term) < fabs(sum) * 1e-17) break;
+        }
+        return sum * exp(-x + a * log(x) - lgamma(a));
+    }
+    /* continued fraction for Q = 1 - P (modified Lentz) */
+    double tiny = 1e-300, b = x + 1.0 - a, c = 1.0 / tiny, d = 1.0 / b, h = d;
+    for (int i = 1; i < 100000; ++i) {
+        double an = -i * (i - a);
+        b += 2.0;
+        d = an * d + b; if (fabs(d) < tiny) d = tiny;
+        c = b + an / c; if (fabs(c) < tiny) c = tiny;
+        d = 1.0 / d;
+        double del = d * c;
+        h *= del;
+        if (fabs(del - 1.0) < 1e-16) break;
+    }
+    return 1.0 - exp(-x + a * log(x) - lgamma(a)) * h;
+}
+
+double glad_oracle_sersic_bn(double n) {
+    double a = 2.0 * n, lo = 0.0, hi = 2.0 * n + 20.0;
+    for (int it = 0; it < 200; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (gammainc_P(a, mid) < 0.5) lo = mid; else hi = mid;
+    }
+    return 0.5 * (lo + hi);
+}
+
+/* Elliptical Sersic, paper's elliptical radius R = sqrt(x^2 + y^2/q^2)
+ * (footnote P:234, Eq. B.2); (dx,dy) already relative to the centre. */
+double glad_oracle_sersic(double dx, double dy, double Ie, double Re, double n, double q,
+                          double phi, double bn) {
+    double c = cos(phi), s = sin(phi);
+    double x = dx * c + dy * s, y = -dx * s + dy * c;
+    double R = sqrt(x * x + y * y / (q * q));
+    return Ie * exp(-bn * (pow(R / Re, 1.0 / n) - 1.0));
+}
+
+/* ------------------------------------------------------------------------ */
+/* EPL deflection in the lens frame (major axis on x).  Paper convention      */
+/* App. B Eq. B.1-B.3; deflection "following Tessore & Metcalf    */
+/* (2015)", formula restated in DESIGN.md reading R-L3:               */
+/*   R_TM = sqrt(q^2 x^2 + y^2), b_TM = q b, b = (2/(1+q))^(1/(gamma-1)) th_E */
+/*   w = (q x + i y)/R_TM, t = gamma-1, f = (1-q)/(1+q)                       */
+/*   alpha = 2 b_TM/(1+q) (b_TM/R_TM)^(t-1) w sum_n a_n,                      */
+/*   a_0 = 1, a_n = a_{n-1} (-f w^2) (2n-(2-t))/(2n+(2-t))                    */
+/* Singular (r_soft = 0), R_TM^2 clamped below at (1e-6)^2.                   */
+/* ------------------------------------------------------------------------ */
+void glad_oracle_epl_alpha(double x, double y, double thetaE, double gamma, double q,
+                           double* ax, double* ay) {
+    double t = gamma - 1.0;
+    if (thetaE == 0.0) { *ax = 0.0; *ay = 0.0; return; } /* no mass: kappa = 0 everywhere */
+    double b = pow(2.0 / (1.0 + q), 1.0 / t) * thetaE;
+    double bTM = q * b;
+    double R2 = q * q * x * x + y * y;
+    if (R2 < 1e-12) R2 = 1e-12;
+    double R = sqrt(R2);
+    double complex w = (q * x + I * y) / R;
+    double f = (1.0 - q) / (1.0 + q);
+    double complex z = -f * w * w, an = 1.0, sum = 1.0;
+    for (int n = 1; n <= 500; ++n) {
+        an *= z * (2.0 * n - (2.0 - t)) / (2.0 * n + (2.0 - t));
+        sum += an;
+        if (cabs(an) < 1e-16) break;
+    }
+    double complex alpha = 2.0 * bTM / (1.0 + q) * pow(bTM / R, t - 1.0) * w * sum;
+    *ax = creal(alpha);
+    *ay = cimag(alpha);
+}
+
+/* Total deflection at image-plane position (thx, thy): EPL (rotated by phi_PA
+ * about the lens centre) + external shear (Eq. 49, origin = lens centre,
+ * reading R-L5) + point mass alpha = thE2 * D/|D|^2 (reading R-L6). */
+void glad_oracle_deflection(const double* p, double thx, double thy, double* ax, double* ay) {
+    double dx = thx - p[0], dy = thy - p[1];
+    double c = cos(p[5]), s = sin(p[5]);
+    double xl = dx * c + dy * s, yl = -dx * s + dy * c;
+    double axl, ayl;
+    glad_oracle_epl_alpha(xl, yl, p[2], p[3], p[4], &axl, &ayl);
+    double a_x = axl * c - ayl * s, a_y = axl * s + ayl * c;
+    double c2 = cos(2.0 * p[7]), s2 = sin(2.0 * p[7]);
+    a_x += p[6] * (dx * c2 + dy * s2);
+    a_y += p[6] * (dx * s2 - dy * c2);
+    double r2 = dx * dx + dy * dy;
+    if (r2 < 1e-12) r2 = 1e-12;
+    a_x += p[8] * dx / r2;
+    a_y += p[8] * dy / r2;
+    *ax = a_x;
+    *ay = a_y;
+}
+
+static int lens_params_valid(const double* p) {
+    if (!(p[2] >= 0.0)) return 0;                       /* theta_E */
+    if (!(p[3] > 1.0 && p[3] < 3.0)) return 0;          /* gamma in (1,3) */
+    if (!(p[4] > 0.0 && p[4] <= 1.0)) return 0;         /* q */
+    if (!(p[8] >= 0.0)) return 0;                       /* theta_E,BH^2 */
+    const int off[3] = {11, 16, 21};                    /* Ie,Re,n,q,phi of the 3 Sersics */
+    for (int c = 0; c < 3; ++c) {
+        const double* s = p + off[c];
+        if (s[0] == 0.0) continue;                      /* disabled component */
+        if (!(s[1] > 0.0 && s[2] > 0.0 && s[3] > 0.0 && s[3] <= 1.0)) return 0;
+    }
+    return 1;
+}
+
+/*
+ * Lensing half, for B parameter vectors.
+ *   lens   [B,26] float32 parameter vectors (layout in include/glad.h, restated in DESIGN.md)
+ *   grid   nx, ny, supersample s, pixel size pix, (x0,y0) = centre of pixel (0,0)   (reading R-L1)
+ *   psf    [kpsf,kpsf] float32, odd kpsf, NOT renormalised                         (reading R-L8)
+ *   data, ivar [ny,nx] float32
+ * Outputs (either may be NULL): images [B,ny,nx] fp64 PSF-convolved model; chi2 [B] fp64;
+ * flags [B] int32 (FLAG_LENS_INVALID -> image NaN, chi2 +inf).
+ */
+int glad_oracle_lens_image_batch(const float* lens, int B, int nx, int ny, int s, double pix,
+                                 double x0, double y0, const float* psf, int kpsf,
+                                 const float* data, const float* ivar, double* images,
+                                 double* chi2, int32_t* flags) {
+    if (B < 0 || nx <= 0 || ny <= 0 || s <= 0 || kpsf <= 0 || (kpsf % 2) == 0) return -1;
+    int npx = nx * ny, c = kpsf / 2;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int b = 0; b < B; ++b) {
+        double p[ORACLE_NLENS];
+        for (int i = 0; i < ORACLE_NLENS; ++i) p[i] = (double)lens[(size_t)b * ORACLE_NLENS + i];
+        if (flags) flags[b] = 0;
+        if (!lens_params_valid(p)) {
+            if (flags) flags[b] |= FLAG_LENS_INVALID;
+            if (images) for (int i = 0; i < npx; ++i) images[(size_t)b * npx + i] = NAN;
+            if (chi2) chi2[b] = INFINITY;
+            continue;
+        }
+        double bn_s = p[11] != 0.0 ? glad_oracle_sersic_bn(p[13]) : 0.0;
+        double bn_1 = p[16] != 0.0 ? glad_oracle_sersic_bn(p[18]) : 0.0;
+        double bn_2 = p[21] != 0.0 ? glad_oracle_sersic_bn(p[23]) : 0.0;
+        double* binned = (double*)malloc(sizeof(double) * npx);
+        /* a1-a3: ray-shoot every sub-pixel centre (Eq. 33), evaluate light, mean (R-L2) */
+        for (int iy = 0; iy < ny; ++iy)
+            for (int ix = 0; ix < nx; ++ix) {
+                double acc = 0.0;
+                for (int sb = 0; sb < s; ++sb)
+                    for (int sa = 0; sa < s; ++sa) {
+                        double thx = x0 + ix * pix + ((sa + 0.5) / s - 0.5) * pix;
+                        double thy = y0 + iy * pix + ((sb + 0.5) / s - 0.5) * pix;
+                        double ax, ay;
+                        glad_oracle_deflection(p, thx, thy, &ax, &ay);
+                        double bx = thx - ax, by = thy - ay; /* beta = theta - alpha */
+                        double v = 0.0;
+                        if (p[11] != 0.0)
+                            v += glad_oracle_sersic(bx - p[9], by - p[10], p[11], p[12], p[13],
+                                                    p[14], p[15], bn_s);
+                        if (p[16] != 0.0)
+                            v += glad_oracle_sersic(thx - p[0], thy - p[1], p[16], p[17], p[18],
+                                                    p[19], p[20], bn_1);
+                        if (p[21] != 0.0)
+                            v += glad_oracle_sersic(thx - p[0], thy - p[1], p[21], p[22], p[23],
+                                                    p[24], p[25], bn_2);
+                        acc += v;
+                    }
+                binned[iy * nx + ix] = acc / (double)(s * s);
+            }
+        /* a4: m = binned (*) PSF, "same", zero outside (Eq. 38, R-L8); chi2 (Eq. 48) */
+        double x2 = 0.0;
+        for (int iy = 0; iy < ny; ++iy)
+            for (int ix = 0; ix < nx; ++ix) {
+                double m = 0.0;
+                for (int dy = 0; dy < kpsf; ++dy)
+                    for (int dx = 0; dx < kpsf; ++dx) {
+                        int sy = iy - (dy - c), sx = ix - (dx - c);
+                        if (sy < 0 || sy >= ny || sx < 0 || sx >= nx) continue;
+                        m += (double)psf[dy * kpsf + dx] * binned[sy * nx + sx];
+                    }
+                if (images) images[(size_t)b * npx + iy * nx + ix] = m;
+                if (data && ivar) {
+                    double r = (double)data[iy * nx + ix] - m;
+                    x2 += (double)ivar[iy * nx + ix] * r * r;
+                }
+            }
+        if (chi2) chi2[b] = x2;
+        free(binned);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------ */
+/* Dynamics half.                                                             */
+/* ------------------------------------------------------------------------ */
+
+/*
+ * Integrand-summed second moment at ONE sky position, lengths in pc:
+ * cylindrically-aligned axisymmetric JAM, single quadrature over u in (0,1)
+ * (paper defers to Cappellari at P:228; reading R-D1 states it):
+ *
+ *  [Sigma v2_los](x',y') = 4 pi^{3/2} G  sum_u w_u sum_k sum_j nu0_k q_j rho0_j u^2
+ *        [ s_k^2 q_k^2 (cos^2 i + b_k sin^2 i) + D x'^2 sin^2 i ]
+ *        / [ (1 - C u^2) sqrt( (A + B cos^2 i) [1 - (1-q_j^2) u^2] ) ]
+ *        exp{ -A [ x'^2 + y'^2 (A+B)/(A + B cos^2 i) ] }
+ *  A = (u^2/s_j^2 + 1/s_k^2)/2
+ *  B = { (1-q_k^2)/(s_k^2 q_k^2) + (1-q_j^2) u^4 / (s_j^2 [1-(1-q_j^2)u^2]) } / 2
+ *  C = 1 - q_j^2 - s_k^2 q_k^2 / s_j^2
+ *  D = 1 - b_k q_k^2 - [ (1-b_k) C + (1-q_j^2) b_k ] u^2
+ *
+ * k = luminous Gaussian (sigma_k, intrinsic q_k, nu0_k, b_k = 1/(1-beta_z,k)),
+ * j = mass Gaussian (sigma_j, q_j, rho0_j).
+ */
+double glad_oracle_jam_sigv2_point(double xp, double yp, double inc, int nl, const double* sig_k,
+                                   const double* q_k, const double* nu0_k, const double* b_k,
+                                   int nm, const double* sig_j, const double* q_j,
+                                   const double* rho0_j, int nu, const double* u_nodes,
+                                   const double* u_weights) {
+    double ci = cos(inc), si = sin(inc), ci2 = ci * ci, si2 = si * si;
+    double total = 0.0;
+    for (int iu = 0; iu < nu; ++iu) {
+        double u = u_nodes[iu], u2 = u * u, node = 0.0;
+        for (int k = 0; k < nl; ++k)
+            for (int j = 0; j < nm; ++j) {
+                double sk2 = sig_k[k] * sig_k[k], sj2 = sig_j[j] * sig_j[j];
+                double qk2 = q_k[k] * q_k[k], qj2 = q_j[j] * q_j[j];
+                double g = 1.0 - (1.0 - qj2) * u2;
+                double A = 0.5 * (u2 / sj2 + 1.0 / sk2);
+                double Bc = 0.5 * ((1.0 - qk2) / (sk2 * qk2) + (1.0 - qj2) * u2 * u2 / (sj2 * g));
+                double C = 1.0 - qj2 - sk2 * qk2 / sj2;
+                double D = 1.0 - b_k[k] * qk2 - ((1.0 - b_k[k]) * C + (1.0 - qj2) * b_k[k]) * u2;
+                double E = A + Bc * ci2;
+                double numer = sk2 * qk2 * (ci2 + b_k[k] * si2) + D * xp * xp * si2;
+                double denom = (1.0 - C * u2) * sqrt(E * g);
+                double ex = exp(-A * (xp * xp + yp * yp * (A + Bc) / E));
+                node += nu0_k[k] * q_j[j] * rho0_j[j] * u2 * numer / denom * ex;
+            }
+        total += u_weights[iu] * node;
+    }
+    return 4.0 * pow(PI, 1.5) * G_NEWTON * total;
+}
+
+/* Deprojection of one Gaussian (Eq. 22, Eq. 23/25 P:176,186):
+ * q = sqrt(q'^2 - cos^2 i)/sin i ; dens0 = surf0 q' / (q sigma sqrt(2 pi)).
+ * Returns 0 if not deprojectable. */
+static int deproject(double surf0, double sigma_pc, double qp, double inc, double* q,
+                     double* dens0) {
+    double ci = cos(inc), si = sin(inc);
+    double d = qp * qp - ci * ci;
+    if (!(d > 0.0) || !(si > 0.0) || !(qp > 0.0) || !(sigma_pc > 0.0)) return 0;
+    *q = sqrt(d) / si;
+    *dens0 = surf0 * qp / (*q * sigma_pc * sqrt(2.0 * PI));
+    return 1;
+}
+
+/*
+ * a7 + a8 on given maps: num = Sv2 (*) K, den = S (*) K, true convolution,
+ * "same" size, zero outside (Eq. 27, reading R-D6); V2_l = sum_{p in l} num / sum_{p in l} den;
+ * v_l = sqrt(V2_l) (Eq. 28); chi2_D = sum_l ivar_l (obs_l - v_l)^2 (Eq. 32, diagonal
+ * covariance, reading R-D7).  Returns 1 if any bin is empty or has V2 < 0 (v = NaN there).
+ */
+int glad_oracle_kin_bins(const double* sv2, const double* sb, int nx, int ny, const int32_t* bin_id,
+                         int nbins, const float* kern, int kk, const float* vrms_obs,
+                         const float* vrms_ivar, double* vrms, double* chi2) {
+    int c = kk / 2, bad = 0;
+    double* bnum = calloc(nbins, sizeof(double));
+    double* bden = calloc(nbins, sizeof(double));
+    int* bcnt = calloc(nbins, sizeof(int));
+    for (int iy = 0; iy < ny; ++iy)
+        for (int ix = 0; ix < nx; ++ix) {
+            int l = bin_id[iy * nx + ix];
+            if (l < 0 || l >= nbins) continue;
+            double num = 0.0, den = 0.0;
+            for (int dy = 0; dy < kk; ++dy)
+                for (int dx = 0; dx < kk; ++dx) {
+                    int sy = iy - (dy - c), sx = ix - (dx - c);
+                    if (sy < 0 || sy >= ny || sx < 0 || sx >= nx) continue;
+                    double w = kern[dy * kk + dx];
+                    num += w * sv2[sy * nx + sx];
+                    den += w * sb[sy * nx + sx];
+                }
+            bnum[l] += num;
+            bden[l] += den;
+            bcnt[l] += 1;
+        }
+    double x2 = 0.0;
+    for (int l = 0; l < nbins; ++l) {
+        double v2 = (bcnt[l] > 0 && bden[l] > 0.0) ? bnum[l] / bden[l] : NAN;
+        double v = (v2 >= 0.0) ? sqrt(v2) : NAN;
+        if (!(v == v)) bad = 1;
+        if (vrms) vrms[l] = v;
+        if (vrms_obs && vrms_ivar) {
+            double r = (double)vrms_obs[l] - v;
+            x2 += (double)vrms_ivar[l] * r * r;
+        }
+    }
+    if (chi2) *chi2 = x2;
+    free(bnum); free(bden); free(bcnt);
+    return bad;
+}
+
+/*
+ * Dynamics half, for B parameter vectors.
+ *   dyn      [B,4] float32 {inclination rad, D_d Mpc, M_BH Msun, Upsilon}
+ *   lum_mge  [.,n_lum,3] float32 rows {I0 Lsun/pc^2, sigma' arcsec, q'}; lum_stride floats
+ *            between vectors (0 = one table shared by all)
+ *   mass_mge [.,n_mass,3] likewise {Sigma0 Msun/pc^2, sigma' arcsec, q'}
+ *   beta     [B,n_lum] (beta_per_gaussian) or [B] : beta_z,k  (reading R-D2)
+ *   sky grid xs[nx], ys[ny] arcsec, galaxy-aligned tensor grid (reading R-D5)
+ *   bin_id   [ny,nx] int32 in [0,nbins) or -1; kern [kk,kk] float32 odd kk
+ *   vrms_obs, vrms_ivar [nbins]; u_nodes, u_weights [nu]  (reading R-D4)
+ * Outputs (may be NULL): vrms [B,nbins], chi2 [B], v2map [B,ny,nx] = raw Sigma*v2_los map,
+ * sbmap [B,ny,nx] = Sigma map, flags [B].
+ */
+int glad_oracle_jam_vrms_batch(const float* dyn, int B, const float* lum_mge, int n_lum,
+                               long lum_stride, const float* mass_mge, int n_mass,
+                               long mass_stride, const float* beta, int beta_per_gaussian, int nx,
+                               int ny, const float* xs, const float* ys, const int32_t* bin_id,
+                               int nbins, const float* kern, int kk, const float* vrms_obs,
+                               const float* vrms_ivar, const float* u_nodes,
+                               const float* u_weights, int nu, double* vrms, double* chi2,
+                               double* v2map, double* sbmap, int32_t* flags) {
+    if (B < 0 || n_lum <= 0 || n_mass < 0 || nx <= 0 || ny <= 0 || nbins <= 0 || kk <= 0 ||
+        (kk % 2) == 0 || nu <= 0)
+        return -1;
+    int npx = nx * ny;
+    double* un = (double*)malloc(sizeof(double) * nu);
+    double* uw = (double*)malloc(sizeof(double) * nu);
+    for (int i = 0; i < nu; ++i) { un[i] = u_nodes[i]; uw[i] = u_weights[i]; }
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int b = 0; b < B; ++b) {
+        double inc = dyn[b * ORACLE_NDYN + 0], Dd = dyn[b * ORACLE_NDYN + 1];
+        double Mbh = dyn[b * ORACLE_NDYN + 2], ups = dyn[b * ORACLE_NDYN + 3];
+        double pc_per_arcsec = Dd * PI / 0.648; /* D_d[Mpc] 1e6 pi/648000 */
+        const float* lt = lum_mge + (size_t)b * lum_stride;
+        const float* mt = mass_mge + (size_t)b * mass_stride;
+        int nm = n_mass + (Mbh > 0.0 ? 1 : 0);
+        double *sk = malloc(sizeof(double) * n_lum), *qk = malloc(sizeof(double) * n_lum),
+               *nu0 = malloc(sizeof(double) * n_lum), *bk = malloc(sizeof(double) * n_lum),
+               *sj = malloc(sizeof(double) * (nm + 1)), *qj = malloc(sizeof(double) * (nm + 1)),
+               *rho0 = malloc(sizeof(double) * (nm + 1));
+        double* sv2 = malloc(sizeof(double) * npx);
+        double* sb = malloc(sizeof(double) * npx);
+        int ok = (Dd > 0.0) && (Mbh >= 0.0);
+        for (int k = 0; k < n_lum && ok; ++k) {
+            sk[k] = (double)lt[3 * k + 1] * pc_per_arcsec;
+            ok = deproject((double)lt[3 * k + 0], sk[k], (double)lt[3 * k + 2], inc, &qk[k], &nu0[k]);
+            double bz = beta_per_gaussian ? (double)beta[(size_t)b * n_lum + k] : (double)beta[b];
+            if (!(bz < 1.0)) ok = 0;
+            bk[k] = 1.0 / (1.0 - bz);
+        }
+        for (int j = 0; j < n_mass && ok; ++j) {
+            sj[j] = (double)mt[3 * j + 1] * pc_per_arcsec;
+            ok = deproject(ups * (double)mt[3 * j + 0], sj[j], (double)mt[3 * j + 2], inc, &qj[j],
+                           &rho0[j]);
+        }
+        if (ok && Mbh > 0.0) { /* reading R-D3: BH = one round Gaussian of sigma 0.01" */
+            sj[n_mass] = SIGMA_BH_ARCSEC * pc_per_arcsec;
+            double surf0 = Mbh / (2.0 * PI * sj[n_mass] * sj[n_mass]);
+            ok = deproject(surf0, sj[n_mass], 1.0, inc, &qj[n_mass], &rho0[n_mass]);
+        }
+        int32_t fl = 0;
+        if (!ok) {
+            fl |= FLAG_DYN_INVALID;
+            if (vrms) for (int l = 0; l < nbins; ++l) vrms[(size_t)b * nbins + l] = NAN;
+            if (chi2) chi2[b] = INFINITY;
+            if (v2map) for (int i = 0; i < npx; ++i) v2map[(size_t)b * npx + i] = NAN;
+            if (sbmap) for (int i = 0; i < npx; ++i) sbmap[(size_t)b * npx + i] = NAN;
+        } else {
+            /* a6: quadrature at every pixel centre; Sigma map (Eq. 21) */
+            for (int iy = 0; iy < ny; ++iy)
+                for (int ix = 0; ix < nx; ++ix) {
+                    double xa = xs[ix], ya = ys[iy]; /* arcsec */
+                    sv2[iy * nx + ix] = glad_oracle_jam_sigv2_point(
+                        xa * pc_per_arcsec, ya * pc_per_arcsec, inc, n_lum, sk, qk, nu0, bk, nm, sj,
+                        qj, rho0, nu, un, uw);
+                    double sbv = 0.0;
+                    for (int k = 0; k < n_lum; ++k) {
+                        double s = lt[3 * k + 1], qp = lt[3 * k + 2];
+                        sbv += (double)lt[3 * k + 0] *
+                               exp(-(xa * xa + ya * ya / (qp * qp)) / (2.0 * s * s));
+                    }
+                    sb[iy * nx + ix] = sbv;
+                }
+            if (v2map) memcpy(v2map + (size_t)b * npx, sv2, sizeof(double) * npx);
+            if (sbmap) memcpy(sbmap + (size_t)b * npx, sb, sizeof(double) * npx);
+            /* a7 + a8 */
+            double* vout = malloc(sizeof(double) * nbins);
+            double x2 = 0.0;
+            int bad = glad_oracle_kin_bins(sv2, sb, nx, ny, bin_id, nbins, kern, kk, vrms_obs, vrms_ivar,
+                                           vout, &x2);
+            if (bad) fl |= FLAG_BIN_INVALID;
+            if (vrms) memcpy(vrms + (size_t)b * nbins, vout, sizeof(double) * nbins);
+            if (chi2) chi2[b] = bad ? INFINITY : x2;
+            free(vout);
+        }
+        if (flags) flags[b] = fl;
+        free(sk); free(qk); free(nu0); free(bk); free(sj); free(qj); free(rho0);
+        free(sv2); free(sb);
+    }
+    free(un); free(uw);
+    return 0;
+}
+
+/* Joint: lnL = -(chi2_L + chi2_D)/2, no normalisation constant (Eq. 52-53
+ * restricted to the pixel term and chi2_dyn; R-J1); -inf where either half is invalid. */
+void glad_oracle_joint(const double* chi2_lens, const double* chi2_dyn, int B, double* loglike) {
+    for (int b = 0; b < B; ++b) {
+        double s = chi2_lens[b] + chi2_dyn[b];
+        loglike[b] = (isfinite(s)) ? -0.5 * s : -INFINITY;
+    }
+}
+
+/* theta_E,BH^2 [arcsec^2] = 4 G M (1+z_d) / (c^2 D_dt), from Eq. 4 P:75 (host helper). */
+double glad_oracle_bh_theta2(double Mbh_msun, double Ddt_mpc, double zd) {
+    const double c_kms = 299792.458;
+    double rad2 = 4.0 * G_NEWTON * Mbh_msun * (1.0 + zd) / (c_kms * c_kms * Ddt_mpc * 1e6);
+    double arcsec_per_rad = 648000.0 / PI;
+    return rad2 * arcsec_per_rad * arcsec_per_rad;
+}
