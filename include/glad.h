@@ -1,0 +1,185 @@
+/*
+ * glad.h -- C ABI of libglad: batched joint lensing + dynamics log-likelihood on one
+ * NVIDIA B200 (sm_100a).  Method: arXiv 2504.01302 ("GLaD"); "P:n" = PAPER.md line n;
+ * "R-xx" = a reading listed in DESIGN.md where the paper prints no formula.
+ *
+ * Conventions common to every call
+ *   - All `d_` pointers are DEVICE pointers owned by the caller.  The library never
+ *     allocates or frees caller-visible memory; a context keeps grow-only device scratch.
+ *     Static-data pointers passed to glad_set_* are BORROWED: keep them alive and unchanged
+ *     until they are replaced or the context is destroyed.
+ *   - Batch calls only ENQUEUE work on the context's stream and return; no host sync, no
+ *     implicit D2H copy.  glad_set_kin_data is the one exception (documented there).
+ *   - Errors detectable on the host return a negative glad_status at once; a CUDA
+ *     launch/runtime error returns GLAD_ECUDA with the CUDA text in glad_last_error().
+ *     No exceptions, no exit(), no printing.  There is no CPU fallback.
+ *   - A physically invalid parameter VECTOR is not an error: its outputs are
+ *     lnL = -INFINITY, chi2 = +INFINITY, v_rms/image = NaN and a bit is set in d_flags[b].
+ *   - Angles in radians counter-clockwise from +x (Table 3 note); lengths in arcsec.
+ */
+#ifndef GLAD_H
+#define GLAD_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct glad_ctx glad_ctx; /* opaque */
+
+typedef enum {
+    GLAD_OK = 0,
+    GLAD_EINVAL = -1, /* null pointer / bad scalar argument */
+    GLAD_ESHAPE = -2, /* size outside what the kernels support (see each call) */
+    GLAD_ECUDA = -3,  /* CUDA runtime error; text in glad_last_error */
+    GLAD_ENOMEM = -4, /* scratch allocation failed */
+    GLAD_ESTATE = -5  /* static data for this call not set */
+} glad_status;
+
+/* per-vector flag bits written to d_flags */
+#define GLAD_FLAG_LENS_INVALID 1 /* theta_E<0, gamma not in (1,3), q not in (0,1], Sersic R_e,n,q <= 0 */
+#define GLAD_FLAG_DYN_INVALID 2  /* not deprojectable (Eq. 22), D_d<=0, M_BH<0, beta_z>=1 */
+#define GLAD_FLAG_BIN_INVALID 4  /* a bin is empty or has V^2 < 0 (negative density) */
+
+/*
+ * Lens parameter vector, GLAD_NLENS floats:
+ *   [0..5]   EPL          x_l, y_l, theta_E, gamma, q, phi_PA    (App. B Eq. B.1-B.3; R-L3:
+ *                         singular, r_soft = 0)
+ *   [6..7]   ext. shear   gamma_ext, phi_ext, origin at the lens centre (Eq. 49; R-L5)
+ *   [8]      point mass   theta_E,BH^2 [arcsec^2]                 (R-L6; see glad_bh_theta2)
+ *   [9..15]  source       x_s, y_s, I_e, R_e, n, q_s, phi_s   elliptical Sersic at beta (R-L7)
+ *   [16..20] lens light 1 I_e, R_e, n, q, phi   centred on the lens centre, evaluated at theta
+ *   [21..25] lens light 2 I_e, R_e, n, q, phi   (I_e = 0 disables a component)
+ * Elliptical radius R = sqrt(x^2 + y^2/q^2) everywhere (Eq. B.2).
+ */
+#define GLAD_NLENS 26
+/* Dynamics parameter vector: inclination [rad], D_d [Mpc], M_BH [Msun], Upsilon (multiplies the
+ * mass-MGE surface densities, not the BH). */
+#define GLAD_NDYN 4
+/* MGE table row: surface density [Lsun/pc^2 or Msun/pc^2], sigma' [arcsec], q' (Eq. 21, 24 P:166,182) */
+#define GLAD_MGE_ROW 3
+
+/* limits of the kernels (GLAD_ESHAPE beyond them) */
+#define GLAD_MAX_IMAGE_PIXELS 40000 /* nx*ny of the lens image (staged whole in shared memory) */
+#define GLAD_MAX_PSF 31             /* kpsf and kk */
+#define GLAD_MAX_GAUSS 64           /* n_lum, n_mass (+1 for the BH) */
+#define GLAD_MAX_SKY 256            /* nx, ny of the kinematic grid */
+#define GLAD_MAX_NODES 1024
+#define GLAD_MAX_BINS 1024
+
+/* Create a context on `device` whose work is enqueued on `cuda_stream` (a cudaStream_t, borrowed;
+ * NULL = the legacy default stream).  Returns GLAD_ECUDA if the device is not sm_100. */
+glad_status glad_create(glad_ctx** out, int device, void* cuda_stream);
+void glad_destroy(glad_ctx* ctx);
+/* Context-owned string describing the last error on this context ("" if none). Never free it. */
+const char* glad_last_error(const glad_ctx* ctx);
+/* Library version string and the symbols it exports (static). */
+const char* glad_version(void);
+
+/* Image grid: pixel (iy,ix) centre at (x0 + ix*pix, y0 + iy*pix); row index grows with +y (R-L1).
+ * Each pixel is the mean of supersample^2 sub-pixel samples at offsets ((a+1/2)/s - 1/2)*pix (R-L2). */
+typedef struct {
+    int nx, ny, supersample;
+    float pix, x0, y0;
+} glad_image_grid;
+
+/* Static lensing data.  d_data, d_ivar: [ny,nx] (ivar = 1/sigma^2, 0 masks a pixel); either may be NULL
+ * if chi2 is never requested.  d_psf: [kpsf,kpsf], kpsf odd <= GLAD_MAX_PSF, used as given (not
+ * renormalised); the model is the TRUE convolution m[y,x] = sum psf[dy,dx] img[y-(dy-c), x-(dx-c)],
+ * c = kpsf/2, zero outside the image (Eq. 38, (N_d,N_d) Table 1; R-L8).  The PSF is copied
+ * into the context (on the stream); data/ivar are borrowed. */
+glad_status glad_set_image_data(glad_ctx* ctx, const glad_image_grid* grid, const float* d_data,
+                                const float* d_ivar, const float* d_psf, int kpsf);
+
+/* Kinematic sky grid: tensor product xs[ix] x ys[iy] in the galaxy-aligned frame, x' = projected major
+ * axis (R-D5), pixel centres, arcsec. */
+typedef struct {
+    int nx, ny;
+    const float* d_xs;
+    const float* d_ys;
+} glad_sky_grid;
+
+/* Static kinematic data.  d_bin_id [ny,nx] in [0,nbins) or -1 (unused spaxel); d_kernel [kk,kk], kk odd
+ * <= GLAD_MAX_PSF = PSF_kin (x) pixel aperture, applied to numerator and denominator of Eq. 27
+ * with the same true-convolution / zero-pad convention as the image PSF (R-D6); d_vrms_obs, d_vrms_ivar
+ * [nbins] (may be NULL if chi2 is never requested); d_u_nodes, d_u_weights [nu] = quadrature rule on
+ * u in (0,1) (R-D4).  All pointers borrowed.
+ * SYNCHRONOUS (setup call): copies xs, ys and bin_id to the host once to detect a grid that is mirror-
+ * symmetric about x' = 0 and/or y' = 0 (then only one half per axis is integrated -- the integrand is even),
+ * validates the bin ids, and precomputes the static bin x kernel weights on the device.  The folded grid may
+ * have at most 512 tiles of 8x8 pixels (GLAD_ESHAPE otherwise). */
+glad_status glad_set_kin_data(glad_ctx* ctx, const glad_sky_grid* grid, const int32_t* d_bin_id,
+                              int nbins, const float* d_kernel, int kk, const float* d_vrms_obs,
+                              const float* d_vrms_ivar, const float* d_u_nodes,
+                              const float* d_u_weights, int nu);
+
+/*
+ * Lensing half.  For each of the B vectors: ray-shoot every sub-pixel centre
+ * theta through EPL + shear + point mass, beta = theta - alpha (Eq. 33); evaluate the Sersic
+ * source at beta and the lens light at theta; average to pixels; convolve with the PSF; and reduce
+ * chi2_L = sum ivar (data - model)^2 (Eq. 48 P:374 with the pixel term of Eq. 37, diagonal C_d).
+ *   d_lens_params [B,GLAD_NLENS]; d_images [B,ny,nx] or NULL; d_chi2 [B] or NULL; d_flags [B] or NULL
+ *   (flags are OVERWRITTEN with the lens bits).
+ * GLAD_ESTATE if glad_set_image_data was not called (or d_chi2 != NULL without data/ivar).
+ */
+glad_status glad_lens_image_batch(glad_ctx* ctx, const float* d_lens_params, int B, float* d_images,
+                                  float* d_chi2, int32_t* d_flags);
+
+/*
+ * Dynamics half (rows a5-a8).  Cylindrically-aligned axisymmetric Jeans model on MGEs (the paper defers
+ * the formula to Cappellari at P:228; R-D1 states it): for every sky pixel
+ *   [Sigma v_los^2](x',y') = 4 pi^{3/2} G sum_u w_u sum_k sum_j T(u,j,k; x',y')
+ * over quadrature nodes u, luminous Gaussians k (deprojected by Eq. 22-23; b_k = 1/(1-beta_z,k),
+ * R-D2) and mass Gaussians j (Eq. 25, times Upsilon) plus, if M_BH > 0, one round Gaussian of
+ * sigma = 0.01" and mass M_BH (R-D3); Sigma from Eq. 21; then Eq. 27-28 with the
+ * kernel and bins of glad_set_kin_data, and chi2_D = sum_l ivar_l (obs_l - v_l)^2 (Eq. 32; R-D7).
+ *   d_dyn_params [B,GLAD_NDYN]
+ *   d_lum_mge  rows {I0, sigma', q'} x n_lum ; lum_stride = floats between consecutive vectors, 0 = shared
+ *   d_mass_mge rows {Sigma0, sigma', q'} x n_mass (n_mass may be 0) ; mass_stride likewise
+ *   d_beta [B,n_lum] if beta_per_gaussian else [B]
+ *   d_vrms [B,nbins] or NULL ; d_chi2 [B] or NULL ; d_v2map [B,ny,nx] or NULL (raw Sigma*v_los^2 map,
+ *   (km/s)^2 Lsun/pc^2) ; d_flags [B] or NULL (OVERWRITTEN with the dynamics bits).
+ */
+glad_status glad_jam_vrms_batch(glad_ctx* ctx, const float* d_dyn_params, int B,
+                                const float* d_lum_mge, int n_lum, long lum_stride,
+                                const float* d_mass_mge, int n_mass, long mass_stride,
+                                const float* d_beta, int beta_per_gaussian, float* d_vrms,
+                                float* d_chi2, float* d_v2map, int32_t* d_flags);
+
+/*
+ * Joint (row a9): both halves on the context stream, then lnL[b] = -(chi2_L[b] + chi2_D[b])/2 with no
+ * normalisation constant (Eq. 52-53 P:410-416 restricted to the pixel term and chi2_dyn; the image-
+ * position and time-delay terms are the paper's CPU terms), -INFINITY where a half is invalid.
+ *   d_loglike [B]; d_chi2_lens, d_chi2_dyn [B] or NULL; d_flags [B] or NULL (union of both halves' bits).
+ */
+glad_status glad_joint_loglike_batch(glad_ctx* ctx, const float* d_lens_params,
+                                     const float* d_dyn_params, int B, const float* d_lum_mge,
+                                     int n_lum, long lum_stride, const float* d_mass_mge, int n_mass,
+                                     long mass_stride, const float* d_beta, int beta_per_gaussian,
+                                     float* d_loglike, float* d_chi2_lens, float* d_chi2_dyn,
+                                     int32_t* d_flags);
+
+/*
+ * Host-buffer variant of glad_joint_loglike_batch (the end-to-end call a CPU sampler makes): all pointers are
+ * HOST pointers (pinned memory recommended).  Copies the parameter vectors, MGE tables and beta to context-
+ * owned device staging on the stream, runs the joint path, copies lnL (and chi2 / flags if non-NULL) back and
+ * SYNCHRONISES the stream before returning.  Table sizes follow the strides: n_lum*3 floats if lum_stride == 0
+ * else B*lum_stride; likewise for mass.
+ */
+glad_status glad_joint_loglike_host(glad_ctx* ctx, const float* h_lens_params, const float* h_dyn_params, int B,
+                                    const float* h_lum_mge, int n_lum, long lum_stride, const float* h_mass_mge,
+                                    int n_mass, long mass_stride, const float* h_beta, int beta_per_gaussian,
+                                    float* h_loglike, float* h_chi2_lens, float* h_chi2_dyn, int32_t* h_flags);
+
+/* Host helper: theta_E,BH^2 [arcsec^2] = 4 G M_BH (1+z_d) / (c^2 D_dt) (from Eq. 4), so that the
+ * caller keeps lens[8] consistent with dyn[2] and the sampled D_dt.  Pure host arithmetic. */
+double glad_bh_theta2(double mbh_msun, double ddt_mpc, double z_d);
+
+/* Number of kernel launches enqueued by this context since creation (for bench.py's gpu_launches). */
+long glad_launch_count(const glad_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GLAD_H */

@@ -1,0 +1,212 @@
+"""Thin ctypes binding of libglad (include/glad.h).  Argument marshalling only: every step of the
+path runs in the CUDA kernels.  PyTorch supplies device memory and the stream, nothing else.
+There is no fallback: a missing library or a failing call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from .build import LIB, build
+
+NLENS, NDYN = 26, 4
+FLAG_LENS_INVALID, FLAG_DYN_INVALID, FLAG_BIN_INVALID = 1, 2, 4
+
+_lib = None
+EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "glad_set_image_data",
+           "glad_set_kin_data", "glad_lens_image_batch", "glad_jam_vrms_batch", "glad_joint_loglike_batch",
+           "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count"]
+
+
+class GladError(RuntimeError):
+    pass
+
+
+class ImageGrid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("supersample", C.c_int),
+                ("pix", C.c_float), ("x0", C.c_float), ("y0", C.c_float)]
+
+
+class SkyGrid(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("d_xs", C.c_void_p), ("d_ys", C.c_void_p)]
+
+
+def load(rebuild: bool = False):
+    """Load libglad.so (building it in-tree if it is missing or stale and nvcc is present)."""
+    global _lib
+    if _lib is not None and not rebuild:
+        return _lib
+    if rebuild or not os.path.exists(LIB):
+        build(force=rebuild)
+    if not os.path.exists(LIB):
+        raise GladError(f"libglad.so not found at {LIB}: run __graft_entry__.build()")
+    L = C.CDLL(LIB)
+    vp, i, l = C.c_void_p, C.c_int, C.c_long
+    L.glad_create.restype = i
+    L.glad_create.argtypes = [C.POINTER(vp), i, vp]
+    L.glad_destroy.restype = None
+    L.glad_destroy.argtypes = [vp]
+    L.glad_last_error.restype = C.c_char_p
+    L.glad_last_error.argtypes = [vp]
+    L.glad_version.restype = C.c_char_p
+    L.glad_set_image_data.restype = i
+    L.glad_set_image_data.argtypes = [vp, C.POINTER(ImageGrid), vp, vp, vp, i]
+    L.glad_set_kin_data.restype = i
+    L.glad_set_kin_data.argtypes = [vp, C.POINTER(SkyGrid), vp, i, vp, i, vp, vp, vp, vp, i]
+    L.glad_lens_image_batch.restype = i
+    L.glad_lens_image_batch.argtypes = [vp, vp, i, vp, vp, vp]
+    L.glad_jam_vrms_batch.restype = i
+    L.glad_jam_vrms_batch.argtypes = [vp, vp, i, vp, i, l, vp, i, l, vp, i, vp, vp, vp, vp]
+    L.glad_joint_loglike_batch.restype = i
+    L.glad_joint_loglike_batch.argtypes = [vp, vp, vp, i, vp, i, l, vp, i, l, vp, i, vp, vp, vp, vp]
+    L.glad_joint_loglike_host.restype = i
+    L.glad_joint_loglike_host.argtypes = [vp, vp, vp, i, vp, i, l, vp, i, l, vp, i, vp, vp, vp, vp]
+    L.glad_bh_theta2.restype = C.c_double
+    L.glad_bh_theta2.argtypes = [C.c_double] * 3
+    L.glad_launch_count.restype = l
+    L.glad_launch_count.argtypes = [vp]
+    _lib = L
+    return L
+
+
+def bh_theta2(mbh_msun: float, ddt_mpc: float, z_d: float) -> float:
+    return float(load().glad_bh_theta2(mbh_msun, ddt_mpc, z_d))
+
+
+def _dev(t, dtype, device):
+    if t is None:
+        return None
+    if isinstance(t, np.ndarray):
+        t = torch.from_numpy(np.ascontiguousarray(t))
+    return t.to(device=device, dtype=dtype).contiguous()
+
+
+def _p(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+class Glad:
+    """One libglad context bound to torch's current stream on `device`."""
+
+    def __init__(self, device: int | str = 0):
+        if not torch.cuda.is_available():
+            raise GladError("libglad needs a CUDA device (sm_100); there is no CPU path")
+        self.device = torch.device("cuda", device) if isinstance(device, int) else torch.device(device)
+        self.lib = load()
+        self._keep = {}
+        ctx = C.c_void_p()
+        with torch.cuda.device(self.device):
+            self.stream = torch.cuda.current_stream()
+            st = self.lib.glad_create(C.byref(ctx), self.device.index or 0, C.c_void_p(self.stream.cuda_stream))
+        if st != 0:
+            raise GladError(f"glad_create failed with status {st} (device is not sm_100?)")
+        self.ctx = ctx
+        self.image_shape = None
+        self.sky_shape = None
+        self.nbins = 0
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            self.lib.glad_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st):
+        if st != 0:
+            raise GladError(f"libglad status {st}: {self.lib.glad_last_error(self.ctx).decode()}")
+
+    @property
+    def launch_count(self) -> int:
+        return int(self.lib.glad_launch_count(self.ctx))
+
+    # ---- static data -------------------------------------------------------------------------
+    def set_image_data(self, grid: dict, psf, data=None, ivar=None):
+        f = torch.float32
+        k = {"psf": _dev(psf, f, self.device), "data": _dev(data, f, self.device), "ivar": _dev(ivar, f, self.device)}
+        g = ImageGrid(int(grid["nx"]), int(grid["ny"]), int(grid["supersample"]), float(grid["pix"]),
+                      float(grid["x0"]), float(grid["y0"]))
+        self._check(self.lib.glad_set_image_data(self.ctx, C.byref(g), _p(k["data"]), _p(k["ivar"]), _p(k["psf"]),
+                                                 int(k["psf"].shape[0])))
+        self._keep["image"] = k
+        self.image_shape = (g.ny, g.nx)
+
+    def set_kin_data(self, kin: dict):
+        f = torch.float32
+        k = {n: _dev(kin.get(n), f, self.device) for n in ("xs", "ys", "kernel", "vrms_obs", "vrms_ivar", "u_nodes", "u_weights")}
+        k["bin_id"] = _dev(kin["bin_id"], torch.int32, self.device)
+        g = SkyGrid(int(k["xs"].numel()), int(k["ys"].numel()), k["xs"].data_ptr(), k["ys"].data_ptr())
+        self._check(self.lib.glad_set_kin_data(self.ctx, C.byref(g), _p(k["bin_id"]), int(kin["nbins"]), _p(k["kernel"]),
+                                               int(k["kernel"].shape[0]), _p(k["vrms_obs"]), _p(k["vrms_ivar"]),
+                                               _p(k["u_nodes"]), _p(k["u_weights"]), int(k["u_nodes"].numel())))
+        self._keep["kin"] = k
+        self.sky_shape = (g.ny, g.nx)
+        self.nbins = int(kin["nbins"])
+
+    # ---- batch calls (device tensors in, device tensors out; enqueue only) --------------------
+    def lens_image_batch(self, lens_params, want_images=True, want_chi2=True, out=None):
+        p = _dev(lens_params, torch.float32, self.device).reshape(-1, NLENS)
+        B = p.shape[0]
+        out = out or {}
+        img = out.get("images") if want_images else None
+        if want_images and img is None:
+            img = torch.empty((B,) + self.image_shape, dtype=torch.float32, device=self.device)
+        chi2 = (out.get("chi2") if out.get("chi2") is not None else torch.empty(B, dtype=torch.float32, device=self.device)) if want_chi2 else None
+        flags = out.get("flags") if out.get("flags") is not None else torch.empty(B, dtype=torch.int32, device=self.device)
+        self._check(self.lib.glad_lens_image_batch(self.ctx, _p(p), B, _p(img), _p(chi2), _p(flags)))
+        return {"images": img, "chi2": chi2, "flags": flags}
+
+    def _tables(self, lum_mge, mass_mge, beta):
+        f = torch.float32
+        lum, mass, beta = _dev(lum_mge, f, self.device), _dev(mass_mge, f, self.device), _dev(beta, f, self.device)
+        n_lum, n_mass = lum.shape[-2], mass.shape[-2]
+        ls = 0 if lum.dim() == 2 else n_lum * 3
+        ms = 0 if mass.dim() == 2 else n_mass * 3
+        return lum, n_lum, ls, mass, n_mass, ms, beta, (1 if beta.dim() == 2 else 0)
+
+    def jam_vrms_batch(self, dyn_params, lum_mge, mass_mge, beta, want_chi2=True, want_map=False):
+        d = _dev(dyn_params, torch.float32, self.device).reshape(-1, NDYN)
+        B = d.shape[0]
+        lum, nl, ls, mass, nm, ms, bt, pg = self._tables(lum_mge, mass_mge, beta)
+        vrms = torch.empty((B, self.nbins), dtype=torch.float32, device=self.device)
+        chi2 = torch.empty(B, dtype=torch.float32, device=self.device) if want_chi2 else None
+        v2map = torch.empty((B,) + self.sky_shape, dtype=torch.float32, device=self.device) if want_map else None
+        flags = torch.empty(B, dtype=torch.int32, device=self.device)
+        self._check(self.lib.glad_jam_vrms_batch(self.ctx, _p(d), B, _p(lum), nl, ls, _p(mass) if nm else None, nm, ms,
+                                                 _p(bt), pg, _p(vrms), _p(chi2), _p(v2map), _p(flags)))
+        return {"vrms": vrms, "chi2": chi2, "v2map": v2map, "flags": flags}
+
+    def joint_loglike_batch(self, lens_params, dyn_params, lum_mge, mass_mge, beta, out=None):
+        p = _dev(lens_params, torch.float32, self.device).reshape(-1, NLENS)
+        d = _dev(dyn_params, torch.float32, self.device).reshape(-1, NDYN)
+        B = p.shape[0]
+        if d.shape[0] != B:
+            raise GladError("lens and dyn batches differ")
+        lum, nl, ls, mass, nm, ms, bt, pg = self._tables(lum_mge, mass_mge, beta)
+        out = out or {}
+        mk = lambda n, dt: out.get(n) if out.get(n) is not None else torch.empty(B, dtype=dt, device=self.device)
+        ll, c2l, c2d, fl = mk("loglike", torch.float32), mk("chi2_lens", torch.float32), mk("chi2_dyn", torch.float32), mk("flags", torch.int32)
+        self._check(self.lib.glad_joint_loglike_batch(self.ctx, _p(p), _p(d), B, _p(lum), nl, ls, _p(mass) if nm else None,
+                                                      nm, ms, _p(bt), pg, _p(ll), _p(c2l), _p(c2d), _p(fl)))
+        return {"loglike": ll, "chi2_lens": c2l, "chi2_dyn": c2d, "flags": fl}
+
+    def joint_loglike_host(self, lens_params, dyn_params, lum_mge, mass_mge, beta, loglike_out):
+        """Host (CPU, ideally pinned) tensors in, host tensor out; copies + sync inside the C call."""
+        for t in (lens_params, dyn_params, lum_mge, mass_mge, beta, loglike_out):
+            if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+                raise GladError("joint_loglike_host wants contiguous float32 CPU tensors")
+        B = lens_params.shape[0]
+        nl, nm = lum_mge.shape[-2], mass_mge.shape[-2]
+        ls = 0 if lum_mge.dim() == 2 else nl * 3
+        ms = 0 if mass_mge.dim() == 2 else nm * 3
+        self._check(self.lib.glad_joint_loglike_host(self.ctx, _p(lens_params), _p(dyn_params), B, _p(lum_mge), nl, ls,
+                                                     _p(mass_mge) if nm else None, nm, ms, _p(beta), 1 if beta.dim() == 2 else 0,
+                                                     _p(loglike_out), None, None, None))
+        return loglike_out

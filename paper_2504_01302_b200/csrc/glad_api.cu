@@ -1,0 +1,333 @@
+// C ABI of libglad (include/glad.h): context, static data, argument checks, scratch, launch order.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <vector>
+
+#include "glad_internal.h"
+
+static glad_status fail(glad_ctx* c, glad_status st, const char* fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return st;
+}
+static glad_status cuda_fail(glad_ctx* c, cudaError_t e, const char* what) {
+    return fail(c, GLAD_ECUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+#define CU(call, what)                                           \
+    do {                                                         \
+        cudaError_t e__ = (call);                                \
+        if (e__ != cudaSuccess) return cuda_fail(c, e__, what);  \
+    } while (0)
+
+template <typename T>
+static glad_status grow(glad_ctx* c, T** p, size_t* cap, size_t need) {
+    if (need <= *cap) return GLAD_OK;
+    // the stream may still be using the old block: free is stream-ordered w.r.t. nothing, so sync first
+    cudaStreamSynchronize(c->stream);
+    if (*p) cudaFree(*p);
+    *p = nullptr;
+    *cap = 0;
+    size_t n = need + need / 4;
+    if (cudaMalloc((void**)p, n * sizeof(T)) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, GLAD_ENOMEM, "cudaMalloc of %zu bytes failed", n * sizeof(T));
+    }
+    *cap = n;
+    return GLAD_OK;
+}
+
+extern "C" {
+
+const char* glad_version(void) { return "libglad 0.1 (sm_100a)"; }
+
+glad_status glad_create(glad_ctx** out, int device, void* cuda_stream) {
+    if (!out) return GLAD_EINVAL;
+    *out = nullptr;
+    glad_ctx* c = new glad_ctx();
+    memset(c, 0, sizeof(*c));
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    cudaDeviceProp prop;
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess || prop.major != 10) {
+        delete c;
+        return GLAD_ECUDA;
+    }
+    c->sm_count = prop.multiProcessorCount;
+    *out = c;
+    return GLAD_OK;
+}
+
+static void free_kin(glad_ctx* c) {
+    void* ps[] = {c->d_xf2, c->d_yf2, c->d_xf, c->d_yf, c->d_foldx, c->d_foldy, c->d_unfoldx, c->d_unfoldy,
+                  c->d_binw, c->d_bin_cnt};
+    for (void* p : ps) if (p) cudaFree(p);
+    c->d_xf2 = c->d_yf2 = c->d_xf = c->d_yf = nullptr;
+    c->d_foldx = c->d_foldy = c->d_unfoldx = c->d_unfoldy = nullptr;
+    c->d_binw = nullptr;
+    c->d_bin_cnt = nullptr;
+}
+
+void glad_destroy(glad_ctx* c) {
+    if (!c) return;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    free_kin(c);
+    void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage};
+    for (void* p : ps) if (p) cudaFree(p);
+    delete c;
+}
+
+const char* glad_last_error(const glad_ctx* c) { return c ? c->err : "null context"; }
+long glad_launch_count(const glad_ctx* c) { return c ? c->launches : 0; }
+
+double glad_bh_theta2(double mbh_msun, double ddt_mpc, double z_d) {
+    const double G = 0.004301, ckms = 299792.458, PI = 3.14159265358979323846;
+    double rad2 = 4.0 * G * mbh_msun * (1.0 + z_d) / (ckms * ckms * ddt_mpc * 1e6);
+    double as = 648000.0 / PI;
+    return rad2 * as * as;
+}
+
+glad_status glad_set_image_data(glad_ctx* c, const glad_image_grid* g, const float* d_data, const float* d_ivar,
+                                const float* d_psf, int kpsf) {
+    if (!c) return GLAD_EINVAL;
+    if (!g || !d_psf) return fail(c, GLAD_EINVAL, "glad_set_image_data: null grid or psf");
+    if (g->nx <= 0 || g->ny <= 0 || g->supersample <= 0 || !(g->pix > 0.f))
+        return fail(c, GLAD_EINVAL, "glad_set_image_data: bad grid %dx%d s=%d pix=%g", g->nx, g->ny, g->supersample, g->pix);
+    if ((long)g->nx * g->ny > GLAD_MAX_IMAGE_PIXELS)
+        return fail(c, GLAD_ESHAPE, "glad_set_image_data: %dx%d pixels exceed GLAD_MAX_IMAGE_PIXELS", g->nx, g->ny);
+    if (kpsf <= 0 || (kpsf % 2) == 0) return fail(c, GLAD_EINVAL, "glad_set_image_data: kpsf must be odd, got %d", kpsf);
+    if (kpsf > GLAD_MAX_PSF) return fail(c, GLAD_ESHAPE, "glad_set_image_data: kpsf %d > GLAD_MAX_PSF", kpsf);
+    if ((d_data == nullptr) != (d_ivar == nullptr)) return fail(c, GLAD_EINVAL, "glad_set_image_data: data and ivar go together");
+    cudaSetDevice(c->device);
+    if (!c->d_psf) CU(cudaMalloc((void**)&c->d_psf, sizeof(float) * GLAD_MAX_PSF * GLAD_MAX_PSF), "cudaMalloc psf");
+    CU(cudaMemcpyAsync(c->d_psf, d_psf, sizeof(float) * kpsf * kpsf, cudaMemcpyDeviceToDevice, c->stream), "copy psf");
+    c->grid = *g;
+    c->d_data = d_data;
+    c->d_ivar = d_ivar;
+    c->kpsf = kpsf;
+    c->have_image = true;
+    return GLAD_OK;
+}
+
+}  // extern "C"
+
+// fold one axis: returns folded length; fills fold[n] (full -> folded), coords of the folded axis, unfold[2*nf]
+static int fold_axis(const std::vector<float>& x, std::vector<int>& fold, std::vector<float>& xf, std::vector<int>& unfold) {
+    int n = (int)x.size();
+    bool sym = n > 1;
+    for (int i = 0; i < n && sym; ++i) sym = (x[i] == -x[n - 1 - i]);
+    fold.assign(n, 0);
+    if (!sym) {
+        xf = x;
+        unfold.assign(2 * n, -1);
+        for (int i = 0; i < n; ++i) { fold[i] = i; unfold[2 * i] = i; }
+        return n;
+    }
+    int nf = (n + 1) / 2, h = n / 2;   // folded index 0 = innermost
+    xf.assign(nf, 0.f);
+    unfold.assign(2 * nf, -1);
+    for (int i = 0; i < n; ++i) {
+        int f = (i >= h) ? i - h : (n - 1 - i) - h;   // n odd: centre i = h -> 0
+        fold[i] = f;
+        xf[f] = fabsf(x[i]);
+        if (unfold[2 * f] < 0) unfold[2 * f] = i; else unfold[2 * f + 1] = i;
+    }
+    return nf;
+}
+
+template <typename T>
+static cudaError_t upload(T** dst, const std::vector<T>& v) {
+    cudaError_t e = cudaMalloc((void**)dst, sizeof(T) * (v.size() ? v.size() : 1));
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(*dst, v.data(), sizeof(T) * v.size(), cudaMemcpyHostToDevice);
+}
+
+extern "C" {
+
+glad_status glad_set_kin_data(glad_ctx* c, const glad_sky_grid* g, const int32_t* d_bin_id, int nbins, const float* d_kernel,
+                              int kk, const float* d_vobs, const float* d_vivar, const float* d_un, const float* d_uw, int nu) {
+    if (!c) return GLAD_EINVAL;
+    if (!g || !g->d_xs || !g->d_ys || !d_bin_id || !d_kernel || !d_un || !d_uw)
+        return fail(c, GLAD_EINVAL, "glad_set_kin_data: null pointer");
+    if (g->nx <= 0 || g->ny <= 0 || nbins <= 0 || nu <= 0) return fail(c, GLAD_EINVAL, "glad_set_kin_data: bad sizes");
+    if (g->nx > GLAD_MAX_SKY || g->ny > GLAD_MAX_SKY || nbins > GLAD_MAX_BINS || nu > GLAD_MAX_NODES)
+        return fail(c, GLAD_ESHAPE, "glad_set_kin_data: grid %dx%d / nbins %d / nu %d exceed the limits", g->nx, g->ny, nbins, nu);
+    if (kk <= 0 || (kk % 2) == 0) return fail(c, GLAD_EINVAL, "glad_set_kin_data: kk must be odd, got %d", kk);
+    if (kk > GLAD_MAX_PSF) return fail(c, GLAD_ESHAPE, "glad_set_kin_data: kk %d > GLAD_MAX_PSF", kk);
+    if ((d_vobs == nullptr) != (d_vivar == nullptr)) return fail(c, GLAD_EINVAL, "glad_set_kin_data: vrms_obs and vrms_ivar go together");
+    cudaSetDevice(c->device);
+    CU(cudaStreamSynchronize(c->stream), "sync");
+    std::vector<float> xs(g->nx), ys(g->ny);
+    std::vector<int32_t> bins((size_t)g->nx * g->ny);
+    CU(cudaMemcpy(xs.data(), g->d_xs, sizeof(float) * g->nx, cudaMemcpyDeviceToHost), "copy xs");
+    CU(cudaMemcpy(ys.data(), g->d_ys, sizeof(float) * g->ny, cudaMemcpyDeviceToHost), "copy ys");
+    CU(cudaMemcpy(bins.data(), d_bin_id, sizeof(int32_t) * bins.size(), cudaMemcpyDeviceToHost), "copy bin_id");
+    std::vector<int> cnt(nbins, 0);
+    for (int32_t l : bins) {
+        if (l >= nbins) return fail(c, GLAD_EINVAL, "glad_set_kin_data: bin id %d >= nbins %d", (int)l, nbins);
+        if (l >= 0) cnt[l]++;
+    }
+    std::vector<int> fx, fy, ux, uy;
+    std::vector<float> xf, yf;
+    int nxf = fold_axis(xs, fx, xf, ux), nyf = fold_axis(ys, fy, yf, uy);
+    int tiles = ((nxf + JQ_T - 1) / JQ_T) * ((nyf + JQ_T - 1) / JQ_T);
+    if (tiles > 512) return fail(c, GLAD_ESHAPE, "glad_set_kin_data: folded grid %dx%d needs %d thread tiles (> 512)", nxf, nyf, tiles);
+    std::vector<float> xf2(nxf), yf2(nyf);
+    for (int i = 0; i < nxf; ++i) xf2[i] = xf[i] * xf[i];
+    for (int i = 0; i < nyf; ++i) yf2[i] = yf[i] * yf[i];
+    free_kin(c);
+    c->have_kin = false;
+    CU(upload(&c->d_xf, xf), "upload"); CU(upload(&c->d_yf, yf), "upload");
+    CU(upload(&c->d_xf2, xf2), "upload"); CU(upload(&c->d_yf2, yf2), "upload");
+    CU(upload(&c->d_foldx, fx), "upload"); CU(upload(&c->d_foldy, fy), "upload");
+    CU(upload(&c->d_unfoldx, ux), "upload"); CU(upload(&c->d_unfoldy, uy), "upload");
+    CU(upload(&c->d_bin_cnt, cnt), "upload");
+    CU(cudaMalloc((void**)&c->d_binw, sizeof(float) * (size_t)nbins * nxf * nyf), "cudaMalloc bin weights");
+    c->nx = g->nx; c->ny = g->ny; c->nxf = nxf; c->nyf = nyf; c->nbins = nbins; c->kk = kk; c->nu = nu;
+    c->d_xs = g->d_xs; c->d_ys = g->d_ys; c->d_bin_id = d_bin_id; c->d_kernel = d_kernel;
+    c->d_vobs = d_vobs; c->d_vivar = d_vivar; c->d_un = d_un; c->d_uw = d_uw;
+    CU(launch_kin_weights(c), "kin_weights_kernel");
+    CU(cudaStreamSynchronize(c->stream), "kin_weights_kernel");
+    c->have_kin = true;
+    return GLAD_OK;
+}
+
+}  // extern "C"
+
+static glad_status lens_impl(glad_ctx* c, const float* d_lens, int B, float* d_images, float* d_chi2, int32_t* d_flags) {
+    if (!c->have_image) return fail(c, GLAD_ESTATE, "lens: glad_set_image_data not called");
+    if (d_chi2 && !c->d_data) return fail(c, GLAD_ESTATE, "lens: chi2 requested but no data/ivar set");
+    glad_status st = grow(c, &c->d_lens_const, &c->lens_const_cap, (size_t)B * LC_SIZE);
+    if (st != GLAD_OK) return st;
+    CU(launch_lens_prep(c, d_lens, B), "lens_prep_kernel");
+    CU(launch_lens_image(c, B, d_images, d_chi2, d_flags), "lens_image_kernel");
+    return GLAD_OK;
+}
+
+static glad_status jam_impl(glad_ctx* c, const float* d_dyn, int B, const float* d_lum, int nl, long lum_stride,
+                            const float* d_mass, int nm, long mass_stride, const float* d_beta, int per_gaussian,
+                            float* d_vrms, float* d_chi2, float* d_v2map, int32_t* d_flags) {
+    if (!c->have_kin) return fail(c, GLAD_ESTATE, "jam: glad_set_kin_data not called");
+    if (d_chi2 && !c->d_vobs) return fail(c, GLAD_ESTATE, "jam: chi2 requested but no vrms_obs/vrms_ivar set");
+    if (!d_lum || !d_beta || (nm > 0 && !d_mass)) return fail(c, GLAD_EINVAL, "jam: null table pointer");
+    if (nl <= 0 || nm < 0) return fail(c, GLAD_EINVAL, "jam: n_lum %d / n_mass %d", nl, nm);
+    if (nl > GLAD_MAX_GAUSS || nm > GLAD_MAX_GAUSS) return fail(c, GLAD_ESHAPE, "jam: more than GLAD_MAX_GAUSS Gaussians");
+    if (lum_stride < 0 || mass_stride < 0) return fail(c, GLAD_EINVAL, "jam: negative stride");
+    const int nmx = nm + 1;
+    int NG;
+    if (jam_quad_geometry(c, &NG) < 0) return fail(c, GLAD_ESHAPE, "jam: sky grid too large");
+    // K-slices: enough CTAs for >= 4 per SM when the batch is small
+    long M = (long)c->nu * nmx * nl;
+    int NCH = (int)((M + NG * JQ_MI - 1) / (NG * JQ_MI));
+    int S = (4 * c->sm_count + B - 1) / B;
+    if (S > 32) S = 32;
+    if (S > NCH) S = NCH;
+    if (S < 1) S = 1;
+    glad_status st = grow(c, &c->d_jam_tab, &c->jam_tab_cap, (size_t)B * jam_table_floats(nl, nmx));
+    if (st != GLAD_OK) return st;
+    st = grow(c, &c->d_partial, &c->partial_cap, (size_t)B * S * c->nxf * c->nyf);
+    if (st != GLAD_OK) return st;
+    CU(launch_jam_prep(c, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian), "jam_prep_kernel");
+    CU(launch_jam_quad(c, B, nl, nmx, S), "jam_quad_kernel");
+    CU(launch_jam_post(c, B, nl, nmx, S, d_vrms, d_chi2, d_v2map, d_flags), "jam_post_kernel");
+    return GLAD_OK;
+}
+
+extern "C" {
+
+glad_status glad_lens_image_batch(glad_ctx* c, const float* d_lens, int B, float* d_images, float* d_chi2, int32_t* d_flags) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && !d_lens)) return fail(c, GLAD_EINVAL, "glad_lens_image_batch: B=%d / null params", B);
+    if (B == 0) return GLAD_OK;
+    cudaSetDevice(c->device);
+    return lens_impl(c, d_lens, B, d_images, d_chi2, d_flags);
+}
+
+glad_status glad_jam_vrms_batch(glad_ctx* c, const float* d_dyn, int B, const float* d_lum, int nl, long lum_stride,
+                                const float* d_mass, int nm, long mass_stride, const float* d_beta, int per_gaussian,
+                                float* d_vrms, float* d_chi2, float* d_v2map, int32_t* d_flags) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && !d_dyn)) return fail(c, GLAD_EINVAL, "glad_jam_vrms_batch: B=%d / null params", B);
+    if (B == 0) return GLAD_OK;
+    cudaSetDevice(c->device);
+    return jam_impl(c, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian, d_vrms, d_chi2,
+                    d_v2map, d_flags);
+}
+
+glad_status glad_joint_loglike_batch(glad_ctx* c, const float* d_lens, const float* d_dyn, int B, const float* d_lum, int nl,
+                                     long lum_stride, const float* d_mass, int nm, long mass_stride, const float* d_beta,
+                                     int per_gaussian, float* d_loglike, float* d_chi2_lens, float* d_chi2_dyn,
+                                     int32_t* d_flags) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && (!d_lens || !d_dyn || !d_loglike))) return fail(c, GLAD_EINVAL, "glad_joint_loglike_batch: B=%d / null pointer", B);
+    if (B == 0) return GLAD_OK;
+    cudaSetDevice(c->device);
+    glad_status st = grow(c, &c->d_tmp, &c->tmp_cap, (size_t)2 * B);
+    if (st != GLAD_OK) return st;
+    st = grow(c, &c->d_tmpflags, &c->tmpflags_cap, (size_t)2 * B);
+    if (st != GLAD_OK) return st;
+    float* c2l = d_chi2_lens ? d_chi2_lens : c->d_tmp;
+    float* c2d = d_chi2_dyn ? d_chi2_dyn : c->d_tmp + B;
+    int32_t *fl = c->d_tmpflags, *fd = c->d_tmpflags + B;
+    st = lens_impl(c, d_lens, B, nullptr, c2l, fl);
+    if (st != GLAD_OK) return st;
+    st = jam_impl(c, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian, nullptr, c2d, nullptr, fd);
+    if (st != GLAD_OK) return st;
+    CU(launch_joint(c, B, c2l, c2d, fl, fd, d_loglike, d_flags), "joint_kernel");
+    return GLAD_OK;
+}
+
+glad_status glad_joint_loglike_host(glad_ctx* c, const float* h_lens, const float* h_dyn, int B, const float* h_lum, int nl,
+                                    long lum_stride, const float* h_mass, int nm, long mass_stride, const float* h_beta,
+                                    int per_gaussian, float* h_loglike, float* h_chi2_lens, float* h_chi2_dyn,
+                                    int32_t* h_flags) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && (!h_lens || !h_dyn || !h_loglike || !h_lum || !h_beta || (nm > 0 && !h_mass))))
+        return fail(c, GLAD_EINVAL, "glad_joint_loglike_host: B=%d / null pointer", B);
+    if (nl <= 0 || nm < 0 || lum_stride < 0 || mass_stride < 0) return fail(c, GLAD_EINVAL, "glad_joint_loglike_host: bad table sizes");
+    if (B == 0) return GLAD_OK;
+    cudaSetDevice(c->device);
+    auto r4 = [](size_t n) { return (n + 3) & ~(size_t)3; };
+    size_t n_lens = r4((size_t)B * GLAD_NLENS), n_dyn = r4((size_t)B * GLAD_NDYN);
+    size_t n_lum = r4(lum_stride ? (size_t)B * lum_stride : (size_t)nl * 3);
+    size_t n_mass = r4(mass_stride ? (size_t)B * mass_stride : (size_t)nm * 3);
+    size_t n_beta = r4(per_gaussian ? (size_t)B * nl : (size_t)B), n_out = r4((size_t)B);
+    glad_status st = grow(c, &c->d_stage, &c->stage_cap, n_lens + n_dyn + n_lum + n_mass + n_beta + 4 * n_out);
+    if (st != GLAD_OK) return st;
+    float* d_lens = c->d_stage;
+    float* d_dyn = d_lens + n_lens;
+    float* d_lum = d_dyn + n_dyn;
+    float* d_mass = d_lum + n_lum;
+    float* d_beta = d_mass + n_mass;
+    float* d_ll = d_beta + n_beta;
+    float* d_c2l = d_ll + n_out;
+    float* d_c2d = d_c2l + n_out;
+    int32_t* d_fl = (int32_t*)(d_c2d + n_out);
+    cudaStream_t s = c->stream;
+    CU(cudaMemcpyAsync(d_lens, h_lens, sizeof(float) * B * GLAD_NLENS, cudaMemcpyHostToDevice, s), "H2D lens");
+    CU(cudaMemcpyAsync(d_dyn, h_dyn, sizeof(float) * B * GLAD_NDYN, cudaMemcpyHostToDevice, s), "H2D dyn");
+    CU(cudaMemcpyAsync(d_lum, h_lum, sizeof(float) * (lum_stride ? (size_t)B * lum_stride : (size_t)nl * 3), cudaMemcpyHostToDevice, s), "H2D lum");
+    if (nm > 0)
+        CU(cudaMemcpyAsync(d_mass, h_mass, sizeof(float) * (mass_stride ? (size_t)B * mass_stride : (size_t)nm * 3), cudaMemcpyHostToDevice, s), "H2D mass");
+    CU(cudaMemcpyAsync(d_beta, h_beta, sizeof(float) * (per_gaussian ? (size_t)B * nl : (size_t)B), cudaMemcpyHostToDevice, s), "H2D beta");
+    st = glad_joint_loglike_batch(c, d_lens, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian,
+                                  d_ll, d_c2l, d_c2d, d_fl);
+    if (st != GLAD_OK) return st;
+    CU(cudaMemcpyAsync(h_loglike, d_ll, sizeof(float) * B, cudaMemcpyDeviceToHost, s), "D2H loglike");
+    if (h_chi2_lens) CU(cudaMemcpyAsync(h_chi2_lens, d_c2l, sizeof(float) * B, cudaMemcpyDeviceToHost, s), "D2H chi2");
+    if (h_chi2_dyn) CU(cudaMemcpyAsync(h_chi2_dyn, d_c2d, sizeof(float) * B, cudaMemcpyDeviceToHost, s), "D2H chi2");
+    if (h_flags) CU(cudaMemcpyAsync(h_flags, d_fl, sizeof(int32_t) * B, cudaMemcpyDeviceToHost, s), "D2H flags");
+    CU(cudaStreamSynchronize(s), "joint (host) sync");
+    return GLAD_OK;
+}
+
+}  // extern "C"

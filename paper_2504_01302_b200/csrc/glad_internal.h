@@ -1,0 +1,97 @@
+// Internal declarations shared by the .cu files of libglad (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "glad.h"
+
+// ---------------------------------------------------------------------------------------------
+// Lens half: per-vector constants prepared in fp64 by lens_prep_kernel (row a0), read by
+// lens_image_kernel.  Indices into a float[LC_SIZE] block.
+// ---------------------------------------------------------------------------------------------
+#define GLAD_EPL_MAX_TERMS 40
+enum LensConstIdx {
+    LC_XL = 0, LC_YL, LC_COSPA, LC_SINPA, LC_Q, LC_NEGF,  // -f = -(1-q)/(1+q)
+    LC_PREF,      // 2 b_TM^t / (1+q)   (0 if theta_E = 0)
+    LC_HEXP,      // -(t-1)/2 : alpha magnitude = PREF * (R_TM^2)^HEXP
+    LC_NTERMS,    // number of series terms (int stored as float)
+    LC_SH_C, LC_SH_S,  // gamma_ext cos 2phi_ext, gamma_ext sin 2phi_ext
+    LC_BH,        // theta_E,BH^2
+    LC_VALID,     // 1 valid / 0 invalid
+    LC_SERSIC0 = 16,   // 3 components x 8 floats: xc, yc, cos, sin, 1/q^2, amp = Ie e^bn, k1 = bn log2e Re^(-1/n), h = 1/(2n)
+    LC_SERIES = 40,    // c_n, n = 1..GLAD_EPL_MAX_TERMS : (2n-(2-t))/(2n+(2-t))
+    LC_SIZE = 80
+};
+#define LC_SERSIC_STRIDE 8
+
+// ---------------------------------------------------------------------------------------------
+// Dynamics half: per-vector table block prepared in fp64 by jam_prep_kernel (rows a0/a5).
+// Layout (floats): header[JT_HDR] | 8 x nl (per luminous Gaussian) | 3 x nmx (per mass Gaussian,
+// nmx = n_mass+1 slots, the last for the BH) | 2 x nmx*nl (per pair), padded to a multiple of 4.
+// ---------------------------------------------------------------------------------------------
+#define JT_HDR 8
+enum JamHdrIdx { JH_SCALE = 0, JH_COS2I, JH_SIN2I, JH_NM, JH_VALID };
+enum JamLumIdx { JL_INVS2 = 0, JL_BKQ, JL_S0, JL_D0, JL_NKS, JL_I0, JL_E1, JL_E2, JL_COUNT };
+enum JamMassIdx { JM_INVS2 = 0, JM_OMQ2, JM_MJ, JM_COUNT };
+
+static inline __host__ __device__ int jam_table_floats(int nl, int nmx) {
+    int n = JT_HDR + JL_COUNT * nl + JM_COUNT * nmx + 2 * nmx * nl;
+    return (n + 3) & ~3;
+}
+
+// Thread tile of the quadrature contraction (outputs per thread = JQ_T x JQ_T) and rows of the
+// contraction each thread group consumes per staged chunk.
+#define JQ_T 8
+#define JQ_MI 8
+
+struct glad_ctx {
+    int device;
+    cudaStream_t stream;
+    int sm_count;
+    char err[512];
+    long launches;
+
+    // lensing static data
+    bool have_image;
+    glad_image_grid grid;
+    const float* d_data;
+    const float* d_ivar;
+    float* d_psf;  // ctx-owned copy [kpsf*kpsf]
+    int kpsf;
+
+    // kinematic static data
+    bool have_kin;
+    int nx, ny, nbins, kk, nu;
+    int nxf, nyf;           // folded grid (== nx, ny if not mirror-symmetric)
+    const float *d_xs, *d_ys, *d_kernel, *d_vobs, *d_vivar, *d_un, *d_uw;
+    const int32_t* d_bin_id;
+    float *d_xf2, *d_yf2;   // ctx-owned: squared coordinates of the folded grid [nxf], [nyf]
+    float *d_xf, *d_yf;     // folded coordinates
+    int *d_foldx, *d_foldy; // ctx-owned: full index -> folded index [nx], [ny]
+    int *d_unfoldx, *d_unfoldy; // ctx-owned: folded index -> its (up to 2) full indices, -1 = none [2*nxf], [2*nyf]
+    float* d_binw;          // ctx-owned: W_f[l][pf] = sum_{p in bin l} K(p - p') over the unfolded images p' of
+                            // folded pixel pf  [nbins, nyf*nxf]  (static: bins and kernel are static data)
+    int* d_bin_cnt;         // ctx-owned: spaxels per bin [nbins]
+
+    // grow-only scratch
+    float* d_lens_const; size_t lens_const_cap;
+    float* d_jam_tab;    size_t jam_tab_cap;
+    float* d_partial;    size_t partial_cap;
+    float* d_tmp;        size_t tmp_cap;     // chi2_L, chi2_D [B] each
+    int32_t* d_tmpflags; size_t tmpflags_cap; // flags_L, flags_D [B] each
+    float* d_stage;      size_t stage_cap;   // device staging of glad_joint_loglike_host
+};
+
+// kernel launchers (return cudaGetLastError())
+cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B);
+cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2, int32_t* d_flags);
+cudaError_t launch_jam_prep(glad_ctx* c, const float* d_dyn, int B, const float* d_lum, int nl, long lum_stride,
+                            const float* d_mass, int nm, long mass_stride, const float* d_beta, int per_gaussian);
+cudaError_t launch_jam_quad(glad_ctx* c, int B, int nl, int nmx, int S);
+cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d_vrms, float* d_chi2,
+                            float* d_v2map, int32_t* d_flags);
+cudaError_t launch_joint(glad_ctx* c, int B, const float* d_c2l, const float* d_c2d, const int32_t* d_fl,
+                         const int32_t* d_fd, float* d_loglike, int32_t* d_flags);
+cudaError_t launch_kin_weights(glad_ctx* c);
+// launch geometry of the quadrature kernel for the current sky grid: threads per CTA, thread groups
+int jam_quad_geometry(const glad_ctx* c, int* groups);

@@ -1,0 +1,292 @@
+// Lensing half of libglad for sm_100a: rows a0-a4 of SURVEY.md 8(a).
+//   lens_prep_kernel  : per-vector constants in fp64 -> fp32 (EPL normalisation Eq. B.3, series
+//                       coefficients, Sersic b_n root, rotations); validity flag.
+//   lens_image_kernel : one CTA per parameter vector.  Ray-shoot every sub-pixel (Eq. 33), evaluate
+//                       source at beta and lens light at theta, bin down into a whole-image shared-memory
+//                       tile, convolve with the PSF from shared memory (Eq. 38), reduce chi2 with
+//                       warp shuffles (Eq. 48).  No intermediate ever touches HBM.
+#include <math.h>
+
+#include "glad_internal.h"
+
+// ------------------------------------------------------------------------------------------------
+// fp64 helpers for the prep kernel
+// ------------------------------------------------------------------------------------------------
+// Regularised lower incomplete gamma P(a,x) (series / Lentz continued fraction).
+__device__ static double gamma_p(double a, double x) {
+    if (x <= 0.0) return 0.0;
+    double lg = lgamma(a);
+    if (x < a + 1.0) {
+        double ap = a, del = 1.0 / a, sum = del;
+        for (int n = 0; n < 2000; ++n) {
+            ap += 1.0;
+            del *= x / ap;
+            sum += del;
+            if (fabs(del) < fabs(sum) * 1e-16) break;
+        }
+        return sum * exp(-x + a * log(x) - lg);
+    }
+    const double FPMIN = 1e-290;
+    double b = x + 1.0 - a, c = 1.0 / FPMIN, d = 1.0 / b, h = d;
+    for (int i = 1; i < 2000; ++i) {
+        double an = -(double)i * ((double)i - a);
+        b += 2.0;
+        d = an * d + b;
+        if (fabs(d) < FPMIN) d = FPMIN;
+        c = b + an / c;
+        if (fabs(c) < FPMIN) c = FPMIN;
+        d = 1.0 / d;
+        double del = d * c;
+        h *= del;
+        if (fabs(del - 1.0) < 1e-15) break;
+    }
+    return 1.0 - exp(-x + a * log(x) - lg) * h;
+}
+
+// Sersic b_n: root of P(2n, b) = 1/2 by safeguarded Newton (reading R-L7).
+__device__ static double sersic_bn(double n) {
+    double a = 2.0 * n;
+    double lo = 0.0, hi = a + 25.0;
+    double b = a - 1.0 / 3.0;
+    if (b <= 0.0) b = 0.5 * a;
+    double lg = lgamma(a);
+    for (int it = 0; it < 60; ++it) {
+        double f = gamma_p(a, b) - 0.5;
+        if (f > 0.0) hi = b; else lo = b;
+        double fp = exp(-b + (a - 1.0) * log(b) - lg);
+        double nb = b - f / fp;
+        if (!(nb > lo && nb < hi)) nb = 0.5 * (lo + hi);
+        if (fabs(nb - b) < 1e-15 * b) { b = nb; break; }
+        b = nb;
+    }
+    return b;
+}
+
+__global__ void lens_prep_kernel(const float* __restrict__ params, int B, float* __restrict__ consts) {
+    int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    const float* p = params + (size_t)b * GLAD_NLENS;
+    float* c = consts + (size_t)b * LC_SIZE;
+    double xl = p[0], yl = p[1], thE = p[2], gam = p[3], q = p[4], pa = p[5];
+    bool valid = (thE >= 0.0) && (gam > 1.0 && gam < 3.0) && (q > 0.0 && q <= 1.0) && (p[8] >= 0.f);
+    for (int k = 0; k < 3; ++k) {
+        const float* s = p + (k == 0 ? 11 : (k == 1 ? 16 : 21));
+        if (s[0] != 0.f && !(s[1] > 0.f && s[2] > 0.f && s[3] > 0.f && s[3] <= 1.f)) valid = false;
+    }
+    for (int i = 0; i < LC_SIZE; ++i) c[i] = 0.f;
+    c[LC_VALID] = valid ? 1.f : 0.f;
+    if (!valid) return;
+    double t = gam - 1.0;
+    double f = (1.0 - q) / (1.0 + q);
+    double bTM = q * pow(2.0 / (1.0 + q), 1.0 / t) * thE;  // b_TM = q b, b from Eq. B.3
+    c[LC_XL] = (float)xl; c[LC_YL] = (float)yl;
+    c[LC_COSPA] = (float)cos(pa); c[LC_SINPA] = (float)sin(pa);
+    c[LC_Q] = (float)q; c[LC_NEGF] = (float)(-f);
+    c[LC_PREF] = (thE > 0.0) ? (float)(2.0 * pow(bTM, t) / (1.0 + q)) : 0.f;
+    c[LC_HEXP] = (float)(-0.5 * (t - 1.0));
+    int nt = 0;
+    if (f > 1e-12) {
+        nt = (int)ceil(log(2e-8) / log(f)) + 1;
+        if (nt < 1) nt = 1;
+        if (nt > GLAD_EPL_MAX_TERMS) nt = GLAD_EPL_MAX_TERMS;
+    }
+    c[LC_NTERMS] = (float)nt;
+    for (int n = 1; n <= GLAD_EPL_MAX_TERMS; ++n)
+        c[LC_SERIES + n - 1] = (float)((2.0 * n - (2.0 - t)) / (2.0 * n + (2.0 - t)));
+    c[LC_SH_C] = (float)((double)p[6] * cos(2.0 * (double)p[7]));
+    c[LC_SH_S] = (float)((double)p[6] * sin(2.0 * (double)p[7]));
+    c[LC_BH] = p[8];
+    for (int k = 0; k < 3; ++k) {
+        const float* s = p + (k == 0 ? 11 : (k == 1 ? 16 : 21));
+        float* o = c + LC_SERSIC0 + k * LC_SERSIC_STRIDE;
+        double Ie = s[0], Re = s[1], n = s[2], qs = s[3], phi = s[4];
+        o[0] = (k == 0) ? p[9] : (float)xl;
+        o[1] = (k == 0) ? p[10] : (float)yl;
+        if (Ie == 0.0) { o[5] = 0.f; continue; }
+        double bn = sersic_bn(n);
+        o[2] = (float)cos(phi); o[3] = (float)sin(phi);
+        o[4] = (float)(1.0 / (qs * qs));
+        o[5] = (float)(Ie * exp(bn));                                  // I(0)
+        o[6] = (float)(bn * 1.4426950408889634 * pow(Re, -1.0 / n));   // I = amp 2^(-k1 (R^2)^h)
+        o[7] = (float)(0.5 / n);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// main kernel
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float ex2f(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float lg2f(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+__device__ __forceinline__ float sersic_eval(const float* __restrict__ o, float px, float py) {
+    float dx = px - o[0], dy = py - o[1];
+    float x = dx * o[2] + dy * o[3];
+    float y = dy * o[2] - dx * o[3];
+    float R2 = fmaf(y * y, o[4], x * x);
+    float pw = ex2f(o[7] * lg2f(R2));      // (R^2)^(1/2n); R2 = 0 -> 0
+    return o[5] * ex2f(-o[6] * pw);
+}
+
+// One ray: returns source(beta) + lens light(theta).
+__device__ __forceinline__ float shoot(const float* __restrict__ c, float thx, float thy, int nterms,
+                                       bool has_src, bool has_l1, bool has_l2) {
+    float dx = thx - c[LC_XL], dy = thy - c[LC_YL];
+    float cs = c[LC_COSPA], sn = c[LC_SINPA];
+    float x = dx * cs + dy * sn, y = dy * cs - dx * sn;
+    float qx = c[LC_Q] * x;
+    float R2 = fmaxf(fmaf(qx, qx, y * y), 1e-12f);
+    float rinv = rsqrtf(R2);
+    float wr = qx * rinv, wi = y * rinv;
+    float negf = c[LC_NEGF];
+    float zr = negf * (wr * wr - wi * wi), zi = negf * (2.f * wr * wi);
+    // Horner: h_n = 1 + c_n z h_{n+1}, sum = h_1
+    float hr = 1.f, hi = 0.f;
+    for (int n = nterms; n >= 1; --n) {
+        float cn = c[LC_SERIES + n - 1];
+        float tr = fmaf(zr, hr, -zi * hi), ti = fmaf(zr, hi, zi * hr);
+        hr = fmaf(cn, tr, 1.f);
+        hi = cn * ti;
+    }
+    float mag = c[LC_PREF] * ex2f(c[LC_HEXP] * lg2f(R2));
+    float ar = mag * (wr * hr - wi * hi), ai = mag * (wr * hi + wi * hr);
+    float ax = ar * cs - ai * sn, ay = ar * sn + ai * cs;
+    ax = fmaf(c[LC_SH_C], dx, fmaf(c[LC_SH_S], dy, ax));
+    ay = fmaf(c[LC_SH_S], dx, fmaf(-c[LC_SH_C], dy, ay));
+    float r2 = fmaxf(fmaf(dx, dx, dy * dy), 1e-12f);
+    float bh = __fdividef(c[LC_BH], r2);
+    ax = fmaf(bh, dx, ax);
+    ay = fmaf(bh, dy, ay);
+    float v = 0.f;
+    if (has_src) v += sersic_eval(c + LC_SERSIC0, thx - ax, thy - ay);
+    if (has_l1) v += sersic_eval(c + LC_SERSIC0 + LC_SERSIC_STRIDE, thx, thy);
+    if (has_l2) v += sersic_eval(c + LC_SERSIC0 + 2 * LC_SERSIC_STRIDE, thx, thy);
+    return v;
+}
+
+#define LENS_STRIP 8
+
+__global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict__ consts, glad_image_grid g,
+                                                         const float* __restrict__ psf, int kpsf,
+                                                         const float* __restrict__ data,
+                                                         const float* __restrict__ ivar, float* __restrict__ images,
+                                                         float* __restrict__ chi2, int32_t* __restrict__ flags) {
+    extern __shared__ __align__(16) float smem[];
+    const int b = blockIdx.x, tid = threadIdx.x, nthr = blockDim.x;
+    const int nx = g.nx, ny = g.ny, npx = nx * ny, ss = g.supersample;
+    float* c = smem;                       // LC_SIZE
+    float* spsf = smem + LC_SIZE;          // kpsf^2 (padded to 4)
+    float* img = spsf + ((kpsf * kpsf + 3) & ~3);  // npx
+    __shared__ float red[32];
+
+    for (int i = tid; i < LC_SIZE; i += nthr) c[i] = consts[(size_t)b * LC_SIZE + i];
+    for (int i = tid; i < kpsf * kpsf; i += nthr) spsf[i] = psf[i];
+    __syncthreads();
+    const bool valid = c[LC_VALID] != 0.f;
+    if (!valid) {
+        if (images) for (int i = tid; i < npx; i += nthr) images[(size_t)b * npx + i] = __int_as_float(0x7fc00000);
+        if (tid == 0) {
+            if (chi2) chi2[b] = __int_as_float(0x7f800000);
+            if (flags) flags[b] = GLAD_FLAG_LENS_INVALID;
+        }
+        return;
+    }
+    const int nterms = (int)c[LC_NTERMS];
+    const bool has_src = c[LC_SERSIC0 + 5] != 0.f;
+    const bool has_l1 = c[LC_SERSIC0 + LC_SERSIC_STRIDE + 5] != 0.f;
+    const bool has_l2 = c[LC_SERSIC0 + 2 * LC_SERSIC_STRIDE + 5] != 0.f;
+    const float inv_s = 1.f / (float)ss, inv_s2 = 1.f / (float)(ss * ss);
+
+    // rows a1-a3: rays -> binned pixel in shared memory
+    for (int p = tid; p < npx; p += nthr) {
+        int iy = p / nx, ix = p - iy * nx;
+        float acc = 0.f;
+        for (int sb = 0; sb < ss; ++sb) {
+            float thy = fmaf(g.pix, (float)iy + (((float)sb + 0.5f) * inv_s - 0.5f), g.y0);
+            for (int sa = 0; sa < ss; ++sa) {
+                float thx = fmaf(g.pix, (float)ix + (((float)sa + 0.5f) * inv_s - 0.5f), g.x0);
+                acc += shoot(c, thx, thy, nterms, has_src, has_l1, has_l2);
+            }
+        }
+        img[p] = acc * inv_s2;
+    }
+    __syncthreads();
+
+    // row a4: PSF convolution from shared memory + chi2
+    const int cc = kpsf / 2;
+    const int nstrip_x = (nx + LENS_STRIP - 1) / LENS_STRIP;
+    const int nstrips = ny * nstrip_x;
+    float part = 0.f;
+    for (int st = tid; st < nstrips; st += nthr) {
+        int y = st / nstrip_x, x0 = (st - y * nstrip_x) * LENS_STRIP;
+        float out[LENS_STRIP];
+#pragma unroll
+        for (int j = 0; j < LENS_STRIP; ++j) out[j] = 0.f;
+        for (int dy = 0; dy < kpsf; ++dy) {
+            int sy = y + cc - dy;
+            if (sy < 0 || sy >= ny) continue;
+            const float* row = img + sy * nx;
+            const float* prow = spsf + dy * kpsf;
+            // out[j] += psf[dy][dx] * img[sy][x0 + j + cc - dx]; walk the source column e = x0-cc .. x0+cc+STRIP-1,
+            // keeping w[j] = psf[dy][cc + j - (e - x0)] in a sliding window.
+            float w[LENS_STRIP];
+#pragma unroll
+            for (int j = 0; j < LENS_STRIP; ++j) w[j] = 0.f;
+            for (int e = -cc; e < cc + LENS_STRIP; ++e) {
+#pragma unroll
+                for (int j = LENS_STRIP - 1; j > 0; --j) w[j] = w[j - 1];   // dx(j) = cc + j - e
+                int dx0 = cc - e;
+                w[0] = (dx0 >= 0 && dx0 < kpsf) ? prow[dx0] : 0.f;
+                int sx = x0 + e;
+                float v = (sx >= 0 && sx < nx) ? row[sx] : 0.f;
+#pragma unroll
+                for (int j = 0; j < LENS_STRIP; ++j) out[j] = fmaf(w[j], v, out[j]);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < LENS_STRIP; ++j) {
+            int x = x0 + j;
+            if (x < nx) {
+                int p = y * nx + x;
+                if (images) images[(size_t)b * npx + p] = out[j];
+                if (chi2) {
+                    float r = data[p] - out[j];
+                    part = fmaf(ivar[p] * r, r, part);
+                }
+            }
+        }
+    }
+    if (chi2) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+        if ((tid & 31) == 0) red[tid >> 5] = part;
+        __syncthreads();
+        if (tid < 32) {
+            float v = (tid < (nthr >> 5)) ? red[tid] : 0.f;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (tid == 0) chi2[b] = v;
+        }
+    }
+    if (flags && tid == 0) flags[b] = 0;
+}
+
+cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B) {
+    lens_prep_kernel<<<(B + 63) / 64, 64, 0, c->stream>>>(d_params, B, c->d_lens_const);
+    c->launches++;
+    return cudaGetLastError();
+}
+
+cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2, int32_t* d_flags) {
+    int npx = c->grid.nx * c->grid.ny;
+    size_t smem = sizeof(float) * (LC_SIZE + ((c->kpsf * c->kpsf + 3) & ~3) + npx);
+    static size_t configured = 0;
+    if (smem > configured) {
+        cudaError_t e = cudaFuncSetAttribute(lens_image_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        configured = smem;
+    }
+    lens_image_kernel<<<B, 512, smem, c->stream>>>(c->d_lens_const, c->grid, c->d_psf, c->kpsf, c->d_data, c->d_ivar,
+                                                  d_images, d_chi2, d_flags);
+    c->launches++;
+    return cudaGetLastError();
+}

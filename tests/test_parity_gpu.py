@@ -1,0 +1,141 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 CPU oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json's: 1e-4 relative per model-image pixel and per v_rms
+bin, 1e-5 relative on the (joint and lens-only) log-likelihood; pixels below 1e-6 of the image maximum
+are compared absolutely."""
+import math
+
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+PIX_RTOL, BIN_RTOL, LNL_RTOL = 1e-4, 1e-4, 1e-5
+
+
+@pytest.fixture(scope="module")
+def glad_mod():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_2504_01302_b200 as m
+    return m
+
+
+def oracle_data_model(oracle):
+    def dm(w):
+        img = vr = None
+        if w["lens"]:
+            img = oracle.lens_image_batch(w["lens"]["params"], w["lens"]["grid"], w["lens"]["psf"])["images"][0]
+        if w["dyn"]:
+            d = w["dyn"]
+            vr = oracle.jam_vrms_batch(d["params"], d["lum_mge"], d["mass_mge"], d["beta"], d["kin"])["vrms"][0]
+        return img, vr
+    return dm
+
+
+def check_images(gpu, ref):
+    for b in range(ref.shape[0]):
+        mx = np.abs(ref[b]).max()
+        tol = PIX_RTOL * np.maximum(np.abs(ref[b]), 1e-6 * mx)
+        bad = np.abs(gpu[b] - ref[b]) > tol
+        assert not bad.any(), f"vector {b}: {bad.sum()} pixels off, worst rel {np.max(np.abs(gpu[b] - ref[b]) / np.maximum(np.abs(ref[b]), 1e-6 * mx)):.2e}"
+
+
+def rel(a, b):
+    return np.max(np.abs(np.asarray(a, np.float64) - b) / np.abs(b))
+
+
+def run_lens(glad_mod, oracle, wl, idx=None, images=True):
+    L = wl["lens"]
+    g = glad_mod.Glad(0)
+    g.set_image_data(L["grid"], L["psf"], L["data"], L["ivar"])
+    out = g.lens_image_batch(L["params"], want_images=images)
+    sub = L["params"] if idx is None else L["params"][idx]
+    ref = oracle.lens_image_batch(sub, L["grid"], L["psf"], L["data"], L["ivar"], want_images=images)
+    sel = slice(None) if idx is None else idx
+    if images:
+        check_images(out["images"].cpu().numpy()[sel].astype(np.float64), ref["images"])
+    chi = out["chi2"].cpu().numpy()[sel]
+    assert rel(chi, ref["chi2"]) < LNL_RTOL, (chi, ref["chi2"])
+    assert (out["flags"].cpu().numpy() == 0).all()
+    g.close()
+    return chi, ref["chi2"]
+
+
+def run_jam(glad_mod, oracle, wl, idx=None, maps=True):
+    D = wl["dyn"]
+    g = glad_mod.Glad(0)
+    g.set_kin_data(D["kin"])
+    out = g.jam_vrms_batch(D["params"], D["lum_mge"], D["mass_mge"], D["beta"], want_map=maps)
+    s = wl if idx is None else workloads.subset(wl, idx)
+    d = s["dyn"]
+    ref = oracle.jam_vrms_batch(d["params"], d["lum_mge"], d["mass_mge"], d["beta"], d["kin"], want_maps=maps)
+    sel = slice(None) if idx is None else idx
+    v = out["vrms"].cpu().numpy()[sel]
+    assert rel(v, ref["vrms"]) < BIN_RTOL
+    if maps:
+        assert rel(out["v2map"].cpu().numpy()[sel], ref["v2map"]) < BIN_RTOL
+    chi = out["chi2"].cpu().numpy()[sel].astype(np.float64)
+    # chi2_D alone near the truth is ill-conditioned: bound it by the v_rms tolerance
+    kin = D["kin"]
+    slack = 2 * np.sqrt(ref["chi2"] * np.sum(kin["vrms_ivar"].astype(np.float64) * (BIN_RTOL * ref["vrms"]) ** 2, axis=1)) + 1e-3
+    assert (np.abs(chi - ref["chi2"]) <= slack).all(), (chi, ref["chi2"])
+    assert (out["flags"].cpu().numpy() == 0).all()
+    g.close()
+    return chi, ref["chi2"]
+
+
+def run_joint(glad_mod, oracle, wl, idx=None):
+    L, D = wl["lens"], wl["dyn"]
+    g = glad_mod.Glad(0)
+    g.set_image_data(L["grid"], L["psf"], L["data"], L["ivar"])
+    g.set_kin_data(D["kin"])
+    out = g.joint_loglike_batch(L["params"], D["params"], D["lum_mge"], D["mass_mge"], D["beta"])
+    s = wl if idx is None else workloads.subset(wl, idx)
+    ol = oracle.lens_image_batch(s["lens"]["params"], L["grid"], L["psf"], L["data"], L["ivar"], want_images=False)
+    d = s["dyn"]
+    od = oracle.jam_vrms_batch(d["params"], d["lum_mge"], d["mass_mge"], d["beta"], d["kin"])
+    ref = oracle.joint_loglike(ol["chi2"], od["chi2"])
+    sel = slice(None) if idx is None else idx
+    ll = out["loglike"].cpu().numpy()[sel]
+    assert rel(ll, ref) < LNL_RTOL, (ll, ref)
+    assert rel(out["chi2_lens"].cpu().numpy()[sel], ol["chi2"]) < LNL_RTOL
+    g.close()
+    return ll, ref
+
+
+# ------------------------------------------------------------------------------------------- configs
+def test_c1_tiny_full_batch(glad_mod, oracle):
+    wl = workloads.make_workload("C1", oracle_data_model(oracle))
+    run_lens(glad_mod, oracle, wl)
+    run_jam(glad_mod, oracle, wl)
+    run_joint(glad_mod, oracle, wl)
+
+
+def test_c2_rxj1131_subbatch_and_full_batch_samples(glad_mod, oracle):
+    wl = workloads.make_workload("C2", oracle_data_model(oracle))
+    idx = np.array([0, 1, 2, 3, 100, 511, 777, 1023])
+    run_lens(glad_mod, oracle, wl, idx)                 # full batch of 1024 on the GPU, 8 sampled vs the oracle
+    run_jam(glad_mod, oracle, wl, idx)
+    run_joint(glad_mod, oracle, wl, idx)
+
+
+def test_c3_dynamics_sweep_cells(glad_mod, oracle):
+    dm = oracle_data_model(oracle)
+    for name, idx in (("C3-10-40-256", [0, 1, 2, 3, 4, 5, 6, 255]), ("C3-40-80-256", [0, 200]), ("C3-20-160-256", [0, 77])):
+        wl = workloads.make_workload(name, dm)
+        run_jam(glad_mod, oracle, wl, np.array(idx), maps=True)
+
+
+def test_c4_lens_only_subbatch(glad_mod, oracle):
+    wl = workloads.make_workload("C4", oracle_data_model(oracle), B=512)
+    run_lens(glad_mod, oracle, wl, np.array([0, 1, 2, 3, 4, 5, 6, 7, 300, 511]))
+
+
+def test_c5_joint_stress_subbatch(glad_mod, oracle):
+    wl = workloads.make_workload("C5", oracle_data_model(oracle), B=160)
+    idx = np.array([0, 1, 159])
+    run_lens(glad_mod, oracle, wl, idx)
+    run_joint(glad_mod, oracle, wl, idx)
