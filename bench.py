@@ -1,0 +1,308 @@
+#!/usr/bin/env python
+"""bench.py -- joint log-likelihood evaluations / s on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (rows a0-a9: glad_joint_loglike_batch) over one batch of the
+RXJ1131-shaped synthetic workload (BASELINE.json configs[1] = "C2": 1024 parameter vectors).
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--impl ours|reference]
+N > 1 is launched by torch.distributed.run; batch elements are independent, so every rank evaluates its
+own full batch with no data-path collective ("weak" scaling); NCCL is used only for the barrier and the
+max-over-ranks of the device time.  Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "joint_loglike_evals_per_s"
+UNIT = "evals/s"
+FP32_LANES_PER_SM = 128
+
+
+def read_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p))
+        except Exception:
+            pass
+    return {}
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.proc = index, [], None
+
+    def run(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            for line in self.proc.stdout:
+                self.rows.append([c.strip() for c in line.split(",")])
+        except Exception:
+            pass
+
+    def stop(self) -> dict:
+        if self.proc:
+            self.proc.terminate()
+        self.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def oracle_data_model():
+    import oracle
+
+    def dm(w):
+        img = vr = None
+        if w["lens"]:
+            img = oracle.lens_image_batch(w["lens"]["params"], w["lens"]["grid"], w["lens"]["psf"])["images"][0]
+        if w["dyn"]:
+            d = w["dyn"]
+            vr = oracle.jam_vrms_batch(d["params"], d["lum_mge"], d["mass_mge"], d["beta"], d["kin"])["vrms"][0]
+        return img, vr
+    return dm
+
+
+def gpu_data_model(device):
+    """Mock data from the library's own forward model at the truth vector (what a user does to make a mock)."""
+    from paper_2504_01302_b200 import Glad
+
+    def dm(w):
+        g = Glad(device)
+        img = vr = None
+        if w["lens"]:
+            g.set_image_data(w["lens"]["grid"], w["lens"]["psf"])
+            img = g.lens_image_batch(w["lens"]["params"], want_chi2=False)["images"][0].cpu().numpy()
+        if w["dyn"]:
+            d = w["dyn"]
+            kin = dict(d["kin"]); kin["vrms_obs"] = kin["vrms_ivar"] = None
+            g.set_kin_data(kin)
+            vr = g.jam_vrms_batch(d["params"], d["lum_mge"], d["mass_mge"], d["beta"], want_chi2=False)["vrms"][0].cpu().numpy()
+        g.close()
+        return img, vr
+    return dm
+
+
+def oracle_joint(wl):
+    import oracle
+    L, D = wl["lens"], wl["dyn"]
+    c2l = oracle.lens_image_batch(L["params"], L["grid"], L["psf"], L["data"], L["ivar"], want_images=False)["chi2"]
+    c2d = oracle.jam_vrms_batch(D["params"], D["lum_mge"], D["mass_mge"], D["beta"], D["kin"])["chi2"]
+    return oracle.joint_loglike(c2l, c2d)
+
+
+def workload_terms(wl):
+    """Contraction size of row a6 per vector: K = nu * (n_mass + BH) * n_lum."""
+    D = wl["dyn"]
+    nm = D["mass_mge"].shape[-2] + (D["params"][:, 2] > 0).astype(np.int64)
+    return D["kin"]["u_nodes"].size * nm * D["lum_mge"].shape[-2]
+
+
+def run_reference(args, rank):
+    """--impl reference: the fp64 CPU oracle as it stands on the box's host cores, bounded sample per step."""
+    if rank != 0:
+        return
+    import oracle
+    import workloads
+    oracle.build()
+    n_sample = args.ref_sample
+    wl = workloads.make_workload(args.config, oracle_data_model(), B=n_sample)
+    for _ in range(args.warmup if args.warmup < 1 else 1):
+        oracle_joint(workloads.subset(wl, [0]))
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_joint(wl)
+    dt = time.perf_counter() - t0
+    value = n_sample * args.steps / dt
+    cores = oracle.num_threads()
+    sample = f"{n_sample} seeded {args.config} vectors per step (element 0 = truth), OpenMP over the batch"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.config} (BASELINE.json configs[1], RXJ1131-shaped joint model), bounded sample"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import workloads
+    from paper_2504_01302_b200 import Glad
+
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    wl = workloads.make_workload(args.config, gpu_data_model(local_rank), B=args.batch)
+    L, D = wl["lens"], wl["dyn"]
+    B = wl["B"]
+    g = Glad(local_rank)
+    g.set_image_data(L["grid"], L["psf"], L["data"], L["ivar"])
+    g.set_kin_data(D["kin"])
+    dev = torch.device("cuda", local_rank)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32))
+    host = {k: t(v).pin_memory() for k, v in (("lens", L["params"]), ("dyn", D["params"]), ("lum", D["lum_mge"]),
+                                               ("mass", D["mass_mge"]), ("beta", D["beta"]))}
+    d = {k: v.to(dev) for k, v in host.items()}
+    out = {"loglike": torch.empty(B, device=dev), "chi2_lens": torch.empty(B, device=dev),
+           "chi2_dyn": torch.empty(B, device=dev), "flags": torch.empty(B, dtype=torch.int32, device=dev)}
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)   # > 126 MB L2
+
+    def step():
+        g.joint_loglike_batch(d["lens"], d["dyn"], d["lum"], d["mass"], d["beta"], out=out)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.25)
+    g.profile_enable(True)
+    g.profile_read()
+    n0 = g.launch_count
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    for (e0, e1) in evs:
+        flush.zero_()                       # L2 flush between timed iterations (outside the per-step events)
+        e0.record()
+        step()
+        e1.record()
+    barrier()
+    launches = g.launch_count - n0
+    prof = g.profile_read()
+    g.profile_enable(False)
+    ms = float(sum(e0.elapsed_time(e1) for e0, e1 in evs))
+
+    # end to end through the host-buffer C entry point: H2D of every input + D2H of lnL inside the timed region
+    h_out = torch.empty(B, dtype=torch.float32).pin_memory()
+    e2e_steps = max(3, min(args.steps, 10))
+    g.joint_loglike_host(host["lens"], host["dyn"], host["lum"], host["mass"], host["beta"], h_out)
+    barrier()
+    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a0.record()
+    for _ in range(e2e_steps):
+        g.joint_loglike_host(host["lens"], host["dyn"], host["lum"], host["mass"], host["beta"], h_out)
+    a1.record()
+    barrier()
+    e2e_ms = a0.elapsed_time(a1)
+    clocks = sampler.stop()
+
+    if dist is not None:
+        tt = torch.tensor([ms, e2e_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms, e2e_ms = float(tt[0]), float(tt[1])
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    ms_per_step = ms / args.steps
+    value = world * B / (ms_per_step * 1e-3)
+    e2e_value = world * B / (e2e_ms / e2e_steps * 1e-3)
+    h2d = sum(v.numel() * 4 for v in host.values())
+    # roofline of the dominant kernel (row a6, jam_quad): algorithmic flops = 2 per (folded pixel, contraction row)
+    peaks = read_peaks()
+    props = torch.cuda.get_device_properties(local_rank)
+    sm_max = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+    peak_tf = props.multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    nx, ny = D["kin"]["xs"].size, D["kin"]["ys"].size
+    npf = ((nx + 1) // 2) * ((ny + 1) // 2)           # the bench grids are mirror-symmetric in both axes
+    flops_per_launch = 2.0 * npf * float(workload_terms(wl).sum())
+    q_ms, q_n = prof["jam_quad"]
+    q_avg = q_ms / max(q_n, 1)
+    achieved = flops_per_launch / (q_avg * 1e-3) / 1e12 if q_n else None
+    shares = {k: round(v[0] / ms, 4) for k, v in prof.items()}
+    roofline = {"bound": "alu", "kernel": "jam_quad_kernel", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": (achieved / peak_tf) if achieved else None, "traffic": None,
+                "peak_source": f"{props.multi_processor_count} SM x 128 FP32 lanes x 2 flop x {sm_max:.0f} MHz (DESIGN.md)",
+                "ms_per_launch": q_avg, "algorithmic_flops_per_launch": flops_per_launch, "kernel_share_of_step": shares}
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        ns = args.ref_sample
+        cwl = workloads.make_workload(args.config, oracle_data_model(), B=ns)
+        t0 = time.perf_counter()
+        oracle_joint(cwl)
+        dt = time.perf_counter() - t0
+        cpu = {"value": ns / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{ns} seeded {args.config} vectors (element 0 = truth), one pass, OpenMP over the batch"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": f"{args.config} (BASELINE.json configs[1], RXJ1131-shaped joint model)", "batch_per_gpu": B,
+                       "image": f"{L['grid']['nx']}x{L['grid']['ny']} s={L['grid']['supersample']} psf={L['psf'].shape[0]}",
+                       "jam": f"{D['lum_mge'].shape[-2]}+{D['mass_mge'].shape[-2]}(+BH) Gaussians, {nx}x{ny} sky grid, "
+                              f"{D['kin']['nbins']} bins, {D['kin']['u_nodes'].size} nodes",
+                       "l2": "256 MiB buffer zeroed between timed steps (outside the per-step events)",
+                       "parallelism": f"dp{world} (independent batches, no collective)"},
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": B * 4,
+                    "steps": e2e_steps, "api": "glad_joint_loglike_host (pinned host buffers)"},
+            "roofline": roofline, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    g.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C2")
+    ap.add_argument("--batch", type=int, default=None, help="override the per-GPU batch (default: the config's)")
+    ap.add_argument("--ref-sample", type=int, default=16, help="vectors per oracle pass (cpu_baseline / reference)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if world == 1 and args.gpus > 1:
+        # convenience: re-launch under torch.distributed.run
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", "29531", os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
+    run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

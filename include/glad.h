@@ -176,6 +176,16 @@ glad_status glad_joint_loglike_host(glad_ctx* ctx, const float* h_lens_params, c
  * caller keeps lens[8] consistent with dyn[2] and the sampled D_dt.  Pure host arithmetic. */
 double glad_bh_theta2(double mbh_msun, double ddt_mpc, double z_d);
 
+/*
+ * Optional per-kernel timing for bench.py's roofline line: when enabled, a CUDA event pair is recorded on the
+ * context stream around every kernel launch (at most 2048 launches between reads).  glad_profile_read
+ * SYNCHRONISES the stream, adds the elapsed times to per-kernel totals, copies them out and clears them.
+ * Kernel order: 0 lens_prep, 1 lens_image, 2 jam_prep, 3 jam_quad, 4 jam_post, 5 joint.
+ */
+#define GLAD_NKERNELS 6
+glad_status glad_profile_enable(glad_ctx* ctx, int on);
+glad_status glad_profile_read(glad_ctx* ctx, double* ms_out /*[GLAD_NKERNELS]*/, long* count_out /*[GLAD_NKERNELS]*/);
+
 /* Number of kernel launches enqueued by this context since creation (for bench.py's gpu_launches). */
 long glad_launch_count(const glad_ctx* ctx);
 

@@ -18,7 +18,8 @@ FLAG_LENS_INVALID, FLAG_DYN_INVALID, FLAG_BIN_INVALID = 1, 2, 4
 _lib = None
 EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "glad_set_image_data",
            "glad_set_kin_data", "glad_lens_image_batch", "glad_jam_vrms_batch", "glad_joint_loglike_batch",
-           "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count"]
+           "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count", "glad_profile_enable",
+           "glad_profile_read"]
 
 
 class GladError(RuntimeError):
@@ -66,6 +67,10 @@ def load(rebuild: bool = False):
     L.glad_joint_loglike_host.argtypes = [vp, vp, vp, i, vp, i, l, vp, i, l, vp, i, vp, vp, vp, vp]
     L.glad_bh_theta2.restype = C.c_double
     L.glad_bh_theta2.argtypes = [C.c_double] * 3
+    L.glad_profile_enable.restype = i
+    L.glad_profile_enable.argtypes = [vp, i]
+    L.glad_profile_read.restype = i
+    L.glad_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_long)]
     L.glad_launch_count.restype = l
     L.glad_launch_count.argtypes = [vp]
     _lib = L
@@ -127,6 +132,18 @@ class Glad:
     def launch_count(self) -> int:
         return int(self.lib.glad_launch_count(self.ctx))
 
+    KERNELS = ("lens_prep", "lens_image", "jam_prep", "jam_quad", "jam_post", "joint")
+
+    def profile_enable(self, on: bool = True):
+        self._check(self.lib.glad_profile_enable(self.ctx, 1 if on else 0))
+
+    def profile_read(self) -> dict:
+        """{kernel: (total ms, launches)} since the last read (synchronises the stream)."""
+        ms = (C.c_double * 6)()
+        cnt = (C.c_long * 6)()
+        self._check(self.lib.glad_profile_read(self.ctx, ms, cnt))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(self.KERNELS)}
+
     # ---- static data -------------------------------------------------------------------------
     def set_image_data(self, grid: dict, psf, data=None, ivar=None):
         f = torch.float32
@@ -157,7 +174,7 @@ class Glad:
         out = out or {}
         img = out.get("images") if want_images else None
         if want_images and img is None:
-            img = torch.empty((B,) + self.image_shape, dtype=torch.float32, device=self.device)
+            img = torch.empty((B,) + (self.image_shape or (0, 0)), dtype=torch.float32, device=self.device)
         chi2 = (out.get("chi2") if out.get("chi2") is not None else torch.empty(B, dtype=torch.float32, device=self.device)) if want_chi2 else None
         flags = out.get("flags") if out.get("flags") is not None else torch.empty(B, dtype=torch.int32, device=self.device)
         self._check(self.lib.glad_lens_image_batch(self.ctx, _p(p), B, _p(img), _p(chi2), _p(flags)))
@@ -177,7 +194,7 @@ class Glad:
         lum, nl, ls, mass, nm, ms, bt, pg = self._tables(lum_mge, mass_mge, beta)
         vrms = torch.empty((B, self.nbins), dtype=torch.float32, device=self.device)
         chi2 = torch.empty(B, dtype=torch.float32, device=self.device) if want_chi2 else None
-        v2map = torch.empty((B,) + self.sky_shape, dtype=torch.float32, device=self.device) if want_map else None
+        v2map = torch.empty((B,) + (self.sky_shape or (0, 0)), dtype=torch.float32, device=self.device) if want_map else None
         flags = torch.empty(B, dtype=torch.int32, device=self.device)
         self._check(self.lib.glad_jam_vrms_batch(self.ctx, _p(d), B, _p(lum), nl, ls, _p(mass) if nm else None, nm, ms,
                                                  _p(bt), pg, _p(vrms), _p(chi2), _p(v2map), _p(flags)))

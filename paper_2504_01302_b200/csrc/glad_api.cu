@@ -83,7 +83,33 @@ void glad_destroy(glad_ctx* c) {
     free_kin(c);
     void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage};
     for (void* p : ps) if (p) cudaFree(p);
+    for (cudaEvent_t e : c->prof_ev) if (e) cudaEventDestroy(e);
     delete c;
+}
+
+glad_status glad_profile_enable(glad_ctx* c, int on) {
+    if (!c) return GLAD_EINVAL;
+    c->prof_on = on != 0;
+    return GLAD_OK;
+}
+
+glad_status glad_profile_read(glad_ctx* c, double* ms_out, long* count_out) {
+    if (!c || !ms_out || !count_out) return GLAD_EINVAL;
+    cudaSetDevice(c->device);
+    CU(cudaStreamSynchronize(c->stream), "profile sync");
+    for (int i = 0; i < c->prof_n; ++i) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]) == cudaSuccess) {
+            c->prof_ms[c->prof_id[i]] += ms;
+            c->prof_cnt[c->prof_id[i]] += 1;
+        }
+    }
+    c->prof_n = 0;
+    for (int k = 0; k < GLAD_NKERNELS; ++k) {
+        ms_out[k] = c->prof_ms[k]; count_out[k] = c->prof_cnt[k];
+        c->prof_ms[k] = 0.0; c->prof_cnt[k] = 0;
+    }
+    return GLAD_OK;
 }
 
 const char* glad_last_error(const glad_ctx* c) { return c ? c->err : "null context"; }

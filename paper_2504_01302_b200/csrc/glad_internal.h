@@ -44,6 +44,9 @@ static inline __host__ __device__ int jam_table_floats(int nl, int nmx) {
 #define JQ_T 8
 #define JQ_MI 8
 
+#define GLAD_PROF_MAX 2048
+enum GladKernelId { GK_LENS_PREP = 0, GK_LENS_IMAGE, GK_JAM_PREP, GK_JAM_QUAD, GK_JAM_POST, GK_JOINT };
+
 struct glad_ctx {
     int device;
     cudaStream_t stream;
@@ -80,6 +83,28 @@ struct glad_ctx {
     float* d_tmp;        size_t tmp_cap;     // chi2_L, chi2_D [B] each
     int32_t* d_tmpflags; size_t tmpflags_cap; // flags_L, flags_D [B] each
     float* d_stage;      size_t stage_cap;   // device staging of glad_joint_loglike_host
+
+    // optional per-kernel timing (glad_profile_*): CUDA events on the context stream around each launch
+    bool prof_on;
+    int prof_n;
+    cudaEvent_t prof_ev[2 * GLAD_PROF_MAX];
+    int prof_id[GLAD_PROF_MAX];
+    double prof_ms[GLAD_NKERNELS];
+    long prof_cnt[GLAD_NKERNELS];
+};
+
+// Records an event pair around one launch when profiling is on (RAII; the launch goes between ctor and dtor).
+struct ProfScope {
+    glad_ctx* c; int slot;
+    ProfScope(glad_ctx* ctx, int id) : c(ctx), slot(-1) {
+        c->launches++;
+        if (!c->prof_on || c->prof_n >= GLAD_PROF_MAX) return;
+        slot = c->prof_n++;
+        c->prof_id[slot] = id;
+        if (!c->prof_ev[2 * slot]) { cudaEventCreate(&c->prof_ev[2 * slot]); cudaEventCreate(&c->prof_ev[2 * slot + 1]); }
+        cudaEventRecord(c->prof_ev[2 * slot], c->stream);
+    }
+    ~ProfScope() { if (slot >= 0) cudaEventRecord(c->prof_ev[2 * slot + 1], c->stream); }
 };
 
 // kernel launchers (return cudaGetLastError())

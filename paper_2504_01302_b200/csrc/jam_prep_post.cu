@@ -136,18 +136,18 @@ __global__ void kin_weights_kernel(const int32_t* __restrict__ bin_id, const flo
 
 cudaError_t launch_kin_weights(glad_ctx* c) {
     long n = (long)c->nbins * c->nxf * c->nyf;
+    c->launches++;
     kin_weights_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(c->d_bin_id, c->d_kernel, c->kk, c->nx, c->ny,
                                                                          c->nxf, c->nyf, c->d_unfoldx, c->d_unfoldy,
                                                                          c->nbins, c->d_binw);
-    c->launches++;
     return cudaGetLastError();
 }
 
 cudaError_t launch_jam_prep(glad_ctx* c, const float* d_dyn, int B, const float* d_lum, int nl, long lum_stride,
                             const float* d_mass, int nm, long mass_stride, const float* d_beta, int per_gaussian) {
+    ProfScope ps(c, GK_JAM_PREP);
     jam_prep_kernel<<<B, 128, 0, c->stream>>>(d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta,
                                              per_gaussian, c->d_jam_tab);
-    c->launches++;
     return cudaGetLastError();
 }
 
@@ -254,11 +254,11 @@ cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d
         if (e != cudaSuccess) return e;
         configured = smem;
     }
+    ProfScope ps(c, GK_JAM_POST);
     jam_post_kernel<<<B, 256, smem, c->stream>>>(c->d_jam_tab, jam_table_floats(nl, nmx), nl, nmx, c->d_partial, S, c->nx,
                                                 c->ny, c->nxf, c->nyf, c->d_xf2, c->d_yf2, c->d_foldx, c->d_foldy,
                                                 c->d_binw, c->d_bin_cnt, c->nbins, c->d_vobs, c->d_vivar, d_vrms,
                                                 d_chi2, d_v2map, d_flags);
-    c->launches++;
     return cudaGetLastError();
 }
 
@@ -276,7 +276,7 @@ __global__ void joint_kernel(int B, const float* __restrict__ c2l, const float* 
 
 cudaError_t launch_joint(glad_ctx* c, int B, const float* d_c2l, const float* d_c2d, const int32_t* d_fl,
                          const int32_t* d_fd, float* d_loglike, int32_t* d_flags) {
+    ProfScope ps(c, GK_JOINT);
     joint_kernel<<<(B + 127) / 128, 128, 0, c->stream>>>(B, d_c2l, d_c2d, d_fl, d_fd, d_loglike, d_flags);
-    c->launches++;
     return cudaGetLastError();
 }

@@ -219,7 +219,7 @@ cudaError_t launch_jam_quad(glad_ctx* c, int B, int nl, int nmx, int S) {
         if (e != cudaSuccess) return e;
         configured = smem;
     }
+    ProfScope ps(c, GK_JAM_QUAD);
     jam_quad_kernel<<<B * S, NT, smem, c->stream>>>(a);
-    c->launches++;
     return cudaGetLastError();
 }

@@ -271,8 +271,8 @@ __global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict
 }
 
 cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B) {
+    ProfScope ps(c, GK_LENS_PREP);
     lens_prep_kernel<<<(B + 63) / 64, 64, 0, c->stream>>>(d_params, B, c->d_lens_const);
-    c->launches++;
     return cudaGetLastError();
 }
 
@@ -285,8 +285,8 @@ cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2
         if (e != cudaSuccess) return e;
         configured = smem;
     }
+    ProfScope ps(c, GK_LENS_IMAGE);
     lens_image_kernel<<<B, 512, smem, c->stream>>>(c->d_lens_const, c->grid, c->d_psf, c->kpsf, c->d_data, c->d_ivar,
                                                   d_images, d_chi2, d_flags);
-    c->launches++;
     return cudaGetLastError();
 }

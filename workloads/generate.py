@@ -118,7 +118,10 @@ def _lum_mge_sersic(n_ser, re, qp, n, scale=1000.0):
     prof = np.exp(-bn * ((r / re) ** (1.0 / n_ser) - 1.0))
     sig = np.geomspace(0.02, 10.0, n)
     basis = np.exp(-r[:, None] ** 2 / (2 * sig[None, :] ** 2)) / prof[:, None]
-    amp, _ = nnls(basis, np.ones_like(r))
+    try:
+        amp, _ = nnls(basis, np.ones_like(r), maxiter=200 * n)
+    except RuntimeError:                       # scipy's active-set NNLS may cycle; any non-negative table will do
+        amp = np.maximum(np.linalg.lstsq(basis, np.ones_like(r), rcond=1e-8)[0], 0.0)
     amp = np.maximum(amp, 1e-4 * amp.max())
     return np.stack([scale * amp, sig, np.full(n, qp)], axis=1)
 
