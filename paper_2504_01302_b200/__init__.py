@@ -3,3 +3,4 @@ sm_100a CUDA kernels behind the C ABI in include/glad.h.  `Glad` is the thin Pyt
 from .binding import (EXPORTS, FLAG_BIN_INVALID, FLAG_DYN_INVALID, FLAG_LENS_INVALID, NDYN, NLENS, Glad,  # noqa: F401
                       GladError, bh_theta2, load)
 from .build import build  # noqa: F401
+from .sharding import gather_loglike, shard_range  # noqa: F401
