@@ -2,6 +2,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
@@ -62,6 +63,8 @@ glad_status glad_create(glad_ctx** out, int device, void* cuda_stream) {
         return GLAD_ECUDA;
     }
     c->sm_count = prop.multiProcessorCount;
+    const char* jp = getenv("GLAD_JAM_PATH");
+    c->jam_simt = (jp && strcmp(jp, "simt") == 0) ? 1 : 0;
     *out = c;
     return GLAD_OK;
 }
@@ -263,7 +266,8 @@ static glad_status jam_impl(glad_ctx* c, const float* d_dyn, int B, const float*
     st = grow(c, &c->d_partial, &c->partial_cap, (size_t)B * S * c->nxf * c->nyf);
     if (st != GLAD_OK) return st;
     CU(launch_jam_prep(c, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian), "jam_prep_kernel");
-    CU(launch_jam_quad(c, B, nl, nmx, S), "jam_quad_kernel");
+    if (!c->jam_simt && jam_quad_tc_supported(c)) CU(launch_jam_quad_tc(c, B, nl, nmx, S), "jam_quad_tc_kernel");
+    else CU(launch_jam_quad(c, B, nl, nmx, S), "jam_quad_kernel");
     CU(launch_jam_post(c, B, nl, nmx, S, d_vrms, d_chi2, d_v2map, d_flags), "jam_post_kernel");
     return GLAD_OK;
 }

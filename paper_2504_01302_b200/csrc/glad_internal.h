@@ -53,6 +53,7 @@ struct glad_ctx {
     int sm_count;
     char err[512];
     long launches;
+    int jam_simt;   // 1 = force the FP32 SIMT quadrature kernel (env GLAD_JAM_PATH=simt); default tcgen05
 
     // lensing static data
     bool have_image;
@@ -118,5 +119,8 @@ cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d
 cudaError_t launch_joint(glad_ctx* c, int B, const float* d_c2l, const float* d_c2d, const int32_t* d_fl,
                          const int32_t* d_fd, float* d_loglike, int32_t* d_flags);
 cudaError_t launch_kin_weights(glad_ctx* c);
+// tensor-core (tcgen05) form of row a6; supported when the folded grid has ny_f <= 128 and nx_f <= 256
+bool jam_quad_tc_supported(const glad_ctx* c);
+cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S);
 // launch geometry of the quadrature kernel for the current sky grid: threads per CTA, thread groups
 int jam_quad_geometry(const glad_ctx* c, int* groups);

@@ -19,6 +19,13 @@ def glad_mod():
     return m
 
 
+@pytest.fixture(autouse=True, params=["tc", "simt"])
+def jam_path(request, monkeypatch):
+    """Every edge case runs on both forms of row a6: tcgen05 (default) and the FP32 SIMT kernel."""
+    monkeypatch.setenv("GLAD_JAM_PATH", request.param)
+    return request.param
+
+
 def u_nodes(n):
     return workloads.gauss_legendre_u(n)
 
