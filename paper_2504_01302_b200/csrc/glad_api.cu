@@ -261,6 +261,7 @@ static glad_status jam_impl(glad_ctx* c, const float* d_dyn, int B, const float*
     if (S > 32) S = 32;
     if (S > NCH) S = NCH;
     if (S < 1) S = 1;
+    if (const char* e = getenv("GLAD_JAM_SLICES")) { int v = atoi(e); if (v >= 1 && v <= NCH) S = v; }
     glad_status st = grow(c, &c->d_jam_tab, &c->jam_tab_cap, (size_t)B * jam_table_floats(nl, nmx));
     if (st != GLAD_OK) return st;
     st = grow(c, &c->d_partial, &c->partial_cap, (size_t)B * S * c->nxf * c->nyf);

@@ -1,33 +1,51 @@
 // Row a6 on the 5th-generation tensor cores (tcgen05 + TMEM), the default path of libglad.
 //
 // Same contraction as jam_quad.cu:  S[iy,ix] = sum_m Y[m,iy] * X[m,ix]  with operands generated on the fly,
-// but the operands go from shared memory straight into tcgen05.mma (kind::tf32, fp32 accumulate in TMEM) instead
-// of through registers: profiles/r1a.md shows the FP32 SIMT form is bound by shared-memory -> register operand
-// delivery (an 8x8 register tile needs one LDS wavefront per FFMA issue slot).
+// but the operands go from shared memory straight into tcgen05.mma instead of through registers: profiles/r1a.md
+// shows the FP32 SIMT form is bound by shared-memory -> register operand delivery.
 //
-// fp32-grade accuracy from TF32 tensor cores: every operand value v is split as v = hi + lo with hi = v rounded
-// to TF32 (10-bit mantissa) and lo = v - hi (exact in fp32), and three MMAs are issued per K-step:
-//     D += Yhi*Xhi + Yhi*Xlo + Ylo*Xhi            (the dropped lo*lo term is 2^-22 relative)
+// fp32-grade accuracy from BF16 tensor-core inputs.  Every operand value v is split into NT bf16 terms
+//     v = v1 + v2 (+ v3),   v1 = bf16_rn(v),  v2 = bf16_rn(v - v1),  v3 = bf16_rn(v - v1 - v2)
+// (residuals are exact in fp32; NT = 2 keeps 16 mantissa bits, |error| <= 2^-17 |v|, NT = 3 keeps 24).  With
+// A = [Y1 ; Y2 ; ..] stacked along M and B = [X1 | X2 | ..] stacked along N, ONE kind::f16 MMA per K = 16 step
+// yields every cross product Yi*Xj in its own (row block, column block) of the accumulator; an M <= 128 tile
+// costs the same as M = 128, so the split is paid only in N.  The epilogue adds the blocks.  Folded maps whose
+// NT row blocks do not fit in M = 128 issue NT MMAs per K-step instead: Yt x [X1 | .. | X(NT-t)], all into the
+// same columns (the dropped products are 2^-8NT relative).
+//
+// The tensor core adds into its fp32 accumulator with TRUNCATION (measured on B200: one accumulator over the
+// whole contraction, 3360 K-steps, is biased by -1.4e-4 relative).  So the contraction is cut into groups of
+// FL chunks; each group accumulates in its own TMEM buffer (two alternate) and is then added, with ordinary
+// round-to-nearest FADDs, into fp32 registers that hold the running map.
+//
+// Operand layout = UMMA canonical K-major, no swizzle: core matrix = 8 rows (pixels) x 16 bytes (8 consecutive
+// contraction rows, an "oct"), 128 contiguous bytes; SBO = 128 B between 8-pixel groups, LBO between the two
+// octs of one K = 16 step.  A quarter-warp writes one core matrix with one conflict-free 16-byte store per lane.
 //
 // CTA = (parameter vector, K-slice), 256 threads, all of them operand producers:
 //   chunk c (MC contraction rows):  wait until the MMAs that read stage c%2 have completed (mbarrier armed by
-//   tcgen05.commit) -> coefficients of chunk c+1 -> operands of chunk c into stage c%2 in the UMMA canonical
-//   MN-major no-swizzle layout (8 k-rows x 16 B core matrices) -> fence.proxy.async -> __syncthreads ->
-//   one thread issues 3*MC/8 tcgen05.mma and commits.  The tensor core works on chunk c while the CUDA cores
-//   produce chunk c+1.  Epilogue: tcgen05.ld the accumulator and write this slice's partial map.
+//   tcgen05.commit) -> add finished accumulator groups into registers -> coefficients of the next 256 rows ->
+//   operands of chunk c into stage c%2 -> fence.proxy.async -> __syncthreads -> one thread issues the MMAs of
+//   the chunk and commits.  The tensor core works on chunk c while the CUDA cores produce chunk c+1.
+#include <stdlib.h>
+
 #include "glad_internal.h"
 
 #define LOG2E_F 1.4426950408889634f
 #define TC_THREADS 256
+#define TC_COEF_ROWS 256
 
 struct JTArgs {
     const float* tab; int tabsz; int nl; int nmx;
     const float* un; const float* uw; int nu;
     const float* xf2; const float* yf2; int nxf, nyf;
-    int Mpad, Npad;      // UMMA M (64 / 128) and N
-    int GX, GY;          // real 4-element groups along x and y: ceil(nxf/4), ceil(nyf/4)
-    int MC, lgMC;        // contraction rows per stage (power of two, >= 32)
-    int tmem_cols;       // power of two >= 32, >= Npad
+    int ny8, nxp;        // padded map rows (multiple of 8) and columns (multiple of 8 or 16)
+    int multi;           // 0: A = [Y1;..;Y_NT] in one M=128 tile;  1: NT MMAs per K-step
+    int N;               // accumulator columns = NT * nxp
+    int MC, lgMC;        // contraction rows per stage (power of two, 64..256)
+    int FL;              // chunks per accumulator group (>= 2)
+    int npair, magic;    // block pairs per oct; item -> oct: (item * magic) >> 16 == item / npair
+    int tmem_cols;       // power of two >= 2 * N
     int S;
     float* partial;
 };
@@ -45,57 +63,81 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
                      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     } while (!ok);
 }
-// UMMA shared-memory descriptor, no swizzle, version 1 (sm_100); SBO = 128 B between 16-byte groups along M/N,
-// LBO = byte distance between 8-row K groups (one group per tf32 MMA, so it is never stepped).
+// UMMA shared-memory descriptor: K-major, no swizzle, version 1 (sm_100).  SBO = 128 B between 8-row groups
+// along M/N, LBO = byte distance between the two 16-byte K halves of a K = 16 (bf16) step.
 __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes) {
     uint32_t lo = ((saddr >> 4) & 0x3FFFu) | (((lbo_bytes >> 4) & 0x3FFFu) << 16);
     uint32_t hi = (128u >> 4) | (1u << 14);
     return ((uint64_t)hi << 32) | lo;
 }
-__device__ __forceinline__ void umma_tf32(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
+__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
-// split v = hi + lo, hi on the TF32 grid (round to nearest on the magnitude), lo exact
-__device__ __forceinline__ void split_tf32(float v, float& hi, float& lo) {
-    hi = __uint_as_float((__float_as_uint(v) + 0x1000u) & 0xFFFFE000u);
-    lo = v - hi;
+// {hi: bf16_rn(b), lo: bf16_rn(a)}: element a sits at the lower address
+__device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
+    uint32_t d; asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(b), "f"(a)); return d;
+}
+// split 8 values (one oct of one pixel) into NT bf16 terms and store one 16-byte core-matrix row per term
+template <int NT>
+__device__ __forceinline__ void split_store(float (&v)[8], uint4* dst, int term_stride16) {
+#pragma unroll
+    for (int t = 0; t < NT; ++t) {
+        uint32_t w[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            w[j] = pack_bf16(v[2 * j], v[2 * j + 1]);
+            if (t + 1 < NT) {
+                v[2 * j] -= __uint_as_float(w[j] << 16);
+                v[2 * j + 1] -= __uint_as_float(w[j] & 0xFFFF0000u);
+            }
+        }
+        dst[t * term_stride16] = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+}
+// q = a / d for 0 <= a < 2^24 with inv = 1/d (float): the estimate is off by at most one
+__device__ __forceinline__ int div_small(int a, int d, float inv) {
+    int q = __float2int_rz(__int2float_rn(a) * inv);
+    int r = a - q * d;
+    return r < 0 ? q - 1 : (r >= d ? q + 1 : q);
 }
 
-__global__ void __launch_bounds__(TC_THREADS) jam_quad_tc_kernel(JTArgs a) {
+// NT = bf16 terms per operand value, NACC = accumulator registers per thread (>= N/2, multiple of 8)
+template <int NT, int NACC>
+__global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_kernel(JTArgs a) {
     extern __shared__ __align__(128) float sm[];
     __shared__ __align__(8) uint64_t s_bar[3];     // empty[0], empty[1], done
     __shared__ uint32_t s_tmem;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int b = blockIdx.x / a.S, s = blockIdx.x - b * a.S;
     const float* Tg = a.tab + (size_t)b * a.tabsz;
-    if (__float_as_int(Tg[JH_VALID]) == 0) return;
+    if (__float_as_int(Tg[JH_VALID]) == 0) return;      // post kernel never reads this vector's partials
 
-    const int nl = a.nl, nmx = a.nmx, nu = a.nu, MC = a.MC, GX = a.GX, GY = a.GY;
+    const int nl = a.nl, nmx = a.nmx, nu = a.nu, MC = a.MC, ny8 = a.ny8, nxp = a.nxp, N = a.N;
+    const int nyb = ny8 >> 3, nxb = nxp >> 3, nblk = nyb + nxb;      // 8-pixel blocks per oct: Y blocks, then X blocks
+    const int GA = NT * nyb, GB = NT * nxb;                          // core matrices per oct: the NT terms stacked
     const int nup = (nu + 1) & ~1;
-    // operand stage: [Yhi | Ylo | Xhi | Xlo]; an array holds MC/8 K-steps of G core matrices (8 k-rows x 16 B)
-    const int ysz = MC * GY * 4, xsz = MC * (a.Npad >> 2) * 4;   // floats per array
-    const int stage_floats = 2 * ysz + 2 * xsz;
+    const int a16 = (MC >> 3) * GA * 8, b16 = (MC >> 3) * GB * 8;    // 16-byte units per stage
+    const int stage16 = a16 + b16;
     float* s_tab = sm;
     float* s_u2 = s_tab + a.tabsz;
     float* s_wu2 = s_u2 + nup;
-    float* s_c2 = s_wu2 + nup;                       // (GY + GX) * 4 squared coordinates, y first
-    float* s_coef = s_c2 + (GY + GX) * 4;            // 2 * MC * 4
-    float* s_ops = s_coef + 2 * MC * 4;              // 2 stages + tail pad (the M padding rows are read from beyond Y)
-    s_ops = (float*)(((uintptr_t)s_ops + 127) & ~(uintptr_t)127);
+    float* s_c2 = s_wu2 + nup;                       // ny8 + nxp squared coordinates, y first
+    float4* s_coef = reinterpret_cast<float4*>(sm + ((a.tabsz + 2 * nup + ny8 + nxp + 31) & ~31));   // 2 x 256 rows
+    uint4* s_ops = reinterpret_cast<uint4*>(s_coef + 2 * TC_COEF_ROWS);   // 2 stages + tail pad, 128-byte aligned
 
     for (int i = tid; i < a.tabsz; i += TC_THREADS) s_tab[i] = Tg[i];
     for (int i = tid; i < nu; i += TC_THREADS) { float u = a.un[i]; s_u2[i] = u * u; s_wu2[i] = a.uw[i] * u * u; }
-    for (int i = tid; i < (GY + GX) * 4; i += TC_THREADS) {
+    for (int i = tid; i < ny8 + nxp; i += TC_THREADS) {              // padded pixels: coordinate 0, finite values, never stored
         float v = 0.f;
-        if (i < GY * 4) { if (i < a.nyf) v = a.yf2[i]; }
-        else { int j = i - GY * 4; if (j < a.nxf) v = a.xf2[j]; }
+        if (i < ny8) { if (i < a.nyf) v = a.yf2[i]; }
+        else { int j = i - ny8; if (j < a.nxf) v = a.xf2[j]; }
         s_c2[i] = v;
     }
-    for (int i = tid; i < 2 * stage_floats + 1024; i += TC_THREADS) s_ops[i] = 0.f;   // padding groups stay zero
+    for (int i = tid; i < 2 * stage16 + 128; i += TC_THREADS) s_ops[i] = make_uint4(0u, 0u, 0u, 0u);
     if (tid == 0) {
         mbar_init(smem_u32(&s_bar[0]), 1);
         mbar_init(smem_u32(&s_bar[1]), 1);
@@ -107,7 +149,7 @@ __global__ void __launch_bounds__(TC_THREADS) jam_quad_tc_kernel(JTArgs a) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "r"(a.tmem_cols) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // the zero fill is read by the async proxy
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -120,122 +162,160 @@ __global__ void __launch_bounds__(TC_THREADS) jam_quad_tc_kernel(JTArgs a) {
     const float cos2i = s_tab[JH_COS2I];
     const int nm = __float_as_int(s_tab[JH_NM]);
     const int pairs = nm * nl;
+    const float inv_pairs = 1.f / (float)pairs, inv_nl = 1.f / (float)nl;
     const int M = nu * pairs;
     const int NCH = (M + MC - 1) >> a.lgMC;
     const int c0 = (int)(((long)s * NCH) / a.S), c1 = (int)(((long)(s + 1) * NCH) / a.S);
+    const int nch = c1 - c0;
 
-    auto coef = [&](int c, int buf) {
-        if (c >= c1) return;
-        for (int i = tid; i < MC; i += TC_THREADS) {
-            int m = c * MC + i;
-            float4 o = make_float4(0.f, 0.f, 0.f, 0.f);      // (P, Q, F0, F1); rows past the end contribute 0
-            if (m < M) {
-                int iu = m / pairs, rem = m - iu * pairs;
-                int j = rem / nl, k = rem - j * nl;
-                float u2 = s_u2[iu];
-                float omq2 = TM[JM_OMQ2 * nmx + j];
-                float auj = u2 * TM[JM_INVS2 * nmx + j];
-                float gg = 1.f - omq2 * u2;
-                float bb = omq2 * u2 * auj / gg;
-                float A = 0.5f * (auj + TL[JL_INVS2 * nl + k]);
-                float Bc = 0.5f * (TL[JL_BKQ * nl + k] + bb);
-                float E = fmaf(Bc, cos2i, A);
-                float D = fmaf(-TD[j * nl + k], u2, TL[JL_D0 * nl + k]);
-                float inv = rsqrtf(E * gg) / (1.f - TC[j * nl + k] * u2);
-                float pref = s_wu2[iu] * TM[JM_MJ * nmx + j] * inv;
-                o.x = A * LOG2E_F;
-                o.y = A * (A + Bc) / E * LOG2E_F;
-                o.z = pref * TL[JL_S0 * nl + k];
-                o.w = pref * TL[JL_NKS * nl + k] * D;
+    // per contraction row: (-P log2e, -Q log2e, F0, F1); rows past the end have F0 = F1 = 0 and contribute 0
+    auto coef_block = [&](int cbk) {
+        const int m = cbk * TC_COEF_ROWS + tid;
+        float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (m < M) {
+            const int iu = div_small(m, pairs, inv_pairs), rem = m - iu * pairs;
+            const int j = div_small(rem, nl, inv_nl), k = rem - j * nl;
+            const float u2 = s_u2[iu];
+            const float omq2 = TM[JM_OMQ2 * nmx + j];
+            const float auj = u2 * TM[JM_INVS2 * nmx + j];
+            const float gg = 1.f - omq2 * u2;
+            const float bb = __fdividef(omq2 * u2 * auj, gg);
+            const float A = 0.5f * (auj + TL[JL_INVS2 * nl + k]);
+            const float Bc = 0.5f * (TL[JL_BKQ * nl + k] + bb);
+            const float E = fmaf(Bc, cos2i, A);
+            const float D = fmaf(-TD[j * nl + k], u2, TL[JL_D0 * nl + k]);
+            const float inv = __fdividef(rsqrtf(E * gg), 1.f - TC[j * nl + k] * u2);
+            const float pref = s_wu2[iu] * TM[JM_MJ * nmx + j] * inv;
+            o.x = -A * LOG2E_F;
+            o.y = -__fdividef(A * (A + Bc), E) * LOG2E_F;
+            o.z = pref * TL[JL_S0 * nl + k];
+            o.w = pref * TL[JL_NKS * nl + k] * D;
+        }
+        s_coef[(cbk & 1) * TC_COEF_ROWS + tid] = o;
+    };
+    // item = (oct o, block pair p) per quarter-warp; lane l8 = pixel; the pair shares the 8 coefficient rows of o
+    const int qw = tid >> 3, l8 = tid & 7;
+    const int items = (MC >> 3) * a.npair;
+    auto produce = [&](int c, int buf) {
+        const float4* cf = s_coef + (((c * MC) >> 8) & 1) * TC_COEF_ROWS + ((c * MC) & (TC_COEF_ROWS - 1));
+        uint4* stA = s_ops + buf * stage16;
+        uint4* stB = stA + a16;
+        for (int it = qw; it < items; it += TC_THREADS / 8) {
+            const int o = (it * a.magic) >> 16, p = it - o * a.npair;
+            float4 k[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) k[r] = cf[8 * o + r];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int blk = p + h * a.npair;
+                if (blk >= nblk) break;
+                float v[8];
+                if (blk < nyb) {
+                    const float q = s_c2[blk * 8 + l8];
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) v[r] = ex2_tc(k[r].y * q);
+                    split_store<NT>(v, stA + (o * GA + blk) * 8 + l8, nyb * 8);
+                } else {
+                    const int bx = blk - nyb;
+                    const float q = s_c2[ny8 + bx * 8 + l8];
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) v[r] = fmaf(k[r].w, q, k[r].z) * ex2_tc(k[r].x * q);
+                    split_store<NT>(v, stB + (o * GB + bx) * 8 + l8, nxb * 8);
+                }
             }
-            reinterpret_cast<float4*>(s_coef)[buf * MC + i] = o;
         }
     };
-    // item e -> (group g = e / MC, row m = e % MC): consecutive lanes take consecutive rows of one group, so the
-    // coefficient loads and the 16-byte operand stores of a quarter-warp are contiguous (conflict-free).
-    auto produce = [&](int buf) {
-        const float4* cf = reinterpret_cast<const float4*>(s_coef) + buf * MC;
-        const float4* c2 = reinterpret_cast<const float4*>(s_c2);
-        float* st = s_ops + (size_t)buf * stage_floats;
-        const int items = MC * (GY + GX);
-        for (int e = tid; e < items; e += TC_THREADS) {
-            const int g = e >> a.lgMC, m = e & (MC - 1);
-            const float4 k = cf[m], q = c2[g];
-            float4 v, hi, lo;
-            float* dst;
-            if (g < GY) {                                    // warp-uniform (MC >= 32)
-                const float ne = -k.y;
-                v.x = ex2_tc(ne * q.x); v.y = ex2_tc(ne * q.y); v.z = ex2_tc(ne * q.z); v.w = ex2_tc(ne * q.w);
-                dst = st + (((m >> 3) * GY + g) * 8 + (m & 7)) * 4;
-                split_tf32(v.x, hi.x, lo.x); split_tf32(v.y, hi.y, lo.y); split_tf32(v.z, hi.z, lo.z); split_tf32(v.w, hi.w, lo.w);
-                *reinterpret_cast<float4*>(dst) = hi;
-                *reinterpret_cast<float4*>(dst + ysz) = lo;
-            } else {
-                const float ne = -k.x;
-                v.x = fmaf(k.w, q.x, k.z) * ex2_tc(ne * q.x);
-                v.y = fmaf(k.w, q.y, k.z) * ex2_tc(ne * q.y);
-                v.z = fmaf(k.w, q.z, k.z) * ex2_tc(ne * q.z);
-                v.w = fmaf(k.w, q.w, k.z) * ex2_tc(ne * q.w);
-                dst = st + 2 * ysz + (((m >> 3) * (a.Npad >> 2) + (g - GY)) * 8 + (m & 7)) * 4;
-                split_tf32(v.x, hi.x, lo.x); split_tf32(v.y, hi.y, lo.y); split_tf32(v.z, hi.z, lo.z); split_tf32(v.w, hi.w, lo.w);
-                *reinterpret_cast<float4*>(dst) = hi;
-                *reinterpret_cast<float4*>(dst + xsz) = lo;
-            }
+
+    // running map in registers: thread (lane quarter q, column half) holds D[32q + lane][half * NACC + i]
+    float acc[NACC];
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) acc[i] = 0.f;
+    const int lq = warp & 3, half = warp >> 2;
+    const uint32_t dstride = (uint32_t)a.tmem_cols >> 1;                // columns between the two accumulator buffers
+    auto flush = [&](int g) {
+        const uint32_t taddr = tmem + ((uint32_t)(32 * lq) << 16) + (uint32_t)(g & 1) * dstride + (uint32_t)(half * NACC);
+#pragma unroll
+        for (int i = 0; i < NACC; i += 8) {
+            uint32_t r[8];
+            asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                         : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                         : "r"(taddr + (uint32_t)i));
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (int j = 0; j < 8; ++j) acc[i + j] += __uint_as_float(r[j]);
         }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     };
 
-    // instruction descriptor: D fp32, A/B tf32, both MN-major, N>>3, M>>4
-    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)(a.Npad >> 3) << 17) |
-                           ((uint32_t)(a.Mpad >> 4) << 24);
+    // instruction descriptor: D fp32, A/B bf16, both K-major, M = 128, N>>3 filled per MMA
+    const uint32_t idesc_base = (1u << 4) | (1u << 7) | (1u << 10) | (8u << 24);
     const uint32_t ops_addr = smem_u32(s_ops);
-    const uint32_t ystep = GY * 128, xstep = (a.Npad >> 2) * 128;   // bytes per K-step inside an array
+    const uint32_t a_lbo = GA * 128, b_lbo = GB * 128;                  // bytes between the two octs of a K-step
 
-    coef(c0, 0);
-    __syncthreads();
-    for (int c = c0; c < c1; ++c) {
-        const int it = c - c0, buf = it & 1;
-        if (it >= 2) mbar_wait(smem_u32(&s_bar[buf]), ((it >> 1) - 1) & 1);   // MMAs of chunk c-2 have read this stage
-        coef(c + 1, buf ^ 1);
-        produce(buf);
+    int gf = 0;                                                         // next accumulator group to add into acc
+    if (nch > 0) {
+        coef_block((c0 * MC) >> 8);
+        __syncthreads();
+    }
+    for (int it = 0; it < nch; ++it) {
+        const int c = c0 + it, buf = it & 1;
+        if (it >= 2) {
+            mbar_wait(smem_u32(&s_bar[buf]), ((it >> 1) - 1) & 1);      // MMAs up to chunk it-2 are complete
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            while ((gf + 1) * a.FL - 1 <= it - 2) flush(gf++);
+        }
+        if (it == 0 || ((c * MC) & (TC_COEF_ROWS - 1)) == 0) coef_block(((c * MC) >> 8) + 1);
+        produce(c, buf);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
         if (tid == 0) {
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const uint32_t sb = ops_addr + (uint32_t)buf * stage_floats * 4;
-            for (int ks = 0; ks < (MC >> 3); ++ks) {
-                const uint64_t yhi = umma_desc(sb + ks * ystep, ystep), ylo = umma_desc(sb + ysz * 4 + ks * ystep, ystep);
-                const uint64_t xhi = umma_desc(sb + 2 * ysz * 4 + ks * xstep, xstep);
-                const uint64_t xlo = umma_desc(sb + 2 * ysz * 4 + xsz * 4 + ks * xstep, xstep);
-                umma_tf32(tmem, yhi, xhi, idesc, (it | ks) ? 1u : 0u);
-                umma_tf32(tmem, yhi, xlo, idesc, 1u);
-                umma_tf32(tmem, ylo, xhi, idesc, 1u);
+            const int g = it / a.FL;
+            const uint32_t d = tmem + (uint32_t)(g & 1) * dstride;
+            const uint32_t sa = ops_addr + (uint32_t)buf * stage16 * 16, sb = sa + a16 * 16;
+            uint32_t accum = (it - g * a.FL) ? 1u : 0u;
+            for (int ks = 0; ks < (MC >> 4); ++ks) {
+                const uint64_t bd = umma_desc(sb + ks * 2 * b_lbo, b_lbo);
+                if (!a.multi) {
+                    umma_bf16(d, umma_desc(sa + ks * 2 * a_lbo, a_lbo), bd, idesc_base | ((uint32_t)(N >> 3) << 17), accum);
+                } else {
+#pragma unroll
+                    for (int t = 0; t < NT; ++t) {
+                        umma_bf16(d, umma_desc(sa + ks * 2 * a_lbo + t * nyb * 128, a_lbo), bd,
+                                  idesc_base | ((uint32_t)(((NT - t) * nxp) >> 3) << 17), accum);
+                        accum = 1u;
+                    }
+                }
+                accum = 1u;
             }
             umma_commit(smem_u32(&s_bar[buf]));
-            if (c == c1 - 1) umma_commit(smem_u32(&s_bar[2]));
+            if (it == nch - 1) umma_commit(smem_u32(&s_bar[2]));
         }
         __syncwarp();
     }
 
-    // epilogue: TMEM -> registers -> this slice's partial map
+    // epilogue: remaining groups -> registers -> shared memory (fold the term blocks) -> this slice's partial map
     const int npf = a.nxf * a.nyf;
     float* out = a.partial + ((size_t)b * a.S + s) * npf;
-    if (c1 > c0) {
-        mbar_wait(smem_u32(&s_bar[2]), 0);
+    if (nch > 0) {
+        mbar_wait(smem_u32(&s_bar[2]), 0);                               // all MMAs done: the stages are free
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const int q = warp & 3, half = warp >> 2;                       // lane quarter, column half
-        const int row = (a.Mpad == 64) ? (lane < 16 ? 16 * q + lane : -1) : 32 * q + lane;
-        for (int cb = half * 8; cb < a.Npad; cb += 16) {
-            uint32_t r[8];
-            const uint32_t taddr = tmem + ((uint32_t)(32 * q) << 16) + (uint32_t)cb;
-            asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                         : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-                         : "r"(taddr));
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-            if (row >= 0 && row < a.nyf) {
+        while (gf * a.FL < nch) flush(gf++);
+        float* scr = reinterpret_cast<float*>(s_ops);                    // [128][N]
+        const int row = 32 * lq + lane;
 #pragma unroll
-                for (int j = 0; j < 8; ++j)
-                    if (cb + j < a.nxf) out[row * a.nxf + cb + j] = __uint_as_float(r[j]);
-            }
+        for (int i = 0; i < NACC; ++i) {
+            const int col = half * NACC + i;
+            if (col < N) scr[row * N + col] = acc[i];
+        }
+        __syncthreads();
+        const int TR = a.multi ? 1 : NT;
+        for (int i = tid; i < npf; i += TC_THREADS) {
+            const int iy = i / a.nxf, ix = i - iy * a.nxf;
+            float v = 0.f;
+            for (int tr = 0; tr < TR; ++tr)
+                for (int tc = 0; tc < NT; ++tc) v += scr[(tr * ny8 + iy) * N + tc * nxp + ix];
+            out[i] = v;
         }
     } else {
         for (int i = tid; i < npf; i += TC_THREADS) out[i] = 0.f;
@@ -245,35 +325,76 @@ __global__ void __launch_bounds__(TC_THREADS) jam_quad_tc_kernel(JTArgs a) {
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(a.tmem_cols) : "memory");
 }
 
-bool jam_quad_tc_supported(const glad_ctx* c) { return c->nyf <= 128 && c->nxf <= 256; }
+// bf16 terms per operand: 2 by default (16 mantissa bits, per-term error <= 2^-16), 3 with GLAD_JAM_TERMS=3
+static int tc_terms() {
+    const char* e = getenv("GLAD_JAM_TERMS");
+    return (e && atoi(e) == 3) ? 3 : 2;
+}
 
-cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S) {
-    JTArgs a;
-    a.tab = c->d_jam_tab; a.tabsz = jam_table_floats(nl, nmx); a.nl = nl; a.nmx = nmx;
-    a.un = c->d_un; a.uw = c->d_uw; a.nu = c->nu;
-    a.xf2 = c->d_xf2; a.yf2 = c->d_yf2; a.nxf = c->nxf; a.nyf = c->nyf;
-    a.Mpad = c->nyf <= 64 ? 64 : 128;
-    int nalign = a.Mpad == 64 ? 8 : 16;
-    a.Npad = ((c->nxf + nalign - 1) / nalign) * nalign;
-    a.GX = (c->nxf + 3) / 4; a.GY = (c->nyf + 3) / 4;
-    a.tmem_cols = 32;
-    while (a.tmem_cols < a.Npad) a.tmem_cols <<= 1;
-    a.S = S; a.partial = c->d_partial;
-    size_t fixed = (size_t)a.tabsz + 2 * (size_t)((c->nu + 1) & ~1) + (size_t)(a.GX + a.GY) * 4;
-    size_t smem = 0;
-    for (a.MC = 64, a.lgMC = 6; a.MC >= 32; a.MC >>= 1, --a.lgMC) {
-        size_t stage = (size_t)2 * a.MC * a.GY * 4 + (size_t)2 * a.MC * (a.Npad >> 2) * 4;
-        smem = sizeof(float) * (fixed + 2 * (size_t)a.MC * 4 + 2 * stage + 1024) + 256;
-        if (smem <= 100 * 1024 || a.MC == 32) break;
-    }
-    if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
+static bool tc_geometry(const glad_ctx* c, JTArgs* a, int* nacc) {
+    const int NT = tc_terms();
+    a->ny8 = (c->nyf + 7) & ~7;
+    if (a->ny8 > 128) return false;
+    a->multi = NT * a->ny8 > 128 ? 1 : 0;
+    a->nxp = (NT == 3 || a->multi) ? ((c->nxf + 15) & ~15) : ((c->nxf + 7) & ~7);
+    a->N = NT * a->nxp;
+    if (a->N > 256) return false;
+    *nacc = a->N / 2 <= 40 ? 40 : (a->N / 2 <= 64 ? 64 : 128);
+    a->tmem_cols = *nacc == 128 ? 512 : 256;
+    return true;
+}
+
+bool jam_quad_tc_supported(const glad_ctx* c) { JTArgs a; int nacc; return tc_geometry(c, &a, &nacc); }
+
+template <int NT, int NACC>
+static cudaError_t tc_launch(const JTArgs& a, int grid, size_t smem, cudaStream_t st) {
     static size_t configured = 0;
     if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(jam_quad_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(jam_quad_tc_kernel<NT, NACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    ProfScope ps(c, GK_JAM_QUAD);
-    jam_quad_tc_kernel<<<B * S, TC_THREADS, smem, c->stream>>>(a);
+    jam_quad_tc_kernel<NT, NACC><<<grid, TC_THREADS, smem, st>>>(a);
     return cudaGetLastError();
+}
+
+cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S) {
+    JTArgs a;
+    int nacc;
+    if (!tc_geometry(c, &a, &nacc)) return cudaErrorInvalidConfiguration;
+    const int NT = tc_terms();
+    a.tab = c->d_jam_tab; a.tabsz = jam_table_floats(nl, nmx); a.nl = nl; a.nmx = nmx;
+    a.un = c->d_un; a.uw = c->d_uw; a.nu = c->nu;
+    a.xf2 = c->d_xf2; a.yf2 = c->d_yf2; a.nxf = c->nxf; a.nyf = c->nyf;
+    a.S = S; a.partial = c->d_partial;
+    const int nblk = (a.ny8 + a.nxp) >> 3;
+    a.npair = (nblk + 1) / 2;
+    const size_t fixed = (((size_t)a.tabsz + 2 * (size_t)((c->nu + 1) & ~1) + (size_t)(a.ny8 + a.nxp) + 31) & ~(size_t)31) * 4 +
+                         2 * TC_COEF_ROWS * 16;
+    const size_t budget = nacc <= 40 ? 112 * 1024 : 220 * 1024;          // two CTAs per SM when the map is small
+    size_t smem = 0;
+    for (a.MC = 128, a.lgMC = 7; a.MC >= 64; a.MC >>= 1, --a.lgMC) {
+        size_t ops = 2 * (size_t)a.MC * NT * (a.ny8 + a.nxp) * 2 + 2048;  // two stages + the M = 128 over-read
+        const size_t scr = (size_t)128 * a.N * 4;                        // epilogue scratch reuses the stages
+        if (ops < scr) ops = scr;
+        smem = fixed + ops;
+        if (smem <= budget || a.MC == 64) break;
+    }
+    if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
+    a.FL = 512 / a.MC;
+    if (const char* e = getenv("GLAD_JAM_FLUSH")) { int v = atoi(e); if (v >= 1) a.FL = v; }
+    // exact division by npair over the item range, as a multiply-shift
+    a.magic = 65536 / a.npair + 1;
+    for (int it = 0; it < (a.MC >> 3) * a.npair; ++it)
+        if (((it * a.magic) >> 16) != it / a.npair) return cudaErrorInvalidConfiguration;
+    ProfScope ps(c, GK_JAM_QUAD);
+    const int grid = B * S;
+    if (NT == 2) {
+        if (nacc == 40) return tc_launch<2, 40>(a, grid, smem, c->stream);
+        if (nacc == 64) return tc_launch<2, 64>(a, grid, smem, c->stream);
+        return tc_launch<2, 128>(a, grid, smem, c->stream);
+    }
+    if (nacc == 40) return tc_launch<3, 40>(a, grid, smem, c->stream);
+    if (nacc == 64) return tc_launch<3, 64>(a, grid, smem, c->stream);
+    return tc_launch<3, 128>(a, grid, smem, c->stream);
 }
