@@ -22,17 +22,20 @@
 // contraction rows, an "oct"), 128 contiguous bytes; SBO = 128 B between 8-pixel groups, LBO between the two
 // octs of one K = 16 step.  A quarter-warp writes one core matrix with one conflict-free 16-byte store per lane.
 //
-// CTA = (parameter vector, K-slice), 256 threads, all of them operand producers:
-//   chunk c (MC contraction rows):  wait until the MMAs that read stage c%2 have completed (mbarrier armed by
-//   tcgen05.commit) -> add finished accumulator groups into registers -> coefficients of the next 256 rows ->
-//   operands of chunk c into stage c%2 -> fence.proxy.async -> __syncthreads -> one thread issues the MMAs of
-//   the chunk and commits.  The tensor core works on chunk c while the CUDA cores produce chunk c+1.
+// CTA = (parameter vector, K-slice), 8 producer warps + 1 MMA warp, no CTA-wide barrier in the main loop:
+//   producer warp, chunk c (MC contraction rows):  wait until the MMAs that read stage c%2 have completed
+//   (mbarrier armed by tcgen05.commit) -> add finished accumulator groups into registers -> its share of the
+//   coefficients of the next 256 rows -> its items (oct, 8-pixel block) of chunk c into stage c%2 ->
+//   fence.proxy.async -> bar.arrive on the stage's "full" named barrier (does not block).
+//   MMA warp, chunk c:  bar.sync on "full" -> one lane issues the MMAs of the chunk and commits to "empty".
+//   The tensor core works on chunk c while the CUDA cores produce chunk c+1.
 #include <stdlib.h>
 
 #include "glad_internal.h"
 
 #define LOG2E_F 1.4426950408889634f
-#define TC_THREADS 256
+#define TC_PRODUCERS 256
+#define TC_THREADS (TC_PRODUCERS + 32)
 #define TC_COEF_ROWS 256
 
 struct JTArgs {
@@ -43,8 +46,7 @@ struct JTArgs {
     int multi;           // 0: A = [Y1;..;Y_NT] in one M=128 tile;  1: NT MMAs per K-step
     int N;               // accumulator columns = NT * nxp
     int MC, lgMC;        // contraction rows per stage (power of two, 64..256)
-    int FL;              // chunks per accumulator group (>= 2)
-    int npair, magic;    // block pairs per oct; item -> oct: (item * magic) >> 16 == item / npair
+    int FL;              // chunks per accumulator group (>= 1)
     int tmem_cols;       // power of two >= 2 * N
     int S;
     float* partial;
@@ -105,6 +107,9 @@ __device__ __forceinline__ int div_small(int a, int d, float inv) {
     return r < 0 ? q - 1 : (r >= d ? q + 1 : q);
 }
 
+__device__ __forceinline__ void bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+__device__ __forceinline__ void bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+
 // NT = bf16 terms per operand value, NACC = accumulator registers per thread (>= N/2, multiple of 8)
 template <int NT, int NACC>
 __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_kernel(JTArgs a) {
@@ -126,8 +131,9 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
     float* s_u2 = s_tab + a.tabsz;
     float* s_wu2 = s_u2 + nup;
     float* s_c2 = s_wu2 + nup;                       // ny8 + nxp squared coordinates, y first
-    float4* s_coef = reinterpret_cast<float4*>(sm + ((a.tabsz + 2 * nup + ny8 + nxp + 31) & ~31));   // 2 x 256 rows
-    uint4* s_ops = reinterpret_cast<uint4*>(s_coef + 2 * TC_COEF_ROWS);   // 2 stages + tail pad, 128-byte aligned
+    // coefficient ring: 3 blocks of 256 rows, per block [-Q log2e | -P log2e | F0 | F1] x 256 floats
+    float* s_coef = sm + ((a.tabsz + 2 * nup + ny8 + nxp + 31) & ~31);
+    uint4* s_ops = reinterpret_cast<uint4*>(s_coef + 3 * 4 * TC_COEF_ROWS);   // 2 stages + tail pad, 128-byte aligned
 
     for (int i = tid; i < a.tabsz; i += TC_THREADS) s_tab[i] = Tg[i];
     for (int i = tid; i < nu; i += TC_THREADS) { float u = a.un[i]; s_u2[i] = u * u; s_wu2[i] = a.uw[i] * u * u; }
@@ -155,170 +161,200 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = s_tmem;
 
-    const float* TL = s_tab + JT_HDR;
-    const float* TM = TL + JL_COUNT * nl;
-    const float* TC = TM + JM_COUNT * nmx;
-    const float* TD = TC + nmx * nl;
-    const float cos2i = s_tab[JH_COS2I];
     const int nm = __float_as_int(s_tab[JH_NM]);
     const int pairs = nm * nl;
-    const float inv_pairs = 1.f / (float)pairs, inv_nl = 1.f / (float)nl;
     const int M = nu * pairs;
     const int NCH = (M + MC - 1) >> a.lgMC;
     const int c0 = (int)(((long)s * NCH) / a.S), c1 = (int)(((long)(s + 1) * NCH) / a.S);
     const int nch = c1 - c0;
-
-    // per contraction row: (-P log2e, -Q log2e, F0, F1); rows past the end have F0 = F1 = 0 and contribute 0
-    auto coef_block = [&](int cbk) {
-        const int m = cbk * TC_COEF_ROWS + tid;
-        float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (m < M) {
-            const int iu = div_small(m, pairs, inv_pairs), rem = m - iu * pairs;
-            const int j = div_small(rem, nl, inv_nl), k = rem - j * nl;
-            const float u2 = s_u2[iu];
-            const float omq2 = TM[JM_OMQ2 * nmx + j];
-            const float auj = u2 * TM[JM_INVS2 * nmx + j];
-            const float gg = 1.f - omq2 * u2;
-            const float bb = __fdividef(omq2 * u2 * auj, gg);
-            const float A = 0.5f * (auj + TL[JL_INVS2 * nl + k]);
-            const float Bc = 0.5f * (TL[JL_BKQ * nl + k] + bb);
-            const float E = fmaf(Bc, cos2i, A);
-            const float D = fmaf(-TD[j * nl + k], u2, TL[JL_D0 * nl + k]);
-            const float inv = __fdividef(rsqrtf(E * gg), 1.f - TC[j * nl + k] * u2);
-            const float pref = s_wu2[iu] * TM[JM_MJ * nmx + j] * inv;
-            o.x = -A * LOG2E_F;
-            o.y = -__fdividef(A * (A + Bc), E) * LOG2E_F;
-            o.z = pref * TL[JL_S0 * nl + k];
-            o.w = pref * TL[JL_NKS * nl + k] * D;
-        }
-        s_coef[(cbk & 1) * TC_COEF_ROWS + tid] = o;
-    };
-    // item = (oct o, block pair p) per quarter-warp; lane l8 = pixel; the pair shares the 8 coefficient rows of o
-    const int qw = tid >> 3, l8 = tid & 7;
-    const int items = (MC >> 3) * a.npair;
-    auto produce = [&](int c, int buf) {
-        const float4* cf = s_coef + (((c * MC) >> 8) & 1) * TC_COEF_ROWS + ((c * MC) & (TC_COEF_ROWS - 1));
-        uint4* stA = s_ops + buf * stage16;
-        uint4* stB = stA + a16;
-        for (int it = qw; it < items; it += TC_THREADS / 8) {
-            const int o = (it * a.magic) >> 16, p = it - o * a.npair;
-            float4 k[8];
-#pragma unroll
-            for (int r = 0; r < 8; ++r) k[r] = cf[8 * o + r];
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int blk = p + h * a.npair;
-                if (blk >= nblk) break;
-                float v[8];
-                if (blk < nyb) {
-                    const float q = s_c2[blk * 8 + l8];
-#pragma unroll
-                    for (int r = 0; r < 8; ++r) v[r] = ex2_tc(k[r].y * q);
-                    split_store<NT>(v, stA + (o * GA + blk) * 8 + l8, nyb * 8);
-                } else {
-                    const int bx = blk - nyb;
-                    const float q = s_c2[ny8 + bx * 8 + l8];
-#pragma unroll
-                    for (int r = 0; r < 8; ++r) v[r] = fmaf(k[r].w, q, k[r].z) * ex2_tc(k[r].x * q);
-                    split_store<NT>(v, stB + (o * GB + bx) * 8 + l8, nxb * 8);
-                }
-            }
-        }
-    };
-
-    // running map in registers: thread (lane quarter q, column half) holds D[32q + lane][half * NACC + i]
-    float acc[NACC];
-#pragma unroll
-    for (int i = 0; i < NACC; ++i) acc[i] = 0.f;
-    const int lq = warp & 3, half = warp >> 2;
     const uint32_t dstride = (uint32_t)a.tmem_cols >> 1;                // columns between the two accumulator buffers
-    auto flush = [&](int g) {
-        const uint32_t taddr = tmem + ((uint32_t)(32 * lq) << 16) + (uint32_t)(g & 1) * dstride + (uint32_t)(half * NACC);
-#pragma unroll
-        for (int i = 0; i < NACC; i += 8) {
-            uint32_t r[8];
-            asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                         : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-                         : "r"(taddr + (uint32_t)i));
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-            for (int j = 0; j < 8; ++j) acc[i + j] += __uint_as_float(r[j]);
-        }
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    };
 
-    // instruction descriptor: D fp32, A/B bf16, both K-major, M = 128, N>>3 filled per MMA
-    const uint32_t idesc_base = (1u << 4) | (1u << 7) | (1u << 10) | (8u << 24);
-    const uint32_t ops_addr = smem_u32(s_ops);
-    const uint32_t a_lbo = GA * 128, b_lbo = GB * 128;                  // bytes between the two octs of a K-step
-
-    int gf = 0;                                                         // next accumulator group to add into acc
-    if (nch > 0) {
-        coef_block((c0 * MC) >> 8);
-        __syncthreads();
-    }
-    for (int it = 0; it < nch; ++it) {
-        const int c = c0 + it, buf = it & 1;
-        if (it >= 2) {
-            mbar_wait(smem_u32(&s_bar[buf]), ((it >> 1) - 1) & 1);      // MMAs up to chunk it-2 are complete
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            while ((gf + 1) * a.FL - 1 <= it - 2) flush(gf++);
-        }
-        if (it == 0 || ((c * MC) & (TC_COEF_ROWS - 1)) == 0) coef_block(((c * MC) >> 8) + 1);
-        produce(c, buf);
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        __syncthreads();
-        if (tid == 0) {
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const int g = it / a.FL;
-            const uint32_t d = tmem + (uint32_t)(g & 1) * dstride;
-            const uint32_t sa = ops_addr + (uint32_t)buf * stage16 * 16, sb = sa + a16 * 16;
-            uint32_t accum = (it - g * a.FL) ? 1u : 0u;
-            for (int ks = 0; ks < (MC >> 4); ++ks) {
-                const uint64_t bd = umma_desc(sb + ks * 2 * b_lbo, b_lbo);
-                if (!a.multi) {
-                    umma_bf16(d, umma_desc(sa + ks * 2 * a_lbo, a_lbo), bd, idesc_base | ((uint32_t)(N >> 3) << 17), accum);
-                } else {
+    if (warp == TC_PRODUCERS / 32) {
+        // ------------------------------------------------------------------ MMA warp
+        // instruction descriptor: D fp32, A/B bf16, both K-major, M = 128, N>>3 filled per MMA
+        const uint32_t idesc_base = (1u << 4) | (1u << 7) | (1u << 10) | (8u << 24);
+        const uint32_t ops_addr = smem_u32(s_ops);
+        const uint32_t a_lbo = GA * 128, b_lbo = GB * 128;              // bytes between the two octs of a K-step
+        for (int it = 0; it < nch; ++it) {
+            const int buf = it & 1;
+            bar_sync(1 + buf, TC_THREADS);                              // every producer has written its share of chunk it
+            if (lane == 0) {
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const int g = it / a.FL;
+                const uint32_t d = tmem + (uint32_t)(g & 1) * dstride;
+                const uint32_t sa = ops_addr + (uint32_t)buf * stage16 * 16, sb = sa + a16 * 16;
+                uint32_t accum = (it - g * a.FL) ? 1u : 0u;
+                for (int ks = 0; ks < (MC >> 4); ++ks) {
+                    const uint64_t bd = umma_desc(sb + ks * 2 * b_lbo, b_lbo);
+                    if (!a.multi) {
+                        umma_bf16(d, umma_desc(sa + ks * 2 * a_lbo, a_lbo), bd, idesc_base | ((uint32_t)(N >> 3) << 17), accum);
+                    } else {
 #pragma unroll
-                    for (int t = 0; t < NT; ++t) {
-                        umma_bf16(d, umma_desc(sa + ks * 2 * a_lbo + t * nyb * 128, a_lbo), bd,
-                                  idesc_base | ((uint32_t)(((NT - t) * nxp) >> 3) << 17), accum);
-                        accum = 1u;
+                        for (int t = 0; t < NT; ++t) {
+                            umma_bf16(d, umma_desc(sa + ks * 2 * a_lbo + t * nyb * 128, a_lbo), bd,
+                                      idesc_base | ((uint32_t)(((NT - t) * nxp) >> 3) << 17), accum);
+                            accum = 1u;
+                        }
                     }
+                    accum = 1u;
                 }
-                accum = 1u;
+                umma_commit(smem_u32(&s_bar[buf]));
+                if (it == nch - 1) umma_commit(smem_u32(&s_bar[2]));
             }
-            umma_commit(smem_u32(&s_bar[buf]));
-            if (it == nch - 1) umma_commit(smem_u32(&s_bar[2]));
-        }
-        __syncwarp();
-    }
-
-    // epilogue: remaining groups -> registers -> shared memory (fold the term blocks) -> this slice's partial map
-    const int npf = a.nxf * a.nyf;
-    float* out = a.partial + ((size_t)b * a.S + s) * npf;
-    if (nch > 0) {
-        mbar_wait(smem_u32(&s_bar[2]), 0);                               // all MMAs done: the stages are free
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        while (gf * a.FL < nch) flush(gf++);
-        float* scr = reinterpret_cast<float*>(s_ops);                    // [128][N]
-        const int row = 32 * lq + lane;
-#pragma unroll
-        for (int i = 0; i < NACC; ++i) {
-            const int col = half * NACC + i;
-            if (col < N) scr[row * N + col] = acc[i];
-        }
-        __syncthreads();
-        const int TR = a.multi ? 1 : NT;
-        for (int i = tid; i < npf; i += TC_THREADS) {
-            const int iy = i / a.nxf, ix = i - iy * a.nxf;
-            float v = 0.f;
-            for (int tr = 0; tr < TR; ++tr)
-                for (int tc = 0; tc < NT; ++tc) v += scr[(tr * ny8 + iy) * N + tc * nxp + ix];
-            out[i] = v;
+            __syncwarp();
         }
     } else {
-        for (int i = tid; i < npf; i += TC_THREADS) out[i] = 0.f;
+        // ------------------------------------------------------------------ producer warps
+        const float* TL = s_tab + JT_HDR;
+        const float* TM = TL + JL_COUNT * nl;
+        const float* TC = TM + JM_COUNT * nmx;
+        const float* TD = TC + nmx * nl;
+        const float cos2i = s_tab[JH_COS2I];
+        const float inv_pairs = 1.f / (float)pairs, inv_nl = 1.f / (float)nl;
+
+        // row m = cbk*256 + tid of the contraction: (-Q log2e, -P log2e, F0, F1); rows past the end have F0 = F1 = 0
+        // and contribute 0.  Ring slot cbk % 3: a block is written while the previous one is read and the one
+        // before that may still be read by a warp that lags one chunk behind (needs MC <= 128).
+        auto coef_block = [&](int cbk) {
+            const int m = cbk * TC_COEF_ROWS + tid;
+            float cq = 0.f, cp = 0.f, f0 = 0.f, f1 = 0.f;
+            if (m < M) {
+                const int iu = div_small(m, pairs, inv_pairs), rem = m - iu * pairs;
+                const int j = div_small(rem, nl, inv_nl), k = rem - j * nl;
+                const float u2 = s_u2[iu];
+                const float omq2 = TM[JM_OMQ2 * nmx + j];
+                const float auj = u2 * TM[JM_INVS2 * nmx + j];
+                const float gg = 1.f - omq2 * u2;
+                const float bb = __fdividef(omq2 * u2 * auj, gg);
+                const float A = 0.5f * (auj + TL[JL_INVS2 * nl + k]);
+                const float Bc = 0.5f * (TL[JL_BKQ * nl + k] + bb);
+                const float E = fmaf(Bc, cos2i, A);
+                const float D = fmaf(-TD[j * nl + k], u2, TL[JL_D0 * nl + k]);
+                const float inv = __fdividef(rsqrtf(E * gg), 1.f - TC[j * nl + k] * u2);
+                const float pref = s_wu2[iu] * TM[JM_MJ * nmx + j] * inv;
+                cp = -A * LOG2E_F;
+                cq = -__fdividef(A * (A + Bc), E) * LOG2E_F;
+                f0 = pref * TL[JL_S0 * nl + k];
+                f1 = pref * TL[JL_NKS * nl + k] * D;
+            }
+            float* dst = s_coef + (cbk % 3) * (4 * TC_COEF_ROWS) + tid;
+            dst[0] = cq; dst[TC_COEF_ROWS] = cp; dst[2 * TC_COEF_ROWS] = f0; dst[3 * TC_COEF_ROWS] = f1;
+        };
+
+        // item = (oct o, 8-pixel block) per quarter-warp; lane l8 = pixel; 8 values = the 8 rows of o.  Y items and
+        // X items run in separate loops so that a warp never diverges between the two formulas; the quarter-warp ->
+        // item map of the X loop is shifted by half the CTA so that ragged item counts even out.
+        const int qw = tid >> 3, l8 = tid & 7;
+        const float inv_nyb = 1.f / (float)nyb, inv_nxb = 1.f / (float)nxb;
+        const int nyi = (MC >> 3) * nyb, nxi = (MC >> 3) * nxb;
+        const int dyo = 32 / nyb, dyb = 32 - dyo * nyb, dxo = 32 / nxb, dxb = 32 - dxo * nxb;
+        const int qy = qw, qx = (qw + 16) & 31;
+        const int oy0 = div_small(qy, nyb, inv_nyb), by0 = qy - oy0 * nyb;
+        const int ox0 = div_small(qx, nxb, inv_nxb), bx0 = qx - ox0 * nxb;
+        auto produce = [&](int c, int buf) {
+            const int row0 = c * MC;
+            const float* cb = s_coef + ((row0 >> 8) % 3) * (4 * TC_COEF_ROWS) + (row0 & (TC_COEF_ROWS - 1));
+            uint4* stA = s_ops + buf * stage16;
+            uint4* stB = stA + a16;
+            {
+                int o = oy0, blk = by0;
+                for (int i = qy; i < nyi; i += 32) {
+                    const float q = s_c2[blk * 8 + l8];
+                    const float4 e0 = *reinterpret_cast<const float4*>(cb + 8 * o);
+                    const float4 e1 = *reinterpret_cast<const float4*>(cb + 8 * o + 4);
+                    float v[8];
+                    v[0] = ex2_tc(e0.x * q); v[1] = ex2_tc(e0.y * q); v[2] = ex2_tc(e0.z * q); v[3] = ex2_tc(e0.w * q);
+                    v[4] = ex2_tc(e1.x * q); v[5] = ex2_tc(e1.y * q); v[6] = ex2_tc(e1.z * q); v[7] = ex2_tc(e1.w * q);
+                    split_store<NT>(v, stA + (o * GA + blk) * 8 + l8, nyb * 8);
+                    blk += dyb; o += dyo;
+                    if (blk >= nyb) { blk -= nyb; ++o; }
+                }
+            }
+            {
+                int o = ox0, blk = bx0;
+                for (int i = qx; i < nxi; i += 32) {
+                    const float q = s_c2[ny8 + blk * 8 + l8];
+                    const float* cx = cb + TC_COEF_ROWS + 8 * o;
+                    const float4 p0 = *reinterpret_cast<const float4*>(cx), p1 = *reinterpret_cast<const float4*>(cx + 4);
+                    const float4 g0 = *reinterpret_cast<const float4*>(cx + TC_COEF_ROWS), g1 = *reinterpret_cast<const float4*>(cx + TC_COEF_ROWS + 4);
+                    const float4 h0 = *reinterpret_cast<const float4*>(cx + 2 * TC_COEF_ROWS), h1 = *reinterpret_cast<const float4*>(cx + 2 * TC_COEF_ROWS + 4);
+                    float v[8];
+                    v[0] = fmaf(h0.x, q, g0.x) * ex2_tc(p0.x * q); v[1] = fmaf(h0.y, q, g0.y) * ex2_tc(p0.y * q);
+                    v[2] = fmaf(h0.z, q, g0.z) * ex2_tc(p0.z * q); v[3] = fmaf(h0.w, q, g0.w) * ex2_tc(p0.w * q);
+                    v[4] = fmaf(h1.x, q, g1.x) * ex2_tc(p1.x * q); v[5] = fmaf(h1.y, q, g1.y) * ex2_tc(p1.y * q);
+                    v[6] = fmaf(h1.z, q, g1.z) * ex2_tc(p1.z * q); v[7] = fmaf(h1.w, q, g1.w) * ex2_tc(p1.w * q);
+                    split_store<NT>(v, stB + (o * GB + blk) * 8 + l8, nxb * 8);
+                    blk += dxb; o += dxo;
+                    if (blk >= nxb) { blk -= nxb; ++o; }
+                }
+            }
+        };
+
+        // running map in registers: thread (lane quarter lq, column half) holds D[32 lq + lane][half * NACC + i]
+        float acc[NACC];
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) acc[i] = 0.f;
+        const int lq = warp & 3, half = warp >> 2;
+        auto flush = [&](int g) {
+            const uint32_t taddr = tmem + ((uint32_t)(32 * lq) << 16) + (uint32_t)(g & 1) * dstride + (uint32_t)(half * NACC);
+#pragma unroll
+            for (int i = 0; i < NACC; i += 8) {
+                uint32_t r[8];
+                asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                             : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                             : "r"(taddr + (uint32_t)i));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int j = 0; j < 8; ++j) acc[i + j] += __uint_as_float(r[j]);
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        };
+
+        int gf = 0;                                                     // next accumulator group to add into acc
+        if (nch > 0) {
+            coef_block((c0 * MC) >> 8);
+            coef_block(((c0 * MC) >> 8) + 1);
+            bar_sync(3, TC_PRODUCERS);
+        }
+        for (int it = 0; it < nch; ++it) {
+            const int c = c0 + it, buf = it & 1;
+            if (it >= 2) {
+                mbar_wait(smem_u32(&s_bar[buf]), ((it >> 1) - 1) & 1);  // MMAs up to chunk it-2 are complete
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                while ((gf + 1) * a.FL - 1 <= it - 2) flush(gf++);
+            }
+            if (it > 0 && ((c * MC) & (TC_COEF_ROWS - 1)) == 0) coef_block(((c * MC) >> 8) + 1);
+            produce(c, buf);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            bar_arrive(1 + buf, TC_THREADS);
+        }
+
+        // epilogue: remaining groups -> registers -> shared memory (fold the term blocks) -> this slice's partial map
+        const int npf = a.nxf * a.nyf;
+        float* out = a.partial + ((size_t)b * a.S + s) * npf;
+        if (nch > 0) {
+            mbar_wait(smem_u32(&s_bar[2]), 0);                           // all MMAs done: the stages are free
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            while (gf * a.FL < nch) flush(gf++);
+            float* scr = reinterpret_cast<float*>(s_ops);                // [128][N]
+            const int row = 32 * lq + lane;
+#pragma unroll
+            for (int i = 0; i < NACC; ++i) {
+                const int col = half * NACC + i;
+                if (col < N) scr[row * N + col] = acc[i];
+            }
+            bar_sync(3, TC_PRODUCERS);
+            const int TR = a.multi ? 1 : NT;
+            for (int i = tid; i < npf; i += TC_PRODUCERS) {
+                const int iy = i / a.nxf, ix = i - iy * a.nxf;
+                float v = 0.f;
+                for (int tr = TR - 1; tr >= 0; --tr)                      // small cross terms first
+                    for (int tc = NT - 1; tc >= 0; --tc) v += scr[(tr * ny8 + iy) * N + tc * nxp + ix];
+                out[i] = v;
+            }
+        } else {
+            for (int i = tid; i < npf; i += TC_PRODUCERS) out[i] = 0.f;
+        }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
@@ -367,10 +403,8 @@ cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S) {
     a.un = c->d_un; a.uw = c->d_uw; a.nu = c->nu;
     a.xf2 = c->d_xf2; a.yf2 = c->d_yf2; a.nxf = c->nxf; a.nyf = c->nyf;
     a.S = S; a.partial = c->d_partial;
-    const int nblk = (a.ny8 + a.nxp) >> 3;
-    a.npair = (nblk + 1) / 2;
     const size_t fixed = (((size_t)a.tabsz + 2 * (size_t)((c->nu + 1) & ~1) + (size_t)(a.ny8 + a.nxp) + 31) & ~(size_t)31) * 4 +
-                         2 * TC_COEF_ROWS * 16;
+                         3 * TC_COEF_ROWS * 16;
     const size_t budget = nacc <= 40 ? 112 * 1024 : 220 * 1024;          // two CTAs per SM when the map is small
     size_t smem = 0;
     for (a.MC = 128, a.lgMC = 7; a.MC >= 64; a.MC >>= 1, --a.lgMC) {
@@ -383,10 +417,6 @@ cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S) {
     if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
     a.FL = 512 / a.MC;
     if (const char* e = getenv("GLAD_JAM_FLUSH")) { int v = atoi(e); if (v >= 1) a.FL = v; }
-    // exact division by npair over the item range, as a multiply-shift
-    a.magic = 65536 / a.npair + 1;
-    for (int it = 0; it < (a.MC >> 3) * a.npair; ++it)
-        if (((it * a.magic) >> 16) != it / a.npair) return cudaErrorInvalidConfiguration;
     ProfScope ps(c, GK_JAM_QUAD);
     const int grid = B * S;
     if (NT == 2) {
