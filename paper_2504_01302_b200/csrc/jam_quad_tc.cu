@@ -63,6 +63,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     do {
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (!ok) __nanosleep(32);
     } while (!ok);
 }
 // UMMA shared-memory descriptor: K-major, no swizzle, version 1 (sm_100).  SBO = 128 B between 8-row groups
@@ -83,19 +84,26 @@ __device__ __forceinline__ void umma_commit(uint32_t bar) {
 __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
     uint32_t d; asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(b), "f"(a)); return d;
 }
-// split 8 values (one oct of one pixel) into NT bf16 terms and store one 16-byte core-matrix row per term
+// packed fp32x2 arithmetic (FMUL2 / FFMA2 / FADD2): one issue slot for two lanes-worth of fp32 work
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void unpk2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 ex2_2(f32x2 x) { float a, b; unpk2(x, a, b); return pk2(ex2_tc(a), ex2_tc(b)); }
+// split 4 pairs (the 8 rows of one oct, one pixel) into NT bf16 terms and store one 16-byte core-matrix row per term
 template <int NT>
-__device__ __forceinline__ void split_store(float (&v)[8], uint4* dst, int term_stride16) {
+__device__ __forceinline__ void split_store(f32x2 (&v)[4], uint4* dst, int term_stride16) {
 #pragma unroll
     for (int t = 0; t < NT; ++t) {
         uint32_t w[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            w[j] = pack_bf16(v[2 * j], v[2 * j + 1]);
-            if (t + 1 < NT) {
-                v[2 * j] -= __uint_as_float(w[j] << 16);
-                v[2 * j + 1] -= __uint_as_float(w[j] & 0xFFFF0000u);
-            }
+            float lo, hi;
+            unpk2(v[j], lo, hi);
+            w[j] = pack_bf16(lo, hi);
+            if (t + 1 < NT) v[j] = sub2(v[j], pk2(__uint_as_float(w[j] << 16), __uint_as_float(w[j] & 0xFFFF0000u)));
         }
         dst[t * term_stride16] = make_uint4(w[0], w[1], w[2], w[3]);
     }
@@ -122,7 +130,7 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
     if (__float_as_int(Tg[JH_VALID]) == 0) return;      // post kernel never reads this vector's partials
 
     const int nl = a.nl, nmx = a.nmx, nu = a.nu, MC = a.MC, ny8 = a.ny8, nxp = a.nxp, N = a.N;
-    const int nyb = ny8 >> 3, nxb = nxp >> 3, nblk = nyb + nxb;      // 8-pixel blocks per oct: Y blocks, then X blocks
+    const int nyb = ny8 >> 3, nxb = nxp >> 3;                        // 8-pixel blocks per oct: Y blocks, X blocks
     const int GA = NT * nyb, GB = NT * nxb;                          // core matrices per oct: the NT terms stacked
     const int nup = (nu + 1) & ~1;
     const int a16 = (MC >> 3) * GA * 8, b16 = (MC >> 3) * GB * 8;    // 16-byte units per stage
@@ -241,51 +249,46 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
             dst[0] = cq; dst[TC_COEF_ROWS] = cp; dst[2 * TC_COEF_ROWS] = f0; dst[3 * TC_COEF_ROWS] = f1;
         };
 
-        // item = (oct o, 8-pixel block) per quarter-warp; lane l8 = pixel; 8 values = the 8 rows of o.  Y items and
-        // X items run in separate loops so that a warp never diverges between the two formulas; the quarter-warp ->
-        // item map of the X loop is shifted by half the CTA so that ragged item counts even out.
+        // Quarter-warp = one oct o of the chunk (8 contraction rows), lane l8 = pixel within an 8-pixel block.  The
+        // thread loads the 8 rows' coefficients once (LDS.128 delivers 512 B per warp whatever the broadcast, so
+        // coefficient loads are paid per thread, not per address) and reuses them over its share of the Y blocks,
+        // then of the X blocks.  The blocks of an oct are cut into NG = 32/(MC/8) contiguous groups; a warp holds
+        // one group index (no divergence) and four octs; the X group is mirrored so that ragged splits even out.
         const int qw = tid >> 3, l8 = tid & 7;
-        const float inv_nyb = 1.f / (float)nyb, inv_nxb = 1.f / (float)nxb;
-        const int nyi = (MC >> 3) * nyb, nxi = (MC >> 3) * nxb;
-        const int dyo = 32 / nyb, dyb = 32 - dyo * nyb, dxo = 32 / nxb, dxb = 32 - dxo * nxb;
-        const int qy = qw, qx = (qw + 16) & 31;
-        const int oy0 = div_small(qy, nyb, inv_nyb), by0 = qy - oy0 * nyb;
-        const int ox0 = div_small(qx, nxb, inv_nxb), bx0 = qx - ox0 * nxb;
+        const int NG = 256 / MC;                                        // 2 (MC = 128) or 4 (MC = 64)
+        const int g = warp & (NG - 1), oct = (qw & 3) + 4 * (warp / NG);
+        const int yb0 = (g * nyb) / NG, yb1 = ((g + 1) * nyb) / NG;
+        const int xb0 = ((NG - 1 - g) * nxb) / NG, xb1 = ((NG - g) * nxb) / NG;
         auto produce = [&](int c, int buf) {
             const int row0 = c * MC;
-            const float* cb = s_coef + ((row0 >> 8) % 3) * (4 * TC_COEF_ROWS) + (row0 & (TC_COEF_ROWS - 1));
-            uint4* stA = s_ops + buf * stage16;
-            uint4* stB = stA + a16;
+            const float* cb = s_coef + ((row0 >> 8) % 3) * (4 * TC_COEF_ROWS) + (row0 & (TC_COEF_ROWS - 1)) + 8 * oct;
+            uint4* stA = s_ops + buf * stage16 + oct * GA * 8 + l8;
+            uint4* stB = s_ops + buf * stage16 + a16 + oct * GB * 8 + l8;
             {
-                int o = oy0, blk = by0;
-                for (int i = qy; i < nyi; i += 32) {
+                const float4 e0 = *reinterpret_cast<const float4*>(cb), e1 = *reinterpret_cast<const float4*>(cb + 4);
+                for (int blk = yb0; blk < yb1; ++blk) {
                     const float q = s_c2[blk * 8 + l8];
-                    const float4 e0 = *reinterpret_cast<const float4*>(cb + 8 * o);
-                    const float4 e1 = *reinterpret_cast<const float4*>(cb + 8 * o + 4);
-                    float v[8];
-                    v[0] = ex2_tc(e0.x * q); v[1] = ex2_tc(e0.y * q); v[2] = ex2_tc(e0.z * q); v[3] = ex2_tc(e0.w * q);
-                    v[4] = ex2_tc(e1.x * q); v[5] = ex2_tc(e1.y * q); v[6] = ex2_tc(e1.z * q); v[7] = ex2_tc(e1.w * q);
-                    split_store<NT>(v, stA + (o * GA + blk) * 8 + l8, nyb * 8);
-                    blk += dyb; o += dyo;
-                    if (blk >= nyb) { blk -= nyb; ++o; }
+                    const f32x2 qq = pk2(q, q);
+                    f32x2 v[4];
+                    v[0] = ex2_2(mul2(pk2(e0.x, e0.y), qq)); v[1] = ex2_2(mul2(pk2(e0.z, e0.w), qq));
+                    v[2] = ex2_2(mul2(pk2(e1.x, e1.y), qq)); v[3] = ex2_2(mul2(pk2(e1.z, e1.w), qq));
+                    split_store<NT>(v, stA + blk * 8, nyb * 8);
                 }
             }
             {
-                int o = ox0, blk = bx0;
-                for (int i = qx; i < nxi; i += 32) {
+                const float* cx = cb + TC_COEF_ROWS;
+                const float4 p0 = *reinterpret_cast<const float4*>(cx), p1 = *reinterpret_cast<const float4*>(cx + 4);
+                const float4 g0 = *reinterpret_cast<const float4*>(cx + TC_COEF_ROWS), g1 = *reinterpret_cast<const float4*>(cx + TC_COEF_ROWS + 4);
+                const float4 h0 = *reinterpret_cast<const float4*>(cx + 2 * TC_COEF_ROWS), h1 = *reinterpret_cast<const float4*>(cx + 2 * TC_COEF_ROWS + 4);
+                for (int blk = xb0; blk < xb1; ++blk) {
                     const float q = s_c2[ny8 + blk * 8 + l8];
-                    const float* cx = cb + TC_COEF_ROWS + 8 * o;
-                    const float4 p0 = *reinterpret_cast<const float4*>(cx), p1 = *reinterpret_cast<const float4*>(cx + 4);
-                    const float4 g0 = *reinterpret_cast<const float4*>(cx + TC_COEF_ROWS), g1 = *reinterpret_cast<const float4*>(cx + TC_COEF_ROWS + 4);
-                    const float4 h0 = *reinterpret_cast<const float4*>(cx + 2 * TC_COEF_ROWS), h1 = *reinterpret_cast<const float4*>(cx + 2 * TC_COEF_ROWS + 4);
-                    float v[8];
-                    v[0] = fmaf(h0.x, q, g0.x) * ex2_tc(p0.x * q); v[1] = fmaf(h0.y, q, g0.y) * ex2_tc(p0.y * q);
-                    v[2] = fmaf(h0.z, q, g0.z) * ex2_tc(p0.z * q); v[3] = fmaf(h0.w, q, g0.w) * ex2_tc(p0.w * q);
-                    v[4] = fmaf(h1.x, q, g1.x) * ex2_tc(p1.x * q); v[5] = fmaf(h1.y, q, g1.y) * ex2_tc(p1.y * q);
-                    v[6] = fmaf(h1.z, q, g1.z) * ex2_tc(p1.z * q); v[7] = fmaf(h1.w, q, g1.w) * ex2_tc(p1.w * q);
-                    split_store<NT>(v, stB + (o * GB + blk) * 8 + l8, nxb * 8);
-                    blk += dxb; o += dxo;
-                    if (blk >= nxb) { blk -= nxb; ++o; }
+                    const f32x2 qq = pk2(q, q);
+                    f32x2 v[4];
+                    v[0] = mul2(fma2(pk2(h0.x, h0.y), qq, pk2(g0.x, g0.y)), ex2_2(mul2(pk2(p0.x, p0.y), qq)));
+                    v[1] = mul2(fma2(pk2(h0.z, h0.w), qq, pk2(g0.z, g0.w)), ex2_2(mul2(pk2(p0.z, p0.w), qq)));
+                    v[2] = mul2(fma2(pk2(h1.x, h1.y), qq, pk2(g1.x, g1.y)), ex2_2(mul2(pk2(p1.x, p1.y), qq)));
+                    v[3] = mul2(fma2(pk2(h1.z, h1.w), qq, pk2(g1.z, g1.w)), ex2_2(mul2(pk2(p1.z, p1.w), qq)));
+                    split_store<NT>(v, stB + blk * 8, nxb * 8);
                 }
             }
         };
