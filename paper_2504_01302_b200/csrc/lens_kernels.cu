@@ -43,12 +43,15 @@ __device__ static double gamma_p(double a, double x) {
     return 1.0 - exp(-x + a * log(x) - lg) * h;
 }
 
-// Sersic b_n: root of P(2n, b) = 1/2 by safeguarded Newton (reading R-L7).
+// Sersic b_n: root of P(2n, b) = 1/2 by safeguarded Newton (reading R-L7), started from the asymptotic
+// expansion b ~ 2n - 1/3 + 4/(405 n) + 46/(25515 n^2) + 131/(1148175 n^3) - 2194697/(30690717750 n^4)
+// (Ciotti & Bertin 1999) so that two steps reach fp64 round-off.
 __device__ static double sersic_bn(double n) {
     double a = 2.0 * n;
     double lo = 0.0, hi = a + 25.0;
-    double b = a - 1.0 / 3.0;
-    if (b <= 0.0) b = 0.5 * a;
+    const double rn = 1.0 / n;
+    double b = a - 1.0 / 3.0 + rn * (4.0 / 405.0 + rn * (46.0 / 25515.0 + rn * (131.0 / 1148175.0 - rn * (2194697.0 / 30690717750.0))));
+    if (!(b > 0.0 && b < hi) || n < 0.36) b = (a > 1.0 / 3.0) ? a - 1.0 / 3.0 : 0.5 * a;
     double lg = lgamma(a);
     for (int it = 0; it < 60; ++it) {
         double f = gamma_p(a, b) - 0.5;
@@ -62,8 +65,11 @@ __device__ static double sersic_bn(double n) {
     return b;
 }
 
-__global__ void lens_prep_kernel(const float* __restrict__ params, int B, float* __restrict__ consts) {
-    int b = blockIdx.x * blockDim.x + threadIdx.x;
+// 4 warps per 32 parameter vectors (lane = vector): warp role 0 = EPL / shear / point mass / validity, roles 1..3 =
+// one Sersic component each (the b_n root is the only long serial chain of the kernel; a warp never mixes roles).
+#define LENS_PREP_ROLES 4
+__global__ void __launch_bounds__(32 * LENS_PREP_ROLES) lens_prep_kernel(const float* __restrict__ params, int B, float* __restrict__ consts) {
+    const int b = blockIdx.x * 32 + (threadIdx.x & 31), role = threadIdx.x >> 5;
     if (b >= B) return;
     const float* p = params + (size_t)b * GLAD_NLENS;
     float* c = consts + (size_t)b * LC_SIZE;
@@ -73,17 +79,36 @@ __global__ void lens_prep_kernel(const float* __restrict__ params, int B, float*
         const float* s = p + (k == 0 ? 11 : (k == 1 ? 16 : 21));
         if (s[0] != 0.f && !(s[1] > 0.f && s[2] > 0.f && s[3] > 0.f && s[3] <= 1.f)) valid = false;
     }
-    for (int i = 0; i < LC_SIZE; ++i) c[i] = 0.f;
+    if (role > 0) {
+        const int k = role - 1;
+        const float* s = p + (k == 0 ? 11 : (k == 1 ? 16 : 21));
+        float* o = c + LC_SERSIC0 + k * LC_SERSIC_STRIDE;
+        for (int i = 0; i < LC_SERSIC_STRIDE; ++i) o[i] = 0.f;
+        if (!valid) return;
+        double Ie = s[0], Re = s[1], n = s[2], qs = s[3], phi = s[4];
+        o[0] = (k == 0) ? p[9] : (float)xl;
+        o[1] = (k == 0) ? p[10] : (float)yl;
+        if (Ie == 0.0) return;
+        double bn = sersic_bn(n);
+        o[2] = (float)cos(phi); o[3] = (float)sin(phi);
+        o[4] = (float)(1.0 / (qs * qs));
+        o[5] = (float)(Ie * exp(bn));                                  // I(0)
+        o[6] = (float)(bn * 1.4426950408889634 * pow(Re, -1.0 / n));   // I = amp 2^(-k1 (R^2)^h)
+        o[7] = (float)(0.5 / n);
+        return;
+    }
+    for (int i = 0; i < LC_SERSIC0; ++i) c[i] = 0.f;
+    for (int i = LC_SERIES; i < LC_SIZE; ++i) c[i] = 0.f;
     c[LC_VALID] = valid ? 1.f : 0.f;
     if (!valid) return;
-    double t = gam - 1.0;
+    double tt = gam - 1.0;
     double f = (1.0 - q) / (1.0 + q);
-    double bTM = q * pow(2.0 / (1.0 + q), 1.0 / t) * thE;  // b_TM = q b, b from Eq. B.3
+    double bTM = q * pow(2.0 / (1.0 + q), 1.0 / tt) * thE;  // b_TM = q b, b from Eq. B.3
     c[LC_XL] = (float)xl; c[LC_YL] = (float)yl;
     c[LC_COSPA] = (float)cos(pa); c[LC_SINPA] = (float)sin(pa);
     c[LC_Q] = (float)q; c[LC_NEGF] = (float)(-f);
-    c[LC_PREF] = (thE > 0.0) ? (float)(2.0 * pow(bTM, t) / (1.0 + q)) : 0.f;
-    c[LC_HEXP] = (float)(-0.5 * (t - 1.0));
+    c[LC_PREF] = (thE > 0.0) ? (float)(2.0 * pow(bTM, tt) / (1.0 + q)) : 0.f;
+    c[LC_HEXP] = (float)(-0.5 * (tt - 1.0));
     int nt = 0;
     if (f > 1e-12) {
         nt = (int)ceil(log(2e-8) / log(f)) + 1;
@@ -92,24 +117,10 @@ __global__ void lens_prep_kernel(const float* __restrict__ params, int B, float*
     }
     c[LC_NTERMS] = (float)nt;
     for (int n = 1; n <= GLAD_EPL_MAX_TERMS; ++n)
-        c[LC_SERIES + n - 1] = (float)((2.0 * n - (2.0 - t)) / (2.0 * n + (2.0 - t)));
+        c[LC_SERIES + n - 1] = (float)((2.0 * n - (2.0 - tt)) / (2.0 * n + (2.0 - tt)));
     c[LC_SH_C] = (float)((double)p[6] * cos(2.0 * (double)p[7]));
     c[LC_SH_S] = (float)((double)p[6] * sin(2.0 * (double)p[7]));
     c[LC_BH] = p[8];
-    for (int k = 0; k < 3; ++k) {
-        const float* s = p + (k == 0 ? 11 : (k == 1 ? 16 : 21));
-        float* o = c + LC_SERSIC0 + k * LC_SERSIC_STRIDE;
-        double Ie = s[0], Re = s[1], n = s[2], qs = s[3], phi = s[4];
-        o[0] = (k == 0) ? p[9] : (float)xl;
-        o[1] = (k == 0) ? p[10] : (float)yl;
-        if (Ie == 0.0) { o[5] = 0.f; continue; }
-        double bn = sersic_bn(n);
-        o[2] = (float)cos(phi); o[3] = (float)sin(phi);
-        o[4] = (float)(1.0 / (qs * qs));
-        o[5] = (float)(Ie * exp(bn));                                  // I(0)
-        o[6] = (float)(bn * 1.4426950408889634 * pow(Re, -1.0 / n));   // I = amp 2^(-k1 (R^2)^h)
-        o[7] = (float)(0.5 / n);
-    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -163,7 +174,17 @@ __device__ __forceinline__ float shoot(const float* __restrict__ c, float thx, f
     return v;
 }
 
-#define LENS_STRIP 8
+// PSF convolution geometry: a thread owns LENS_STRIP consecutive output pixels of one row; taps are consumed
+// LENS_TAPS at a time with every register index static, so the inner block is LENS_STRIP*LENS_TAPS FFMAs on
+// LENS_STRIP+LENS_TAPS-1 source pixels and LENS_TAPS taps held in registers.  The binned image sits in shared memory
+// with a zero halo (left cc+LENS_TAPS, right cc+LENS_STRIP-1) and one zero row, so the loop has no bounds tests;
+// the row pitch is odd and consecutive lanes own consecutive rows, so source loads are bank-conflict free and
+// tap loads are broadcasts.
+#define LENS_STRIP 16
+#define LENS_TAPS 8
+static inline __host__ __device__ int lens_tap_pitch(int kpsf) { return (kpsf + LENS_TAPS - 1) & ~(LENS_TAPS - 1); }
+static inline __host__ __device__ int lens_halo_left(int kpsf) { return kpsf / 2 + LENS_TAPS; }
+static inline __host__ __device__ int lens_img_pitch(int nx, int kpsf) { return (nx + 2 * (kpsf / 2) + LENS_TAPS + LENS_STRIP - 1) | 1; }
 
 __global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict__ consts, glad_image_grid g,
                                                          const float* __restrict__ psf, int kpsf,
@@ -173,13 +194,18 @@ __global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict
     extern __shared__ __align__(16) float smem[];
     const int b = blockIdx.x, tid = threadIdx.x, nthr = blockDim.x;
     const int nx = g.nx, ny = g.ny, npx = nx * ny, ss = g.supersample;
+    const int KP = lens_tap_pitch(kpsf), HL = lens_halo_left(kpsf), pitch = lens_img_pitch(nx, kpsf);
     float* c = smem;                       // LC_SIZE
-    float* spsf = smem + LC_SIZE;          // kpsf^2 (padded to 4)
-    float* img = spsf + ((kpsf * kpsf + 3) & ~3);  // npx
+    float* spsf = smem + LC_SIZE;          // kpsf rows x KP taps, zero padded
+    float* img = spsf + kpsf * KP;         // (ny + 1) rows x pitch, zero halo, last row zero
     __shared__ float red[32];
 
     for (int i = tid; i < LC_SIZE; i += nthr) c[i] = consts[(size_t)b * LC_SIZE + i];
-    for (int i = tid; i < kpsf * kpsf; i += nthr) spsf[i] = psf[i];
+    for (int i = tid; i < kpsf * KP; i += nthr) {
+        int r = i / KP, k = i - r * KP;
+        spsf[i] = k < kpsf ? psf[r * kpsf + k] : 0.f;
+    }
+    for (int i = tid; i < (ny + 1) * pitch; i += nthr) img[i] = 0.f;
     __syncthreads();
     const bool valid = c[LC_VALID] != 0.f;
     if (!valid) {
@@ -207,39 +233,38 @@ __global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict
                 acc += shoot(c, thx, thy, nterms, has_src, has_l1, has_l2);
             }
         }
-        img[p] = acc * inv_s2;
+        img[iy * pitch + HL + ix] = acc * inv_s2;
     }
     __syncthreads();
 
-    // row a4: PSF convolution from shared memory + chi2
+    // row a4: PSF convolution from shared memory + chi2.  out[x] = sum_dy sum_dx psf[dy][dx] img[y+cc-dy][x+cc-dx]
     const int cc = kpsf / 2;
     const int nstrip_x = (nx + LENS_STRIP - 1) / LENS_STRIP;
-    const int nstrips = ny * nstrip_x;
+    const int nitems = ny * nstrip_x;
     float part = 0.f;
-    for (int st = tid; st < nstrips; st += nthr) {
-        int y = st / nstrip_x, x0 = (st - y * nstrip_x) * LENS_STRIP;
+    for (int t = tid; t < nitems; t += nthr) {
+        const int sx = t / ny, y = t - sx * ny, x0 = sx * LENS_STRIP;
         float out[LENS_STRIP];
 #pragma unroll
         for (int j = 0; j < LENS_STRIP; ++j) out[j] = 0.f;
         for (int dy = 0; dy < kpsf; ++dy) {
             int sy = y + cc - dy;
-            if (sy < 0 || sy >= ny) continue;
-            const float* row = img + sy * nx;
-            const float* prow = spsf + dy * kpsf;
-            // out[j] += psf[dy][dx] * img[sy][x0 + j + cc - dx]; walk the source column e = x0-cc .. x0+cc+STRIP-1,
-            // keeping w[j] = psf[dy][cc + j - (e - x0)] in a sliding window.
-            float w[LENS_STRIP];
+            sy = ((unsigned)sy < (unsigned)ny) ? sy : ny;                   // out of range -> the zero row
+            // source column of (output j, tap dx = c8 + d) in halo coordinates: x0 + HL + cc - c8 + (j - d)
+            const float* row = img + sy * pitch + x0 + HL + cc - (LENS_TAPS - 1);
+            const float* prow = spsf + dy * KP;
+            for (int c8 = 0; c8 < KP; c8 += LENS_TAPS) {
+                const float4 pa = *reinterpret_cast<const float4*>(prow + c8);
+                const float4 pb = *reinterpret_cast<const float4*>(prow + c8 + 4);
+                const float p[LENS_TAPS] = {pa.x, pa.y, pa.z, pa.w, pb.x, pb.y, pb.z, pb.w};
+                const float* r = row - c8;
+                float s[LENS_STRIP + LENS_TAPS - 1];
 #pragma unroll
-            for (int j = 0; j < LENS_STRIP; ++j) w[j] = 0.f;
-            for (int e = -cc; e < cc + LENS_STRIP; ++e) {
+                for (int i = 0; i < LENS_STRIP + LENS_TAPS - 1; ++i) s[i] = r[i];
 #pragma unroll
-                for (int j = LENS_STRIP - 1; j > 0; --j) w[j] = w[j - 1];   // dx(j) = cc + j - e
-                int dx0 = cc - e;
-                w[0] = (dx0 >= 0 && dx0 < kpsf) ? prow[dx0] : 0.f;
-                int sx = x0 + e;
-                float v = (sx >= 0 && sx < nx) ? row[sx] : 0.f;
+                for (int d = 0; d < LENS_TAPS; ++d)
 #pragma unroll
-                for (int j = 0; j < LENS_STRIP; ++j) out[j] = fmaf(w[j], v, out[j]);
+                    for (int j = 0; j < LENS_STRIP; ++j) out[j] = fmaf(p[d], s[j - d + LENS_TAPS - 1], out[j]);
             }
         }
 #pragma unroll
@@ -272,13 +297,14 @@ __global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict
 
 cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B) {
     ProfScope ps(c, GK_LENS_PREP);
-    lens_prep_kernel<<<(B + 63) / 64, 64, 0, c->stream>>>(d_params, B, c->d_lens_const);
+    lens_prep_kernel<<<(B + 31) / 32, 32 * LENS_PREP_ROLES, 0, c->stream>>>(d_params, B, c->d_lens_const);
     return cudaGetLastError();
 }
 
 cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2, int32_t* d_flags) {
-    int npx = c->grid.nx * c->grid.ny;
-    size_t smem = sizeof(float) * (LC_SIZE + ((c->kpsf * c->kpsf + 3) & ~3) + npx);
+    size_t smem = sizeof(float) * (LC_SIZE + (size_t)c->kpsf * lens_tap_pitch(c->kpsf) +
+                                   (size_t)(c->grid.ny + 1) * lens_img_pitch(c->grid.nx, c->kpsf));
+    if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
     static size_t configured = 0;
     if (smem > configured) {
         cudaError_t e = cudaFuncSetAttribute(lens_image_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
