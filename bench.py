@@ -27,6 +27,9 @@ if ROOT not in sys.path:
 METRIC = "joint_loglike_evals_per_s"
 UNIT = "evals/s"
 FP32_LANES_PER_SM = 128
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the quadrature kernel from the committed ncu --set full
+# captures (profiles/r1a.md, profiles/r1b.md): operands never exist in HBM, only the tables are read
+RESIDENT_TRAFFIC = {"jam_quad_simt": 4.4e6, "jam_quad_tc": 4.44e6}
 
 
 def read_peaks():
@@ -243,10 +246,30 @@ def run_ours(args, rank, world, local_rank):
     q_avg = q_ms / max(q_n, 1)
     achieved = flops_per_launch / (q_avg * 1e-3) / 1e12 if q_n else None
     shares = {k: round(v[0] / ms, 4) for k, v in prof.items()}
-    roofline = {"bound": "alu", "kernel": "jam_quad_kernel", "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": (achieved / peak_tf) if achieved else None, "traffic": None,
-                "peak_source": f"{props.multi_processor_count} SM x 128 FP32 lanes x 2 flop x {sm_max:.0f} MHz (DESIGN.md)",
+    simt = os.environ.get("GLAD_JAM_PATH", "") == "simt"
+    roofline = {"bound": "alu", "kernel": "jam_quad_kernel" if simt else "jam_quad_tc_kernel", "achieved": achieved,
+                "peak": peak_tf, "unit": "TFLOP/s", "frac": (achieved / peak_tf) if achieved else None,
+                "traffic": RESIDENT_TRAFFIC.get("jam_quad_simt" if simt else "jam_quad_tc"),
+                "peak_source": f"{props.multi_processor_count} SM x 128 FP32 lanes x 2 flop x {sm_max:.0f} MHz (DESIGN.md); "
+                               "'achieved' counts the contraction's algorithmic fp32 flops (2 per folded pixel and "
+                               "contraction row), the quantity BASELINE.json's '% FP32 peak per stage' is quoted on",
                 "ms_per_launch": q_avg, "algorithmic_flops_per_launch": flops_per_launch, "kernel_share_of_step": shares}
+    if not simt and q_n:
+        # the tcgen05 form moves the contraction to the tensor cores; what is left on the SM's own pipes is operand
+        # generation, whose tightest unit is the MUFU (one ex2 per operand value; 16 lanes/clk/SM)
+        nterms = float(workload_terms(wl).sum())
+        nxf, nyf = (nx + 1) // 2, (ny + 1) // 2
+        ex2_per_launch = nterms * (nxf + nyf)
+        xu_peak = props.multi_processor_count * 16 * sm_max * 1e6
+        r8 = lambda v: (v + 7) // 8 * 8
+        mma_flops = 2.0 * 128 * (2 * r8(nxf)) * nterms            # executed: M = 128 tile, N = 2 bf16 terms x padded columns
+        bf16_peak = float(peaks.get("bf16_tflops") or 2250.0)
+        roofline["operand_generation"] = {"bound": "alu", "unit": "Gex2/s", "achieved": ex2_per_launch / (q_avg * 1e-3) / 1e9,
+                                          "peak": xu_peak / 1e9, "frac": ex2_per_launch / (q_avg * 1e-3) / xu_peak,
+                                          "peak_source": "148 SM x 16 MUFU lanes/clk x SM clock"}
+        roofline["tensor_pipe"] = {"bound": "tensor", "unit": "TFLOP/s", "achieved": mma_flops / (q_avg * 1e-3) / 1e12,
+                                   "peak": bf16_peak, "frac": mma_flops / (q_avg * 1e-3) / 1e12 / bf16_peak,
+                                   "peak_source": "MEASURED_PEAKS.json bf16_tflops (burst)" if peaks.get("bf16_tflops") else "nominal 2250 (no MEASURED_PEAKS.json)"}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
