@@ -63,7 +63,6 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     do {
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-        if (!ok) __nanosleep(32);
     } while (!ok);
 }
 // UMMA shared-memory descriptor: K-major, no swizzle, version 1 (sm_100).  SBO = 128 B between 8-row groups
@@ -132,19 +131,33 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
     const int nl = a.nl, nmx = a.nmx, nu = a.nu, MC = a.MC, ny8 = a.ny8, nxp = a.nxp, N = a.N;
     const int nyb = ny8 >> 3, nxb = nxp >> 3;                        // 8-pixel blocks per oct: Y blocks, X blocks
     const int GA = NT * nyb, GB = NT * nxb;                          // core matrices per oct: the NT terms stacked
-    const int nup = (nu + 1) & ~1;
     const int a16 = (MC >> 3) * GA * 8, b16 = (MC >> 3) * GB * 8;    // 16-byte units per stage
     const int stage16 = a16 + b16;
-    float* s_tab = sm;
-    float* s_u2 = s_tab + a.tabsz;
-    float* s_wu2 = s_u2 + nup;
-    float* s_c2 = s_wu2 + nup;                       // ny8 + nxp squared coordinates, y first
+    // per-vector tables re-laid out for the coefficient block (one wide load per table and row):
+    //   s_lk[k] = (1/s_k^2, b_k-term, S0_k, NKS_k), s_ld[k] = D0_k, s_mj[j] = (1/s_j^2, 1-q_j^2, M_j, 0),
+    //   s_jk[j*nl+k] = (C_jk, D_jk), s_uw[iu] = (u^2, w u^2)
+    const float* TLg = Tg + JT_HDR;
+    const float* TMg = TLg + JL_COUNT * nl;
+    const float* TCg = TMg + JM_COUNT * nmx;
+    const float* TDg = TCg + nmx * nl;
+    float4* s_lk = reinterpret_cast<float4*>(sm);
+    float4* s_mj = s_lk + nl;
+    float2* s_jk = reinterpret_cast<float2*>(s_mj + nmx);
+    float2* s_uw = s_jk + nmx * nl;
+    float* s_ld = reinterpret_cast<float*>(s_uw + nu);
+    float* s_c2 = s_ld + ((nl + 3) & ~3);            // ny8 + nxp squared coordinates, y first
     // coefficient ring: 3 blocks of 256 rows, per block [-Q log2e | -P log2e | F0 | F1] x 256 floats
-    float* s_coef = sm + ((a.tabsz + 2 * nup + ny8 + nxp + 31) & ~31);
+    float* s_coef = sm + ((4 * nl + 4 * nmx + 2 * nmx * nl + 2 * nu + ((nl + 3) & ~3) + ny8 + nxp + 31) & ~31);
     uint4* s_ops = reinterpret_cast<uint4*>(s_coef + 3 * 4 * TC_COEF_ROWS);   // 2 stages + tail pad, 128-byte aligned
 
-    for (int i = tid; i < a.tabsz; i += TC_THREADS) s_tab[i] = Tg[i];
-    for (int i = tid; i < nu; i += TC_THREADS) { float u = a.un[i]; s_u2[i] = u * u; s_wu2[i] = a.uw[i] * u * u; }
+    for (int k = tid; k < nl; k += TC_THREADS) {
+        s_lk[k] = make_float4(TLg[JL_INVS2 * nl + k], TLg[JL_BKQ * nl + k], TLg[JL_S0 * nl + k], TLg[JL_NKS * nl + k]);
+        s_ld[k] = TLg[JL_D0 * nl + k];
+    }
+    for (int j = tid; j < nmx; j += TC_THREADS)
+        s_mj[j] = make_float4(TMg[JM_INVS2 * nmx + j], TMg[JM_OMQ2 * nmx + j], TMg[JM_MJ * nmx + j], 0.f);
+    for (int i = tid; i < nmx * nl; i += TC_THREADS) s_jk[i] = make_float2(TCg[i], TDg[i]);
+    for (int i = tid; i < nu; i += TC_THREADS) { float u = a.un[i]; s_uw[i] = make_float2(u * u, a.uw[i] * u * u); }
     for (int i = tid; i < ny8 + nxp; i += TC_THREADS) {              // padded pixels: coordinate 0, finite values, never stored
         float v = 0.f;
         if (i < ny8) { if (i < a.nyf) v = a.yf2[i]; }
@@ -169,7 +182,7 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem = s_tmem;
 
-    const int nm = __float_as_int(s_tab[JH_NM]);
+    const int nm = __float_as_int(Tg[JH_NM]);
     const int pairs = nm * nl;
     const int M = nu * pairs;
     const int NCH = (M + MC - 1) >> a.lgMC;
@@ -192,19 +205,26 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
                 const uint32_t d = tmem + (uint32_t)(g & 1) * dstride;
                 const uint32_t sa = ops_addr + (uint32_t)buf * stage16 * 16, sb = sa + a16 * 16;
                 uint32_t accum = (it - g * a.FL) ? 1u : 0u;
-                for (int ks = 0; ks < (MC >> 4); ++ks) {
-                    const uint64_t bd = umma_desc(sb + ks * 2 * b_lbo, b_lbo);
-                    if (!a.multi) {
-                        umma_bf16(d, umma_desc(sa + ks * 2 * a_lbo, a_lbo), bd, idesc_base | ((uint32_t)(N >> 3) << 17), accum);
-                    } else {
+                // descriptors advance by one K-step (two octs) per MMA: only the 14-bit start-address field changes
+                uint64_t ad = umma_desc(sa, a_lbo), bd = umma_desc(sb, b_lbo);
+                const uint64_t ad_step = (uint64_t)((2 * a_lbo) >> 4), bd_step = (uint64_t)((2 * b_lbo) >> 4);
+                const uint32_t idesc1 = idesc_base | ((uint32_t)(N >> 3) << 17);
+                if (!a.multi) {
+#pragma unroll 4
+                    for (int ks = 0; ks < (MC >> 4); ++ks) {
+                        umma_bf16(d, ad, bd, idesc1, accum);
+                        accum = 1u; ad += ad_step; bd += bd_step;
+                    }
+                } else {
+                    for (int ks = 0; ks < (MC >> 4); ++ks) {
 #pragma unroll
                         for (int t = 0; t < NT; ++t) {
-                            umma_bf16(d, umma_desc(sa + ks * 2 * a_lbo + t * nyb * 128, a_lbo), bd,
+                            umma_bf16(d, ad + (uint64_t)((t * nyb * 128) >> 4), bd,
                                       idesc_base | ((uint32_t)(((NT - t) * nxp) >> 3) << 17), accum);
                             accum = 1u;
                         }
+                        ad += ad_step; bd += bd_step;
                     }
-                    accum = 1u;
                 }
                 umma_commit(smem_u32(&s_bar[buf]));
                 if (it == nch - 1) umma_commit(smem_u32(&s_bar[2]));
@@ -213,40 +233,51 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
         }
     } else {
         // ------------------------------------------------------------------ producer warps
-        const float* TL = s_tab + JT_HDR;
-        const float* TM = TL + JL_COUNT * nl;
-        const float* TC = TM + JM_COUNT * nmx;
-        const float* TD = TC + nmx * nl;
-        const float cos2i = s_tab[JH_COS2I];
-        const float inv_pairs = 1.f / (float)pairs, inv_nl = 1.f / (float)nl;
+        const float cos2i = Tg[JH_COS2I];
 
-        // row m = cbk*256 + tid of the contraction: (-Q log2e, -P log2e, F0, F1); rows past the end have F0 = F1 = 0
-        // and contribute 0.  Ring slot cbk % 3: a block is written while the previous one is read and the one
-        // before that may still be read by a warp that lags one chunk behind (needs MC <= 128).
-        auto coef_block = [&](int cbk) {
-            const int m = cbk * TC_COEF_ROWS + tid;
+        // Coefficients of contraction row m = (iu, j, k), k fastest: (-Q log2e, -P log2e, F0, F1); rows past the end have
+        // F0 = F1 = 0 and contribute 0.  Blocks of 256 rows are computed in order, so the thread's (iu, j, k) advances
+        // by 256 rows with two carries instead of two divisions.  Ring slot = block % 3: a block is written while the
+        // previous one is read and the one before that may still be read by a warp that lags one chunk behind
+        // (needs MC <= 128: the reader of block b+1 has passed the "empty" wait of a chunk every producer wrote b+1 in).
+        const int adv_u = TC_COEF_ROWS / pairs, adv_r = TC_COEF_ROWS - adv_u * pairs, adv_j = adv_r / nl, adv_k = adv_r - adv_j * nl;
+        // the thread's (iu, j, k) lives in shared memory between calls: registers are the scarce resource here
+        int* s_row = reinterpret_cast<int*>(s_ops + 2 * stage16 + 128) + tid;            // [3][TC_PRODUCERS]
+        {
+            const int m = ((c0 * MC) >> 8) * TC_COEF_ROWS + tid;
+            const int iu = m / pairs, rem = m - iu * pairs, j = rem / nl;
+            s_row[0] = iu; s_row[TC_PRODUCERS] = j; s_row[2 * TC_PRODUCERS] = rem - j * nl;
+        }
+        auto coef_block = [&](int cslot) {
+            int ciu = s_row[0], cj = s_row[TC_PRODUCERS], ck = s_row[2 * TC_PRODUCERS];
             float cq = 0.f, cp = 0.f, f0 = 0.f, f1 = 0.f;
-            if (m < M) {
-                const int iu = div_small(m, pairs, inv_pairs), rem = m - iu * pairs;
-                const int j = div_small(rem, nl, inv_nl), k = rem - j * nl;
-                const float u2 = s_u2[iu];
-                const float omq2 = TM[JM_OMQ2 * nmx + j];
-                const float auj = u2 * TM[JM_INVS2 * nmx + j];
-                const float gg = 1.f - omq2 * u2;
-                const float bb = __fdividef(omq2 * u2 * auj, gg);
-                const float A = 0.5f * (auj + TL[JL_INVS2 * nl + k]);
-                const float Bc = 0.5f * (TL[JL_BKQ * nl + k] + bb);
+            if (ciu < nu) {
+                const float2 uw = s_uw[ciu];
+                const float4 mj = s_mj[cj];
+                const float4 lk = s_lk[ck];
+                const float2 jk = s_jk[cj * nl + ck];
+                const float d0 = s_ld[ck];
+                const float u2 = uw.x;
+                const float t = mj.y * u2, auj = u2 * mj.x;
+                const float gg = 1.f - t;
+                const float bb = t * auj * __frcp_rn(gg);
+                const float A = 0.5f * (auj + lk.x);
+                const float Bc = 0.5f * (lk.y + bb);
                 const float E = fmaf(Bc, cos2i, A);
-                const float D = fmaf(-TD[j * nl + k], u2, TL[JL_D0 * nl + k]);
-                const float inv = __fdividef(rsqrtf(E * gg), 1.f - TC[j * nl + k] * u2);
-                const float pref = s_wu2[iu] * TM[JM_MJ * nmx + j] * inv;
+                const float D = fmaf(-jk.y, u2, d0);
+                const float inv = rsqrtf(E * gg) * __frcp_rn(fmaf(-jk.x, u2, 1.f));
+                const float pref = uw.y * mj.z * inv;
                 cp = -A * LOG2E_F;
-                cq = -__fdividef(A * (A + Bc), E) * LOG2E_F;
-                f0 = pref * TL[JL_S0 * nl + k];
-                f1 = pref * TL[JL_NKS * nl + k] * D;
+                cq = -(A * (A + Bc)) * __frcp_rn(E) * LOG2E_F;
+                f0 = pref * lk.z;
+                f1 = pref * lk.w * D;
             }
-            float* dst = s_coef + (cbk % 3) * (4 * TC_COEF_ROWS) + tid;
+            float* dst = s_coef + cslot * (4 * TC_COEF_ROWS) + tid;
             dst[0] = cq; dst[TC_COEF_ROWS] = cp; dst[2 * TC_COEF_ROWS] = f0; dst[3 * TC_COEF_ROWS] = f1;
+            ck += adv_k; if (ck >= nl) { ck -= nl; ++cj; }
+            cj += adv_j; if (cj >= nm) { cj -= nm; ++ciu; }
+            ciu += adv_u;
+            s_row[0] = ciu; s_row[TC_PRODUCERS] = cj; s_row[2 * TC_PRODUCERS] = ck;
         };
 
         // Quarter-warp = one oct o of the chunk (8 contraction rows), lane l8 = pixel within an 8-pixel block.  The
@@ -259,9 +290,9 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
         const int g = warp & (NG - 1), oct = (qw & 3) + 4 * (warp / NG);
         const int yb0 = (g * nyb) / NG, yb1 = ((g + 1) * nyb) / NG;
         const int xb0 = ((NG - 1 - g) * nxb) / NG, xb1 = ((NG - g) * nxb) / NG;
-        auto produce = [&](int c, int buf) {
-            const int row0 = c * MC;
-            const float* cb = s_coef + ((row0 >> 8) % 3) * (4 * TC_COEF_ROWS) + (row0 & (TC_COEF_ROWS - 1)) + 8 * oct;
+        int pslot = ((c0 * MC) >> 8) % 3, crow = (c0 * MC) & (TC_COEF_ROWS - 1);   // ring slot / row offset of the chunk being read
+        auto produce = [&](int buf) {
+            const float* cb = s_coef + pslot * (4 * TC_COEF_ROWS) + crow + 8 * oct;
             uint4* stA = s_ops + buf * stage16 + oct * GA * 8 + l8;
             uint4* stB = s_ops + buf * stage16 + a16 + oct * GB * 8 + l8;
             {
@@ -314,20 +345,23 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
         };
 
         int gf = 0;                                                     // next accumulator group to add into acc
+        const uint32_t bar_empty = smem_u32(&s_bar[0]);
         if (nch > 0) {
-            coef_block((c0 * MC) >> 8);
-            coef_block(((c0 * MC) >> 8) + 1);
+            coef_block(pslot);
+            coef_block(pslot == 2 ? 0 : pslot + 1);
             bar_sync(3, TC_PRODUCERS);
         }
         for (int it = 0; it < nch; ++it) {
-            const int c = c0 + it, buf = it & 1;
+            const int buf = it & 1;
             if (it >= 2) {
-                mbar_wait(smem_u32(&s_bar[buf]), ((it >> 1) - 1) & 1);  // MMAs up to chunk it-2 are complete
+                mbar_wait(bar_empty + 8 * buf, ((it >> 1) - 1) & 1);    // MMAs up to chunk it-2 are complete
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 while ((gf + 1) * a.FL - 1 <= it - 2) flush(gf++);
             }
-            if (it > 0 && ((c * MC) & (TC_COEF_ROWS - 1)) == 0) coef_block(((c * MC) >> 8) + 1);
-            produce(c, buf);
+            if (it > 0 && crow == 0) coef_block(pslot == 2 ? 0 : pslot + 1);    // first chunk of a block: prepare the next one
+            produce(buf);
+            crow += MC;
+            if (crow == TC_COEF_ROWS) { crow = 0; pslot = pslot == 2 ? 0 : pslot + 1; }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             bar_arrive(1 + buf, TC_THREADS);
         }
@@ -406,12 +440,12 @@ cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S) {
     a.un = c->d_un; a.uw = c->d_uw; a.nu = c->nu;
     a.xf2 = c->d_xf2; a.yf2 = c->d_yf2; a.nxf = c->nxf; a.nyf = c->nyf;
     a.S = S; a.partial = c->d_partial;
-    const size_t fixed = (((size_t)a.tabsz + 2 * (size_t)((c->nu + 1) & ~1) + (size_t)(a.ny8 + a.nxp) + 31) & ~(size_t)31) * 4 +
-                         3 * TC_COEF_ROWS * 16;
+    const size_t fixed = (((size_t)4 * nl + 4 * nmx + 2 * (size_t)nmx * nl + 2 * (size_t)c->nu + ((nl + 3) & ~3) +
+                           (size_t)(a.ny8 + a.nxp) + 31) & ~(size_t)31) * 4 + 3 * TC_COEF_ROWS * 16;
     const size_t budget = nacc <= 40 ? 112 * 1024 : 220 * 1024;          // two CTAs per SM when the map is small
     size_t smem = 0;
     for (a.MC = 128, a.lgMC = 7; a.MC >= 64; a.MC >>= 1, --a.lgMC) {
-        size_t ops = 2 * (size_t)a.MC * NT * (a.ny8 + a.nxp) * 2 + 2048;  // two stages + the M = 128 over-read
+        size_t ops = 2 * (size_t)a.MC * NT * (a.ny8 + a.nxp) * 2 + 2048 + 3 * TC_PRODUCERS * 4;  // two stages + the M = 128 over-read + row state
         const size_t scr = (size_t)128 * a.N * 4;                        // epilogue scratch reuses the stages
         if (ops < scr) ops = scr;
         smem = fixed + ops;
