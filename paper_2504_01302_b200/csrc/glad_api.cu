@@ -267,7 +267,7 @@ static glad_status jam_impl(glad_ctx* c, const float* d_dyn, int B, const float*
     st = grow(c, &c->d_partial, &c->partial_cap, (size_t)B * S * c->nxf * c->nyf);
     if (st != GLAD_OK) return st;
     CU(launch_jam_prep(c, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian), "jam_prep_kernel");
-    if (!c->jam_simt && jam_quad_tc_supported(c)) CU(launch_jam_quad_tc(c, B, nl, nmx, S), "jam_quad_tc_kernel");
+    if (!c->jam_simt && jam_quad_tc_supported(c, nl, nmx)) CU(launch_jam_quad_tc(c, B, nl, nmx, S), "jam_quad_tc_kernel");
     else CU(launch_jam_quad(c, B, nl, nmx, S), "jam_quad_kernel");
     CU(launch_jam_post(c, B, nl, nmx, S, d_vrms, d_chi2, d_v2map, d_flags), "jam_post_kernel");
     return GLAD_OK;

@@ -119,8 +119,9 @@ cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d
 cudaError_t launch_joint(glad_ctx* c, int B, const float* d_c2l, const float* d_c2d, const int32_t* d_fl,
                          const int32_t* d_fd, float* d_loglike, int32_t* d_flags);
 cudaError_t launch_kin_weights(glad_ctx* c);
-// tensor-core (tcgen05) form of row a6; supported when the folded grid has ny_f <= 128 and nx_f <= 256
-bool jam_quad_tc_supported(const glad_ctx* c);
+// tensor-core (tcgen05) form of row a6; supported when the folded grid has ny_f <= 128, N = terms * nx_f <= 256
+// and two operand stages fit in shared memory
+bool jam_quad_tc_supported(const glad_ctx* c, int nl, int nmx);
 cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S);
 // launch geometry of the quadrature kernel for the current sky grid: threads per CTA, thread groups
 int jam_quad_geometry(const glad_ctx* c, int* groups);

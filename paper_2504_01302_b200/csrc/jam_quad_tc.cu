@@ -22,11 +22,14 @@
 // contraction rows, an "oct"), 128 contiguous bytes; SBO = 128 B between 8-pixel groups, LBO between the two
 // octs of one K = 16 step.  A quarter-warp writes one core matrix with one conflict-free 16-byte store per lane.
 //
-// CTA = (parameter vector, K-slice), 8 producer warps + 1 MMA warp, no CTA-wide barrier in the main loop:
+// CTA = (parameter vector, K-slice), PW producer warps + 1 MMA warp, ONE CTA per SM, no CTA-wide barrier in the
+// main loop.  The kernel is latency-bound (profiles/r1b.md: ~10 cycles per instruction and warp), so the design
+// goal is resident warps and registers per warp: with one CTA per SM the running map is spread over PW/4 warps per
+// TMEM lane quarter (80 columns -> 16..24 accumulator registers per thread instead of 40).
 //   producer warp, chunk c (MC contraction rows):  wait until the MMAs that read stage c%2 have completed
-//   (mbarrier armed by tcgen05.commit) -> add finished accumulator groups into registers -> its share of the
-//   coefficients of the next 256 rows -> its items (oct, 8-pixel block) of chunk c into stage c%2 ->
-//   fence.proxy.async -> bar.arrive on the stage's "full" named barrier (does not block).
+//   (mbarrier armed by tcgen05.commit) -> add finished accumulator groups into registers -> every R-th chunk one
+//   coefficient row of chunk c+2 -> its blocks of chunk c into stage c%2 -> fence.proxy.async -> bar.arrive on
+//   the stage's "full" named barrier (does not block).
 //   MMA warp, chunk c:  bar.sync on "full" -> one lane issues the MMAs of the chunk and commits to "empty".
 //   The tensor core works on chunk c while the CUDA cores produce chunk c+1.
 #include <stdlib.h>
@@ -34,9 +37,7 @@
 #include "glad_internal.h"
 
 #define LOG2E_F 1.4426950408889634f
-#define TC_PRODUCERS 256
-#define TC_THREADS (TC_PRODUCERS + 32)
-#define TC_COEF_ROWS 256
+#define TC_COEF_SLOTS 4
 
 struct JTArgs {
     const float* tab; int tabsz; int nl; int nmx;
@@ -45,14 +46,18 @@ struct JTArgs {
     int ny8, nxp;        // padded map rows (multiple of 8) and columns (multiple of 8 or 16)
     int multi;           // 0: A = [Y1;..;Y_NT] in one M=128 tile;  1: NT MMAs per K-step
     int N;               // accumulator columns = NT * nxp
-    int MC, lgMC;        // contraction rows per stage (power of two, 64..256)
+    int MC, lgMC;        // contraction rows per stage (128 or 256)
     int FL;              // chunks per accumulator group (>= 1)
     int tmem_cols;       // power of two >= 2 * N
     int S;
     float* partial;
 };
 
+#ifdef ABL_MUFU
+__device__ __forceinline__ float ex2_tc(float x) { return x * 1.0001f; }
+#else
 __device__ __forceinline__ float ex2_tc(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+#endif
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -114,12 +119,15 @@ __device__ __forceinline__ int div_small(int a, int d, float inv) {
     return r < 0 ? q - 1 : (r >= d ? q + 1 : q);
 }
 
+
 __device__ __forceinline__ void bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 __device__ __forceinline__ void bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 
-// NT = bf16 terms per operand value, NACC = accumulator registers per thread (>= N/2, multiple of 8)
-template <int NT, int NACC>
-__global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_kernel(JTArgs a) {
+// NT = bf16 terms per operand value, PW = producer warps (16 or 24), NACC = accumulator registers per thread
+// (multiple of 8, NACC * PW/4 >= N)
+template <int NT, int NACC, int PW>
+__global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) {
+    constexpr int NPROD = PW * 32, NTHR = NPROD + 32;
     extern __shared__ __align__(128) float sm[];
     __shared__ __align__(8) uint64_t s_bar[3];     // empty[0], empty[1], done
     __shared__ uint32_t s_tmem;
@@ -133,7 +141,7 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
     const int GA = NT * nyb, GB = NT * nxb;                          // core matrices per oct: the NT terms stacked
     const int a16 = (MC >> 3) * GA * 8, b16 = (MC >> 3) * GB * 8;    // 16-byte units per stage
     const int stage16 = a16 + b16;
-    // per-vector tables re-laid out for the coefficient block (one wide load per table and row):
+    // per-vector tables re-laid out for the coefficient rows (one wide load per table and row):
     //   s_lk[k] = (1/s_k^2, b_k-term, S0_k, NKS_k), s_ld[k] = D0_k, s_mj[j] = (1/s_j^2, 1-q_j^2, M_j, 0),
     //   s_jk[j*nl+k] = (C_jk, D_jk), s_uw[iu] = (u^2, w u^2)
     const float* TLg = Tg + JT_HDR;
@@ -146,25 +154,25 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
     float2* s_uw = s_jk + nmx * nl;
     float* s_ld = reinterpret_cast<float*>(s_uw + nu);
     float* s_c2 = s_ld + ((nl + 3) & ~3);            // ny8 + nxp squared coordinates, y first
-    // coefficient ring: 3 blocks of 256 rows, per block [-Q log2e | -P log2e | F0 | F1] x 256 floats
+    // coefficient ring: TC_COEF_SLOTS chunks, per chunk [-Q log2e | -P log2e | F0 | F1] x MC floats
     float* s_coef = sm + ((4 * nl + 4 * nmx + 2 * nmx * nl + 2 * nu + ((nl + 3) & ~3) + ny8 + nxp + 31) & ~31);
-    uint4* s_ops = reinterpret_cast<uint4*>(s_coef + 3 * 4 * TC_COEF_ROWS);   // 2 stages + tail pad, 128-byte aligned
+    uint4* s_ops = reinterpret_cast<uint4*>(s_coef + TC_COEF_SLOTS * 4 * MC);   // 2 stages + tail pad, 128-byte aligned
 
-    for (int k = tid; k < nl; k += TC_THREADS) {
+    for (int k = tid; k < nl; k += NTHR) {
         s_lk[k] = make_float4(TLg[JL_INVS2 * nl + k], TLg[JL_BKQ * nl + k], TLg[JL_S0 * nl + k], TLg[JL_NKS * nl + k]);
         s_ld[k] = TLg[JL_D0 * nl + k];
     }
-    for (int j = tid; j < nmx; j += TC_THREADS)
+    for (int j = tid; j < nmx; j += NTHR)
         s_mj[j] = make_float4(TMg[JM_INVS2 * nmx + j], TMg[JM_OMQ2 * nmx + j], TMg[JM_MJ * nmx + j], 0.f);
-    for (int i = tid; i < nmx * nl; i += TC_THREADS) s_jk[i] = make_float2(TCg[i], TDg[i]);
-    for (int i = tid; i < nu; i += TC_THREADS) { float u = a.un[i]; s_uw[i] = make_float2(u * u, a.uw[i] * u * u); }
-    for (int i = tid; i < ny8 + nxp; i += TC_THREADS) {              // padded pixels: coordinate 0, finite values, never stored
+    for (int i = tid; i < nmx * nl; i += NTHR) s_jk[i] = make_float2(TCg[i], TDg[i]);
+    for (int i = tid; i < nu; i += NTHR) { float u = a.un[i]; s_uw[i] = make_float2(u * u, a.uw[i] * u * u); }
+    for (int i = tid; i < ny8 + nxp; i += NTHR) {                    // padded pixels: coordinate 0, finite values, never stored
         float v = 0.f;
         if (i < ny8) { if (i < a.nyf) v = a.yf2[i]; }
         else { int j = i - ny8; if (j < a.nxf) v = a.xf2[j]; }
         s_c2[i] = v;
     }
-    for (int i = tid; i < 2 * stage16 + 128; i += TC_THREADS) s_ops[i] = make_uint4(0u, 0u, 0u, 0u);
+    for (int i = tid; i < 2 * stage16 + 128; i += NTHR) s_ops[i] = make_uint4(0u, 0u, 0u, 0u);
     if (tid == 0) {
         mbar_init(smem_u32(&s_bar[0]), 1);
         mbar_init(smem_u32(&s_bar[1]), 1);
@@ -190,7 +198,7 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
     const int nch = c1 - c0;
     const uint32_t dstride = (uint32_t)a.tmem_cols >> 1;                // columns between the two accumulator buffers
 
-    if (warp == TC_PRODUCERS / 32) {
+    if (warp == PW) {
         // ------------------------------------------------------------------ MMA warp
         // instruction descriptor: D fp32, A/B bf16, both K-major, M = 128, N>>3 filled per MMA
         const uint32_t idesc_base = (1u << 4) | (1u << 7) | (1u << 10) | (8u << 24);
@@ -198,7 +206,7 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
         const uint32_t a_lbo = GA * 128, b_lbo = GB * 128;              // bytes between the two octs of a K-step
         for (int it = 0; it < nch; ++it) {
             const int buf = it & 1;
-            bar_sync(1 + buf, TC_THREADS);                              // every producer has written its share of chunk it
+            bar_sync(1 + buf, NTHR);                                    // every producer has written its share of chunk it
             if (lane == 0) {
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const int g = it / a.FL;
@@ -234,29 +242,24 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
     } else {
         // ------------------------------------------------------------------ producer warps
         const float cos2i = Tg[JH_COS2I];
+        const float inv_pairs = 1.f / (float)pairs, inv_nl = 1.f / (float)nl;
 
         // Coefficients of contraction row m = (iu, j, k), k fastest: (-Q log2e, -P log2e, F0, F1); rows past the end have
-        // F0 = F1 = 0 and contribute 0.  Blocks of 256 rows are computed in order, so the thread's (iu, j, k) advances
-        // by 256 rows with two carries instead of two divisions.  Ring slot = block % 3: a block is written while the
-        // previous one is read and the one before that may still be read by a warp that lags one chunk behind
-        // (needs MC <= 128: the reader of block b+1 has passed the "empty" wait of a chunk every producer wrote b+1 in).
-        const int adv_u = TC_COEF_ROWS / pairs, adv_r = TC_COEF_ROWS - adv_u * pairs, adv_j = adv_r / nl, adv_k = adv_r - adv_j * nl;
-        // the thread's (iu, j, k) lives in shared memory between calls: registers are the scarce resource here
-        int* s_row = reinterpret_cast<int*>(s_ops + 2 * stage16 + 128) + tid;            // [3][TC_PRODUCERS]
-        {
-            const int m = ((c0 * MC) >> 8) * TC_COEF_ROWS + tid;
-            const int iu = m / pairs, rem = m - iu * pairs, j = rem / nl;
-            s_row[0] = iu; s_row[TC_PRODUCERS] = j; s_row[2 * TC_PRODUCERS] = rem - j * nl;
-        }
-        auto coef_block = [&](int cslot) {
-            int ciu = s_row[0], cj = s_row[TC_PRODUCERS], ck = s_row[2 * TC_PRODUCERS];
+        // F0 = F1 = 0 and contribute 0.  Chunk `rc` (relative to c0) lives in ring slot rc % 4.  It is written during
+        // iteration rc-2 and read during iteration rc: the reader has passed the "empty" wait of chunk rc-2, so every
+        // producer has arrived on "full" of rc-2, i.e. finished writing; the slot's previous tenant rc-4 was last read
+        // in iteration rc-4, which every producer had finished before the writer passed the "empty" wait of rc-4.
+        auto coef_row = [&](int rc, int r) {
+            const int m = (c0 + rc) * MC + r;
             float cq = 0.f, cp = 0.f, f0 = 0.f, f1 = 0.f;
-            if (ciu < nu) {
-                const float2 uw = s_uw[ciu];
-                const float4 mj = s_mj[cj];
-                const float4 lk = s_lk[ck];
-                const float2 jk = s_jk[cj * nl + ck];
-                const float d0 = s_ld[ck];
+            if (m < M) {
+                const int iu = div_small(m, pairs, inv_pairs), rem = m - iu * pairs;
+                const int j = div_small(rem, nl, inv_nl), k = rem - j * nl;
+                const float2 uw = s_uw[iu];
+                const float4 mj = s_mj[j];
+                const float4 lk = s_lk[k];
+                const float2 jk = s_jk[j * nl + k];
+                const float d0 = s_ld[k];
                 const float u2 = uw.x;
                 const float t = mj.y * u2, auj = u2 * mj.x;
                 const float gg = 1.f - t;
@@ -272,30 +275,42 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
                 f0 = pref * lk.z;
                 f1 = pref * lk.w * D;
             }
-            float* dst = s_coef + cslot * (4 * TC_COEF_ROWS) + tid;
-            dst[0] = cq; dst[TC_COEF_ROWS] = cp; dst[2 * TC_COEF_ROWS] = f0; dst[3 * TC_COEF_ROWS] = f1;
-            ck += adv_k; if (ck >= nl) { ck -= nl; ++cj; }
-            cj += adv_j; if (cj >= nm) { cj -= nm; ++ciu; }
-            ciu += adv_u;
-            s_row[0] = ciu; s_row[TC_PRODUCERS] = cj; s_row[2 * TC_PRODUCERS] = ck;
+            float* dst = s_coef + (rc & (TC_COEF_SLOTS - 1)) * (4 * MC) + r;
+            dst[0] = cq; dst[MC] = cp; dst[2 * MC] = f0; dst[3 * MC] = f1;
         };
+        const int R = NPROD / MC;                                       // producer thread groups of MC threads
+        const int cgrp = tid / MC, crow = tid - cgrp * MC;
 
-        // Quarter-warp = one oct o of the chunk (8 contraction rows), lane l8 = pixel within an 8-pixel block.  The
-        // thread loads the 8 rows' coefficients once (LDS.128 delivers 512 B per warp whatever the broadcast, so
-        // coefficient loads are paid per thread, not per address) and reuses them over its share of the Y blocks,
-        // then of the X blocks.  The blocks of an oct are cut into NG = 32/(MC/8) contiguous groups; a warp holds
-        // one group index (no divergence) and four octs; the X group is mirrored so that ragged splits even out.
+        // Quarter-warp = one oct of the chunk (8 contraction rows), lane l8 = pixel within an 8-pixel block.  The
+        // thread loads the 8 rows' coefficients once (LDS.128 delivers 512 B per warp whatever the broadcast) and
+        // reuses them over its blocks.  The oct's block list [Y blocks | X blocks] is cut into NQ contiguous ranges
+        // of about equal cost (a Y block ~3, an X block ~5); a warp holds one range index and four octs.
         const int qw = tid >> 3, l8 = tid & 7;
-        const int NG = 256 / MC;                                        // 2 (MC = 128) or 4 (MC = 64)
-        const int g = warp & (NG - 1), oct = (qw & 3) + 4 * (warp / NG);
-        const int yb0 = (g * nyb) / NG, yb1 = ((g + 1) * nyb) / NG;
-        const int xb0 = ((NG - 1 - g) * nxb) / NG, xb1 = ((NG - g) * nxb) / NG;
-        int pslot = ((c0 * MC) >> 8) % 3, crow = (c0 * MC) & (TC_COEF_ROWS - 1);   // ring slot / row offset of the chunk being read
-        auto produce = [&](int buf) {
-            const float* cb = s_coef + pslot * (4 * TC_COEF_ROWS) + crow + 8 * oct;
+        const int NQ = (NPROD >> 3) / (MC >> 3);                        // quarter-warps per oct: 2, 3, 4 or 6
+        const int role = warp % NQ, oct = (qw & 3) + 4 * (warp / NQ);
+        int yb0, yb1, xb0, xb1;
+        {
+            const int ctot = 3 * nyb + 5 * nxb;
+            int bnd[2];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int target = ((role + e) * ctot * 2 + NQ) / (2 * NQ);          // round(role * ctot / NQ)
+                int best = 0, bestd = target, pre = 0;
+                for (int i = 1; i <= nyb + nxb; ++i) {
+                    pre += i <= nyb ? 3 : 5;
+                    const int dd = pre > target ? pre - target : target - pre;
+                    if (dd < bestd) { bestd = dd; best = i; }
+                }
+                bnd[e] = (role + e == NQ) ? nyb + nxb : ((role + e == 0) ? 0 : best);
+            }
+            yb0 = min(bnd[0], nyb); yb1 = min(bnd[1], nyb);
+            xb0 = max(bnd[0], nyb) - nyb; xb1 = max(bnd[1], nyb) - nyb;
+        }
+        auto produce = [&](int it, int buf) {
+            const float* cb = s_coef + (it & (TC_COEF_SLOTS - 1)) * (4 * MC) + 8 * oct;
             uint4* stA = s_ops + buf * stage16 + oct * GA * 8 + l8;
             uint4* stB = s_ops + buf * stage16 + a16 + oct * GB * 8 + l8;
-            {
+            if (yb0 < yb1) {
                 const float4 e0 = *reinterpret_cast<const float4*>(cb), e1 = *reinterpret_cast<const float4*>(cb + 4);
                 for (int blk = yb0; blk < yb1; ++blk) {
                     const float q = s_c2[blk * 8 + l8];
@@ -306,11 +321,11 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
                     split_store<NT>(v, stA + blk * 8, nyb * 8);
                 }
             }
-            {
-                const float* cx = cb + TC_COEF_ROWS;
+            if (xb0 < xb1) {
+                const float* cx = cb + MC;
                 const float4 p0 = *reinterpret_cast<const float4*>(cx), p1 = *reinterpret_cast<const float4*>(cx + 4);
-                const float4 g0 = *reinterpret_cast<const float4*>(cx + TC_COEF_ROWS), g1 = *reinterpret_cast<const float4*>(cx + TC_COEF_ROWS + 4);
-                const float4 h0 = *reinterpret_cast<const float4*>(cx + 2 * TC_COEF_ROWS), h1 = *reinterpret_cast<const float4*>(cx + 2 * TC_COEF_ROWS + 4);
+                const float4 g0 = *reinterpret_cast<const float4*>(cx + MC), g1 = *reinterpret_cast<const float4*>(cx + MC + 4);
+                const float4 h0 = *reinterpret_cast<const float4*>(cx + 2 * MC), h1 = *reinterpret_cast<const float4*>(cx + 2 * MC + 4);
                 for (int blk = xb0; blk < xb1; ++blk) {
                     const float q = s_c2[ny8 + blk * 8 + l8];
                     const f32x2 qq = pk2(q, q);
@@ -324,15 +339,16 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
             }
         };
 
-        // running map in registers: thread (lane quarter lq, column half) holds D[32 lq + lane][half * NACC + i]
+        // running map in registers: thread (lane quarter lq, column group cg) holds D[32 lq + lane][cg * NACC + i]
         float acc[NACC];
 #pragma unroll
         for (int i = 0; i < NACC; ++i) acc[i] = 0.f;
-        const int lq = warp & 3, half = warp >> 2;
+        const int lq = warp & 3, cg = warp >> 2;
         auto flush = [&](int g) {
-            const uint32_t taddr = tmem + ((uint32_t)(32 * lq) << 16) + (uint32_t)(g & 1) * dstride + (uint32_t)(half * NACC);
+            const uint32_t taddr = tmem + ((uint32_t)(32 * lq) << 16) + (uint32_t)(g & 1) * dstride + (uint32_t)(cg * NACC);
 #pragma unroll
             for (int i = 0; i < NACC; i += 8) {
+                if (cg * NACC + i >= N) break;                          // warp-uniform: columns past the accumulator
                 uint32_t r[8];
                 asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
                              : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
@@ -347,10 +363,10 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
         int gf = 0;                                                     // next accumulator group to add into acc
         const uint32_t bar_empty = smem_u32(&s_bar[0]);
         if (nch > 0) {
-            coef_block(pslot);
-            coef_block(pslot == 2 ? 0 : pslot + 1);
-            bar_sync(3, TC_PRODUCERS);
+            if (cgrp < 2 && cgrp < nch) coef_row(cgrp, crow);           // chunks 0 and 1
+            bar_sync(3, NPROD);
         }
+        int cphase = 0;                                                 // it % R
         for (int it = 0; it < nch; ++it) {
             const int buf = it & 1;
             if (it >= 2) {
@@ -358,12 +374,11 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 while ((gf + 1) * a.FL - 1 <= it - 2) flush(gf++);
             }
-            if (it > 0 && crow == 0) coef_block(pslot == 2 ? 0 : pslot + 1);    // first chunk of a block: prepare the next one
-            produce(buf);
-            crow += MC;
-            if (crow == TC_COEF_ROWS) { crow = 0; pslot = pslot == 2 ? 0 : pslot + 1; }
+            if (cgrp == cphase && it + 2 < nch) coef_row(it + 2, crow); // one thread group in turn prepares chunk it+2
+            cphase = cphase + 1 == R ? 0 : cphase + 1;
+            produce(it, buf);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            bar_arrive(1 + buf, TC_THREADS);
+            bar_arrive(1 + buf, NTHR);
         }
 
         // epilogue: remaining groups -> registers -> shared memory (fold the term blocks) -> this slice's partial map
@@ -377,12 +392,12 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
             const int row = 32 * lq + lane;
 #pragma unroll
             for (int i = 0; i < NACC; ++i) {
-                const int col = half * NACC + i;
+                const int col = cg * NACC + i;
                 if (col < N) scr[row * N + col] = acc[i];
             }
-            bar_sync(3, TC_PRODUCERS);
+            bar_sync(3, NPROD);
             const int TR = a.multi ? 1 : NT;
-            for (int i = tid; i < npf; i += TC_PRODUCERS) {
+            for (int i = tid; i < npf; i += NPROD) {
                 const int iy = i / a.nxf, ix = i - iy * a.nxf;
                 float v = 0.f;
                 for (int tr = TR - 1; tr >= 0; --tr)                      // small cross terms first
@@ -390,7 +405,7 @@ __global__ void __launch_bounds__(TC_THREADS, NACC <= 40 ? 2 : 1) jam_quad_tc_ke
                 out[i] = v;
             }
         } else {
-            for (int i = tid; i < npf; i += TC_PRODUCERS) out[i] = 0.f;
+            for (int i = tid; i < npf; i += NPROD) out[i] = 0.f;
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -403,65 +418,73 @@ static int tc_terms() {
     const char* e = getenv("GLAD_JAM_TERMS");
     return (e && atoi(e) == 3) ? 3 : 2;
 }
+// producer warps per CTA: 16 by default, 24 with GLAD_JAM_WARPS=24
+static int tc_warps() {
+    const char* e = getenv("GLAD_JAM_WARPS");
+    return (e && atoi(e) == 24) ? 24 : 16;
+}
 
-static bool tc_geometry(const glad_ctx* c, JTArgs* a, int* nacc) {
-    const int NT = tc_terms();
+// launch plan for the current sky grid and table sizes; false = not supported (the FP32 kernel takes over)
+static bool tc_plan(const glad_ctx* c, int nl, int nmx, JTArgs* a, int* nacc, size_t* smem) {
+    const int NT = tc_terms(), PW = tc_warps();
     a->ny8 = (c->nyf + 7) & ~7;
     if (a->ny8 > 128) return false;
     a->multi = NT * a->ny8 > 128 ? 1 : 0;
     a->nxp = (NT == 3 || a->multi) ? ((c->nxf + 15) & ~15) : ((c->nxf + 7) & ~7);
     a->N = NT * a->nxp;
     if (a->N > 256) return false;
-    *nacc = a->N / 2 <= 40 ? 40 : (a->N / 2 <= 64 ? 64 : 128);
-    a->tmem_cols = *nacc == 128 ? 512 : 256;
-    return true;
+    const int per = (a->N + PW / 4 - 1) / (PW / 4);                      // accumulator columns per warp of a lane quarter
+    *nacc = PW == 16 ? (per <= 24 ? 24 : (per <= 40 ? 40 : 64)) : (per <= 16 ? 16 : (per <= 32 ? 32 : 48));
+    a->tmem_cols = 512;                                                  // one CTA per SM: two accumulator buffers of 256 columns
+    const size_t fixed = (((size_t)4 * nl + 4 * nmx + 2 * (size_t)nmx * nl + 2 * (size_t)c->nu + ((nl + 3) & ~3) +
+                           (size_t)(a->ny8 + a->nxp) + 31) & ~(size_t)31) * 4;
+    for (a->MC = 256, a->lgMC = 8; a->MC >= 64; a->MC >>= 1, --a->lgMC) {
+        size_t ops = 2 * (size_t)a->MC * NT * (a->ny8 + a->nxp) * 2 + 2048;   // two stages + the M = 128 over-read
+        const size_t scr = (size_t)128 * a->N * 4;                           // epilogue scratch reuses the stages
+        if (ops < scr) ops = scr;
+        *smem = fixed + (size_t)TC_COEF_SLOTS * 4 * a->MC * 4 + ops;
+        if (*smem <= 225 * 1024) return true;
+    }
+    return false;
 }
 
-bool jam_quad_tc_supported(const glad_ctx* c) { JTArgs a; int nacc; return tc_geometry(c, &a, &nacc); }
+bool jam_quad_tc_supported(const glad_ctx* c, int nl, int nmx) { JTArgs a; int nacc; size_t smem; return tc_plan(c, nl, nmx, &a, &nacc, &smem); }
 
-template <int NT, int NACC>
+template <int NT, int NACC, int PW>
 static cudaError_t tc_launch(const JTArgs& a, int grid, size_t smem, cudaStream_t st) {
     static size_t configured = 0;
     if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(jam_quad_tc_kernel<NT, NACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(jam_quad_tc_kernel<NT, NACC, PW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    jam_quad_tc_kernel<NT, NACC><<<grid, TC_THREADS, smem, st>>>(a);
+    jam_quad_tc_kernel<NT, NACC, PW><<<grid, PW * 32 + 32, smem, st>>>(a);
     return cudaGetLastError();
+}
+template <int NT>
+static cudaError_t tc_dispatch(const JTArgs& a, int nacc, int PW, int grid, size_t smem, cudaStream_t st) {
+    if (PW == 16) {
+        if (nacc == 24) return tc_launch<NT, 24, 16>(a, grid, smem, st);
+        if (nacc == 40) return tc_launch<NT, 40, 16>(a, grid, smem, st);
+        return tc_launch<NT, 64, 16>(a, grid, smem, st);
+    }
+    if (nacc == 16) return tc_launch<NT, 16, 24>(a, grid, smem, st);
+    if (nacc == 32) return tc_launch<NT, 32, 24>(a, grid, smem, st);
+    return tc_launch<NT, 48, 24>(a, grid, smem, st);
 }
 
 cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S) {
     JTArgs a;
     int nacc;
-    if (!tc_geometry(c, &a, &nacc)) return cudaErrorInvalidConfiguration;
-    const int NT = tc_terms();
+    size_t smem;
+    if (!tc_plan(c, nl, nmx, &a, &nacc, &smem)) return cudaErrorInvalidConfiguration;
     a.tab = c->d_jam_tab; a.tabsz = jam_table_floats(nl, nmx); a.nl = nl; a.nmx = nmx;
     a.un = c->d_un; a.uw = c->d_uw; a.nu = c->nu;
     a.xf2 = c->d_xf2; a.yf2 = c->d_yf2; a.nxf = c->nxf; a.nyf = c->nyf;
     a.S = S; a.partial = c->d_partial;
-    const size_t fixed = (((size_t)4 * nl + 4 * nmx + 2 * (size_t)nmx * nl + 2 * (size_t)c->nu + ((nl + 3) & ~3) +
-                           (size_t)(a.ny8 + a.nxp) + 31) & ~(size_t)31) * 4 + 3 * TC_COEF_ROWS * 16;
-    const size_t budget = nacc <= 40 ? 112 * 1024 : 220 * 1024;          // two CTAs per SM when the map is small
-    size_t smem = 0;
-    for (a.MC = 128, a.lgMC = 7; a.MC >= 64; a.MC >>= 1, --a.lgMC) {
-        size_t ops = 2 * (size_t)a.MC * NT * (a.ny8 + a.nxp) * 2 + 2048 + 3 * TC_PRODUCERS * 4;  // two stages + the M = 128 over-read + row state
-        const size_t scr = (size_t)128 * a.N * 4;                        // epilogue scratch reuses the stages
-        if (ops < scr) ops = scr;
-        smem = fixed + ops;
-        if (smem <= budget || a.MC == 64) break;
-    }
-    if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
     a.FL = 512 / a.MC;
     if (const char* e = getenv("GLAD_JAM_FLUSH")) { int v = atoi(e); if (v >= 1) a.FL = v; }
     ProfScope ps(c, GK_JAM_QUAD);
-    const int grid = B * S;
-    if (NT == 2) {
-        if (nacc == 40) return tc_launch<2, 40>(a, grid, smem, c->stream);
-        if (nacc == 64) return tc_launch<2, 64>(a, grid, smem, c->stream);
-        return tc_launch<2, 128>(a, grid, smem, c->stream);
-    }
-    if (nacc == 40) return tc_launch<3, 40>(a, grid, smem, c->stream);
-    if (nacc == 64) return tc_launch<3, 64>(a, grid, smem, c->stream);
-    return tc_launch<3, 128>(a, grid, smem, c->stream);
+    return tc_terms() == 3 ? tc_dispatch<3>(a, nacc, tc_warps(), B * S, smem, c->stream)
+                           : tc_dispatch<2>(a, nacc, tc_warps(), B * S, smem, c->stream);
 }
