@@ -37,7 +37,6 @@
 #include "glad_internal.h"
 
 #define LOG2E_F 1.4426950408889634f
-#define TC_COEF_SLOTS 4
 
 struct JTArgs {
     const float* tab; int tabsz; int nl; int nmx;
@@ -48,6 +47,7 @@ struct JTArgs {
     int N;               // accumulator columns = NT * nxp
     int MC, lgMC;        // contraction rows per stage (128 or 256)
     int FL;              // chunks per accumulator group (>= 1)
+    int cslots;          // coefficient ring slots (power of two >= NPROD/MC + 3)
     int tmem_cols;       // power of two >= 2 * N
     int S;
     float* partial;
@@ -154,9 +154,9 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
     float2* s_uw = s_jk + nmx * nl;
     float* s_ld = reinterpret_cast<float*>(s_uw + nu);
     float* s_c2 = s_ld + ((nl + 3) & ~3);            // ny8 + nxp squared coordinates, y first
-    // coefficient ring: TC_COEF_SLOTS chunks, per chunk [-Q log2e | -P log2e | F0 | F1] x MC floats
+    // coefficient ring: a.cslots chunks, per chunk [-Q log2e | -P log2e | F0 | F1] x MC floats
     float* s_coef = sm + ((4 * nl + 4 * nmx + 2 * nmx * nl + 2 * nu + ((nl + 3) & ~3) + ny8 + nxp + 31) & ~31);
-    uint4* s_ops = reinterpret_cast<uint4*>(s_coef + TC_COEF_SLOTS * 4 * MC);   // 2 stages + tail pad, 128-byte aligned
+    uint4* s_ops = reinterpret_cast<uint4*>(s_coef + a.cslots * 4 * MC);   // 2 stages + tail pad, 128-byte aligned
 
     for (int k = tid; k < nl; k += NTHR) {
         s_lk[k] = make_float4(TLg[JL_INVS2 * nl + k], TLg[JL_BKQ * nl + k], TLg[JL_S0 * nl + k], TLg[JL_NKS * nl + k]);
@@ -245,10 +245,13 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
         const float inv_pairs = 1.f / (float)pairs, inv_nl = 1.f / (float)nl;
 
         // Coefficients of contraction row m = (iu, j, k), k fastest: (-Q log2e, -P log2e, F0, F1); rows past the end have
-        // F0 = F1 = 0 and contribute 0.  Chunk `rc` (relative to c0) lives in ring slot rc % 4.  It is written during
-        // iteration rc-2 and read during iteration rc: the reader has passed the "empty" wait of chunk rc-2, so every
-        // producer has arrived on "full" of rc-2, i.e. finished writing; the slot's previous tenant rc-4 was last read
-        // in iteration rc-4, which every producer had finished before the writer passed the "empty" wait of rc-4.
+        // F0 = F1 = 0 and contribute 0.  Chunk `rc` (relative to c0) lives in ring slot rc % cslots.  Every R-th
+        // iteration (R = NPROD / MC) ALL producer threads write one row each of chunks it+2 .. it+R+1, so the warps stay
+        // in step (a group taking turns would skew them by one coefficient block per chunk, and with two operand
+        // stages any skew ends in the "empty" wait).  A chunk is therefore written at iteration <= rc-2 and read during
+        // iteration rc: the reader has passed the "empty" wait of chunk rc-2, so every producer has arrived on "full"
+        // of rc-2, i.e. finished writing.  While a thread writes in iteration `it` the slowest warp can still be
+        // reading chunk it-1 (the writer passed the "empty" wait of it-2): slots it-1 .. it+R+1 are live, cslots >= R+3.
         auto coef_row = [&](int rc, int r) {
             const int m = (c0 + rc) * MC + r;
             float cq = 0.f, cp = 0.f, f0 = 0.f, f1 = 0.f;
@@ -275,7 +278,7 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
                 f0 = pref * lk.z;
                 f1 = pref * lk.w * D;
             }
-            float* dst = s_coef + (rc & (TC_COEF_SLOTS - 1)) * (4 * MC) + r;
+            float* dst = s_coef + (rc & (a.cslots - 1)) * (4 * MC) + r;
             dst[0] = cq; dst[MC] = cp; dst[2 * MC] = f0; dst[3 * MC] = f1;
         };
         const int R = NPROD / MC;                                       // producer thread groups of MC threads
@@ -284,20 +287,24 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
         // Quarter-warp = one oct of the chunk (8 contraction rows), lane l8 = pixel within an 8-pixel block.  The
         // thread loads the 8 rows' coefficients once (LDS.128 delivers 512 B per warp whatever the broadcast) and
         // reuses them over its blocks.  The oct's block list [Y blocks | X blocks] is cut into NQ contiguous ranges
-        // of about equal cost (a Y block ~3, an X block ~5); a warp holds one range index and four octs.
+        // of about equal cost (profiles/r1c.md: a Y block is 51 issue slots, an X block 53); a warp holds one range
+        // index ("role") and four octs.  Roles alternate every four warps so that each of the SM's four schedulers
+        // (warp % 4) sees every role: the ranges are never exactly equal.
         const int qw = tid >> 3, l8 = tid & 7;
-        const int NQ = (NPROD >> 3) / (MC >> 3);                        // quarter-warps per oct: 2, 3, 4 or 6
-        const int role = warp % NQ, oct = (qw & 3) + 4 * (warp / NQ);
+        const int NQ = (NPROD >> 3) / (MC >> 3);                        // quarter-warps per oct: 2, 4 or 8
+        const bool mix = (PW % (4 * NQ)) == 0;
+        const int role = mix ? (warp >> 2) % NQ : warp % NQ;
+        const int oct = (qw & 3) + 4 * (mix ? (warp & 3) + 4 * (warp / (4 * NQ)) : warp / NQ);
         int yb0, yb1, xb0, xb1;
         {
-            const int ctot = 3 * nyb + 5 * nxb;
+            const int ctot = 20 * nyb + 21 * nxb;
             int bnd[2];
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 const int target = ((role + e) * ctot * 2 + NQ) / (2 * NQ);          // round(role * ctot / NQ)
                 int best = 0, bestd = target, pre = 0;
                 for (int i = 1; i <= nyb + nxb; ++i) {
-                    pre += i <= nyb ? 3 : 5;
+                    pre += i <= nyb ? 20 : 21;
                     const int dd = pre > target ? pre - target : target - pre;
                     if (dd < bestd) { bestd = dd; best = i; }
                 }
@@ -307,7 +314,7 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
             xb0 = max(bnd[0], nyb) - nyb; xb1 = max(bnd[1], nyb) - nyb;
         }
         auto produce = [&](int it, int buf) {
-            const float* cb = s_coef + (it & (TC_COEF_SLOTS - 1)) * (4 * MC) + 8 * oct;
+            const float* cb = s_coef + (it & (a.cslots - 1)) * (4 * MC) + 8 * oct;
             uint4* stA = s_ops + buf * stage16 + oct * GA * 8 + l8;
             uint4* stB = s_ops + buf * stage16 + a16 + oct * GB * 8 + l8;
             if (yb0 < yb1) {
@@ -374,7 +381,7 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 while ((gf + 1) * a.FL - 1 <= it - 2) flush(gf++);
             }
-            if (cgrp == cphase && it + 2 < nch) coef_row(it + 2, crow); // one thread group in turn prepares chunk it+2
+            if (cphase == 0 && it + 2 + cgrp < nch) coef_row(it + 2 + cgrp, crow);   // chunks it+2 .. it+R+1, one row per thread
             cphase = cphase + 1 == R ? 0 : cphase + 1;
             produce(it, buf);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -442,7 +449,8 @@ static bool tc_plan(const glad_ctx* c, int nl, int nmx, JTArgs* a, int* nacc, si
         size_t ops = 2 * (size_t)a->MC * NT * (a->ny8 + a->nxp) * 2 + 2048;   // two stages + the M = 128 over-read
         const size_t scr = (size_t)128 * a->N * 4;                           // epilogue scratch reuses the stages
         if (ops < scr) ops = scr;
-        *smem = fixed + (size_t)TC_COEF_SLOTS * 4 * a->MC * 4 + ops;
+        a->cslots = (PW * 32 / a->MC) <= 4 ? 8 : 16;
+        *smem = fixed + (size_t)a->cslots * 4 * a->MC * 4 + ops;
         if (*smem <= 225 * 1024) return true;
     }
     return false;
