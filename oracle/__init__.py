@@ -69,6 +69,12 @@ def lib():
         L.glad_oracle_joint.argtypes = [dp, dp, i, dp]
         L.glad_oracle_bh_theta2.restype = d
         L.glad_oracle_bh_theta2.argtypes = [d, d, d]
+        L.glad_oracle_mge_f_sigma.restype = d
+        L.glad_oracle_mge_f_sigma.argtypes = [i, dp, d, i]
+        L.glad_oracle_mge1d.restype = i
+        L.glad_oracle_mge1d.argtypes = [i, dp, i, d, d, i, dp]
+        L.glad_oracle_sigma_crit.restype = d
+        L.glad_oracle_sigma_crit.argtypes = [d, d, d]
         _lib = L
     return _lib
 
@@ -194,3 +200,58 @@ def joint_loglike(chi2_lens, chi2_dyn):
     out = np.empty_like(a)
     lib().glad_oracle_joint(_ptr(a, C.c_double), _ptr(b, C.c_double), a.size, _ptr(out, C.c_double))
     return out
+
+
+# ---- 1-D MGE of a radial profile (Eq. 44-46) ----
+PROFILE_SERSIC, PROFILE_EPL = 0, 1
+MGE_EULER_P = 12          # reading R-M1 (the paper does not print P)
+
+
+def mge_f_sigma(kind, prof, sigma, P=MGE_EULER_P) -> float:
+    """Eq. 45 at one sigma.  prof = [I_e, R_e, n, q'] (Sersic) or [scale, theta_E, gamma, q] (EPL)."""
+    pr = np.ascontiguousarray(prof, dtype=np.float64)
+    assert pr.size == 4
+    return float(lib().glad_oracle_mge_f_sigma(int(kind), _ptr(pr, C.c_double), float(sigma), int(P)))
+
+
+def mge1d(kind, prof, n_gauss, sigma_lo, sigma_hi, P=MGE_EULER_P):
+    """Eq. 46: rows {A_n, sigma_n, q'} [n_gauss,3] (fp64) of one profile."""
+    pr = np.ascontiguousarray(prof, dtype=np.float64)
+    assert pr.size == 4
+    out = np.empty((int(n_gauss), 3), np.float64)
+    rc = lib().glad_oracle_mge1d(int(kind), _ptr(pr, C.c_double), int(n_gauss), float(sigma_lo), float(sigma_hi),
+                                 int(P), _ptr(out, C.c_double))
+    if rc != 0:
+        raise ValueError("oracle: bad mge1d arguments")
+    return out
+
+
+def mge1d_batch(kind, prof, n_gauss, sigma_lo, sigma_hi, P=MGE_EULER_P):
+    """prof [B,4] float32 (the array the CUDA path reads) -> [B,n_gauss,3] fp64."""
+    prof = _f32(prof).reshape(-1, 4)
+    return np.stack([mge1d(kind, prof[b].astype(np.float64), n_gauss, sigma_lo, sigma_hi, P) for b in range(prof.shape[0])])
+
+
+def sigma_crit(Ddt_mpc, Dd_mpc, zd) -> float:
+    return float(lib().glad_oracle_sigma_crit(float(Ddt_mpc), float(Dd_mpc), float(zd)))
+
+
+def model_tables(lens, dyn, ddt, zd, n_lum, n_mass, lum_range, mass_range, P=MGE_EULER_P):
+    """The self-consistent joint model of P:406 / Fig. 2 (reading R-M3): from the lens vector and the distances
+    derive (a) the luminous MGE = Eq. 46 of lens-light Sersic #1 (lens[16:20]), (b) the mass MGE = Eq. 46 of
+    Sigma_crit * kappa_epl (Eq. 13, B.1-B.3), (c) lens[8] = theta_E,BH^2 from M_BH = dyn[2] (Eq. 4).
+    Returns (lens' [B,26] float32, lum [B,n_lum,3] float32, mass [B,n_mass,3] float32): tables rounded to the
+    float32 the batch calls take."""
+    lens = _f32(lens).reshape(-1, NLENS).copy()
+    dyn = _f32(dyn).reshape(-1, NDYN)
+    ddt = _f32(ddt).reshape(-1)
+    B = lens.shape[0]
+    lum = np.empty((B, n_lum, 3), np.float32)
+    mass = np.empty((B, n_mass, 3), np.float32)
+    for b in range(B):
+        Ie, Re, n, q = (float(v) for v in lens[b, 16:20])
+        lum[b] = mge1d(PROFILE_SERSIC, [Ie, Re, n, q], n_lum, *lum_range, P=P)
+        sc = sigma_crit(float(ddt[b]), float(dyn[b, 1]), zd)
+        mass[b] = mge1d(PROFILE_EPL, [sc, float(lens[b, 2]), float(lens[b, 3]), float(lens[b, 4])], n_mass, *mass_range, P=P)
+        lens[b, 8] = bh_theta2(float(dyn[b, 2]), float(ddt[b]), zd)
+    return lens, lum, mass

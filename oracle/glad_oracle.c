@@ -28,6 +28,8 @@
  *                           inclination independence, evenness, linearity
  *   PSF / bins (kin) ...... constant-field invariance, delta kernel
  *   joint ................. additivity, -inf propagation
+ *   1-D MGE (8(f) rank 1) . power-law closed form, Gaussian profile, profiles
+ *                           summed back to the paper's ~0.5 %, linearity
  * Overall numbers: PARITY UNPINNED against any published value -- the paper
  * prints no model image, v_rms map or likelihood value for any parameter
  * vector.
@@ -485,4 +487,91 @@ double glad_oracle_bh_theta2(double Mbh_msun, double Ddt_mpc, double zd) {
     double rad2 = 4.0 * G_NEWTON * Mbh_msun * (1.0 + zd) / (c_kms * c_kms * Ddt_mpc * 1e6);
     double arcsec_per_rad = 648000.0 / PI;
     return rad2 * arcsec_per_rad * arcsec_per_rad;
+}
+
+/* ------------------------------------------------------------------------ */
+/* 1-D multi-Gaussian expansion of a radial profile    */
+/* (Eq. 44-46, "following Shajib (2019)"), the step between the    */
+/* two halves of the joint model ("we decompose I_light and Sigma_int  */
+/* into multiple Gaussian components").                                       */
+/*                                                                            */
+/*   Eq. 44   f(sigma) = 1/(i sigma^2) sqrt(2/pi) int_C z F(z) e^{z^2/2s^2} dz */
+/*   Eq. 45   f(sigma) ~ sum_{n=0}^{2P} eta_n Re F(sigma chi_n)                */
+/*   Eq. 46   F(R) ~ sum_n A_n exp(-R^2 / 2 sigma_n^2)  (the printed exponent  */
+/*            lost its minus sign), A_n = w_n f(sigma_n) dln(sigma)/sqrt(2pi), */
+/*            sigma_n log-spaced, R = sqrt(x^2 + y^2/q^2) (footnote P:234)     */
+/* The paper says eta_n, chi_n "can be precomputed" and prints neither; they   */
+/* are the Euler-algorithm constants of the cited method (reading    */
+/* R-M1):  chi_n = sqrt(2 P ln10 / 3 + 2 pi i n),                              */
+/*         eta_n = (-1)^n 2 sqrt(2 pi) 10^{P/3} xi_n,  xi_0 = 1/2,             */
+/*         xi_n = 1 (1 <= n <= P), xi_2P = 2^-P,                               */
+/*         xi_{2P-n} = xi_{2P-n+1} + 2^-P binom(P, n)  (0 < n < P).            */
+/* w_n ("fixed weighting factors") = trapezoid weights in ln(sigma): 1/2 at    */
+/* both ends, 1 inside (R-M2).                                                 */
+/* Profiles F(z), z complex, principal branches:                              */
+/*   kind 0, Sersic (R-L7):  prof = {I_e, R_e, n, q'}                          */
+/*           F = I_e exp(-b_n ((z/R_e)^{1/n} - 1))                             */
+/*   kind 1, EPL convergence (Eq. B.1-B.3, r_soft = 0 as in R-L3):             */
+/*           prof = {scale, theta_E, gamma, q},  F = scale (3-gamma)/2 (b/z)^{gamma-1} */
+/* Output rows {A_n, sigma_n, q'}.  Returns 0, or -1 on bad arguments.         */
+/* Pins (tests/test_oracle_mge.py): the power law has the closed form          */
+/*   f(sigma) = sqrt(2pi) 2^{1-t/2}/Gamma(t/2) sigma^-t; F = Gaussian of width */
+/*   s gives an expansion concentrated at sigma = s; the expansion summed back */
+/*   reproduces Sersic and power-law profiles to the accuracy the paper prints */
+/*   (~0.5 % with 21 Gaussians); amplitudes linear in the profile       */
+/*   scale; sigma_n geometric.                                                 */
+/* ------------------------------------------------------------------------ */
+static double binom_d(int n, int k) {
+    double r = 1.0;
+    for (int i = 1; i <= k; ++i) r = r * (double)(n - k + i) / (double)i;
+    return r;
+}
+
+static double complex mge_profile(int kind, const double* prof, double bn, double complex z) {
+    if (kind == 0) {
+        double complex w = cpow(z / prof[1], 1.0 / prof[2]);
+        return prof[0] * cexp(-bn * (w - 1.0));
+    }
+    double t = prof[2] - 1.0;
+    double b = pow(2.0 / (1.0 + prof[3]), 1.0 / t) * prof[1];        /* Eq. B.3 */
+    return prof[0] * 0.5 * (3.0 - prof[2]) * cpow(b / z, t);          /* Eq. B.1 */
+}
+
+/* Eq. 45 at one sigma */
+double glad_oracle_mge_f_sigma(int kind, const double* prof, double sigma, int P) {
+    if (P < 1 || P > 20) return NAN;
+    double xi[41];
+    xi[0] = 0.5;
+    for (int n = 1; n <= P; ++n) xi[n] = 1.0;
+    xi[2 * P] = ldexp(1.0, -P);
+    for (int n = 1; n < P; ++n) xi[2 * P - n] = xi[2 * P - n + 1] + ldexp(1.0, -P) * binom_d(P, n);
+    double bn = kind == 0 ? glad_oracle_sersic_bn(prof[2]) : 0.0;
+    double sum = 0.0;
+    for (int n = 0; n <= 2 * P; ++n) {
+        double complex chi = csqrt(2.0 * P * log(10.0) / 3.0 + 2.0 * PI * n * I);
+        double eta = ((n & 1) ? -1.0 : 1.0) * 2.0 * sqrt(2.0 * PI) * pow(10.0, P / 3.0) * xi[n];
+        sum += eta * creal(mge_profile(kind, prof, bn, sigma * chi));
+    }
+    return sum;
+}
+
+int glad_oracle_mge1d(int kind, const double* prof, int n_gauss, double sigma_lo, double sigma_hi, int P,
+                      double* mge /* [n_gauss,3] */) {
+    if ((kind != 0 && kind != 1) || n_gauss < 2 || !(sigma_lo > 0.0) || !(sigma_hi > sigma_lo) || P < 1 || P > 20)
+        return -1;
+    double dln = log(sigma_hi / sigma_lo) / (n_gauss - 1);
+    for (int n = 0; n < n_gauss; ++n) {
+        double sigma = sigma_lo * exp(dln * n);
+        double w = (n == 0 || n == n_gauss - 1) ? 0.5 : 1.0;
+        mge[3 * n + 0] = w * glad_oracle_mge_f_sigma(kind, prof, sigma, P) * dln / sqrt(2.0 * PI);   /* Eq. 46 */
+        mge[3 * n + 1] = sigma;
+        mge[3 * n + 2] = prof[3];
+    }
+    return 0;
+}
+
+/* Eq. 13: Sigma_crit = c^2/(4 pi G) D_dt / ((1+z_d) D_d^2), in Msun/pc^2 for distances in Mpc. */
+double glad_oracle_sigma_crit(double Ddt_mpc, double Dd_mpc, double zd) {
+    const double c_kms = 299792.458;
+    return c_kms * c_kms / (4.0 * PI * G_NEWTON) * (Ddt_mpc * 1e6) / ((1.0 + zd) * (Dd_mpc * 1e6) * (Dd_mpc * 1e6));
 }
