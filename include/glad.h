@@ -172,6 +172,43 @@ glad_status glad_joint_loglike_host(glad_ctx* ctx, const float* h_lens_params, c
                                     int n_mass, long mass_stride, const float* h_beta, int beta_per_gaussian,
                                     float* h_loglike, float* h_chi2_lens, float* h_chi2_dyn, int32_t* h_flags);
 
+/*
+ * the step between the two halves (Fig. 2: "we decompose I_light and Sigma_int into
+ * multiple Gaussian components").  1-D multi-Gaussian expansion of a radial profile F(R), R = sqrt(x^2 + y^2/q'^2)
+ * (footnote P:234), by the integral transform of Eq. 44 evaluated with the Euler sum of Eq. 45 of
+ * order P (2P+1 complex profile evaluations per Gaussian; P in [1,15], 0 = default 12; DESIGN.md R-M1 states the
+ * constants eta_n, chi_n the paper leaves out) on n_gauss >= 2 log-spaced sigma_n in [sigma_lo, sigma_hi]:
+ *   A_n = w_n f(sigma_n) dln(sigma) / sqrt(2 pi)   (Eq. 46; w = 1/2 at both ends, 1 inside, R-M2).
+ * d_prof [B,GLAD_NPROF] float, one row per vector:
+ *   GLAD_PROFILE_SERSIC : {I_e, R_e, n, q'}            F = I_e exp(-b_n ((R/R_e)^(1/n) - 1))        (R-L7)
+ *   GLAD_PROFILE_EPL    : {scale, theta_E, gamma, q}   F = scale (3-gamma)/2 (b/R)^(gamma-1), b of Eq. B.3
+ * d_mge [B,n_gauss,3] rows {A_n, sigma_n, q'}: the MGE row layout glad_jam_vrms_batch reads (stride 3*n_gauss).
+ * fp64 arithmetic, fp32 rows.  Enqueues on the context stream; device pointers owned by the caller.
+ * GLAD_EINVAL on a bad kind / range / order, GLAD_ESHAPE if n_gauss > GLAD_MAX_GAUSS.
+ */
+typedef enum { GLAD_PROFILE_SERSIC = 0, GLAD_PROFILE_EPL = 1 } glad_profile_kind;
+#define GLAD_NPROF 4
+glad_status glad_mge1d_batch(glad_ctx* ctx, int kind, const float* d_prof, int B, int n_gauss, float sigma_lo,
+                             float sigma_hi, int euler_order, float* d_mge);
+
+/*
+ * Self-consistent joint model (R-M3; Fig. 2): ONE sampler vector per evaluation.  On the device, per vector:
+ *   luminous MGE = Eq. 46 of the lens-light Sersic #1 (lens[16..19] = I_e, R_e, n, q), n_lum Gaussians on
+ *                  [lum_sigma_lo, lum_sigma_hi];
+ *   mass MGE     = Eq. 46 of Sigma_crit * kappa_epl(theta_E, gamma, q) with Sigma_crit(D_dt, D_d, z_d) of Eq. 13
+ *                  (D_d = dyn[1]), n_mass Gaussians on [mass_sigma_lo, mass_sigma_hi] (the paper goes to 50");
+ *   lens[8]      = theta_E,BH^2 of M_BH = dyn[2] and D_dt (Eq. 4); the caller's lens[8] is ignored;
+ * then exactly glad_joint_loglike_batch with these per-vector tables (Upsilon = dyn[3] still multiplies the mass MGE).
+ *   d_ddt [B] time-delay distances in Mpc; z_d lens redshift; other arguments as glad_joint_loglike_batch.
+ *   d_lum_mge_out [B,n_lum,3] / d_mass_mge_out [B,n_mass,3]: the derived tables, or NULL.
+ */
+glad_status glad_joint_loglike_model_batch(glad_ctx* ctx, const float* d_lens_params, const float* d_dyn_params,
+                                           const float* d_ddt, float z_d, int B, int n_lum, float lum_sigma_lo,
+                                           float lum_sigma_hi, int n_mass, float mass_sigma_lo, float mass_sigma_hi,
+                                           const float* d_beta, int beta_per_gaussian, float* d_loglike,
+                                           float* d_chi2_lens, float* d_chi2_dyn, int32_t* d_flags,
+                                           float* d_lum_mge_out, float* d_mass_mge_out);
+
 /* Host helper: theta_E,BH^2 [arcsec^2] = 4 G M_BH (1+z_d) / (c^2 D_dt) (from Eq. 4), so that the
  * caller keeps lens[8] consistent with dyn[2] and the sampled D_dt.  Pure host arithmetic. */
 double glad_bh_theta2(double mbh_msun, double ddt_mpc, double z_d);
@@ -180,9 +217,9 @@ double glad_bh_theta2(double mbh_msun, double ddt_mpc, double z_d);
  * Optional per-kernel timing for bench.py's roofline line: when enabled, a CUDA event pair is recorded on the
  * context stream around every kernel launch (at most 2048 launches between reads).  glad_profile_read
  * SYNCHRONISES the stream, adds the elapsed times to per-kernel totals, copies them out and clears them.
- * Kernel order: 0 lens_prep, 1 lens_image, 2 jam_prep, 3 jam_quad, 4 jam_post, 5 joint.
+ * Kernel order: 0 lens_prep, 1 lens_image, 2 jam_prep, 3 jam_quad, 4 jam_post, 5 joint, 6 mge (model_prep + mge1d).
  */
-#define GLAD_NKERNELS 6
+#define GLAD_NKERNELS 7
 glad_status glad_profile_enable(glad_ctx* ctx, int on);
 glad_status glad_profile_read(glad_ctx* ctx, double* ms_out /*[GLAD_NKERNELS]*/, long* count_out /*[GLAD_NKERNELS]*/);
 

@@ -12,14 +12,15 @@ import torch
 
 from .build import LIB, build
 
-NLENS, NDYN = 26, 4
+NLENS, NDYN, NPROF = 26, 4, 4
+PROFILE_SERSIC, PROFILE_EPL = 0, 1
 FLAG_LENS_INVALID, FLAG_DYN_INVALID, FLAG_BIN_INVALID = 1, 2, 4
 
 _lib = None
 EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "glad_set_image_data",
            "glad_set_kin_data", "glad_lens_image_batch", "glad_jam_vrms_batch", "glad_joint_loglike_batch",
            "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count", "glad_profile_enable",
-           "glad_profile_read"]
+           "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch"]
 
 
 class GladError(RuntimeError):
@@ -71,6 +72,11 @@ def load(rebuild: bool = False):
     L.glad_profile_enable.argtypes = [vp, i]
     L.glad_profile_read.restype = i
     L.glad_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_long)]
+    L.glad_mge1d_batch.restype = i
+    L.glad_mge1d_batch.argtypes = [vp, i, vp, i, i, C.c_float, C.c_float, i, vp]
+    L.glad_joint_loglike_model_batch.restype = i
+    L.glad_joint_loglike_model_batch.argtypes = [vp, vp, vp, vp, C.c_float, i, i, C.c_float, C.c_float, i, C.c_float,
+                                                 C.c_float, vp, i, vp, vp, vp, vp, vp, vp]
     L.glad_launch_count.restype = l
     L.glad_launch_count.argtypes = [vp]
     _lib = L
@@ -132,15 +138,15 @@ class Glad:
     def launch_count(self) -> int:
         return int(self.lib.glad_launch_count(self.ctx))
 
-    KERNELS = ("lens_prep", "lens_image", "jam_prep", "jam_quad", "jam_post", "joint")
+    KERNELS = ("lens_prep", "lens_image", "jam_prep", "jam_quad", "jam_post", "joint", "mge")
 
     def profile_enable(self, on: bool = True):
         self._check(self.lib.glad_profile_enable(self.ctx, 1 if on else 0))
 
     def profile_read(self) -> dict:
         """{kernel: (total ms, launches)} since the last read (synchronises the stream)."""
-        ms = (C.c_double * 6)()
-        cnt = (C.c_long * 6)()
+        ms = (C.c_double * len(self.KERNELS))()
+        cnt = (C.c_long * len(self.KERNELS))()
         self._check(self.lib.glad_profile_read(self.ctx, ms, cnt))
         return {k: (ms[i], cnt[i]) for i, k in enumerate(self.KERNELS)}
 
@@ -227,3 +233,32 @@ class Glad:
                                                      _p(mass_mge) if nm else None, nm, ms, _p(beta), 1 if beta.dim() == 2 else 0,
                                                      _p(loglike_out), None, None, None))
         return loglike_out
+
+    # ---- on-device 1-D MGE and the self-consistent joint model ----------------
+    def mge1d_batch(self, kind, prof, n_gauss, sigma_lo, sigma_hi, euler_order=0):
+        pr = _dev(prof, torch.float32, self.device).reshape(-1, NPROF)
+        B = pr.shape[0]
+        mge = torch.empty((B, int(n_gauss), 3), dtype=torch.float32, device=self.device)
+        self._check(self.lib.glad_mge1d_batch(self.ctx, int(kind), _p(pr), B, int(n_gauss), float(sigma_lo), float(sigma_hi),
+                                              int(euler_order), _p(mge)))
+        return mge
+
+    def joint_loglike_model_batch(self, lens_params, dyn_params, ddt, z_d, n_lum, lum_range, n_mass, mass_range, beta,
+                                  want_tables=False, out=None):
+        p = _dev(lens_params, torch.float32, self.device).reshape(-1, NLENS)
+        d = _dev(dyn_params, torch.float32, self.device).reshape(-1, NDYN)
+        dt = _dev(ddt, torch.float32, self.device).reshape(-1)
+        bt = _dev(beta, torch.float32, self.device)
+        B = p.shape[0]
+        if d.shape[0] != B or dt.shape[0] != B:
+            raise GladError("lens, dyn and ddt batches differ")
+        out = out or {}
+        mk = lambda n, ty: out.get(n) if out.get(n) is not None else torch.empty(B, dtype=ty, device=self.device)
+        ll, c2l, c2d, fl = mk("loglike", torch.float32), mk("chi2_lens", torch.float32), mk("chi2_dyn", torch.float32), mk("flags", torch.int32)
+        lum = torch.empty((B, int(n_lum), 3), dtype=torch.float32, device=self.device) if want_tables else None
+        mass = torch.empty((B, int(n_mass), 3), dtype=torch.float32, device=self.device) if want_tables else None
+        self._check(self.lib.glad_joint_loglike_model_batch(
+            self.ctx, _p(p), _p(d), _p(dt), float(z_d), B, int(n_lum), float(lum_range[0]), float(lum_range[1]), int(n_mass),
+            float(mass_range[0]), float(mass_range[1]), _p(bt), 1 if bt.dim() == 2 else 0, _p(ll), _p(c2l), _p(c2d), _p(fl),
+            _p(lum), _p(mass)))
+        return {"loglike": ll, "chi2_lens": c2l, "chi2_dyn": c2d, "flags": fl, "lum_mge": lum, "mass_mge": mass}

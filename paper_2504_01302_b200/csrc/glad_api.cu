@@ -84,7 +84,7 @@ void glad_destroy(glad_ctx* c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     free_kin(c);
-    void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage};
+    void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage, c->d_model};
     for (void* p : ps) if (p) cudaFree(p);
     for (cudaEvent_t e : c->prof_ev) if (e) cudaEventDestroy(e);
     delete c;
@@ -359,6 +359,58 @@ glad_status glad_joint_loglike_host(glad_ctx* c, const float* h_lens, const floa
     if (h_flags) CU(cudaMemcpyAsync(h_flags, d_fl, sizeof(int32_t) * B, cudaMemcpyDeviceToHost, s), "D2H flags");
     CU(cudaStreamSynchronize(s), "joint (host) sync");
     return GLAD_OK;
+}
+
+static glad_status mge_check(glad_ctx* c, const char* who, int n, float lo, float hi) {
+    if (n < 2 || !(lo > 0.f) || !(hi > lo)) return fail(c, GLAD_EINVAL, "%s: n_gauss %d on [%g, %g]", who, n, lo, hi);
+    if (n > GLAD_MAX_GAUSS) return fail(c, GLAD_ESHAPE, "%s: more than GLAD_MAX_GAUSS Gaussians", who);
+    return GLAD_OK;
+}
+#define MGE_DEFAULT_ORDER 12
+
+glad_status glad_mge1d_batch(glad_ctx* c, int kind, const float* d_prof, int B, int n_gauss, float sigma_lo, float sigma_hi,
+                             int P, float* d_mge) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && (!d_prof || !d_mge))) return fail(c, GLAD_EINVAL, "glad_mge1d_batch: B=%d / null pointer", B);
+    if (kind != GLAD_PROFILE_SERSIC && kind != GLAD_PROFILE_EPL) return fail(c, GLAD_EINVAL, "glad_mge1d_batch: profile kind %d", kind);
+    if (P == 0) P = MGE_DEFAULT_ORDER;
+    if (P < 1 || P > 15) return fail(c, GLAD_EINVAL, "glad_mge1d_batch: Euler order %d outside [1,15]", P);
+    glad_status st = mge_check(c, "glad_mge1d_batch", n_gauss, sigma_lo, sigma_hi);
+    if (st != GLAD_OK) return st;
+    if (B == 0) return GLAD_OK;
+    cudaSetDevice(c->device);
+    CU(launch_mge1d(c, kind, d_prof, B, n_gauss, sigma_lo, sigma_hi, P, d_mge), "mge1d_kernel");
+    return GLAD_OK;
+}
+
+glad_status glad_joint_loglike_model_batch(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, float zd,
+                                           int B, int nl, float lum_lo, float lum_hi, int nm, float mass_lo, float mass_hi,
+                                           const float* d_beta, int per_gaussian, float* d_loglike, float* d_chi2_lens,
+                                           float* d_chi2_dyn, int32_t* d_flags, float* d_lum_out, float* d_mass_out) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && (!d_lens || !d_dyn || !d_ddt || !d_beta || !d_loglike)))
+        return fail(c, GLAD_EINVAL, "glad_joint_loglike_model_batch: B=%d / null pointer", B);
+    if (!(zd > -1.f)) return fail(c, GLAD_EINVAL, "glad_joint_loglike_model_batch: z_d = %g", zd);
+    glad_status st = mge_check(c, "glad_joint_loglike_model_batch (luminous)", nl, lum_lo, lum_hi);
+    if (st != GLAD_OK) return st;
+    st = mge_check(c, "glad_joint_loglike_model_batch (mass)", nm, mass_lo, mass_hi);
+    if (st != GLAD_OK) return st;
+    if (B == 0) return GLAD_OK;
+    cudaSetDevice(c->device);
+    const size_t n_lens = (size_t)B * GLAD_NLENS, n_prof = (size_t)B * GLAD_NPROF;
+    const size_t n_lum = (size_t)B * nl * 3, n_mass = (size_t)B * nm * 3;
+    st = grow(c, &c->d_model, &c->model_cap, n_lens + 2 * n_prof + n_lum + n_mass);
+    if (st != GLAD_OK) return st;
+    float* m_lens = c->d_model;
+    float* m_pl = m_lens + n_lens;
+    float* m_pm = m_pl + n_prof;
+    float* m_lum = d_lum_out ? d_lum_out : m_pm + n_prof;
+    float* m_mass = d_mass_out ? d_mass_out : m_pm + n_prof + n_lum;
+    CU(launch_model_prep(c, d_lens, d_dyn, d_ddt, (double)zd, B, m_lens, m_pl, m_pm), "model_prep_kernel");
+    CU(launch_mge1d(c, GLAD_PROFILE_SERSIC, m_pl, B, nl, lum_lo, lum_hi, MGE_DEFAULT_ORDER, m_lum), "mge1d_kernel");
+    CU(launch_mge1d(c, GLAD_PROFILE_EPL, m_pm, B, nm, mass_lo, mass_hi, MGE_DEFAULT_ORDER, m_mass), "mge1d_kernel");
+    return glad_joint_loglike_batch(c, m_lens, d_dyn, B, m_lum, nl, 3L * nl, m_mass, nm, 3L * nm, d_beta, per_gaussian,
+                                    d_loglike, d_chi2_lens, d_chi2_dyn, d_flags);
 }
 
 }  // extern "C"

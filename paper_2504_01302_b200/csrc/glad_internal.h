@@ -45,7 +45,7 @@ static inline __host__ __device__ int jam_table_floats(int nl, int nmx) {
 #define JQ_MI 8
 
 #define GLAD_PROF_MAX 2048
-enum GladKernelId { GK_LENS_PREP = 0, GK_LENS_IMAGE, GK_JAM_PREP, GK_JAM_QUAD, GK_JAM_POST, GK_JOINT };
+enum GladKernelId { GK_LENS_PREP = 0, GK_LENS_IMAGE, GK_JAM_PREP, GK_JAM_QUAD, GK_JAM_POST, GK_JOINT, GK_MGE };
 
 struct glad_ctx {
     int device;
@@ -84,6 +84,7 @@ struct glad_ctx {
     float* d_tmp;        size_t tmp_cap;     // chi2_L, chi2_D [B] each
     int32_t* d_tmpflags; size_t tmpflags_cap; // flags_L, flags_D [B] each
     float* d_stage;      size_t stage_cap;   // device staging of glad_joint_loglike_host
+    float* d_model;      size_t model_cap;   // glad_joint_loglike_model_batch: lens', profile rows, derived MGE tables
 
     // optional per-kernel timing (glad_profile_*): CUDA events on the context stream around each launch
     bool prof_on;
@@ -119,6 +120,10 @@ cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d
 cudaError_t launch_joint(glad_ctx* c, int B, const float* d_c2l, const float* d_c2d, const int32_t* d_fl,
                          const int32_t* d_fd, float* d_loglike, int32_t* d_flags);
 cudaError_t launch_kin_weights(glad_ctx* c);
+cudaError_t launch_mge1d(glad_ctx* c, int kind, const float* d_prof, int B, int n_gauss, float sigma_lo, float sigma_hi,
+                         int P, float* d_mge);
+cudaError_t launch_model_prep(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, double zd, int B,
+                              float* d_lens_out, float* d_prof_lum, float* d_prof_mass);
 // tensor-core (tcgen05) form of row a6; supported when the folded grid has ny_f <= 128, N = terms * nx_f <= 256
 // and two operand stages fit in shared memory
 bool jam_quad_tc_supported(const glad_ctx* c, int nl, int nmx);

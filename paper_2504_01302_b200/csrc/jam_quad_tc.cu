@@ -313,35 +313,45 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
             yb0 = min(bnd[0], nyb); yb1 = min(bnd[1], nyb);
             xb0 = max(bnd[0], nyb) - nyb; xb1 = max(bnd[1], nyb) - nyb;
         }
+        // per-thread constants of the block loops: first squared coordinate, first destination row, trip counts
+        const float* const qy0 = s_c2 + yb0 * 8 + l8;
+        const float* const qx0 = s_c2 + ny8 + xb0 * 8 + l8;
+        const int offA = oct * GA * 8 + l8 + yb0 * 8, offB = a16 + oct * GB * 8 + l8 + xb0 * 8;
+        const int nyblk = yb1 - yb0, nxblk = xb1 - xb0;
+        const int tsA = nyb * 8, tsB = nxb * 8;                          // 16-byte units between the bf16 terms of a value
         auto produce = [&](int it, int buf) {
             const float* cb = s_coef + (it & (a.cslots - 1)) * (4 * MC) + 8 * oct;
-            uint4* stA = s_ops + buf * stage16 + oct * GA * 8 + l8;
-            uint4* stB = s_ops + buf * stage16 + a16 + oct * GB * 8 + l8;
-            if (yb0 < yb1) {
+            uint4* const stage = s_ops + buf * stage16;
+            if (nyblk > 0) {
                 const float4 e0 = *reinterpret_cast<const float4*>(cb), e1 = *reinterpret_cast<const float4*>(cb + 4);
-                for (int blk = yb0; blk < yb1; ++blk) {
-                    const float q = s_c2[blk * 8 + l8];
+                const f32x2 c0 = pk2(e0.x, e0.y), c1 = pk2(e0.z, e0.w), c2 = pk2(e1.x, e1.y), c3 = pk2(e1.z, e1.w);
+                const float* qp = qy0;
+                uint4* dst = stage + offA;
+                for (int n = nyblk; n > 0; --n, qp += 8, dst += 8) {
+                    const float q = *qp;
                     const f32x2 qq = pk2(q, q);
                     f32x2 v[4];
-                    v[0] = ex2_2(mul2(pk2(e0.x, e0.y), qq)); v[1] = ex2_2(mul2(pk2(e0.z, e0.w), qq));
-                    v[2] = ex2_2(mul2(pk2(e1.x, e1.y), qq)); v[3] = ex2_2(mul2(pk2(e1.z, e1.w), qq));
-                    split_store<NT>(v, stA + blk * 8, nyb * 8);
+                    v[0] = ex2_2(mul2(c0, qq)); v[1] = ex2_2(mul2(c1, qq));
+                    v[2] = ex2_2(mul2(c2, qq)); v[3] = ex2_2(mul2(c3, qq));
+                    split_store<NT>(v, dst, tsA);
                 }
             }
-            if (xb0 < xb1) {
+            if (nxblk > 0) {
                 const float* cx = cb + MC;
                 const float4 p0 = *reinterpret_cast<const float4*>(cx), p1 = *reinterpret_cast<const float4*>(cx + 4);
                 const float4 g0 = *reinterpret_cast<const float4*>(cx + MC), g1 = *reinterpret_cast<const float4*>(cx + MC + 4);
                 const float4 h0 = *reinterpret_cast<const float4*>(cx + 2 * MC), h1 = *reinterpret_cast<const float4*>(cx + 2 * MC + 4);
-                for (int blk = xb0; blk < xb1; ++blk) {
-                    const float q = s_c2[ny8 + blk * 8 + l8];
+                const float* qp = qx0;
+                uint4* dst = stage + offB;
+                for (int n = nxblk; n > 0; --n, qp += 8, dst += 8) {
+                    const float q = *qp;
                     const f32x2 qq = pk2(q, q);
                     f32x2 v[4];
                     v[0] = mul2(fma2(pk2(h0.x, h0.y), qq, pk2(g0.x, g0.y)), ex2_2(mul2(pk2(p0.x, p0.y), qq)));
                     v[1] = mul2(fma2(pk2(h0.z, h0.w), qq, pk2(g0.z, g0.w)), ex2_2(mul2(pk2(p0.z, p0.w), qq)));
                     v[2] = mul2(fma2(pk2(h1.x, h1.y), qq, pk2(g1.x, g1.y)), ex2_2(mul2(pk2(p1.x, p1.y), qq)));
                     v[3] = mul2(fma2(pk2(h1.z, h1.w), qq, pk2(g1.z, g1.w)), ex2_2(mul2(pk2(p1.z, p1.w), qq)));
-                    split_store<NT>(v, stB + blk * 8, nxb * 8);
+                    split_store<NT>(v, dst, tsB);
                 }
             }
         };

@@ -176,7 +176,7 @@ def make_workload(name: str, data_model=None, B: int | None = None) -> dict:
     Ie_1[0], Re_1[0], n_1[0], q_1[0] = 0.02, 1.85, 4.0, 0.8
     inc[0], dd[0], ddt[0], ups[0] = math.radians(84.3), 775.0, 1823.0, 1.0
 
-    wl = {"name": name, "B": B, "lens": None, "dyn": None}
+    wl = {"name": name, "B": B, "lens": None, "dyn": None, "ddt": ddt.astype(np.float32), "z_d": Z_D}
 
     if L:
         p = np.zeros((B, NLENS))
@@ -236,7 +236,8 @@ def make_workload(name: str, data_model=None, B: int | None = None) -> dict:
 def subset(wl: dict, idx) -> dict:
     """Same static data, only the batch elements `idx` (for parity sub-batches)."""
     idx = np.asarray(idx, dtype=np.int64)
-    out = {"name": wl["name"], "B": int(idx.size), "lens": None, "dyn": None}
+    out = {"name": wl["name"], "B": int(idx.size), "lens": None, "dyn": None,
+           "ddt": np.ascontiguousarray(wl["ddt"][idx]), "z_d": wl["z_d"]}
     if wl["lens"]:
         out["lens"] = dict(wl["lens"])
         out["lens"]["params"] = np.ascontiguousarray(wl["lens"]["params"][idx])
