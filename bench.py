@@ -30,6 +30,11 @@ FP32_LANES_PER_SM = 128
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the quadrature kernel from the committed ncu --set full
 # captures (profiles/r1a.md, profiles/r1b.md): operands never exist in HBM, only the tables are read
 RESIDENT_TRAFFIC = {"jam_quad_simt": 4.4e6, "jam_quad_tc": 4.44e6}
+# Executed FP32 flops of lens_image_kernel per parameter vector (FFMA = 2, FMUL = FADD = 1; MUFU not counted) from the
+# same captures' smsp__sass_thread_inst_executed_op_{ffma,fmul,fadd}_pred_on (profiles/r1b.md: 8.05e9 FFMA, 2.60e9
+# FMUL, 0.63e9 FADD per 1024-vector C2 launch).  SURVEY.md 8(d)'s algorithmic estimate for C2 is 1.82e7 per vector
+# (40 000 rays x ~235 flop + 10 000 pixels x 2 x 441 PSF taps).
+LENS_FP32_FLOPS_PER_VECTOR = {"C2": 1.888e7}
 
 
 def read_peaks():
@@ -221,6 +226,33 @@ def run_ours(args, rank, world, local_rank):
     e2e_ms = a0.elapsed_time(a1)
     clocks = sampler.stop()
 
+    # the self-consistent entry (lens vector + distances -> MGE tables on the device -> both halves);
+    # reported beside the headline, not instead of it (the headline keeps BASELINE.json's table inputs)
+    model = None
+    if rank == 0:
+        ddt = t(wl["ddt"]).to(dev)
+        nlm, nmm = D["lum_mge"].shape[-2], D["mass_mge"].shape[-2]
+        margs = (d["lens"], d["dyn"], ddt, wl["z_d"], nlm, (0.02, 10.0), nmm, (0.02, 50.0), d["beta"])
+        for _ in range(3):
+            g.joint_loglike_model_batch(*margs, out=out)
+        torch.cuda.synchronize()
+        g.profile_enable(True)
+        g.profile_read()
+        m_steps = max(3, min(args.steps, 10))
+        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        m0.record()
+        for _ in range(m_steps):
+            g.joint_loglike_model_batch(*margs, out=out)
+        m1.record()
+        torch.cuda.synchronize()
+        mp = g.profile_read()
+        g.profile_enable(False)
+        m_ms = m0.elapsed_time(m1) / m_steps
+        model = {"api": "glad_joint_loglike_model_batch", "value": B / (m_ms * 1e-3), "unit": UNIT, "ms_per_step": m_ms,
+                 "mge_ms_per_step": mp["mge"][0] / m_steps, "mge_launches_per_step": mp["mge"][1] / m_steps,
+                 "tables": f"{nlm} luminous (Sersic, 0.02-10 arcsec) + {nmm} mass (EPL, 0.02-50 arcsec) Gaussians per vector, Euler order 12",
+                 "paper_context": "1-D MGE of one profile: ~2e-4 s on one A100 (P:356, Table 2)"}
+
     if dist is not None:
         tt = torch.tensor([ms, e2e_ms], device=dev, dtype=torch.float64)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
@@ -271,6 +303,16 @@ def run_ours(args, rank, world, local_rank):
                                    "peak": bf16_peak, "frac": mma_flops / (q_avg * 1e-3) / 1e12 / bf16_peak,
                                    "peak_source": "MEASURED_PEAKS.json bf16_tflops (burst)" if peaks.get("bf16_tflops") else "nominal 2250 (no MEASURED_PEAKS.json)"}
 
+    # BASELINE.json's metric asks for the % of FP32 peak per stage: the lensing stage (ray-shoot + bin-down + PSF + chi2)
+    l_ms, l_n = prof["lens_image"]
+    if args.config in LENS_FP32_FLOPS_PER_VECTOR and l_n:
+        lf = LENS_FP32_FLOPS_PER_VECTOR[args.config] * B
+        l_avg = l_ms / l_n
+        roofline["lens_image"] = {"bound": "alu", "kernel": "lens_image_kernel", "unit": "TFLOP/s",
+                                  "achieved": lf / (l_avg * 1e-3) / 1e12, "peak": peak_tf,
+                                  "frac": lf / (l_avg * 1e-3) / 1e12 / peak_tf, "ms_per_launch": l_avg,
+                                  "flops_per_launch": lf, "flops_source": "executed FP32 flops counted by ncu (profiles/r1b.md)"}
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         import oracle
@@ -295,7 +337,7 @@ def run_ours(args, rank, world, local_rank):
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": B * 4,
                     "steps": e2e_steps, "api": "glad_joint_loglike_host (pinned host buffers)"},
-            "roofline": roofline, "cpu_baseline": cpu}
+            "roofline": roofline, "cpu_baseline": cpu, "model_entry": model}
     print(json.dumps(line), flush=True)
     g.close()
     if dist is not None:

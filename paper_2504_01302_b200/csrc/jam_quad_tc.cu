@@ -58,6 +58,8 @@ __device__ __forceinline__ float ex2_tc(float x) { return x * 1.0001f; }
 #else
 __device__ __forceinline__ float ex2_tc(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 #endif
+__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -81,6 +83,9 @@ __device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint6
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
+#ifdef ABL_MMA       // timing experiments only (never defined in the product build): producers without tensor work
+#define umma_bf16(...) ((void)0)
+#endif
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
@@ -96,19 +101,29 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.f32x
 __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 __device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 ex2_2(f32x2 x) { float a, b; unpk2(x, a, b); return pk2(ex2_tc(a), ex2_tc(b)); }
+// a -= bf16 low half of w, b -= bf16 high half of w, exactly (mixed-precision FHFMA.BF16: one issue slot per value,
+// no unpacking of the bf16 pair into fp32 registers)
+__device__ __forceinline__ void bf16_residual(uint32_t w, float& a, float& b) {
+    asm("{\n\t.reg .b16 l, h, m;\n\tmov.b32 {l, h}, %2;\n\tmov.b16 m, 0xBF80;\n\t"
+        "fma.rn.f32.bf16 %0, l, m, %0;\n\tfma.rn.f32.bf16 %1, h, m, %1;\n\t}" : "+f"(a), "+f"(b) : "r"(w));
+}
 // split 4 pairs (the 8 rows of one oct, one pixel) into NT bf16 terms and store one 16-byte core-matrix row per term
 template <int NT>
 __device__ __forceinline__ void split_store(f32x2 (&v)[4], uint4* dst, int term_stride16) {
+    float lo[4], hi[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) unpk2(v[j], lo[j], hi[j]);
 #pragma unroll
     for (int t = 0; t < NT; ++t) {
         uint32_t w[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            float lo, hi;
-            unpk2(v[j], lo, hi);
-            w[j] = pack_bf16(lo, hi);
-            if (t + 1 < NT) v[j] = sub2(v[j], pk2(__uint_as_float(w[j] << 16), __uint_as_float(w[j] & 0xFFFF0000u)));
+            w[j] = pack_bf16(lo[j], hi[j]);
+            if (t + 1 < NT) bf16_residual(w[j], lo[j], hi[j]);
         }
+#ifdef ABL_STS       // timing experiments only: keep the values alive without the shared-memory store
+        if (w[0] == 0x12345678u && w[3] == 0x9abcdef0u)
+#endif
         dst[t * term_stride16] = make_uint4(w[0], w[1], w[2], w[3]);
     }
 }
@@ -123,14 +138,15 @@ __device__ __forceinline__ int div_small(int a, int d, float inv) {
 __device__ __forceinline__ void bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 __device__ __forceinline__ void bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 
-// NT = bf16 terms per operand value, PW = producer warps (16 or 24), NACC = accumulator registers per thread
-// (multiple of 8, NACC * PW/4 >= N)
+// NT = bf16 terms per operand value, PW = producer warps, NACC = accumulator registers per thread (multiple of 8,
+// NACC * PW/4 >= nxp: the NT column blocks [X1 | X2 | ..] of the accumulator are added into the same registers)
 template <int NT, int NACC, int PW>
 __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) {
     constexpr int NPROD = PW * 32, NTHR = NPROD + 32;
     extern __shared__ __align__(128) float sm[];
     __shared__ __align__(8) uint64_t s_bar[3];     // empty[0], empty[1], done
     __shared__ uint32_t s_tmem;
+    __shared__ int s_stride[3];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int b = blockIdx.x / a.S, s = blockIdx.x - b * a.S;
     const float* Tg = a.tab + (size_t)b * a.tabsz;
@@ -252,12 +268,14 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
         // iteration rc: the reader has passed the "empty" wait of chunk rc-2, so every producer has arrived on "full"
         // of rc-2, i.e. finished writing.  While a thread writes in iteration `it` the slowest warp can still be
         // reading chunk it-1 (the writer passed the "empty" wait of it-2): slots it-1 .. it+R+1 are live, cslots >= R+3.
-        auto coef_row = [&](int rc, int r) {
-            const int m = (c0 + rc) * MC + r;
+        // one row from its (iu, j, k): 3 MUFU.RCP + 1 MUFU.RSQ (approx, <= 2 ulp: the operands carry 16 bits)
+        auto coef_store = [&](int rc, int r, int iu, int j, int k) {
             float cq = 0.f, cp = 0.f, f0 = 0.f, f1 = 0.f;
-            if (m < M) {
-                const int iu = div_small(m, pairs, inv_pairs), rem = m - iu * pairs;
-                const int j = div_small(rem, nl, inv_nl), k = rem - j * nl;
+#ifdef ABL_COEF      // timing experiments only
+            if (iu < 0) {
+#else
+            if (iu < nu) {
+#endif
                 const float2 uw = s_uw[iu];
                 const float4 mj = s_mj[j];
                 const float4 lk = s_lk[k];
@@ -266,20 +284,26 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
                 const float u2 = uw.x;
                 const float t = mj.y * u2, auj = u2 * mj.x;
                 const float gg = 1.f - t;
-                const float bb = t * auj * __frcp_rn(gg);
+                const float bb = t * auj * rcp_approx(gg);
                 const float A = 0.5f * (auj + lk.x);
                 const float Bc = 0.5f * (lk.y + bb);
                 const float E = fmaf(Bc, cos2i, A);
                 const float D = fmaf(-jk.y, u2, d0);
-                const float inv = rsqrtf(E * gg) * __frcp_rn(fmaf(-jk.x, u2, 1.f));
+                const float inv = rsqrt_approx(E * gg) * rcp_approx(fmaf(-jk.x, u2, 1.f));
                 const float pref = uw.y * mj.z * inv;
                 cp = -A * LOG2E_F;
-                cq = -(A * (A + Bc)) * __frcp_rn(E) * LOG2E_F;
+                cq = -(A * (A + Bc)) * rcp_approx(E) * LOG2E_F;
                 f0 = pref * lk.z;
                 f1 = pref * lk.w * D;
             }
             float* dst = s_coef + (rc & (a.cslots - 1)) * (4 * MC) + r;
             dst[0] = cq; dst[MC] = cp; dst[2 * MC] = f0; dst[3 * MC] = f1;
+        };
+        auto coef_row = [&](int rc, int r) {                            // prologue: index split by division
+            const int m = (c0 + rc) * MC + r;
+            const int iu = div_small(m, pairs, inv_pairs), rem = m - iu * pairs;
+            const int j = div_small(rem, nl, inv_nl), k = rem - j * nl;
+            coef_store(rc, r, iu, j, k);
         };
         const int R = NPROD / MC;                                       // producer thread groups of MC threads
         const int cgrp = tid / MC, crow = tid - cgrp * MC;
@@ -356,34 +380,53 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
             }
         };
 
-        // running map in registers: thread (lane quarter lq, column group cg) holds D[32 lq + lane][cg * NACC + i]
+        // running map in registers: thread (lane quarter lq, column group cg) holds sum_tc D[32 lq + lane][tc nxp + cg NACC + i]
         float acc[NACC];
 #pragma unroll
         for (int i = 0; i < NACC; ++i) acc[i] = 0.f;
         const int lq = warp & 3, cg = warp >> 2;
         auto flush = [&](int g) {
+#ifdef ABL_FLUSH     // timing experiments only
+            if (g >= 0) return;
+#endif
             const uint32_t taddr = tmem + ((uint32_t)(32 * lq) << 16) + (uint32_t)(g & 1) * dstride + (uint32_t)(cg * NACC);
 #pragma unroll
-            for (int i = 0; i < NACC; i += 8) {
-                if (cg * NACC + i >= N) break;                          // warp-uniform: columns past the accumulator
-                uint32_t r[8];
-                asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                             : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
-                             : "r"(taddr + (uint32_t)i));
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            for (int tc = 0; tc < NT; ++tc) {
 #pragma unroll
-                for (int j = 0; j < 8; ++j) acc[i + j] += __uint_as_float(r[j]);
+                for (int i = 0; i < NACC; i += 8) {
+                    if (cg * NACC + i >= nxp) break;                    // warp-uniform: columns past the term block
+                    uint32_t r[8];
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                                 : "r"(taddr + (uint32_t)(tc * nxp + i)));
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) acc[i + j] += __uint_as_float(r[j]);
+                }
             }
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         };
 
         int gf = 0;                                                     // next accumulator group to add into acc
         const uint32_t bar_empty = smem_u32(&s_bar[0]);
+        if (tid == 0) {                                                 // the stride NPROD as (du, dj, dk): CTA-uniform, kept in smem
+            const int sdu = div_small(NPROD, pairs, inv_pairs), srem = NPROD - sdu * pairs;
+            const int sdj = div_small(srem, nl, inv_nl);
+            s_stride[0] = sdu; s_stride[1] = sdj; s_stride[2] = srem - sdj * nl;
+        }
         if (nch > 0) {
             if (cgrp < 2 && cgrp < nch) coef_row(cgrp, crow);           // chunks 0 and 1
             bar_sync(3, NPROD);
         }
         int cphase = 0;                                                 // it % R
+        // In the loop a thread's rows advance by NPROD contraction rows per call: (iu, j, k) is carried, not divided.
+        int ciu, cj, ck;
+        {
+            const int m0 = (c0 + 2 + cgrp) * MC + crow;
+            ciu = div_small(m0, pairs, inv_pairs);
+            const int rem = m0 - ciu * pairs;
+            cj = div_small(rem, nl, inv_nl); ck = rem - cj * nl;
+        }
         for (int it = 0; it < nch; ++it) {
             const int buf = it & 1;
             if (it >= 2) {
@@ -391,7 +434,12 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 while ((gf + 1) * a.FL - 1 <= it - 2) flush(gf++);
             }
-            if (cphase == 0 && it + 2 + cgrp < nch) coef_row(it + 2 + cgrp, crow);   // chunks it+2 .. it+R+1, one row per thread
+            if (cphase == 0) {                                          // chunks it+2 .. it+R+1, one row per thread
+                if (it + 2 + cgrp < nch) coef_store(it + 2 + cgrp, crow, ciu, cj, ck);
+                ck += s_stride[2]; if (ck >= nl) { ck -= nl; ++cj; }
+                cj += s_stride[1]; if (cj >= nm) { cj -= nm; ++ciu; }
+                ciu += s_stride[0];
+            }
             cphase = cphase + 1 == R ? 0 : cphase + 1;
             produce(it, buf);
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -405,20 +453,19 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
             mbar_wait(smem_u32(&s_bar[2]), 0);                           // all MMAs done: the stages are free
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             while (gf * a.FL < nch) flush(gf++);
-            float* scr = reinterpret_cast<float*>(s_ops);                // [128][N]
+            float* scr = reinterpret_cast<float*>(s_ops);                // [128][nxp]
             const int row = 32 * lq + lane;
 #pragma unroll
             for (int i = 0; i < NACC; ++i) {
                 const int col = cg * NACC + i;
-                if (col < N) scr[row * N + col] = acc[i];
+                if (col < nxp) scr[row * nxp + col] = acc[i];
             }
             bar_sync(3, NPROD);
             const int TR = a.multi ? 1 : NT;
             for (int i = tid; i < npf; i += NPROD) {
                 const int iy = i / a.nxf, ix = i - iy * a.nxf;
                 float v = 0.f;
-                for (int tr = TR - 1; tr >= 0; --tr)                      // small cross terms first
-                    for (int tc = NT - 1; tc >= 0; --tc) v += scr[(tr * ny8 + iy) * N + tc * nxp + ix];
+                for (int tr = TR - 1; tr >= 0; --tr) v += scr[(tr * ny8 + iy) * nxp + ix];   // small terms first
                 out[i] = v;
             }
         } else {
@@ -435,29 +482,25 @@ static int tc_terms() {
     const char* e = getenv("GLAD_JAM_TERMS");
     return (e && atoi(e) == 3) ? 3 : 2;
 }
-// producer warps per CTA: 16 by default, 24 with GLAD_JAM_WARPS=24
-static int tc_warps() {
-    const char* e = getenv("GLAD_JAM_WARPS");
-    return (e && atoi(e) == 24) ? 24 : 16;
-}
+#define TC_PW 16    // producer warps per CTA (24 was tried: 72 registers per thread spill, slower)
 
 // launch plan for the current sky grid and table sizes; false = not supported (the FP32 kernel takes over)
 static bool tc_plan(const glad_ctx* c, int nl, int nmx, JTArgs* a, int* nacc, size_t* smem) {
-    const int NT = tc_terms(), PW = tc_warps();
+    const int NT = tc_terms(), PW = TC_PW;
     a->ny8 = (c->nyf + 7) & ~7;
     if (a->ny8 > 128) return false;
     a->multi = NT * a->ny8 > 128 ? 1 : 0;
     a->nxp = (NT == 3 || a->multi) ? ((c->nxf + 15) & ~15) : ((c->nxf + 7) & ~7);
     a->N = NT * a->nxp;
     if (a->N > 256) return false;
-    const int per = (a->N + PW / 4 - 1) / (PW / 4);                      // accumulator columns per warp of a lane quarter
-    *nacc = PW == 16 ? (per <= 24 ? 24 : (per <= 40 ? 40 : 64)) : (per <= 16 ? 16 : (per <= 32 ? 32 : 48));
+    const int per = (a->nxp + PW / 4 - 1) / (PW / 4);                    // accumulator columns per warp of a lane quarter
+    *nacc = per <= 16 ? 16 : (per <= 24 ? 24 : 32);
     a->tmem_cols = 512;                                                  // one CTA per SM: two accumulator buffers of 256 columns
     const size_t fixed = (((size_t)4 * nl + 4 * nmx + 2 * (size_t)nmx * nl + 2 * (size_t)c->nu + ((nl + 3) & ~3) +
                            (size_t)(a->ny8 + a->nxp) + 31) & ~(size_t)31) * 4;
     for (a->MC = 256, a->lgMC = 8; a->MC >= 64; a->MC >>= 1, --a->lgMC) {
         size_t ops = 2 * (size_t)a->MC * NT * (a->ny8 + a->nxp) * 2 + 2048;   // two stages + the M = 128 over-read
-        const size_t scr = (size_t)128 * a->N * 4;                           // epilogue scratch reuses the stages
+        const size_t scr = (size_t)128 * a->nxp * 4;                         // epilogue scratch reuses the stages
         if (ops < scr) ops = scr;
         a->cslots = (PW * 32 / a->MC) <= 4 ? 8 : 16;
         *smem = fixed + (size_t)a->cslots * 4 * a->MC * 4 + ops;
@@ -480,15 +523,10 @@ static cudaError_t tc_launch(const JTArgs& a, int grid, size_t smem, cudaStream_
     return cudaGetLastError();
 }
 template <int NT>
-static cudaError_t tc_dispatch(const JTArgs& a, int nacc, int PW, int grid, size_t smem, cudaStream_t st) {
-    if (PW == 16) {
-        if (nacc == 24) return tc_launch<NT, 24, 16>(a, grid, smem, st);
-        if (nacc == 40) return tc_launch<NT, 40, 16>(a, grid, smem, st);
-        return tc_launch<NT, 64, 16>(a, grid, smem, st);
-    }
-    if (nacc == 16) return tc_launch<NT, 16, 24>(a, grid, smem, st);
-    if (nacc == 32) return tc_launch<NT, 32, 24>(a, grid, smem, st);
-    return tc_launch<NT, 48, 24>(a, grid, smem, st);
+static cudaError_t tc_dispatch(const JTArgs& a, int nacc, int grid, size_t smem, cudaStream_t st) {
+    if (nacc == 16) return tc_launch<NT, 16, 16>(a, grid, smem, st);
+    if (nacc == 24) return tc_launch<NT, 24, 16>(a, grid, smem, st);
+    return tc_launch<NT, 32, 16>(a, grid, smem, st);
 }
 
 cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S) {
@@ -503,6 +541,5 @@ cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S) {
     a.FL = 512 / a.MC;
     if (const char* e = getenv("GLAD_JAM_FLUSH")) { int v = atoi(e); if (v >= 1) a.FL = v; }
     ProfScope ps(c, GK_JAM_QUAD);
-    return tc_terms() == 3 ? tc_dispatch<3>(a, nacc, tc_warps(), B * S, smem, c->stream)
-                           : tc_dispatch<2>(a, nacc, tc_warps(), B * S, smem, c->stream);
+    return tc_terms() == 3 ? tc_dispatch<3>(a, nacc, B * S, smem, c->stream) : tc_dispatch<2>(a, nacc, B * S, smem, c->stream);
 }
