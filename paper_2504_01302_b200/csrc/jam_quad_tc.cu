@@ -351,14 +351,26 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
                 const f32x2 c0 = pk2(e0.x, e0.y), c1 = pk2(e0.z, e0.w), c2 = pk2(e1.x, e1.y), c3 = pk2(e1.z, e1.w);
                 const float* qp = qy0;
                 uint4* dst = stage + offA;
-                for (int n = nyblk; n > 0; --n, qp += 8, dst += 8) {
-                    const float q = *qp;
+                // software pipeline: the MUFU burst of block n+1 is issued before block n is split and stored, so the
+                // XU pipe (4 lanes per scheduler: 8 cycles per warp instruction) works while the warp packs
+                auto yvals = [&](const float* p, f32x2 (&v)[4]) {
+                    const float q = *p;
                     const f32x2 qq = pk2(q, q);
-                    f32x2 v[4];
                     v[0] = ex2_2(mul2(c0, qq)); v[1] = ex2_2(mul2(c1, qq));
                     v[2] = ex2_2(mul2(c2, qq)); v[3] = ex2_2(mul2(c3, qq));
-                    split_store<NT>(v, dst, tsA);
+                };
+                f32x2 cur[4];
+                yvals(qp, cur);
+                for (int n = nyblk - 1; n > 0; --n) {
+                    f32x2 nxt[4];
+                    qp += 8;
+                    yvals(qp, nxt);
+                    split_store<NT>(cur, dst, tsA);
+                    dst += 8;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) cur[j] = nxt[j];
                 }
+                split_store<NT>(cur, dst, tsA);
             }
             if (nxblk > 0) {
                 const float* cx = cb + MC;
@@ -367,16 +379,26 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
                 const float4 h0 = *reinterpret_cast<const float4*>(cx + 2 * MC), h1 = *reinterpret_cast<const float4*>(cx + 2 * MC + 4);
                 const float* qp = qx0;
                 uint4* dst = stage + offB;
-                for (int n = nxblk; n > 0; --n, qp += 8, dst += 8) {
-                    const float q = *qp;
+                auto xvals = [&](const float* p, f32x2 (&v)[4]) {
+                    const float q = *p;
                     const f32x2 qq = pk2(q, q);
-                    f32x2 v[4];
                     v[0] = mul2(fma2(pk2(h0.x, h0.y), qq, pk2(g0.x, g0.y)), ex2_2(mul2(pk2(p0.x, p0.y), qq)));
                     v[1] = mul2(fma2(pk2(h0.z, h0.w), qq, pk2(g0.z, g0.w)), ex2_2(mul2(pk2(p0.z, p0.w), qq)));
                     v[2] = mul2(fma2(pk2(h1.x, h1.y), qq, pk2(g1.x, g1.y)), ex2_2(mul2(pk2(p1.x, p1.y), qq)));
                     v[3] = mul2(fma2(pk2(h1.z, h1.w), qq, pk2(g1.z, g1.w)), ex2_2(mul2(pk2(p1.z, p1.w), qq)));
-                    split_store<NT>(v, dst, tsB);
+                };
+                f32x2 cur[4];
+                xvals(qp, cur);
+                for (int n = nxblk - 1; n > 0; --n) {
+                    f32x2 nxt[4];
+                    qp += 8;
+                    xvals(qp, nxt);
+                    split_store<NT>(cur, dst, tsB);
+                    dst += 8;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) cur[j] = nxt[j];
                 }
+                split_store<NT>(cur, dst, tsB);
             }
         };
 
