@@ -155,6 +155,55 @@ def run_reference(args, rank):
     print(json.dumps(line), flush=True)
 
 
+def run_sweep(args):
+    """--sweep: per-kernel device times of every BASELINE.json config on one GPU (C2/C4/C5 at a bounded batch, three
+    C3 cells), one JSON line per config.  Not the bench line: context for profiles/*.md."""
+    import torch
+    import workloads
+    from paper_2504_01302_b200 import Glad
+    cases = [("C1", None), ("C2", None), ("C3-10-40-4096", None), ("C3-20-80-4096", None), ("C3-40-160-256", None),
+             ("C4", 1024), ("C5", 296)]
+    for name, B in cases:
+        wl = workloads.make_workload(name, gpu_data_model(0), B=B)
+        L, D = wl["lens"], wl["dyn"]
+        g = Glad(0)
+        if L:
+            g.set_image_data(L["grid"], L["psf"], L["data"], L["ivar"])
+        if D:
+            g.set_kin_data(D["kin"])
+
+        def step():
+            if L and D:
+                g.joint_loglike_batch(L["params"], D["params"], D["lum_mge"], D["mass_mge"], D["beta"])
+            elif L:
+                g.lens_image_batch(L["params"], want_images=False)
+            else:
+                g.jam_vrms_batch(D["params"], D["lum_mge"], D["mass_mge"], D["beta"])
+        for _ in range(2):
+            step()
+        torch.cuda.synchronize()
+        g.profile_enable(True)
+        g.profile_read()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n = 3
+        e0.record()
+        for _ in range(n):
+            step()
+        e1.record()
+        torch.cuda.synchronize()
+        prof = g.profile_read()
+        ms = e0.elapsed_time(e1) / n
+        line = {"config": name, "batch": wl["B"], "ms_per_step": ms, "evals_per_s": wl["B"] / (ms * 1e-3),
+                "kernel_ms": {k: round(v[0] / n, 4) for k, v in prof.items() if v[1]}}
+        if D:
+            nx, ny = D["kin"]["xs"].size, D["kin"]["ys"].size
+            fl = 2.0 * ((nx + 1) // 2) * ((ny + 1) // 2) * float(workload_terms(wl).sum())
+            q = prof["jam_quad"][0] / n
+            line["jam_quad_alg_tflops"] = fl / (q * 1e-3) / 1e12
+        print(json.dumps(line), flush=True)
+        g.close()
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import workloads
@@ -354,12 +403,16 @@ def main():
     ap.add_argument("--batch", type=int, default=None, help="override the per-GPU batch (default: the config's)")
     ap.add_argument("--ref-sample", type=int, default=16, help="vectors per oracle pass (cpu_baseline / reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="per-kernel times of every BASELINE.json config (context, not the bench line)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.sweep:
+        run_sweep(args)
         return
     if world == 1 and args.gpus > 1:
         # convenience: re-launch under torch.distributed.run

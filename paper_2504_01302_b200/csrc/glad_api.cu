@@ -32,6 +32,7 @@ static glad_status grow(glad_ctx* c, T** p, size_t* cap, size_t need) {
     if (need <= *cap) return GLAD_OK;
     // the stream may still be using the old block: free is stream-ordered w.r.t. nothing, so sync first
     cudaStreamSynchronize(c->stream);
+    if (c->side_stream) cudaStreamSynchronize(c->side_stream);
     if (*p) cudaFree(*p);
     *p = nullptr;
     *cap = 0;
@@ -65,6 +66,17 @@ glad_status glad_create(glad_ctx** out, int device, void* cuda_stream) {
     c->sm_count = prop.multiProcessorCount;
     const char* jp = getenv("GLAD_JAM_PATH");
     c->jam_simt = (jp && strcmp(jp, "simt") == 0) ? 1 : 0;
+    c->lens_stream = c->stream;
+    const char* ov = getenv("GLAD_OVERLAP");
+    c->overlap = (ov && atoi(ov) == 0) ? 0 : 1;
+    if (c->overlap) {
+        if (cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
+            c->overlap = 0;
+        }
+    }
     *out = c;
     return GLAD_OK;
 }
@@ -83,6 +95,9 @@ void glad_destroy(glad_ctx* c) {
     if (!c) return;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
+    if (c->side_stream) { cudaStreamSynchronize(c->side_stream); cudaStreamDestroy(c->side_stream); }
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     free_kin(c);
     void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage, c->d_model};
     for (void* p : ps) if (p) cudaFree(p);
@@ -309,10 +324,23 @@ glad_status glad_joint_loglike_batch(glad_ctx* c, const float* d_lens, const flo
     float* c2l = d_chi2_lens ? d_chi2_lens : c->d_tmp;
     float* c2d = d_chi2_dyn ? d_chi2_dyn : c->d_tmp + B;
     int32_t *fl = c->d_tmpflags, *fd = c->d_tmpflags + B;
+    // scratch of both halves is grown before the fork (grow() may synchronise and free)
+    st = grow(c, &c->d_lens_const, &c->lens_const_cap, (size_t)B * LC_SIZE);
+    if (st != GLAD_OK) return st;
+    if (c->overlap) {
+        // fork: the lens half (lens_prep's serial b_n roots, then lens_image) runs on the side stream beside jam_prep /
+        // jam_quad; both wait for everything enqueued so far, and the caller's stream waits for the lens half below
+        CU(cudaEventRecord(c->ev_fork, c->stream), "fork");
+        CU(cudaStreamWaitEvent(c->side_stream, c->ev_fork, 0), "fork");
+        c->lens_stream = c->side_stream;
+    }
     st = lens_impl(c, d_lens, B, nullptr, c2l, fl);
-    if (st != GLAD_OK) return st;
-    st = jam_impl(c, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian, nullptr, c2d, nullptr, fd);
-    if (st != GLAD_OK) return st;
+    c->lens_stream = c->stream;
+    if (c->overlap) cudaEventRecord(c->ev_join, c->side_stream);
+    glad_status st2 = st == GLAD_OK ? jam_impl(c, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian,
+                                               nullptr, c2d, nullptr, fd) : st;
+    if (c->overlap) cudaStreamWaitEvent(c->stream, c->ev_join, 0);   // join, also when a half failed: nothing left dangling
+    if (st2 != GLAD_OK) return st2;
     CU(launch_joint(c, B, c2l, c2d, fl, fd, d_loglike, d_flags), "joint_kernel");
     return GLAD_OK;
 }

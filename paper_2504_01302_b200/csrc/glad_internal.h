@@ -54,6 +54,12 @@ struct glad_ctx {
     char err[512];
     long launches;
     int jam_simt;   // 1 = force the FP32 SIMT quadrature kernel (env GLAD_JAM_PATH=simt); default tcgen05
+    // The two halves are independent until joint_kernel: glad_joint_loglike_batch forks the lens half onto a context-owned
+    // side stream (event fork/join on the caller's stream, so the caller still sees plain stream order).  lens_stream is
+    // the stream the lens launchers use: == stream except inside that fork.  GLAD_OVERLAP=0 keeps everything on `stream`.
+    cudaStream_t lens_stream, side_stream;
+    cudaEvent_t ev_fork, ev_join;
+    int overlap;
 
     // lensing static data
     bool have_image;
@@ -98,15 +104,16 @@ struct glad_ctx {
 // Records an event pair around one launch when profiling is on (RAII; the launch goes between ctor and dtor).
 struct ProfScope {
     glad_ctx* c; int slot;
-    ProfScope(glad_ctx* ctx, int id) : c(ctx), slot(-1) {
+    cudaStream_t st;
+    ProfScope(glad_ctx* ctx, int id, cudaStream_t stream = nullptr) : c(ctx), slot(-1), st(stream ? stream : ctx->stream) {
         c->launches++;
         if (!c->prof_on || c->prof_n >= GLAD_PROF_MAX) return;
         slot = c->prof_n++;
         c->prof_id[slot] = id;
         if (!c->prof_ev[2 * slot]) { cudaEventCreate(&c->prof_ev[2 * slot]); cudaEventCreate(&c->prof_ev[2 * slot + 1]); }
-        cudaEventRecord(c->prof_ev[2 * slot], c->stream);
+        cudaEventRecord(c->prof_ev[2 * slot], st);
     }
-    ~ProfScope() { if (slot >= 0) cudaEventRecord(c->prof_ev[2 * slot + 1], c->stream); }
+    ~ProfScope() { if (slot >= 0) cudaEventRecord(c->prof_ev[2 * slot + 1], st); }
 };
 
 // kernel launchers (return cudaGetLastError())

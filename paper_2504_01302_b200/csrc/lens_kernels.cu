@@ -241,8 +241,8 @@ __global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict
 }
 
 cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B) {
-    ProfScope ps(c, GK_LENS_PREP);
-    lens_prep_kernel<<<(B + 31) / 32, 32 * LENS_PREP_ROLES, 0, c->stream>>>(d_params, B, c->d_lens_const);
+    ProfScope ps(c, GK_LENS_PREP, c->lens_stream);
+    lens_prep_kernel<<<(B + 31) / 32, 32 * LENS_PREP_ROLES, 0, c->lens_stream>>>(d_params, B, c->d_lens_const);
     return cudaGetLastError();
 }
 
@@ -256,8 +256,8 @@ cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2
         if (e != cudaSuccess) return e;
         configured = smem;
     }
-    ProfScope ps(c, GK_LENS_IMAGE);
-    lens_image_kernel<<<B, 512, smem, c->stream>>>(c->d_lens_const, c->grid, c->d_psf, c->kpsf, c->d_data, c->d_ivar,
+    ProfScope ps(c, GK_LENS_IMAGE, c->lens_stream);
+    lens_image_kernel<<<B, 512, smem, c->lens_stream>>>(c->d_lens_const, c->grid, c->d_psf, c->kpsf, c->d_data, c->d_ivar,
                                                   d_images, d_chi2, d_flags);
     return cudaGetLastError();
 }
