@@ -223,6 +223,15 @@ double glad_bh_theta2(double mbh_msun, double ddt_mpc, double z_d);
 glad_status glad_profile_enable(glad_ctx* ctx, int on);
 glad_status glad_profile_read(glad_ctx* ctx, double* ms_out /*[GLAD_NKERNELS]*/, long* count_out /*[GLAD_NKERNELS]*/);
 
+/*
+ * glad_joint_loglike_batch (and the entries built on it) run the lens half on a context-owned side stream beside the
+ * dynamics half, joined by events before the joint kernel; the caller's stream still sees plain stream order.
+ * glad_set_overlap(ctx, 0) keeps every kernel on the caller's stream (bench.py uses it for per-kernel timing, where
+ * overlapped event times would include waiting for SMs); default on (environment GLAD_OVERLAP=0 turns it off at creation).
+ * Returns GLAD_ESTATE if the side stream could not be created.
+ */
+glad_status glad_set_overlap(glad_ctx* ctx, int on);
+
 /* Number of kernel launches enqueued by this context since creation (for bench.py's gpu_launches). */
 long glad_launch_count(const glad_ctx* ctx);
 

@@ -20,7 +20,7 @@ _lib = None
 EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "glad_set_image_data",
            "glad_set_kin_data", "glad_lens_image_batch", "glad_jam_vrms_batch", "glad_joint_loglike_batch",
            "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count", "glad_profile_enable",
-           "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch"]
+           "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch", "glad_set_overlap"]
 
 
 class GladError(RuntimeError):
@@ -77,6 +77,8 @@ def load(rebuild: bool = False):
     L.glad_joint_loglike_model_batch.restype = i
     L.glad_joint_loglike_model_batch.argtypes = [vp, vp, vp, vp, C.c_float, i, i, C.c_float, C.c_float, i, C.c_float,
                                                  C.c_float, vp, i, vp, vp, vp, vp, vp, vp]
+    L.glad_set_overlap.restype = i
+    L.glad_set_overlap.argtypes = [vp, i]
     L.glad_launch_count.restype = l
     L.glad_launch_count.argtypes = [vp]
     _lib = L
@@ -139,6 +141,9 @@ class Glad:
         return int(self.lib.glad_launch_count(self.ctx))
 
     KERNELS = ("lens_prep", "lens_image", "jam_prep", "jam_quad", "jam_post", "joint", "mge")
+
+    def set_overlap(self, on: bool):
+        self._check(self.lib.glad_set_overlap(self.ctx, 1 if on else 0))
 
     def profile_enable(self, on: bool = True):
         self._check(self.lib.glad_profile_enable(self.ctx, 1 if on else 0))

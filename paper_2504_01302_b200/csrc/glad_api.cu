@@ -68,15 +68,15 @@ glad_status glad_create(glad_ctx** out, int device, void* cuda_stream) {
     c->jam_simt = (jp && strcmp(jp, "simt") == 0) ? 1 : 0;
     c->lens_stream = c->stream;
     const char* ov = getenv("GLAD_OVERLAP");
-    c->overlap = (ov && atoi(ov) == 0) ? 0 : 1;
-    if (c->overlap) {
-        if (cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking) != cudaSuccess ||
-            cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
-            cudaGetLastError();
-            c->overlap = 0;
-        }
+    if (cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        c->side_ok = 0;
+    } else {
+        c->side_ok = 1;
     }
+    c->overlap = (c->side_ok && !(ov && atoi(ov) == 0)) ? 1 : 0;
     *out = c;
     return GLAD_OK;
 }
@@ -127,6 +127,13 @@ glad_status glad_profile_read(glad_ctx* c, double* ms_out, long* count_out) {
         ms_out[k] = c->prof_ms[k]; count_out[k] = c->prof_cnt[k];
         c->prof_ms[k] = 0.0; c->prof_cnt[k] = 0;
     }
+    return GLAD_OK;
+}
+
+glad_status glad_set_overlap(glad_ctx* c, int on) {
+    if (!c) return GLAD_EINVAL;
+    if (on && !c->side_ok) return fail(c, GLAD_ESTATE, "glad_set_overlap: no side stream");
+    c->overlap = on ? 1 : 0;
     return GLAD_OK;
 }
 

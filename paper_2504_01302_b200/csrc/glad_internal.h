@@ -59,7 +59,7 @@ struct glad_ctx {
     // the stream the lens launchers use: == stream except inside that fork.  GLAD_OVERLAP=0 keeps everything on `stream`.
     cudaStream_t lens_stream, side_stream;
     cudaEvent_t ev_fork, ev_join;
-    int overlap;
+    int overlap, side_ok;
 
     // lensing static data
     bool have_image;
