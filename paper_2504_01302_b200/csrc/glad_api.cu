@@ -432,18 +432,14 @@ glad_status glad_joint_loglike_model_batch(glad_ctx* c, const float* d_lens, con
     if (st != GLAD_OK) return st;
     if (B == 0) return GLAD_OK;
     cudaSetDevice(c->device);
-    const size_t n_lens = (size_t)B * GLAD_NLENS, n_prof = (size_t)B * GLAD_NPROF;
-    const size_t n_lum = (size_t)B * nl * 3, n_mass = (size_t)B * nm * 3;
-    st = grow(c, &c->d_model, &c->model_cap, n_lens + 2 * n_prof + n_lum + n_mass);
+    const size_t n_lens = (size_t)B * GLAD_NLENS, n_lum = (size_t)B * nl * 3, n_mass = (size_t)B * nm * 3;
+    st = grow(c, &c->d_model, &c->model_cap, n_lens + n_lum + n_mass);
     if (st != GLAD_OK) return st;
     float* m_lens = c->d_model;
-    float* m_pl = m_lens + n_lens;
-    float* m_pm = m_pl + n_prof;
-    float* m_lum = d_lum_out ? d_lum_out : m_pm + n_prof;
-    float* m_mass = d_mass_out ? d_mass_out : m_pm + n_prof + n_lum;
-    CU(launch_model_prep(c, d_lens, d_dyn, d_ddt, (double)zd, B, m_lens, m_pl, m_pm), "model_prep_kernel");
-    CU(launch_mge1d(c, GLAD_PROFILE_SERSIC, m_pl, B, nl, lum_lo, lum_hi, MGE_DEFAULT_ORDER, m_lum), "mge1d_kernel");
-    CU(launch_mge1d(c, GLAD_PROFILE_EPL, m_pm, B, nm, mass_lo, mass_hi, MGE_DEFAULT_ORDER, m_mass), "mge1d_kernel");
+    float* m_lum = d_lum_out ? d_lum_out : m_lens + n_lens;
+    float* m_mass = d_mass_out ? d_mass_out : m_lens + n_lens + n_lum;
+    CU(launch_model(c, d_lens, d_dyn, d_ddt, (double)zd, B, nl, lum_lo, lum_hi, nm, mass_lo, mass_hi, MGE_DEFAULT_ORDER, m_lens,
+                    m_lum, m_mass), "model_kernel");
     return glad_joint_loglike_batch(c, m_lens, d_dyn, B, m_lum, nl, 3L * nl, m_mass, nm, 3L * nm, d_beta, per_gaussian,
                                     d_loglike, d_chi2_lens, d_chi2_dyn, d_flags);
 }
