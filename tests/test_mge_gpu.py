@@ -100,3 +100,30 @@ def test_joint_model_matches_oracle(glad_mod, oracle, name, B, n_lum, n_mass):
     o2 = g.joint_loglike_batch(l2, D["params"], out["lum_mge"], out["mass_mge"], D["beta"])
     assert np.array_equal(o2["chi2_dyn"].cpu().numpy(), out["chi2_dyn"].cpu().numpy())
     g.close()
+
+
+def test_joint_model_argument_errors_and_invalid_vectors(glad_mod, oracle):
+    wl = workloads.make_workload("C1", None)
+    L, D = wl["lens"], wl["dyn"]
+    lens = L["params"].copy()
+    lens[:, 16:21] = np.array([1e-9, 0.8, 3.0, 0.8, 0.0], np.float32)
+    g = glad_mod.Glad(0)
+    g.set_image_data(L["grid"], L["psf"], L["data"], L["ivar"])
+    g.set_kin_data(D["kin"])
+    ok = dict(n_lum=10, lum=LUM_RANGE, n_mass=10, mass=MASS_RANGE, zd=wl["z_d"])
+    for bad in (dict(n_lum=1), dict(n_mass=65), dict(lum=(0.0, 1.0)), dict(mass=(5.0, 1.0)), dict(zd=-1.0)):
+        a = dict(ok); a.update(bad)
+        with pytest.raises(glad_mod.GladError):
+            g.joint_loglike_model_batch(lens, D["params"], wl["ddt"], a["zd"], a["n_lum"], a["lum"], a["n_mass"], a["mass"], D["beta"])
+    with pytest.raises(glad_mod.GladError):
+        g.joint_loglike_model_batch(lens, D["params"], wl["ddt"][:3], wl["z_d"], 10, LUM_RANGE, 10, MASS_RANGE, D["beta"])
+    # a physically invalid vector (gamma outside (1,3)) is flagged, lnL = -inf, the rest of the batch is untouched
+    good = g.joint_loglike_model_batch(lens, D["params"], wl["ddt"], wl["z_d"], 10, LUM_RANGE, 10, MASS_RANGE, D["beta"])
+    ll_good = good["loglike"].cpu().numpy().copy()
+    lens_bad = lens.copy(); lens_bad[2, 3] = 3.5
+    out = g.joint_loglike_model_batch(lens_bad, D["params"], wl["ddt"], wl["z_d"], 10, LUM_RANGE, 10, MASS_RANGE, D["beta"])
+    ll = out["loglike"].cpu().numpy()
+    assert np.isneginf(ll[2]) and out["flags"].cpu().numpy()[2] != 0
+    keep = np.arange(8) != 2
+    assert np.array_equal(ll[keep], ll_good[keep]) and (out["flags"].cpu().numpy()[keep] == 0).all()
+    g.close()

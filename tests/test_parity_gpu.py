@@ -124,18 +124,50 @@ def test_c2_rxj1131_subbatch_and_full_batch_samples(glad_mod, oracle):
 
 def test_c3_dynamics_sweep_cells(glad_mod, oracle):
     dm = oracle_data_model(oracle)
-    for name, idx in (("C3-10-40-256", [0, 1, 2, 3, 4, 5, 6, 255]), ("C3-40-80-256", [0, 200]), ("C3-20-160-256", [0, 77])):
+    for name, idx in (("C3-10-40-256", [0, 1, 2, 3, 4, 5, 6, 255]), ("C3-40-80-256", [0, 200]), ("C3-20-160-256", [0, 77]),
+                      ("C3-10-40-4096", [0, 1, 2047, 4095]), ("C3-20-80-4096", [0, 4095])):   # the last two: BASELINE's large batch
         wl = workloads.make_workload(name, dm)
         run_jam(glad_mod, oracle, wl, np.array(idx), maps=True)
 
 
-def test_c4_lens_only_subbatch(glad_mod, oracle):
-    wl = workloads.make_workload("C4", oracle_data_model(oracle), B=512)
-    run_lens(glad_mod, oracle, wl, np.array([0, 1, 2, 3, 4, 5, 6, 7, 300, 511]))
+def test_c4_lens_only_full_batch(glad_mod, oracle):
+    """BASELINE.json configs[3] at its full size (8192 vectors in one launch); 10 sampled vectors against the oracle."""
+    wl = workloads.make_workload("C4", oracle_data_model(oracle))
+    assert wl["B"] == 8192
+    run_lens(glad_mod, oracle, wl, np.array([0, 1, 2, 3, 4, 5, 6, 7, 4096, 8191]))
 
 
-def test_c5_joint_stress_subbatch(glad_mod, oracle):
-    wl = workloads.make_workload("C5", oracle_data_model(oracle), B=160)
-    idx = np.array([0, 1, 159])
-    run_lens(glad_mod, oracle, wl, idx)
+def test_c5_joint_stress_full_batch(glad_mod, oracle):
+    """BASELINE.json configs[4] at its full size (4096 vectors, 200x200 image, 160x160 sky grid, 256 nodes); the oracle
+    takes about a core-minute per vector, so three are sampled."""
+    wl = workloads.make_workload("C5", oracle_data_model(oracle))
+    assert wl["B"] == 4096
+    idx = np.array([0, 1, 4095])
+    run_lens(glad_mod, oracle, wl, idx, images=False)
     run_joint(glad_mod, oracle, wl, idx)
+
+
+def test_two_streams_equal_one_stream(glad_mod, oracle):
+    """glad_joint_loglike_batch runs the lens half on the context's side stream (fork/join by events).  The
+    kernels and their inputs are the same, so the results are bitwise those of the one-stream order
+    (glad_set_overlap(0)), also when calls are queued back to back and when the scratch has to grow in between."""
+    import torch
+    wl = workloads.make_workload("C1", oracle_data_model(oracle))
+    L, D = wl["lens"], wl["dyn"]
+    g = glad_mod.Glad(0)
+    g.set_image_data(L["grid"], L["psf"], L["data"], L["ivar"])
+    g.set_kin_data(D["kin"])
+    args = (L["params"], D["params"], D["lum_mge"], D["mass_mge"], D["beta"])
+    big = tuple(np.concatenate([a] * 5) if a.shape[0] == 8 else a for a in args)        # 40 vectors: the scratch grows
+    res = {}
+    for mode in (True, False):
+        g.set_overlap(mode)
+        outs = [g.joint_loglike_batch(*args) for _ in range(3)] + [g.joint_loglike_batch(*big)] + [g.joint_loglike_batch(*args)]
+        torch.cuda.synchronize()
+        res[mode] = [{k: v.cpu().numpy().copy() for k, v in o.items()} for o in outs]
+    for a, b in zip(res[True], res[False]):
+        for k in ("loglike", "chi2_lens", "chi2_dyn", "flags"):
+            assert np.array_equal(a[k], b[k]), k
+    assert np.array_equal(res[True][0]["loglike"], res[True][4]["loglike"])
+    assert np.array_equal(res[True][3]["loglike"][:8], res[True][0]["loglike"])
+    g.close()
