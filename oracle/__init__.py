@@ -58,6 +58,10 @@ def lib():
         L.glad_oracle_deflection.argtypes = [dp, d, d, dp, dp]
         L.glad_oracle_lens_image_batch.restype = i
         L.glad_oracle_lens_image_batch.argtypes = [fp, i, i, i, i, d, d, d, fp, i, fp, fp, dp, dp, ip]
+        L.glad_oracle_lens_image_batch_kinds.restype = i
+        L.glad_oracle_lens_image_batch_kinds.argtypes = [fp, i, i, i, i, d, d, d, fp, i, fp, fp, ip, dp, dp, ip]
+        L.glad_oracle_chameleon.restype = d
+        L.glad_oracle_chameleon.argtypes = [d] * 7
         L.glad_oracle_jam_sigv2_point.restype = d
         L.glad_oracle_jam_sigv2_point.argtypes = [d, d, d, i, dp, dp, dp, dp, i, dp, dp, dp, i, dp, dp]
         L.glad_oracle_jam_vrms_batch.restype = i
@@ -110,8 +114,17 @@ def bh_theta2(Mbh, Ddt_mpc, zd) -> float:
     return float(lib().glad_oracle_bh_theta2(float(Mbh), float(Ddt_mpc), float(zd)))
 
 
-def lens_image_batch(lens, grid, psf, data=None, ivar=None, want_images=True):
-    """grid = dict(nx, ny, supersample, pix, x0, y0). Returns dict(images, chi2, flags)."""
+LIGHT_SERSIC, LIGHT_CHAMELEON = 0, 1
+
+
+def chameleon(dx, dy, I0, wc, wt, q, phi) -> float:
+    """Eq. 47 (P:370)."""
+    return float(lib().glad_oracle_chameleon(dx, dy, I0, wc, wt, q, phi))
+
+
+def lens_image_batch(lens, grid, psf, data=None, ivar=None, want_images=True, kinds=None):
+    """grid = dict(nx, ny, supersample, pix, x0, y0). kinds = None (all Sersic) or 3 ints (source, lens light 1, 2):
+    0 Sersic, 1 Chameleon (slot = {I_0, w_c, w_t, q, phi}). Returns dict(images, chi2, flags)."""
     lens = _f32(lens).reshape(-1, NLENS)
     B = lens.shape[0]
     nx, ny = int(grid["nx"]), int(grid["ny"])
@@ -121,9 +134,10 @@ def lens_image_batch(lens, grid, psf, data=None, ivar=None, want_images=True):
     images = np.empty((B, ny, nx), np.float64) if want_images else None
     chi2 = np.empty(B, np.float64)
     flags = np.zeros(B, np.int32)
-    rc = lib().glad_oracle_lens_image_batch(
+    kk = None if kinds is None else np.ascontiguousarray(kinds, dtype=np.int32).reshape(3)
+    rc = lib().glad_oracle_lens_image_batch_kinds(
         _ptr(lens, C.c_float), B, nx, ny, int(grid["supersample"]), float(grid["pix"]), float(grid["x0"]),
-        float(grid["y0"]), _ptr(psf, C.c_float), k, _ptr(data, C.c_float), _ptr(ivar, C.c_float),
+        float(grid["y0"]), _ptr(psf, C.c_float), k, _ptr(data, C.c_float), _ptr(ivar, C.c_float), _ptr(kk, C.c_int32),
         _ptr(images, C.c_double), _ptr(chi2, C.c_double), _ptr(flags, C.c_int32))
     if rc != 0:
         raise ValueError("oracle: bad lens arguments")

@@ -28,6 +28,8 @@
  *                           inclination independence, evenness, linearity
  *   PSF / bins (kin) ...... constant-field invariance, delta kernel
  *   joint ................. additivity, -inf propagation
+ *   Chameleon light ....... total flux closed form, w_t -> inf cored isothermal,
+ *                           Eq. 47 on the axes, = Sersic-free image pipeline
  *   1-D MGE (8(f) rank 1) . power-law closed form, Gaussian profile, profiles
  *                           summed back to the paper's ~0.5 %, linearity
  * Overall numbers: PARITY UNPINNED against any published value -- the paper
@@ -168,7 +170,21 @@ void glad_oracle_deflection(const double* p, double thx, double thy, double* ax,
     *ay = a_y;
 }
 
-static int lens_params_valid(const double* p) {
+/* Chameleon light profile, Eq. 47: the paper's lens-light model (two of them), a difference of two cored
+ * isothermal profiles with core radii w_c < w_t; R^2 = x^2 + y^2/q^2 in the component frame.
+ * SURVEY.md 8(f) rank 4 (light part).  Slot layout when a component is of this kind: {I_0, w_c, w_t, q, phi}. */
+double glad_oracle_chameleon(double dx, double dy, double I0, double wc, double wt, double q, double phi) {
+    double c = cos(phi), s = sin(phi);
+    double x = dx * c + dy * s, y = -dx * s + dy * c;
+    double R2 = x * x + y * y / (q * q);
+    double opq = 1.0 + q;
+    return I0 / opq * (1.0 / sqrt(R2 + 4.0 * wc * wc / (opq * opq)) - 1.0 / sqrt(R2 + 4.0 * wt * wt / (opq * opq)));
+}
+
+/* kinds[c] (c = source, lens light 1, lens light 2): 0 = Sersic (R-L7), 1 = Chameleon (Eq. 47); NULL = all Sersic */
+static int lens_params_valid_kinds(const double* p, const int* kinds);
+static int lens_params_valid(const double* p) { return lens_params_valid_kinds(p, NULL); }
+static int lens_params_valid_kinds(const double* p, const int* kinds) {
     if (!(p[2] >= 0.0)) return 0;                       /* theta_E */
     if (!(p[3] > 1.0 && p[3] < 3.0)) return 0;          /* gamma in (1,3) */
     if (!(p[4] > 0.0 && p[4] <= 1.0)) return 0;         /* q */
@@ -177,6 +193,10 @@ static int lens_params_valid(const double* p) {
     for (int c = 0; c < 3; ++c) {
         const double* s = p + off[c];
         if (s[0] == 0.0) continue;                      /* disabled component */
+        if (kinds && kinds[c] == 1) {                   /* Chameleon: 0 < w_c < w_t (positive profile), q in (0,1] */
+            if (!(s[1] > 0.0 && s[2] > s[1] && s[3] > 0.0 && s[3] <= 1.0)) return 0;
+            continue;
+        }
         if (!(s[1] > 0.0 && s[2] > 0.0 && s[3] > 0.0 && s[3] <= 1.0)) return 0;
     }
     return 1;
@@ -191,26 +211,39 @@ static int lens_params_valid(const double* p) {
  * Outputs (either may be NULL): images [B,ny,nx] fp64 PSF-convolved model; chi2 [B] fp64;
  * flags [B] int32 (FLAG_LENS_INVALID -> image NaN, chi2 +inf).
  */
+int glad_oracle_lens_image_batch_kinds(const float* lens, int B, int nx, int ny, int s, double pix,
+                                       double x0, double y0, const float* psf, int kpsf,
+                                       const float* data, const float* ivar, const int* kinds,
+                                       double* images, double* chi2, int32_t* flags);
 int glad_oracle_lens_image_batch(const float* lens, int B, int nx, int ny, int s, double pix,
                                  double x0, double y0, const float* psf, int kpsf,
                                  const float* data, const float* ivar, double* images,
                                  double* chi2, int32_t* flags) {
+    return glad_oracle_lens_image_batch_kinds(lens, B, nx, ny, s, pix, x0, y0, psf, kpsf, data, ivar, NULL, images, chi2, flags);
+}
+/* same, with the light profile kind of each component (see lens_params_valid_kinds) */
+int glad_oracle_lens_image_batch_kinds(const float* lens, int B, int nx, int ny, int s, double pix,
+                                       double x0, double y0, const float* psf, int kpsf,
+                                       const float* data, const float* ivar, const int* kinds,
+                                       double* images, double* chi2, int32_t* flags) {
     if (B < 0 || nx <= 0 || ny <= 0 || s <= 0 || kpsf <= 0 || (kpsf % 2) == 0) return -1;
+    if (kinds) for (int c = 0; c < 3; ++c) if (kinds[c] != 0 && kinds[c] != 1) return -1;
+    const int ks = kinds ? kinds[0] : 0, k1 = kinds ? kinds[1] : 0, k2 = kinds ? kinds[2] : 0;
     int npx = nx * ny, c = kpsf / 2;
 #pragma omp parallel for schedule(dynamic, 1)
     for (int b = 0; b < B; ++b) {
         double p[ORACLE_NLENS];
         for (int i = 0; i < ORACLE_NLENS; ++i) p[i] = (double)lens[(size_t)b * ORACLE_NLENS + i];
         if (flags) flags[b] = 0;
-        if (!lens_params_valid(p)) {
+        if (!lens_params_valid_kinds(p, kinds)) {
             if (flags) flags[b] |= FLAG_LENS_INVALID;
             if (images) for (int i = 0; i < npx; ++i) images[(size_t)b * npx + i] = NAN;
             if (chi2) chi2[b] = INFINITY;
             continue;
         }
-        double bn_s = p[11] != 0.0 ? glad_oracle_sersic_bn(p[13]) : 0.0;
-        double bn_1 = p[16] != 0.0 ? glad_oracle_sersic_bn(p[18]) : 0.0;
-        double bn_2 = p[21] != 0.0 ? glad_oracle_sersic_bn(p[23]) : 0.0;
+        double bn_s = (p[11] != 0.0 && !ks) ? glad_oracle_sersic_bn(p[13]) : 0.0;
+        double bn_1 = (p[16] != 0.0 && !k1) ? glad_oracle_sersic_bn(p[18]) : 0.0;
+        double bn_2 = (p[21] != 0.0 && !k2) ? glad_oracle_sersic_bn(p[23]) : 0.0;
         double* binned = (double*)malloc(sizeof(double) * npx);
         /* a1-a3: ray-shoot every sub-pixel centre (Eq. 33), evaluate light, mean (R-L2) */
         for (int iy = 0; iy < ny; ++iy)
@@ -225,14 +258,14 @@ int glad_oracle_lens_image_batch(const float* lens, int B, int nx, int ny, int s
                         double bx = thx - ax, by = thy - ay; /* beta = theta - alpha */
                         double v = 0.0;
                         if (p[11] != 0.0)
-                            v += glad_oracle_sersic(bx - p[9], by - p[10], p[11], p[12], p[13],
-                                                    p[14], p[15], bn_s);
+                            v += ks ? glad_oracle_chameleon(bx - p[9], by - p[10], p[11], p[12], p[13], p[14], p[15])
+                                    : glad_oracle_sersic(bx - p[9], by - p[10], p[11], p[12], p[13], p[14], p[15], bn_s);
                         if (p[16] != 0.0)
-                            v += glad_oracle_sersic(thx - p[0], thy - p[1], p[16], p[17], p[18],
-                                                    p[19], p[20], bn_1);
+                            v += k1 ? glad_oracle_chameleon(thx - p[0], thy - p[1], p[16], p[17], p[18], p[19], p[20])
+                                    : glad_oracle_sersic(thx - p[0], thy - p[1], p[16], p[17], p[18], p[19], p[20], bn_1);
                         if (p[21] != 0.0)
-                            v += glad_oracle_sersic(thx - p[0], thy - p[1], p[21], p[22], p[23],
-                                                    p[24], p[25], bn_2);
+                            v += k2 ? glad_oracle_chameleon(thx - p[0], thy - p[1], p[21], p[22], p[23], p[24], p[25])
+                                    : glad_oracle_sersic(thx - p[0], thy - p[1], p[21], p[22], p[23], p[24], p[25], bn_2);
                         acc += v;
                     }
                 binned[iy * nx + ix] = acc / (double)(s * s);
