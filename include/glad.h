@@ -224,6 +224,19 @@ glad_status glad_profile_enable(glad_ctx* ctx, int on);
 glad_status glad_profile_read(glad_ctx* ctx, double* ms_out /*[GLAD_NKERNELS]*/, long* count_out /*[GLAD_NKERNELS]*/);
 
 /*
+ * SURVEY 8(f) rank 4, light part: the paper models the lens light with Chameleon profiles (Eq. 47),
+ *   I = I_0/(1+q) [ (x^2 + y^2/q^2 + 4 w_c^2/(1+q)^2)^(-1/2) - (x^2 + y^2/q^2 + 4 w_t^2/(1+q)^2)^(-1/2) ].
+ * Each of the three light components (source, lens light 1, lens light 2) is a Sersic (default) or a Chameleon for the
+ * whole batch; a Chameleon component reads its five shape slots as {I_0, w_c, w_t, q, phi} instead of {I_e, R_e, n, q, phi}
+ * (source: lens[11..15], lens light: lens[16..20], lens[21..25]); valid iff 0 < w_c < w_t and 0 < q <= 1, I_0 = 0 disables it.
+ * Takes effect for the batch calls enqueued afterwards.  The luminous tracer of glad_joint_loglike_model_batch stays the
+ * Sersic expansion: that entry returns GLAD_ESTATE while lens light 1 is a Chameleon.
+ */
+#define GLAD_LIGHT_SERSIC 0
+#define GLAD_LIGHT_CHAMELEON 1
+glad_status glad_set_light_profiles(glad_ctx* ctx, int source_kind, int lens1_kind, int lens2_kind);
+
+/*
  * glad_joint_loglike_batch (and the entries built on it) run the lens half on a context-owned side stream beside the
  * dynamics half, joined by events before the joint kernel; the caller's stream still sees plain stream order.
  * glad_set_overlap(ctx, 0) keeps every kernel on the caller's stream (bench.py uses it for per-kernel timing, where

@@ -14,13 +14,14 @@ from .build import LIB, build
 
 NLENS, NDYN, NPROF = 26, 4, 4
 PROFILE_SERSIC, PROFILE_EPL = 0, 1
+LIGHT_SERSIC, LIGHT_CHAMELEON = 0, 1
 FLAG_LENS_INVALID, FLAG_DYN_INVALID, FLAG_BIN_INVALID = 1, 2, 4
 
 _lib = None
 EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "glad_set_image_data",
            "glad_set_kin_data", "glad_lens_image_batch", "glad_jam_vrms_batch", "glad_joint_loglike_batch",
            "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count", "glad_profile_enable",
-           "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch", "glad_set_overlap"]
+           "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch", "glad_set_overlap", "glad_set_light_profiles"]
 
 
 class GladError(RuntimeError):
@@ -77,6 +78,8 @@ def load(rebuild: bool = False):
     L.glad_joint_loglike_model_batch.restype = i
     L.glad_joint_loglike_model_batch.argtypes = [vp, vp, vp, vp, C.c_float, i, i, C.c_float, C.c_float, i, C.c_float,
                                                  C.c_float, vp, i, vp, vp, vp, vp, vp, vp]
+    L.glad_set_light_profiles.restype = i
+    L.glad_set_light_profiles.argtypes = [vp, i, i, i]
     L.glad_set_overlap.restype = i
     L.glad_set_overlap.argtypes = [vp, i]
     L.glad_launch_count.restype = l
@@ -141,6 +144,10 @@ class Glad:
         return int(self.lib.glad_launch_count(self.ctx))
 
     KERNELS = ("lens_prep", "lens_image", "jam_prep", "jam_quad", "jam_post", "joint", "mge")
+
+    def set_light_profiles(self, source=0, lens1=0, lens2=0):
+        """0 = Sersic, 1 = Chameleon (Eq. 47) per light component, for the batch calls that follow."""
+        self._check(self.lib.glad_set_light_profiles(self.ctx, int(source), int(lens1), int(lens2)))
 
     def set_overlap(self, on: bool):
         self._check(self.lib.glad_set_overlap(self.ctx, 1 if on else 0))

@@ -130,6 +130,18 @@ glad_status glad_profile_read(glad_ctx* c, double* ms_out, long* count_out) {
     return GLAD_OK;
 }
 
+glad_status glad_set_light_profiles(glad_ctx* c, int source_kind, int lens1_kind, int lens2_kind) {
+    if (!c) return GLAD_EINVAL;
+    const int k[3] = {source_kind, lens1_kind, lens2_kind};
+    int bits = 0;
+    for (int i = 0; i < 3; ++i) {
+        if (k[i] != GLAD_LIGHT_SERSIC && k[i] != GLAD_LIGHT_CHAMELEON) return fail(c, GLAD_EINVAL, "glad_set_light_profiles: kind %d", k[i]);
+        if (k[i] == GLAD_LIGHT_CHAMELEON) bits |= 1 << i;
+    }
+    c->light_kinds = bits;
+    return GLAD_OK;
+}
+
 glad_status glad_set_overlap(glad_ctx* c, int on) {
     if (!c) return GLAD_EINVAL;
     if (on && !c->side_ok) return fail(c, GLAD_ESTATE, "glad_set_overlap: no side stream");
@@ -426,6 +438,7 @@ glad_status glad_joint_loglike_model_batch(glad_ctx* c, const float* d_lens, con
     if (B < 0 || (B > 0 && (!d_lens || !d_dyn || !d_ddt || !d_beta || !d_loglike)))
         return fail(c, GLAD_EINVAL, "glad_joint_loglike_model_batch: B=%d / null pointer", B);
     if (!(zd > -1.f)) return fail(c, GLAD_EINVAL, "glad_joint_loglike_model_batch: z_d = %g", zd);
+    if (c->light_kinds & 2) return fail(c, GLAD_ESTATE, "glad_joint_loglike_model_batch: lens light 1 is a Chameleon, the tracer expansion is Sersic-only");
     glad_status st = mge_check(c, "glad_joint_loglike_model_batch (luminous)", nl, lum_lo, lum_hi);
     if (st != GLAD_OK) return st;
     st = mge_check(c, "glad_joint_loglike_model_batch (mass)", nm, mass_lo, mass_hi);

@@ -62,6 +62,7 @@ struct glad_ctx {
     int overlap, side_ok;
 
     // lensing static data
+    int light_kinds;   // bit k set: light component k (0 source, 1-2 lens light) is a Chameleon (glad_set_light_profiles)
     bool have_image;
     glad_image_grid grid;
     const float* d_data;

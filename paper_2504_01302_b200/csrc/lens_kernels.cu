@@ -13,7 +13,7 @@
 // 4 warps per 32 parameter vectors (lane = vector): warp role 0 = EPL / shear / point mass / validity, roles 1..3 =
 // one Sersic component each (the b_n root is the only long serial chain of the kernel; a warp never mixes roles).
 #define LENS_PREP_ROLES 4
-__global__ void __launch_bounds__(32 * LENS_PREP_ROLES) lens_prep_kernel(const float* __restrict__ params, int B, float* __restrict__ consts) {
+__global__ void __launch_bounds__(32 * LENS_PREP_ROLES) lens_prep_kernel(const float* __restrict__ params, int B, int kinds, float* __restrict__ consts) {
     const int b = blockIdx.x * 32 + (threadIdx.x & 31), role = threadIdx.x >> 5;
     if (b >= B) return;
     const float* p = params + (size_t)b * GLAD_NLENS;
@@ -22,7 +22,8 @@ __global__ void __launch_bounds__(32 * LENS_PREP_ROLES) lens_prep_kernel(const f
     bool valid = (thE >= 0.0) && (gam > 1.0 && gam < 3.0) && (q > 0.0 && q <= 1.0) && (p[8] >= 0.f);
     for (int k = 0; k < 3; ++k) {
         const float* s = p + (k == 0 ? 11 : (k == 1 ? 16 : 21));
-        if (s[0] != 0.f && !(s[1] > 0.f && s[2] > 0.f && s[3] > 0.f && s[3] <= 1.f)) valid = false;
+        const bool cham = (kinds >> k) & 1;                            // Chameleon (Eq. 47): 0 < w_c < w_t
+        if (s[0] != 0.f && !(s[1] > 0.f && (cham ? s[2] > s[1] : s[2] > 0.f) && s[3] > 0.f && s[3] <= 1.f)) valid = false;
     }
     if (role > 0) {
         const int k = role - 1;
@@ -34,6 +35,16 @@ __global__ void __launch_bounds__(32 * LENS_PREP_ROLES) lens_prep_kernel(const f
         o[0] = (k == 0) ? p[9] : (float)xl;
         o[1] = (k == 0) ? p[10] : (float)yl;
         if (Ie == 0.0) return;
+        if ((kinds >> k) & 1) {
+            // Chameleon, Eq. 47: slot = {I_0, w_c, w_t, q, phi}; I = amp (1/sqrt(R^2 + a_c) - 1/sqrt(R^2 + a_t)), a = 4 w^2/(1+q)^2
+            const double opq = 1.0 + qs;
+            o[2] = (float)cos(phi); o[3] = (float)sin(phi);
+            o[4] = (float)(1.0 / (qs * qs));
+            o[5] = (float)(Ie / opq);
+            o[6] = (float)(4.0 * Re * Re / (opq * opq));                   // a_c
+            o[7] = (float)(4.0 * (n * n - Re * Re) / (opq * opq));         // a_t - a_c, formed in fp64
+            return;
+        }
         double bn = sersic_bn(n);
         o[2] = (float)cos(phi); o[3] = (float)sin(phi);
         o[4] = (float)(1.0 / (qs * qs));
@@ -83,9 +94,27 @@ __device__ __forceinline__ float sersic_eval(const float* __restrict__ o, float 
     return o[5] * ex2f(-o[6] * pw);
 }
 
+__device__ __forceinline__ float chameleon_eval(const float* __restrict__ o, float px, float py) {
+    float dx = px - o[0], dy = py - o[1];
+    float x = dx * o[2] + dy * o[3];
+    float y = dy * o[2] - dx * o[3];
+    float R2 = fmaf(y * y, o[4], x * x);
+    // 1/s_c - 1/s_t = (a_t - a_c) / (s_c s_t (s_c + s_t)): no cancellation at large R or for close core radii
+    float uc = R2 + o[6], ut = uc + o[7];
+    float rc = rsqrtf(uc), rt = rsqrtf(ut);
+    return o[5] * o[7] * rc * rt * __fdividef(1.f, fmaf(uc, rc, ut * rt));
+}
+// CH = some component is a Chameleon (kinds bit k set); the all-Sersic instantiation is the code of rows a1-a2 as before
+template <bool CH>
+__device__ __forceinline__ float light_eval(int kinds, int k, const float* __restrict__ o, float px, float py) {
+    if (CH && ((kinds >> k) & 1)) return chameleon_eval(o, px, py);
+    return sersic_eval(o, px, py);
+}
+
 // One ray: returns source(beta) + lens light(theta).
+template <bool CH>
 __device__ __forceinline__ float shoot(const float* __restrict__ c, float thx, float thy, int nterms,
-                                       bool has_src, bool has_l1, bool has_l2) {
+                                       bool has_src, bool has_l1, bool has_l2, int kinds) {
     float dx = thx - c[LC_XL], dy = thy - c[LC_YL];
     float cs = c[LC_COSPA], sn = c[LC_SINPA];
     float x = dx * cs + dy * sn, y = dy * cs - dx * sn;
@@ -113,9 +142,9 @@ __device__ __forceinline__ float shoot(const float* __restrict__ c, float thx, f
     ax = fmaf(bh, dx, ax);
     ay = fmaf(bh, dy, ay);
     float v = 0.f;
-    if (has_src) v += sersic_eval(c + LC_SERSIC0, thx - ax, thy - ay);
-    if (has_l1) v += sersic_eval(c + LC_SERSIC0 + LC_SERSIC_STRIDE, thx, thy);
-    if (has_l2) v += sersic_eval(c + LC_SERSIC0 + 2 * LC_SERSIC_STRIDE, thx, thy);
+    if (has_src) v += light_eval<CH>(kinds, 0, c + LC_SERSIC0, thx - ax, thy - ay);
+    if (has_l1) v += light_eval<CH>(kinds, 1, c + LC_SERSIC0 + LC_SERSIC_STRIDE, thx, thy);
+    if (has_l2) v += light_eval<CH>(kinds, 2, c + LC_SERSIC0 + 2 * LC_SERSIC_STRIDE, thx, thy);
     return v;
 }
 
@@ -131,7 +160,8 @@ static inline __host__ __device__ int lens_tap_pitch(int kpsf) { return (kpsf + 
 static inline __host__ __device__ int lens_halo_left(int kpsf) { return kpsf / 2 + LENS_TAPS; }
 static inline __host__ __device__ int lens_img_pitch(int nx, int kpsf) { return (nx + 2 * (kpsf / 2) + LENS_TAPS + LENS_STRIP - 1) | 1; }
 
-__global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict__ consts, glad_image_grid g,
+template <bool CH>
+__global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict__ consts, int kinds, glad_image_grid g,
                                                          const float* __restrict__ psf, int kpsf,
                                                          const float* __restrict__ data,
                                                          const float* __restrict__ ivar, float* __restrict__ images,
@@ -175,7 +205,7 @@ __global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict
             float thy = fmaf(g.pix, (float)iy + (((float)sb + 0.5f) * inv_s - 0.5f), g.y0);
             for (int sa = 0; sa < ss; ++sa) {
                 float thx = fmaf(g.pix, (float)ix + (((float)sa + 0.5f) * inv_s - 0.5f), g.x0);
-                acc += shoot(c, thx, thy, nterms, has_src, has_l1, has_l2);
+                acc += shoot<CH>(c, thx, thy, nterms, has_src, has_l1, has_l2, kinds);
             }
         }
         img[iy * pitch + HL + ix] = acc * inv_s2;
@@ -242,7 +272,7 @@ __global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict
 
 cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B) {
     ProfScope ps(c, GK_LENS_PREP, c->lens_stream);
-    lens_prep_kernel<<<(B + 31) / 32, 32 * LENS_PREP_ROLES, 0, c->lens_stream>>>(d_params, B, c->d_lens_const);
+    lens_prep_kernel<<<(B + 31) / 32, 32 * LENS_PREP_ROLES, 0, c->lens_stream>>>(d_params, B, c->light_kinds, c->d_lens_const);
     return cudaGetLastError();
 }
 
@@ -250,14 +280,20 @@ cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2
     size_t smem = sizeof(float) * (LC_SIZE + (size_t)c->kpsf * lens_tap_pitch(c->kpsf) +
                                    (size_t)(c->grid.ny + 1) * lens_img_pitch(c->grid.nx, c->kpsf));
     if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
-    static size_t configured = 0;
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(lens_image_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    static size_t configured[2] = {0, 0};
+    const int ch = c->light_kinds != 0;
+    if (smem > configured[ch]) {
+        cudaError_t e = ch ? cudaFuncSetAttribute(lens_image_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+                           : cudaFuncSetAttribute(lens_image_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        configured = smem;
+        configured[ch] = smem;
     }
     ProfScope ps(c, GK_LENS_IMAGE, c->lens_stream);
-    lens_image_kernel<<<B, 512, smem, c->lens_stream>>>(c->d_lens_const, c->grid, c->d_psf, c->kpsf, c->d_data, c->d_ivar,
-                                                  d_images, d_chi2, d_flags);
+    if (ch)
+        lens_image_kernel<true><<<B, 512, smem, c->lens_stream>>>(c->d_lens_const, c->light_kinds, c->grid, c->d_psf, c->kpsf,
+                                                                 c->d_data, c->d_ivar, d_images, d_chi2, d_flags);
+    else
+        lens_image_kernel<false><<<B, 512, smem, c->lens_stream>>>(c->d_lens_const, 0, c->grid, c->d_psf, c->kpsf, c->d_data,
+                                                                  c->d_ivar, d_images, d_chi2, d_flags);
     return cudaGetLastError();
 }
