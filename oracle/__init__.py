@@ -217,7 +217,7 @@ def joint_loglike(chi2_lens, chi2_dyn):
 
 
 # ---- 1-D MGE of a radial profile (Eq. 44-46) ----
-PROFILE_SERSIC, PROFILE_EPL = 0, 1
+PROFILE_SERSIC, PROFILE_EPL, PROFILE_CHAMELEON = 0, 1, 2
 MGE_EULER_P = 12          # reading R-M1 (the paper does not print P)
 
 
@@ -250,9 +250,9 @@ def sigma_crit(Ddt_mpc, Dd_mpc, zd) -> float:
     return float(lib().glad_oracle_sigma_crit(float(Ddt_mpc), float(Dd_mpc), float(zd)))
 
 
-def model_tables(lens, dyn, ddt, zd, n_lum, n_mass, lum_range, mass_range, P=MGE_EULER_P):
+def model_tables(lens, dyn, ddt, zd, n_lum, n_mass, lum_range, mass_range, P=MGE_EULER_P, tracer_kind=PROFILE_SERSIC):
     """The self-consistent joint model of P:406 / Fig. 2 (reading R-M3): from the lens vector and the distances
-    derive (a) the luminous MGE = Eq. 46 of lens-light Sersic #1 (lens[16:20]), (b) the mass MGE = Eq. 46 of
+    derive (a) the luminous MGE = Eq. 46 of lens-light component #1 (lens[16:20]; Sersic, or Chameleon with tracer_kind), (b) the mass MGE = Eq. 46 of
     Sigma_crit * kappa_epl (Eq. 13, B.1-B.3), (c) lens[8] = theta_E,BH^2 from M_BH = dyn[2] (Eq. 4).
     Returns (lens' [B,26] float32, lum [B,n_lum,3] float32, mass [B,n_mass,3] float32): tables rounded to the
     float32 the batch calls take."""
@@ -264,7 +264,7 @@ def model_tables(lens, dyn, ddt, zd, n_lum, n_mass, lum_range, mass_range, P=MGE
     mass = np.empty((B, n_mass, 3), np.float32)
     for b in range(B):
         Ie, Re, n, q = (float(v) for v in lens[b, 16:20])
-        lum[b] = mge1d(PROFILE_SERSIC, [Ie, Re, n, q], n_lum, *lum_range, P=P)
+        lum[b] = mge1d(tracer_kind, [Ie, Re, n, q], n_lum, *lum_range, P=P)   # Chameleon tracer: the slots are {I_0, w_c, w_t, q}
         sc = sigma_crit(float(ddt[b]), float(dyn[b, 1]), zd)
         mass[b] = mge1d(PROFILE_EPL, [sc, float(lens[b, 2]), float(lens[b, 3]), float(lens[b, 4])], n_mass, *mass_range, P=P)
         lens[b, 8] = bh_theta2(float(dyn[b, 2]), float(ddt[b]), zd)

@@ -546,6 +546,10 @@ double glad_oracle_bh_theta2(double Mbh_msun, double Ddt_mpc, double zd) {
 /*           F = I_e exp(-b_n ((z/R_e)^{1/n} - 1))                             */
 /*   kind 1, EPL convergence (Eq. B.1-B.3, r_soft = 0 as in R-L3):             */
 /*           prof = {scale, theta_E, gamma, q},  F = scale (3-gamma)/2 (b/z)^{gamma-1} */
+/*   kind 2, Chameleon (Eq. 47, the paper's I_light):  prof = {I_0, w_c, w_t, q'}          */
+/*           F = I_0/(1+q) [ (z^2 + 4 w_c^2/(1+q)^2)^{-1/2} - (z^2 + 4 w_t^2/(1+q)^2)^{-1/2} ]  */
+/*           exact transform: 1/sqrt(R^2+a) = sqrt(2/pi) int dln(s) s^-1 e^{-a/2s^2} e^{-R^2/2s^2}, */
+/*           so f(sigma) = I_0/(1+q) (2/sigma) (e^{-a_c/2 sigma^2} - e^{-a_t/2 sigma^2})  (pin)    */
 /* Output rows {A_n, sigma_n, q'}.  Returns 0, or -1 on bad arguments.         */
 /* Pins (tests/test_oracle_mge.py): the power law has the closed form          */
 /*   f(sigma) = sqrt(2pi) 2^{1-t/2}/Gamma(t/2) sigma^-t; F = Gaussian of width */
@@ -564,6 +568,11 @@ static double complex mge_profile(int kind, const double* prof, double bn, doubl
     if (kind == 0) {
         double complex w = cpow(z / prof[1], 1.0 / prof[2]);
         return prof[0] * cexp(-bn * (w - 1.0));
+    }
+    if (kind == 2) {   /* Chameleon, Eq. 47: prof = {I_0, w_c, w_t, q} */
+        double opq = 1.0 + prof[3];
+        double ac = 4.0 * prof[1] * prof[1] / (opq * opq), at = 4.0 * prof[2] * prof[2] / (opq * opq);
+        return prof[0] / opq * (1.0 / csqrt(z * z + ac) - 1.0 / csqrt(z * z + at));
     }
     double t = prof[2] - 1.0;
     double b = pow(2.0 / (1.0 + prof[3]), 1.0 / t) * prof[1];        /* Eq. B.3 */
@@ -590,7 +599,7 @@ double glad_oracle_mge_f_sigma(int kind, const double* prof, double sigma, int P
 
 int glad_oracle_mge1d(int kind, const double* prof, int n_gauss, double sigma_lo, double sigma_hi, int P,
                       double* mge /* [n_gauss,3] */) {
-    if ((kind != 0 && kind != 1) || n_gauss < 2 || !(sigma_lo > 0.0) || !(sigma_hi > sigma_lo) || P < 1 || P > 20)
+    if ((kind != 0 && kind != 1 && kind != 2) || n_gauss < 2 || !(sigma_lo > 0.0) || !(sigma_hi > sigma_lo) || P < 1 || P > 20)
         return -1;
     double dln = log(sigma_hi / sigma_lo) / (n_gauss - 1);
     for (int n = 0; n < n_gauss; ++n) {

@@ -100,7 +100,7 @@ def test_rows_layout_weights_and_linearity():
     m2 = oracle.mge1d(oracle.PROFILE_SERSIC, [6.0, 1.2, 3.0, 0.7], 15, 0.05, 20.0)
     assert np.allclose(m2[:, 0], 3.0 * m[:, 0], rtol=1e-12)
     with pytest.raises(ValueError):
-        oracle.mge1d(2, prof, 15, 0.05, 20.0)
+        oracle.mge1d(3, prof, 15, 0.05, 20.0)
     with pytest.raises(ValueError):
         oracle.mge1d(0, prof, 15, 20.0, 0.05)
 
@@ -143,3 +143,22 @@ def test_model_tables_compose_the_joint_model():
     # element 0 is the truth vector with D_dt = 1823: its generator mass table is the same model
     ref = wl["dyn"]["mass_mge"][0]
     assert np.allclose(mass[0, 1:-1, 0], ref[1:-1, 0], rtol=1e-6)
+
+
+def test_chameleon_transform_closed_form():
+    """1/sqrt(R^2 + a) = sqrt(2/pi) int dln(sigma) sigma^-1 exp(-a/2 sigma^2) exp(-R^2/2 sigma^2) (Laplace transform of
+    t^-1/2), so the exact Eq. 44 of the Chameleon (Eq. 47) is f = I_0/(1+q) (2/sigma)(e^{-a_c/2 sigma^2} - e^{-a_t/2 sigma^2}),
+    a = 4 w^2/(1+q)^2.  Absolute accuracy of the Euler sum: ~1e-8 of the profile's scale at that sigma."""
+    for I0, wc, wt, q in ((1.3, 0.1, 0.9, 0.8), (0.2, 0.03, 0.5, 0.6), (2.0, 0.4, 2.5, 1.0)):
+        ac, at = 4 * wc * wc / (1 + q) ** 2, 4 * wt * wt / (1 + q) ** 2
+        for sigma in (0.02, 0.1, 0.5, 2.0, 20.0):
+            exact = I0 / (1 + q) * (2 / sigma) * (math.exp(-ac / (2 * sigma ** 2)) - math.exp(-at / (2 * sigma ** 2)))
+            got = oracle.mge_f_sigma(oracle.PROFILE_CHAMELEON, [I0, wc, wt, q], sigma)
+            assert abs(got - exact) < 3e-8 * I0 / (1 + q) * (2 / sigma), (sigma, got, exact)
+    # summed back (Eq. 46), 21 Gaussians reproduce the profile over the image
+    R = np.geomspace(0.1, 5.0, 100)
+    m = oracle.mge1d(oracle.PROFILE_CHAMELEON, [1.3, 0.1, 0.9, 0.8], 21, 0.02, 50.0)
+    want = np.array([oracle.chameleon(r, 0.0, 1.3, 0.1, 0.9, 0.8, 0.0) for r in R])
+    err = np.abs(_sum_back(m, R) / want - 1.0)
+    assert err.max() < 0.012, err.max()
+    assert np.allclose(m[:, 2], 0.8)
