@@ -182,18 +182,19 @@ glad_status glad_joint_loglike_host(glad_ctx* ctx, const float* h_lens_params, c
  * d_prof [B,GLAD_NPROF] float, one row per vector:
  *   GLAD_PROFILE_SERSIC : {I_e, R_e, n, q'}            F = I_e exp(-b_n ((R/R_e)^(1/n) - 1))        (R-L7)
  *   GLAD_PROFILE_EPL    : {scale, theta_E, gamma, q}   F = scale (3-gamma)/2 (b/R)^(gamma-1), b of Eq. B.3
+ *   GLAD_PROFILE_CHAMELEON : {I_0, w_c, w_t, q'}       F of Eq. 47, the paper's I_light
  * d_mge [B,n_gauss,3] rows {A_n, sigma_n, q'}: the MGE row layout glad_jam_vrms_batch reads (stride 3*n_gauss).
  * fp64 arithmetic, fp32 rows.  Enqueues on the context stream; device pointers owned by the caller.
  * GLAD_EINVAL on a bad kind / range / order, GLAD_ESHAPE if n_gauss > GLAD_MAX_GAUSS.
  */
-typedef enum { GLAD_PROFILE_SERSIC = 0, GLAD_PROFILE_EPL = 1 } glad_profile_kind;
+typedef enum { GLAD_PROFILE_SERSIC = 0, GLAD_PROFILE_EPL = 1, GLAD_PROFILE_CHAMELEON = 2 } glad_profile_kind;
 #define GLAD_NPROF 4
 glad_status glad_mge1d_batch(glad_ctx* ctx, int kind, const float* d_prof, int B, int n_gauss, float sigma_lo,
                              float sigma_hi, int euler_order, float* d_mge);
 
 /*
  * Self-consistent joint model (R-M3; Fig. 2): ONE sampler vector per evaluation.  On the device, per vector:
- *   luminous MGE = Eq. 46 of the lens-light Sersic #1 (lens[16..19] = I_e, R_e, n, q), n_lum Gaussians on
+ *   luminous MGE = Eq. 46 of lens-light component #1 (lens[16..19]; Sersic or Chameleon, glad_set_light_profiles), n_lum Gaussians on
  *                  [lum_sigma_lo, lum_sigma_hi];
  *   mass MGE     = Eq. 46 of Sigma_crit * kappa_epl(theta_E, gamma, q) with Sigma_crit(D_dt, D_d, z_d) of Eq. 13
  *                  (D_d = dyn[1]), n_mass Gaussians on [mass_sigma_lo, mass_sigma_hi] (the paper goes to 50");
@@ -229,8 +230,8 @@ glad_status glad_profile_read(glad_ctx* ctx, double* ms_out /*[GLAD_NKERNELS]*/,
  * Each of the three light components (source, lens light 1, lens light 2) is a Sersic (default) or a Chameleon for the
  * whole batch; a Chameleon component reads its five shape slots as {I_0, w_c, w_t, q, phi} instead of {I_e, R_e, n, q, phi}
  * (source: lens[11..15], lens light: lens[16..20], lens[21..25]); valid iff 0 < w_c < w_t and 0 < q <= 1, I_0 = 0 disables it.
- * Takes effect for the batch calls enqueued afterwards.  The luminous tracer of glad_joint_loglike_model_batch stays the
- * Sersic expansion: that entry returns GLAD_ESTATE while lens light 1 is a Chameleon.
+ * Takes effect for the batch calls enqueued afterwards; glad_joint_loglike_model_batch then expands lens light 1 as a
+ * Chameleon for the luminous tracer (GLAD_PROFILE_CHAMELEON).
  */
 #define GLAD_LIGHT_SERSIC 0
 #define GLAD_LIGHT_CHAMELEON 1

@@ -13,7 +13,7 @@ import torch
 from .build import LIB, build
 
 NLENS, NDYN, NPROF = 26, 4, 4
-PROFILE_SERSIC, PROFILE_EPL = 0, 1
+PROFILE_SERSIC, PROFILE_EPL, PROFILE_CHAMELEON = 0, 1, 2
 LIGHT_SERSIC, LIGHT_CHAMELEON = 0, 1
 FLAG_LENS_INVALID, FLAG_DYN_INVALID, FLAG_BIN_INVALID = 1, 2, 4
 

@@ -419,7 +419,7 @@ glad_status glad_mge1d_batch(glad_ctx* c, int kind, const float* d_prof, int B, 
                              int P, float* d_mge) {
     if (!c) return GLAD_EINVAL;
     if (B < 0 || (B > 0 && (!d_prof || !d_mge))) return fail(c, GLAD_EINVAL, "glad_mge1d_batch: B=%d / null pointer", B);
-    if (kind != GLAD_PROFILE_SERSIC && kind != GLAD_PROFILE_EPL) return fail(c, GLAD_EINVAL, "glad_mge1d_batch: profile kind %d", kind);
+    if (kind != GLAD_PROFILE_SERSIC && kind != GLAD_PROFILE_EPL && kind != GLAD_PROFILE_CHAMELEON) return fail(c, GLAD_EINVAL, "glad_mge1d_batch: profile kind %d", kind);
     if (P == 0) P = MGE_DEFAULT_ORDER;
     if (P < 1 || P > 15) return fail(c, GLAD_EINVAL, "glad_mge1d_batch: Euler order %d outside [1,15]", P);
     glad_status st = mge_check(c, "glad_mge1d_batch", n_gauss, sigma_lo, sigma_hi);
@@ -438,7 +438,6 @@ glad_status glad_joint_loglike_model_batch(glad_ctx* c, const float* d_lens, con
     if (B < 0 || (B > 0 && (!d_lens || !d_dyn || !d_ddt || !d_beta || !d_loglike)))
         return fail(c, GLAD_EINVAL, "glad_joint_loglike_model_batch: B=%d / null pointer", B);
     if (!(zd > -1.f)) return fail(c, GLAD_EINVAL, "glad_joint_loglike_model_batch: z_d = %g", zd);
-    if (c->light_kinds & 2) return fail(c, GLAD_ESTATE, "glad_joint_loglike_model_batch: lens light 1 is a Chameleon, the tracer expansion is Sersic-only");
     glad_status st = mge_check(c, "glad_joint_loglike_model_batch (luminous)", nl, lum_lo, lum_hi);
     if (st != GLAD_OK) return st;
     st = mge_check(c, "glad_joint_loglike_model_batch (mass)", nm, mass_lo, mass_hi);
@@ -451,7 +450,7 @@ glad_status glad_joint_loglike_model_batch(glad_ctx* c, const float* d_lens, con
     float* m_lens = c->d_model;
     float* m_lum = d_lum_out ? d_lum_out : m_lens + n_lens;
     float* m_mass = d_mass_out ? d_mass_out : m_lens + n_lens + n_lum;
-    CU(launch_model(c, d_lens, d_dyn, d_ddt, (double)zd, B, nl, lum_lo, lum_hi, nm, mass_lo, mass_hi, MGE_DEFAULT_ORDER, m_lens,
+    CU(launch_model(c, d_lens, d_dyn, d_ddt, (double)zd, B, (c->light_kinds & 2) ? GLAD_PROFILE_CHAMELEON : GLAD_PROFILE_SERSIC, nl, lum_lo, lum_hi, nm, mass_lo, mass_hi, MGE_DEFAULT_ORDER, m_lens,
                     m_lum, m_mass), "model_kernel");
     return glad_joint_loglike_batch(c, m_lens, d_dyn, B, m_lum, nl, 3L * nl, m_mass, nm, 3L * nm, d_beta, per_gaussian,
                                     d_loglike, d_chi2_lens, d_chi2_dyn, d_flags);

@@ -130,7 +130,7 @@ cudaError_t launch_joint(glad_ctx* c, int B, const float* d_c2l, const float* d_
 cudaError_t launch_kin_weights(glad_ctx* c);
 cudaError_t launch_mge1d(glad_ctx* c, int kind, const float* d_prof, int B, int n_gauss, float sigma_lo, float sigma_hi,
                          int P, float* d_mge);
-cudaError_t launch_model(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, double zd, int B, int n_lum,
+cudaError_t launch_model(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, double zd, int B, int tracer_kind, int n_lum,
                          float lum_lo, float lum_hi, int n_mass, float mass_lo, float mass_hi, int P, float* d_lens_out,
                          float* d_lum, float* d_mass);
 // tensor-core (tcgen05) form of row a6; supported when the folded grid has ny_f <= 128, N = terms * nx_f <= 256

@@ -77,6 +77,12 @@ __device__ static void mge_rows(int kind, double p0, double p1, double p2, doubl
             if (kind == GLAD_PROFILE_SERSIC) {
                 const cplx w = cpow_real({z.re / p1, z.im / p1}, 1.0 / p2);
                 re = p0 * cexp_d({-bn * (w.re - 1.0), -bn * w.im}).re;
+            } else if (kind == GLAD_PROFILE_CHAMELEON) {
+                // Eq. 47 at complex radius: p0/(1+q) [ (z^2 + a_c)^(-1/2) - (z^2 + a_t)^(-1/2) ], a = 4 w^2/(1+q)^2
+                const double opq = 1.0 + qp, ac = 4.0 * p1 * p1 / (opq * opq), at = 4.0 * p2 * p2 / (opq * opq);
+                const cplx z2 = {z.re * z.re - z.im * z.im, 2.0 * z.re * z.im};
+                const cplx ic = cpow_real({z2.re + ac, z2.im}, -0.5), it = cpow_real({z2.re + at, z2.im}, -0.5);
+                re = p0 / opq * (ic.re - it.re);
             } else {
                 const double n2 = z.re * z.re + z.im * z.im;               // b/z = b conj(z)/|z|^2
                 re = p0 * 0.5 * (3.0 - p2) * cpow_real({bepl * z.re / n2, -bepl * z.im / n2}, t).re;   // Eq. B.1
@@ -126,7 +132,7 @@ cudaError_t launch_mge1d(glad_ctx* c, int kind, const float* d_prof, int B, int 
 // R-M3 in one launch: CTA per vector.  Thread 0 derives theta_E,BH^2 (Eq. 4), Sigma_crit (Eq. 13) and the Sersic b_n, the
 // whole CTA copies the lens vector, then all warps expand the lens-light Sersic and Sigma_crit kappa_epl (Eq. 46).
 __global__ void __launch_bounds__(256) model_kernel(const float* __restrict__ lens, const float* __restrict__ dyn,
-                                                    const float* __restrict__ ddt, double zd, int B, int n_lum, double lum_lo,
+                                                    const float* __restrict__ ddt, double zd, int B, int tracer_kind, int n_lum, double lum_lo,
                                                     double lum_dln, int n_mass, double mass_lo, double mass_dln,
                                                     const __grid_constant__ EulerConsts ec, float* __restrict__ lens_out,
                                                     float* __restrict__ lum, float* __restrict__ mass) {
@@ -143,19 +149,19 @@ __global__ void __launch_bounds__(256) model_kernel(const float* __restrict__ le
         // Eq. 13: Sigma_crit = c^2/(4 pi G) D_dt / ((1+z_d) D_d^2)  [Msun/pc^2, distances Mpc -> pc]; rounded to fp32 like a
         // profile row of glad_mge1d_batch
         s_sc = (double)(float)(MGE_C_KMS * MGE_C_KMS / (4.0 * MGE_PI * MGE_G_NEWTON) * (Ddt * 1e6) / ((1.0 + zd) * (Dd * 1e6) * (Dd * 1e6)));
-        s_bn = sersic_bn((double)L[18]);
+        s_bn = tracer_kind == GLAD_PROFILE_SERSIC ? sersic_bn((double)L[18]) : 0.0;
     }
     __syncthreads();
-    mge_rows(GLAD_PROFILE_SERSIC, L[16], L[17], L[18], L[19], s_bn, ec, n_lum, lum_lo, lum_dln, lum + (size_t)b * n_lum * 3);
+    mge_rows(tracer_kind, L[16], L[17], L[18], L[19], s_bn, ec, n_lum, lum_lo, lum_dln, lum + (size_t)b * n_lum * 3);
     mge_rows(GLAD_PROFILE_EPL, s_sc, L[2], L[3], L[4], 0.0, ec, n_mass, mass_lo, mass_dln, mass + (size_t)b * n_mass * 3);
 }
 
-cudaError_t launch_model(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, double zd, int B, int n_lum,
+cudaError_t launch_model(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, double zd, int B, int tracer_kind, int n_lum,
                          float lum_lo, float lum_hi, int n_mass, float mass_lo, float mass_hi, int P, float* d_lens_out,
                          float* d_lum, float* d_mass) {
     ProfScope ps(c, GK_MGE);
     const double ldln = log((double)lum_hi / (double)lum_lo) / (n_lum - 1), mdln = log((double)mass_hi / (double)mass_lo) / (n_mass - 1);
-    model_kernel<<<B, 256, 0, c->stream>>>(d_lens, d_dyn, d_ddt, zd, B, n_lum, (double)lum_lo, ldln, n_mass, (double)mass_lo, mdln,
+    model_kernel<<<B, 256, 0, c->stream>>>(d_lens, d_dyn, d_ddt, zd, B, tracer_kind, n_lum, (double)lum_lo, ldln, n_mass, (double)mass_lo, mdln,
                                            euler_consts(P), d_lens_out, d_lum, d_mass);
     return cudaGetLastError();
 }

@@ -86,8 +86,43 @@ def test_chameleon_validity_and_errors(glad_mod, oracle):
     assert np.isinf(out["chi2"].cpu().numpy()[1:3]).all()
     with pytest.raises(glad_mod.GladError):
         g.set_light_profiles(0, 2, 0)
-    D = workloads.make_workload("C1", None)["dyn"]
-    g.set_kin_data(D["kin"])
-    with pytest.raises(glad_mod.GladError):     # the tracer expansion of the model entry is Sersic-only
-        g.joint_loglike_model_batch(p[:4], D["params"][:4], np.full(4, 1823.0, np.float32), 0.295, 10, (0.02, 10.0), 10, (0.02, 50.0), D["beta"][:4])
+    g.close()
+
+
+def test_joint_model_with_chameleon_tracer(glad_mod, oracle):
+    """the paper decomposes I_light (Chameleons) into Gaussians for the dynamics.  With lens light 1 switched to a
+    Chameleon the self-consistent entry expands it (GLAD_PROFILE_CHAMELEON) as the luminous tracer."""
+    B = 10
+    wl = chameleon_workload(B, False)
+    L = wl["lens"]
+    p = L["params"].copy()
+    p[:, 21] = 0.0                                   # one Chameleon = the tracer; lens light 2 off
+    p[:, 19] = p[:, 4]
+    D = workloads.make_workload("C2", None, B=B)["dyn"]
+    kinds = [0, 1, 0]
+    lum_range, mass_range = (0.02, 10.0), (0.02, 50.0)
+    l2, lum, mass = oracle.model_tables(p, D["params"], wl["ddt"], wl["z_d"], 16, 20, lum_range, mass_range,
+                                        tracer_kind=oracle.PROFILE_CHAMELEON)
+    img = oracle.lens_image_batch(l2[:1], L["grid"], L["psf"], kinds=kinds)["images"][0]
+    vr = oracle.jam_vrms_batch(D["params"][:1], lum[:1], mass[:1], D["beta"][:1], D["kin"])["vrms"][0]
+    nrng = np.random.default_rng(5)
+    data = (img + nrng.normal(0, 0.01, img.shape)).astype(np.float32)
+    ivar = np.full(img.shape, 1e4, np.float32)
+    kin = dict(D["kin"])
+    kin["vrms_obs"] = (vr * (1 + nrng.normal(0, 0.02, vr.shape))).astype(np.float32)
+    kin["vrms_ivar"] = (1.0 / (0.02 * vr) ** 2).astype(np.float32)
+    g = glad_mod.Glad(0)
+    g.set_image_data(L["grid"], L["psf"], data, ivar)
+    g.set_kin_data(kin)
+    g.set_light_profiles(*kinds)
+    out = g.joint_loglike_model_batch(p, D["params"], wl["ddt"], wl["z_d"], 16, lum_range, 20, mass_range, D["beta"], want_tables=True)
+    got = out["lum_mge"].cpu().numpy().astype(np.float64)
+    peak = np.abs(lum[:, :, 0]).max(axis=1, keepdims=True)
+    assert (np.abs(got[:, :, 0] - lum[:, :, 0]) <= 3e-7 * np.abs(lum[:, :, 0]) + 1e-9 * peak).all()
+    ol = oracle.lens_image_batch(l2, L["grid"], L["psf"], data, ivar, want_images=False, kinds=kinds)
+    od = oracle.jam_vrms_batch(D["params"], lum, mass, D["beta"], kin)
+    ref = oracle.joint_loglike(ol["chi2"], od["chi2"])
+    ll = out["loglike"].cpu().numpy().astype(np.float64)
+    assert np.isfinite(ref).all() and (out["flags"].cpu().numpy() == 0).all()
+    assert np.max(np.abs(ll - ref) / np.abs(ref)) < 1e-5, (ll, ref)
     g.close()
