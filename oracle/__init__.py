@@ -79,6 +79,13 @@ def lib():
         L.glad_oracle_mge1d.argtypes = [i, dp, i, d, d, i, dp]
         L.glad_oracle_sigma_crit.restype = d
         L.glad_oracle_sigma_crit.argtypes = [d, d, d]
+        L.glad_oracle_potential.restype = d
+        L.glad_oracle_potential.argtypes = [dp, d, d]
+        L.glad_oracle_hessian.restype = None
+        L.glad_oracle_hessian.argtypes = [dp, d, d, dp]
+        L.glad_oracle_tdelay_const.restype = d
+        L.glad_oracle_quasar_batch.restype = i
+        L.glad_oracle_quasar_batch.argtypes = [fp, fp, i, i, dp, dp, i, dp, dp, dp, dp, dp, dp, dp, dp]
         _lib = L
     return _lib
 
@@ -269,3 +276,47 @@ def model_tables(lens, dyn, ddt, zd, n_lum, n_mass, lum_range, mass_range, P=MGE
         mass[b] = mge1d(PROFILE_EPL, [sc, float(lens[b, 2]), float(lens[b, 3]), float(lens[b, 4])], n_mass, *mass_range, P=P)
         lens[b, 8] = bh_theta2(float(dyn[b, 2]), float(ddt[b]), zd)
     return lens, lum, mass
+
+
+# ---- SURVEY.md 8(f) rank 4 (quasar part): image-position and time-delay chi^2 (Eq. 35-36) ----
+def potential(params, thx, thy) -> float:
+    """psi(theta) of EPL + shear + point mass (readings R-Q4)."""
+    p = np.ascontiguousarray(params, dtype=np.float64)
+    assert p.size == NLENS
+    return float(lib().glad_oracle_potential(_ptr(p, C.c_double), float(thx), float(thy)))
+
+
+def hessian(params, thx, thy):
+    """(psi_xx, psi_xy, psi_yy) at theta."""
+    p = np.ascontiguousarray(params, dtype=np.float64)
+    assert p.size == NLENS
+    h = np.empty(3, np.float64)
+    lib().glad_oracle_hessian(_ptr(p, C.c_double), float(thx), float(thy), _ptr(h, C.c_double))
+    return h
+
+
+def tdelay_const() -> float:
+    """days per (Mpc arcsec^2)."""
+    return float(lib().glad_oracle_tdelay_const())
+
+
+def quasar_batch(lens, ddt, qso):
+    """qso = dict(theta [n_img,2], sigma_theta [n_img], ref, dt_obs [n_img], sigma_dt [n_img]) (float64).
+    Returns dict(chi2_img, chi2_tmd [B]; theta_pre [B,n_img,2]; dt_pre [B,n_img]; beta [B,2]; last_step [B,n_img])."""
+    lens = _f32(lens).reshape(-1, NLENS)
+    ddt = _f32(ddt).reshape(-1)
+    B = lens.shape[0]
+    assert ddt.size == B
+    f = lambda a: np.ascontiguousarray(a, dtype=np.float64)
+    th, st, dt, sd = f(qso["theta"]).reshape(-1, 2), f(qso["sigma_theta"]), f(qso["dt_obs"]), f(qso["sigma_dt"])
+    n = th.shape[0]
+    assert st.size == n and dt.size == n and sd.size == n
+    out = {"chi2_img": np.empty(B), "chi2_tmd": np.empty(B), "theta_pre": np.empty((B, n, 2)),
+           "dt_pre": np.empty((B, n)), "beta": np.empty((B, 2)), "last_step": np.empty((B, n))}
+    P = lambda a: _ptr(a, C.c_double)
+    rc = lib().glad_oracle_quasar_batch(_ptr(lens, C.c_float), _ptr(ddt, C.c_float), B, n, P(th), P(st), int(qso["ref"]),
+                                        P(dt), P(sd), P(out["chi2_img"]), P(out["chi2_tmd"]), P(out["theta_pre"]),
+                                        P(out["dt_pre"]), P(out["beta"]), P(out["last_step"]))
+    if rc != 0:
+        raise ValueError("oracle: bad quasar arguments")
+    return out

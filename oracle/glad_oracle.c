@@ -523,6 +523,170 @@ double glad_oracle_bh_theta2(double Mbh_msun, double Ddt_mpc, double zd) {
 }
 
 /* ------------------------------------------------------------------------ */
+/* SURVEY.md 8(f) rank 4 (quasar part): image-position and time-delay chi^2,  */
+/* Eq. 35-36, built on the Fermat potential of Eq. 1-4. */
+/* The paper prints neither psi nor the Jacobian of the models; both follow   */
+/* from its convergence (App. B) -- DESIGN.md readings R-Q1..R-Q5:            */
+/*   EPL: kappa = (3-gamma)/2 (b/R)^(gamma-1) is homogeneous of degree -t      */
+/*        (t = gamma-1), hence psi of degree 2-t and alpha of degree 1-t, so   */
+/*        (Euler's theorem)  psi = (x alpha_x + y alpha_y)/(2-t)               */
+/*        and, with z = x+iy, alpha = alpha_x + i alpha_y, kappa = d(alpha)/dz,*/
+/*        gamma_c = d(alpha)/d(conj z):  z kappa + conj(z) gamma_c = (1-t) alpha*/
+/*        => gamma_1 + i gamma_2 = [(1-t) alpha z - kappa z^2]/|z|^2 ;         */
+/*        psi_xx = kappa+gamma_1, psi_yy = kappa-gamma_1, psi_xy = gamma_2.    */
+/*   shear (Eq. 49): psi = gamma_ext/2 r^2 cos 2(phi - phi_ext).         */
+/*   point mass: psi = theta_E,BH^2 ln r.                              */
+/* ------------------------------------------------------------------------ */
+
+/* psi(theta) of EPL + shear + point mass; p = lens vector (first 9 entries used) */
+double glad_oracle_potential(const double* p, double thx, double thy) {
+    double dx = thx - p[0], dy = thy - p[1];
+    double c = cos(p[5]), s = sin(p[5]);
+    double xl = dx * c + dy * s, yl = -dx * s + dy * c;
+    double axl, ayl;
+    glad_oracle_epl_alpha(xl, yl, p[2], p[3], p[4], &axl, &ayl);
+    double psi = (xl * axl + yl * ayl) / (3.0 - p[3]);
+    double c2 = cos(2.0 * p[7]), s2 = sin(2.0 * p[7]);
+    psi += 0.5 * p[6] * ((dx * dx - dy * dy) * c2 + 2.0 * dx * dy * s2);
+    double r2 = dx * dx + dy * dy;
+    if (r2 < 1e-12) r2 = 1e-12;
+    psi += 0.5 * p[8] * log(r2);
+    return psi;
+}
+
+/* Hessian of psi: h[0] = psi_xx, h[1] = psi_xy, h[2] = psi_yy (sky frame) */
+void glad_oracle_hessian(const double* p, double thx, double thy, double* h) {
+    double dx = thx - p[0], dy = thy - p[1];
+    double c = cos(p[5]), s = sin(p[5]);
+    double xl = dx * c + dy * s, yl = -dx * s + dy * c;
+    double hxx = 0.0, hxy = 0.0, hyy = 0.0;
+    if (p[2] != 0.0) {
+        double t = p[3] - 1.0, q = p[4];
+        double axl, ayl;
+        glad_oracle_epl_alpha(xl, yl, p[2], p[3], q, &axl, &ayl);
+        double b = pow(2.0 / (1.0 + q), 1.0 / t) * p[2];          /* Eq. B.3 */
+        double R2 = xl * xl + yl * yl / (q * q);                   /* Eq. B.2 */
+        if (q * q * R2 < 1e-12) R2 = 1e-12 / (q * q);
+        double kappa = 0.5 * (2.0 - t) * pow(b * b / R2, 0.5 * t); /* Eq. B.1 */
+        double complex z = xl + I * yl;
+        double r2 = xl * xl + yl * yl;
+        if (r2 < 1e-12) r2 = 1e-12;
+        double complex g = ((1.0 - t) * (axl + I * ayl) * z - kappa * z * z) / r2;
+        double lxx = kappa + creal(g), lyy = kappa - creal(g), lxy = cimag(g);
+        /* rotate the lens-frame tensor back by +phi_PA: H = R L R^T */
+        hxx = c * c * lxx - 2.0 * c * s * lxy + s * s * lyy;
+        hyy = s * s * lxx + 2.0 * c * s * lxy + c * c * lyy;
+        hxy = c * s * (lxx - lyy) + (c * c - s * s) * lxy;
+    }
+    double c2 = cos(2.0 * p[7]), s2 = sin(2.0 * p[7]);
+    hxx += p[6] * c2;
+    hyy -= p[6] * c2;
+    hxy += p[6] * s2;
+    double r2 = dx * dx + dy * dy;
+    if (r2 < 1e-12) r2 = 1e-12;
+    hxx += p[8] * (dy * dy - dx * dx) / (r2 * r2);
+    hyy -= p[8] * (dy * dy - dx * dx) / (r2 * r2);
+    hxy -= 2.0 * p[8] * dx * dy / (r2 * r2);
+    h[0] = hxx; h[1] = hxy; h[2] = hyy;
+}
+
+/* days per (Mpc arcsec^2): D_dt/c of Eq. 3-4 with theta in arcsec and Delta t in days (R-Q5) */
+double glad_oracle_tdelay_const(void) {
+    const double mpc_m = 3.0856775814913673e22, c_ms = 299792458.0, day_s = 86400.0;
+    double arcsec = PI / 648000.0;
+    return mpc_m / c_ms / day_s * arcsec * arcsec;
+}
+
+#define ORACLE_MAX_QIMG 8
+/*
+ * chi^2_img (Eq. 35) and chi^2_tmd (Eq. 36) for B lens vectors, following P:253 step by step:
+ *   1. beta_i = theta_i - alpha(theta_i)                                     (Eq. 33)
+ *   2. mu_i = 1/det(I - Hessian psi(theta_i));  beta_bar = sum |mu_i| beta_i / sum |mu_i|   (R-Q1)
+ *   3. theta_i^pre = the solution of theta - alpha(theta) = beta_bar reached by Newton's method from
+ *      theta_i with the Jacobian A = I - Hessian psi, NEWTON_STEPS full steps                (R-Q2)
+ *   4. chi2_img = sum_i |theta_i - theta_i^pre|^2 / sigma_theta,i^2
+ *   5. phi_i = |theta_i^pre - beta_bar|^2/2 - psi(theta_i^pre)  (Eq. 2);
+ *      dt_i^pre = K D_dt (phi_i - phi_ref)  (Eq. 3-4; R-Q3: at the predicted positions);
+ *      chi2_tmd = sum_{i != ref, sigma_dt,i > 0} (dt_obs,i - dt_i^pre)^2 / sigma_dt,i^2
+ *   lens [B,26] float32 (entries 0..8 used); ddt [B] float32 Mpc; theta_obs [n_img,2], sigma_theta [n_img],
+ *   dt_obs, sigma_dt [n_img] (entry ref ignored; sigma_dt <= 0 = no measurement) double.
+ * Outputs (may be NULL): chi2_img, chi2_tmd [B]; theta_pre [B,n_img,2]; dt_pre [B,n_img]; beta_bar [B,2];
+ * last_step [B,n_img] = length of the last Newton step (how converged step 3 is).
+ * Invalid mass parameters (theta_E < 0, gamma outside (1,3), q outside (0,1]) -> chi2 = +inf, outputs NaN.
+ */
+#define NEWTON_STEPS 12
+int glad_oracle_quasar_batch(const float* lens, const float* ddt, int B, int n_img, const double* theta_obs,
+                             const double* sigma_theta, int ref, const double* dt_obs, const double* sigma_dt,
+                             double* chi2_img, double* chi2_tmd, double* theta_pre, double* dt_pre,
+                             double* beta_bar, double* last_step) {
+    if (n_img < 1 || n_img > ORACLE_MAX_QIMG || ref < 0 || ref >= n_img) return -1;
+    const double K = glad_oracle_tdelay_const();
+#pragma omp parallel for schedule(dynamic)
+    for (int b = 0; b < B; ++b) {
+        double p[ORACLE_NLENS];
+        for (int k = 0; k < ORACLE_NLENS; ++k) p[k] = (double)lens[(size_t)b * ORACLE_NLENS + k];
+        int ok = (p[2] >= 0.0) && (p[3] > 1.0) && (p[3] < 3.0) && (p[4] > 0.0) && (p[4] <= 1.0) && (p[8] >= 0.0);
+        if (!ok) {
+            if (chi2_img) chi2_img[b] = INFINITY;
+            if (chi2_tmd) chi2_tmd[b] = INFINITY;
+            for (int i = 0; i < n_img; ++i) {
+                if (theta_pre) { theta_pre[((size_t)b * n_img + i) * 2] = NAN; theta_pre[((size_t)b * n_img + i) * 2 + 1] = NAN; }
+                if (dt_pre) dt_pre[(size_t)b * n_img + i] = NAN;
+                if (last_step) last_step[(size_t)b * n_img + i] = NAN;
+            }
+            if (beta_bar) { beta_bar[2 * b] = NAN; beta_bar[2 * b + 1] = NAN; }
+            continue;
+        }
+        /* steps 1-2 */
+        double bx = 0.0, by = 0.0, wsum = 0.0;
+        for (int i = 0; i < n_img; ++i) {
+            double tx = theta_obs[2 * i], ty = theta_obs[2 * i + 1], ax, ay, h[3];
+            glad_oracle_deflection(p, tx, ty, &ax, &ay);
+            glad_oracle_hessian(p, tx, ty, h);
+            double det = (1.0 - h[0]) * (1.0 - h[2]) - h[1] * h[1];
+            double w = fabs(1.0 / det);
+            bx += w * (tx - ax);
+            by += w * (ty - ay);
+            wsum += w;
+        }
+        bx /= wsum;
+        by /= wsum;
+        if (beta_bar) { beta_bar[2 * b] = bx; beta_bar[2 * b + 1] = by; }
+        /* steps 3-5 */
+        double phi[ORACLE_MAX_QIMG], c2i = 0.0;
+        for (int i = 0; i < n_img; ++i) {
+            double tx = theta_obs[2 * i], ty = theta_obs[2 * i + 1], step = 0.0;
+            for (int it = 0; it < NEWTON_STEPS; ++it) {
+                double ax, ay, h[3];
+                glad_oracle_deflection(p, tx, ty, &ax, &ay);
+                glad_oracle_hessian(p, tx, ty, h);
+                double fx = tx - ax - bx, fy = ty - ay - by;          /* lens equation residual */
+                double a11 = 1.0 - h[0], a12 = -h[1], a22 = 1.0 - h[2];
+                double det = a11 * a22 - a12 * a12;
+                double sx = (a22 * fx - a12 * fy) / det, sy = (-a12 * fx + a11 * fy) / det;
+                tx -= sx;
+                ty -= sy;
+                step = sqrt(sx * sx + sy * sy);
+            }
+            if (theta_pre) { theta_pre[((size_t)b * n_img + i) * 2] = tx; theta_pre[((size_t)b * n_img + i) * 2 + 1] = ty; }
+            if (last_step) last_step[(size_t)b * n_img + i] = step;
+            double ex = theta_obs[2 * i] - tx, ey = theta_obs[2 * i + 1] - ty;
+            c2i += (ex * ex + ey * ey) / (sigma_theta[i] * sigma_theta[i]);
+            phi[i] = 0.5 * ((tx - bx) * (tx - bx) + (ty - by) * (ty - by)) - glad_oracle_potential(p, tx, ty);
+        }
+        double c2t = 0.0;
+        for (int i = 0; i < n_img; ++i) {
+            double dt = K * (double)ddt[b] * (phi[i] - phi[ref]);
+            if (dt_pre) dt_pre[(size_t)b * n_img + i] = dt;
+            if (i != ref && sigma_dt[i] > 0.0) c2t += (dt_obs[i] - dt) * (dt_obs[i] - dt) / (sigma_dt[i] * sigma_dt[i]);
+        }
+        if (chi2_img) chi2_img[b] = c2i;
+        if (chi2_tmd) chi2_tmd[b] = c2t;
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------ */
 /* 1-D multi-Gaussian expansion of a radial profile    */
 /* (Eq. 44-46, "following Shajib (2019)"), the step between the    */
 /* two halves of the joint model ("we decompose I_light and Sigma_int  */
