@@ -67,6 +67,7 @@ typedef enum {
 #define GLAD_MAX_SKY 256            /* nx, ny of the kinematic grid */
 #define GLAD_MAX_NODES 1024
 #define GLAD_MAX_BINS 1024
+#define GLAD_MAX_QIMG 8             /* lensed quasar images */
 
 /* Create a context on `device` whose work is enqueued on `cuda_stream` (a cudaStream_t, borrowed;
  * NULL = the legacy default stream).  Returns GLAD_ECUDA if the device is not sm_100. */
@@ -218,9 +219,9 @@ double glad_bh_theta2(double mbh_msun, double ddt_mpc, double z_d);
  * Optional per-kernel timing for bench.py's roofline line: when enabled, a CUDA event pair is recorded on the
  * context stream around every kernel launch (at most 2048 launches between reads).  glad_profile_read
  * SYNCHRONISES the stream, adds the elapsed times to per-kernel totals, copies them out and clears them.
- * Kernel order: 0 lens_prep, 1 lens_image, 2 jam_prep, 3 jam_quad, 4 jam_post, 5 joint, 6 mge (mge1d / model kernel).
+ * Kernel order: 0 lens_prep, 1 lens_image, 2 jam_prep, 3 jam_quad, 4 jam_post, 5 joint, 6 mge (mge1d / model kernel), 7 quasar.
  */
-#define GLAD_NKERNELS 7
+#define GLAD_NKERNELS 8
 glad_status glad_profile_enable(glad_ctx* ctx, int on);
 glad_status glad_profile_read(glad_ctx* ctx, double* ms_out /*[GLAD_NKERNELS]*/, long* count_out /*[GLAD_NKERNELS]*/);
 
@@ -245,6 +246,46 @@ glad_status glad_set_light_profiles(glad_ctx* ctx, int source_kind, int lens1_ki
  * Returns GLAD_ESTATE if the side stream could not be created.
  */
 glad_status glad_set_overlap(glad_ctx* ctx, int on);
+
+/*
+ * SURVEY 8(f) rank 4, quasar part: the image-position and time-delay terms of Eq. 53.  The paper keeps them on the
+ * CPU; in a batched sampler they are one more per-vector reduction over the same mass parameters.
+ *
+ * glad_set_quasar_data: HOST pointers, copied into the context (n_img = 0 clears).  h_theta [n_img,2] observed image positions
+ * (x, y) in arcsec, same frame as the image grid; h_sigma_theta [n_img] > 0 positional uncertainties; ref_image = index of the
+ * reference image j of Eq. 36; h_dt_obs [n_img] observed delays Delta t_ij in DAYS relative to the reference image (its own
+ * entry is ignored) and h_sigma_dt [n_img] their uncertainties (<= 0 = that delay is not measured); both NULL = no delays.
+ * GLAD_ESHAPE if n_img > GLAD_MAX_QIMG.
+ *
+ * glad_quasar_chi2_batch, per vector (mass parameters lens[0..8] only; DESIGN.md R-Q1..R-Q5), all arithmetic fp64:
+ *   beta_i = theta_i - alpha(theta_i) (Eq. 33); mu_i = 1/det(I - Hessian psi(theta_i));
+ *   beta_bar = sum |mu_i| beta_i / sum |mu_i|  ("magnification-weighted average");
+ *   theta_i^pre = image of beta_bar reached from theta_i by 12 Newton steps on the lens equation ("map it back");
+ *   chi2_img = sum_i |theta_i - theta_i^pre|^2 / sigma_theta,i^2                                            (Eq. 35)
+ *   dt_i^pre = (D_dt/c) [phi(theta_i^pre, beta_bar) - phi(theta_ref^pre, beta_bar)], phi = |theta-beta|^2/2 - psi(theta)
+ *                                                                                       (Eq. 2-4), in days;
+ *   chi2_tmd = sum_{i != ref} (dt_obs,i - dt_i^pre)^2 / sigma_dt,i^2                                        (Eq. 36)
+ *   d_lens_params [B,GLAD_NLENS]; d_ddt [B] time-delay distances in Mpc; outputs (device, any may be NULL):
+ *   d_chi2_img, d_chi2_tmd [B] float; d_theta_pre [B,n_img,2], d_dt_pre [B,n_img], d_beta [B,2] DOUBLE.
+ *   An invalid mass model (GLAD_FLAG_LENS_INVALID conditions on lens[2..4], lens[8]) gives chi2 = +INFINITY, NaN elsewhere.
+ * GLAD_ESTATE if no quasar data is set.
+ */
+glad_status glad_set_quasar_data(glad_ctx* ctx, int n_img, const double* h_theta, const double* h_sigma_theta, int ref_image,
+                                 const double* h_dt_obs, const double* h_sigma_dt);
+glad_status glad_quasar_chi2_batch(glad_ctx* ctx, const float* d_lens_params, const float* d_ddt, int B, float* d_chi2_img,
+                                   float* d_chi2_tmd, double* d_theta_pre, double* d_dt_pre, double* d_beta);
+
+/*
+ * glad_joint_loglike_model_batch plus the quasar terms: lnL = -(chi2_L + chi2_D + chi2_img + chi2_tmd)/2, every term of
+ * Eq. 53 with the pixel chi2 standing for the extended-source evidence (R-J1).  The quasar kernel reads the derived
+ * lens vector (lens[8] = theta_E,BH^2 of M_BH and D_dt) and runs on the lens half's stream.  d_chi2_img, d_chi2_tmd [B] or NULL.
+ */
+glad_status glad_joint_loglike_full_batch(glad_ctx* ctx, const float* d_lens_params, const float* d_dyn_params,
+                                          const float* d_ddt, float z_d, int B, int n_lum, float lum_sigma_lo,
+                                          float lum_sigma_hi, int n_mass, float mass_sigma_lo, float mass_sigma_hi,
+                                          const float* d_beta, int beta_per_gaussian, float* d_loglike,
+                                          float* d_chi2_lens, float* d_chi2_dyn, float* d_chi2_img, float* d_chi2_tmd,
+                                          int32_t* d_flags);
 
 /* Number of kernel launches enqueued by this context since creation (for bench.py's gpu_launches). */
 long glad_launch_count(const glad_ctx* ctx);

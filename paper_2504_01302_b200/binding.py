@@ -21,7 +21,8 @@ _lib = None
 EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "glad_set_image_data",
            "glad_set_kin_data", "glad_lens_image_batch", "glad_jam_vrms_batch", "glad_joint_loglike_batch",
            "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count", "glad_profile_enable",
-           "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch", "glad_set_overlap", "glad_set_light_profiles"]
+           "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch", "glad_set_overlap", "glad_set_light_profiles",
+           "glad_set_quasar_data", "glad_quasar_chi2_batch", "glad_joint_loglike_full_batch"]
 
 
 class GladError(RuntimeError):
@@ -82,6 +83,14 @@ def load(rebuild: bool = False):
     L.glad_set_light_profiles.argtypes = [vp, i, i, i]
     L.glad_set_overlap.restype = i
     L.glad_set_overlap.argtypes = [vp, i]
+    dp = C.POINTER(C.c_double)
+    L.glad_set_quasar_data.restype = i
+    L.glad_set_quasar_data.argtypes = [vp, i, dp, dp, i, dp, dp]
+    L.glad_quasar_chi2_batch.restype = i
+    L.glad_quasar_chi2_batch.argtypes = [vp, vp, vp, i, vp, vp, vp, vp, vp]
+    L.glad_joint_loglike_full_batch.restype = i
+    L.glad_joint_loglike_full_batch.argtypes = [vp, vp, vp, vp, C.c_float, i, i, C.c_float, C.c_float, i, C.c_float,
+                                                C.c_float, vp, i, vp, vp, vp, vp, vp, vp]
     L.glad_launch_count.restype = l
     L.glad_launch_count.argtypes = [vp]
     _lib = L
@@ -143,7 +152,7 @@ class Glad:
     def launch_count(self) -> int:
         return int(self.lib.glad_launch_count(self.ctx))
 
-    KERNELS = ("lens_prep", "lens_image", "jam_prep", "jam_quad", "jam_post", "joint", "mge")
+    KERNELS = ("lens_prep", "lens_image", "jam_prep", "jam_quad", "jam_post", "joint", "mge", "quasar")
 
     def set_light_profiles(self, source=0, lens1=0, lens2=0):
         """0 = Sersic, 1 = Chameleon (Eq. 47) per light component, for the batch calls that follow."""
@@ -274,3 +283,51 @@ class Glad:
             float(mass_range[0]), float(mass_range[1]), _p(bt), 1 if bt.dim() == 2 else 0, _p(ll), _p(c2l), _p(c2d), _p(fl),
             _p(lum), _p(mass)))
         return {"loglike": ll, "chi2_lens": c2l, "chi2_dyn": c2d, "flags": fl, "lum_mge": lum, "mass_mge": mass}
+
+    # ---- quasar terms (Eq. 35-36) --------------------------------------------------------------
+    def set_quasar_data(self, qso: dict | None):
+        """qso = dict(theta [n_img,2], sigma_theta [n_img], ref, dt_obs [n_img] days, sigma_dt [n_img]) host arrays; None clears."""
+        if qso is None:
+            self._check(self.lib.glad_set_quasar_data(self.ctx, 0, None, None, 0, None, None))
+            self.n_img = 0
+            return
+        f = lambda a: None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+        th, st, dt, sd = f(qso["theta"]), f(qso["sigma_theta"]), f(qso.get("dt_obs")), f(qso.get("sigma_dt"))
+        n = th.size // 2
+        if st.size != n or (dt is not None and (dt.size != n or sd is None or sd.size != n)):
+            raise GladError("quasar arrays differ in length")
+        P = lambda a: None if a is None else a.ctypes.data_as(C.POINTER(C.c_double))
+        self._check(self.lib.glad_set_quasar_data(self.ctx, n, P(th), P(st), int(qso["ref"]), P(dt), P(sd)))
+        self.n_img = n
+
+    def quasar_chi2_batch(self, lens_params, ddt, want_details=True):
+        p = _dev(lens_params, torch.float32, self.device).reshape(-1, NLENS)
+        dt = _dev(ddt, torch.float32, self.device).reshape(-1)
+        B = p.shape[0]
+        if dt.shape[0] != B:
+            raise GladError("lens and ddt batches differ")
+        n = getattr(self, "n_img", 0)
+        c2i = torch.empty(B, dtype=torch.float32, device=self.device)
+        c2t = torch.empty(B, dtype=torch.float32, device=self.device)
+        mk = lambda *shape: torch.empty(shape, dtype=torch.float64, device=self.device) if want_details else None
+        tp, dp, bb = mk(B, n, 2), mk(B, n), mk(B, 2)
+        self._check(self.lib.glad_quasar_chi2_batch(self.ctx, _p(p), _p(dt), B, _p(c2i), _p(c2t), _p(tp), _p(dp), _p(bb)))
+        return {"chi2_img": c2i, "chi2_tmd": c2t, "theta_pre": tp, "dt_pre": dp, "beta": bb}
+
+    def joint_loglike_full_batch(self, lens_params, dyn_params, ddt, z_d, n_lum, lum_range, n_mass, mass_range, beta, out=None):
+        p = _dev(lens_params, torch.float32, self.device).reshape(-1, NLENS)
+        d = _dev(dyn_params, torch.float32, self.device).reshape(-1, NDYN)
+        dt = _dev(ddt, torch.float32, self.device).reshape(-1)
+        bt = _dev(beta, torch.float32, self.device)
+        B = p.shape[0]
+        if d.shape[0] != B or dt.shape[0] != B:
+            raise GladError("lens, dyn and ddt batches differ")
+        out = out or {}
+        mk = lambda n, ty: out.get(n) if out.get(n) is not None else torch.empty(B, dtype=ty, device=self.device)
+        ll, c2l, c2d, fl = mk("loglike", torch.float32), mk("chi2_lens", torch.float32), mk("chi2_dyn", torch.float32), mk("flags", torch.int32)
+        c2i, c2t = mk("chi2_img", torch.float32), mk("chi2_tmd", torch.float32)
+        self._check(self.lib.glad_joint_loglike_full_batch(
+            self.ctx, _p(p), _p(d), _p(dt), float(z_d), B, int(n_lum), float(lum_range[0]), float(lum_range[1]), int(n_mass),
+            float(mass_range[0]), float(mass_range[1]), _p(bt), 1 if bt.dim() == 2 else 0, _p(ll), _p(c2l), _p(c2d), _p(c2i),
+            _p(c2t), _p(fl)))
+        return {"loglike": ll, "chi2_lens": c2l, "chi2_dyn": c2d, "chi2_img": c2i, "chi2_tmd": c2t, "flags": fl}

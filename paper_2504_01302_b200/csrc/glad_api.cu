@@ -99,7 +99,7 @@ void glad_destroy(glad_ctx* c) {
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     free_kin(c);
-    void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage, c->d_model};
+    void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage, c->d_model, c->d_qtmp};
     for (void* p : ps) if (p) cudaFree(p);
     for (cudaEvent_t e : c->prof_ev) if (e) cudaEventDestroy(e);
     delete c;
@@ -328,14 +328,13 @@ glad_status glad_jam_vrms_batch(glad_ctx* c, const float* d_dyn, int B, const fl
                     d_v2map, d_flags);
 }
 
-glad_status glad_joint_loglike_batch(glad_ctx* c, const float* d_lens, const float* d_dyn, int B, const float* d_lum, int nl,
-                                     long lum_stride, const float* d_mass, int nm, long mass_stride, const float* d_beta,
-                                     int per_gaussian, float* d_loglike, float* d_chi2_lens, float* d_chi2_dyn,
-                                     int32_t* d_flags) {
-    if (!c) return GLAD_EINVAL;
-    if (B < 0 || (B > 0 && (!d_lens || !d_dyn || !d_loglike))) return fail(c, GLAD_EINVAL, "glad_joint_loglike_batch: B=%d / null pointer", B);
-    if (B == 0) return GLAD_OK;
-    cudaSetDevice(c->device);
+}  // extern "C"
+
+// Both halves (and, with d_ddt, the quasar terms of Eq. 35-36 on the lens stream) followed by joint_kernel.
+static glad_status joint_impl(glad_ctx* c, const float* d_lens, const float* d_dyn, int B, const float* d_lum, int nl,
+                              long lum_stride, const float* d_mass, int nm, long mass_stride, const float* d_beta,
+                              int per_gaussian, float* d_loglike, float* d_chi2_lens, float* d_chi2_dyn, int32_t* d_flags,
+                              const float* d_ddt, float* d_chi2_img, float* d_chi2_tmd) {
     glad_status st = grow(c, &c->d_tmp, &c->tmp_cap, (size_t)2 * B);
     if (st != GLAD_OK) return st;
     st = grow(c, &c->d_tmpflags, &c->tmpflags_cap, (size_t)2 * B);
@@ -346,6 +345,13 @@ glad_status glad_joint_loglike_batch(glad_ctx* c, const float* d_lens, const flo
     // scratch of both halves is grown before the fork (grow() may synchronise and free)
     st = grow(c, &c->d_lens_const, &c->lens_const_cap, (size_t)B * LC_SIZE);
     if (st != GLAD_OK) return st;
+    float *c2i = nullptr, *c2t = nullptr;
+    if (d_ddt) {
+        st = grow(c, &c->d_qtmp, &c->qtmp_cap, (size_t)2 * B);
+        if (st != GLAD_OK) return st;
+        c2i = d_chi2_img ? d_chi2_img : c->d_qtmp;
+        c2t = d_chi2_tmd ? d_chi2_tmd : c->d_qtmp + B;
+    }
     if (c->overlap) {
         // fork: the lens half (lens_prep's serial b_n roots, then lens_image) runs on the side stream beside jam_prep /
         // jam_quad; both wait for everything enqueued so far, and the caller's stream waits for the lens half below
@@ -354,13 +360,69 @@ glad_status glad_joint_loglike_batch(glad_ctx* c, const float* d_lens, const flo
         c->lens_stream = c->side_stream;
     }
     st = lens_impl(c, d_lens, B, nullptr, c2l, fl);
+    if (st == GLAD_OK && d_ddt) {
+        cudaError_t qe = launch_quasar(c, c->lens_stream, d_lens, d_ddt, B, c2i, c2t, nullptr, nullptr, nullptr);
+        if (qe != cudaSuccess) st = cuda_fail(c, qe, "quasar_kernel");
+    }
     c->lens_stream = c->stream;
     if (c->overlap) cudaEventRecord(c->ev_join, c->side_stream);
     glad_status st2 = st == GLAD_OK ? jam_impl(c, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian,
                                                nullptr, c2d, nullptr, fd) : st;
     if (c->overlap) cudaStreamWaitEvent(c->stream, c->ev_join, 0);   // join, also when a half failed: nothing left dangling
     if (st2 != GLAD_OK) return st2;
-    CU(launch_joint(c, B, c2l, c2d, fl, fd, d_loglike, d_flags), "joint_kernel");
+    CU(launch_joint(c, B, c2l, c2d, c2i, c2t, fl, fd, d_loglike, d_flags), "joint_kernel");
+    return GLAD_OK;
+}
+
+extern "C" {
+
+glad_status glad_joint_loglike_batch(glad_ctx* c, const float* d_lens, const float* d_dyn, int B, const float* d_lum, int nl,
+                                     long lum_stride, const float* d_mass, int nm, long mass_stride, const float* d_beta,
+                                     int per_gaussian, float* d_loglike, float* d_chi2_lens, float* d_chi2_dyn,
+                                     int32_t* d_flags) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && (!d_lens || !d_dyn || !d_loglike))) return fail(c, GLAD_EINVAL, "glad_joint_loglike_batch: B=%d / null pointer", B);
+    if (B == 0) return GLAD_OK;
+    cudaSetDevice(c->device);
+    return joint_impl(c, d_lens, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian, d_loglike,
+                      d_chi2_lens, d_chi2_dyn, d_flags, nullptr, nullptr, nullptr);
+}
+
+glad_status glad_set_quasar_data(glad_ctx* c, int n_img, const double* h_theta, const double* h_sigma_theta, int ref_image,
+                                 const double* h_dt_obs, const double* h_sigma_dt) {
+    if (!c) return GLAD_EINVAL;
+    if (n_img == 0) { c->have_qso = false; return GLAD_OK; }
+    if (n_img < 0 || n_img > GLAD_MAX_QIMG) return fail(c, GLAD_ESHAPE, "glad_set_quasar_data: n_img %d outside [0, GLAD_MAX_QIMG]", n_img);
+    if (!h_theta || !h_sigma_theta) return fail(c, GLAD_EINVAL, "glad_set_quasar_data: null positions");
+    if (ref_image < 0 || ref_image >= n_img) return fail(c, GLAD_EINVAL, "glad_set_quasar_data: reference image %d", ref_image);
+    if ((h_dt_obs == nullptr) != (h_sigma_dt == nullptr)) return fail(c, GLAD_EINVAL, "glad_set_quasar_data: dt_obs and sigma_dt go together");
+    glad_quasar_data q;
+    memset(&q, 0, sizeof(q));
+    q.n_img = n_img;
+    q.ref = ref_image;
+    for (int i = 0; i < n_img; ++i) {
+        if (!(h_sigma_theta[i] > 0.0)) return fail(c, GLAD_EINVAL, "glad_set_quasar_data: sigma_theta[%d] = %g", i, h_sigma_theta[i]);
+        q.theta[2 * i] = h_theta[2 * i];
+        q.theta[2 * i + 1] = h_theta[2 * i + 1];
+        q.ivar_theta[i] = 1.0 / (h_sigma_theta[i] * h_sigma_theta[i]);
+        if (h_dt_obs && i != ref_image && h_sigma_dt[i] > 0.0) {
+            q.dt_obs[i] = h_dt_obs[i];
+            q.ivar_dt[i] = 1.0 / (h_sigma_dt[i] * h_sigma_dt[i]);
+        }
+    }
+    c->qso = q;
+    c->have_qso = true;
+    return GLAD_OK;
+}
+
+glad_status glad_quasar_chi2_batch(glad_ctx* c, const float* d_lens, const float* d_ddt, int B, float* d_chi2_img,
+                                   float* d_chi2_tmd, double* d_theta_pre, double* d_dt_pre, double* d_beta) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && (!d_lens || !d_ddt))) return fail(c, GLAD_EINVAL, "glad_quasar_chi2_batch: B=%d / null pointer", B);
+    if (!c->have_qso) return fail(c, GLAD_ESTATE, "glad_quasar_chi2_batch: glad_set_quasar_data not called");
+    if (B == 0) return GLAD_OK;
+    cudaSetDevice(c->device);
+    CU(launch_quasar(c, c->stream, d_lens, d_ddt, B, d_chi2_img, d_chi2_tmd, d_theta_pre, d_dt_pre, d_beta), "quasar_kernel");
     return GLAD_OK;
 }
 
@@ -430,11 +492,15 @@ glad_status glad_mge1d_batch(glad_ctx* c, int kind, const float* d_prof, int B, 
     return GLAD_OK;
 }
 
-glad_status glad_joint_loglike_model_batch(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, float zd,
-                                           int B, int nl, float lum_lo, float lum_hi, int nm, float mass_lo, float mass_hi,
-                                           const float* d_beta, int per_gaussian, float* d_loglike, float* d_chi2_lens,
-                                           float* d_chi2_dyn, int32_t* d_flags, float* d_lum_out, float* d_mass_out) {
+}  // extern "C"
+
+static glad_status model_impl(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, float zd,
+                              int B, int nl, float lum_lo, float lum_hi, int nm, float mass_lo, float mass_hi,
+                              const float* d_beta, int per_gaussian, float* d_loglike, float* d_chi2_lens,
+                              float* d_chi2_dyn, int32_t* d_flags, float* d_lum_out, float* d_mass_out, bool quasar,
+                              float* d_chi2_img, float* d_chi2_tmd) {
     if (!c) return GLAD_EINVAL;
+    if (quasar && !c->have_qso) return fail(c, GLAD_ESTATE, "glad_joint_loglike_full_batch: glad_set_quasar_data not called");
     if (B < 0 || (B > 0 && (!d_lens || !d_dyn || !d_ddt || !d_beta || !d_loglike)))
         return fail(c, GLAD_EINVAL, "glad_joint_loglike_model_batch: B=%d / null pointer", B);
     if (!(zd > -1.f)) return fail(c, GLAD_EINVAL, "glad_joint_loglike_model_batch: z_d = %g", zd);
@@ -452,8 +518,26 @@ glad_status glad_joint_loglike_model_batch(glad_ctx* c, const float* d_lens, con
     float* m_mass = d_mass_out ? d_mass_out : m_lens + n_lens + n_lum;
     CU(launch_model(c, d_lens, d_dyn, d_ddt, (double)zd, B, (c->light_kinds & 2) ? GLAD_PROFILE_CHAMELEON : GLAD_PROFILE_SERSIC, nl, lum_lo, lum_hi, nm, mass_lo, mass_hi, MGE_DEFAULT_ORDER, m_lens,
                     m_lum, m_mass), "model_kernel");
-    return glad_joint_loglike_batch(c, m_lens, d_dyn, B, m_lum, nl, 3L * nl, m_mass, nm, 3L * nm, d_beta, per_gaussian,
-                                    d_loglike, d_chi2_lens, d_chi2_dyn, d_flags);
+    return joint_impl(c, m_lens, d_dyn, B, m_lum, nl, 3L * nl, m_mass, nm, 3L * nm, d_beta, per_gaussian, d_loglike, d_chi2_lens,
+                      d_chi2_dyn, d_flags, quasar ? d_ddt : nullptr, d_chi2_img, d_chi2_tmd);
+}
+
+extern "C" {
+
+glad_status glad_joint_loglike_model_batch(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, float zd,
+                                           int B, int nl, float lum_lo, float lum_hi, int nm, float mass_lo, float mass_hi,
+                                           const float* d_beta, int per_gaussian, float* d_loglike, float* d_chi2_lens,
+                                           float* d_chi2_dyn, int32_t* d_flags, float* d_lum_out, float* d_mass_out) {
+    return model_impl(c, d_lens, d_dyn, d_ddt, zd, B, nl, lum_lo, lum_hi, nm, mass_lo, mass_hi, d_beta, per_gaussian, d_loglike,
+                      d_chi2_lens, d_chi2_dyn, d_flags, d_lum_out, d_mass_out, false, nullptr, nullptr);
+}
+
+glad_status glad_joint_loglike_full_batch(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, float zd,
+                                          int B, int nl, float lum_lo, float lum_hi, int nm, float mass_lo, float mass_hi,
+                                          const float* d_beta, int per_gaussian, float* d_loglike, float* d_chi2_lens,
+                                          float* d_chi2_dyn, float* d_chi2_img, float* d_chi2_tmd, int32_t* d_flags) {
+    return model_impl(c, d_lens, d_dyn, d_ddt, zd, B, nl, lum_lo, lum_hi, nm, mass_lo, mass_hi, d_beta, per_gaussian, d_loglike,
+                      d_chi2_lens, d_chi2_dyn, d_flags, nullptr, nullptr, true, d_chi2_img, d_chi2_tmd);
 }
 
 }  // extern "C"

@@ -45,7 +45,16 @@ static inline __host__ __device__ int jam_table_floats(int nl, int nmx) {
 #define JQ_MI 8
 
 #define GLAD_PROF_MAX 2048
-enum GladKernelId { GK_LENS_PREP = 0, GK_LENS_IMAGE, GK_JAM_PREP, GK_JAM_QUAD, GK_JAM_POST, GK_JOINT, GK_MGE };
+enum GladKernelId { GK_LENS_PREP = 0, GK_LENS_IMAGE, GK_JAM_PREP, GK_JAM_QUAD, GK_JAM_POST, GK_JOINT, GK_MGE, GK_QUASAR };
+
+// quasar data (glad_set_quasar_data), passed to quasar_kernel by value
+struct glad_quasar_data {
+    int n_img, ref;
+    double theta[2 * GLAD_MAX_QIMG];     // observed image positions (x, y), arcsec
+    double ivar_theta[GLAD_MAX_QIMG];    // 1 / sigma_theta^2
+    double dt_obs[GLAD_MAX_QIMG];        // observed delays relative to image `ref`, days
+    double ivar_dt[GLAD_MAX_QIMG];       // 1 / sigma_dt^2, 0 = no measurement
+};
 
 struct glad_ctx {
     int device;
@@ -70,6 +79,10 @@ struct glad_ctx {
     float* d_psf;  // ctx-owned copy [kpsf*kpsf]
     int kpsf;
 
+    // quasar static data (copied)
+    bool have_qso;
+    glad_quasar_data qso;
+
     // kinematic static data
     bool have_kin;
     int nx, ny, nbins, kk, nu;
@@ -91,6 +104,7 @@ struct glad_ctx {
     float* d_tmp;        size_t tmp_cap;     // chi2_L, chi2_D [B] each
     int32_t* d_tmpflags; size_t tmpflags_cap; // flags_L, flags_D [B] each
     float* d_stage;      size_t stage_cap;   // device staging of glad_joint_loglike_host
+    float* d_qtmp;       size_t qtmp_cap;    // chi2_img, chi2_tmd [B] each (full joint entry)
     float* d_model;      size_t model_cap;   // glad_joint_loglike_model_batch: lens', profile rows, derived MGE tables
 
     // optional per-kernel timing (glad_profile_*): CUDA events on the context stream around each launch
@@ -125,8 +139,10 @@ cudaError_t launch_jam_prep(glad_ctx* c, const float* d_dyn, int B, const float*
 cudaError_t launch_jam_quad(glad_ctx* c, int B, int nl, int nmx, int S);
 cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d_vrms, float* d_chi2,
                             float* d_v2map, int32_t* d_flags);
-cudaError_t launch_joint(glad_ctx* c, int B, const float* d_c2l, const float* d_c2d, const int32_t* d_fl,
-                         const int32_t* d_fd, float* d_loglike, int32_t* d_flags);
+cudaError_t launch_joint(glad_ctx* c, int B, const float* d_c2l, const float* d_c2d, const float* d_c2img, const float* d_c2tmd,
+                         const int32_t* d_fl, const int32_t* d_fd, float* d_loglike, int32_t* d_flags);
+cudaError_t launch_quasar(glad_ctx* c, cudaStream_t st, const float* d_lens, const float* d_ddt, int B, float* d_chi2_img,
+                          float* d_chi2_tmd, double* d_theta_pre, double* d_dt_pre, double* d_beta);
 cudaError_t launch_kin_weights(glad_ctx* c);
 cudaError_t launch_mge1d(glad_ctx* c, int kind, const float* d_prof, int B, int n_gauss, float sigma_lo, float sigma_hi,
                          int P, float* d_mge);

@@ -262,21 +262,24 @@ cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d
     return cudaGetLastError();
 }
 
-// row a9: lnL = -(chi2_L + chi2_D)/2 (Eq. 52-53, R-J1); -inf where a half is invalid
+// row a9: lnL = -(chi2_L + chi2_D [+ chi2_img + chi2_tmd])/2 (Eq. 52-53, R-J1); -inf where a half is invalid
 __global__ void joint_kernel(int B, const float* __restrict__ c2l, const float* __restrict__ c2d,
+                             const float* __restrict__ c2img, const float* __restrict__ c2tmd,
                              const int32_t* __restrict__ fl, const int32_t* __restrict__ fd,
                              float* __restrict__ loglike, int32_t* __restrict__ flags) {
     int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     double s = (double)c2l[b] + (double)c2d[b];
+    if (c2img) s += (double)c2img[b];
+    if (c2tmd) s += (double)c2tmd[b];
     int f = fl[b] | fd[b];
     loglike[b] = (f == 0 && isfinite(s)) ? (float)(-0.5 * s) : -__int_as_float(0x7f800000);
     if (flags) flags[b] = f;
 }
 
-cudaError_t launch_joint(glad_ctx* c, int B, const float* d_c2l, const float* d_c2d, const int32_t* d_fl,
-                         const int32_t* d_fd, float* d_loglike, int32_t* d_flags) {
+cudaError_t launch_joint(glad_ctx* c, int B, const float* d_c2l, const float* d_c2d, const float* d_c2img, const float* d_c2tmd,
+                         const int32_t* d_fl, const int32_t* d_fd, float* d_loglike, int32_t* d_flags) {
     ProfScope ps(c, GK_JOINT);
-    joint_kernel<<<(B + 127) / 128, 128, 0, c->stream>>>(B, d_c2l, d_c2d, d_fl, d_fd, d_loglike, d_flags);
+    joint_kernel<<<(B + 127) / 128, 128, 0, c->stream>>>(B, d_c2l, d_c2d, d_c2img, d_c2tmd, d_fl, d_fd, d_loglike, d_flags);
     return cudaGetLastError();
 }
