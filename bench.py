@@ -318,6 +318,27 @@ def run_ours(args, rank, world, local_rank):
                  "mge_ms_per_step": mp["mge"][0] / m_steps, "mge_launches_per_step": mp["mge"][1] / m_steps,
                  "tables": f"{nlm} luminous (Sersic, 0.02-10 arcsec) + {nmm} mass (EPL, 0.02-50 arcsec) Gaussians per vector, Euler order 12",
                  "paper_context": "1-D MGE of one profile: ~2e-4 s on one A100 (P:356, Table 2)"}
+        # SURVEY 8(f) rank 4 (quasar part): the same entry plus chi2_img + chi2_tmd (Eq. 35-36) = every term of Eq. 53
+        g.set_quasar_data(workloads.quasar_data(args.config))
+        fout = dict(out)
+        for _ in range(3):
+            g.joint_loglike_full_batch(*margs, out=fout)
+        torch.cuda.synchronize()
+        g.profile_enable(True)
+        g.profile_read()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record()
+        for _ in range(m_steps):
+            g.joint_loglike_full_batch(*margs, out=fout)
+        f1.record()
+        torch.cuda.synchronize()
+        fp = g.profile_read()
+        g.profile_enable(False)
+        f_ms = f0.elapsed_time(f1) / m_steps
+        model["full_entry"] = {"api": "glad_joint_loglike_full_batch", "value": B / (f_ms * 1e-3), "unit": UNIT, "ms_per_step": f_ms,
+                               "quasar_ms_per_step": fp["quasar"][0] / m_steps, "quasar_launches_per_step": fp["quasar"][1] / m_steps,
+                               "quasar": "4 images, 3 delays, 12 Newton steps per image, fp64; runs on the lens half's stream",
+                               "paper_context": "image-position and time-delay terms: < 0.1 s on one CPU core, kept on the CPU (P:265-267)"}
 
     if dist is not None:
         tt = torch.tensor([ms, e2e_ms], device=dev, dtype=torch.float64)

@@ -221,3 +221,16 @@ def test_invalid_mass_parameters_give_infinite_chi2(oracle, rxj):
     out = oracle.quasar_batch(bad, [1823.0] * 3, q1)
     assert np.all(np.isinf(out["chi2_img"])) and np.all(np.isinf(out["chi2_tmd"]))
     assert np.all(np.isnan(out["theta_pre"]))
+
+
+@pytest.mark.parametrize("name", ["C1", "C2"])
+def test_stored_quasar_observations_fit_the_truth_vector(oracle, name):
+    """workloads.quasar_data holds rounded mock observations of the truth vector: the oracle must find them consistent
+    with it (chi2 of the order of the 8 + 3 data points) and inconsistent with a vector far from it."""
+    import workloads
+    wl = workloads.make_workload(name, None, B=8)
+    q = workloads.quasar_data(name)
+    out = oracle.quasar_batch(wl["lens"]["params"], wl["ddt"], q)
+    assert np.all(out["last_step"][0] < 1e-12)
+    assert out["chi2_img"][0] < 40.0 and out["chi2_tmd"][0] < 30.0
+    assert np.median(out["chi2_img"][1:] + out["chi2_tmd"][1:]) > 1e3

@@ -233,6 +233,28 @@ def make_workload(name: str, data_model=None, B: int | None = None) -> dict:
     return wl
 
 
+# Synthetic lensed-quasar observations (Eq. 35-36): an RXJ1131-like quad for the truth vector (batch element 0) of each config
+# family.  These are DATA: image positions [arcsec] and delays [days] of a point source at the truth source centre
+# (0.08, -0.05), written once by tests/quasar_util.mock_quasar (oracle deflection + MINPACK, seed 0: positions + N(0, 0.004"),
+# delays x (1 + N(0, 0.03))) and rounded to the digits below; tests/test_oracle_quasar.py checks that the oracle finds them
+# consistent with the truth vector (chi2 of the order of the number of data points).
+_QUASAR = {
+    "C1": dict(theta=[[0.3763, -1.0949], [0.8562, 0.4753], [0.2470, 1.0287], [-0.8162, 0.0215]], ref=0,
+               dt_obs=[0.0, 7.2228, 6.3046, 13.7051], sigma_dt=[0.0, 0.25, 0.25, 0.4112]),
+    "C2": dict(theta=[[-1.4223, -0.0663], [0.4798, -1.8253], [1.4803, 0.5375], [0.1286, 1.7884]], ref=1,
+               dt_obs=[28.9663, 0.0, 18.6398, 10.9334], sigma_dt=[0.8690, 0.0, 0.5592, 0.3280]),
+}
+
+
+def quasar_data(name: str) -> dict:
+    """Quasar observations for config `name` (C4, C5 share C2's truth mass model): dict(theta [4,2], sigma_theta [4], ref,
+    dt_obs [4] days relative to image ref, sigma_dt [4]; 0 = the reference image itself), float64."""
+    q = _QUASAR["C1" if name == "C1" else "C2"]
+    th = np.asarray(q["theta"], np.float64)
+    return dict(theta=th, sigma_theta=np.full(len(th), 0.004), ref=int(q["ref"]),
+                dt_obs=np.asarray(q["dt_obs"], np.float64), sigma_dt=np.asarray(q["sigma_dt"], np.float64))
+
+
 def subset(wl: dict, idx) -> dict:
     """Same static data, only the batch elements `idx` (for parity sub-batches)."""
     idx = np.asarray(idx, dtype=np.int64)
