@@ -79,6 +79,18 @@ def lib():
         L.glad_oracle_mge1d.argtypes = [i, dp, i, d, d, i, dp]
         L.glad_oracle_sigma_crit.restype = d
         L.glad_oracle_sigma_crit.argtypes = [d, d, d]
+        L.glad_oracle_deflection_sheet.restype = None
+        L.glad_oracle_deflection_sheet.argtypes = [dp, d, d, d, d, d, dp, dp]
+        L.glad_oracle_potential_sheet.restype = d
+        L.glad_oracle_potential_sheet.argtypes = [dp, d, d, d, d, d]
+        L.glad_oracle_hessian_sheet.restype = None
+        L.glad_oracle_hessian_sheet.argtypes = [dp, d, d, d, d, d, dp]
+        L.glad_oracle_sheet_kappa.restype = d
+        L.glad_oracle_sheet_kappa.argtypes = [d] * 5
+        L.glad_oracle_lens_image_batch_sheet.restype = i
+        L.glad_oracle_lens_image_batch_sheet.argtypes = [fp, i, i, i, i, d, d, d, fp, i, fp, fp, ip, fp, d, d, dp, dp, ip]
+        L.glad_oracle_quasar_batch_sheet.restype = i
+        L.glad_oracle_quasar_batch_sheet.argtypes = [fp, fp, fp, d, d, i, i, dp, dp, i, dp, dp, dp, dp, dp, dp, dp, dp]
         L.glad_oracle_potential.restype = d
         L.glad_oracle_potential.argtypes = [dp, d, d]
         L.glad_oracle_hessian.restype = None
@@ -109,12 +121,19 @@ def epl_alpha(x, y, thetaE, gamma, q):
     return ax.value, ay.value
 
 
-def deflection(params, thx, thy):
+def deflection(params, thx, thy, lam=1.0, sheet=None):
+    """sheet = (r_core, r_tr) switches the internal mass sheet on (Eq. 6, 50; readings R-S1..3) with constant lam."""
     p = np.ascontiguousarray(params, dtype=np.float64)
     assert p.size == NLENS
     ax, ay = C.c_double(), C.c_double()
-    lib().glad_oracle_deflection(_ptr(p, C.c_double), thx, thy, C.byref(ax), C.byref(ay))
+    rc, rt = sheet if sheet is not None else (0.0, 0.0)
+    lib().glad_oracle_deflection_sheet(_ptr(p, C.c_double), float(lam), float(rc), float(rt), thx, thy, C.byref(ax), C.byref(ay))
     return ax.value, ay.value
+
+
+def sheet_kappa(lam, rc, rt, dx, dy) -> float:
+    """(1 - lam) S(R) of Eq. 50 normalised to S(0) = 1."""
+    return float(lib().glad_oracle_sheet_kappa(float(lam), float(rc), float(rt), float(dx), float(dy)))
 
 
 def bh_theta2(Mbh, Ddt_mpc, zd) -> float:
@@ -129,9 +148,10 @@ def chameleon(dx, dy, I0, wc, wt, q, phi) -> float:
     return float(lib().glad_oracle_chameleon(dx, dy, I0, wc, wt, q, phi))
 
 
-def lens_image_batch(lens, grid, psf, data=None, ivar=None, want_images=True, kinds=None):
+def lens_image_batch(lens, grid, psf, data=None, ivar=None, want_images=True, kinds=None, lam=None, sheet=None):
     """grid = dict(nx, ny, supersample, pix, x0, y0). kinds = None (all Sersic) or 3 ints (source, lens light 1, 2):
-    0 Sersic, 1 Chameleon (slot = {I_0, w_c, w_t, q, phi}). Returns dict(images, chi2, flags)."""
+    0 Sersic, 1 Chameleon (slot = {I_0, w_c, w_t, q, phi}). lam [B] + sheet = (r_core, r_tr): internal mass sheet.
+    Returns dict(images, chi2, flags)."""
     lens = _f32(lens).reshape(-1, NLENS)
     B = lens.shape[0]
     nx, ny = int(grid["nx"]), int(grid["ny"])
@@ -142,10 +162,13 @@ def lens_image_batch(lens, grid, psf, data=None, ivar=None, want_images=True, ki
     chi2 = np.empty(B, np.float64)
     flags = np.zeros(B, np.int32)
     kk = None if kinds is None else np.ascontiguousarray(kinds, dtype=np.int32).reshape(3)
-    rc = lib().glad_oracle_lens_image_batch_kinds(
+    lm = None if lam is None else _f32(lam).reshape(-1)
+    assert lm is None or (lm.size == B and sheet is not None)
+    src, srt = sheet if (sheet is not None and lm is not None) else (0.0, 0.0)
+    rc = lib().glad_oracle_lens_image_batch_sheet(
         _ptr(lens, C.c_float), B, nx, ny, int(grid["supersample"]), float(grid["pix"]), float(grid["x0"]),
         float(grid["y0"]), _ptr(psf, C.c_float), k, _ptr(data, C.c_float), _ptr(ivar, C.c_float), _ptr(kk, C.c_int32),
-        _ptr(images, C.c_double), _ptr(chi2, C.c_double), _ptr(flags, C.c_int32))
+        _ptr(lm, C.c_float), float(src), float(srt), _ptr(images, C.c_double), _ptr(chi2, C.c_double), _ptr(flags, C.c_int32))
     if rc != 0:
         raise ValueError("oracle: bad lens arguments")
     return {"images": images, "chi2": chi2, "flags": flags}
@@ -257,41 +280,57 @@ def sigma_crit(Ddt_mpc, Dd_mpc, zd) -> float:
     return float(lib().glad_oracle_sigma_crit(float(Ddt_mpc), float(Dd_mpc), float(zd)))
 
 
-def model_tables(lens, dyn, ddt, zd, n_lum, n_mass, lum_range, mass_range, P=MGE_EULER_P, tracer_kind=PROFILE_SERSIC):
+def model_tables(lens, dyn, ddt, zd, n_lum, n_mass, lum_range, mass_range, P=MGE_EULER_P, tracer_kind=PROFILE_SERSIC,
+                 lam=None, sheet=None):
     """The self-consistent joint model of P:406 / Fig. 2 (reading R-M3): from the lens vector and the distances
     derive (a) the luminous MGE = Eq. 46 of lens-light component #1 (lens[16:20]; Sersic, or Chameleon with tracer_kind), (b) the mass MGE = Eq. 46 of
     Sigma_crit * kappa_epl (Eq. 13, B.1-B.3), (c) lens[8] = theta_E,BH^2 from M_BH = dyn[2] (Eq. 4).
     Returns (lens' [B,26] float32, lum [B,n_lum,3] float32, mass [B,n_mass,3] float32): tables rounded to the
-    float32 the batch calls take."""
+    float32 the batch calls take.  lam [B] + sheet = dict(rc, rt, n, sigma_lo, sigma_hi): internal mass sheet; the mass
+    table then has n_mass + sheet["n"] rows (lam x the EPL rows, then the sheet's round Gaussians)."""
     lens = _f32(lens).reshape(-1, NLENS).copy()
     dyn = _f32(dyn).reshape(-1, NDYN)
     ddt = _f32(ddt).reshape(-1)
     B = lens.shape[0]
     lum = np.empty((B, n_lum, 3), np.float32)
-    mass = np.empty((B, n_mass, 3), np.float32)
+    mass = None
     for b in range(B):
         Ie, Re, n, q = (float(v) for v in lens[b, 16:20])
         lum[b] = mge1d(tracer_kind, [Ie, Re, n, q], n_lum, *lum_range, P=P)   # Chameleon tracer: the slots are {I_0, w_c, w_t, q}
         sc = sigma_crit(float(ddt[b]), float(dyn[b, 1]), zd)
-        mass[b] = mge1d(PROFILE_EPL, [sc, float(lens[b, 2]), float(lens[b, 3]), float(lens[b, 4])], n_mass, *mass_range, P=P)
+        m = mge1d(PROFILE_EPL, [sc, float(lens[b, 2]), float(lens[b, 3]), float(lens[b, 4])], n_mass, *mass_range, P=P)
+        if lam is not None:
+            # Sigma_int = Sigma_crit [lam kappa_epl + (1 - lam) S(R)] (Eq. 6, 12, 50; readings R-S1..3).  The sheet is round
+            # (q' = 1), the EPL is not, so it gets rows of its own: a round Chameleon-shaped profile (Eq. 47 at q = 1:
+            # I_0/2 (1/sqrt(R^2+w_c^2) - 1/sqrt(R^2+w_t^2))) expanded by Eq. 46 on sheet_n sigmas in [sheet_lo, sheet_hi]
+            lb, rc, rt = float(np.float32(lam[b])), float(sheet["rc"]), float(sheet["rt"])
+            i0 = 2.0 * sc * (1.0 - lb) / (1.0 / rc - 1.0 / rt)
+            sh = mge1d(PROFILE_CHAMELEON, [i0, rc, rt, 1.0], int(sheet["n"]), float(sheet["sigma_lo"]), float(sheet["sigma_hi"]), P=P)
+            m[:, 0] *= lb
+            m = np.concatenate([m, sh])
+        if mass is None:
+            mass = np.empty((B, m.shape[0], 3), np.float32)
+        mass[b] = m
         lens[b, 8] = bh_theta2(float(dyn[b, 2]), float(ddt[b]), zd)
     return lens, lum, mass
 
 
 # ---- SURVEY.md 8(f) rank 4 (quasar part): image-position and time-delay chi^2 (Eq. 35-36 P:253-265) ----
-def potential(params, thx, thy) -> float:
-    """psi(theta) of EPL + shear + point mass (readings R-Q4)."""
+def potential(params, thx, thy, lam=1.0, sheet=None) -> float:
+    """psi(theta) of EPL + shear + point mass (readings R-Q4) [+ internal mass sheet]."""
     p = np.ascontiguousarray(params, dtype=np.float64)
     assert p.size == NLENS
-    return float(lib().glad_oracle_potential(_ptr(p, C.c_double), float(thx), float(thy)))
+    rc, rt = sheet if sheet is not None else (0.0, 0.0)
+    return float(lib().glad_oracle_potential_sheet(_ptr(p, C.c_double), float(lam), float(rc), float(rt), float(thx), float(thy)))
 
 
-def hessian(params, thx, thy):
+def hessian(params, thx, thy, lam=1.0, sheet=None):
     """(psi_xx, psi_xy, psi_yy) at theta."""
     p = np.ascontiguousarray(params, dtype=np.float64)
     assert p.size == NLENS
     h = np.empty(3, np.float64)
-    lib().glad_oracle_hessian(_ptr(p, C.c_double), float(thx), float(thy), _ptr(h, C.c_double))
+    rc, rt = sheet if sheet is not None else (0.0, 0.0)
+    lib().glad_oracle_hessian_sheet(_ptr(p, C.c_double), float(lam), float(rc), float(rt), float(thx), float(thy), _ptr(h, C.c_double))
     return h
 
 
@@ -300,8 +339,9 @@ def tdelay_const() -> float:
     return float(lib().glad_oracle_tdelay_const())
 
 
-def quasar_batch(lens, ddt, qso):
+def quasar_batch(lens, ddt, qso, lam=None, sheet=None):
     """qso = dict(theta [n_img,2], sigma_theta [n_img], ref, dt_obs [n_img], sigma_dt [n_img]) (float64).
+    lam [B] + sheet = (r_core, r_tr): internal mass sheet.
     Returns dict(chi2_img, chi2_tmd [B]; theta_pre [B,n_img,2]; dt_pre [B,n_img]; beta [B,2]; last_step [B,n_img])."""
     lens = _f32(lens).reshape(-1, NLENS)
     ddt = _f32(ddt).reshape(-1)
@@ -314,9 +354,13 @@ def quasar_batch(lens, ddt, qso):
     out = {"chi2_img": np.empty(B), "chi2_tmd": np.empty(B), "theta_pre": np.empty((B, n, 2)),
            "dt_pre": np.empty((B, n)), "beta": np.empty((B, 2)), "last_step": np.empty((B, n))}
     P = lambda a: _ptr(a, C.c_double)
-    rc = lib().glad_oracle_quasar_batch(_ptr(lens, C.c_float), _ptr(ddt, C.c_float), B, n, P(th), P(st), int(qso["ref"]),
-                                        P(dt), P(sd), P(out["chi2_img"]), P(out["chi2_tmd"]), P(out["theta_pre"]),
-                                        P(out["dt_pre"]), P(out["beta"]), P(out["last_step"]))
+    lm = None if lam is None else _f32(lam).reshape(-1)
+    assert lm is None or (lm.size == B and sheet is not None)
+    src, srt = sheet if (sheet is not None and lm is not None) else (0.0, 0.0)
+    rc = lib().glad_oracle_quasar_batch_sheet(_ptr(lens, C.c_float), _ptr(ddt, C.c_float), _ptr(lm, C.c_float), float(src),
+                                              float(srt), B, n, P(th), P(st), int(qso["ref"]), P(dt), P(sd),
+                                              P(out["chi2_img"]), P(out["chi2_tmd"]), P(out["theta_pre"]),
+                                              P(out["dt_pre"]), P(out["beta"]), P(out["last_step"]))
     if rc != 0:
         raise ValueError("oracle: bad quasar arguments")
     return out

@@ -149,16 +149,59 @@ void glad_oracle_epl_alpha(double x, double y, double thetaE, double gamma, doub
     *ay = cimag(alpha);
 }
 
-/* Total deflection at image-plane position (thx, thy): EPL (rotated by phi_PA
+/* ------------------------------------------------------------------------ */
+/* Internal mass sheet, Eq. 6 with the dPIE profile of Eq. 50-51       */
+/* in place of the constant sheet -- DESIGN.md readings R-S1..3:  */
+/*   kappa_int = (1 - lam) S(R) + lam kappa_epl + kappa_BH   (shear outside)  */
+/*   S(R) = [1/sqrt(R^2+rc^2) - 1/sqrt(R^2+rt^2)] / (1/rc - 1/rt),  S(0) = 1,  */
+/*   R^2 = x^2 + y^2 about the lens centre; lam = the constant of Eq. 51.     */
+/* For kappa = A/sqrt(R^2+s^2) (circular): alpha_R = 2A (h - s)/R, h = sqrt(R^2+s^2)*/
+/* (mean convergence inside R), psi = 2A [(h - s) - s ln((s+h)/2s)] (psi(0)=0),*/
+/* Hessian = g I + 2 (kappa - g) x x^T / R^2 with g = alpha_R/R.              */
+/* long double: rc = 45", rt = 45.09" make every term a small difference.     */
+/* ------------------------------------------------------------------------ */
+static void sheet_terms(double lam, double rc, double rt, double dx, double dy, double* ax, double* ay,
+                        double* h, double* psi, double* kap) {
+    /* every term is a difference of two nearly equal numbers (rt - rc << rc): written with h - s = R^2/(h + s),
+     * 1/hc - 1/ht = (rt^2 - rc^2)/((ht + hc) hc ht) and log1p so that nothing is lost for any rc, rt */
+    long double c = rc, t = rt, A = (1.0L - (long double)lam) * c * t / (t - c);      /* (1-lam)/(1/rc - 1/rt) */
+    long double x = dx, y = dy, R2 = x * x + y * y;
+    long double hc = sqrtl(R2 + c * c), ht = sqrtl(R2 + t * t);
+    long double k = A * (t * t - c * c) / ((ht + hc) * hc * ht);                      /* Eq. 50 */
+    long double g = 2.0L * A * (1.0L / (hc + c) - 1.0L / (ht + t));                   /* alpha_R / R */
+    if (ax) *ax = (double)(g * x);
+    if (ay) *ay = (double)(g * y);
+    if (kap) *kap = (double)k;
+    if (h) {
+        long double e = (R2 > 0.0L) ? 2.0L * (k - g) / R2 : 0.0L;
+        h[0] = (double)(g + e * x * x);
+        h[1] = (double)(e * x * y);
+        h[2] = (double)(g + e * y * y);
+    }
+    if (psi) {
+        long double dc = R2 / (hc + c), dt = R2 / (ht + t);                           /* h - s */
+        *psi = (double)(2.0L * A * ((dc - c * log1pl(dc / (2.0L * c))) - (dt - t * log1pl(dt / (2.0L * t)))));
+    }
+}
+
+double glad_oracle_sheet_kappa(double lam, double rc, double rt, double dx, double dy) {
+    double k;
+    sheet_terms(lam, rc, rt, dx, dy, NULL, NULL, NULL, NULL, &k);
+    return k;
+}
+
+/* Total deflection at image-plane position (thx, thy): lam * EPL (rotated by phi_PA
  * about the lens centre) + external shear (Eq. 49, origin = lens centre,
- * reading R-L5) + point mass alpha = thE2 * D/|D|^2 (reading R-L6). */
-void glad_oracle_deflection(const double* p, double thx, double thy, double* ax, double* ay) {
+ * reading R-L5) + point mass alpha = thE2 * D/|D|^2 (reading R-L6) + the mass
+ * sheet (rc > 0; rc <= 0 = no sheet, lam must then be 1). */
+void glad_oracle_deflection_sheet(const double* p, double lam, double rc, double rt, double thx, double thy,
+                                  double* ax, double* ay) {
     double dx = thx - p[0], dy = thy - p[1];
     double c = cos(p[5]), s = sin(p[5]);
     double xl = dx * c + dy * s, yl = -dx * s + dy * c;
     double axl, ayl;
     glad_oracle_epl_alpha(xl, yl, p[2], p[3], p[4], &axl, &ayl);
-    double a_x = axl * c - ayl * s, a_y = axl * s + ayl * c;
+    double a_x = lam * (axl * c - ayl * s), a_y = lam * (axl * s + ayl * c);
     double c2 = cos(2.0 * p[7]), s2 = sin(2.0 * p[7]);
     a_x += p[6] * (dx * c2 + dy * s2);
     a_y += p[6] * (dx * s2 - dy * c2);
@@ -166,8 +209,17 @@ void glad_oracle_deflection(const double* p, double thx, double thy, double* ax,
     if (r2 < 1e-12) r2 = 1e-12;
     a_x += p[8] * dx / r2;
     a_y += p[8] * dy / r2;
+    if (rc > 0.0) {
+        double sx, sy;
+        sheet_terms(lam, rc, rt, dx, dy, &sx, &sy, NULL, NULL, NULL);
+        a_x += sx;
+        a_y += sy;
+    }
     *ax = a_x;
     *ay = a_y;
+}
+void glad_oracle_deflection(const double* p, double thx, double thy, double* ax, double* ay) {
+    glad_oracle_deflection_sheet(p, 1.0, 0.0, 0.0, thx, thy, ax, ay);
 }
 
 /* Chameleon light profile, Eq. 47: the paper's lens-light model (two of them), a difference of two cored
@@ -221,11 +273,27 @@ int glad_oracle_lens_image_batch(const float* lens, int B, int nx, int ny, int s
                                  double* chi2, int32_t* flags) {
     return glad_oracle_lens_image_batch_kinds(lens, B, nx, ny, s, pix, x0, y0, psf, kpsf, data, ivar, NULL, images, chi2, flags);
 }
+int glad_oracle_lens_image_batch_sheet(const float* lens, int B, int nx, int ny, int s, double pix,
+                                       double x0, double y0, const float* psf, int kpsf,
+                                       const float* data, const float* ivar, const int* kinds,
+                                       const float* lambda, double rc, double rt,
+                                       double* images, double* chi2, int32_t* flags);
 /* same, with the light profile kind of each component (see lens_params_valid_kinds) */
 int glad_oracle_lens_image_batch_kinds(const float* lens, int B, int nx, int ny, int s, double pix,
                                        double x0, double y0, const float* psf, int kpsf,
                                        const float* data, const float* ivar, const int* kinds,
                                        double* images, double* chi2, int32_t* flags) {
+    return glad_oracle_lens_image_batch_sheet(lens, B, nx, ny, s, pix, x0, y0, psf, kpsf, data, ivar, kinds, NULL, 0.0, 0.0,
+                                              images, chi2, flags);
+}
+/* same, with the internal mass sheet: lambda [B] float32 (NULL = none), rt > rc > 0 arcsec (R-S1..3);
+ * a non-finite lambda invalidates the vector */
+int glad_oracle_lens_image_batch_sheet(const float* lens, int B, int nx, int ny, int s, double pix,
+                                       double x0, double y0, const float* psf, int kpsf,
+                                       const float* data, const float* ivar, const int* kinds,
+                                       const float* lambda, double rc, double rt,
+                                       double* images, double* chi2, int32_t* flags) {
+    if (lambda && !(rc > 0.0 && rt > rc)) return -1;
     if (B < 0 || nx <= 0 || ny <= 0 || s <= 0 || kpsf <= 0 || (kpsf % 2) == 0) return -1;
     if (kinds) for (int c = 0; c < 3; ++c) if (kinds[c] != 0 && kinds[c] != 1) return -1;
     const int ks = kinds ? kinds[0] : 0, k1 = kinds ? kinds[1] : 0, k2 = kinds ? kinds[2] : 0;
@@ -235,7 +303,8 @@ int glad_oracle_lens_image_batch_kinds(const float* lens, int B, int nx, int ny,
         double p[ORACLE_NLENS];
         for (int i = 0; i < ORACLE_NLENS; ++i) p[i] = (double)lens[(size_t)b * ORACLE_NLENS + i];
         if (flags) flags[b] = 0;
-        if (!lens_params_valid_kinds(p, kinds)) {
+        const double lam = lambda ? (double)lambda[b] : 1.0, src = lambda ? rc : 0.0;
+        if (!lens_params_valid_kinds(p, kinds) || !isfinite(lam)) {
             if (flags) flags[b] |= FLAG_LENS_INVALID;
             if (images) for (int i = 0; i < npx; ++i) images[(size_t)b * npx + i] = NAN;
             if (chi2) chi2[b] = INFINITY;
@@ -254,7 +323,7 @@ int glad_oracle_lens_image_batch_kinds(const float* lens, int B, int nx, int ny,
                         double thx = x0 + ix * pix + ((sa + 0.5) / s - 0.5) * pix;
                         double thy = y0 + iy * pix + ((sb + 0.5) / s - 0.5) * pix;
                         double ax, ay;
-                        glad_oracle_deflection(p, thx, thy, &ax, &ay);
+                        glad_oracle_deflection_sheet(p, lam, src, rt, thx, thy, &ax, &ay);
                         double bx = thx - ax, by = thy - ay; /* beta = theta - alpha */
                         double v = 0.0;
                         if (p[11] != 0.0)
@@ -539,23 +608,37 @@ double glad_oracle_bh_theta2(double Mbh_msun, double Ddt_mpc, double zd) {
 /* ------------------------------------------------------------------------ */
 
 /* psi(theta) of EPL + shear + point mass; p = lens vector (first 9 entries used) */
+double glad_oracle_potential_sheet(const double* p, double lam, double rc, double rt, double thx, double thy);
 double glad_oracle_potential(const double* p, double thx, double thy) {
+    return glad_oracle_potential_sheet(p, 1.0, 0.0, 0.0, thx, thy);
+}
+/* with the internal mass sheet: lam psi_epl + psi_sheet (+ shear, point mass), Eq. 8 with the dPIE sheet */
+double glad_oracle_potential_sheet(const double* p, double lam, double rc, double rt, double thx, double thy) {
     double dx = thx - p[0], dy = thy - p[1];
     double c = cos(p[5]), s = sin(p[5]);
     double xl = dx * c + dy * s, yl = -dx * s + dy * c;
     double axl, ayl;
     glad_oracle_epl_alpha(xl, yl, p[2], p[3], p[4], &axl, &ayl);
-    double psi = (xl * axl + yl * ayl) / (3.0 - p[3]);
+    double psi = lam * (xl * axl + yl * ayl) / (3.0 - p[3]);
     double c2 = cos(2.0 * p[7]), s2 = sin(2.0 * p[7]);
     psi += 0.5 * p[6] * ((dx * dx - dy * dy) * c2 + 2.0 * dx * dy * s2);
     double r2 = dx * dx + dy * dy;
     if (r2 < 1e-12) r2 = 1e-12;
     psi += 0.5 * p[8] * log(r2);
+    if (rc > 0.0) {
+        double ps;
+        sheet_terms(lam, rc, rt, dx, dy, NULL, NULL, NULL, &ps, NULL);
+        psi += ps;
+    }
     return psi;
 }
 
 /* Hessian of psi: h[0] = psi_xx, h[1] = psi_xy, h[2] = psi_yy (sky frame) */
+void glad_oracle_hessian_sheet(const double* p, double lam, double rc, double rt, double thx, double thy, double* h);
 void glad_oracle_hessian(const double* p, double thx, double thy, double* h) {
+    glad_oracle_hessian_sheet(p, 1.0, 0.0, 0.0, thx, thy, h);
+}
+void glad_oracle_hessian_sheet(const double* p, double lam, double rc, double rt, double thx, double thy, double* h) {
     double dx = thx - p[0], dy = thy - p[1];
     double c = cos(p[5]), s = sin(p[5]);
     double xl = dx * c + dy * s, yl = -dx * s + dy * c;
@@ -574,9 +657,14 @@ void glad_oracle_hessian(const double* p, double thx, double thy, double* h) {
         double complex g = ((1.0 - t) * (axl + I * ayl) * z - kappa * z * z) / r2;
         double lxx = kappa + creal(g), lyy = kappa - creal(g), lxy = cimag(g);
         /* rotate the lens-frame tensor back by +phi_PA: H = R L R^T */
-        hxx = c * c * lxx - 2.0 * c * s * lxy + s * s * lyy;
-        hyy = s * s * lxx + 2.0 * c * s * lxy + c * c * lyy;
-        hxy = c * s * (lxx - lyy) + (c * c - s * s) * lxy;
+        hxx = lam * (c * c * lxx - 2.0 * c * s * lxy + s * s * lyy);
+        hyy = lam * (s * s * lxx + 2.0 * c * s * lxy + c * c * lyy);
+        hxy = lam * (c * s * (lxx - lyy) + (c * c - s * s) * lxy);
+    }
+    if (rc > 0.0) {
+        double hs[3];
+        sheet_terms(lam, rc, rt, dx, dy, NULL, NULL, hs, NULL, NULL);
+        hxx += hs[0]; hxy += hs[1]; hyy += hs[2];
     }
     double c2 = cos(2.0 * p[7]), s2 = sin(2.0 * p[7]);
     hxx += p[6] * c2;
@@ -615,17 +703,31 @@ double glad_oracle_tdelay_const(void) {
  * Invalid mass parameters (theta_E < 0, gamma outside (1,3), q outside (0,1]) -> chi2 = +inf, outputs NaN.
  */
 #define NEWTON_STEPS 12
+int glad_oracle_quasar_batch_sheet(const float* lens, const float* ddt, const float* lambda, double rc, double rt, int B,
+                                   int n_img, const double* theta_obs, const double* sigma_theta, int ref,
+                                   const double* dt_obs, const double* sigma_dt, double* chi2_img, double* chi2_tmd,
+                                   double* theta_pre, double* dt_pre, double* beta_bar, double* last_step);
 int glad_oracle_quasar_batch(const float* lens, const float* ddt, int B, int n_img, const double* theta_obs,
                              const double* sigma_theta, int ref, const double* dt_obs, const double* sigma_dt,
                              double* chi2_img, double* chi2_tmd, double* theta_pre, double* dt_pre,
                              double* beta_bar, double* last_step) {
+    return glad_oracle_quasar_batch_sheet(lens, ddt, NULL, 0.0, 0.0, B, n_img, theta_obs, sigma_theta, ref, dt_obs, sigma_dt,
+                                          chi2_img, chi2_tmd, theta_pre, dt_pre, beta_bar, last_step);
+}
+/* same with the internal mass sheet (lambda [B] float32 or NULL; rt > rc > 0) in alpha, the Hessian and psi */
+int glad_oracle_quasar_batch_sheet(const float* lens, const float* ddt, const float* lambda, double rc, double rt, int B,
+                                   int n_img, const double* theta_obs, const double* sigma_theta, int ref,
+                                   const double* dt_obs, const double* sigma_dt, double* chi2_img, double* chi2_tmd,
+                                   double* theta_pre, double* dt_pre, double* beta_bar, double* last_step) {
+    if (lambda && !(rc > 0.0 && rt > rc)) return -1;
     if (n_img < 1 || n_img > ORACLE_MAX_QIMG || ref < 0 || ref >= n_img) return -1;
     const double K = glad_oracle_tdelay_const();
 #pragma omp parallel for schedule(dynamic)
     for (int b = 0; b < B; ++b) {
         double p[ORACLE_NLENS];
         for (int k = 0; k < ORACLE_NLENS; ++k) p[k] = (double)lens[(size_t)b * ORACLE_NLENS + k];
-        int ok = (p[2] >= 0.0) && (p[3] > 1.0) && (p[3] < 3.0) && (p[4] > 0.0) && (p[4] <= 1.0) && (p[8] >= 0.0);
+        const double lam = lambda ? (double)lambda[b] : 1.0, src = lambda ? rc : 0.0;
+        int ok = (p[2] >= 0.0) && (p[3] > 1.0) && (p[3] < 3.0) && (p[4] > 0.0) && (p[4] <= 1.0) && (p[8] >= 0.0) && isfinite(lam);
         if (!ok) {
             if (chi2_img) chi2_img[b] = INFINITY;
             if (chi2_tmd) chi2_tmd[b] = INFINITY;
@@ -641,8 +743,8 @@ int glad_oracle_quasar_batch(const float* lens, const float* ddt, int B, int n_i
         double bx = 0.0, by = 0.0, wsum = 0.0;
         for (int i = 0; i < n_img; ++i) {
             double tx = theta_obs[2 * i], ty = theta_obs[2 * i + 1], ax, ay, h[3];
-            glad_oracle_deflection(p, tx, ty, &ax, &ay);
-            glad_oracle_hessian(p, tx, ty, h);
+            glad_oracle_deflection_sheet(p, lam, src, rt, tx, ty, &ax, &ay);
+            glad_oracle_hessian_sheet(p, lam, src, rt, tx, ty, h);
             double det = (1.0 - h[0]) * (1.0 - h[2]) - h[1] * h[1];
             double w = fabs(1.0 / det);
             bx += w * (tx - ax);
@@ -658,8 +760,8 @@ int glad_oracle_quasar_batch(const float* lens, const float* ddt, int B, int n_i
             double tx = theta_obs[2 * i], ty = theta_obs[2 * i + 1], step = 0.0;
             for (int it = 0; it < NEWTON_STEPS; ++it) {
                 double ax, ay, h[3];
-                glad_oracle_deflection(p, tx, ty, &ax, &ay);
-                glad_oracle_hessian(p, tx, ty, h);
+                glad_oracle_deflection_sheet(p, lam, src, rt, tx, ty, &ax, &ay);
+                glad_oracle_hessian_sheet(p, lam, src, rt, tx, ty, h);
                 double fx = tx - ax - bx, fy = ty - ay - by;          /* lens equation residual */
                 double a11 = 1.0 - h[0], a12 = -h[1], a22 = 1.0 - h[2];
                 double det = a11 * a22 - a12 * a12;
@@ -672,7 +774,7 @@ int glad_oracle_quasar_batch(const float* lens, const float* ddt, int B, int n_i
             if (last_step) last_step[(size_t)b * n_img + i] = step;
             double ex = theta_obs[2 * i] - tx, ey = theta_obs[2 * i + 1] - ty;
             c2i += (ex * ex + ey * ey) / (sigma_theta[i] * sigma_theta[i]);
-            phi[i] = 0.5 * ((tx - bx) * (tx - bx) + (ty - by) * (ty - by)) - glad_oracle_potential(p, tx, ty);
+            phi[i] = 0.5 * ((tx - bx) * (tx - bx) + (ty - by) * (ty - by)) - glad_oracle_potential_sheet(p, lam, src, rt, tx, ty);
         }
         double c2t = 0.0;
         for (int i = 0; i < n_img; ++i) {
