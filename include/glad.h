@@ -287,6 +287,25 @@ glad_status glad_joint_loglike_full_batch(glad_ctx* ctx, const float* d_lens_par
                                           float* d_chi2_lens, float* d_chi2_dyn, float* d_chi2_img, float* d_chi2_tmd,
                                           int32_t* d_flags);
 
+/*
+ * SURVEY 8(f) rank 1, remainder: the internal mass sheet that the joint model exists to constrain (Eq. 5-9).  The paper
+ * stands a dPIE profile with r_core = 45", r_tr = 45.09" for the constant sheet (Eq. 50-51); DESIGN.md R-S1..3:
+ *   kappa_int = (1 - lambda) S(R) + lambda kappa_epl + kappa_BH,   S(R) = [1/sqrt(R^2+r_core^2) - 1/sqrt(R^2+r_tr^2)] / (1/r_core - 1/r_tr),
+ * R^2 = x^2 + y^2 about the lens centre, lambda = the constant of Eq. 51 (one per vector); the external shear (Eq. 49) and the point
+ * mass are outside the transformation.  d_lambda [>= B of the calls that follow] is a DEVICE pointer, BORROWED; NULL switches the
+ * sheet off.  While set:
+ *   - the lens half (glad_lens_image_batch and every joint entry) ray-shoots through lambda alpha_epl + alpha_sheet + shear + point mass;
+ *   - glad_quasar_chi2_batch uses the same alpha, its Jacobian and psi (Eq. 8);
+ *   - glad_joint_loglike_model_batch / _full_batch build the mass MGE of Sigma_crit kappa_int: lambda x the n_mass EPL rows followed by
+ *     n_sheet round (q' = 1) rows, the Eq. 46 expansion of Sigma_crit (1 - lambda) S(R) on [sheet_sigma_lo, sheet_sigma_hi] (the
+ *     profile's transform falls off as sigma^-3 only: take sheet_sigma_hi >> r_tr); n_mass + n_sheet <= GLAD_MAX_GAUSS and
+ *     d_mass_mge_out is then [B, n_mass + n_sheet, 3].  The caller-supplied tables of glad_joint_loglike_batch are used as given.
+ * A non-finite lambda invalidates the vector (GLAD_FLAG_LENS_INVALID).  GLAD_EINVAL unless 0 < r_core < r_tr, n_sheet >= 2,
+ * 0 < sheet_sigma_lo < sheet_sigma_hi.
+ */
+glad_status glad_set_mass_sheet(glad_ctx* ctx, const float* d_lambda, float r_core, float r_tr, int n_sheet,
+                                float sheet_sigma_lo, float sheet_sigma_hi);
+
 /* Number of kernel launches enqueued by this context since creation (for bench.py's gpu_launches). */
 long glad_launch_count(const glad_ctx* ctx);
 

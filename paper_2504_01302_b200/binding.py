@@ -22,7 +22,7 @@ EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "gl
            "glad_set_kin_data", "glad_lens_image_batch", "glad_jam_vrms_batch", "glad_joint_loglike_batch",
            "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count", "glad_profile_enable",
            "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch", "glad_set_overlap", "glad_set_light_profiles",
-           "glad_set_quasar_data", "glad_quasar_chi2_batch", "glad_joint_loglike_full_batch"]
+           "glad_set_quasar_data", "glad_quasar_chi2_batch", "glad_joint_loglike_full_batch", "glad_set_mass_sheet"]
 
 
 class GladError(RuntimeError):
@@ -91,6 +91,8 @@ def load(rebuild: bool = False):
     L.glad_joint_loglike_full_batch.restype = i
     L.glad_joint_loglike_full_batch.argtypes = [vp, vp, vp, vp, C.c_float, i, i, C.c_float, C.c_float, i, C.c_float,
                                                 C.c_float, vp, i, vp, vp, vp, vp, vp, vp]
+    L.glad_set_mass_sheet.restype = i
+    L.glad_set_mass_sheet.argtypes = [vp, vp, C.c_float, C.c_float, i, C.c_float, C.c_float]
     L.glad_launch_count.restype = l
     L.glad_launch_count.argtypes = [vp]
     _lib = L
@@ -277,12 +279,25 @@ class Glad:
         mk = lambda n, ty: out.get(n) if out.get(n) is not None else torch.empty(B, dtype=ty, device=self.device)
         ll, c2l, c2d, fl = mk("loglike", torch.float32), mk("chi2_lens", torch.float32), mk("chi2_dyn", torch.float32), mk("flags", torch.int32)
         lum = torch.empty((B, int(n_lum), 3), dtype=torch.float32, device=self.device) if want_tables else None
-        mass = torch.empty((B, int(n_mass), 3), dtype=torch.float32, device=self.device) if want_tables else None
+        n_tot = int(n_mass) + (self._n_sheet if "lambda" in self._keep else 0)
+        mass = torch.empty((B, n_tot, 3), dtype=torch.float32, device=self.device) if want_tables else None
         self._check(self.lib.glad_joint_loglike_model_batch(
             self.ctx, _p(p), _p(d), _p(dt), float(z_d), B, int(n_lum), float(lum_range[0]), float(lum_range[1]), int(n_mass),
             float(mass_range[0]), float(mass_range[1]), _p(bt), 1 if bt.dim() == 2 else 0, _p(ll), _p(c2l), _p(c2d), _p(fl),
             _p(lum), _p(mass)))
         return {"loglike": ll, "chi2_lens": c2l, "chi2_dyn": c2d, "flags": fl, "lum_mge": lum, "mass_mge": mass}
+
+    # ---- internal mass sheet (Eq. 6, 50) -------------------------------------------------------
+    def set_mass_sheet(self, lam, r_core=45.0, r_tr=45.09, n_sheet=8, sigma_lo=6.0, sigma_hi=2000.0):
+        """lam [B] (kept alive here) switches the sheet on for the batch calls that follow; None switches it off."""
+        if lam is None:
+            self._keep.pop("lambda", None)
+            self._check(self.lib.glad_set_mass_sheet(self.ctx, None, 0.0, 0.0, 0, 0.0, 0.0))
+            return
+        t = _dev(lam, torch.float32, self.device).reshape(-1)
+        self._check(self.lib.glad_set_mass_sheet(self.ctx, _p(t), float(r_core), float(r_tr), int(n_sheet), float(sigma_lo), float(sigma_hi)))
+        self._keep["lambda"] = t
+        self._n_sheet = int(n_sheet)
 
     # ---- quasar terms (Eq. 35-36) --------------------------------------------------------------
     def set_quasar_data(self, qso: dict | None):

@@ -142,6 +142,17 @@ glad_status glad_set_light_profiles(glad_ctx* c, int source_kind, int lens1_kind
     return GLAD_OK;
 }
 
+glad_status glad_set_mass_sheet(glad_ctx* c, const float* d_lambda, float r_core, float r_tr, int n_sheet, float sigma_lo, float sigma_hi) {
+    if (!c) return GLAD_EINVAL;
+    if (!d_lambda) { c->d_lambda = nullptr; return GLAD_OK; }
+    if (!(r_core > 0.f) || !(r_tr > r_core)) return fail(c, GLAD_EINVAL, "glad_set_mass_sheet: radii %g, %g", r_core, r_tr);
+    if (n_sheet < 2 || !(sigma_lo > 0.f) || !(sigma_hi > sigma_lo)) return fail(c, GLAD_EINVAL, "glad_set_mass_sheet: %d Gaussians on [%g, %g]", n_sheet, sigma_lo, sigma_hi);
+    if (n_sheet > GLAD_MAX_GAUSS) return fail(c, GLAD_ESHAPE, "glad_set_mass_sheet: more than GLAD_MAX_GAUSS Gaussians");
+    c->d_lambda = d_lambda;
+    c->ms_rc = r_core; c->ms_rt = r_tr; c->ms_n = n_sheet; c->ms_lo = sigma_lo; c->ms_hi = sigma_hi;
+    return GLAD_OK;
+}
+
 glad_status glad_set_overlap(glad_ctx* c, int on) {
     if (!c) return GLAD_EINVAL;
     if (on && !c->side_ok) return fail(c, GLAD_ESTATE, "glad_set_overlap: no side stream");
@@ -510,7 +521,9 @@ static glad_status model_impl(glad_ctx* c, const float* d_lens, const float* d_d
     if (st != GLAD_OK) return st;
     if (B == 0) return GLAD_OK;
     cudaSetDevice(c->device);
-    const size_t n_lens = (size_t)B * GLAD_NLENS, n_lum = (size_t)B * nl * 3, n_mass = (size_t)B * nm * 3;
+    const int nmt = nm + (c->d_lambda ? c->ms_n : 0);      // the mass sheet adds rows of its own
+    if (nmt > GLAD_MAX_GAUSS) return fail(c, GLAD_ESHAPE, "joint model: n_mass %d + %d sheet Gaussians exceed GLAD_MAX_GAUSS", nm, nmt - nm);
+    const size_t n_lens = (size_t)B * GLAD_NLENS, n_lum = (size_t)B * nl * 3, n_mass = (size_t)B * nmt * 3;
     st = grow(c, &c->d_model, &c->model_cap, n_lens + n_lum + n_mass);
     if (st != GLAD_OK) return st;
     float* m_lens = c->d_model;
@@ -518,7 +531,7 @@ static glad_status model_impl(glad_ctx* c, const float* d_lens, const float* d_d
     float* m_mass = d_mass_out ? d_mass_out : m_lens + n_lens + n_lum;
     CU(launch_model(c, d_lens, d_dyn, d_ddt, (double)zd, B, (c->light_kinds & 2) ? GLAD_PROFILE_CHAMELEON : GLAD_PROFILE_SERSIC, nl, lum_lo, lum_hi, nm, mass_lo, mass_hi, MGE_DEFAULT_ORDER, m_lens,
                     m_lum, m_mass), "model_kernel");
-    return joint_impl(c, m_lens, d_dyn, B, m_lum, nl, 3L * nl, m_mass, nm, 3L * nm, d_beta, per_gaussian, d_loglike, d_chi2_lens,
+    return joint_impl(c, m_lens, d_dyn, B, m_lum, nl, 3L * nl, m_mass, nmt, 3L * nmt, d_beta, per_gaussian, d_loglike, d_chi2_lens,
                       d_chi2_dyn, d_flags, quasar ? d_ddt : nullptr, d_chi2_img, d_chi2_tmd);
 }
 

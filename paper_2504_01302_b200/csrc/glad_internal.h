@@ -18,6 +18,8 @@ enum LensConstIdx {
     LC_SH_C, LC_SH_S,  // gamma_ext cos 2phi_ext, gamma_ext sin 2phi_ext
     LC_BH,        // theta_E,BH^2
     LC_VALID,     // 1 valid / 0 invalid
+    LC_MS_AMP,    // internal mass sheet: (1 - lambda) 2 r_core r_tr (0 = no sheet); LC_PREF then carries lambda
+    LC_MS_RC, LC_MS_RT,
     LC_SERSIC0 = 16,   // 3 components x 8 floats: xc, yc, cos, sin, 1/q^2, amp = Ie e^bn, k1 = bn log2e Re^(-1/n), h = 1/(2n)
     LC_SERIES = 40,    // c_n, n = 1..GLAD_EPL_MAX_TERMS : (2n-(2-t))/(2n+(2-t))
     LC_SIZE = 80
@@ -78,6 +80,11 @@ struct glad_ctx {
     const float* d_ivar;
     float* d_psf;  // ctx-owned copy [kpsf*kpsf]
     int kpsf;
+
+    // internal mass sheet (glad_set_mass_sheet): d_lambda borrowed, NULL = off
+    const float* d_lambda;
+    double ms_rc, ms_rt, ms_lo, ms_hi;
+    int ms_n;
 
     // quasar static data (copied)
     bool have_qso;
@@ -146,6 +153,7 @@ cudaError_t launch_quasar(glad_ctx* c, cudaStream_t st, const float* d_lens, con
 cudaError_t launch_kin_weights(glad_ctx* c);
 cudaError_t launch_mge1d(glad_ctx* c, int kind, const float* d_prof, int B, int n_gauss, float sigma_lo, float sigma_hi,
                          int P, float* d_mge);
+// d_mass has n_mass rows per vector, plus c->ms_n rows of the mass sheet when c->d_lambda is set
 cudaError_t launch_model(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, double zd, int B, int tracer_kind, int n_lum,
                          float lum_lo, float lum_hi, int n_mass, float mass_lo, float mass_hi, int P, float* d_lens_out,
                          float* d_lum, float* d_mass);

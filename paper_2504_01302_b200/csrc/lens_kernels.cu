@@ -13,13 +13,18 @@
 // 4 warps per 32 parameter vectors (lane = vector): warp role 0 = EPL / shear / point mass / validity, roles 1..3 =
 // one Sersic component each (the b_n root is the only long serial chain of the kernel; a warp never mixes roles).
 #define LENS_PREP_ROLES 4
-__global__ void __launch_bounds__(32 * LENS_PREP_ROLES) lens_prep_kernel(const float* __restrict__ params, int B, int kinds, float* __restrict__ consts) {
+__global__ void __launch_bounds__(32 * LENS_PREP_ROLES) lens_prep_kernel(const float* __restrict__ params, int B, int kinds,
+                                                                         const float* __restrict__ lambda, double ms_rc, double ms_rt,
+                                                                         float* __restrict__ consts) {
     const int b = blockIdx.x * 32 + (threadIdx.x & 31), role = threadIdx.x >> 5;
     if (b >= B) return;
     const float* p = params + (size_t)b * GLAD_NLENS;
     float* c = consts + (size_t)b * LC_SIZE;
     double xl = p[0], yl = p[1], thE = p[2], gam = p[3], q = p[4], pa = p[5];
     bool valid = (thE >= 0.0) && (gam > 1.0 && gam < 3.0) && (q > 0.0 && q <= 1.0) && (p[8] >= 0.f);
+    // internal mass sheet (Eq. 6 P:85 with the dPIE profile of Eq. 50; R-S1..3): kappa_int = (1-lam) S(R) + lam kappa_epl
+    const double lam = lambda ? (double)lambda[b] : 1.0;
+    if (!isfinite(lam)) valid = false;
     for (int k = 0; k < 3; ++k) {
         const float* s = p + (k == 0 ? 11 : (k == 1 ? 16 : 21));
         const bool cham = (kinds >> k) & 1;                            // Chameleon (Eq. 47): 0 < w_c < w_t
@@ -63,7 +68,12 @@ __global__ void __launch_bounds__(32 * LENS_PREP_ROLES) lens_prep_kernel(const f
     c[LC_XL] = (float)xl; c[LC_YL] = (float)yl;
     c[LC_COSPA] = (float)cos(pa); c[LC_SINPA] = (float)sin(pa);
     c[LC_Q] = (float)q; c[LC_NEGF] = (float)(-f);
-    c[LC_PREF] = (thE > 0.0) ? (float)(2.0 * pow(bTM, tt) / (1.0 + q)) : 0.f;
+    c[LC_PREF] = (thE > 0.0) ? (float)(lam * 2.0 * pow(bTM, tt) / (1.0 + q)) : 0.f;
+    if (lambda) {
+        c[LC_MS_AMP] = (float)((1.0 - lam) * 2.0 * ms_rc * ms_rt);
+        c[LC_MS_RC] = (float)ms_rc;
+        c[LC_MS_RT] = (float)ms_rt;
+    }
     c[LC_HEXP] = (float)(-0.5 * (tt - 1.0));
     int nt = 0;
     if (f > 1e-12) {
@@ -104,7 +114,8 @@ __device__ __forceinline__ float chameleon_eval(const float* __restrict__ o, flo
     float rc = rsqrtf(uc), rt = rsqrtf(ut);
     return o[5] * o[7] * rc * rt * __fdividef(1.f, fmaf(uc, rc, ut * rt));
 }
-// CH = some component is a Chameleon (kinds bit k set); the all-Sersic instantiation is the code of rows a1-a2 as before
+// CH = some component is a Chameleon (kinds bit k set) or the internal mass sheet is on; the <false> instantiation is the code of
+// rows a1-a2 as before
 template <bool CH>
 __device__ __forceinline__ float light_eval(int kinds, int k, const float* __restrict__ o, float px, float py) {
     if (CH && ((kinds >> k) & 1)) return chameleon_eval(o, px, py);
@@ -141,6 +152,16 @@ __device__ __forceinline__ float shoot(const float* __restrict__ c, float thx, f
     float bh = __fdividef(c[LC_BH], r2);
     ax = fmaf(bh, dx, ax);
     ay = fmaf(bh, dy, ay);
+    if (CH && c[LC_MS_AMP] != 0.f) {
+        // mass sheet: alpha = g (dx, dy), g = (1-lam) 2 rc rt [1 + (rt+rc)/(ht+hc)] / ((hc+rc)(ht+rt)), h = sqrt(R^2 + r^2):
+        // the closed form 2A[(hc-rc) - (ht-rt)]/R^2 with the common factor (rt - rc) divided out (no cancellation in fp32)
+        const float rc = c[LC_MS_RC], rt = c[LC_MS_RT];
+        const float rr = fmaf(dx, dx, dy * dy);
+        const float hc = sqrtf(fmaf(rc, rc, rr)), ht = sqrtf(fmaf(rt, rt, rr));
+        const float gs = c[LC_MS_AMP] * (1.f + (rt + rc) / (ht + hc)) / ((hc + rc) * (ht + rt));   // IEEE divisions: this path is optional
+        ax = fmaf(gs, dx, ax);
+        ay = fmaf(gs, dy, ay);
+    }
     float v = 0.f;
     if (has_src) v += light_eval<CH>(kinds, 0, c + LC_SERSIC0, thx - ax, thy - ay);
     if (has_l1) v += light_eval<CH>(kinds, 1, c + LC_SERSIC0 + LC_SERSIC_STRIDE, thx, thy);
@@ -272,7 +293,8 @@ __global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict
 
 cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B) {
     ProfScope ps(c, GK_LENS_PREP, c->lens_stream);
-    lens_prep_kernel<<<(B + 31) / 32, 32 * LENS_PREP_ROLES, 0, c->lens_stream>>>(d_params, B, c->light_kinds, c->d_lens_const);
+    lens_prep_kernel<<<(B + 31) / 32, 32 * LENS_PREP_ROLES, 0, c->lens_stream>>>(d_params, B, c->light_kinds, c->d_lambda, c->ms_rc,
+                                                                                 c->ms_rt, c->d_lens_const);
     return cudaGetLastError();
 }
 
@@ -281,7 +303,7 @@ cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2
                                    (size_t)(c->grid.ny + 1) * lens_img_pitch(c->grid.nx, c->kpsf));
     if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
     static size_t configured[2] = {0, 0};
-    const int ch = c->light_kinds != 0;
+    const int ch = c->light_kinds != 0 || c->d_lambda != nullptr;
     if (smem > configured[ch]) {
         cudaError_t e = ch ? cudaFuncSetAttribute(lens_image_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
                            : cudaFuncSetAttribute(lens_image_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

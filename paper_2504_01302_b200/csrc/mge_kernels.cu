@@ -61,7 +61,7 @@ static EulerConsts euler_consts(int P) {
 // One profile of one vector: the n_gauss rows {A_n, sigma_n, q'} (Eq. 46).  Called by all warps of the CTA; warp w takes
 // Gaussians w, w + nwarps, ..; lane n = term n of the Euler sum.  bn = Sersic b_n (unused for the EPL).
 __device__ static void mge_rows(int kind, double p0, double p1, double p2, double qp, double bn, const EulerConsts& ec,
-                                int n_gauss, double sigma_lo, double dln, float* __restrict__ out_rows) {
+                                int n_gauss, double sigma_lo, double dln, float* __restrict__ out_rows, double scale = 1.0) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
     const int nterm = 2 * ec.P + 1;
     const double t = p2 - 1.0;
@@ -94,7 +94,7 @@ __device__ static void mge_rows(int kind, double p0, double p1, double p2, doubl
         if (lane == 0) {
             const double w = (g == 0 || g == n_gauss - 1) ? 0.5 : 1.0;
             float* o3 = out_rows + (size_t)g * 3;
-            o3[0] = (float)(w * term * dln / sqrt(2.0 * MGE_PI));
+            o3[0] = (float)(scale * (w * term * dln / sqrt(2.0 * MGE_PI)));
             o3[1] = (float)sigma;
             o3[2] = (float)qp;
         }
@@ -134,7 +134,8 @@ cudaError_t launch_mge1d(glad_ctx* c, int kind, const float* d_prof, int B, int 
 __global__ void __launch_bounds__(256) model_kernel(const float* __restrict__ lens, const float* __restrict__ dyn,
                                                     const float* __restrict__ ddt, double zd, int B, int tracer_kind, int n_lum, double lum_lo,
                                                     double lum_dln, int n_mass, double mass_lo, double mass_dln,
-                                                    const __grid_constant__ EulerConsts ec, float* __restrict__ lens_out,
+                                                    const float* __restrict__ lambda, double ms_rc, double ms_rt, int ms_n, double ms_lo,
+                                                    double ms_dln, const __grid_constant__ EulerConsts ec, float* __restrict__ lens_out,
                                                     float* __restrict__ lum, float* __restrict__ mass) {
     __shared__ double s_bn, s_sc;
     const int b = blockIdx.x;
@@ -153,7 +154,15 @@ __global__ void __launch_bounds__(256) model_kernel(const float* __restrict__ le
     }
     __syncthreads();
     mge_rows(tracer_kind, L[16], L[17], L[18], L[19], s_bn, ec, n_lum, lum_lo, lum_dln, lum + (size_t)b * n_lum * 3);
-    mge_rows(GLAD_PROFILE_EPL, s_sc, L[2], L[3], L[4], 0.0, ec, n_mass, mass_lo, mass_dln, mass + (size_t)b * n_mass * 3);
+    // internal mass sheet (Eq. 6, 12, 50; R-S1..3): Sigma_int = Sigma_crit [lam kappa_epl + (1 - lam) S(R)].  The EPL rows carry lam;
+    // the round sheet (q' = 1) gets ms_n rows of its own after them: it is Eq. 47's shape at q = 1 with I_0/2 = Sigma_crit (1-lam)/(1/rc - 1/rt)
+    const int nm_tot = n_mass + (lambda ? ms_n : 0);
+    const double lam = lambda ? (double)lambda[b] : 1.0;
+    float* M = mass + (size_t)b * nm_tot * 3;
+    mge_rows(GLAD_PROFILE_EPL, s_sc, L[2], L[3], L[4], 0.0, ec, n_mass, mass_lo, mass_dln, M, lam);
+    if (lambda)
+        mge_rows(GLAD_PROFILE_CHAMELEON, 2.0 * s_sc * (1.0 - lam) / (1.0 / ms_rc - 1.0 / ms_rt), ms_rc, ms_rt, 1.0, 0.0, ec, ms_n, ms_lo,
+                 ms_dln, M + (size_t)n_mass * 3);
 }
 
 cudaError_t launch_model(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, double zd, int B, int tracer_kind, int n_lum,
@@ -161,7 +170,8 @@ cudaError_t launch_model(glad_ctx* c, const float* d_lens, const float* d_dyn, c
                          float* d_lum, float* d_mass) {
     ProfScope ps(c, GK_MGE);
     const double ldln = log((double)lum_hi / (double)lum_lo) / (n_lum - 1), mdln = log((double)mass_hi / (double)mass_lo) / (n_mass - 1);
+    const double sdln = (c->d_lambda && c->ms_n > 1) ? log(c->ms_hi / c->ms_lo) / (c->ms_n - 1) : 0.0;
     model_kernel<<<B, 256, 0, c->stream>>>(d_lens, d_dyn, d_ddt, zd, B, tracer_kind, n_lum, (double)lum_lo, ldln, n_mass, (double)mass_lo, mdln,
-                                           euler_consts(P), d_lens_out, d_lum, d_mass);
+                                           c->d_lambda, c->ms_rc, c->ms_rt, c->ms_n, c->ms_lo, sdln, euler_consts(P), d_lens_out, d_lum, d_mass);
     return cudaGetLastError();
 }

@@ -21,13 +21,16 @@
 
 struct MassConst {
     double xl, yl, c, s, q, t, negf, bTM, pref0, sh_c, sh_s, bh;
+    double lam, ms_rc, ms_rt, ms_a;     // internal mass sheet (R-S1..3): ms_a = (1 - lam) rc rt, 0 = none
     int nterms;
-    bool epl;
+    bool epl, sheet;
 };
 
 struct MassEval { double ax, ay, hxx, hxy, hyy, psi; };
 
-__device__ static void mass_const(const float* __restrict__ p, MassConst& m) {
+__device__ static void mass_const(const float* __restrict__ p, double lam, double rc, double rt, bool sheet, MassConst& m) {
+    m.lam = lam; m.sheet = sheet; m.ms_rc = rc; m.ms_rt = rt;
+    m.ms_a = (1.0 - lam) * rc * rt;
     m.xl = p[0]; m.yl = p[1];
     const double thE = p[2], gam = p[3], q = p[4];
     sincos((double)p[5], &m.s, &m.c);
@@ -37,7 +40,7 @@ __device__ static void mass_const(const float* __restrict__ p, MassConst& m) {
     m.negf = -f;
     m.epl = thE > 0.0;
     m.bTM = q * pow(2.0 / (1.0 + q), 1.0 / m.t) * thE;        // b_TM = q b, b of Eq. B.3
-    m.pref0 = 2.0 * m.bTM / (1.0 + q);
+    m.pref0 = lam * 2.0 * m.bTM / (1.0 + q);        // lam kappa_epl: alpha, Hessian and psi of the EPL all carry lam
     int nt = 0;
     if (f > 1e-17) {                                          // |a_n| <= f^n: terms until f^n < 1e-17
         const double est = ceil(log(1e-17) / log(f)) + 1.0;
@@ -74,7 +77,7 @@ __device__ static void mass_eval(const MassConst& m, double thx, double thy, Mas
         const double um = exp((m.t - 1.0) * log(u));       // (b/R)^(t-1)
         const double mag = m.pref0 * um;
         const double alr = mag * (wr * sr - wi * si), ali = mag * (wr * si + wi * sr);
-        const double kap = 0.5 * tt * um * u;              // Eq. B.1: (2-t)/2 (b/R)^t
+        const double kap = m.lam * 0.5 * tt * um * u;      // lam x Eq. B.1: (2-t)/2 (b/R)^t
         double r2 = x * x + y * y;
         if (r2 < 1e-12) r2 = 1e-12;
         const double ir2 = 1.0 / r2;
@@ -106,6 +109,20 @@ __device__ static void mass_eval(const MassConst& m, double thx, double thy, Mas
     hxx += hb; hyy -= hb;
     hxy -= 2.0 * m.bh * dx * dy * ir2 * ir2;
     psi += 0.5 * m.bh * log(r2);
+    if (m.sheet) {
+        // (1 - lam) S(R), S = dPIE of Eq. 50 normalised to S(0) = 1, every difference with (rt - rc) divided out:
+        //   g = alpha_R/R = 2 a [1 + (rt+rc)/(ht+hc)] / ((hc+rc)(ht+rt)),  kappa = a (rt+rc) / ((ht+hc) hc ht),  a = (1-lam) rc rt
+        //   Hessian = g I + 2 (kappa - g) x x^T / R^2 ;  psi = 2 a/(rt-rc) {[dc - rc log1p(dc/2rc)] - [dt - rt log1p(dt/2rt)]}, d = h - r
+        const double rc = m.ms_rc, rt = m.ms_rt, R2 = dx * dx + dy * dy;
+        const double hc = sqrt(R2 + rc * rc), ht = sqrt(R2 + rt * rt);
+        const double g = 2.0 * m.ms_a * (1.0 + (rt + rc) / (ht + hc)) / ((hc + rc) * (ht + rt));
+        const double kp = m.ms_a * (rt + rc) / ((ht + hc) * hc * ht);
+        const double ee = R2 > 0.0 ? 2.0 * (kp - g) / R2 : 0.0;
+        ax += g * dx; ay += g * dy;
+        hxx += g + ee * dx * dx; hyy += g + ee * dy * dy; hxy += ee * dx * dy;
+        const double dc = R2 / (hc + rc), dt = R2 / (ht + rt);
+        psi += 2.0 * m.ms_a / (rt - rc) * ((dc - rc * log1p(dc / (2.0 * rc))) - (dt - rt * log1p(dt / (2.0 * rt))));
+    }
     e.ax = ax; e.ay = ay; e.hxx = hxx; e.hxy = hxy; e.hyy = hyy; e.psi = psi;
 }
 
@@ -115,7 +132,8 @@ __device__ __forceinline__ double group_sum(double v) {
     return v;
 }
 
-__global__ void __launch_bounds__(64) quasar_kernel(const float* __restrict__ lens, const float* __restrict__ ddt, int B,
+__global__ void __launch_bounds__(64) quasar_kernel(const float* __restrict__ lens, const float* __restrict__ ddt,
+                                                    const float* __restrict__ lambda, double ms_rc, double ms_rt, int B,
                                                     const glad_quasar_data qd, float* __restrict__ chi2_img,
                                                     float* __restrict__ chi2_tmd, double* __restrict__ theta_pre,
                                                     double* __restrict__ dt_pre, double* __restrict__ beta_out) {
@@ -125,11 +143,12 @@ __global__ void __launch_bounds__(64) quasar_kernel(const float* __restrict__ le
     const bool vec = b < B;          // whole 8-lane groups are in or out; keep every lane for the shuffles
     if (!vec) b = B - 1;
     const float* p = lens + (size_t)b * GLAD_NLENS;
-    const bool valid = (p[2] >= 0.f) && (p[3] > 1.f && p[3] < 3.f) && (p[4] > 0.f && p[4] <= 1.f) && (p[8] >= 0.f);
+    const double lam = lambda ? (double)lambda[b] : 1.0;
+    const bool valid = (p[2] >= 0.f) && (p[3] > 1.f && p[3] < 3.f) && (p[4] > 0.f && p[4] <= 1.f) && (p[8] >= 0.f) && isfinite(lam);
     const bool img = i < qd.n_img;
     const double inf = __longlong_as_double(0x7ff0000000000000LL), nan = __longlong_as_double(0x7ff8000000000000LL);
     MassConst m;
-    mass_const(p, m);
+    mass_const(p, lam, ms_rc, ms_rt, lambda != nullptr, m);
     const int ii = img ? i : 0;
     const double ox = qd.theta[2 * ii], oy = qd.theta[2 * ii + 1];
     MassEval e;
@@ -176,7 +195,7 @@ cudaError_t launch_quasar(glad_ctx* c, cudaStream_t st, const float* d_lens, con
                           float* d_chi2_tmd, double* d_theta_pre, double* d_dt_pre, double* d_beta) {
     ProfScope ps(c, GK_QUASAR, st);
     const int threads = 64, total = B * QSO_LANES;
-    quasar_kernel<<<(total + threads - 1) / threads, threads, 0, st>>>(d_lens, d_ddt, B, c->qso, d_chi2_img, d_chi2_tmd,
+    quasar_kernel<<<(total + threads - 1) / threads, threads, 0, st>>>(d_lens, d_ddt, c->d_lambda, c->ms_rc, c->ms_rt, B, c->qso, d_chi2_img, d_chi2_tmd,
                                                                       d_theta_pre, d_dt_pre, d_beta);
     return cudaGetLastError();
 }
