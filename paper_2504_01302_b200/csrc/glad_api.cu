@@ -83,12 +83,14 @@ glad_status glad_create(glad_ctx** out, int device, void* cuda_stream) {
 
 static void free_kin(glad_ctx* c) {
     void* ps[] = {c->d_xf2, c->d_yf2, c->d_xf, c->d_yf, c->d_foldx, c->d_foldy, c->d_unfoldx, c->d_unfoldy,
-                  c->d_binw, c->d_bin_cnt};
+                  c->d_binw, c->d_bin_cnt, c->d_binw_ptr, c->d_binw_nz};
     for (void* p : ps) if (p) cudaFree(p);
     c->d_xf2 = c->d_yf2 = c->d_xf = c->d_yf = nullptr;
     c->d_foldx = c->d_foldy = c->d_unfoldx = c->d_unfoldy = nullptr;
     c->d_binw = nullptr;
     c->d_bin_cnt = nullptr;
+    c->d_binw_ptr = nullptr;
+    c->d_binw_nz = nullptr;
 }
 
 void glad_destroy(glad_ctx* c) {
@@ -271,6 +273,23 @@ glad_status glad_set_kin_data(glad_ctx* c, const glad_sky_grid* g, const int32_t
     c->d_vobs = d_vobs; c->d_vivar = d_vivar; c->d_un = d_un; c->d_uw = d_uw;
     CU(launch_kin_weights(c), "kin_weights_kernel");
     CU(cudaStreamSynchronize(c->stream), "kin_weights_kernel");
+    {
+        // compact the static weights: jam_post_kernel walks only the non-zero entries of each bin's row
+        const size_t npf = (size_t)nxf * nyf;
+        std::vector<float> W((size_t)nbins * npf);
+        CU(cudaMemcpy(W.data(), c->d_binw, sizeof(float) * W.size(), cudaMemcpyDeviceToHost), "copy bin weights");
+        std::vector<int> ptr(nbins + 1, 0);
+        std::vector<float2> nz;
+        for (int l = 0; l < nbins; ++l) {
+            for (size_t i = 0; i < npf; ++i) {
+                const float w = W[(size_t)l * npf + i];
+                if (w != 0.f) { float2 e; int idx = (int)i; memcpy(&e.x, &idx, sizeof(int)); e.y = w; nz.push_back(e); }
+            }
+            ptr[l + 1] = (int)nz.size();
+        }
+        CU(upload(&c->d_binw_ptr, ptr), "upload");
+        CU(upload(&c->d_binw_nz, nz), "upload");
+    }
     c->have_kin = true;
     return GLAD_OK;
 }

@@ -103,6 +103,8 @@ struct glad_ctx {
     float* d_binw;          // ctx-owned: W_f[l][pf] = sum_{p in bin l} K(p - p') over the unfolded images p' of
                             // folded pixel pf  [nbins, nyf*nxf]  (static: bins and kernel are static data)
     int* d_bin_cnt;         // ctx-owned: spaxels per bin [nbins]
+    int* d_binw_ptr;        // ctx-owned: the non-zero entries of W_f row by row (the kernel K is compact, so a bin touches a
+    float2* d_binw_nz;      // fraction of the map): row l = entries [ptr[l], ptr[l+1]) of {folded pixel index as int bits, weight}
 
     // grow-only scratch
     float* d_lens_const; size_t lens_const_cap;

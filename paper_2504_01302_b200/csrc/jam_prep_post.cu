@@ -160,7 +160,8 @@ __global__ void __launch_bounds__(256) jam_post_kernel(const float* __restrict__
                                                       const float* __restrict__ partial, int S, int nx, int ny,
                                                       int nxf, int nyf, const float* __restrict__ xf2,
                                                       const float* __restrict__ yf2, const int* __restrict__ foldx,
-                                                      const int* __restrict__ foldy, const float* __restrict__ W,
+                                                      const int* __restrict__ foldy, const int* __restrict__ Wptr,
+                                                      const float2* __restrict__ Wnz,
                                                       const int* __restrict__ bin_cnt, int nbins,
                                                       const float* __restrict__ vobs, const float* __restrict__ vivar,
                                                       float* __restrict__ vrms, float* __restrict__ chi2,
@@ -210,16 +211,18 @@ __global__ void __launch_bounds__(256) jam_post_kernel(const float* __restrict__
             int iy = i / nx, ix = i - iy * nx;
             v2map[(size_t)b * nx * ny + i] = v2f[foldy[iy] * nxf + foldx[ix]];
         }
-    // bins: one warp per bin, lanes over folded pixels (W rows are contiguous -> coalesced)
+    // bins: one warp per bin, lanes over the non-zero weights of its row (contiguous {pixel, weight} pairs -> coalesced 8-byte
+    // loads; the kernel K is compact, so a bin touches ~1/5 of the folded map)
     float cpart = 0.f;
     const int nwarp = nthr >> 5;
     for (int l = warp; l < nbins; l += nwarp) {
-        const float* w = W + (size_t)l * npf;
         float num = 0.f, den = 0.f;
-        for (int i = lane; i < npf; i += 32) {
-            float wi = w[i];
-            num = fmaf(wi, v2f[i], num);
-            den = fmaf(wi, sbf[i], den);
+        const int e1 = Wptr[l + 1];
+        for (int e = Wptr[l] + lane; e < e1; e += 32) {
+            const float2 w = Wnz[e];
+            const int i = __float_as_int(w.x);
+            num = fmaf(w.y, v2f[i], num);
+            den = fmaf(w.y, sbf[i], den);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
@@ -257,7 +260,7 @@ cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d
     ProfScope ps(c, GK_JAM_POST);
     jam_post_kernel<<<B, 256, smem, c->stream>>>(c->d_jam_tab, jam_table_floats(nl, nmx), nl, nmx, c->d_partial, S, c->nx,
                                                 c->ny, c->nxf, c->nyf, c->d_xf2, c->d_yf2, c->d_foldx, c->d_foldy,
-                                                c->d_binw, c->d_bin_cnt, c->nbins, c->d_vobs, c->d_vivar, d_vrms,
+                                                c->d_binw_ptr, c->d_binw_nz, c->d_bin_cnt, c->nbins, c->d_vobs, c->d_vivar, d_vrms,
                                                 d_chi2, d_v2map, d_flags);
     return cudaGetLastError();
 }
