@@ -56,7 +56,7 @@ def compare(out, ref, converged):
         assert not np.isnan(got).any()
 
 
-@pytest.mark.parametrize("B,scale", [(1, 1.0), (5, 1.0), (257, 1.0), (1024, 2.0)])
+@pytest.mark.parametrize("B,scale", [(1, 1.0), (5, 1.0), (257, 1.0), (1024, 2.0), (8192, 1.5)])   # up to BASELINE.json's largest batch
 def test_quasar_terms_match_oracle_on_a_chain(glad_mod, oracle, B, scale):
     p, beta = truth(oracle)
     q = mock_quasar(oracle, p, beta, 1823.0, seed=3)
