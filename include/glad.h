@@ -292,8 +292,8 @@ glad_status glad_joint_loglike_full_batch(glad_ctx* ctx, const float* d_lens_par
  * stands a dPIE profile with r_core = 45", r_tr = 45.09" for the constant sheet (Eq. 50-51); DESIGN.md R-S1..3:
  *   kappa_int = (1 - lambda) S(R) + lambda kappa_epl + kappa_BH,   S(R) = [1/sqrt(R^2+r_core^2) - 1/sqrt(R^2+r_tr^2)] / (1/r_core - 1/r_tr),
  * R^2 = x^2 + y^2 about the lens centre, lambda = the constant of Eq. 51 (one per vector); the external shear (Eq. 49) and the point
- * mass are outside the transformation.  d_lambda [>= B of the calls that follow] is a DEVICE pointer, BORROWED; NULL switches the
- * sheet off.  While set:
+ * mass are outside the transformation.  d_lambda [n_lambda] is a DEVICE pointer, BORROWED; NULL switches the sheet off.  Vector b
+ * of a batch call reads d_lambda[b]; a batch call with B > n_lambda returns GLAD_EINVAL.  While set:
  *   - the lens half (glad_lens_image_batch and every joint entry) ray-shoots through lambda alpha_epl + alpha_sheet + shear + point mass;
  *   - glad_quasar_chi2_batch uses the same alpha, its Jacobian and psi (Eq. 8);
  *   - glad_joint_loglike_model_batch / _full_batch build the mass MGE of Sigma_crit kappa_int: lambda x the n_mass EPL rows followed by
@@ -303,7 +303,7 @@ glad_status glad_joint_loglike_full_batch(glad_ctx* ctx, const float* d_lens_par
  * A non-finite lambda invalidates the vector (GLAD_FLAG_LENS_INVALID).  GLAD_EINVAL unless 0 < r_core < r_tr, n_sheet >= 2,
  * 0 < sheet_sigma_lo < sheet_sigma_hi.
  */
-glad_status glad_set_mass_sheet(glad_ctx* ctx, const float* d_lambda, float r_core, float r_tr, int n_sheet,
+glad_status glad_set_mass_sheet(glad_ctx* ctx, const float* d_lambda, int n_lambda, float r_core, float r_tr, int n_sheet,
                                 float sheet_sigma_lo, float sheet_sigma_hi);
 
 /* Number of kernel launches enqueued by this context since creation (for bench.py's gpu_launches). */

@@ -92,7 +92,7 @@ def load(rebuild: bool = False):
     L.glad_joint_loglike_full_batch.argtypes = [vp, vp, vp, vp, C.c_float, i, i, C.c_float, C.c_float, i, C.c_float,
                                                 C.c_float, vp, i, vp, vp, vp, vp, vp, vp]
     L.glad_set_mass_sheet.restype = i
-    L.glad_set_mass_sheet.argtypes = [vp, vp, C.c_float, C.c_float, i, C.c_float, C.c_float]
+    L.glad_set_mass_sheet.argtypes = [vp, vp, i, C.c_float, C.c_float, i, C.c_float, C.c_float]
     L.glad_launch_count.restype = l
     L.glad_launch_count.argtypes = [vp]
     _lib = L
@@ -292,10 +292,10 @@ class Glad:
         """lam [B] (kept alive here) switches the sheet on for the batch calls that follow; None switches it off."""
         if lam is None:
             self._keep.pop("lambda", None)
-            self._check(self.lib.glad_set_mass_sheet(self.ctx, None, 0.0, 0.0, 0, 0.0, 0.0))
+            self._check(self.lib.glad_set_mass_sheet(self.ctx, None, 0, 0.0, 0.0, 0, 0.0, 0.0))
             return
         t = _dev(lam, torch.float32, self.device).reshape(-1)
-        self._check(self.lib.glad_set_mass_sheet(self.ctx, _p(t), float(r_core), float(r_tr), int(n_sheet), float(sigma_lo), float(sigma_hi)))
+        self._check(self.lib.glad_set_mass_sheet(self.ctx, _p(t), int(t.numel()), float(r_core), float(r_tr), int(n_sheet), float(sigma_lo), float(sigma_hi)))
         self._keep["lambda"] = t
         self._n_sheet = int(n_sheet)
 

@@ -144,13 +144,15 @@ glad_status glad_set_light_profiles(glad_ctx* c, int source_kind, int lens1_kind
     return GLAD_OK;
 }
 
-glad_status glad_set_mass_sheet(glad_ctx* c, const float* d_lambda, float r_core, float r_tr, int n_sheet, float sigma_lo, float sigma_hi) {
+glad_status glad_set_mass_sheet(glad_ctx* c, const float* d_lambda, int n_lambda, float r_core, float r_tr, int n_sheet, float sigma_lo, float sigma_hi) {
     if (!c) return GLAD_EINVAL;
     if (!d_lambda) { c->d_lambda = nullptr; return GLAD_OK; }
+    if (n_lambda <= 0) return fail(c, GLAD_EINVAL, "glad_set_mass_sheet: n_lambda = %d", n_lambda);
     if (!(r_core > 0.f) || !(r_tr > r_core)) return fail(c, GLAD_EINVAL, "glad_set_mass_sheet: radii %g, %g", r_core, r_tr);
     if (n_sheet < 2 || !(sigma_lo > 0.f) || !(sigma_hi > sigma_lo)) return fail(c, GLAD_EINVAL, "glad_set_mass_sheet: %d Gaussians on [%g, %g]", n_sheet, sigma_lo, sigma_hi);
     if (n_sheet > GLAD_MAX_GAUSS) return fail(c, GLAD_ESHAPE, "glad_set_mass_sheet: more than GLAD_MAX_GAUSS Gaussians");
     c->d_lambda = d_lambda;
+    c->n_lambda = n_lambda;
     c->ms_rc = r_core; c->ms_rt = r_tr; c->ms_n = n_sheet; c->ms_lo = sigma_lo; c->ms_hi = sigma_hi;
     return GLAD_OK;
 }
@@ -298,6 +300,7 @@ glad_status glad_set_kin_data(glad_ctx* c, const glad_sky_grid* g, const int32_t
 
 static glad_status lens_impl(glad_ctx* c, const float* d_lens, int B, float* d_images, float* d_chi2, int32_t* d_flags) {
     if (!c->have_image) return fail(c, GLAD_ESTATE, "lens: glad_set_image_data not called");
+    if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "lens: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
     if (d_chi2 && !c->d_data) return fail(c, GLAD_ESTATE, "lens: chi2 requested but no data/ivar set");
     glad_status st = grow(c, &c->d_lens_const, &c->lens_const_cap, (size_t)B * LC_SIZE);
     if (st != GLAD_OK) return st;
@@ -450,6 +453,7 @@ glad_status glad_quasar_chi2_batch(glad_ctx* c, const float* d_lens, const float
     if (!c) return GLAD_EINVAL;
     if (B < 0 || (B > 0 && (!d_lens || !d_ddt))) return fail(c, GLAD_EINVAL, "glad_quasar_chi2_batch: B=%d / null pointer", B);
     if (!c->have_qso) return fail(c, GLAD_ESTATE, "glad_quasar_chi2_batch: glad_set_quasar_data not called");
+    if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "glad_quasar_chi2_batch: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
     if (B == 0) return GLAD_OK;
     cudaSetDevice(c->device);
     CU(launch_quasar(c, c->stream, d_lens, d_ddt, B, d_chi2_img, d_chi2_tmd, d_theta_pre, d_dt_pre, d_beta), "quasar_kernel");
@@ -540,6 +544,7 @@ static glad_status model_impl(glad_ctx* c, const float* d_lens, const float* d_d
     if (st != GLAD_OK) return st;
     if (B == 0) return GLAD_OK;
     cudaSetDevice(c->device);
+    if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "joint model: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
     const int nmt = nm + (c->d_lambda ? c->ms_n : 0);      // the mass sheet adds rows of its own
     if (nmt > GLAD_MAX_GAUSS) return fail(c, GLAD_ESHAPE, "joint model: n_mass %d + %d sheet Gaussians exceed GLAD_MAX_GAUSS", nm, nmt - nm);
     const size_t n_lens = (size_t)B * GLAD_NLENS, n_lum = (size_t)B * nl * 3, n_mass = (size_t)B * nmt * 3;

@@ -84,7 +84,7 @@ struct glad_ctx {
     // internal mass sheet (glad_set_mass_sheet): d_lambda borrowed, NULL = off
     const float* d_lambda;
     double ms_rc, ms_rt, ms_lo, ms_hi;
-    int ms_n;
+    int ms_n, n_lambda;
 
     // quasar static data (copied)
     bool have_qso;

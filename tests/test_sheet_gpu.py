@@ -161,6 +161,9 @@ def test_mass_sheet_errors_and_invalid_lambda(glad_mod, oracle):
     for bad in (dict(r_core=0.0), dict(r_core=50.0), dict(n_sheet=1), dict(n_sheet=65), dict(sigma_lo=0.0), dict(sigma_hi=1.0)):
         with pytest.raises(glad_mod.GladError):
             g.set_mass_sheet(lam, **bad)
+    g.set_mass_sheet(lam[:5])                     # fewer lambdas than vectors
+    with pytest.raises(glad_mod.GladError):
+        g.lens_image_batch(L["params"])
     lam[3] = np.nan
     g.set_mass_sheet(lam)
     out = g.lens_image_batch(L["params"])
