@@ -273,3 +273,17 @@ def subset(wl: dict, idx) -> dict:
             d["lum_mge"] = np.ascontiguousarray(d["lum_mge"][idx])
         out["dyn"] = d
     return out
+
+
+def pixsrc_inputs(wl: dict, nsx: int, nsy: int, seed: int = 7) -> dict:
+    """Inputs of the pixelated-source likelihood (Eq. 37-43) for the lens vectors of `wl`: a source grid per vector
+    centred on that vector's source position (half-width ~U(0.5, 0.8) arcsec, "O(10^3)" source pixels at 32 x 32)
+    and a regularisation constant lambda = 10^U(-1, 1).  Only seeded draws; none of the method's arithmetic."""
+    rng = np.random.default_rng(seed)
+    p = wl["lens"]["params"]
+    B = p.shape[0]
+    hw = rng.uniform(0.5, 0.8, B)
+    ps = 2.0 * hw / (max(nsx, nsy) - 1)
+    sg = np.stack([p[:, 9] - (nsx - 1) / 2 * ps, p[:, 10] - (nsy - 1) / 2 * ps, ps], axis=1).astype(np.float32)
+    lam = (10.0 ** rng.uniform(-1.0, 1.0, B)).astype(np.float32)
+    return dict(src_grids=sg, lam=lam, nsx=int(nsx), nsy=int(nsy))
