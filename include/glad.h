@@ -40,6 +40,7 @@ typedef enum {
 /* per-vector flag bits written to d_flags */
 #define GLAD_FLAG_LENS_INVALID 1 /* theta_E<0, gamma not in (1,3), q not in (0,1], Sersic R_e,n,q <= 0 */
 #define GLAD_FLAG_DYN_INVALID 2  /* not deprojectable (Eq. 22), D_d<=0, M_BH<0, beta_z>=1 */
+#define GLAD_FLAG_PIXSRC_NOT_PD 8 /* glad_pixsrc_evidence_batch: F + lambda g is not positive definite */
 #define GLAD_FLAG_BIN_INVALID 4  /* a bin is empty or has V^2 < 0 (negative density) */
 
 /*
@@ -305,6 +306,34 @@ glad_status glad_joint_loglike_full_batch(glad_ctx* ctx, const float* d_lens_par
  */
 glad_status glad_set_mass_sheet(glad_ctx* ctx, const float* d_lambda, int n_lambda, float r_core, float r_tr, int n_sheet,
                                 float sheet_sigma_lo, float sheet_sigma_hi);
+
+/*
+ * the paper's own extended-image likelihood, the pixelated-source inversion of Eq. 37-43 (
+ * matrix sizes in Table 1), for B parameter vectors at once.  Static data: glad_set_image_data (grid, d_esr = data,
+ * C_d^-1 = diag(ivar) with ivar = 0 masking a pixel out, PSF).  Per vector b (DESIGN.md R-P1..5):
+ *   L   [N_pix, N_s]  image pixel CENTRE theta -> beta = theta - alpha(theta) (Eq. 33; mass part lens[0..8] only, with the
+ *                     internal mass sheet when glad_set_mass_sheet is active), bilinear weights on the source grid of n_sx x n_sy
+ *                     pixels of size d_src_grid[b,2] whose pixel (0,0) is centred at (d_src_grid[b,0], d_src_grid[b,1]); a ray
+ *                     outside the rectangle of source-pixel centres gives a zero row.  The supersampling factor is not used.
+ *   f = B L           (Eq. 38), B = the "same"-size zero-padded PSF convolution of glad_lens_image_batch
+ *   F = f^T C_d^-1 f, D = f^T C_d^-1 d_esr                                                                (Eq. 41-42)
+ *   s_MP = (F + lambda g)^-1 D, lambda = d_lambda_reg[b] > 0                                              (Eq. 40)
+ *       g = Hessian of the curvature regulariser E_S = 1/2 sum_pixels [(s_{i-1} - 2 s_i + s_{i+1})^2 + (same in j)^2], s = 0 outside
+ *   ln P(d_esr | f, lambda, g) = -chi2/2 - lambda E_S(s_MP) - 1/2 ln det(F + lambda g) + N_s/2 ln lambda + 1/2 ln det g
+ *                                - N_d/2 ln 2 pi + 1/2 sum_{ivar>0} ln ivar       (Eq. 43; Suyu et al. 2006 Eq. 19)
+ *       chi2 = sum ivar (f s_MP - d_esr)^2, N_d = number of pixels with ivar > 0.
+ * Arithmetic: rays, D, the Cholesky factorisation, the solve and the evidence in fp64; f and the contraction F in fp32.
+ * All pointers are DEVICE pointers owned by the caller: d_lens_params [B,GLAD_NLENS], d_src_grid [B,3], d_lambda_reg [B];
+ * outputs (any may be NULL): d_logev [B], d_chi2 [B], d_reg [B] (= E_S), d_s_mp [B,n_sy,n_sx], d_model [B,ny,nx] (= f s_MP),
+ * d_flags [B].  An invalid mass model (GLAD_FLAG_LENS_INVALID conditions on lens[2..4], lens[8]), lambda <= 0 or a pixel size
+ * <= 0 gives logev = -INFINITY, chi2 = +INFINITY, NaN elsewhere and GLAD_FLAG_LENS_INVALID; a matrix that is not positive
+ * definite gives the same outputs with GLAD_FLAG_PIXSRC_NOT_PD.  The batch is processed in chunks that fit scratch_mib_max
+ * MiB of context-owned device scratch (<= 0: 8192); one vector needs about 4 N_pix N_s + 8 N_s^2 bytes.
+ * GLAD_ESTATE without image data; GLAD_ESHAPE if n_sx, n_sy < 2, N_s > 4096 or one vector does not fit the scratch limit.
+ */
+glad_status glad_pixsrc_evidence_batch(glad_ctx* ctx, const float* d_lens_params, const float* d_src_grid, const float* d_lambda_reg,
+                                       int n_sx, int n_sy, int B, int scratch_mib_max, float* d_logev, float* d_chi2, float* d_reg,
+                                       float* d_s_mp, float* d_model, int32_t* d_flags);
 
 /* Number of kernel launches enqueued by this context since creation (for bench.py's gpu_launches). */
 long glad_launch_count(const glad_ctx* ctx);

@@ -31,7 +31,7 @@ from __future__ import annotations
 
 import numpy as np
 
-from . import NLENS, deflection, lens_image_batch
+from . import NLENS, deflection
 
 
 def mapping_matrix(params, grid, src_grid):
@@ -142,9 +142,9 @@ def pixsrc_batch(lens, grid, psf, data, ivar, src_grids, lam, nsx, nsy):
     sg = np.ascontiguousarray(src_grids, dtype=np.float32).reshape(B, 3)
     lam = np.ascontiguousarray(lam, dtype=np.float32).reshape(B)
     Bm = blurring_matrix(psf, int(grid["nx"]), int(grid["ny"]))
-    # a vector that row a0 rejects (Eq. 22-style validity of the 26 lens numbers) is rejected here too
-    one = dict(nx=1, ny=1, supersample=1, pix=float(grid["pix"]), x0=1.0, y0=1.0)
-    bad = lens_image_batch(lens, one, np.ones((1, 1), np.float32))["flags"] != 0
+    # the mass part must be a valid model (theta_E >= 0, 1 < gamma < 3, 0 < q <= 1, theta_E,BH^2 >= 0: the GLAD_FLAG_LENS_INVALID
+    # conditions on lens[2..4], lens[8]); the light slots lens[9..25] do not enter Eq. 37-43
+    bad = ~((lens[:, 2] >= 0) & (lens[:, 3] > 1) & (lens[:, 3] < 3) & (lens[:, 4] > 0) & (lens[:, 4] <= 1) & (lens[:, 8] >= 0))
     res = [pixsrc_evidence(lens[b], grid, psf, data, ivar,
                            dict(nx=nsx, ny=nsy, pix=float(sg[b, 2]), x0=float(sg[b, 0]), y0=float(sg[b, 1])),
                            np.float32(-1.0) if (bad[b] or not sg[b, 2] > 0) else lam[b], Bm) for b in range(B)]

@@ -16,13 +16,15 @@ NLENS, NDYN, NPROF = 26, 4, 4
 PROFILE_SERSIC, PROFILE_EPL, PROFILE_CHAMELEON = 0, 1, 2
 LIGHT_SERSIC, LIGHT_CHAMELEON = 0, 1
 FLAG_LENS_INVALID, FLAG_DYN_INVALID, FLAG_BIN_INVALID = 1, 2, 4
+FLAG_PIXSRC_NOT_PD = 8
 
 _lib = None
 EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "glad_set_image_data",
            "glad_set_kin_data", "glad_lens_image_batch", "glad_jam_vrms_batch", "glad_joint_loglike_batch",
            "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count", "glad_profile_enable",
            "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch", "glad_set_overlap", "glad_set_light_profiles",
-           "glad_set_quasar_data", "glad_quasar_chi2_batch", "glad_joint_loglike_full_batch", "glad_set_mass_sheet"]
+           "glad_set_quasar_data", "glad_quasar_chi2_batch", "glad_joint_loglike_full_batch", "glad_set_mass_sheet",
+           "glad_pixsrc_evidence_batch"]
 
 
 class GladError(RuntimeError):
@@ -93,6 +95,8 @@ def load(rebuild: bool = False):
                                                 C.c_float, vp, i, vp, vp, vp, vp, vp, vp]
     L.glad_set_mass_sheet.restype = i
     L.glad_set_mass_sheet.argtypes = [vp, vp, i, C.c_float, C.c_float, i, C.c_float, C.c_float]
+    L.glad_pixsrc_evidence_batch.restype = i
+    L.glad_pixsrc_evidence_batch.argtypes = [vp, vp, vp, vp, i, i, i, i, vp, vp, vp, vp, vp, vp]
     L.glad_launch_count.restype = l
     L.glad_launch_count.argtypes = [vp]
     _lib = L
@@ -328,6 +332,23 @@ class Glad:
         tp, dp, bb = mk(B, n, 2), mk(B, n), mk(B, 2)
         self._check(self.lib.glad_quasar_chi2_batch(self.ctx, _p(p), _p(dt), B, _p(c2i), _p(c2t), _p(tp), _p(dp), _p(bb)))
         return {"chi2_img": c2i, "chi2_tmd": c2t, "theta_pre": tp, "dt_pre": dp, "beta": bb}
+
+    def pixsrc_evidence_batch(self, lens_params, src_grids, lam, nsx, nsy, want_source=True, want_model=True, scratch_mib=0):
+        """Pixelated-source evidence (Eq. 37-43): lens [B,26], src_grids [B,3] = {x_s0, y_s0, p_s}, lam [B]."""
+        p = _dev(lens_params, torch.float32, self.device).reshape(-1, NLENS)
+        sg = _dev(src_grids, torch.float32, self.device).reshape(-1, 3)
+        lm = _dev(lam, torch.float32, self.device).reshape(-1)
+        B = p.shape[0]
+        if sg.shape[0] != B or lm.shape[0] != B:
+            raise GladError("lens, source-grid and lambda batches differ")
+        f32 = lambda *shape: torch.empty(shape, dtype=torch.float32, device=self.device)
+        ev, c2, rg = f32(B), f32(B), f32(B)
+        fl = torch.empty(B, dtype=torch.int32, device=self.device)
+        s = f32(B, int(nsy), int(nsx)) if want_source else None
+        m = f32(B, *self.image_shape) if want_model else None
+        self._check(self.lib.glad_pixsrc_evidence_batch(self.ctx, _p(p), _p(sg), _p(lm), int(nsx), int(nsy), B, int(scratch_mib),
+                                                        _p(ev), _p(c2), _p(rg), _p(s), _p(m), _p(fl)))
+        return {"logev": ev, "chi2": c2, "reg": rg, "s_mp": s, "model": m, "flags": fl}
 
     def joint_loglike_full_batch(self, lens_params, dyn_params, ddt, z_d, n_lum, lum_range, n_mass, mass_range, beta, out=None):
         p = _dev(lens_params, torch.float32, self.device).reshape(-1, NLENS)

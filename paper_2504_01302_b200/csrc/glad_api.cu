@@ -101,7 +101,7 @@ void glad_destroy(glad_ctx* c) {
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     free_kin(c);
-    void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage, c->d_model, c->d_qtmp};
+    void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage, c->d_model, c->d_qtmp, c->d_pix};
     for (void* p : ps) if (p) cudaFree(p);
     for (cudaEvent_t e : c->prof_ev) if (e) cudaEventDestroy(e);
     delete c;
@@ -457,6 +457,45 @@ glad_status glad_quasar_chi2_batch(glad_ctx* c, const float* d_lens, const float
     if (B == 0) return GLAD_OK;
     cudaSetDevice(c->device);
     CU(launch_quasar(c, c->stream, d_lens, d_ddt, B, d_chi2_img, d_chi2_tmd, d_theta_pre, d_dt_pre, d_beta), "quasar_kernel");
+    return GLAD_OK;
+}
+
+glad_status glad_pixsrc_evidence_batch(glad_ctx* c, const float* d_lens, const float* d_src_grid, const float* d_lam, int nsx, int nsy,
+                                       int B, int scratch_mib_max, float* d_logev, float* d_chi2, float* d_reg, float* d_s_mp,
+                                       float* d_model, int32_t* d_flags) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && (!d_lens || !d_src_grid || !d_lam))) return fail(c, GLAD_EINVAL, "glad_pixsrc_evidence_batch: B=%d / null pointer", B);
+    if (!c->have_image || !c->d_data || !c->d_ivar) return fail(c, GLAD_ESTATE, "glad_pixsrc_evidence_batch: glad_set_image_data (with data and ivar) not called");
+    if (nsx < 2 || nsy < 2 || (long)nsx * nsy > 4096) return fail(c, GLAD_ESHAPE, "glad_pixsrc_evidence_batch: source grid %d x %d (need >= 2 x 2, N_s <= 4096)", nsx, nsy);
+    if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "glad_pixsrc_evidence_batch: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
+    if (B == 0) return GLAD_OK;
+    cudaSetDevice(c->device);
+    const int npix = c->grid.nx * c->grid.ny, ns = nsx * nsy;
+    const size_t cap = (size_t)(scratch_mib_max > 0 ? scratch_mib_max : 8192) << 20;
+    const size_t one = pixsrc_scratch_bytes(npix, ns, 1);
+    if (one > cap) return fail(c, GLAD_ESHAPE, "glad_pixsrc_evidence_batch: one vector needs %zu bytes of scratch, limit %zu", one, cap);
+    int Bc = (int)(cap / one);
+    if (Bc > B) Bc = B;
+    if (Bc > 2 * c->sm_count) Bc = 2 * c->sm_count;
+    while (Bc > 1 && pixsrc_scratch_bytes(npix, ns, Bc) > cap) --Bc;
+    glad_status st = grow(c, &c->d_pix, &c->pix_cap, pixsrc_scratch_bytes(npix, ns, Bc));
+    if (st != GLAD_OK) return st;
+    // ln det g in closed form: g = kron(I, T^2) + kron(T^2, I), T the (1,-2,1) matrix with eigenvalues -2 + 2 cos(k pi/(n+1))
+    double logdet_g = 0.0;
+    for (int j = 1; j <= nsy; ++j)
+        for (int i = 1; i <= nsx; ++i) {
+            const double mx = -2.0 + 2.0 * cos(i * M_PI / (nsx + 1)), my = -2.0 + 2.0 * cos(j * M_PI / (nsy + 1));
+            logdet_g += log(mx * mx + my * my);
+        }
+    for (int b0 = 0; b0 < B; b0 += Bc) {
+        const int nb = B - b0 < Bc ? B - b0 : Bc;
+        CU(launch_pixsrc_chunk(c, c->d_pix, d_lens + (size_t)b0 * GLAD_NLENS, d_src_grid + (size_t)b0 * 3, d_lam + b0,
+                               c->d_lambda ? c->d_lambda + b0 : nullptr, nsx, nsy, nb, logdet_g, d_logev ? d_logev + b0 : nullptr,
+                               d_chi2 ? d_chi2 + b0 : nullptr, d_reg ? d_reg + b0 : nullptr,
+                               d_s_mp ? d_s_mp + (size_t)b0 * ns : nullptr, d_model ? d_model + (size_t)b0 * npix : nullptr,
+                               d_flags ? d_flags + b0 : nullptr),
+           "pixsrc kernels");
+    }
     return GLAD_OK;
 }
 

@@ -114,6 +114,7 @@ struct glad_ctx {
     int32_t* d_tmpflags; size_t tmpflags_cap; // flags_L, flags_D [B] each
     float* d_stage;      size_t stage_cap;   // device staging of glad_joint_loglike_host
     float* d_qtmp;       size_t qtmp_cap;    // chi2_img, chi2_tmd [B] each (full joint entry)
+    char* d_pix;         size_t pix_cap;     // glad_pixsrc_evidence_batch: L, f, A, D, s of one chunk (bytes)
     float* d_model;      size_t model_cap;   // glad_joint_loglike_model_batch: lens', profile rows, derived MGE tables
 
     // optional per-kernel timing (glad_profile_*): CUDA events on the context stream around each launch
@@ -159,6 +160,11 @@ cudaError_t launch_mge1d(glad_ctx* c, int kind, const float* d_prof, int B, int 
 cudaError_t launch_model(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, double zd, int B, int tracer_kind, int n_lum,
                          float lum_lo, float lum_hi, int n_mass, float mass_lo, float mass_hi, int P, float* d_lens_out,
                          float* d_lum, float* d_mass);
+// pixelated-source evidence (pixsrc_kernels.cu): bytes of scratch for a chunk of Bc vectors; the whole chain for one chunk
+size_t pixsrc_scratch_bytes(int npix, int ns, int Bc);
+cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens, const float* d_src_grid, const float* d_lam,
+                                const float* d_ms_lambda, int nsx, int nsy, int Bc, double logdet_g, float* d_logev, float* d_chi2,
+                                float* d_reg, float* d_s_mp, float* d_model, int32_t* d_flags);
 // tensor-core (tcgen05) form of row a6; supported when the folded grid has ny_f <= 128, N = terms * nx_f <= 256
 // and two operand stages fit in shared memory
 bool jam_quad_tc_supported(const glad_ctx* c, int nl, int nmx);

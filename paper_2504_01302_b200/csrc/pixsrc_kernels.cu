@@ -1,0 +1,519 @@
+// Pixelated-source extended-image likelihood of libglad for sm_100a (paper Eq. 37-43 P:269-304,
+// Table 1): for every parameter vector
+//   pixsrc_map_kernel    L   : ray-shoot every image pixel centre in fp64 (Eq. 33), bilinear weights on the vector's source grid;
+//                              L is kept as its <= 4 non-zeros per row ({top-left source pixel, (fx, fy)}), never dense
+//   pixsrc_blur_kernel   f = B L (Eq. 38): a warp per image pixel scatters PSF tap x bilinear weight into a shared-memory row
+//                              of N_s floats and streams the row out (f [N_pix, N_s] fp32, the one large intermediate)
+//   pixsrc_syrk_kernel   F = f^T C_d^-1 f (Eq. 41) + lambda g  -> A (lower triangle, fp64 store): 64 x 64 output tiles,
+//                              4 x 4 register micro-tiles, fp32 FFMA over the N_pix contraction
+//   pixsrc_rhs_kernel    D = f^T C_d^-1 d (Eq. 42), fp64 accumulation
+//   pixsrc_chol_kernel   A = L L^T in fp64 (blocked right-looking, one CTA per vector), ln det A, s_MP = A^-1 D (Eq. 40),
+//                              E_S = 1/2 s^T g s from its pixel definition
+//   pixsrc_model_kernel  f s_MP (Eq. 37) and chi^2 = sum ivar (f s - d)^2, a warp per image pixel
+//   pixsrc_final_kernel  the evidence of Eq. 43 (R-P5), flags
+// Readings R-P1..5 are stated in DESIGN.md section 2.
+#include <math.h>
+
+#include "glad_internal.h"
+#include "glad_mass_fp64.cuh"
+
+#define PX_MAP_THREADS 128
+#define PX_BLUR_WARPS 8
+#define PX_TILE 64
+#define PX_BK 16
+#define PX_NB 32           // Cholesky panel width
+#define PX_CHOL_THREADS 256
+#define PX_PP 65           // pitch (doubles) of the k-major panel tiles in shared memory: conflict-free transposed stores
+
+__device__ __forceinline__ bool pixsrc_valid(const float* __restrict__ p, float lam, float ps) {
+    return (p[2] >= 0.f) && (p[3] > 1.f && p[3] < 3.f) && (p[4] > 0.f && p[4] <= 1.f) && (p[8] >= 0.f) && (lam > 0.f) &&
+           isfinite(lam) && (ps > 0.f) && isfinite(ps);
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// L: one thread per image pixel
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(PX_MAP_THREADS) pixsrc_map_kernel(const float* __restrict__ lens, const float* __restrict__ src_grid,
+                                                                    const float* __restrict__ lam_reg, const float* __restrict__ ms_lambda,
+                                                                    double ms_rc, double ms_rt, glad_image_grid g, int nsx, int nsy,
+                                                                    int* __restrict__ idx, float2* __restrict__ wgt) {
+    const int b = blockIdx.y;
+    const int npix = g.nx * g.ny;
+    const float* p = lens + (size_t)b * GLAD_NLENS;
+    __shared__ MassConst m;
+    if (threadIdx.x == 0) mass_const(p, ms_lambda ? (double)ms_lambda[b] : 1.0, ms_rc, ms_rt, ms_lambda != nullptr, m);
+    __syncthreads();
+    const int q = blockIdx.x * PX_MAP_THREADS + threadIdx.x;
+    if (q >= npix) return;
+    const float* sg = src_grid + (size_t)b * 3;
+    int id = -1;
+    float2 w = make_float2(0.f, 0.f);
+    if (pixsrc_valid(p, lam_reg[b], sg[2])) {
+        const int iy = q / g.nx, ix = q - iy * g.nx;
+        const double thx = (double)g.x0 + ix * (double)g.pix, thy = (double)g.y0 + iy * (double)g.pix;
+        MassEval e;
+        mass_eval(m, thx, thy, e);
+        const double tx = (thx - e.ax - (double)sg[0]) / (double)sg[2], ty = (thy - e.ay - (double)sg[1]) / (double)sg[2];
+        if (isfinite(tx) && isfinite(ty) && tx >= 0.0 && ty >= 0.0 && tx < (double)(nsx - 1) && ty < (double)(nsy - 1)) {
+            const int i0 = (int)floor(tx), j0 = (int)floor(ty);
+            id = j0 * nsx + i0;
+            w = make_float2((float)(tx - i0), (float)(ty - j0));
+        }
+    }
+    idx[(size_t)b * npix + q] = id;
+    wgt[(size_t)b * npix + q] = w;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// f = B L: a warp per image pixel, row in shared memory
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(32 * PX_BLUR_WARPS) pixsrc_blur_kernel(const int* __restrict__ idx, const float2* __restrict__ wgt,
+                                                                         const float* __restrict__ psf, int kpsf, int nx, int ny,
+                                                                         int nsx, int ns, int rows_per_cta, float* __restrict__ f) {
+    extern __shared__ float px_rows[];
+    const int b = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int npix = nx * ny, cc = kpsf / 2, k2 = kpsf * kpsf;
+    float* row = px_rows + (size_t)warp * ns;
+    const int* ib = idx + (size_t)b * npix;
+    const float2* wb = wgt + (size_t)b * npix;
+    const int p0 = blockIdx.x * rows_per_cta;
+    for (int r = warp; r < rows_per_cta; r += PX_BLUR_WARPS) {
+        const int p = p0 + r;
+        if (p >= npix) break;
+        for (int i = lane; i < ns; i += 32) row[i] = 0.f;
+        __syncwarp();
+        const int iy = p / nx, ix = p - iy * nx;
+        for (int t = lane; t < k2; t += 32) {
+            const int dy = t / kpsf, dx = t - dy * kpsf;
+            const int sy = iy - (dy - cc), sx = ix - (dx - cc);
+            if (sy < 0 || sy >= ny || sx < 0 || sx >= nx) continue;
+            const int q = sy * nx + sx;
+            const int id = ib[q];
+            if (id < 0) continue;
+            const float2 w = wb[q];
+            const float a = psf[t];
+            const float ax0 = a * (1.f - w.x), ax1 = a * w.x;
+            atomicAdd(&row[id], ax0 * (1.f - w.y));
+            atomicAdd(&row[id + 1], ax1 * (1.f - w.y));
+            atomicAdd(&row[id + nsx], ax0 * w.y);
+            atomicAdd(&row[id + nsx + 1], ax1 * w.y);
+        }
+        __syncwarp();
+        float* out = f + ((size_t)b * npix + p) * ns;
+        for (int i = lane; i < ns; i += 32) out[i] = row[i];
+        __syncwarp();
+    }
+}
+
+// (T^2)[i, i'] of the (1,-2,1) second-difference matrix T with zeros outside, n points (R-P3)
+__device__ __forceinline__ double px_t2(int i, int ip, int n) {
+    const int d = i > ip ? i - ip : ip - i;
+    if (d == 0) return 4.0 + (i > 0 ? 1.0 : 0.0) + (i < n - 1 ? 1.0 : 0.0);
+    if (d == 1) return -4.0;
+    if (d == 2) return 1.0;
+    return 0.0;
+}
+__device__ __forceinline__ double px_curv(int a, int c, int nsx, int nsy) {
+    const int ja = a / nsx, ia = a - ja * nsx, jc = c / nsx, ic = c - jc * nsx;
+    double v = 0.0;
+    if (ja == jc) v += px_t2(ia, ic, nsx);
+    if (ia == ic) v += px_t2(ja, jc, nsy);
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// A = f^T diag(ivar) f + lambda g, lower triangle, 64 x 64 tiles
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) pixsrc_syrk_kernel(const float* __restrict__ f, const float* __restrict__ ivar,
+                                                          const float* __restrict__ lam_reg, int npix, int ns, int nsx, int nsy,
+                                                          double* __restrict__ A) {
+    __shared__ __align__(16) float As[PX_BK][PX_TILE];
+    __shared__ __align__(16) float Bs[PX_BK][PX_TILE];
+    const int b = blockIdx.y;
+    // tile pair (ti >= tj) from the linear index
+    int ti = (int)((sqrtf(8.f * (float)blockIdx.x + 1.f) - 1.f) * 0.5f);
+    while ((ti + 1) * (ti + 2) / 2 <= (int)blockIdx.x) ++ti;
+    while (ti * (ti + 1) / 2 > (int)blockIdx.x) --ti;
+    const int tj = blockIdx.x - ti * (ti + 1) / 2;
+    const int i0 = ti * PX_TILE, j0 = tj * PX_TILE;
+    const float* fb = f + (size_t)b * npix * ns;
+    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+    const int lr = tid >> 4, lc = (tid & 15) * 4;      // staging: row of the K-chunk, 4 consecutive columns
+    float acc[4][4];
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) acc[r][c] = 0.f;
+    for (int p0 = 0; p0 < npix; p0 += PX_BK) {
+        const int p = p0 + lr;
+        float a4[4] = {0.f, 0.f, 0.f, 0.f}, b4[4] = {0.f, 0.f, 0.f, 0.f};
+        if (p < npix) {
+            const float w = ivar[p];
+            const float* rowp = fb + (size_t)p * ns;
+            if (w != 0.f) {
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    if (i0 + lc + e < ns) a4[e] = w * rowp[i0 + lc + e];
+                    if (j0 + lc + e < ns) b4[e] = rowp[j0 + lc + e];
+                }
+            }
+        }
+        __syncthreads();
+        *reinterpret_cast<float4*>(&As[lr][lc]) = make_float4(a4[0], a4[1], a4[2], a4[3]);
+        *reinterpret_cast<float4*>(&Bs[lr][lc]) = make_float4(b4[0], b4[1], b4[2], b4[3]);
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < PX_BK; ++k) {
+            const float4 av = *reinterpret_cast<const float4*>(&As[k][ty * 4]);
+            const float4 bv = *reinterpret_cast<const float4*>(&Bs[k][tx * 4]);
+            const float ar[4] = {av.x, av.y, av.z, av.w}, br[4] = {bv.x, bv.y, bv.z, bv.w};
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) acc[r][c] = fmaf(ar[r], br[c], acc[r][c]);
+        }
+    }
+    const double lam = (double)lam_reg[b];
+    double* Ab = A + (size_t)b * ns * ns;
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int i = i0 + ty * 4 + r, j = j0 + tx * 4 + c;
+            if (i < ns && j <= i) Ab[(size_t)i * ns + j] = (double)acc[r][c] + lam * px_curv(i, j, nsx, nsy);
+        }
+}
+
+// D = f^T (ivar d): thread per source pixel, the image pixels split over blockIdx.y
+__global__ void __launch_bounds__(256) pixsrc_rhs_kernel(const float* __restrict__ f, const float* __restrict__ ivar,
+                                                         const float* __restrict__ data, int npix, int ns, int chunks,
+                                                         double* __restrict__ D) {
+    const int b = blockIdx.z, i = blockIdx.x * 256 + threadIdx.x;
+    if (i >= ns) return;
+    const int per = (npix + chunks - 1) / chunks;
+    const int pa = blockIdx.y * per, pb = min(npix, pa + per);
+    const float* fb = f + (size_t)b * npix * ns;
+    double acc = 0.0;
+    for (int p = pa; p < pb; ++p) {
+        const float w = ivar[p];
+        if (w != 0.f) acc += (double)(w * data[p]) * (double)fb[(size_t)p * ns + i];
+    }
+    atomicAdd(&D[(size_t)b * ns + i], acc);
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Cholesky, solve, regulariser: one CTA per vector, fp64
+// ------------------------------------------------------------------------------------------------------------------
+// out[b*4 + {0,1,2,3}] = {ln det A, E_S, chi2 (filled by pixsrc_model_kernel), not-positive-definite flag}
+__global__ void __launch_bounds__(PX_CHOL_THREADS) pixsrc_chol_kernel(double* __restrict__ A, const double* __restrict__ D, int ns,
+                                                                      int nsx, int nsy, double* __restrict__ s_out,
+                                                                      double* __restrict__ out) {
+    extern __shared__ double px_sm[];
+    double* L11 = px_sm;                         // [32][33]
+    double* Pi = L11 + PX_NB * (PX_NB + 1);      // [32][PX_PP] (k-major): rows of the 64-row tile along the pitch
+    double* Pj = Pi + PX_NB * PX_PP;
+    double* yv = Pj + PX_NB * PX_PP;             // [ns]
+    double* red = yv + ns;                       // [8][32]
+    __shared__ int bad;
+    __shared__ double logdet;
+    const int b = blockIdx.x, tid = threadIdx.x;
+    double* Ab = A + (size_t)b * ns * ns;
+    if (tid == 0) { bad = 0; logdet = 0.0; }
+    __syncthreads();
+
+    for (int k0 = 0; k0 < ns; k0 += PX_NB) {
+        const int nb = min(PX_NB, ns - k0);
+        // diagonal block -> shared
+        for (int e = tid; e < PX_NB * PX_NB; e += PX_CHOL_THREADS) {
+            const int r = e >> 5, c = e & 31;
+            L11[r * (PX_NB + 1) + c] = (r < nb && c <= r) ? Ab[(size_t)(k0 + r) * ns + k0 + c] : (r == c ? 1.0 : 0.0);
+        }
+        __syncthreads();
+        for (int j = 0; j < nb; ++j) {
+            if (tid == 0) {
+                const double d = L11[j * (PX_NB + 1) + j];
+                if (!(d > 0.0) || !isfinite(d)) { bad = 1; L11[j * (PX_NB + 1) + j] = 1.0; }
+                else { L11[j * (PX_NB + 1) + j] = sqrt(d); logdet += log(d); }
+            }
+            __syncthreads();
+            const double dj = L11[j * (PX_NB + 1) + j];
+            if (tid > j && tid < nb) L11[tid * (PX_NB + 1) + j] /= dj;
+            __syncthreads();
+            for (int e = tid; e < PX_NB * PX_NB; e += PX_CHOL_THREADS) {
+                const int r = e >> 5, c = e & 31;
+                if (c > j && r >= c && r < nb) L11[r * (PX_NB + 1) + c] -= L11[r * (PX_NB + 1) + j] * L11[c * (PX_NB + 1) + j];
+            }
+            __syncthreads();
+        }
+        // write the factored diagonal block back
+        for (int e = tid; e < PX_NB * PX_NB; e += PX_CHOL_THREADS) {
+            const int r = e >> 5, c = e & 31;
+            if (r < nb && c <= r) Ab[(size_t)(k0 + r) * ns + k0 + c] = L11[r * (PX_NB + 1) + c];
+        }
+        const int r0 = k0 + nb;
+        if (r0 >= ns) break;
+        // panel: L21[i, :] = A[i, k0:k0+nb] L11^-T, a thread per row (nb == PX_NB here: only the last block is ragged)
+        for (int i = r0 + tid; i < ns; i += PX_CHOL_THREADS) {
+            double x[PX_NB];
+            double* arow = Ab + (size_t)i * ns + k0;
+#pragma unroll
+            for (int c = 0; c < PX_NB; ++c) x[c] = arow[c];
+#pragma unroll
+            for (int c = 0; c < PX_NB; ++c) {
+                double v = x[c];
+#pragma unroll
+                for (int k = 0; k < c; ++k) v -= x[k] * L11[c * (PX_NB + 1) + k];
+                x[c] = v / L11[c * (PX_NB + 1) + c];
+            }
+#pragma unroll
+            for (int c = 0; c < PX_NB; ++c) arow[c] = x[c];
+        }
+        __syncthreads();
+        // trailing update: A[i, j] -= sum_k L21[i, k] L21[j, k], i >= j >= r0, 64 x 64 tiles
+        const int nt = (ns - r0 + PX_TILE - 1) / PX_TILE;
+        const int ty = tid >> 4, tx = tid & 15;
+        for (int ti = 0; ti < nt; ++ti)
+            for (int tj = 0; tj <= ti; ++tj) {
+                const int ib = r0 + ti * PX_TILE, jb = r0 + tj * PX_TILE;
+                for (int e = tid; e < PX_NB * PX_TILE; e += PX_CHOL_THREADS) {
+                    const int r = e >> 5, k = e & 31;          // consecutive threads read consecutive k of one row
+                    Pi[k * PX_PP + r] = (ib + r < ns) ? Ab[(size_t)(ib + r) * ns + k0 + k] : 0.0;
+                    Pj[k * PX_PP + r] = (jb + r < ns) ? Ab[(size_t)(jb + r) * ns + k0 + k] : 0.0;
+                }
+                __syncthreads();
+                double acc[4][4];
+#pragma unroll
+                for (int r = 0; r < 4; ++r)
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) acc[r][c] = 0.0;
+#pragma unroll 8
+                for (int k = 0; k < PX_NB; ++k) {
+                    double ar[4], br[4];
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) { ar[r] = Pi[k * PX_PP + ty * 4 + r]; br[r] = Pj[k * PX_PP + tx * 4 + r]; }
+#pragma unroll
+                    for (int r = 0; r < 4; ++r)
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) acc[r][c] = fma(ar[r], br[c], acc[r][c]);
+                }
+#pragma unroll
+                for (int r = 0; r < 4; ++r)
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        const int i = ib + ty * 4 + r, j = jb + tx * 4 + c;
+                        if (i < ns && j <= i) Ab[(size_t)i * ns + j] -= acc[r][c];
+                    }
+                __syncthreads();
+            }
+    }
+    __syncthreads();
+
+    // forward substitution L y = D
+    const int warp = tid >> 5, lane = tid & 31;
+    const double* Db = D + (size_t)b * ns;
+    for (int k0 = 0; k0 < ns; k0 += PX_NB) {
+        const int nb = min(PX_NB, ns - k0);
+        for (int r = warp; r < nb; r += PX_CHOL_THREADS / 32) {
+            const double* lrow = Ab + (size_t)(k0 + r) * ns;
+            double v = 0.0;
+            for (int c = lane; c < k0; c += 32) v += lrow[c] * yv[c];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane == 0) yv[k0 + r] = Db[k0 + r] - v;
+        }
+        __syncthreads();
+        if (warp == 0) {
+            for (int r = 0; r < nb; ++r) {
+                const double* lrow = Ab + (size_t)(k0 + r) * ns + k0;
+                double v = (lane < r) ? lrow[lane] * yv[k0 + lane] : 0.0;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                if (lane == 0) yv[k0 + r] = (yv[k0 + r] - v) / lrow[r];
+                __syncwarp();
+            }
+        }
+        __syncthreads();
+    }
+    // backward substitution L^T s = y (s overwrites yv from the end)
+    const int nblk = (ns + PX_NB - 1) / PX_NB;
+    for (int kb = nblk - 1; kb >= 0; --kb) {
+        const int k0 = kb * PX_NB, nb = min(PX_NB, ns - k0);
+        // t_c = sum_{r >= k0 + nb} L[r, k0 + c] s_r : 8 row groups x 32 columns
+        double v = 0.0;
+        if (lane < nb)
+            for (int r = k0 + nb + warp; r < ns; r += PX_CHOL_THREADS / 32) v += Ab[(size_t)r * ns + k0 + lane] * yv[r];
+        red[warp * 32 + lane] = v;
+        __syncthreads();
+        if (warp == 0) {
+            double t = 0.0;
+#pragma unroll
+            for (int g2 = 0; g2 < PX_CHOL_THREADS / 32; ++g2) t += red[g2 * 32 + lane];
+            if (lane < nb) yv[k0 + lane] -= t;
+            __syncwarp();
+            for (int c = nb - 1; c >= 0; --c) {
+                // s_c = (y_c - sum_{r in block, r > c} L[k0 + r, k0 + c] s_r) / L[c, c]
+                double u = (lane > c && lane < nb) ? Ab[(size_t)(k0 + lane) * ns + k0 + c] * yv[k0 + lane] : 0.0;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) u += __shfl_xor_sync(0xffffffffu, u, o);
+                if (lane == 0) yv[k0 + c] = (yv[k0 + c] - u) / Ab[(size_t)(k0 + c) * ns + k0 + c];
+                __syncwarp();
+            }
+        }
+        __syncthreads();
+    }
+    // E_S = 1/2 sum_pixels [(s_{i-1} - 2 s_i + s_{i+1})^2 + (s_{j-1} - 2 s_j + s_{j+1})^2], s = 0 outside (R-P3)
+    double es = 0.0;
+    for (int a = tid; a < ns; a += PX_CHOL_THREADS) {
+        const int j = a / nsx, i = a - j * nsx;
+        const double s0 = yv[a];
+        const double dx = (i > 0 ? yv[a - 1] : 0.0) - 2.0 * s0 + (i < nsx - 1 ? yv[a + 1] : 0.0);
+        const double dy = (j > 0 ? yv[a - nsx] : 0.0) - 2.0 * s0 + (j < nsy - 1 ? yv[a + nsx] : 0.0);
+        es += 0.5 * (dx * dx + dy * dy);
+        s_out[(size_t)b * ns + a] = s0;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) es += __shfl_xor_sync(0xffffffffu, es, o);
+    __syncthreads();
+    if (lane == 0) red[warp] = es;
+    __syncthreads();
+    if (tid == 0) {
+        double t = 0.0;
+        for (int w = 0; w < PX_CHOL_THREADS / 32; ++w) t += red[w];
+        out[(size_t)b * 4 + 0] = logdet;
+        out[(size_t)b * 4 + 1] = t;
+        out[(size_t)b * 4 + 3] = bad ? 1.0 : 0.0;
+    }
+}
+
+// model = f s, chi2 = sum ivar (model - d)^2 : a warp per image pixel, 64 pixels per CTA
+__global__ void __launch_bounds__(256) pixsrc_model_kernel(const float* __restrict__ f, const double* __restrict__ s,
+                                                           const float* __restrict__ ivar, const float* __restrict__ data, int npix,
+                                                           int ns, float* __restrict__ model, long model_stride,
+                                                           double* __restrict__ out) {
+    extern __shared__ double px_s[];
+    const int b = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int i = threadIdx.x; i < ns; i += 256) px_s[i] = s[(size_t)b * ns + i];
+    __syncthreads();
+    double c2 = 0.0;
+    const int per = 64;
+    for (int r = warp; r < per; r += 8) {
+        const int p = blockIdx.x * per + r;
+        if (p >= npix) break;
+        const float* row = f + ((size_t)b * npix + p) * ns;
+        double v = 0.0;
+        for (int i = lane; i < ns; i += 32) v += (double)row[i] * px_s[i];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) {
+            if (model) model[(size_t)b * model_stride + p] = (float)v;
+            const double w = (double)ivar[p];
+            if (w != 0.0) { const double rr = v - (double)data[p]; c2 += w * rr * rr; }
+        }
+    }
+    if (lane == 0 && c2 != 0.0) atomicAdd(&out[(size_t)b * 4 + 2], c2);
+}
+
+// N_d and sum ln ivar over the unmasked pixels (static data; one CTA)
+__global__ void __launch_bounds__(256) pixsrc_static_kernel(const float* __restrict__ ivar, int npix, double* __restrict__ st) {
+    __shared__ double r1[256], r2[256];
+    double n = 0.0, sl = 0.0;
+    for (int p = threadIdx.x; p < npix; p += 256) {
+        const float w = ivar[p];
+        if (w > 0.f) { n += 1.0; sl += log((double)w); }
+    }
+    r1[threadIdx.x] = n; r2[threadIdx.x] = sl;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) { r1[threadIdx.x] += r1[threadIdx.x + o]; r2[threadIdx.x] += r2[threadIdx.x + o]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { st[0] = r1[0]; st[1] = r2[0]; }
+}
+
+__global__ void pixsrc_final_kernel(const float* __restrict__ lens, const float* __restrict__ src_grid, const float* __restrict__ lam_reg,
+                                    const float* __restrict__ ms_lambda, const double* __restrict__ out, const double* __restrict__ st,
+                                    const double* __restrict__ s, double logdet_g, int B, int ns, int npix, float* __restrict__ logev,
+                                    float* __restrict__ chi2, float* __restrict__ reg, float* __restrict__ s_mp, float* __restrict__ model,
+                                    int32_t* __restrict__ flags) {
+    const int b = blockIdx.x;
+    if (b >= B) return;
+    const float lam = lam_reg[b];
+    bool valid = pixsrc_valid(lens + (size_t)b * GLAD_NLENS, lam, src_grid[(size_t)b * 3 + 2]);
+    if (ms_lambda && !isfinite(ms_lambda[b])) valid = false;
+    const bool notpd = out[(size_t)b * 4 + 3] != 0.0;
+    const bool ok = valid && !notpd;
+    const float inf = __int_as_float(0x7f800000), nan = __int_as_float(0x7fc00000);
+    if (threadIdx.x == 0) {
+        const double c2 = out[(size_t)b * 4 + 2], es = out[(size_t)b * 4 + 1], ld = out[(size_t)b * 4 + 0];
+        const double ev = -0.5 * c2 - (double)lam * es - 0.5 * ld + 0.5 * ns * log((double)lam) + 0.5 * logdet_g -
+                          0.5 * st[0] * 1.8378770664093454836 + 0.5 * st[1];
+        if (logev) logev[b] = ok ? (float)ev : -inf;
+        if (chi2) chi2[b] = ok ? (float)c2 : inf;
+        if (reg) reg[b] = ok ? (float)es : nan;
+        if (flags) flags[b] = (valid ? 0 : GLAD_FLAG_LENS_INVALID) | ((valid && notpd) ? GLAD_FLAG_PIXSRC_NOT_PD : 0);
+    }
+    if (s_mp)
+        for (int i = threadIdx.x; i < ns; i += blockDim.x) s_mp[(size_t)b * ns + i] = ok ? (float)s[(size_t)b * ns + i] : nan;
+    if (model && !ok)
+        for (int i = threadIdx.x; i < npix; i += blockDim.x) model[(size_t)b * npix + i] = nan;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// launcher: one chunk of Bc vectors through the whole chain on c->stream.  Scratch layout (bytes): pixsrc_scratch_bytes.
+// ------------------------------------------------------------------------------------------------------------------
+static inline size_t px_align(size_t n) { return (n + 255) & ~(size_t)255; }
+
+size_t pixsrc_scratch_bytes(int npix, int ns, int Bc) {
+    return px_align(sizeof(int) * (size_t)Bc * npix) + px_align(sizeof(float2) * (size_t)Bc * npix) +
+           px_align(sizeof(float) * (size_t)Bc * npix * ns) + px_align(sizeof(double) * (size_t)Bc * ns * ns) +
+           2 * px_align(sizeof(double) * (size_t)Bc * ns) + px_align(sizeof(double) * (size_t)Bc * 4) + px_align(sizeof(double) * 2);
+}
+
+cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens, const float* d_src_grid, const float* d_lam,
+                                const float* d_ms_lambda, int nsx, int nsy, int Bc, double logdet_g, float* d_logev, float* d_chi2,
+                                float* d_reg, float* d_s_mp, float* d_model, int32_t* d_flags) {
+    const int nx = c->grid.nx, ny = c->grid.ny, npix = nx * ny, ns = nsx * nsy;
+    cudaStream_t st = c->stream;
+    char* q = (char*)scratch;
+    int* idx = (int*)q;            q += px_align(sizeof(int) * (size_t)Bc * npix);
+    float2* wgt = (float2*)q;      q += px_align(sizeof(float2) * (size_t)Bc * npix);
+    float* f = (float*)q;          q += px_align(sizeof(float) * (size_t)Bc * npix * ns);
+    double* A = (double*)q;        q += px_align(sizeof(double) * (size_t)Bc * ns * ns);
+    double* D = (double*)q;        q += px_align(sizeof(double) * (size_t)Bc * ns);
+    double* s = (double*)q;        q += px_align(sizeof(double) * (size_t)Bc * ns);
+    double* out = (double*)q;      q += px_align(sizeof(double) * (size_t)Bc * 4);
+    double* stat = (double*)q;
+    cudaError_t e;
+    if ((e = cudaMemsetAsync(D, 0, sizeof(double) * (size_t)Bc * ns, st)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(out, 0, sizeof(double) * (size_t)Bc * 4, st)) != cudaSuccess) return e;
+
+    const int rows_per_cta = 64;
+    const size_t sm_blur = sizeof(float) * (size_t)PX_BLUR_WARPS * ns;
+    const size_t sm_chol = sizeof(double) * ((size_t)PX_NB * (PX_NB + 1) + 2 * PX_NB * PX_PP + ns + 8 * 32);
+    static size_t cfg_blur = 0, cfg_chol = 0;
+    if (sm_blur > 227 * 1024 || sm_chol > 227 * 1024) return cudaErrorInvalidConfiguration;
+    if (sm_blur > cfg_blur) {
+        if ((e = cudaFuncSetAttribute(pixsrc_blur_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_blur)) != cudaSuccess) return e;
+        cfg_blur = sm_blur;
+    }
+    if (sm_chol > cfg_chol) {
+        if ((e = cudaFuncSetAttribute(pixsrc_chol_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_chol)) != cudaSuccess) return e;
+        cfg_chol = sm_chol;
+    }
+    pixsrc_static_kernel<<<1, 256, 0, st>>>(c->d_ivar, npix, stat);
+    pixsrc_map_kernel<<<dim3((npix + PX_MAP_THREADS - 1) / PX_MAP_THREADS, Bc), PX_MAP_THREADS, 0, st>>>(
+        d_lens, d_src_grid, d_lam, d_ms_lambda, c->ms_rc, c->ms_rt, c->grid, nsx, nsy, idx, wgt);
+    pixsrc_blur_kernel<<<dim3((npix + rows_per_cta - 1) / rows_per_cta, Bc), 32 * PX_BLUR_WARPS, sm_blur, st>>>(
+        idx, wgt, c->d_psf, c->kpsf, nx, ny, nsx, ns, rows_per_cta, f);
+    const int nt = (ns + PX_TILE - 1) / PX_TILE;
+    pixsrc_syrk_kernel<<<dim3(nt * (nt + 1) / 2, Bc), 256, 0, st>>>(f, c->d_ivar, d_lam, npix, ns, nsx, nsy, A);
+    const int chunks = 16;
+    pixsrc_rhs_kernel<<<dim3((ns + 255) / 256, chunks, Bc), 256, 0, st>>>(f, c->d_ivar, c->d_data, npix, ns, chunks, D);
+    pixsrc_chol_kernel<<<Bc, PX_CHOL_THREADS, sm_chol, st>>>(A, D, ns, nsx, nsy, s, out);
+    pixsrc_model_kernel<<<dim3((npix + 63) / 64, Bc), 256, sizeof(double) * ns, st>>>(f, s, c->d_ivar, c->d_data, npix, ns, d_model,
+                                                                                      (long)npix, out);
+    pixsrc_final_kernel<<<Bc, 128, 0, st>>>(d_lens, d_src_grid, d_lam, d_ms_lambda, out, stat, s, logdet_g, Bc, ns, npix, d_logev, d_chi2,
+                                            d_reg, d_s_mp, d_model, d_flags);
+    c->launches += 8;
+    return cudaGetLastError();
+}
