@@ -341,6 +341,8 @@ class Glad:
         B = p.shape[0]
         if sg.shape[0] != B or lm.shape[0] != B:
             raise GladError("lens, source-grid and lambda batches differ")
+        if getattr(self, "image_shape", None) is None:
+            raise GladError("set_image_data has not been called")
         f32 = lambda *shape: torch.empty(shape, dtype=torch.float32, device=self.device)
         ev, c2, rg = f32(B), f32(B), f32(B)
         fl = torch.empty(B, dtype=torch.int32, device=self.device)

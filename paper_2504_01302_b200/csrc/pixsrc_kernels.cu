@@ -69,7 +69,8 @@ __global__ void __launch_bounds__(PX_MAP_THREADS) pixsrc_map_kernel(const float*
 // ------------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(32 * PX_BLUR_WARPS) pixsrc_blur_kernel(const int* __restrict__ idx, const float2* __restrict__ wgt,
                                                                          const float* __restrict__ psf, int kpsf, int nx, int ny,
-                                                                         int nsx, int ns, int rows_per_cta, float* __restrict__ f) {
+                                                                         int nsx, int ns, int rows_per_cta, float* __restrict__ f,
+                                                                         int2* __restrict__ rng) {
     extern __shared__ float px_rows[];
     const int b = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int npix = nx * ny, cc = kpsf / 2, k2 = kpsf * kpsf;
@@ -83,6 +84,7 @@ __global__ void __launch_bounds__(32 * PX_BLUR_WARPS) pixsrc_blur_kernel(const i
         for (int i = lane; i < ns; i += 32) row[i] = 0.f;
         __syncwarp();
         const int iy = p / nx, ix = p - iy * nx;
+        int lo = 0x7fffffff, hi = -1;             // first and last source pixel this row touches (row-major index)
         for (int t = lane; t < k2; t += 32) {
             const int dy = t / kpsf, dx = t - dy * kpsf;
             const int sy = iy - (dy - cc), sx = ix - (dx - cc);
@@ -97,7 +99,15 @@ __global__ void __launch_bounds__(32 * PX_BLUR_WARPS) pixsrc_blur_kernel(const i
             atomicAdd(&row[id + 1], ax1 * (1.f - w.y));
             atomicAdd(&row[id + nsx], ax0 * w.y);
             atomicAdd(&row[id + nsx + 1], ax1 * w.y);
+            lo = min(lo, id);
+            hi = max(hi, id + nsx + 1);
         }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+            hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+        }
+        if (lane == 0) rng[(size_t)b * npix + p] = make_int2(lo, hi);
         __syncwarp();
         float* out = f + ((size_t)b * npix + p) * ns;
         for (int i = lane; i < ns; i += 32) out[i] = row[i];
@@ -125,8 +135,8 @@ __device__ __forceinline__ double px_curv(int a, int c, int nsx, int nsy) {
 // A = f^T diag(ivar) f + lambda g, lower triangle, 64 x 64 tiles
 // ------------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) pixsrc_syrk_kernel(const float* __restrict__ f, const float* __restrict__ ivar,
-                                                          const float* __restrict__ lam_reg, int npix, int ns, int nsx, int nsy,
-                                                          double* __restrict__ A) {
+                                                          const int2* __restrict__ rng, const float* __restrict__ lam_reg, int npix,
+                                                          int ns, int nsx, int nsy, double* __restrict__ A) {
     __shared__ __align__(16) float As[PX_BK][PX_TILE];
     __shared__ __align__(16) float Bs[PX_BK][PX_TILE];
     const int b = blockIdx.y;
@@ -144,21 +154,28 @@ __global__ void __launch_bounds__(256) pixsrc_syrk_kernel(const float* __restric
     for (int r = 0; r < 4; ++r)
 #pragma unroll
         for (int c = 0; c < 4; ++c) acc[r][c] = 0.f;
+    const int2* rb = rng + (size_t)b * npix;
     for (int p0 = 0; p0 < npix; p0 += PX_BK) {
         const int p = p0 + lr;
-        float a4[4] = {0.f, 0.f, 0.f, 0.f}, b4[4] = {0.f, 0.f, 0.f, 0.f};
+        // a row of f is non-zero only on [lo, hi] (the PSF footprint mapped into the source plane): a chunk of PX_BK image pixels
+        // none of which touches both column tiles contributes nothing to this output tile and is skipped (uniform decision)
+        float w = 0.f;
+        bool hit = false;
         if (p < npix) {
-            const float w = ivar[p];
+            w = ivar[p];
+            const int2 r = rb[p];
+            hit = (w != 0.f) && r.x <= i0 + PX_TILE - 1 && r.y >= i0 && r.x <= j0 + PX_TILE - 1 && r.y >= j0;
+        }
+        if (!__syncthreads_or(hit)) continue;     // also orders the previous chunk's reads before the stores below
+        float a4[4] = {0.f, 0.f, 0.f, 0.f}, b4[4] = {0.f, 0.f, 0.f, 0.f};
+        if (hit) {
             const float* rowp = fb + (size_t)p * ns;
-            if (w != 0.f) {
 #pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    if (i0 + lc + e < ns) a4[e] = w * rowp[i0 + lc + e];
-                    if (j0 + lc + e < ns) b4[e] = rowp[j0 + lc + e];
-                }
+            for (int e = 0; e < 4; ++e) {
+                if (i0 + lc + e < ns) a4[e] = w * rowp[i0 + lc + e];
+                if (j0 + lc + e < ns) b4[e] = rowp[j0 + lc + e];
             }
         }
-        __syncthreads();
         *reinterpret_cast<float4*>(&As[lr][lc]) = make_float4(a4[0], a4[1], a4[2], a4[3]);
         *reinterpret_cast<float4*>(&Bs[lr][lc]) = make_float4(b4[0], b4[1], b4[2], b4[3]);
         __syncthreads();
@@ -464,7 +481,7 @@ __global__ void pixsrc_final_kernel(const float* __restrict__ lens, const float*
 static inline size_t px_align(size_t n) { return (n + 255) & ~(size_t)255; }
 
 size_t pixsrc_scratch_bytes(int npix, int ns, int Bc) {
-    return px_align(sizeof(int) * (size_t)Bc * npix) + px_align(sizeof(float2) * (size_t)Bc * npix) +
+    return px_align(sizeof(int) * (size_t)Bc * npix) + px_align(sizeof(float2) * (size_t)Bc * npix) + px_align(sizeof(int2) * (size_t)Bc * npix) +
            px_align(sizeof(float) * (size_t)Bc * npix * ns) + px_align(sizeof(double) * (size_t)Bc * ns * ns) +
            2 * px_align(sizeof(double) * (size_t)Bc * ns) + px_align(sizeof(double) * (size_t)Bc * 4) + px_align(sizeof(double) * 2);
 }
@@ -477,6 +494,7 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
     char* q = (char*)scratch;
     int* idx = (int*)q;            q += px_align(sizeof(int) * (size_t)Bc * npix);
     float2* wgt = (float2*)q;      q += px_align(sizeof(float2) * (size_t)Bc * npix);
+    int2* rng = (int2*)q;          q += px_align(sizeof(int2) * (size_t)Bc * npix);
     float* f = (float*)q;          q += px_align(sizeof(float) * (size_t)Bc * npix * ns);
     double* A = (double*)q;        q += px_align(sizeof(double) * (size_t)Bc * ns * ns);
     double* D = (double*)q;        q += px_align(sizeof(double) * (size_t)Bc * ns);
@@ -504,9 +522,9 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
     pixsrc_map_kernel<<<dim3((npix + PX_MAP_THREADS - 1) / PX_MAP_THREADS, Bc), PX_MAP_THREADS, 0, st>>>(
         d_lens, d_src_grid, d_lam, d_ms_lambda, c->ms_rc, c->ms_rt, c->grid, nsx, nsy, idx, wgt);
     pixsrc_blur_kernel<<<dim3((npix + rows_per_cta - 1) / rows_per_cta, Bc), 32 * PX_BLUR_WARPS, sm_blur, st>>>(
-        idx, wgt, c->d_psf, c->kpsf, nx, ny, nsx, ns, rows_per_cta, f);
+        idx, wgt, c->d_psf, c->kpsf, nx, ny, nsx, ns, rows_per_cta, f, rng);
     const int nt = (ns + PX_TILE - 1) / PX_TILE;
-    pixsrc_syrk_kernel<<<dim3(nt * (nt + 1) / 2, Bc), 256, 0, st>>>(f, c->d_ivar, d_lam, npix, ns, nsx, nsy, A);
+    pixsrc_syrk_kernel<<<dim3(nt * (nt + 1) / 2, Bc), 256, 0, st>>>(f, c->d_ivar, rng, d_lam, npix, ns, nsx, nsy, A);
     const int chunks = 16;
     pixsrc_rhs_kernel<<<dim3((ns + 255) / 256, chunks, Bc), 256, 0, st>>>(f, c->d_ivar, c->d_data, npix, ns, chunks, D);
     pixsrc_chol_kernel<<<Bc, PX_CHOL_THREADS, sm_chol, st>>>(A, D, ns, nsx, nsy, s, out);

@@ -1,0 +1,121 @@
+"""GPU parity of the pixelated-source evidence (glad_pixsrc_evidence_batch; paper Eq. 37-43) against the dense fp64
+oracle (oracle/pixsrc.py) on the same seeded inputs.  Tolerances: 1e-5 relative on the log-evidence (the
+bar BASELINE.json sets for a log-likelihood), 1e-4 relative on chi2 and E_S, 1e-4 of the image maximum per model pixel; the
+source pixels are compared to 2e-3 of max |s_MP| (they are the solution of a system whose condition number reaches 1e5-1e6, fed
+by an fp32 contraction; the evidence is stationary in s_MP, so it does not inherit that error)."""
+import numpy as np
+import pytest
+
+import workloads
+from test_parity_gpu import glad_mod, oracle_data_model  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+EV_RTOL, C2_RTOL, PIX_RTOL, SRC_RTOL = 1e-5, 1e-4, 1e-4, 2e-3
+
+
+def _compare(out, ref, sel=None):
+    sel = np.arange(ref["logev"].size) if sel is None else sel
+    ok = ref["flag"] == 0
+    ev = out["logev"].cpu().numpy().astype(np.float64)[sel]
+    c2 = out["chi2"].cpu().numpy().astype(np.float64)[sel]
+    rg = out["reg"].cpu().numpy().astype(np.float64)[sel]
+    fl = out["flags"].cpu().numpy()[sel]
+    assert np.array_equal(fl != 0, ~ok)
+    assert np.all(ev[~ok] == -np.inf) and np.all(c2[~ok] == np.inf)
+    assert np.max(np.abs(ev[ok] - ref["logev"][ok]) / np.abs(ref["logev"][ok])) < EV_RTOL
+    assert np.max(np.abs(c2[ok] - ref["chi2"][ok]) / ref["chi2"][ok]) < C2_RTOL
+    assert np.max(np.abs(rg[ok] - ref["reg"][ok]) / ref["reg"][ok]) < 10 * C2_RTOL
+    if out["model"] is not None:
+        m = out["model"].cpu().numpy().astype(np.float64)[sel]
+        for b in np.nonzero(ok)[0]:
+            assert np.max(np.abs(m[b] - ref["model"][b])) < PIX_RTOL * np.abs(ref["model"][b]).max()
+        assert np.all(np.isnan(m[~ok]))
+    if out["s_mp"] is not None:
+        s = out["s_mp"].cpu().numpy().astype(np.float64)[sel]
+        for b in np.nonzero(ok)[0]:
+            assert np.max(np.abs(s[b] - ref["s_mp"][b])) < SRC_RTOL * np.abs(ref["s_mp"][b]).max()
+        assert np.all(np.isnan(s[~ok]))
+
+
+def _setup(glad_mod, oracle, name, B):
+    wl = workloads.make_workload(name, oracle_data_model(oracle), B=B)
+    L = wl["lens"]
+    g = glad_mod.Glad(0)
+    g.set_image_data(L["grid"], L["psf"], L["data"], L["ivar"])
+    return wl, L, g
+
+
+@pytest.mark.parametrize("nsx,nsy", [(12, 12), (9, 14), (32, 20)])
+def test_c1_parity_ragged_source_grids(glad_mod, oracle, nsx, nsy):
+    """C1 image (40 x 40, 5 x 5 PSF); N_s = 144, 126, 640: ragged 64-tiles and Cholesky panels, n_sx != n_sy; masked pixels;
+    one invalid mass model, one lambda <= 0, one pixel size <= 0."""
+    from oracle import pixsrc
+    wl, L, g = _setup(glad_mod, oracle, "C1", 8)
+    ivar = L["ivar"].copy()
+    ivar[:3, :] = 0.0
+    ivar[17:20, 5:9] = 0.0
+    g.set_image_data(L["grid"], L["psf"], L["data"], ivar)
+    pin = workloads.pixsrc_inputs(wl, nsx, nsy)
+    lens = L["params"].copy()
+    lens[5, 4] = 1.3                       # q > 1
+    pin["lam"][6] = 0.0
+    pin["src_grids"][7, 2] = -0.01
+    out = g.pixsrc_evidence_batch(lens, pin["src_grids"], pin["lam"], nsx, nsy)
+    ref = pixsrc.pixsrc_batch(lens, L["grid"], L["psf"], L["data"], ivar, pin["src_grids"], pin["lam"], nsx, nsy)
+    assert list(ref["flag"]) == [0, 0, 0, 0, 0, 1, 1, 1]
+    _compare(out, ref)
+    assert list(out["flags"].cpu().numpy()[5:]) == [glad_mod.FLAG_LENS_INVALID] * 3
+
+
+def test_c2_parity_paper_sizes(glad_mod, oracle):
+    """C2 image (100 x 100 = the paper's N_d ~ 1e4, 21 x 21 PSF), 32 x 32 source pixels (N_s ~ 1e3, Table 1): the whole
+    batch of 300 vectors runs in two scratch chunks on the device, three of them are checked against the dense oracle."""
+    from oracle import pixsrc
+    wl, L, g = _setup(glad_mod, oracle, "C2", 300)
+    pin = workloads.pixsrc_inputs(wl, 32, 32)
+    out = g.pixsrc_evidence_batch(L["params"], pin["src_grids"], pin["lam"], 32, 32, want_model=True, want_source=True)
+    sel = np.array([0, 151, 299])
+    ref = pixsrc.pixsrc_batch(L["params"][sel], L["grid"], L["psf"], L["data"], L["ivar"], pin["src_grids"][sel], pin["lam"][sel], 32, 32)
+    assert np.all(ref["flag"] == 0)
+    _compare(out, ref, sel)
+    ev = out["logev"].cpu().numpy()
+    assert np.all(np.isfinite(ev)) and np.all(out["flags"].cpu().numpy() == 0)
+    # chunking does not change results: the same vectors alone, in a scratch limit that holds one vector at a time
+    one = g.pixsrc_evidence_batch(L["params"][sel], pin["src_grids"][sel], pin["lam"][sel], 32, 32, want_model=False, want_source=False,
+                                  scratch_mib=64)
+    assert np.allclose(one["logev"].cpu().numpy(), ev[sel], rtol=2e-6)
+
+
+def test_mass_sheet_degeneracy_of_the_evidence(glad_mod, oracle):
+    """Eq. 5-9: with a (numerically flat) internal sheet, lambda_int x EPL and the source plane scaled by lambda_int, L is unchanged,
+    so the evidence is too - the property holds at any size and needs no oracle."""
+    import torch
+    wl, L, g = _setup(glad_mod, oracle, "C1", 4)
+    pin = workloads.pixsrc_inputs(wl, 16, 16)
+    lens = L["params"].copy()
+    lens[:, 6] = 0.0                      # shear and point mass are outside the transformation
+    lens[:, 8] = 0.0
+    base = g.pixsrc_evidence_batch(lens, pin["src_grids"], pin["lam"], 16, 16)
+    lam_int = torch.tensor([0.8, 0.9, 1.1, 0.95], dtype=torch.float32, device="cuda")
+    g.set_mass_sheet(lam_int, r_core=4000.0, r_tr=8000.0)
+    sg = pin["src_grids"] * lam_int.cpu().numpy()[:, None]
+    # the sheet pulls rays towards its own centre = the lens centre: beta -> lam beta about the lens centre
+    c = lens[:, 0:2] * (1.0 - lam_int.cpu().numpy()[:, None])
+    sg[:, 0:2] += c
+    sh = g.pixsrc_evidence_batch(lens, sg, pin["lam"], 16, 16)
+    g.set_mass_sheet(None)
+    assert np.allclose(sh["chi2"].cpu().numpy(), base["chi2"].cpu().numpy(), rtol=2e-4)
+    assert np.allclose(sh["logev"].cpu().numpy(), base["logev"].cpu().numpy(), rtol=2e-5)
+
+
+def test_errors(glad_mod, oracle):
+    wl, L, g = _setup(glad_mod, oracle, "C1", 2)
+    pin = workloads.pixsrc_inputs(wl, 8, 8)
+    with pytest.raises(glad_mod.GladError):
+        g.pixsrc_evidence_batch(L["params"], pin["src_grids"], pin["lam"], 1, 8)
+    with pytest.raises(glad_mod.GladError):
+        g.pixsrc_evidence_batch(L["params"], pin["src_grids"], pin["lam"], 80, 80)
+    g2 = glad_mod.Glad(0)
+    with pytest.raises(glad_mod.GladError):
+        g2.pixsrc_evidence_batch(L["params"], pin["src_grids"], pin["lam"], 8, 8)
