@@ -220,9 +220,10 @@ double glad_bh_theta2(double mbh_msun, double ddt_mpc, double z_d);
  * Optional per-kernel timing for bench.py's roofline line: when enabled, a CUDA event pair is recorded on the
  * context stream around every kernel launch (at most 2048 launches between reads).  glad_profile_read
  * SYNCHRONISES the stream, adds the elapsed times to per-kernel totals, copies them out and clears them.
- * Kernel order: 0 lens_prep, 1 lens_image, 2 jam_prep, 3 jam_quad, 4 jam_post, 5 joint, 6 mge (mge1d / model kernel), 7 quasar.
+ * Kernel order: 0 lens_prep, 1 lens_image, 2 jam_prep, 3 jam_quad, 4 jam_post, 5 joint, 6 mge (mge1d / model kernel), 7 quasar,
+ * 8 pixsrc_map, 9 pixsrc_blur, 10 pixsrc_syrk, 11 pixsrc_rhs, 12 pixsrc_chol, 13 pixsrc_model (+ static / final kernels).
  */
-#define GLAD_NKERNELS 8
+#define GLAD_NKERNELS 14
 glad_status glad_profile_enable(glad_ctx* ctx, int on);
 glad_status glad_profile_read(glad_ctx* ctx, double* ms_out /*[GLAD_NKERNELS]*/, long* count_out /*[GLAD_NKERNELS]*/);
 

@@ -158,7 +158,8 @@ class Glad:
     def launch_count(self) -> int:
         return int(self.lib.glad_launch_count(self.ctx))
 
-    KERNELS = ("lens_prep", "lens_image", "jam_prep", "jam_quad", "jam_post", "joint", "mge", "quasar")
+    KERNELS = ("lens_prep", "lens_image", "jam_prep", "jam_quad", "jam_post", "joint", "mge", "quasar",
+               "pixsrc_map", "pixsrc_blur", "pixsrc_syrk", "pixsrc_rhs", "pixsrc_chol", "pixsrc_model")
 
     def set_light_profiles(self, source=0, lens1=0, lens2=0):
         """0 = Sersic, 1 = Chameleon (Eq. 47) per light component, for the batch calls that follow."""

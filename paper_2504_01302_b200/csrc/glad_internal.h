@@ -47,7 +47,8 @@ static inline __host__ __device__ int jam_table_floats(int nl, int nmx) {
 #define JQ_MI 8
 
 #define GLAD_PROF_MAX 2048
-enum GladKernelId { GK_LENS_PREP = 0, GK_LENS_IMAGE, GK_JAM_PREP, GK_JAM_QUAD, GK_JAM_POST, GK_JOINT, GK_MGE, GK_QUASAR };
+enum GladKernelId { GK_LENS_PREP = 0, GK_LENS_IMAGE, GK_JAM_PREP, GK_JAM_QUAD, GK_JAM_POST, GK_JOINT, GK_MGE, GK_QUASAR,
+                    GK_PIX_MAP, GK_PIX_BLUR, GK_PIX_SYRK, GK_PIX_RHS, GK_PIX_CHOL, GK_PIX_MODEL };
 
 // quasar data (glad_set_quasar_data), passed to quasar_kernel by value
 struct glad_quasar_data {

@@ -222,7 +222,7 @@ __global__ void __launch_bounds__(256) pixsrc_rhs_kernel(const float* __restrict
 // Cholesky, solve, regulariser: one CTA per vector, fp64
 // ------------------------------------------------------------------------------------------------------------------
 // out[b*4 + {0,1,2,3}] = {ln det A, E_S, chi2 (filled by pixsrc_model_kernel), not-positive-definite flag}
-__global__ void __launch_bounds__(PX_CHOL_THREADS) pixsrc_chol_kernel(double* __restrict__ A, const double* __restrict__ D, int ns,
+__global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_chol_kernel(double* __restrict__ A, const double* __restrict__ D, int ns,
                                                                       int nsx, int nsy, double* __restrict__ s_out,
                                                                       double* __restrict__ out) {
     extern __shared__ double px_sm[];
@@ -298,16 +298,23 @@ __global__ void __launch_bounds__(PX_CHOL_THREADS) pixsrc_chol_kernel(double* __
                     Pj[k * PX_PP + r] = (jb + r < ns) ? Ab[(size_t)(jb + r) * ns + k0 + k] : 0.0;
                 }
                 __syncthreads();
-                double acc[4][4];
+                // thread (ty, tx): rows ib + 4 ty + r, columns jb + tx + 16 c (consecutive lanes on consecutive columns: the Pj reads
+                // are conflict-free and the read-modify-write of A is coalesced); A is fetched before the k loop so that its latency
+                // hides behind the 512 DFMAs
+                double cur[4][4], acc[4][4];
 #pragma unroll
                 for (int r = 0; r < 4; ++r)
 #pragma unroll
-                    for (int c = 0; c < 4; ++c) acc[r][c] = 0.0;
+                    for (int c = 0; c < 4; ++c) {
+                        const int i = ib + ty * 4 + r, j = jb + tx + 16 * c;
+                        cur[r][c] = (i < ns && j <= i) ? Ab[(size_t)i * ns + j] : 0.0;
+                        acc[r][c] = 0.0;
+                    }
 #pragma unroll 8
                 for (int k = 0; k < PX_NB; ++k) {
                     double ar[4], br[4];
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) { ar[r] = Pi[k * PX_PP + ty * 4 + r]; br[r] = Pj[k * PX_PP + tx * 4 + r]; }
+                    for (int r = 0; r < 4; ++r) { ar[r] = Pi[k * PX_PP + ty * 4 + r]; br[r] = Pj[k * PX_PP + tx + 16 * r]; }
 #pragma unroll
                     for (int r = 0; r < 4; ++r)
 #pragma unroll
@@ -317,8 +324,8 @@ __global__ void __launch_bounds__(PX_CHOL_THREADS) pixsrc_chol_kernel(double* __
                 for (int r = 0; r < 4; ++r)
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
-                        const int i = ib + ty * 4 + r, j = jb + tx * 4 + c;
-                        if (i < ns && j <= i) Ab[(size_t)i * ns + j] -= acc[r][c];
+                        const int i = ib + ty * 4 + r, j = jb + tx + 16 * c;
+                        if (i < ns && j <= i) Ab[(size_t)i * ns + j] = cur[r][c] - acc[r][c];
                     }
                 __syncthreads();
             }
@@ -519,19 +526,38 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
         cfg_chol = sm_chol;
     }
     pixsrc_static_kernel<<<1, 256, 0, st>>>(c->d_ivar, npix, stat);
-    pixsrc_map_kernel<<<dim3((npix + PX_MAP_THREADS - 1) / PX_MAP_THREADS, Bc), PX_MAP_THREADS, 0, st>>>(
-        d_lens, d_src_grid, d_lam, d_ms_lambda, c->ms_rc, c->ms_rt, c->grid, nsx, nsy, idx, wgt);
-    pixsrc_blur_kernel<<<dim3((npix + rows_per_cta - 1) / rows_per_cta, Bc), 32 * PX_BLUR_WARPS, sm_blur, st>>>(
-        idx, wgt, c->d_psf, c->kpsf, nx, ny, nsx, ns, rows_per_cta, f, rng);
-    const int nt = (ns + PX_TILE - 1) / PX_TILE;
-    pixsrc_syrk_kernel<<<dim3(nt * (nt + 1) / 2, Bc), 256, 0, st>>>(f, c->d_ivar, rng, d_lam, npix, ns, nsx, nsy, A);
-    const int chunks = 16;
-    pixsrc_rhs_kernel<<<dim3((ns + 255) / 256, chunks, Bc), 256, 0, st>>>(f, c->d_ivar, c->d_data, npix, ns, chunks, D);
-    pixsrc_chol_kernel<<<Bc, PX_CHOL_THREADS, sm_chol, st>>>(A, D, ns, nsx, nsy, s, out);
-    pixsrc_model_kernel<<<dim3((npix + 63) / 64, Bc), 256, sizeof(double) * ns, st>>>(f, s, c->d_ivar, c->d_data, npix, ns, d_model,
-                                                                                      (long)npix, out);
+    c->launches++;
+    {
+        ProfScope ps(c, GK_PIX_MAP);
+        pixsrc_map_kernel<<<dim3((npix + PX_MAP_THREADS - 1) / PX_MAP_THREADS, Bc), PX_MAP_THREADS, 0, st>>>(
+            d_lens, d_src_grid, d_lam, d_ms_lambda, c->ms_rc, c->ms_rt, c->grid, nsx, nsy, idx, wgt);
+    }
+    {
+        ProfScope ps(c, GK_PIX_BLUR);
+        pixsrc_blur_kernel<<<dim3((npix + rows_per_cta - 1) / rows_per_cta, Bc), 32 * PX_BLUR_WARPS, sm_blur, st>>>(
+            idx, wgt, c->d_psf, c->kpsf, nx, ny, nsx, ns, rows_per_cta, f, rng);
+    }
+    {
+        ProfScope ps(c, GK_PIX_SYRK);
+        const int nt = (ns + PX_TILE - 1) / PX_TILE;
+        pixsrc_syrk_kernel<<<dim3(nt * (nt + 1) / 2, Bc), 256, 0, st>>>(f, c->d_ivar, rng, d_lam, npix, ns, nsx, nsy, A);
+    }
+    {
+        ProfScope ps(c, GK_PIX_RHS);
+        const int chunks = 16;
+        pixsrc_rhs_kernel<<<dim3((ns + 255) / 256, chunks, Bc), 256, 0, st>>>(f, c->d_ivar, c->d_data, npix, ns, chunks, D);
+    }
+    {
+        ProfScope ps(c, GK_PIX_CHOL);
+        pixsrc_chol_kernel<<<Bc, PX_CHOL_THREADS, sm_chol, st>>>(A, D, ns, nsx, nsy, s, out);
+    }
+    {
+        ProfScope ps(c, GK_PIX_MODEL);
+        pixsrc_model_kernel<<<dim3((npix + 63) / 64, Bc), 256, sizeof(double) * ns, st>>>(f, s, c->d_ivar, c->d_data, npix, ns, d_model,
+                                                                                          (long)npix, out);
+    }
     pixsrc_final_kernel<<<Bc, 128, 0, st>>>(d_lens, d_src_grid, d_lam, d_ms_lambda, out, stat, s, logdet_g, Bc, ns, npix, d_logev, d_chi2,
                                             d_reg, d_s_mp, d_model, d_flags);
-    c->launches += 8;
+    c->launches++;
     return cudaGetLastError();
 }
