@@ -329,7 +329,7 @@ glad_status glad_set_mass_sheet(glad_ctx* ctx, const float* d_lambda, int n_lamb
  * d_flags [B].  An invalid mass model (GLAD_FLAG_LENS_INVALID conditions on lens[2..4], lens[8]), lambda <= 0 or a pixel size
  * <= 0 gives logev = -INFINITY, chi2 = +INFINITY, NaN elsewhere and GLAD_FLAG_LENS_INVALID; a matrix that is not positive
  * definite gives the same outputs with GLAD_FLAG_PIXSRC_NOT_PD.  The batch is processed in chunks that fit scratch_mib_max
- * MiB of context-owned device scratch (<= 0: 8192); one vector needs about 4 N_pix N_s + 8 N_s^2 bytes.
+ * MiB of context-owned device scratch (<= 0: 16384); one vector needs about 4 N_pix N_s + 8 N_s^2 bytes.
  * GLAD_ESTATE without image data; GLAD_ESHAPE if n_sx, n_sy < 2, N_s > 4096 or one vector does not fit the scratch limit.
  */
 glad_status glad_pixsrc_evidence_batch(glad_ctx* ctx, const float* d_lens_params, const float* d_src_grid, const float* d_lambda_reg,

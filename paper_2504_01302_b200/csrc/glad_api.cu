@@ -471,7 +471,7 @@ glad_status glad_pixsrc_evidence_batch(glad_ctx* c, const float* d_lens, const f
     if (B == 0) return GLAD_OK;
     cudaSetDevice(c->device);
     const int npix = c->grid.nx * c->grid.ny, ns = nsx * nsy;
-    const size_t cap = (size_t)(scratch_mib_max > 0 ? scratch_mib_max : 8192) << 20;
+    const size_t cap = (size_t)(scratch_mib_max > 0 ? scratch_mib_max : 16384) << 20;
     const size_t one = pixsrc_scratch_bytes(npix, ns, 1);
     if (one > cap) return fail(c, GLAD_ESHAPE, "glad_pixsrc_evidence_batch: one vector needs %zu bytes of scratch, limit %zu", one, cap);
     int Bc = (int)(cap / one);
