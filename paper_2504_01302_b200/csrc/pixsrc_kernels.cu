@@ -4,8 +4,8 @@
 //                              L is kept as its <= 4 non-zeros per row ({top-left source pixel, (fx, fy)}), never dense
 //   pixsrc_blur_kernel   f = B L (Eq. 38): a warp per image pixel scatters PSF tap x bilinear weight into a shared-memory row
 //                              of N_s floats and streams the row out (f [N_pix, N_s] fp32, the one large intermediate)
-//   pixsrc_syrk_kernel   F = f^T C_d^-1 f (Eq. 41) + lambda g  -> A (lower triangle, fp64 store): 64 x 64 output tiles,
-//                              4 x 4 register micro-tiles, fp32 FFMA over the N_pix contraction
+//   pixsrc_syrk_kernel   F = f^T C_d^-1 f (Eq. 41) + lambda g  -> A (lower triangle, fp64 store): 128 x 128 output tiles,
+//                              8 x 8 register tiles, fp32 FFMA over the N_pix contraction
 //   pixsrc_rhs_kernel    D = f^T C_d^-1 d (Eq. 42), fp64 accumulation
 //   pixsrc_chol_kernel   A = L L^T in fp64 (blocked right-looking, one CTA per vector), ln det A, s_MP = A^-1 D (Eq. 40),
 //                              E_S = 1/2 s^T g s from its pixel definition
@@ -132,71 +132,117 @@ __device__ __forceinline__ double px_curv(int a, int c, int nsx, int nsy) {
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// A = f^T diag(ivar) f + lambda g, lower triangle, 64 x 64 tiles
+// A = f^T diag(ivar) f + lambda g, lower triangle, 128 x 128 output tiles, 8 x 8 register tiles (as four 4 x 4 quadrants 64 apart,
+// so that every LDS.128 of a quarter-warp is contiguous): 4 LDS.128 per 64 FFMA
 // ------------------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) pixsrc_syrk_kernel(const float* __restrict__ f, const float* __restrict__ ivar,
-                                                          const int2* __restrict__ rng, const float* __restrict__ lam_reg, int npix,
-                                                          int ns, int nsx, int nsy, double* __restrict__ A) {
-    __shared__ __align__(16) float As[PX_BK][PX_TILE];
-    __shared__ __align__(16) float Bs[PX_BK][PX_TILE];
+#define PX_ST 128
+__device__ __forceinline__ void px_cp_async16(void* smem, const void* gmem) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void px_cp_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void px_cp_wait1() { asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
+
+// Two shared-memory stages filled by cp.async (no staging registers): chunk c+1 streams in while chunk c is contracted.  ivar
+// stays out of the copies: row k of a chunk is scaled by Ws[k] when the a operand is read (and skipped when Ws[k] = 0).
+__global__ void __launch_bounds__(256, 2) pixsrc_syrk_kernel(const float* __restrict__ f, const float* __restrict__ ivar,
+                                                             const int2* __restrict__ rng, const float* __restrict__ lam_reg, int npix,
+                                                             int ns, int nsx, int nsy, double* __restrict__ A) {
+    __shared__ __align__(16) float As[2][PX_BK][PX_ST];
+    __shared__ __align__(16) float Bs[2][PX_BK][PX_ST];
+    __shared__ float Ws[2][PX_BK];
     const int b = blockIdx.y;
     // tile pair (ti >= tj) from the linear index
     int ti = (int)((sqrtf(8.f * (float)blockIdx.x + 1.f) - 1.f) * 0.5f);
     while ((ti + 1) * (ti + 2) / 2 <= (int)blockIdx.x) ++ti;
     while (ti * (ti + 1) / 2 > (int)blockIdx.x) --ti;
     const int tj = blockIdx.x - ti * (ti + 1) / 2;
-    const int i0 = ti * PX_TILE, j0 = tj * PX_TILE;
+    const int i0 = ti * PX_ST, j0 = tj * PX_ST;
     const float* fb = f + (size_t)b * npix * ns;
     const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
-    const int lr = tid >> 4, lc = (tid & 15) * 4;      // staging: row of the K-chunk, 4 consecutive columns
-    float acc[4][4];
-#pragma unroll
-    for (int r = 0; r < 4; ++r)
-#pragma unroll
-        for (int c = 0; c < 4; ++c) acc[r][c] = 0.f;
+    const int lr = tid >> 4, lc = (tid & 15) * 8;      // staging: row of the K-chunk, 8 consecutive columns
+    const bool vec4 = (ns & 3) == 0;
     const int2* rb = rng + (size_t)b * npix;
-    for (int p0 = 0; p0 < npix; p0 += PX_BK) {
+    float acc[8][8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) acc[r][c] = 0.f;
+
+    // A row of f is non-zero only on [lo, hi] (the PSF footprint mapped into the source plane, recorded by the blur kernel): a row
+    // that misses either column tile contributes nothing to this output tile; it is stored as zeros with weight 0, and a chunk
+    // of PX_BK image pixels without any hit is skipped altogether (uniform decision).
+    auto fill = [&](int st, int p0) -> bool {
         const int p = p0 + lr;
-        // a row of f is non-zero only on [lo, hi] (the PSF footprint mapped into the source plane): a chunk of PX_BK image pixels
-        // none of which touches both column tiles contributes nothing to this output tile and is skipped (uniform decision)
         float w = 0.f;
         bool hit = false;
         if (p < npix) {
             w = ivar[p];
             const int2 r = rb[p];
-            hit = (w != 0.f) && r.x <= i0 + PX_TILE - 1 && r.y >= i0 && r.x <= j0 + PX_TILE - 1 && r.y >= j0;
+            hit = (w != 0.f) && r.x <= i0 + PX_ST - 1 && r.y >= i0 && r.x <= j0 + PX_ST - 1 && r.y >= j0;
         }
-        if (!__syncthreads_or(hit)) continue;     // also orders the previous chunk's reads before the stores below
-        float a4[4] = {0.f, 0.f, 0.f, 0.f}, b4[4] = {0.f, 0.f, 0.f, 0.f};
-        if (hit) {
-            const float* rowp = fb + (size_t)p * ns;
+        if ((tid & 15) == 0) Ws[st][lr] = hit ? w : 0.f;
+        float* as = &As[st][lr][lc];
+        float* bs = &Bs[st][lr][lc];
+        const float* rowp = fb + (size_t)p * ns;
+        const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                if (i0 + lc + e < ns) a4[e] = w * rowp[i0 + lc + e];
-                if (j0 + lc + e < ns) b4[e] = rowp[j0 + lc + e];
+        for (int h = 0; h < 2; ++h) {
+            const int ca = i0 + lc + 4 * h, cb = j0 + lc + 4 * h;
+            if (hit && vec4 && ca < ns) px_cp_async16(as + 4 * h, rowp + ca);
+            else if (hit && !vec4) {
+                float v[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) v[e] = (ca + e < ns) ? rowp[ca + e] : 0.f;
+                *reinterpret_cast<float4*>(as + 4 * h) = make_float4(v[0], v[1], v[2], v[3]);
+            } else *reinterpret_cast<float4*>(as + 4 * h) = z;
+            if (hit && vec4 && cb < ns) px_cp_async16(bs + 4 * h, rowp + cb);
+            else if (hit && !vec4) {
+                float v[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) v[e] = (cb + e < ns) ? rowp[cb + e] : 0.f;
+                *reinterpret_cast<float4*>(bs + 4 * h) = make_float4(v[0], v[1], v[2], v[3]);
+            } else *reinterpret_cast<float4*>(bs + 4 * h) = z;
+        }
+        return hit;
+    };
+
+    const int nch = (npix + PX_BK - 1) / PX_BK;
+    bool hit_cur = fill(0, 0);
+    px_cp_commit();
+    for (int ch = 0; ch < nch; ++ch) {
+        const int st = ch & 1;
+        bool hit_nxt = false;
+        if (ch + 1 < nch) hit_nxt = fill(st ^ 1, (ch + 1) * PX_BK);
+        px_cp_commit();
+        px_cp_wait1();                                   // this thread's copies of chunk ch have landed
+        if (__syncthreads_or(hit_cur)) {                 // ... and after the barrier everybody's have
+#pragma unroll 2
+            for (int k = 0; k < PX_BK; ++k) {
+                const float wk = Ws[st][k];
+                if (wk == 0.f) continue;                 // uniform: a row that does not count
+                const float4 a0 = *reinterpret_cast<const float4*>(&As[st][k][ty * 4]);
+                const float4 a1 = *reinterpret_cast<const float4*>(&As[st][k][64 + ty * 4]);
+                const float4 b0 = *reinterpret_cast<const float4*>(&Bs[st][k][tx * 4]);
+                const float4 b1 = *reinterpret_cast<const float4*>(&Bs[st][k][64 + tx * 4]);
+                const float ar[8] = {wk * a0.x, wk * a0.y, wk * a0.z, wk * a0.w, wk * a1.x, wk * a1.y, wk * a1.z, wk * a1.w};
+                const float br[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+#pragma unroll
+                for (int r = 0; r < 8; ++r)
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) acc[r][c] = fmaf(ar[r], br[c], acc[r][c]);
             }
+            __syncthreads();                             // stage st is refilled two chunks from now
         }
-        *reinterpret_cast<float4*>(&As[lr][lc]) = make_float4(a4[0], a4[1], a4[2], a4[3]);
-        *reinterpret_cast<float4*>(&Bs[lr][lc]) = make_float4(b4[0], b4[1], b4[2], b4[3]);
-        __syncthreads();
-#pragma unroll
-        for (int k = 0; k < PX_BK; ++k) {
-            const float4 av = *reinterpret_cast<const float4*>(&As[k][ty * 4]);
-            const float4 bv = *reinterpret_cast<const float4*>(&Bs[k][tx * 4]);
-            const float ar[4] = {av.x, av.y, av.z, av.w}, br[4] = {bv.x, bv.y, bv.z, bv.w};
-#pragma unroll
-            for (int r = 0; r < 4; ++r)
-#pragma unroll
-                for (int c = 0; c < 4; ++c) acc[r][c] = fmaf(ar[r], br[c], acc[r][c]);
-        }
+        hit_cur = hit_nxt;
     }
     const double lam = (double)lam_reg[b];
     double* Ab = A + (size_t)b * ns * ns;
 #pragma unroll
-    for (int r = 0; r < 4; ++r)
+    for (int r = 0; r < 8; ++r)
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            const int i = i0 + ty * 4 + r, j = j0 + tx * 4 + c;
+        for (int c = 0; c < 8; ++c) {
+            const int i = i0 + (r >> 2) * 64 + ty * 4 + (r & 3), j = j0 + (c >> 2) * 64 + tx * 4 + (c & 3);
             if (i < ns && j <= i) Ab[(size_t)i * ns + j] = (double)acc[r][c] + lam * px_curv(i, j, nsx, nsy);
         }
 }
@@ -539,7 +585,7 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
     }
     {
         ProfScope ps(c, GK_PIX_SYRK);
-        const int nt = (ns + PX_TILE - 1) / PX_TILE;
+        const int nt = (ns + PX_ST - 1) / PX_ST;
         pixsrc_syrk_kernel<<<dim3(nt * (nt + 1) / 2, Bc), 256, 0, st>>>(f, c->d_ivar, rng, d_lam, npix, ns, nsx, nsy, A);
     }
     {

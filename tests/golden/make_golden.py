@@ -42,11 +42,22 @@ def mge_values():
             "mge_epl_sc1_te1.65_g2_q0.8_21g_0.02_50": oracle.mge1d(oracle.PROFILE_EPL, [1.0, 1.65, 2.0, 0.8], 21, 0.02, 50.0)[:, 0]}
 
 
+def pixsrc_values():
+    """Pixelated-source evidence (Eq. 37-43) of the 8 C1 vectors on 16 x 12 source grids (workloads.pixsrc_inputs)."""
+    from oracle import pixsrc
+    wl = workloads.make_workload("C1", data_model)
+    L = wl["lens"]
+    pin = workloads.pixsrc_inputs(wl, 16, 12)
+    r = pixsrc.pixsrc_batch(L["params"], L["grid"], L["psf"], L["data"], L["ivar"], pin["src_grids"], pin["lam"], 16, 12)
+    return {"c1_pixsrc_logev_16x12": r["logev"], "c1_pixsrc_chi2_16x12": r["chi2"], "c1_pixsrc_smp_vec0_16x12": r["s_mp"][0].reshape(-1)}
+
+
 def main():
     oracle.build()
     vals = {}
     vals.update(c1_values())
     vals.update(mge_values())
+    vals.update(pixsrc_values())
     for name, v in vals.items():
         np.savetxt(os.path.join(HERE, name + ".txt"), np.atleast_1d(v), fmt="%.17e",
                    header=f"{name}: written by tests/golden/make_golden.py from oracle/ only (fp64); not a published value")

@@ -20,7 +20,8 @@ def test_oracle_reproduces_golden(oracle):
     vals = {}
     vals.update(make_golden.c1_values())
     vals.update(make_golden.mge_values())
-    assert len(vals) == 7
+    vals.update(make_golden.pixsrc_values())
+    assert len(vals) == 10
     for name, v in vals.items():
         ref = load(name)
         assert np.allclose(np.ravel(v), np.ravel(ref), rtol=1e-10, atol=0), name
@@ -54,4 +55,11 @@ def test_gpu_matches_golden_c1(oracle):
         a = g.mge1d_batch(kind, np.array([prof], np.float32), 21, 0.02, 50.0).cpu().numpy()[0, :, 0].astype(np.float64)
         r = load(name)
         assert np.all(np.abs(a - r) <= 3e-7 * np.abs(r) + 1e-9 * np.abs(r).max())
+    pin = workloads.pixsrc_inputs(wl, 16, 12)
+    po = g.pixsrc_evidence_batch(L["params"], pin["src_grids"], pin["lam"], 16, 12)
+    ev, c2 = load("c1_pixsrc_logev_16x12"), load("c1_pixsrc_chi2_16x12")
+    assert np.max(np.abs(po["logev"].cpu().numpy() - ev) / np.abs(ev)) < 1e-5
+    assert np.max(np.abs(po["chi2"].cpu().numpy() - c2) / c2) < 1e-4
+    s0 = load("c1_pixsrc_smp_vec0_16x12")
+    assert np.max(np.abs(po["s_mp"].cpu().numpy()[0].reshape(-1) - s0)) < 2e-3 * np.abs(s0).max()
     g.close()

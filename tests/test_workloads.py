@@ -39,3 +39,14 @@ def test_sweep_cells_and_subset():
     s = workloads.subset(w, [0, 3])
     assert s["B"] == 2 and np.array_equal(s["dyn"]["params"][1], w["dyn"]["params"][3])
     assert s["dyn"]["mass_mge"].shape[0] == 2
+
+
+def test_pixsrc_inputs():
+    w = workloads.make_workload("C2", B=5)
+    a, b = workloads.pixsrc_inputs(w, 32, 24), workloads.pixsrc_inputs(w, 32, 24)
+    assert a["src_grids"].shape == (5, 3) and a["src_grids"].dtype == np.float32 and a["lam"].shape == (5,)
+    assert np.array_equal(a["src_grids"], b["src_grids"]) and np.array_equal(a["lam"], b["lam"])
+    assert (a["lam"] > 0).all() and (a["src_grids"][:, 2] > 0).all()
+    # the grid is centred on the vector's source position
+    cx = a["src_grids"][:, 0] + 15.5 * a["src_grids"][:, 2]
+    assert np.allclose(cx, w["lens"]["params"][:, 9], atol=1e-5)
