@@ -204,6 +204,42 @@ def run_sweep(args):
         g.close()
 
 
+def run_pixsrc_sweep(args):
+    """--pixsrc-sweep: glad_pixsrc_evidence_batch over source-grid resolutions (the axis of the paper's Fig. 1: "various
+    source resolutions commonly adopted in practice") on the C2 image data, one JSON line per resolution.  Context, not the
+    bench line."""
+    import torch
+    import workloads
+    from paper_2504_01302_b200 import Glad
+    B = 296
+    wl = workloads.make_workload("C2", gpu_data_model(0), B=B)
+    L = wl["lens"]
+    g = Glad(0)
+    g.set_image_data(L["grid"], L["psf"], L["data"], L["ivar"])
+    npx = L["grid"]["nx"] * L["grid"]["ny"]
+    for n_s in (16, 24, 32, 40, 48, 64):
+        pin = workloads.pixsrc_inputs(wl, n_s, n_s)
+        a = (torch.from_numpy(L["params"]).cuda(), torch.from_numpy(pin["src_grids"]).cuda(), torch.from_numpy(pin["lam"]).cuda(), n_s, n_s)
+        out = g.pixsrc_evidence_batch(*a, want_source=False, want_model=False)
+        torch.cuda.synchronize()
+        g.profile_enable(True)
+        g.profile_read()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n = 2
+        e0.record()
+        for _ in range(n):
+            out = g.pixsrc_evidence_batch(*a, want_source=False, want_model=False)
+        e1.record()
+        torch.cuda.synchronize()
+        prof = g.profile_read()
+        ms = e0.elapsed_time(e1) / n
+        print(json.dumps({"workload": "C2 image data", "N_d": npx, "N_s": n_s * n_s, "batch": B, "ms_per_call": ms,
+                          "evidences_per_s": B / (ms * 1e-3), "ms_per_evidence": ms / B,
+                          "finite": int(torch.isfinite(out["logev"]).sum().item()),
+                          "kernel_ms": {k[7:]: round(v[0] / n, 3) for k, v in prof.items() if v[1] and k.startswith("pixsrc_")}}), flush=True)
+    g.close()
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import workloads
@@ -490,6 +526,7 @@ def main():
     ap.add_argument("--batch", type=int, default=None, help="override the per-GPU batch (default: the config's)")
     ap.add_argument("--ref-sample", type=int, default=16, help="vectors per oracle pass (cpu_baseline / reference)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--pixsrc-sweep", action="store_true", help="pixelated-source evidence over source-grid resolutions (context)")
     ap.add_argument("--sweep", action="store_true", help="per-kernel times of every BASELINE.json config (context, not the bench line)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -497,6 +534,9 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.pixsrc_sweep:
+        run_pixsrc_sweep(args)
         return
     if args.sweep:
         run_sweep(args)

@@ -87,6 +87,18 @@ def test_c2_parity_paper_sizes(glad_mod, oracle):
     assert np.allclose(one["logev"].cpu().numpy(), ev[sel], rtol=2e-6)
 
 
+def test_c1_parity_maximum_source_grid(glad_mod, oracle):
+    """N_s = 64 x 64 = 4096, the largest source grid the entry accepts (more source pixels than the 1600 image pixels: most of them
+    are held by the regulariser alone), two vectors."""
+    from oracle import pixsrc
+    wl, L, g = _setup(glad_mod, oracle, "C1", 2)
+    pin = workloads.pixsrc_inputs(wl, 64, 64)
+    out = g.pixsrc_evidence_batch(L["params"], pin["src_grids"], pin["lam"], 64, 64)
+    ref = pixsrc.pixsrc_batch(L["params"], L["grid"], L["psf"], L["data"], L["ivar"], pin["src_grids"], pin["lam"], 64, 64)
+    assert np.all(ref["flag"] == 0)
+    _compare(out, ref)
+
+
 def test_mass_sheet_degeneracy_of_the_evidence(glad_mod, oracle):
     """Eq. 5-9: with a (numerically flat) internal sheet, lambda_int x EPL and the source plane scaled by lambda_int, L is unchanged,
     so the evidence is too - the property holds at any size and needs no oracle."""
