@@ -52,3 +52,15 @@ def test_product_does_not_import_oracle_or_work_dir():
                 src = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in src.lower() or f == "__init__.py" and False, f"{f} mentions the oracle"
                 assert "_work" not in src
+
+
+def test_binding_constants_match_header():
+    """The binding sizes its profile arrays from its own KERNELS tuple and mirrors the flag / size constants: they must equal glad.h's."""
+    import paper_2504_01302_b200 as m
+    from paper_2504_01302_b200.binding import Glad
+    txt = open(os.path.join(ROOT, "include", "glad.h")).read()
+    dv = {k: int(v) for k, v in re.findall(r"#define\s+(GLAD_[A-Z0-9_]+)\s+(-?\d+)\b", txt)}
+    assert dv["GLAD_NKERNELS"] == len(Glad.KERNELS)
+    assert dv["GLAD_NLENS"] == m.NLENS and dv["GLAD_NDYN"] == m.NDYN
+    assert (dv["GLAD_FLAG_LENS_INVALID"], dv["GLAD_FLAG_DYN_INVALID"], dv["GLAD_FLAG_BIN_INVALID"], dv["GLAD_FLAG_PIXSRC_NOT_PD"]) == \
+        (m.FLAG_LENS_INVALID, m.FLAG_DYN_INVALID, m.FLAG_BIN_INVALID, m.FLAG_PIXSRC_NOT_PD)
