@@ -8,8 +8,12 @@
  *     allocates or frees caller-visible memory; a context keeps grow-only device scratch.
  *     Static-data pointers passed to glad_set_* are BORROWED: keep them alive and unchanged
  *     until they are replaced or the context is destroyed.
- *   - Batch calls only ENQUEUE work on the context's stream and return; no host sync, no
- *     implicit D2H copy.  glad_set_kin_data is the one exception (documented there).
+ *   - Batch calls only ENQUEUE work on the context's stream and return; no implicit D2H copy and
+ *     no host sync, except that a call which needs MORE context scratch than any call before it
+ *     (the first call, or a larger batch) synchronises the context's streams once while the
+ *     scratch is re-allocated.  glad_set_kin_data is synchronous (documented there).
+ *   - Every call makes the context's device current for its own duration and restores the
+ *     caller's current device before returning.  The library reads no environment variable.
  *   - Errors detectable on the host return a negative glad_status at once; a CUDA
  *     launch/runtime error returns GLAD_ECUDA with the CUDA text in glad_last_error().
  *     No exceptions, no exit(), no printing.  There is no CPU fallback.
@@ -62,7 +66,9 @@ typedef enum {
 #define GLAD_MGE_ROW 3
 
 /* limits of the kernels (GLAD_ESHAPE beyond them) */
-#define GLAD_MAX_IMAGE_PIXELS 40000 /* nx*ny of the lens image (staged whole in shared memory) */
+#define GLAD_MAX_IMAGE_PIXELS 40000 /* nx*ny of the lens image (staged whole in shared memory): the exact condition, checked by
+                                       glad_set_image_data, is 4 (80 + kpsf ceil8(kpsf) + (ny + 1) pitch) <= 232448 bytes with
+                                       pitch = (nx + 2 (kpsf/2) + 23) | 1 floats per padded row */
 #define GLAD_MAX_PSF 31             /* kpsf and kk */
 #define GLAD_MAX_GAUSS 64           /* n_lum, n_mass (+1 for the BH) */
 #define GLAD_MAX_SKY 256            /* nx, ny of the kinematic grid */
@@ -110,7 +116,9 @@ typedef struct {
  * SYNCHRONOUS (setup call): copies xs, ys and bin_id to the host once to detect a grid that is mirror-
  * symmetric about x' = 0 and/or y' = 0 (then only one half per axis is integrated -- the integrand is even),
  * validates the bin ids, and precomputes the static bin x kernel weights on the device.  The folded grid may
- * have at most 512 tiles of 8x8 pixels (GLAD_ESHAPE otherwise). */
+ * have at most 512 tiles of 8x8 pixels, and 4 (2 nxf nyf + n_lum (nxf + nyf)) bytes -- both folded maps plus the luminous
+ * Gaussians' separable factors, staged in shared memory by the binning kernel -- must fit 232448 bytes: checked here for
+ * n_lum = 1 and in the batch call for its n_lum (GLAD_ESHAPE otherwise). */
 glad_status glad_set_kin_data(glad_ctx* ctx, const glad_sky_grid* grid, const int32_t* d_bin_id,
                               int nbins, const float* d_kernel, int kk, const float* d_vrms_obs,
                               const float* d_vrms_ivar, const float* d_u_nodes,
@@ -241,6 +249,19 @@ glad_status glad_profile_read(glad_ctx* ctx, double* ms_out /*[GLAD_NKERNELS]*/,
 glad_status glad_set_light_profiles(glad_ctx* ctx, int source_kind, int lens1_kind, int lens2_kind);
 
 /*
+ * Options of the quadrature (row a6), fixed for the context until changed; 0 selects the default of each.
+ *   path         GLAD_JAM_AUTO: tcgen05 tensor-core contraction where the folded grid fits (<= 128 rows, terms * columns <= 256),
+ *                the FP32 SIMT kernel otherwise; GLAD_JAM_SIMT: always the FP32 SIMT kernel.
+ *   bf16_terms   operand values are split into 2 (default: 16 mantissa bits) or 3 (24 bits) bf16 terms on the tcgen05 path.
+ *   flush_chunks operand chunks per TMEM accumulator group before the group is added into fp32 registers (default: 512 rows).
+ *   k_slices     CTAs per parameter vector along the contraction (default: enough for 4 CTAs per SM on small batches).
+ * The arithmetic of a context therefore never depends on the caller's environment.  GLAD_EINVAL on a bad value.
+ */
+#define GLAD_JAM_AUTO 0
+#define GLAD_JAM_SIMT 1
+glad_status glad_set_jam_options(glad_ctx* ctx, int path, int bf16_terms, int flush_chunks, int k_slices);
+
+/*
  * glad_joint_loglike_batch (and the entries built on it) run the lens half on a context-owned side stream beside the
  * dynamics half, joined by events before the joint kernel; the caller's stream still sees plain stream order.
  * glad_set_overlap(ctx, 0) keeps every kernel on the caller's stream (bench.py uses it for per-kernel timing, where
@@ -329,7 +350,8 @@ glad_status glad_set_mass_sheet(glad_ctx* ctx, const float* d_lambda, int n_lamb
  * d_flags [B].  An invalid mass model (GLAD_FLAG_LENS_INVALID conditions on lens[2..4], lens[8]), lambda <= 0 or a pixel size
  * <= 0 gives logev = -INFINITY, chi2 = +INFINITY, NaN elsewhere and GLAD_FLAG_LENS_INVALID; a matrix that is not positive
  * definite gives the same outputs with GLAD_FLAG_PIXSRC_NOT_PD.  The batch is processed in chunks that fit scratch_mib_max
- * MiB of context-owned device scratch (<= 0: 16384); one vector needs about 4 N_pix N_s + 8 N_s^2 bytes.
+ * MiB of context-owned device scratch (<= 0: 16384; the block is allocated at exactly the chunk's size, never above the limit);
+ * one vector needs about 4 N_pix N_s + 8 N_s^2 bytes.
  * GLAD_ESTATE without image data; GLAD_ESHAPE if n_sx, n_sy < 2, N_s > 4096 or one vector does not fit the scratch limit.
  */
 glad_status glad_pixsrc_evidence_batch(glad_ctx* ctx, const float* d_lens_params, const float* d_src_grid, const float* d_lambda_reg,

@@ -24,7 +24,7 @@ EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "gl
            "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count", "glad_profile_enable",
            "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch", "glad_set_overlap", "glad_set_light_profiles",
            "glad_set_quasar_data", "glad_quasar_chi2_batch", "glad_joint_loglike_full_batch", "glad_set_mass_sheet",
-           "glad_pixsrc_evidence_batch"]
+           "glad_pixsrc_evidence_batch", "glad_set_jam_options"]
 
 
 class GladError(RuntimeError):
@@ -97,6 +97,8 @@ def load(rebuild: bool = False):
     L.glad_set_mass_sheet.argtypes = [vp, vp, i, C.c_float, C.c_float, i, C.c_float, C.c_float]
     L.glad_pixsrc_evidence_batch.restype = i
     L.glad_pixsrc_evidence_batch.argtypes = [vp, vp, vp, vp, i, i, i, i, vp, vp, vp, vp, vp, vp]
+    L.glad_set_jam_options.restype = i
+    L.glad_set_jam_options.argtypes = [vp, i, i, i, i]
     L.glad_launch_count.restype = l
     L.glad_launch_count.argtypes = [vp]
     _lib = L
@@ -122,6 +124,8 @@ def _p(t):
 class Glad:
     """One libglad context bound to torch's current stream on `device`."""
 
+    DEFAULT_JAM_PATH = "auto"      # tests flip this class attribute to run every case on the FP32 SIMT form of row a6 as well
+
     def __init__(self, device: int | str = 0):
         if not torch.cuda.is_available():
             raise GladError("libglad needs a CUDA device (sm_100); there is no CPU path")
@@ -135,6 +139,8 @@ class Glad:
         if st != 0:
             raise GladError(f"glad_create failed with status {st} (device is not sm_100?)")
         self.ctx = ctx
+        if self.DEFAULT_JAM_PATH != "auto":
+            self.set_jam_options(path=self.DEFAULT_JAM_PATH)
         self.image_shape = None
         self.sky_shape = None
         self.nbins = 0
@@ -164,6 +170,10 @@ class Glad:
     def set_light_profiles(self, source=0, lens1=0, lens2=0):
         """0 = Sersic, 1 = Chameleon (Eq. 47) per light component, for the batch calls that follow."""
         self._check(self.lib.glad_set_light_profiles(self.ctx, int(source), int(lens1), int(lens2)))
+
+    def set_jam_options(self, path: str = "auto", terms: int = 0, flush: int = 0, slices: int = 0):
+        """Row a6 options: path "auto" (tcgen05 where the grid fits) or "simt"; bf16 terms 2/3; 0 = default."""
+        self._check(self.lib.glad_set_jam_options(self.ctx, {"auto": 0, "tc": 0, "simt": 1}[path], int(terms), int(flush), int(slices)))
 
     def set_overlap(self, on: bool):
         self._check(self.lib.glad_set_overlap(self.ctx, 1 if on else 0))

@@ -27,8 +27,10 @@ static glad_status cuda_fail(glad_ctx* c, cudaError_t e, const char* what) {
         if (e__ != cudaSuccess) return cuda_fail(c, e__, what);  \
     } while (0)
 
+// Grow-only scratch.  A growth synchronises both streams (the old block may be in use) -- the one hidden host sync of a batch
+// call, on its first use or when a larger batch arrives.  `exact`: no 25 % headroom (blocks sized against a caller's limit).
 template <typename T>
-static glad_status grow(glad_ctx* c, T** p, size_t* cap, size_t need) {
+static glad_status grow(glad_ctx* c, T** p, size_t* cap, size_t need, bool exact = false) {
     if (need <= *cap) return GLAD_OK;
     // the stream may still be using the old block: free is stream-ordered w.r.t. nothing, so sync first
     cudaStreamSynchronize(c->stream);
@@ -36,7 +38,7 @@ static glad_status grow(glad_ctx* c, T** p, size_t* cap, size_t need) {
     if (*p) cudaFree(*p);
     *p = nullptr;
     *cap = 0;
-    size_t n = need + need / 4;
+    size_t n = exact ? need : need + need / 4;
     if (cudaMalloc((void**)p, n * sizeof(T)) != cudaSuccess) {
         cudaGetLastError();
         return fail(c, GLAD_ENOMEM, "cudaMalloc of %zu bytes failed", n * sizeof(T));
@@ -56,18 +58,18 @@ glad_status glad_create(glad_ctx** out, int device, void* cuda_stream) {
     memset(c, 0, sizeof(*c));
     c->device = device;
     c->stream = (cudaStream_t)cuda_stream;
-    cudaDeviceProp prop;
-    cudaError_t e = cudaSetDevice(device);
-    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
-    if (e != cudaSuccess || prop.major != 10) {
+    int major = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+    if (e != cudaSuccess || major != 10) {
+        cudaGetLastError();
         delete c;
         return GLAD_ECUDA;
     }
-    c->sm_count = prop.multiProcessorCount;
-    const char* jp = getenv("GLAD_JAM_PATH");
-    c->jam_simt = (jp && strcmp(jp, "simt") == 0) ? 1 : 0;
+    DeviceScope ds(c);
+    c->jam_simt = 0; c->jam_terms = 2; c->jam_flush = 0; c->jam_slices = 0;
     c->lens_stream = c->stream;
-    const char* ov = getenv("GLAD_OVERLAP");
     if (cudaStreamCreateWithFlags(&c->side_stream, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
@@ -76,7 +78,7 @@ glad_status glad_create(glad_ctx** out, int device, void* cuda_stream) {
     } else {
         c->side_ok = 1;
     }
-    c->overlap = (c->side_ok && !(ov && atoi(ov) == 0)) ? 1 : 0;
+    c->overlap = c->side_ok;
     *out = c;
     return GLAD_OK;
 }
@@ -95,7 +97,8 @@ static void free_kin(glad_ctx* c) {
 
 void glad_destroy(glad_ctx* c) {
     if (!c) return;
-    cudaSetDevice(c->device);
+    {
+    DeviceScope ds(c);
     cudaStreamSynchronize(c->stream);
     if (c->side_stream) { cudaStreamSynchronize(c->side_stream); cudaStreamDestroy(c->side_stream); }
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
@@ -104,6 +107,7 @@ void glad_destroy(glad_ctx* c) {
     void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage, c->d_model, c->d_qtmp, c->d_pix};
     for (void* p : ps) if (p) cudaFree(p);
     for (cudaEvent_t e : c->prof_ev) if (e) cudaEventDestroy(e);
+    }
     delete c;
 }
 
@@ -115,7 +119,7 @@ glad_status glad_profile_enable(glad_ctx* c, int on) {
 
 glad_status glad_profile_read(glad_ctx* c, double* ms_out, long* count_out) {
     if (!c || !ms_out || !count_out) return GLAD_EINVAL;
-    cudaSetDevice(c->device);
+    DeviceScope ds(c);
     CU(cudaStreamSynchronize(c->stream), "profile sync");
     for (int i = 0; i < c->prof_n; ++i) {
         float ms = 0.f;
@@ -157,6 +161,18 @@ glad_status glad_set_mass_sheet(glad_ctx* c, const float* d_lambda, int n_lambda
     return GLAD_OK;
 }
 
+glad_status glad_set_jam_options(glad_ctx* c, int path, int bf16_terms, int flush_chunks, int k_slices) {
+    if (!c) return GLAD_EINVAL;
+    if (path != GLAD_JAM_AUTO && path != GLAD_JAM_SIMT) return fail(c, GLAD_EINVAL, "glad_set_jam_options: path %d", path);
+    if (bf16_terms != 0 && bf16_terms != 2 && bf16_terms != 3) return fail(c, GLAD_EINVAL, "glad_set_jam_options: %d bf16 terms (2 or 3)", bf16_terms);
+    if (flush_chunks < 0 || k_slices < 0) return fail(c, GLAD_EINVAL, "glad_set_jam_options: negative option");
+    c->jam_simt = path == GLAD_JAM_SIMT;
+    c->jam_terms = bf16_terms ? bf16_terms : 2;
+    c->jam_flush = flush_chunks;
+    c->jam_slices = k_slices;
+    return GLAD_OK;
+}
+
 glad_status glad_set_overlap(glad_ctx* c, int on) {
     if (!c) return GLAD_EINVAL;
     if (on && !c->side_ok) return fail(c, GLAD_ESTATE, "glad_set_overlap: no side stream");
@@ -185,7 +201,13 @@ glad_status glad_set_image_data(glad_ctx* c, const glad_image_grid* g, const flo
     if (kpsf <= 0 || (kpsf % 2) == 0) return fail(c, GLAD_EINVAL, "glad_set_image_data: kpsf must be odd, got %d", kpsf);
     if (kpsf > GLAD_MAX_PSF) return fail(c, GLAD_ESHAPE, "glad_set_image_data: kpsf %d > GLAD_MAX_PSF", kpsf);
     if ((d_data == nullptr) != (d_ivar == nullptr)) return fail(c, GLAD_EINVAL, "glad_set_image_data: data and ivar go together");
-    cudaSetDevice(c->device);
+    {
+        const size_t need = lens_image_smem_bytes(g->nx, g->ny, kpsf);
+        if (need > (size_t)c->smem_optin)
+            return fail(c, GLAD_ESHAPE, "glad_set_image_data: a %d x %d image with a %d x %d PSF needs %zu bytes of shared memory (rows padded by the PSF halo), limit %d",
+                        g->nx, g->ny, kpsf, kpsf, need, c->smem_optin);
+    }
+    DeviceScope ds(c);
     if (!c->d_psf) CU(cudaMalloc((void**)&c->d_psf, sizeof(float) * GLAD_MAX_PSF * GLAD_MAX_PSF), "cudaMalloc psf");
     CU(cudaMemcpyAsync(c->d_psf, d_psf, sizeof(float) * kpsf * kpsf, cudaMemcpyDeviceToDevice, c->stream), "copy psf");
     c->grid = *g;
@@ -242,7 +264,7 @@ glad_status glad_set_kin_data(glad_ctx* c, const glad_sky_grid* g, const int32_t
     if (kk <= 0 || (kk % 2) == 0) return fail(c, GLAD_EINVAL, "glad_set_kin_data: kk must be odd, got %d", kk);
     if (kk > GLAD_MAX_PSF) return fail(c, GLAD_ESHAPE, "glad_set_kin_data: kk %d > GLAD_MAX_PSF", kk);
     if ((d_vobs == nullptr) != (d_vivar == nullptr)) return fail(c, GLAD_EINVAL, "glad_set_kin_data: vrms_obs and vrms_ivar go together");
-    cudaSetDevice(c->device);
+    DeviceScope ds(c);
     CU(cudaStreamSynchronize(c->stream), "sync");
     std::vector<float> xs(g->nx), ys(g->ny);
     std::vector<int32_t> bins((size_t)g->nx * g->ny);
@@ -259,6 +281,14 @@ glad_status glad_set_kin_data(glad_ctx* c, const glad_sky_grid* g, const int32_t
     int nxf = fold_axis(xs, fx, xf, ux), nyf = fold_axis(ys, fy, yf, uy);
     int tiles = ((nxf + JQ_T - 1) / JQ_T) * ((nyf + JQ_T - 1) / JQ_T);
     if (tiles > 512) return fail(c, GLAD_ESHAPE, "glad_set_kin_data: folded grid %dx%d needs %d thread tiles (> 512)", nxf, nyf, tiles);
+    {
+        // jam_post_kernel stages both folded maps plus (nxf + nyf) floats per luminous Gaussian: necessary condition here
+        // (one Gaussian), the exact one in the batch call, which knows n_lum
+        const size_t need = jam_post_smem_bytes(nxf, nyf, 1);
+        if (need > (size_t)c->smem_optin)
+            return fail(c, GLAD_ESHAPE, "glad_set_kin_data: folded grid %dx%d needs %zu bytes of shared memory in the binning kernel, limit %d",
+                        nxf, nyf, need, c->smem_optin);
+    }
     std::vector<float> xf2(nxf), yf2(nyf);
     for (int i = 0; i < nxf; ++i) xf2[i] = xf[i] * xf[i];
     for (int i = 0; i < nyf; ++i) yf2[i] = yf[i] * yf[i];
@@ -321,6 +351,9 @@ static glad_status jam_impl(glad_ctx* c, const float* d_dyn, int B, const float*
     const int nmx = nm + 1;
     int NG;
     if (jam_quad_geometry(c, &NG) < 0) return fail(c, GLAD_ESHAPE, "jam: sky grid too large");
+    if (jam_post_smem_bytes(c->nxf, c->nyf, nl) > (size_t)c->smem_optin)
+        return fail(c, GLAD_ESHAPE, "jam: folded grid %dx%d with %d luminous Gaussians needs %zu bytes of shared memory in the binning kernel, limit %d",
+                    c->nxf, c->nyf, nl, jam_post_smem_bytes(c->nxf, c->nyf, nl), c->smem_optin);
     // K-slices: enough CTAs for >= 4 per SM when the batch is small
     long M = (long)c->nu * nmx * nl;
     int NCH = (int)((M + NG * JQ_MI - 1) / (NG * JQ_MI));
@@ -328,7 +361,7 @@ static glad_status jam_impl(glad_ctx* c, const float* d_dyn, int B, const float*
     if (S > 32) S = 32;
     if (S > NCH) S = NCH;
     if (S < 1) S = 1;
-    if (const char* e = getenv("GLAD_JAM_SLICES")) { int v = atoi(e); if (v >= 1 && v <= NCH) S = v; }
+    if (c->jam_slices >= 1) S = c->jam_slices < NCH ? c->jam_slices : NCH;
     glad_status st = grow(c, &c->d_jam_tab, &c->jam_tab_cap, (size_t)B * jam_table_floats(nl, nmx));
     if (st != GLAD_OK) return st;
     st = grow(c, &c->d_partial, &c->partial_cap, (size_t)B * S * c->nxf * c->nyf);
@@ -346,7 +379,7 @@ glad_status glad_lens_image_batch(glad_ctx* c, const float* d_lens, int B, float
     if (!c) return GLAD_EINVAL;
     if (B < 0 || (B > 0 && !d_lens)) return fail(c, GLAD_EINVAL, "glad_lens_image_batch: B=%d / null params", B);
     if (B == 0) return GLAD_OK;
-    cudaSetDevice(c->device);
+    DeviceScope ds(c);
     return lens_impl(c, d_lens, B, d_images, d_chi2, d_flags);
 }
 
@@ -356,7 +389,7 @@ glad_status glad_jam_vrms_batch(glad_ctx* c, const float* d_dyn, int B, const fl
     if (!c) return GLAD_EINVAL;
     if (B < 0 || (B > 0 && !d_dyn)) return fail(c, GLAD_EINVAL, "glad_jam_vrms_batch: B=%d / null params", B);
     if (B == 0) return GLAD_OK;
-    cudaSetDevice(c->device);
+    DeviceScope ds(c);
     return jam_impl(c, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian, d_vrms, d_chi2,
                     d_v2map, d_flags);
 }
@@ -416,7 +449,7 @@ glad_status glad_joint_loglike_batch(glad_ctx* c, const float* d_lens, const flo
     if (!c) return GLAD_EINVAL;
     if (B < 0 || (B > 0 && (!d_lens || !d_dyn || !d_loglike))) return fail(c, GLAD_EINVAL, "glad_joint_loglike_batch: B=%d / null pointer", B);
     if (B == 0) return GLAD_OK;
-    cudaSetDevice(c->device);
+    DeviceScope ds(c);
     return joint_impl(c, d_lens, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian, d_loglike,
                       d_chi2_lens, d_chi2_dyn, d_flags, nullptr, nullptr, nullptr);
 }
@@ -455,7 +488,7 @@ glad_status glad_quasar_chi2_batch(glad_ctx* c, const float* d_lens, const float
     if (!c->have_qso) return fail(c, GLAD_ESTATE, "glad_quasar_chi2_batch: glad_set_quasar_data not called");
     if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "glad_quasar_chi2_batch: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
     if (B == 0) return GLAD_OK;
-    cudaSetDevice(c->device);
+    DeviceScope ds(c);
     CU(launch_quasar(c, c->stream, d_lens, d_ddt, B, d_chi2_img, d_chi2_tmd, d_theta_pre, d_dt_pre, d_beta), "quasar_kernel");
     return GLAD_OK;
 }
@@ -469,7 +502,7 @@ glad_status glad_pixsrc_evidence_batch(glad_ctx* c, const float* d_lens, const f
     if (nsx < 2 || nsy < 2 || (long)nsx * nsy > 4096) return fail(c, GLAD_ESHAPE, "glad_pixsrc_evidence_batch: source grid %d x %d (need >= 2 x 2, N_s <= 4096)", nsx, nsy);
     if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "glad_pixsrc_evidence_batch: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
     if (B == 0) return GLAD_OK;
-    cudaSetDevice(c->device);
+    DeviceScope ds(c);
     const int npix = c->grid.nx * c->grid.ny, ns = nsx * nsy;
     const size_t cap = (size_t)(scratch_mib_max > 0 ? scratch_mib_max : 16384) << 20;
     const size_t one = pixsrc_scratch_bytes(npix, ns, 1);
@@ -478,7 +511,7 @@ glad_status glad_pixsrc_evidence_batch(glad_ctx* c, const float* d_lens, const f
     if (Bc > B) Bc = B;
     if (Bc > 2 * c->sm_count) Bc = 2 * c->sm_count;
     while (Bc > 1 && pixsrc_scratch_bytes(npix, ns, Bc) > cap) --Bc;
-    glad_status st = grow(c, &c->d_pix, &c->pix_cap, pixsrc_scratch_bytes(npix, ns, Bc));
+    glad_status st = grow(c, &c->d_pix, &c->pix_cap, pixsrc_scratch_bytes(npix, ns, Bc), true);
     if (st != GLAD_OK) return st;
     // ln det g in closed form: g = kron(I, T^2) + kron(T^2, I), T the (1,-2,1) matrix with eigenvalues -2 + 2 cos(k pi/(n+1))
     double logdet_g = 0.0;
@@ -508,7 +541,7 @@ glad_status glad_joint_loglike_host(glad_ctx* c, const float* h_lens, const floa
         return fail(c, GLAD_EINVAL, "glad_joint_loglike_host: B=%d / null pointer", B);
     if (nl <= 0 || nm < 0 || lum_stride < 0 || mass_stride < 0) return fail(c, GLAD_EINVAL, "glad_joint_loglike_host: bad table sizes");
     if (B == 0) return GLAD_OK;
-    cudaSetDevice(c->device);
+    DeviceScope ds(c);
     auto r4 = [](size_t n) { return (n + 3) & ~(size_t)3; };
     size_t n_lens = r4((size_t)B * GLAD_NLENS), n_dyn = r4((size_t)B * GLAD_NDYN);
     size_t n_lum = r4(lum_stride ? (size_t)B * lum_stride : (size_t)nl * 3);
@@ -560,7 +593,7 @@ glad_status glad_mge1d_batch(glad_ctx* c, int kind, const float* d_prof, int B, 
     glad_status st = mge_check(c, "glad_mge1d_batch", n_gauss, sigma_lo, sigma_hi);
     if (st != GLAD_OK) return st;
     if (B == 0) return GLAD_OK;
-    cudaSetDevice(c->device);
+    DeviceScope ds(c);
     CU(launch_mge1d(c, kind, d_prof, B, n_gauss, sigma_lo, sigma_hi, P, d_mge), "mge1d_kernel");
     return GLAD_OK;
 }
@@ -582,7 +615,7 @@ static glad_status model_impl(glad_ctx* c, const float* d_lens, const float* d_d
     st = mge_check(c, "glad_joint_loglike_model_batch (mass)", nm, mass_lo, mass_hi);
     if (st != GLAD_OK) return st;
     if (B == 0) return GLAD_OK;
-    cudaSetDevice(c->device);
+    DeviceScope ds(c);
     if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "joint model: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
     const int nmt = nm + (c->d_lambda ? c->ms_n : 0);      // the mass sheet adds rows of its own
     if (nmt > GLAD_MAX_GAUSS) return fail(c, GLAD_ESHAPE, "joint model: n_mass %d + %d sheet Gaussians exceed GLAD_MAX_GAUSS", nm, nmt - nm);

@@ -9,7 +9,8 @@
 // Lens half: per-vector constants prepared in fp64 by lens_prep_kernel (row a0), read by
 // lens_image_kernel.  Indices into a float[LC_SIZE] block.
 // ---------------------------------------------------------------------------------------------
-#define GLAD_EPL_MAX_TERMS 40
+#define GLAD_EPL_MAX_TERMS 40     // series coefficients stored per vector (enough for q >= 0.2 at 2e-8)
+#define GLAD_EPL_TERMS_CAP 500    // terms summed at most (DESIGN.md R-L3): coefficients past the table are formed on the fly
 enum LensConstIdx {
     LC_XL = 0, LC_YL, LC_COSPA, LC_SINPA, LC_Q, LC_NEGF,  // -f = -(1-q)/(1+q)
     LC_PREF,      // 2 b_TM^t / (1+q)   (0 if theta_E = 0)
@@ -65,10 +66,15 @@ struct glad_ctx {
     int sm_count;
     char err[512];
     long launches;
-    int jam_simt;   // 1 = force the FP32 SIMT quadrature kernel (env GLAD_JAM_PATH=simt); default tcgen05
+    int smem_optin; // cudaDevAttrMaxSharedMemoryPerBlockOptin of `device`
+    // row a6 options (glad_set_jam_options): nothing in the library reads the environment
+    int jam_simt;   // 1 = force the FP32 SIMT quadrature kernel; default tcgen05 where the grid fits
+    int jam_terms;  // bf16 terms per operand value on the tcgen05 path: 2 (default) or 3
+    int jam_flush;  // chunks per TMEM accumulator group, 0 = default (512 contraction rows)
+    int jam_slices; // K-slices per vector, 0 = automatic
     // The two halves are independent until joint_kernel: glad_joint_loglike_batch forks the lens half onto a context-owned
     // side stream (event fork/join on the caller's stream, so the caller still sees plain stream order).  lens_stream is
-    // the stream the lens launchers use: == stream except inside that fork.  GLAD_OVERLAP=0 keeps everything on `stream`.
+    // the stream the lens launchers use: == stream except inside that fork.  glad_set_overlap(ctx, 0) keeps everything on `stream`.
     cudaStream_t lens_stream, side_stream;
     cudaEvent_t ev_fork, ev_join;
     int overlap, side_ok;
@@ -142,6 +148,20 @@ struct ProfScope {
     ~ProfScope() { if (slot >= 0) cudaEventRecord(c->prof_ev[2 * slot + 1], st); }
 };
 
+// Opt a kernel in to the device's maximum dynamic shared memory.  The attribute is per function AND per device, so it is set
+// (to the same value every time) before each launch instead of being cached in a process-wide static: a second context on
+// another GPU, or another host thread, sees the same state.  Cost: a few microseconds of host time per launch.
+template <typename K>
+static inline cudaError_t smem_optin(const glad_ctx* c, K kernel) {
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
+}
+// Every entry point makes the context's device current and restores the caller's on return.
+struct DeviceScope {
+    int prev;
+    explicit DeviceScope(const glad_ctx* c) : prev(-1) { if (cudaGetDevice(&prev) != cudaSuccess) prev = -1; if (prev != c->device) cudaSetDevice(c->device); else prev = -1; }
+    ~DeviceScope() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 // kernel launchers (return cudaGetLastError())
 cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B);
 cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2, int32_t* d_flags);
@@ -170,5 +190,8 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
 // and two operand stages fit in shared memory
 bool jam_quad_tc_supported(const glad_ctx* c, int nl, int nmx);
 cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S);
+// dynamic shared memory of lens_image_kernel / jam_post_kernel for given sizes (checked when the static data is set)
+size_t lens_image_smem_bytes(int nx, int ny, int kpsf);
+size_t jam_post_smem_bytes(int nxf, int nyf, int nl);
 // launch geometry of the quadrature kernel for the current sky grid: threads per CTA, thread groups
 int jam_quad_geometry(const glad_ctx* c, int* groups);

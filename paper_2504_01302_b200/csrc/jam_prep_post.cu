@@ -247,16 +247,16 @@ __global__ void __launch_bounds__(256) jam_post_kernel(const float* __restrict__
     }
 }
 
+size_t jam_post_smem_bytes(int nxf, int nyf, int nl) {
+    return sizeof(float) * (2 * (size_t)nxf * nyf + (size_t)nl * (nxf + nyf));
+}
+
 cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d_vrms, float* d_chi2,
                             float* d_v2map, int32_t* d_flags) {
-    int npf = c->nxf * c->nyf;
-    size_t smem = sizeof(float) * (2 * (size_t)npf + (size_t)nl * (c->nxf + c->nyf));
-    static size_t configured = 0;
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(jam_post_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
+    const size_t smem = jam_post_smem_bytes(c->nxf, c->nyf, nl);
+    if (smem > (size_t)c->smem_optin) return cudaErrorInvalidConfiguration;   // glad_set_kin_data checks this up front
+    cudaError_t e = smem_optin(c, jam_post_kernel);
+    if (e != cudaSuccess) return e;
     ProfScope ps(c, GK_JAM_POST);
     jam_post_kernel<<<B, 256, smem, c->stream>>>(c->d_jam_tab, jam_table_floats(nl, nmx), nl, nmx, c->d_partial, S, c->nx,
                                                 c->ny, c->nxf, c->nyf, c->d_xf2, c->d_yf2, c->d_foldx, c->d_foldy,

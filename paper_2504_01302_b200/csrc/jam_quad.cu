@@ -213,12 +213,8 @@ cudaError_t launch_jam_quad(glad_ctx* c, int B, int nl, int nmx, int S) {
     if ((size_t)nxp * nyp > ops) ops = (size_t)nxp * nyp;
     size_t smem = sizeof(float) * ((size_t)a.tabsz + 2 * (size_t)((c->nu + 1) & ~1) + RS + 2 * (size_t)MC * 4 + ops);
     if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
-    static size_t configured = 0;
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(jam_quad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
+    cudaError_t e = smem_optin(c, jam_quad_kernel);
+    if (e != cudaSuccess) return e;
     ProfScope ps(c, GK_JAM_QUAD);
     jam_quad_kernel<<<B * S, NT, smem, c->stream>>>(a);
     return cudaGetLastError();

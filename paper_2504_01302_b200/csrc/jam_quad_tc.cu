@@ -32,8 +32,6 @@
 //   the stage's "full" named barrier (does not block).
 //   MMA warp, chunk c:  bar.sync on "full" -> one lane issues the MMAs of the chunk and commits to "empty".
 //   The tensor core works on chunk c while the CUDA cores produce chunk c+1.
-#include <stdlib.h>
-
 #include "glad_internal.h"
 
 #define LOG2E_F 1.4426950408889634f
@@ -53,11 +51,7 @@ struct JTArgs {
     float* partial;
 };
 
-#ifdef ABL_MUFU
-__device__ __forceinline__ float ex2_tc(float x) { return x * 1.0001f; }
-#else
 __device__ __forceinline__ float ex2_tc(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-#endif
 __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -83,9 +77,6 @@ __device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint6
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
-#ifdef ABL_MMA       // timing experiments only (never defined in the product build): producers without tensor work
-#define umma_bf16(...) ((void)0)
-#endif
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
@@ -121,9 +112,6 @@ __device__ __forceinline__ void split_store(f32x2 (&v)[4], uint4* dst, int term_
             w[j] = pack_bf16(lo[j], hi[j]);
             if (t + 1 < NT) bf16_residual(w[j], lo[j], hi[j]);
         }
-#ifdef ABL_STS       // timing experiments only: keep the values alive without the shared-memory store
-        if (w[0] == 0x12345678u && w[3] == 0x9abcdef0u)
-#endif
         dst[t * term_stride16] = make_uint4(w[0], w[1], w[2], w[3]);
     }
 }
@@ -271,11 +259,7 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
         // one row from its (iu, j, k): 3 MUFU.RCP + 1 MUFU.RSQ (approx, <= 2 ulp: the operands carry 16 bits)
         auto coef_store = [&](int rc, int r, int iu, int j, int k) {
             float cq = 0.f, cp = 0.f, f0 = 0.f, f1 = 0.f;
-#ifdef ABL_COEF      // timing experiments only
-            if (iu < 0) {
-#else
             if (iu < nu) {
-#endif
                 const float2 uw = s_uw[iu];
                 const float4 mj = s_mj[j];
                 const float4 lk = s_lk[k];
@@ -408,9 +392,6 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
         for (int i = 0; i < NACC; ++i) acc[i] = 0.f;
         const int lq = warp & 3, cg = warp >> 2;
         auto flush = [&](int g) {
-#ifdef ABL_FLUSH     // timing experiments only
-            if (g >= 0) return;
-#endif
             const uint32_t taddr = tmem + ((uint32_t)(32 * lq) << 16) + (uint32_t)(g & 1) * dstride + (uint32_t)(cg * NACC);
 #pragma unroll
             for (int tc = 0; tc < NT; ++tc) {
@@ -499,16 +480,13 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(a.tmem_cols) : "memory");
 }
 
-// bf16 terms per operand: 2 by default (16 mantissa bits, per-term error <= 2^-16), 3 with GLAD_JAM_TERMS=3
-static int tc_terms() {
-    const char* e = getenv("GLAD_JAM_TERMS");
-    return (e && atoi(e) == 3) ? 3 : 2;
-}
+// bf16 terms per operand: 2 by default (16 mantissa bits, per-term error <= 2^-16), 3 after glad_set_jam_options(.., 3, ..)
+static int tc_terms(const glad_ctx* c) { return c->jam_terms == 3 ? 3 : 2; }
 #define TC_PW 16    // producer warps per CTA (24 was tried: 72 registers per thread spill, slower)
 
 // launch plan for the current sky grid and table sizes; false = not supported (the FP32 kernel takes over)
 static bool tc_plan(const glad_ctx* c, int nl, int nmx, JTArgs* a, int* nacc, size_t* smem) {
-    const int NT = tc_terms(), PW = TC_PW;
+    const int NT = tc_terms(c), PW = TC_PW;
     a->ny8 = (c->nyf + 7) & ~7;
     if (a->ny8 > 128) return false;
     a->multi = NT * a->ny8 > 128 ? 1 : 0;
@@ -534,21 +512,17 @@ static bool tc_plan(const glad_ctx* c, int nl, int nmx, JTArgs* a, int* nacc, si
 bool jam_quad_tc_supported(const glad_ctx* c, int nl, int nmx) { JTArgs a; int nacc; size_t smem; return tc_plan(c, nl, nmx, &a, &nacc, &smem); }
 
 template <int NT, int NACC, int PW>
-static cudaError_t tc_launch(const JTArgs& a, int grid, size_t smem, cudaStream_t st) {
-    static size_t configured = 0;
-    if (smem > configured) {
-        cudaError_t e = cudaFuncSetAttribute(jam_quad_tc_kernel<NT, NACC, PW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = smem;
-    }
+static cudaError_t tc_launch(const glad_ctx* c, const JTArgs& a, int grid, size_t smem, cudaStream_t st) {
+    cudaError_t e = smem_optin(c, jam_quad_tc_kernel<NT, NACC, PW>);
+    if (e != cudaSuccess) return e;
     jam_quad_tc_kernel<NT, NACC, PW><<<grid, PW * 32 + 32, smem, st>>>(a);
     return cudaGetLastError();
 }
 template <int NT>
-static cudaError_t tc_dispatch(const JTArgs& a, int nacc, int grid, size_t smem, cudaStream_t st) {
-    if (nacc == 16) return tc_launch<NT, 16, 16>(a, grid, smem, st);
-    if (nacc == 24) return tc_launch<NT, 24, 16>(a, grid, smem, st);
-    return tc_launch<NT, 32, 16>(a, grid, smem, st);
+static cudaError_t tc_dispatch(const glad_ctx* c, const JTArgs& a, int nacc, int grid, size_t smem, cudaStream_t st) {
+    if (nacc == 16) return tc_launch<NT, 16, 16>(c, a, grid, smem, st);
+    if (nacc == 24) return tc_launch<NT, 24, 16>(c, a, grid, smem, st);
+    return tc_launch<NT, 32, 16>(c, a, grid, smem, st);
 }
 
 cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S) {
@@ -561,7 +535,7 @@ cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S) {
     a.xf2 = c->d_xf2; a.yf2 = c->d_yf2; a.nxf = c->nxf; a.nyf = c->nyf;
     a.S = S; a.partial = c->d_partial;
     a.FL = 512 / a.MC;
-    if (const char* e = getenv("GLAD_JAM_FLUSH")) { int v = atoi(e); if (v >= 1) a.FL = v; }
+    if (c->jam_flush >= 1) a.FL = c->jam_flush;
     ProfScope ps(c, GK_JAM_QUAD);
-    return tc_terms() == 3 ? tc_dispatch<3>(a, nacc, B * S, smem, c->stream) : tc_dispatch<2>(a, nacc, B * S, smem, c->stream);
+    return tc_terms(c) == 3 ? tc_dispatch<3>(c, a, nacc, B * S, smem, c->stream) : tc_dispatch<2>(c, a, nacc, B * S, smem, c->stream);
 }

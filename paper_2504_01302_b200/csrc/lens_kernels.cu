@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(32 * LENS_PREP_ROLES) lens_prep_kernel(const f
     if (f > 1e-12) {
         nt = (int)ceil(log(2e-8) / log(f)) + 1;
         if (nt < 1) nt = 1;
-        if (nt > GLAD_EPL_MAX_TERMS) nt = GLAD_EPL_MAX_TERMS;
+        if (nt > GLAD_EPL_TERMS_CAP) nt = GLAD_EPL_TERMS_CAP;
     }
     c[LC_NTERMS] = (float)nt;
     for (int n = 1; n <= GLAD_EPL_MAX_TERMS; ++n)
@@ -137,6 +137,18 @@ __device__ __forceinline__ float shoot(const float* __restrict__ c, float thx, f
     float zr = negf * (wr * wr - wi * wi), zi = negf * (2.f * wr * wi);
     // Horner: h_n = 1 + c_n z h_{n+1}, sum = h_1
     float hr = 1.f, hi = 0.f;
+    if (nterms > GLAD_EPL_MAX_TERMS) {
+        // very flat mass (q < 0.2): the terms past the stored table take c_n = (2n - a)/(2n + a), a = 2 - t = 1 + 2 HEXP, on the fly
+        const float a2t = fmaf(2.f, c[LC_HEXP], 1.f);
+        for (int n = nterms; n > GLAD_EPL_MAX_TERMS; --n) {
+            const float tn = 2.f * (float)n;
+            const float cn = __fdividef(tn - a2t, tn + a2t);
+            float tr = fmaf(zr, hr, -zi * hi), ti = fmaf(zr, hi, zi * hr);
+            hr = fmaf(cn, tr, 1.f);
+            hi = cn * ti;
+        }
+        nterms = GLAD_EPL_MAX_TERMS;
+    }
     for (int n = nterms; n >= 1; --n) {
         float cn = c[LC_SERIES + n - 1];
         float tr = fmaf(zr, hr, -zi * hi), ti = fmaf(zr, hi, zi * hr);
@@ -298,18 +310,16 @@ cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B) {
     return cudaGetLastError();
 }
 
+size_t lens_image_smem_bytes(int nx, int ny, int kpsf) {
+    return sizeof(float) * (LC_SIZE + (size_t)kpsf * lens_tap_pitch(kpsf) + (size_t)(ny + 1) * lens_img_pitch(nx, kpsf));
+}
+
 cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2, int32_t* d_flags) {
-    size_t smem = sizeof(float) * (LC_SIZE + (size_t)c->kpsf * lens_tap_pitch(c->kpsf) +
-                                   (size_t)(c->grid.ny + 1) * lens_img_pitch(c->grid.nx, c->kpsf));
-    if (smem > 227 * 1024) return cudaErrorInvalidConfiguration;
-    static size_t configured[2] = {0, 0};
+    const size_t smem = lens_image_smem_bytes(c->grid.nx, c->grid.ny, c->kpsf);
+    if (smem > (size_t)c->smem_optin) return cudaErrorInvalidConfiguration;   // glad_set_image_data checks this up front
     const int ch = c->light_kinds != 0 || c->d_lambda != nullptr;
-    if (smem > configured[ch]) {
-        cudaError_t e = ch ? cudaFuncSetAttribute(lens_image_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
-                           : cudaFuncSetAttribute(lens_image_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured[ch] = smem;
-    }
+    cudaError_t e = ch ? smem_optin(c, lens_image_kernel<true>) : smem_optin(c, lens_image_kernel<false>);
+    if (e != cudaSuccess) return e;
     ProfScope ps(c, GK_LENS_IMAGE, c->lens_stream);
     if (ch)
         lens_image_kernel<true><<<B, 512, smem, c->lens_stream>>>(c->d_lens_const, c->light_kinds, c->grid, c->d_psf, c->kpsf,

@@ -561,16 +561,9 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
     const int rows_per_cta = 64;
     const size_t sm_blur = sizeof(float) * (size_t)PX_BLUR_WARPS * ns;
     const size_t sm_chol = sizeof(double) * ((size_t)PX_NB * (PX_NB + 1) + 2 * PX_NB * PX_PP + ns + 8 * 32);
-    static size_t cfg_blur = 0, cfg_chol = 0;
     if (sm_blur > 227 * 1024 || sm_chol > 227 * 1024) return cudaErrorInvalidConfiguration;
-    if (sm_blur > cfg_blur) {
-        if ((e = cudaFuncSetAttribute(pixsrc_blur_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_blur)) != cudaSuccess) return e;
-        cfg_blur = sm_blur;
-    }
-    if (sm_chol > cfg_chol) {
-        if ((e = cudaFuncSetAttribute(pixsrc_chol_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_chol)) != cudaSuccess) return e;
-        cfg_chol = sm_chol;
-    }
+    if ((e = smem_optin(c, pixsrc_blur_kernel)) != cudaSuccess) return e;
+    if ((e = smem_optin(c, pixsrc_chol_kernel)) != cudaSuccess) return e;
     pixsrc_static_kernel<<<1, 256, 0, st>>>(c->d_ivar, npix, stat);
     c->launches++;
     {
