@@ -67,7 +67,7 @@ typedef enum {
 
 /* limits of the kernels (GLAD_ESHAPE beyond them) */
 #define GLAD_MAX_IMAGE_PIXELS 40000 /* nx*ny of the lens image (staged whole in shared memory): the exact condition, checked by
-                                       glad_set_image_data, is 4 (80 + kpsf ceil8(kpsf) + (ny + 1) pitch) <= 232448 bytes with
+                                       glad_set_image_data, is 4 (80 + kpsf ceil8(kpsf) + (ny + 1) pitch) <= 231424 bytes with
                                        pitch = (nx + 2 (kpsf/2) + 23) | 1 floats per padded row */
 #define GLAD_MAX_PSF 31             /* kpsf and kk */
 #define GLAD_MAX_GAUSS 64           /* n_lum, n_mass (+1 for the BH) */
@@ -117,7 +117,7 @@ typedef struct {
  * symmetric about x' = 0 and/or y' = 0 (then only one half per axis is integrated -- the integrand is even),
  * validates the bin ids, and precomputes the static bin x kernel weights on the device.  The folded grid may
  * have at most 512 tiles of 8x8 pixels, and 4 (2 nxf nyf + n_lum (nxf + nyf)) bytes -- both folded maps plus the luminous
- * Gaussians' separable factors, staged in shared memory by the binning kernel -- must fit 232448 bytes: checked here for
+ * Gaussians' separable factors, staged in shared memory by the binning kernel -- must fit 231424 bytes: checked here for
  * n_lum = 1 and in the batch call for its n_lum (GLAD_ESHAPE otherwise). */
 glad_status glad_set_kin_data(glad_ctx* ctx, const glad_sky_grid* grid, const int32_t* d_bin_id,
                               int nbins, const float* d_kernel, int kk, const float* d_vrms_obs,

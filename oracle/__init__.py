@@ -18,6 +18,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "glad_oracle.c")
+_SRCS = [_SRC, os.path.join(_HERE, "jam_sph_oracle.c")]
 _LIB = os.path.join(_HERE, "libglad_oracle.so")
 _lib = None
 
@@ -27,8 +28,8 @@ FLAG_LENS_INVALID, FLAG_DYN_INVALID, FLAG_BIN_INVALID = 1, 2, 4
 
 
 def build(force: bool = False) -> str:
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"]
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(f) for f in _SRCS):
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, *_SRCS, "-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 
@@ -98,6 +99,13 @@ def lib():
         L.glad_oracle_tdelay_const.restype = d
         L.glad_oracle_quasar_batch.restype = i
         L.glad_oracle_quasar_batch.argtypes = [fp, fp, i, i, dp, dp, i, dp, dp, dp, dp, dp, dp, dp, dp]
+        L.glad_oracle_jam_sph_intrinsic.restype = None
+        L.glad_oracle_jam_sph_intrinsic.argtypes = [d, d, i, dp, dp, dp, dp, i, dp, dp, dp, d, i, dp, dp, i, dp, dp, dp]
+        L.glad_oracle_jam_sph_los.restype = d
+        L.glad_oracle_jam_sph_los.argtypes = [d, d, d, i, dp, dp, dp, i, dp, i, dp, dp, d, i, dp, dp]
+        L.glad_oracle_jam_sph_vrms_batch.restype = i
+        L.glad_oracle_jam_sph_vrms_batch.argtypes = [fp, i, fp, i, C.c_long, fp, i, C.c_long, fp, i, i, i, fp, fp, ip, i, fp, i,
+                                                     fp, fp, i, fp, i, fp, i, fp, fp, i, fp, fp, i, fp, fp, dp, dp, dp, dp, ip]
         _lib = L
     return _lib
 
@@ -363,4 +371,68 @@ def quasar_batch(lens, ddt, qso, lam=None, sheet=None):
                                               P(out["dt_pre"]), P(out["beta"]), P(out["last_step"]))
     if rc != 0:
         raise ValueError("oracle: bad quasar arguments")
+    return out
+
+
+# ------------------------------------------------------------------------------------------------
+# JAM_sph (oracle/jam_sph_oracle.c)
+# ------------------------------------------------------------------------------------------------
+def jam_sph_intrinsic(r, theta, sig_k, q_k, nu0_k, beta_k, sig_j, q_j, mass_j, rcut, tau, wtau, un, uw):
+    """(nu v_r^2, nu v_theta^2, nu v_phi^2, nu) at one point (r [pc], theta), intrinsic tables in pc / Msun."""
+    f = lambda a: np.ascontiguousarray(a, dtype=np.float64)
+    sig_k, q_k, nu0_k, beta_k, sig_j, q_j, mass_j, tau, wtau, un, uw = map(
+        f, (sig_k, q_k, nu0_k, beta_k, sig_j, q_j, mass_j, tau, wtau, un, uw))
+    out = np.zeros(4)
+    P = lambda a: _ptr(a, C.c_double)
+    lib().glad_oracle_jam_sph_intrinsic(float(r), float(theta), sig_k.size, P(sig_k), P(q_k), P(nu0_k), P(beta_k),
+                                        sig_j.size, P(sig_j), P(q_j), P(mass_j), float(rcut), tau.size, P(tau), P(wtau),
+                                        un.size, P(un), P(uw), P(out))
+    return out
+
+
+def jam_sph_los(xp, yp, inc, sig_k, q_k, nu0_k, rgrid, thgrid, ratios, rcut, zeta, wz) -> float:
+    """int nu v_z'^2 dz' at one sky point (pc), ratios [3,nr,nth] on the polar grid (pc, rad)."""
+    f = lambda a: np.ascontiguousarray(a, dtype=np.float64)
+    sig_k, q_k, nu0_k, rgrid, thgrid, ratios, zeta, wz = map(f, (sig_k, q_k, nu0_k, rgrid, thgrid, ratios, zeta, wz))
+    P = lambda a: _ptr(a, C.c_double)
+    return float(lib().glad_oracle_jam_sph_los(float(xp), float(yp), float(inc), sig_k.size, P(sig_k), P(q_k), P(nu0_k),
+                                               rgrid.size, P(rgrid), thgrid.size, P(thgrid), P(ratios), float(rcut),
+                                               zeta.size, P(zeta), P(wz)))
+
+
+def jam_sph_vrms_batch(dyn, lum_mge, mass_mge, beta, kin, sph, want_maps=False):
+    """kin as jam_vrms_batch (u_nodes unused); sph = dict(rgrid, thgrid, tau, wtau, un, uw, zeta, wz); beta = beta_ani.
+    Returns dict(vrms, chi2, flags[, v2map, moments [B,3,nr,nth]])."""
+    dyn = _f32(dyn).reshape(-1, NDYN)
+    B = dyn.shape[0]
+    lum, mass, beta = _f32(lum_mge), _f32(mass_mge), _f32(beta)
+    n_lum, n_mass = lum.shape[-2], mass.shape[-2]
+    lum_stride = 0 if lum.ndim == 2 else n_lum * 3
+    mass_stride = 0 if mass.ndim == 2 else n_mass * 3
+    per_g = 1 if beta.ndim == 2 else 0
+    xs, ys = _f32(kin["xs"]), _f32(kin["ys"])
+    nx, ny = xs.size, ys.size
+    bin_id = np.ascontiguousarray(kin["bin_id"], dtype=np.int32)
+    nbins = int(kin["nbins"])
+    kern = _f32(kin["kernel"])
+    vo, vi = _f32(kin.get("vrms_obs")), _f32(kin.get("vrms_ivar"))
+    a = {k: _f32(sph[k]) for k in ("rgrid", "thgrid", "tau", "wtau", "un", "uw", "zeta", "wz")}
+    nr, nth = a["rgrid"].size, a["thgrid"].size
+    vrms = np.empty((B, nbins), np.float64)
+    chi2 = np.empty(B, np.float64)
+    flags = np.zeros(B, np.int32)
+    v2map = np.empty((B, ny, nx), np.float64) if want_maps else None
+    mom = np.empty((B, 3, nr, nth), np.float64) if want_maps else None
+    F = C.c_float
+    rc = lib().glad_oracle_jam_sph_vrms_batch(
+        _ptr(dyn, F), B, _ptr(lum, F), n_lum, lum_stride, _ptr(mass, F), n_mass, mass_stride, _ptr(beta, F), per_g, nx, ny,
+        _ptr(xs, F), _ptr(ys, F), _ptr(bin_id, C.c_int32), nbins, _ptr(kern, F), kern.shape[0], _ptr(vo, F), _ptr(vi, F),
+        nr, _ptr(a["rgrid"], F), nth, _ptr(a["thgrid"], F), a["tau"].size, _ptr(a["tau"], F), _ptr(a["wtau"], F),
+        a["un"].size, _ptr(a["un"], F), _ptr(a["uw"], F), a["zeta"].size, _ptr(a["zeta"], F), _ptr(a["wz"], F),
+        _ptr(vrms, C.c_double), _ptr(chi2, C.c_double), _ptr(v2map, C.c_double), _ptr(mom, C.c_double), _ptr(flags, C.c_int32))
+    if rc != 0:
+        raise ValueError("oracle: bad jam_sph arguments")
+    out = {"vrms": vrms, "chi2": chi2, "flags": flags}
+    if want_maps:
+        out["v2map"], out["moments"] = v2map, mom
     return out

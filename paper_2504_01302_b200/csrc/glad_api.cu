@@ -203,9 +203,9 @@ glad_status glad_set_image_data(glad_ctx* c, const glad_image_grid* g, const flo
     if ((d_data == nullptr) != (d_ivar == nullptr)) return fail(c, GLAD_EINVAL, "glad_set_image_data: data and ivar go together");
     {
         const size_t need = lens_image_smem_bytes(g->nx, g->ny, kpsf);
-        if (need > (size_t)c->smem_optin)
+        if (need > (size_t)glad_smem_dynamic_max(c))
             return fail(c, GLAD_ESHAPE, "glad_set_image_data: a %d x %d image with a %d x %d PSF needs %zu bytes of shared memory (rows padded by the PSF halo), limit %d",
-                        g->nx, g->ny, kpsf, kpsf, need, c->smem_optin);
+                        g->nx, g->ny, kpsf, kpsf, need, glad_smem_dynamic_max(c));
     }
     DeviceScope ds(c);
     if (!c->d_psf) CU(cudaMalloc((void**)&c->d_psf, sizeof(float) * GLAD_MAX_PSF * GLAD_MAX_PSF), "cudaMalloc psf");
@@ -285,9 +285,9 @@ glad_status glad_set_kin_data(glad_ctx* c, const glad_sky_grid* g, const int32_t
         // jam_post_kernel stages both folded maps plus (nxf + nyf) floats per luminous Gaussian: necessary condition here
         // (one Gaussian), the exact one in the batch call, which knows n_lum
         const size_t need = jam_post_smem_bytes(nxf, nyf, 1);
-        if (need > (size_t)c->smem_optin)
+        if (need > (size_t)glad_smem_dynamic_max(c))
             return fail(c, GLAD_ESHAPE, "glad_set_kin_data: folded grid %dx%d needs %zu bytes of shared memory in the binning kernel, limit %d",
-                        nxf, nyf, need, c->smem_optin);
+                        nxf, nyf, need, glad_smem_dynamic_max(c));
     }
     std::vector<float> xf2(nxf), yf2(nyf);
     for (int i = 0; i < nxf; ++i) xf2[i] = xf[i] * xf[i];
@@ -351,9 +351,9 @@ static glad_status jam_impl(glad_ctx* c, const float* d_dyn, int B, const float*
     const int nmx = nm + 1;
     int NG;
     if (jam_quad_geometry(c, &NG) < 0) return fail(c, GLAD_ESHAPE, "jam: sky grid too large");
-    if (jam_post_smem_bytes(c->nxf, c->nyf, nl) > (size_t)c->smem_optin)
+    if (jam_post_smem_bytes(c->nxf, c->nyf, nl) > (size_t)glad_smem_dynamic_max(c))
         return fail(c, GLAD_ESHAPE, "jam: folded grid %dx%d with %d luminous Gaussians needs %zu bytes of shared memory in the binning kernel, limit %d",
-                    c->nxf, c->nyf, nl, jam_post_smem_bytes(c->nxf, c->nyf, nl), c->smem_optin);
+                    c->nxf, c->nyf, nl, jam_post_smem_bytes(c->nxf, c->nyf, nl), glad_smem_dynamic_max(c));
     // K-slices: enough CTAs for >= 4 per SM when the batch is small
     long M = (long)c->nu * nmx * nl;
     int NCH = (int)((M + NG * JQ_MI - 1) / (NG * JQ_MI));

@@ -149,12 +149,20 @@ struct ProfScope {
 };
 
 // Opt a kernel in to the device's maximum dynamic shared memory.  The attribute is per function AND per device, so it is set
-// (to the same value every time) before each launch instead of being cached in a process-wide static: a second context on
+// (to the same value every time: the device limit minus the kernel's static shared memory) before each launch instead of being cached in a process-wide static: a second context on
 // another GPU, or another host thread, sees the same state.  Cost: a few microseconds of host time per launch.
 template <typename K>
 static inline cudaError_t smem_optin(const glad_ctx* c, K kernel) {
-    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin);
+    // the limit covers static + dynamic shared memory; a kernel's static size is a property of its code, not of the device
+    static const int static_bytes = [kernel] {
+        cudaFuncAttributes fa;
+        return cudaFuncGetAttributes(&fa, kernel) == cudaSuccess ? (int)fa.sharedSizeBytes : 1024;
+    }();
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin - static_bytes);
 }
+// Dynamic shared memory a launch may ask for: the device's opt-in limit minus 1 KB kept for the kernels' static shared memory
+// (reduction scratch, barriers).  The shape checks made when static data is set use this number.
+static inline int glad_smem_dynamic_max(const glad_ctx* c) { return c->smem_optin - 1024; }
 // Every entry point makes the context's device current and restores the caller's on return.
 struct DeviceScope {
     int prev;

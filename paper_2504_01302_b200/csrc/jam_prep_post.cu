@@ -254,7 +254,7 @@ size_t jam_post_smem_bytes(int nxf, int nyf, int nl) {
 cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d_vrms, float* d_chi2,
                             float* d_v2map, int32_t* d_flags) {
     const size_t smem = jam_post_smem_bytes(c->nxf, c->nyf, nl);
-    if (smem > (size_t)c->smem_optin) return cudaErrorInvalidConfiguration;   // glad_set_kin_data checks this up front
+    if (smem > (size_t)glad_smem_dynamic_max(c)) return cudaErrorInvalidConfiguration;   // glad_set_kin_data checks this up front
     cudaError_t e = smem_optin(c, jam_post_kernel);
     if (e != cudaSuccess) return e;
     ProfScope ps(c, GK_JAM_POST);

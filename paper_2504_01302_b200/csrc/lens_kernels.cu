@@ -316,7 +316,7 @@ size_t lens_image_smem_bytes(int nx, int ny, int kpsf) {
 
 cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2, int32_t* d_flags) {
     const size_t smem = lens_image_smem_bytes(c->grid.nx, c->grid.ny, c->kpsf);
-    if (smem > (size_t)c->smem_optin) return cudaErrorInvalidConfiguration;   // glad_set_image_data checks this up front
+    if (smem > (size_t)glad_smem_dynamic_max(c)) return cudaErrorInvalidConfiguration;   // glad_set_image_data checks this up front
     const int ch = c->light_kinds != 0 || c->d_lambda != nullptr;
     cudaError_t e = ch ? smem_optin(c, lens_image_kernel<true>) : smem_optin(c, lens_image_kernel<false>);
     if (e != cudaSuccess) return e;

@@ -64,6 +64,44 @@ def gauss_legendre_u(n: int):
     return (t * t).astype(np.float32), (2.0 * t * w).astype(np.float32)
 
 
+# 7-point Kronrod extension of the 3-point Gauss rule on [-1, 1] (the pair Shampine's TwoD uses): nodes, weights
+_K7_X = np.array([-0.9604912687080203, -0.7745966692414834, -0.4342437493468026, 0.0,
+                  0.4342437493468026, 0.7745966692414834, 0.9604912687080203])
+_K7_W = np.array([0.1046562260264673, 0.2684880898683334, 0.4013974147759622, 0.4509165386584741,
+                  0.4013974147759622, 0.2684880898683334, 0.1046562260264673])
+
+
+def kronrod_composite(panels: int):
+    """Composite 7-point Kronrod rule on (0,1): `panels` equal sub-intervals.  The paper's fixed mesh (the region cut into
+    64 sub-regions, each into four rectangles, Gauss-Kronrod in each) is 16 x 16 rectangles = this rule with panels = 16 in each
+    of the two directions (112 x 112 nodes)."""
+    h = 1.0 / panels
+    x = np.concatenate([(p + 0.5 * (_K7_X + 1.0)) * h for p in range(panels)])
+    w = np.concatenate([0.5 * h * _K7_W for _ in range(panels)])
+    return x, w
+
+
+def jam_sph_rules(kin: dict, panels: int = 16, nr: int = 20, nth: int = 10, nz: int = 96, u_decades: float = 5.0,
+                  sigma_max: float = 0.0) -> dict:
+    """Inputs of the JAM_sph path (readings R-SPH1..4) for the sky grid of `kin`: polar grid (20 x 10 = "over 200
+    points in polar coordinates") log-spaced in r from half the smallest pixel radius to the larger of 3 x the largest pixel
+    radius and 4 x sigma_max (the widest luminous Gaussian: the LOS integral reaches that far), uniform in theta
+    on [0, pi/2]; radial rule tau on (0,1) and potential rule u = 10^(-u_decades (1 - t)) (log-spaced: the u^2 exp(-a u^2) peaks
+    of a sigma = 0.01" black hole seen from r' ~ 60" sit at u ~ 1e-4), both from the composite Kronrod mesh; LOS rule = nz-point
+    Gauss-Legendre on (-1,1)."""
+    xs, ys = np.asarray(kin["xs"], np.float64), np.asarray(kin["ys"], np.float64)
+    rad = np.hypot(*np.meshgrid(xs, ys))
+    rmin = max(0.5 * float(rad[rad > 0].min()) if (rad > 0).any() else 1e-3, 1e-4)
+    rmax = max(3.0 * float(rad.max()) if rad.max() > 0 else 1.0, 4.0 * float(sigma_max))
+    t, w = kronrod_composite(panels)
+    L = u_decades * np.log(10.0)
+    u = np.exp(-L * (1.0 - t))
+    z, wz = np.polynomial.legendre.leggauss(nz)
+    f = np.float32
+    return dict(rgrid=np.geomspace(rmin, rmax, nr).astype(f), thgrid=np.linspace(0.0, 0.5 * np.pi, nth).astype(f),
+                tau=t.astype(f), wtau=w.astype(f), un=u.astype(f), uw=(L * u * w).astype(f), zeta=z.astype(f), wz=wz.astype(f))
+
+
 def _psf(kind: str, k: int, pix: float, fwhm: float) -> np.ndarray:
     c = k // 2
     yy, xx = np.mgrid[0:k, 0:k]
