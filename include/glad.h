@@ -229,9 +229,10 @@ double glad_bh_theta2(double mbh_msun, double ddt_mpc, double z_d);
  * context stream around every kernel launch (at most 2048 launches between reads).  glad_profile_read
  * SYNCHRONISES the stream, adds the elapsed times to per-kernel totals, copies them out and clears them.
  * Kernel order: 0 lens_prep, 1 lens_image, 2 jam_prep, 3 jam_quad, 4 jam_post, 5 joint, 6 mge (mge1d / model kernel), 7 quasar,
- * 8 pixsrc_map, 9 pixsrc_blur, 10 pixsrc_syrk, 11 pixsrc_rhs, 12 pixsrc_chol, 13 pixsrc_model (+ static / final kernels).
+ * 8 pixsrc_map, 9 pixsrc_blur, 10 pixsrc_syrk, 11 pixsrc_rhs, 12 pixsrc_chol, 13 pixsrc_model (+ static / final kernels),
+ * 14 jam_sph (intrinsic moments), 15 jam_sph_los.
  */
-#define GLAD_NKERNELS 14
+#define GLAD_NKERNELS 16
 glad_status glad_profile_enable(glad_ctx* ctx, int on);
 glad_status glad_profile_read(glad_ctx* ctx, double* ms_out /*[GLAD_NKERNELS]*/, long* count_out /*[GLAD_NKERNELS]*/);
 
@@ -357,6 +358,40 @@ glad_status glad_set_mass_sheet(glad_ctx* ctx, const float* d_lambda, int n_lamb
 glad_status glad_pixsrc_evidence_batch(glad_ctx* ctx, const float* d_lens_params, const float* d_src_grid, const float* d_lambda_reg,
                                        int n_sx, int n_sy, int B, int scratch_mib_max, float* d_logev, float* d_chi2, float* d_reg,
                                        float* d_s_mp, float* d_model, int32_t* d_flags);
+
+/*
+ * JAM_sph, the dynamics the paper itself runs -- the axisymmetric Jeans equations with a SPHERICALLY-aligned
+ * velocity ellipsoid (Eq. 17-18, beta_ani = 1 - v_theta^2/v_r^2 Eq. 20), solved for the intrinsic moments
+ * v_r^2, v_theta^2, v_phi^2 "at the required positions ... in polar coordinates" by a NON-ADAPTIVE 2-D quadrature, then
+ * projected along the line of sight (Eq. 26), convolved and binned (Eq. 27-28) and compared (Eq. 32).  The paper prints no
+ * solution formula (it defers to Cappellari 2020 at P:228); DESIGN.md R-SPH1..6 derive it from Eq. 17-18:
+ *   nu v_r^2 (r,th) = int_r^r_cut (r'/r)^(2 beta) nu(r',th') (r'^2/z') dPhi/dz'(r',th') dr'/r',  sin th' = sin th (r/r')^(1-beta),
+ *   nu v_th^2 = (1-beta) nu v_r^2,   nu v_phi^2 = (1-beta) [nu v_r^2 + tan th d(nu v_r^2)/dth] + nu tan th dPhi/dth,
+ * Phi the MGE potential (a u-integral on (0,1) per mass Gaussian), per luminous Gaussian k with its own beta_k, r_cut = 6 max sigma_k.
+ *
+ * glad_set_jam_sph_rules: DEVICE pointers, BORROWED; d_rgrid = NULL clears.
+ *   d_rgrid [nr] ascending radii (arcsec), d_thgrid [nth] ascending polar angles in [0, pi/2] (from the symmetry axis): the polar
+ *     grid; the moment ratios are interpolated bilinearly in (ln r, theta), clamped at the grid edges (R-SPH2, R-SPH3);
+ *   d_tau, d_wtau [nt]: rule on (0,1) for r' = r (r_cut/r)^tau;  d_un, d_uw [nu]: rule on (0,1) for the potential integral (the
+ *     paper's mesh, 64 sub-regions x 4 Gauss-Kronrod rectangles P:360, is 112 x 112 nodes);
+ *   d_zeta, d_wz [nz]: rule on (-1,1) for z' = rho_0 sinh(a zeta), rho_0 = max(sky radius, rgrid[0]), a = asinh(r_cut/rho_0) (R-SPH4).
+ *   GLAD_ESHAPE beyond nr <= GLAD_MAX_SPH_R, nth <= GLAD_MAX_SPH_TH, nt, nu, nz <= GLAD_MAX_NODES.
+ *
+ * glad_jam_sph_vrms_batch: arguments and outputs as glad_jam_vrms_batch (sky grid, kernel, bins, data from glad_set_kin_data; its
+ * u rule is not used), except that d_beta holds beta_ani (< 1, else GLAD_FLAG_DYN_INVALID) and
+ *   d_moments [B,3,nr,nth] or NULL receives v_r^2, v_theta^2, v_phi^2 in (km/s)^2 on the polar grid.
+ * d_v2map is int nu v_z'^2 dz' (km^2 s^-2 Lsun pc^-2).  fp32 arithmetic with fp64-prepared tables.  GLAD_ESTATE without kinematic
+ * data or rules; GLAD_ESHAPE if 20 (n_mass + 1) nu bytes of potential table do not fit shared memory.
+ */
+#define GLAD_MAX_SPH_R 128
+#define GLAD_MAX_SPH_TH 64
+glad_status glad_set_jam_sph_rules(glad_ctx* ctx, const float* d_rgrid, int nr, const float* d_thgrid, int nth, const float* d_tau,
+                                   const float* d_wtau, int nt, const float* d_u_nodes, const float* d_u_weights, int nu,
+                                   const float* d_zeta, const float* d_wz, int nz);
+glad_status glad_jam_sph_vrms_batch(glad_ctx* ctx, const float* d_dyn_params, int B, const float* d_lum_mge, int n_lum,
+                                    long lum_stride, const float* d_mass_mge, int n_mass, long mass_stride, const float* d_beta,
+                                    int beta_per_gaussian, float* d_vrms, float* d_chi2, float* d_v2map, float* d_moments,
+                                    int32_t* d_flags);
 
 /* Number of kernel launches enqueued by this context since creation (for bench.py's gpu_launches). */
 long glad_launch_count(const glad_ctx* ctx);

@@ -24,7 +24,7 @@ EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "gl
            "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count", "glad_profile_enable",
            "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch", "glad_set_overlap", "glad_set_light_profiles",
            "glad_set_quasar_data", "glad_quasar_chi2_batch", "glad_joint_loglike_full_batch", "glad_set_mass_sheet",
-           "glad_pixsrc_evidence_batch", "glad_set_jam_options"]
+           "glad_pixsrc_evidence_batch", "glad_set_jam_options", "glad_set_jam_sph_rules", "glad_jam_sph_vrms_batch"]
 
 
 class GladError(RuntimeError):
@@ -97,6 +97,10 @@ def load(rebuild: bool = False):
     L.glad_set_mass_sheet.argtypes = [vp, vp, i, C.c_float, C.c_float, i, C.c_float, C.c_float]
     L.glad_pixsrc_evidence_batch.restype = i
     L.glad_pixsrc_evidence_batch.argtypes = [vp, vp, vp, vp, i, i, i, i, vp, vp, vp, vp, vp, vp]
+    L.glad_set_jam_sph_rules.restype = i
+    L.glad_set_jam_sph_rules.argtypes = [vp, vp, i, vp, i, vp, vp, i, vp, vp, i, vp, vp, i]
+    L.glad_jam_sph_vrms_batch.restype = i
+    L.glad_jam_sph_vrms_batch.argtypes = [vp, vp, i, vp, i, l, vp, i, l, vp, i, vp, vp, vp, vp, vp]
     L.glad_set_jam_options.restype = i
     L.glad_set_jam_options.argtypes = [vp, i, i, i, i]
     L.glad_launch_count.restype = l
@@ -165,7 +169,7 @@ class Glad:
         return int(self.lib.glad_launch_count(self.ctx))
 
     KERNELS = ("lens_prep", "lens_image", "jam_prep", "jam_quad", "jam_post", "joint", "mge", "quasar",
-               "pixsrc_map", "pixsrc_blur", "pixsrc_syrk", "pixsrc_rhs", "pixsrc_chol", "pixsrc_model")
+               "pixsrc_map", "pixsrc_blur", "pixsrc_syrk", "pixsrc_rhs", "pixsrc_chol", "pixsrc_model", "jam_sph", "jam_sph_los")
 
     def set_light_profiles(self, source=0, lens1=0, lens2=0):
         """0 = Sersic, 1 = Chameleon (Eq. 47) per light component, for the batch calls that follow."""
@@ -243,6 +247,30 @@ class Glad:
         self._check(self.lib.glad_jam_vrms_batch(self.ctx, _p(d), B, _p(lum), nl, ls, _p(mass) if nm else None, nm, ms,
                                                  _p(bt), pg, _p(vrms), _p(chi2), _p(v2map), _p(flags)))
         return {"vrms": vrms, "chi2": chi2, "v2map": v2map, "flags": flags}
+
+    def set_jam_sph_rules(self, sph: dict):
+        """sph = dict(rgrid, thgrid, tau, wtau, un, uw, zeta, wz): polar grid and the three rules of the JAM_sph path."""
+        k = {n: _dev(sph[n], torch.float32, self.device) for n in ("rgrid", "thgrid", "tau", "wtau", "un", "uw", "zeta", "wz")}
+        self._check(self.lib.glad_set_jam_sph_rules(self.ctx, _p(k["rgrid"]), int(k["rgrid"].numel()), _p(k["thgrid"]),
+                                                    int(k["thgrid"].numel()), _p(k["tau"]), _p(k["wtau"]), int(k["tau"].numel()),
+                                                    _p(k["un"]), _p(k["uw"]), int(k["un"].numel()), _p(k["zeta"]), _p(k["wz"]),
+                                                    int(k["zeta"].numel())))
+        self._keep["sph"] = k
+        self.sph_shape = (int(k["rgrid"].numel()), int(k["thgrid"].numel()))
+
+    def jam_sph_vrms_batch(self, dyn_params, lum_mge, mass_mge, beta, want_chi2=True, want_map=False, want_moments=False):
+        """JAM_sph (the paper's dynamics): beta = beta_ani; outputs as jam_vrms_batch plus moments [B,3,nr,nth]."""
+        d = _dev(dyn_params, torch.float32, self.device).reshape(-1, NDYN)
+        B = d.shape[0]
+        lum, nl, ls, mass, nm, ms, bt, pg = self._tables(lum_mge, mass_mge, beta)
+        vrms = torch.empty((B, self.nbins), dtype=torch.float32, device=self.device)
+        chi2 = torch.empty(B, dtype=torch.float32, device=self.device) if want_chi2 else None
+        v2map = torch.empty((B,) + (self.sky_shape or (0, 0)), dtype=torch.float32, device=self.device) if want_map else None
+        mom = torch.empty((B, 3) + self.sph_shape, dtype=torch.float32, device=self.device) if want_moments else None
+        flags = torch.empty(B, dtype=torch.int32, device=self.device)
+        self._check(self.lib.glad_jam_sph_vrms_batch(self.ctx, _p(d), B, _p(lum), nl, ls, _p(mass) if nm else None, nm, ms,
+                                                     _p(bt), pg, _p(vrms), _p(chi2), _p(v2map), _p(mom), _p(flags)))
+        return {"vrms": vrms, "chi2": chi2, "v2map": v2map, "moments": mom, "flags": flags}
 
     def joint_loglike_batch(self, lens_params, dyn_params, lum_mge, mass_mge, beta, out=None):
         p = _dev(lens_params, torch.float32, self.device).reshape(-1, NLENS)

@@ -104,7 +104,8 @@ void glad_destroy(glad_ctx* c) {
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     free_kin(c);
-    void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage, c->d_model, c->d_qtmp, c->d_pix};
+    void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage, c->d_model, c->d_qtmp, c->d_pix,
+                  c->d_sph_tab, c->d_sph_rat};
     for (void* p : ps) if (p) cudaFree(p);
     for (cudaEvent_t e : c->prof_ev) if (e) cudaEventDestroy(e);
     }
@@ -392,6 +393,64 @@ glad_status glad_jam_vrms_batch(glad_ctx* c, const float* d_dyn, int B, const fl
     DeviceScope ds(c);
     return jam_impl(c, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian, d_vrms, d_chi2,
                     d_v2map, d_flags);
+}
+
+}  // extern "C"
+
+extern "C" {
+
+glad_status glad_set_jam_sph_rules(glad_ctx* c, const float* d_rgrid, int nr, const float* d_thgrid, int nth, const float* d_tau,
+                                   const float* d_wtau, int nt, const float* d_un, const float* d_uw, int nu, const float* d_zeta,
+                                   const float* d_wz, int nz) {
+    if (!c) return GLAD_EINVAL;
+    if (!d_rgrid) { c->have_sph = false; return GLAD_OK; }
+    if (!d_thgrid || !d_tau || !d_wtau || !d_un || !d_uw || !d_zeta || !d_wz) return fail(c, GLAD_EINVAL, "glad_set_jam_sph_rules: null pointer");
+    if (nr < 1 || nth < 1 || nt < 1 || nu < 1 || nz < 1) return fail(c, GLAD_EINVAL, "glad_set_jam_sph_rules: bad sizes");
+    if (nr > GLAD_MAX_SPH_R || nth > GLAD_MAX_SPH_TH || nt > GLAD_MAX_NODES || nu > GLAD_MAX_NODES || nz > GLAD_MAX_NODES)
+        return fail(c, GLAD_ESHAPE, "glad_set_jam_sph_rules: polar grid %d x %d / rules %d, %d, %d exceed the limits", nr, nth, nt, nu, nz);
+    c->d_sph_r = d_rgrid; c->sph_nr = nr; c->d_sph_th = d_thgrid; c->sph_nth = nth;
+    c->d_sph_tau = d_tau; c->d_sph_wtau = d_wtau; c->sph_nt = nt;
+    c->d_sph_un = d_un; c->d_sph_uw = d_uw; c->sph_nu = nu;
+    c->d_sph_zeta = d_zeta; c->d_sph_wz = d_wz; c->sph_nz = nz;
+    c->have_sph = true;
+    return GLAD_OK;
+}
+
+glad_status glad_jam_sph_vrms_batch(glad_ctx* c, const float* d_dyn, int B, const float* d_lum, int nl, long lum_stride,
+                                    const float* d_mass, int nm, long mass_stride, const float* d_beta, int per_gaussian,
+                                    float* d_vrms, float* d_chi2, float* d_v2map, float* d_moments, int32_t* d_flags) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && !d_dyn)) return fail(c, GLAD_EINVAL, "glad_jam_sph_vrms_batch: B=%d / null params", B);
+    if (!c->have_kin) return fail(c, GLAD_ESTATE, "glad_jam_sph_vrms_batch: glad_set_kin_data not called");
+    if (!c->have_sph) return fail(c, GLAD_ESTATE, "glad_jam_sph_vrms_batch: glad_set_jam_sph_rules not called");
+    if (d_chi2 && !c->d_vobs) return fail(c, GLAD_ESTATE, "glad_jam_sph_vrms_batch: chi2 requested but no vrms_obs/vrms_ivar set");
+    if (!d_lum || !d_beta || (nm > 0 && !d_mass)) return fail(c, GLAD_EINVAL, "glad_jam_sph_vrms_batch: null table pointer");
+    if (nl <= 0 || nm < 0) return fail(c, GLAD_EINVAL, "glad_jam_sph_vrms_batch: n_lum %d / n_mass %d", nl, nm);
+    if (nl > GLAD_MAX_GAUSS || nm > GLAD_MAX_GAUSS) return fail(c, GLAD_ESHAPE, "glad_jam_sph_vrms_batch: more than GLAD_MAX_GAUSS Gaussians");
+    if (lum_stride < 0 || mass_stride < 0) return fail(c, GLAD_EINVAL, "glad_jam_sph_vrms_batch: negative stride");
+    if (B == 0) return GLAD_OK;
+    DeviceScope ds(c);
+    const int nmx = nm + 1;
+    if (!jam_sph_supported(c, nl, nmx))
+        return fail(c, GLAD_ESHAPE, "glad_jam_sph_vrms_batch: the potential table of %d mass Gaussians x %d u-nodes does not fit shared memory", nmx, c->sph_nu);
+    if (jam_post_smem_bytes(c->nxf, c->nyf, nl) > (size_t)glad_smem_dynamic_max(c))
+        return fail(c, GLAD_ESHAPE, "glad_jam_sph_vrms_batch: folded grid %dx%d with %d luminous Gaussians does not fit the binning kernel", c->nxf, c->nyf, nl);
+    glad_status st = grow(c, &c->d_jam_tab, &c->jam_tab_cap, (size_t)B * jam_table_floats(nl, nmx));
+    if (st != GLAD_OK) return st;
+    st = grow(c, &c->d_sph_tab, &c->sph_tab_cap, (size_t)B * jam_sph_table_floats(nl, nmx, c->sph_nu));
+    if (st != GLAD_OK) return st;
+    st = grow(c, &c->d_partial, &c->partial_cap, (size_t)B * c->nxf * c->nyf);
+    if (st != GLAD_OK) return st;
+    float* rat = d_moments;
+    if (!rat) {
+        st = grow(c, &c->d_sph_rat, &c->sph_rat_cap, (size_t)B * 3 * c->sph_nr * c->sph_nth);
+        if (st != GLAD_OK) return st;
+        rat = c->d_sph_rat;
+    }
+    CU(launch_jam_prep(c, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian), "jam_prep_kernel");
+    CU(launch_jam_sph(c, d_dyn, B, d_lum, nl, lum_stride, d_mass, nm, mass_stride, d_beta, per_gaussian, rat), "jam_sph kernels");
+    CU(launch_jam_post(c, B, nl, nmx, 1, d_vrms, d_chi2, d_v2map, d_flags, 1.f), "jam_post_kernel");
+    return GLAD_OK;
 }
 
 }  // extern "C"

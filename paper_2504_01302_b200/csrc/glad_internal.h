@@ -49,7 +49,7 @@ static inline __host__ __device__ int jam_table_floats(int nl, int nmx) {
 
 #define GLAD_PROF_MAX 2048
 enum GladKernelId { GK_LENS_PREP = 0, GK_LENS_IMAGE, GK_JAM_PREP, GK_JAM_QUAD, GK_JAM_POST, GK_JOINT, GK_MGE, GK_QUASAR,
-                    GK_PIX_MAP, GK_PIX_BLUR, GK_PIX_SYRK, GK_PIX_RHS, GK_PIX_CHOL, GK_PIX_MODEL };
+                    GK_PIX_MAP, GK_PIX_BLUR, GK_PIX_SYRK, GK_PIX_RHS, GK_PIX_CHOL, GK_PIX_MODEL, GK_JAM_SPH, GK_JAM_SPH_LOS };
 
 // quasar data (glad_set_quasar_data), passed to quasar_kernel by value
 struct glad_quasar_data {
@@ -112,6 +112,13 @@ struct glad_ctx {
     int* d_bin_cnt;         // ctx-owned: spaxels per bin [nbins]
     int* d_binw_ptr;        // ctx-owned: the non-zero entries of W_f row by row (the kernel K is compact, so a bin touches a
     float2* d_binw_nz;      // fraction of the map): row l = entries [ptr[l], ptr[l+1]) of {folded pixel index as int bits, weight}
+
+    // JAM_sph rules (glad_set_jam_sph_rules): borrowed device pointers
+    bool have_sph;
+    int sph_nr, sph_nth, sph_nt, sph_nu, sph_nz;
+    const float *d_sph_r, *d_sph_th, *d_sph_tau, *d_sph_wtau, *d_sph_un, *d_sph_uw, *d_sph_zeta, *d_sph_wz;
+    float* d_sph_tab;    size_t sph_tab_cap;    // per-vector JAM_sph tables
+    float* d_sph_rat;    size_t sph_rat_cap;    // [B,3,nr,nth] moment ratios when the caller does not ask for them
 
     // grow-only scratch
     float* d_lens_const; size_t lens_const_cap;
@@ -176,8 +183,16 @@ cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2
 cudaError_t launch_jam_prep(glad_ctx* c, const float* d_dyn, int B, const float* d_lum, int nl, long lum_stride,
                             const float* d_mass, int nm, long mass_stride, const float* d_beta, int per_gaussian);
 cudaError_t launch_jam_quad(glad_ctx* c, int B, int nl, int nmx, int S);
+// unit_scale <= 0: the partial maps are in the cylindrical quadrature's units (scale from the table header)
 cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d_vrms, float* d_chi2,
-                            float* d_v2map, int32_t* d_flags);
+                            float* d_v2map, int32_t* d_flags, float unit_scale = 0.f);
+// JAM_sph (jam_sph.cu): prep + intrinsic moments on the polar grid + LOS integral into c->d_partial (one slice, final units);
+// needs c->d_jam_tab from launch_jam_prep (validity) and c->d_sph_tab sized jam_sph_table_floats() per vector
+size_t jam_sph_table_floats(int nl, int nmx, int nu);
+bool jam_sph_supported(const glad_ctx* c, int nl, int nmx);
+cudaError_t launch_jam_sph(glad_ctx* c, const float* d_dyn, int B, const float* d_lum, int nl, long lum_stride,
+                           const float* d_mass, int nm, long mass_stride, const float* d_beta, int per_gaussian,
+                           float* d_ratios);
 cudaError_t launch_joint(glad_ctx* c, int B, const float* d_c2l, const float* d_c2d, const float* d_c2img, const float* d_c2tmd,
                          const int32_t* d_fl, const int32_t* d_fd, float* d_loglike, int32_t* d_flags);
 cudaError_t launch_quasar(glad_ctx* c, cudaStream_t st, const float* d_lens, const float* d_ddt, int B, float* d_chi2_img,

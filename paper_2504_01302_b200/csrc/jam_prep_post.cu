@@ -165,7 +165,8 @@ __global__ void __launch_bounds__(256) jam_post_kernel(const float* __restrict__
                                                       const int* __restrict__ bin_cnt, int nbins,
                                                       const float* __restrict__ vobs, const float* __restrict__ vivar,
                                                       float* __restrict__ vrms, float* __restrict__ chi2,
-                                                      float* __restrict__ v2map, int32_t* __restrict__ flags) {
+                                                      float* __restrict__ v2map, int32_t* __restrict__ flags,
+                                                      float unit_scale) {
     extern __shared__ __align__(16) float sm[];
     const int b = blockIdx.x, tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5;
     const int npf = nxf * nyf;
@@ -189,7 +190,7 @@ __global__ void __launch_bounds__(256) jam_post_kernel(const float* __restrict__
         return;
     }
     if (tid == 0) s_badbin = 0;
-    const float scale = T[JH_SCALE];
+    const float scale = unit_scale > 0.f ? unit_scale : T[JH_SCALE];   // JAM_sph maps arrive in final units
     const float* P = partial + (size_t)b * S * npf;
     for (int i = tid; i < npf; i += nthr) {
         float a = 0.f;
@@ -252,7 +253,7 @@ size_t jam_post_smem_bytes(int nxf, int nyf, int nl) {
 }
 
 cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d_vrms, float* d_chi2,
-                            float* d_v2map, int32_t* d_flags) {
+                            float* d_v2map, int32_t* d_flags, float unit_scale) {
     const size_t smem = jam_post_smem_bytes(c->nxf, c->nyf, nl);
     if (smem > (size_t)glad_smem_dynamic_max(c)) return cudaErrorInvalidConfiguration;   // glad_set_kin_data checks this up front
     cudaError_t e = smem_optin(c, jam_post_kernel);
@@ -261,7 +262,7 @@ cudaError_t launch_jam_post(glad_ctx* c, int B, int nl, int nmx, int S, float* d
     jam_post_kernel<<<B, 256, smem, c->stream>>>(c->d_jam_tab, jam_table_floats(nl, nmx), nl, nmx, c->d_partial, S, c->nx,
                                                 c->ny, c->nxf, c->nyf, c->d_xf2, c->d_yf2, c->d_foldx, c->d_foldy,
                                                 c->d_binw_ptr, c->d_binw_nz, c->d_bin_cnt, c->nbins, c->d_vobs, c->d_vivar, d_vrms,
-                                                d_chi2, d_v2map, d_flags);
+                                                d_chi2, d_v2map, d_flags, unit_scale);
     return cudaGetLastError();
 }
 
