@@ -27,14 +27,50 @@ if ROOT not in sys.path:
 METRIC = "joint_loglike_evals_per_s"
 UNIT = "evals/s"
 FP32_LANES_PER_SM = 128
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the quadrature kernel from the committed ncu --set full
-# captures (profiles/r1a.md, profiles/r1b.md): operands never exist in HBM, only the tables are read
-RESIDENT_TRAFFIC = {"jam_quad_simt": 4.4e6, "jam_quad_tc": 4.44e6}
-# Executed FP32 flops of lens_image_kernel per parameter vector (FFMA = 2, FMUL = FADD = 1; MUFU not counted) from the
-# same captures' smsp__sass_thread_inst_executed_op_{ffma,fmul,fadd}_pred_on (profiles/r1b.md: 8.05e9 FFMA, 2.60e9
-# FMUL, 0.63e9 FADD per 1024-vector C2 launch).  SURVEY.md 8(d)'s algorithmic estimate for C2 is 1.82e7 per vector
-# (40 000 rays x ~235 flop + 10 000 pixels x 2 x 441 PSF taps).
-LENS_FP32_FLOPS_PER_VECTOR = {"C2": 1.888e7}
+# ncu --set full numbers (DRAM traffic, executed FP32 instructions) are NOT typed in here: they are read from the committed capture
+# summaries that profiles/current_capture.txt lists, each with the sha256 of the kernel source it was taken from.  When the
+# source has changed since, the capture is stale and the key is reported as null with the reason.
+CAPTURE_INDEX = os.path.join(ROOT, "profiles", "current_capture.txt")
+_UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+
+
+def load_capture(key: str) -> dict:
+    """{'fresh': bool, 'file': csv path, 'metrics': {name: value (bytes for byte units)}, 'note': str}"""
+    import hashlib
+    out = {"fresh": False, "file": None, "metrics": {}, "note": "no capture listed in profiles/current_capture.txt"}
+    if not os.path.exists(CAPTURE_INDEX):
+        return out
+    for line in open(CAPTURE_INDEX):
+        f = line.split()
+        if len(f) < 4 or f[0] != key:
+            continue
+        csv_path, src, sha = os.path.join(ROOT, f[1]), os.path.join(ROOT, f[2]), f[3]
+        out["file"] = f[1]
+        if not (os.path.exists(csv_path) and os.path.exists(src)):
+            out["note"] = "capture file or kernel source missing"
+            return out
+        now = hashlib.sha256(open(src, "rb").read()).hexdigest()[:16]
+        for row in open(csv_path).read().splitlines()[1:]:
+            c = row.split(",")
+            if len(c) >= 3:
+                try:
+                    out["metrics"][c[0]] = float(c[2]) * _UNIT.get(c[1], 1.0)
+                except ValueError:
+                    pass
+        out["fresh"] = now == sha
+        out["note"] = (f"{f[1]} (taken at sha256[:16] of {f[2]} = {sha}" + (")" if out["fresh"] else f"; the source is now {now}: STALE)"))
+        return out
+    return out
+
+
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
 
 
 def read_peaks():
@@ -240,6 +276,112 @@ def run_pixsrc_sweep(args):
     g.close()
 
 
+NCU_KEEP = ("Kernel Name", "gpu__time_duration.sum", "dram__bytes_read.sum", "dram__bytes_write.sum", "launch__", "sm__throughput",
+            "sm__warps_active", "smsp__issue_active", "sm__inst_executed_pipe_", "sm__pipe_fma_cycles", "sm__pipe_fp64", "sm__pipe_tensor",
+            "l1tex__throughput", "lts__throughput", "dram__throughput", "l1tex__data_pipe_", "l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum",
+            "smsp__inst_executed.sum", "smsp__average_warp", "sm__cycles_elapsed", "smsp__sass_thread_inst_executed_op_")
+
+
+def ncu_summary(args):
+    """--ncu-summary REP: filter `ncu -i REP --page raw --csv` (run here, no GPU needed) down to the metrics the write-ups and this
+    bench use, write it to --out (a .csv under profiles/) and record it in profiles/current_capture.txt with the sha256 of the
+    kernel source, so that load_capture() can tell a fresh capture from a stale one."""
+    import csv
+    import hashlib
+    import io
+    raw = subprocess.run(["ncu", "-i", args.ncu_summary, "--page", "raw", "--csv"], check=True, capture_output=True, text=True).stdout
+    rows = list(csv.reader(io.StringIO(raw)))
+    h, u = rows[0], rows[1]
+    v = rows[2 + args.capture_row]
+    with open(os.path.join(ROOT, args.out), "w") as f:
+        f.write("metric,unit,value\n")
+        for i, name in enumerate(h):
+            if any(name.startswith(k) for k in NCU_KEEP) and not name.endswith("_not_issued.ratio"):
+                f.write(f"{name},{u[i]},{v[i].replace(',', ' ')}\n")
+    sha = hashlib.sha256(open(os.path.join(ROOT, args.capture_source), "rb").read()).hexdigest()[:16]
+    lines = [l for l in (open(CAPTURE_INDEX).read().splitlines() if os.path.exists(CAPTURE_INDEX) else []) if l.split()[:1] != [args.capture_key]]
+    lines.append(f"{args.capture_key} {args.out} {args.capture_source} {sha}")
+    open(CAPTURE_INDEX, "w").write("\n".join(lines) + "\n")
+    print(f"wrote {args.out}; {args.capture_key} -> sha {sha}")
+
+
+def peak_tf_of(dev, clocks):
+    import torch
+    peaks = read_peaks()
+    sm_max = float(peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+    return torch.cuda.get_device_properties(dev).multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+
+
+def run_configs(args, device, peak_tf, clocks):
+    """Every other BASELINE.json config at its FULL batch on one GPU (C1; two C3 cells; C4 at 8192; C5 at 4096): evals/s, the two
+    stage kernels' ms per launch and their fractions.  Per-kernel times on one stream (glad_set_overlap(0)); the step time with the
+    default two streams."""
+    import torch
+    import workloads
+    from paper_2504_01302_b200 import Glad
+    sm_max = float(read_peaks().get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0)
+    xu_peak = torch.cuda.get_device_properties(device).multi_processor_count * 16 * sm_max * 1e6
+    rows = {}
+    for name in ("C1", "C3-10-40-4096", "C3-40-160-256", "C4", "C5"):
+        wl = workloads.make_workload(name, gpu_data_model(device))
+        L, D, B = wl["lens"], wl["dyn"], wl["B"]
+        g = Glad(device)
+        if L:
+            g.set_image_data(L["grid"], L["psf"], L["data"], L["ivar"])
+        if D:
+            g.set_kin_data(D["kin"])
+        dev = torch.device("cuda", device)
+        tt = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).to(dev)
+        lp = tt(L["params"]) if L else None
+        da = tuple(tt(D[k]) for k in ("params", "lum_mge", "mass_mge", "beta")) if D else None
+
+        def step():
+            if L and D:
+                g.joint_loglike_batch(lp, *da)
+            elif L:
+                g.lens_image_batch(lp, want_images=False)
+            else:
+                g.jam_vrms_batch(*da)
+        n = 3
+        for _ in range(2):
+            step()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            step()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / n
+        g.set_overlap(False)
+        step()
+        torch.cuda.synchronize()
+        g.profile_enable(True); g.profile_read()
+        for _ in range(n):
+            step()
+        prof = g.profile_read(); g.profile_enable(False)
+        row = {"batch": B, "ms_per_step": ms, "evals_per_s": B / (ms * 1e-3),
+               "kernel_ms": {k: round(v[0] / n, 4) for k, v in prof.items() if v[1]}}
+        if D:
+            nx, ny = D["kin"]["xs"].size, D["kin"]["ys"].size
+            nxf, nyf = (nx + 1) // 2, (ny + 1) // 2
+            terms = float(workload_terms(wl).sum())
+            q = prof["jam_quad"][0] / n
+            row["jam_quad"] = {"ms_per_launch": q, "xu_frac": terms * (nxf + nyf) / (q * 1e-3) / xu_peak,
+                               "fp32_equivalent_tflops": 2.0 * nxf * nyf * terms / (q * 1e-3) / 1e12,
+                               "fp32_equivalent_frac": 2.0 * nxf * nyf * terms / (q * 1e-3) / 1e12 / peak_tf}
+        if L:
+            ss, kp, npx = L["grid"]["supersample"], L["psf"].shape[0], L["grid"]["nx"] * L["grid"]["ny"]
+            alg = B * (npx * ss * ss * 235.0 + npx * 2.0 * kp * kp)
+            li = prof["lens_image"][0] / n
+            row["lens_image"] = {"ms_per_launch": li, "algorithmic_tflops": alg / (li * 1e-3) / 1e12, "frac_algorithmic": alg / (li * 1e-3) / 1e12 / peak_tf}
+        rows[name] = row
+        g.close()
+        del g
+        torch.cuda.empty_cache()
+    return rows
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import workloads
@@ -255,6 +397,10 @@ def run_ours(args, rank, world, local_rank):
     L, D = wl["lens"], wl["dyn"]
     B = wl["B"]
     g = Glad(local_rank)
+    if args.jam_path == "simt":
+        g.set_jam_options(path="simt")
+    if args.no_overlap:
+        g.set_overlap(False)
     g.set_image_data(L["grid"], L["psf"], L["data"], L["ivar"])
     g.set_kin_data(D["kin"])
     dev = torch.device("cuda", local_rank)
@@ -297,7 +443,7 @@ def run_ours(args, rank, world, local_rank):
     ms = float(sum(e0.elapsed_time(e1) for e0, e1 in evs))
     # Per-kernel durations for the roofline: the same K steps again on ONE stream (glad_set_overlap(0)), because with the
     # lens half on the side stream an event pair around lens_image also times its wait for SMs held by jam_quad.
-    overlapped = os.environ.get("GLAD_OVERLAP", "1") != "0"
+    overlapped = not args.no_overlap
     if overlapped:
         g.set_overlap(False)
         step()
@@ -413,6 +559,81 @@ def run_ours(args, rank, world, local_rank):
             "cholesky": {"kernel": "pixsrc_chol_kernel", "ms_per_launch": chol_ms, "fp64_gflops": chol_flops / (chol_ms * 1e-3) / 1e9},
             "paper_context": "extended-image step, one vector, 64 x 64 source grid, N_d ~ 1e4: 0.21 s on one A100 in fp64, 2 s with GLEE on one CPU core (Table 2 P:453-458); other hardware, context only"}
 
+    if rank == 0:
+        # JAM_sph, the paper's own dynamics, on the same dynamics inputs with the paper's mesh (P:358-362:
+        # 16 x 16 rectangles of 7 x 7 Kronrod nodes; 20 x 10 polar points)
+        sph = workloads.jam_sph_rules(D["kin"], sigma_max=float(D["lum_mge"][..., 1].max()))
+        g.set_jam_sph_rules(sph)
+        sargs = (d["dyn"], d["lum"], d["mass"], d["beta"])
+        for _ in range(2):
+            g.jam_sph_vrms_batch(*sargs)
+        torch.cuda.synchronize()
+        g.profile_enable(True); g.profile_read()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s_steps = 3
+        s0.record()
+        for _ in range(s_steps):
+            g.jam_sph_vrms_batch(*sargs)
+        s1.record()
+        torch.cuda.synchronize()
+        sp = g.profile_read(); g.profile_enable(False)
+        s_ms = s0.elapsed_time(s1) / s_steps
+        i_ms = sp["jam_sph"][0] / s_steps
+        npol, nt_, nu_ = sph["rgrid"].size * sph["thgrid"].size, sph["tau"].size, sph["un"].size
+        nmj = D["mass_mge"].shape[-2] + (D["params"][:, 2] > 0).astype(np.int64)
+        nlj = D["lum_mge"].shape[-2]
+        groups = 1 if D["beta"].ndim == 1 else nlj
+        ex2 = float(np.sum(groups * npol * nt_ * (nmj * nu_ + nlj) + npol * (nmj * nu_ + nlj)))
+        xu_peak = torch.cuda.get_device_properties(dev).multi_processor_count * 16 * float(clocks.get("sm_max_mhz") or 1965.0) * 1e6
+        model["jam_sph_entry"] = {
+            "api": "glad_jam_sph_vrms_batch", "value": B / (s_ms * 1e-3), "unit": "dynamics evals/s", "ms_per_step": s_ms,
+            "kernel_ms": {k: sp[k][0] / s_steps for k in ("jam_prep", "jam_sph", "jam_sph_los", "jam_post")},
+            "sizes": f"{npol} polar points x {nt_} x {nu_} quadrature nodes, {nlj} luminous x {D['mass_mge'].shape[-2]}(+BH) mass Gaussians, one beta_ani per vector",
+            "roofline": {"bound": "alu", "kernel": "jam_sph_intr_kernel", "unit": "Gex2/s", "achieved": ex2 / (i_ms * 1e-3) / 1e9, "peak": xu_peak / 1e9,
+                         "frac": ex2 / (i_ms * 1e-3) / xu_peak, "ms_per_launch": i_ms, "algorithmic_ex2_per_launch": ex2,
+                         "peak_source": "148 SM x 16 MUFU lanes/clk x sm_max MHz (XU pipe): one ex2 per (polar point, radial node, mass Gaussian, u node) "
+                                        "+ one per luminous Gaussian -- the product form that one beta_ani allows (DESIGN.md)"},
+            "paper_context": "intrinsic moments at > 200 polar points, 42 x 95 Gaussians, ONE parameter vector: 0.32 s on one A100 in fp64, 13 s with JamPy on a CPU "
+                             "(Table 2 P:456-461); other hardware and table sizes, context only"}
+
+    configs = None
+    if rank == 0 and world == 1 and not args.no_configs:
+        configs = run_configs(args, local_rank, peak_tf_of(dev, clocks), clocks)
+
+    # Strong scaling of the lens-only large batch (BASELINE.json configs[3], 8192 vectors): ONE batch cut into contiguous chunks by
+    # paper_2504_01302_b200.sharding, each rank evaluates its chunk, one all-gather of lnL (32 KB) -- the only exchange a sampler needs
+    strong = None
+    if not args.no_configs:
+        from paper_2504_01302_b200.sharding import gather_loglike, shard_range
+        w4 = workloads.make_workload("C4", gpu_data_model(local_rank))
+        lo, hi = shard_range(w4["B"], rank, world)
+        g4 = Glad(local_rank)
+        g4.set_image_data(w4["lens"]["grid"], w4["lens"]["psf"], w4["lens"]["data"], w4["lens"]["ivar"])
+        p4 = t(w4["lens"]["params"][lo:hi]).to(dev)
+
+        def strong_step():
+            c2 = g4.lens_image_batch(p4, want_images=False)["chi2"]
+            return gather_loglike(-0.5 * c2, w4["B"], rank, world, dist)
+        for _ in range(2):
+            full = strong_step()
+        barrier()
+        q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        q0.record()
+        for _ in range(3):
+            full = strong_step()
+        q1.record()
+        barrier()
+        q_ms4 = q0.elapsed_time(q1) / 3
+        if dist is not None:
+            tq = torch.tensor([q_ms4], device=dev, dtype=torch.float64)
+            dist.all_reduce(tq, op=dist.ReduceOp.MAX)
+            q_ms4 = float(tq[0])
+        strong = {"workload": "C4 (BASELINE.json configs[3]): ONE batch of 8192 lens-only vectors", "scaling": "strong", "n_gpus": world,
+                  "vectors_per_rank": hi - lo, "ms_per_step": q_ms4, "value": w4["B"] / (q_ms4 * 1e-3), "unit": "lens-only lnL evals/s",
+                  "collective": "one all_gather of 8192 floats per step (sharding.gather_loglike)" if world > 1 else "none at N = 1",
+                  "gathered_finite": int(torch.isfinite(full).sum().item())}
+        g4.close()
+
     if dist is not None:
         tt = torch.tensor([ms, e2e_ms], device=dev, dtype=torch.float64)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
@@ -438,10 +659,12 @@ def run_ours(args, rank, world, local_rank):
     q_avg = q_ms / max(q_n, 1)
     achieved = flops_per_launch / (q_avg * 1e-3) / 1e12 if q_n else None
     shares = {k: round(v[0] / ms_serial, 4) for k, v in prof.items() if v[1]}
-    simt = os.environ.get("GLAD_JAM_PATH", "") == "simt"
+    simt = args.jam_path == "simt"
+    cap_q = load_capture("jam_quad_simt" if simt else "jam_quad_tc")
+    traffic = (cap_q["metrics"].get("dram__bytes_read.sum", 0.0) + cap_q["metrics"].get("dram__bytes_write.sum", 0.0)) if cap_q["fresh"] else None
     roofline = {"bound": "alu", "kernel": "jam_quad_kernel" if simt else "jam_quad_tc_kernel", "achieved": achieved,
                 "peak": peak_tf, "unit": "TFLOP/s", "frac": (achieved / peak_tf) if achieved else None,
-                "traffic": RESIDENT_TRAFFIC.get("jam_quad_simt" if simt else "jam_quad_tc"),
+                "traffic": traffic, "traffic_source": cap_q["note"],
                 "peak_source": f"{props.multi_processor_count} SM x 128 FP32 lanes x 2 flop x {sm_max:.0f} MHz (DESIGN.md); "
                                "'achieved' counts the contraction's algorithmic fp32 flops (2 per folded pixel and "
                                "contraction row), the quantity BASELINE.json's '% FP32 peak per stage' is quoted on",
@@ -477,28 +700,53 @@ def run_ours(args, rank, world, local_rank):
 
     # BASELINE.json's metric asks for the % of FP32 peak per stage: the lensing stage (ray-shoot + bin-down + PSF + chi2)
     l_ms, l_n = prof["lens_image"]
-    if args.config in LENS_FP32_FLOPS_PER_VECTOR and l_n:
-        lf = LENS_FP32_FLOPS_PER_VECTOR[args.config] * B
+    if l_n:
+        cap_l = load_capture("lens_image")
+        m = cap_l["metrics"]
         l_avg = l_ms / l_n
-        roofline["lens_image"] = {"bound": "alu", "kernel": "lens_image_kernel", "unit": "TFLOP/s",
-                                  "achieved": lf / (l_avg * 1e-3) / 1e12, "peak": peak_tf,
-                                  "frac": lf / (l_avg * 1e-3) / 1e12 / peak_tf, "ms_per_launch": l_avg,
-                                  "flops_per_launch": lf, "flops_source": "executed FP32 flops counted by ncu (profiles/r1b.md)"}
+        ss, kp = L["grid"]["supersample"], L["psf"].shape[0]
+        npx_img = L["grid"]["nx"] * L["grid"]["ny"]
+        alg = B * (npx_img * ss * ss * 235.0 + npx_img * 2.0 * kp * kp)      # ~235 flop per ray + 2 K^2 per pixel
+        roofline["lens_image"] = {"bound": "alu", "kernel": "lens_image_kernel", "unit": "TFLOP/s", "peak": peak_tf, "ms_per_launch": l_avg,
+                                  "algorithmic_flops_per_launch": alg, "achieved_algorithmic": alg / (l_avg * 1e-3) / 1e12,
+                                  "frac_algorithmic": alg / (l_avg * 1e-3) / 1e12 / peak_tf}
+        k3 = ["smsp__sass_thread_inst_executed_op_%s_pred_on.sum" % o for o in ("ffma", "fmul", "fadd")]
+        if cap_l["fresh"] and args.config == "C2" and all(k in m for k in k3) and m.get("launch__grid_size") == B:
+            lf = 2.0 * m[k3[0]] + m[k3[1]] + m[k3[2]]
+            roofline["lens_image"].update({"flops_per_launch": lf, "achieved": lf / (l_avg * 1e-3) / 1e12, "frac": lf / (l_avg * 1e-3) / 1e12 / peak_tf,
+                                           "flops_source": "executed FP32 flops (FFMA = 2, FMUL = FADD = 1) counted by ncu: " + cap_l["note"]})
+        else:
+            roofline["lens_image"].update({"flops_per_launch": None, "achieved": None, "frac": None,
+                                           "flops_source": "no fresh ncu capture of the executed flops for this workload: " + cap_l["note"]})
+
+    # the same contraction with three bf16 terms per operand (24 mantissa bits): the price of the wider arithmetic, beside the default
+    if rank == 0 and not simt:
+        g.set_jam_options(terms=3)
+        jargs = (d["dyn"], d["lum"], d["mass"], d["beta"])
+        g.jam_vrms_batch(*jargs)
+        torch.cuda.synchronize()
+        g.profile_enable(True); g.profile_read()
+        for _ in range(3):
+            g.jam_vrms_batch(*jargs)
+        p3 = g.profile_read(); g.profile_enable(False)
+        g.set_jam_options(terms=2)
+        roofline["three_term_ms_per_launch"] = p3["jam_quad"][0] / max(p3["jam_quad"][1], 1)
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         import oracle
         oracle.build()
-        ns = args.ref_sample
+        ns = args.cpu_sample
         cwl = workloads.make_workload(args.config, oracle_data_model(), B=ns)
         t0 = time.perf_counter()
         oracle_joint(cwl)
         dt = time.perf_counter() - t0
-        cpu = {"value": ns / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-               "sample": f"{ns} seeded {args.config} vectors (element 0 = truth), one pass, OpenMP over the batch"}
+        cpu = {"value": ns / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "cpu_model": cpu_model(), "nproc": os.cpu_count(),
+               "seconds": dt, "sample": f"{ns} seeded {args.config} vectors (element 0 = truth), one pass, OpenMP over the batch"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32 (fp64-prepared per-vector constants; row a6 contraction on 2-term split-bf16 tensor-core operands, fp32 accumulate)" if not simt else "f32",
             "data": "synthetic",
             "config": {"workload": f"{args.config} (BASELINE.json configs[1], RXJ1131-shaped joint model)", "batch_per_gpu": B,
                        "image": f"{L['grid']['nx']}x{L['grid']['ny']} s={L['grid']['supersample']} psf={L['psf'].shape[0]}",
@@ -509,7 +757,7 @@ def run_ours(args, rank, world, local_rank):
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": B * 4,
                     "steps": e2e_steps, "api": "glad_joint_loglike_host (pinned host buffers)"},
-            "roofline": roofline, "cpu_baseline": cpu, "model_entry": model}
+            "roofline": roofline, "cpu_baseline": cpu, "model_entry": model, "configs": configs, "strong_scaling_entry": strong}
     print(json.dumps(line), flush=True)
     g.close()
     if dist is not None:
@@ -524,11 +772,23 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2")
     ap.add_argument("--batch", type=int, default=None, help="override the per-GPU batch (default: the config's)")
-    ap.add_argument("--ref-sample", type=int, default=16, help="vectors per oracle pass (cpu_baseline / reference)")
+    ap.add_argument("--ref-sample", type=int, default=16, help="vectors per oracle step of --impl reference (K steps must end within minutes)")
+    ap.add_argument("--cpu-sample", type=int, default=64, help="vectors of the one oracle pass behind cpu_baseline (SURVEY 8(d): 64 for C2)")
+    ap.add_argument("--jam-path", default="auto", choices=["auto", "simt"], help="row a6 kernel: tcgen05 where it fits (default) or the FP32 SIMT form")
+    ap.add_argument("--no-overlap", action="store_true", help="keep both halves on one stream (glad_set_overlap(0))")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config block (C1, C3 cells, C4, C5)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--pixsrc-sweep", action="store_true", help="pixelated-source evidence over source-grid resolutions (context)")
     ap.add_argument("--sweep", action="store_true", help="per-kernel times of every BASELINE.json config (context, not the bench line)")
+    ap.add_argument("--ncu-summary", default=None, help="an .ncu-rep to summarise into --out and register in profiles/current_capture.txt")
+    ap.add_argument("--capture-key", default="jam_quad_tc")
+    ap.add_argument("--capture-source", default="paper_2504_01302_b200/csrc/jam_quad_tc.cu")
+    ap.add_argument("--capture-row", type=int, default=0, help="which profiled launch of the report")
+    ap.add_argument("--out", default=None)
     args = ap.parse_args()
+    if args.ncu_summary:
+        ncu_summary(args)
+        return
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

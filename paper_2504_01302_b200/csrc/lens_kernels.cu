@@ -123,7 +123,9 @@ __device__ __forceinline__ float light_eval(int kinds, int k, const float* __res
 }
 
 // One ray: returns source(beta) + lens light(theta).
-template <bool CH>
+// LONG = the vector needs more series terms than the stored table holds (q < 0.2): a separate instantiation, so that the
+// code of the common case is exactly the table-driven loop
+template <bool CH, bool LONG>
 __device__ __forceinline__ float shoot(const float* __restrict__ c, float thx, float thy, int nterms,
                                        bool has_src, bool has_l1, bool has_l2, int kinds) {
     float dx = thx - c[LC_XL], dy = thy - c[LC_YL];
@@ -137,7 +139,7 @@ __device__ __forceinline__ float shoot(const float* __restrict__ c, float thx, f
     float zr = negf * (wr * wr - wi * wi), zi = negf * (2.f * wr * wi);
     // Horner: h_n = 1 + c_n z h_{n+1}, sum = h_1
     float hr = 1.f, hi = 0.f;
-    if (nterms > GLAD_EPL_MAX_TERMS) {
+    if (LONG) {
         // very flat mass (q < 0.2): the terms past the stored table take c_n = (2n - a)/(2n + a), a = 2 - t = 1 + 2 HEXP, on the fly
         const float a2t = fmaf(2.f, c[LC_HEXP], 1.f);
         for (int n = nterms; n > GLAD_EPL_MAX_TERMS; --n) {
@@ -193,8 +195,38 @@ static inline __host__ __device__ int lens_tap_pitch(int kpsf) { return (kpsf + 
 static inline __host__ __device__ int lens_halo_left(int kpsf) { return kpsf / 2 + LENS_TAPS; }
 static inline __host__ __device__ int lens_img_pitch(int nx, int kpsf) { return (nx + 2 * (kpsf / 2) + LENS_TAPS + LENS_STRIP - 1) | 1; }
 
+// rows a1-a3 for one vector: every sub-pixel ray, averaged into the binned image in shared memory
+template <bool CH, bool LONG>
+__device__ __forceinline__ void ray_pass(const float* __restrict__ c, const glad_image_grid& g, float* __restrict__ img, int pitch,
+                                         int HL, int nterms, int kinds) {
+    const int tid = threadIdx.x, nthr = blockDim.x, nx = g.nx, npx = g.nx * g.ny, ss = g.supersample;
+    const bool has_src = c[LC_SERSIC0 + 5] != 0.f;
+    const bool has_l1 = c[LC_SERSIC0 + LC_SERSIC_STRIDE + 5] != 0.f;
+    const bool has_l2 = c[LC_SERSIC0 + 2 * LC_SERSIC_STRIDE + 5] != 0.f;
+    const float inv_s = 1.f / (float)ss, inv_s2 = 1.f / (float)(ss * ss);
+    for (int p = tid; p < npx; p += nthr) {
+        int iy = p / nx, ix = p - iy * nx;
+        float acc = 0.f;
+        for (int sb = 0; sb < ss; ++sb) {
+            float thy = fmaf(g.pix, (float)iy + (((float)sb + 0.5f) * inv_s - 0.5f), g.y0);
+            for (int sa = 0; sa < ss; ++sa) {
+                float thx = fmaf(g.pix, (float)ix + (((float)sa + 0.5f) * inv_s - 0.5f), g.x0);
+                acc += shoot<CH, LONG>(c, thx, thy, nterms, has_src, has_l1, has_l2, kinds);
+            }
+        }
+        img[iy * pitch + HL + ix] = acc * inv_s2;
+    }
+}
+
+// out of line: the rare long-series loop must not raise the register count of the kernel (2 CTAs of 512 threads per SM)
 template <bool CH>
-__global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict__ consts, int kinds, glad_image_grid g,
+__device__ __noinline__ void ray_pass_long(const float* __restrict__ c, const glad_image_grid& g, float* __restrict__ img, int pitch,
+                                           int HL, int nterms, int kinds) {
+    ray_pass<CH, true>(c, g, img, pitch, HL, nterms, kinds);
+}
+
+template <bool CH>
+__global__ void __launch_bounds__(512, 2) lens_image_kernel(const float* __restrict__ consts, int kinds, glad_image_grid g,
                                                          const float* __restrict__ psf, int kpsf,
                                                          const float* __restrict__ data,
                                                          const float* __restrict__ ivar, float* __restrict__ images,
@@ -225,24 +257,10 @@ __global__ void __launch_bounds__(512) lens_image_kernel(const float* __restrict
         return;
     }
     const int nterms = (int)c[LC_NTERMS];
-    const bool has_src = c[LC_SERSIC0 + 5] != 0.f;
-    const bool has_l1 = c[LC_SERSIC0 + LC_SERSIC_STRIDE + 5] != 0.f;
-    const bool has_l2 = c[LC_SERSIC0 + 2 * LC_SERSIC_STRIDE + 5] != 0.f;
-    const float inv_s = 1.f / (float)ss, inv_s2 = 1.f / (float)(ss * ss);
 
     // rows a1-a3: rays -> binned pixel in shared memory
-    for (int p = tid; p < npx; p += nthr) {
-        int iy = p / nx, ix = p - iy * nx;
-        float acc = 0.f;
-        for (int sb = 0; sb < ss; ++sb) {
-            float thy = fmaf(g.pix, (float)iy + (((float)sb + 0.5f) * inv_s - 0.5f), g.y0);
-            for (int sa = 0; sa < ss; ++sa) {
-                float thx = fmaf(g.pix, (float)ix + (((float)sa + 0.5f) * inv_s - 0.5f), g.x0);
-                acc += shoot<CH>(c, thx, thy, nterms, has_src, has_l1, has_l2, kinds);
-            }
-        }
-        img[iy * pitch + HL + ix] = acc * inv_s2;
-    }
+    if (nterms > GLAD_EPL_MAX_TERMS) ray_pass_long<CH>(c, g, img, pitch, HL, nterms, kinds);        // CTA-uniform: one vector per CTA
+    else ray_pass<CH, false>(c, g, img, pitch, HL, nterms, kinds);
     __syncthreads();
 
     // row a4: PSF convolution from shared memory + chi2.  out[x] = sum_dy sum_dx psf[dy][dx] img[y+cc-dy][x+cc-dx]
