@@ -99,6 +99,16 @@ def lib():
         L.glad_oracle_tdelay_const.restype = d
         L.glad_oracle_quasar_batch.restype = i
         L.glad_oracle_quasar_batch.argtypes = [fp, fp, i, i, dp, dp, i, dp, dp, dp, dp, dp, dp, dp, dp]
+        L.glad_oracle_set_cse_table.restype = i
+        L.glad_oracle_set_cse_table.argtypes = [i, dp, dp]
+        L.glad_oracle_nfw_kappa.restype = d
+        L.glad_oracle_nfw_kappa.argtypes = [d]
+        L.glad_oracle_enfw.restype = None
+        L.glad_oracle_enfw.argtypes = [dp, d, d, dp, dp, dp, dp, dp]
+        L.glad_oracle_lens_image_batch_halo.restype = i
+        L.glad_oracle_lens_image_batch_halo.argtypes = [fp, i, i, i, i, d, d, d, fp, i, fp, fp, ip, fp, d, d, fp, dp, dp, ip]
+        L.glad_oracle_quasar_batch_halo.restype = i
+        L.glad_oracle_quasar_batch_halo.argtypes = [fp, fp, fp, d, d, fp, i, i, dp, dp, i, dp, dp, dp, dp, dp, dp, dp, dp]
         L.glad_oracle_jam_sph_intrinsic.restype = None
         L.glad_oracle_jam_sph_intrinsic.argtypes = [d, d, i, dp, dp, dp, dp, i, dp, dp, dp, d, i, dp, dp, i, dp, dp, dp]
         L.glad_oracle_jam_sph_los.restype = d
@@ -156,7 +166,7 @@ def chameleon(dx, dy, I0, wc, wt, q, phi) -> float:
     return float(lib().glad_oracle_chameleon(dx, dy, I0, wc, wt, q, phi))
 
 
-def lens_image_batch(lens, grid, psf, data=None, ivar=None, want_images=True, kinds=None, lam=None, sheet=None):
+def lens_image_batch(lens, grid, psf, data=None, ivar=None, want_images=True, kinds=None, lam=None, sheet=None, enfw=None):
     """grid = dict(nx, ny, supersample, pix, x0, y0). kinds = None (all Sersic) or 3 ints (source, lens light 1, 2):
     0 Sersic, 1 Chameleon (slot = {I_0, w_c, w_t, q, phi}). lam [B] + sheet = (r_core, r_tr): internal mass sheet.
     Returns dict(images, chi2, flags)."""
@@ -173,10 +183,12 @@ def lens_image_batch(lens, grid, psf, data=None, ivar=None, want_images=True, ki
     lm = None if lam is None else _f32(lam).reshape(-1)
     assert lm is None or (lm.size == B and sheet is not None)
     src, srt = sheet if (sheet is not None and lm is not None) else (0.0, 0.0)
-    rc = lib().glad_oracle_lens_image_batch_sheet(
+    nf = None if enfw is None else _f32(enfw).reshape(B, 4)          # eNFW halo {rho_s, r_s, q, phi} per vector (set_cse_table first)
+    rc = lib().glad_oracle_lens_image_batch_halo(
         _ptr(lens, C.c_float), B, nx, ny, int(grid["supersample"]), float(grid["pix"]), float(grid["x0"]),
         float(grid["y0"]), _ptr(psf, C.c_float), k, _ptr(data, C.c_float), _ptr(ivar, C.c_float), _ptr(kk, C.c_int32),
-        _ptr(lm, C.c_float), float(src), float(srt), _ptr(images, C.c_double), _ptr(chi2, C.c_double), _ptr(flags, C.c_int32))
+        _ptr(lm, C.c_float), float(src), float(srt), _ptr(nf, C.c_float), _ptr(images, C.c_double), _ptr(chi2, C.c_double),
+        _ptr(flags, C.c_int32))
     if rc != 0:
         raise ValueError("oracle: bad lens arguments")
     return {"images": images, "chi2": chi2, "flags": flags}
@@ -347,7 +359,7 @@ def tdelay_const() -> float:
     return float(lib().glad_oracle_tdelay_const())
 
 
-def quasar_batch(lens, ddt, qso, lam=None, sheet=None):
+def quasar_batch(lens, ddt, qso, lam=None, sheet=None, enfw=None):
     """qso = dict(theta [n_img,2], sigma_theta [n_img], ref, dt_obs [n_img], sigma_dt [n_img]) (float64).
     lam [B] + sheet = (r_core, r_tr): internal mass sheet.
     Returns dict(chi2_img, chi2_tmd [B]; theta_pre [B,n_img,2]; dt_pre [B,n_img]; beta [B,2]; last_step [B,n_img])."""
@@ -365,8 +377,9 @@ def quasar_batch(lens, ddt, qso, lam=None, sheet=None):
     lm = None if lam is None else _f32(lam).reshape(-1)
     assert lm is None or (lm.size == B and sheet is not None)
     src, srt = sheet if (sheet is not None and lm is not None) else (0.0, 0.0)
-    rc = lib().glad_oracle_quasar_batch_sheet(_ptr(lens, C.c_float), _ptr(ddt, C.c_float), _ptr(lm, C.c_float), float(src),
-                                              float(srt), B, n, P(th), P(st), int(qso["ref"]), P(dt), P(sd),
+    nf = None if enfw is None else _f32(enfw).reshape(B, 4)
+    rc = lib().glad_oracle_quasar_batch_halo(_ptr(lens, C.c_float), _ptr(ddt, C.c_float), _ptr(lm, C.c_float), float(src),
+                                              float(srt), _ptr(nf, C.c_float), B, n, P(th), P(st), int(qso["ref"]), P(dt), P(sd),
                                               P(out["chi2_img"]), P(out["chi2_tmd"]), P(out["theta_pre"]),
                                               P(out["dt_pre"]), P(out["beta"]), P(out["last_step"]))
     if rc != 0:
@@ -436,3 +449,28 @@ def jam_sph_vrms_batch(dyn, lum_mge, mass_mge, beta, kin, sph, want_maps=False):
     if want_maps:
         out["v2map"], out["moments"] = v2map, mom
     return out
+
+
+# ------------------------------------------------------------------------------------------------
+# eNFW halo through core-steep ellipsoids (mass part; Appendix A)
+# ------------------------------------------------------------------------------------------------
+def set_cse_table(A, s):
+    """The (A_i, s_i) table of Eq. A.3 -- an input of the method (workloads.cse_table()); also used by MGE profile kind 3."""
+    A, s = np.ascontiguousarray(A, dtype=np.float64), np.ascontiguousarray(s, dtype=np.float64)
+    assert A.size == s.size
+    if lib().glad_oracle_set_cse_table(int(A.size), _ptr(A, C.c_double), _ptr(s, C.c_double)) != 0:
+        raise ValueError("oracle: CSE table too long")
+
+
+def nfw_kappa(u) -> float:
+    """Eq. A.1 with rho_s = 1."""
+    return float(lib().glad_oracle_nfw_kappa(float(u)))
+
+
+def enfw(nf, dx, dy):
+    """dict(kappa, ax, ay, h [3] = (xx, xy, yy), psi) of the halo nf = {rho_s, r_s, q, phi} at offset (dx, dy) from its centre."""
+    nf = np.ascontiguousarray(nf, dtype=np.float64)
+    k, ax, ay, ps = C.c_double(), C.c_double(), C.c_double(), C.c_double()
+    h = np.empty(3)
+    lib().glad_oracle_enfw(_ptr(nf, C.c_double), float(dx), float(dy), C.byref(k), C.byref(ax), C.byref(ay), _ptr(h, C.c_double), C.byref(ps))
+    return {"kappa": k.value, "ax": ax.value, "ay": ay.value, "h": h, "psi": ps.value}

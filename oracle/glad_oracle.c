@@ -190,12 +190,97 @@ double glad_oracle_sheet_kappa(double lam, double rc, double rt, double dx, doub
     return k;
 }
 
+/* ------------------------------------------------------------------------ */
+/* SURVEY.md 8(f) rank 4, mass part: elliptical NFW halo through core-steep    */
+/* ellipsoids (Appendix A, Eq. A.1-A.7).                            */
+/*   kappa_enfw(x,y) = rho_s sum_i A_i kappa_CSE(u; s_i)              (Eq. A.3) */
+/*   kappa_CSE(u; s) = 1 / (2 (s^2 + u^2)^(3/2))                      (Eq. A.4) */
+/*   u^2 = X^2 + Y^2/q^2, (X, Y) = (sqrt(q)/r_s) (x, y) in the halo frame (A.2) */
+/*   psi_CSE(X,Y) = q/(2s) ln Psi - q/s ln[(1+q) s]                   (Eq. A.6) */
+/*   Psi = (psi_s + s)^2 + (1-q^2) X^2, psi_s = sqrt(q^2 (s^2 + X^2) + Y^2)     */
+/*   (Psi: Oguri 2021, not printed in the paper; pinned here by Poisson's       */
+/*   equation, Eq. 7: Laplacian psi_CSE = 2 kappa_CSE by finite differences).   */
+/* Amplitudes follow from Eq. 7 and the scaling of Eq. A.2 (reading R-N2: the   */
+/* prefactor printed in Eq. A.7 is not consistent with Eq. A.3 by one power of  */
+/* r_s): psi = (rho_s r_s^2 / q) sum A_i psi_CSE, alpha = (rho_s r_s/sqrt q)    */
+/* sum A_i grad psi_CSE, Hessian = rho_s sum A_i Hess psi_CSE.                  */
+/* The table (A_i, s_i) is an INPUT of the method ("predetermined";      */
+/* reading R-N1): set once with glad_oracle_set_cse_table.                      */
+/* Halo vector nf = {rho_s, r_s [arcsec], q, phi}; centre = lens centre;        */
+/* rho_s = 0 switches the halo off.                                             */
+/* ------------------------------------------------------------------------ */
+#define ORACLE_MAX_CSE 128
+static int g_ncse = 0;
+static double g_cse_A[ORACLE_MAX_CSE], g_cse_s[ORACLE_MAX_CSE];
+int glad_oracle_set_cse_table(int n, const double* A, const double* s) {
+    if (n < 0 || n > ORACLE_MAX_CSE) return -1;
+    g_ncse = n;
+    for (int i = 0; i < n; ++i) { g_cse_A[i] = A[i]; g_cse_s[i] = s[i]; }
+    return 0;
+}
+/* Eq. A.1 with rho_s = 1 */
+double glad_oracle_nfw_kappa(double u) {
+    if (u < 1.0) { double t = sqrt(1.0 - u * u); return 0.5 / (u * u - 1.0) * (1.0 - atanh(t) / t); }
+    if (u > 1.0) { double t = sqrt(u * u - 1.0); return 0.5 / (u * u - 1.0) * (1.0 - atan(t) / t); }
+    return 1.0 / 6.0;
+}
+/* kappa, alpha, Hessian (h[0..2] = xx, xy, yy) and psi of the halo at offset (dx, dy) from its centre, sky frame;
+ * any output may be NULL */
+void glad_oracle_enfw(const double* nf, double dx, double dy, double* kappa, double* ax, double* ay, double* h, double* psi) {
+    double rho = nf[0], rs = nf[1], q = nf[2], c = cos(nf[3]), s = sin(nf[3]);
+    double xh = dx * c + dy * s, yh = -dx * s + dy * c;          /* halo frame */
+    double sc = sqrt(q) / rs, X = sc * xh, Y = sc * yh;
+    double k = 0.0, aX = 0.0, aY = 0.0, hXX = 0.0, hXY = 0.0, hYY = 0.0, ps = 0.0;
+    for (int i = 0; i < g_ncse; ++i) {
+        double A = g_cse_A[i], si = g_cse_s[i];
+        double u2 = X * X + Y * Y / (q * q);
+        k += A * 0.5 / pow(si * si + u2, 1.5);
+        double pss = sqrt(q * q * (si * si + X * X) + Y * Y), a = pss + si;
+        double Psi = a * a + (1.0 - q * q) * X * X;
+        double sX = q * q * X / pss, sY = Y / pss;               /* d psi_s */
+        double sXX = q * q / pss - q * q * q * q * X * X / (pss * pss * pss), sYY = 1.0 / pss - Y * Y / (pss * pss * pss),
+               sXY = -q * q * X * Y / (pss * pss * pss);
+        double PX = 2.0 * a * sX + 2.0 * (1.0 - q * q) * X, PY = 2.0 * a * sY;
+        double PXX = 2.0 * sX * sX + 2.0 * a * sXX + 2.0 * (1.0 - q * q), PYY = 2.0 * sY * sY + 2.0 * a * sYY,
+               PXY = 2.0 * sX * sY + 2.0 * a * sXY;
+        double f = A * q / (2.0 * si);
+        aX += f * PX / Psi;
+        aY += f * PY / Psi;
+        hXX += f * (PXX / Psi - PX * PX / (Psi * Psi));
+        hYY += f * (PYY / Psi - PY * PY / (Psi * Psi));
+        hXY += f * (PXY / Psi - PX * PY / (Psi * Psi));
+        ps += A * (q / (2.0 * si) * log(Psi) - q / si * log((1.0 + q) * si));
+    }
+    double amp = rho * rs / sqrt(q);
+    if (kappa) *kappa = rho * k;
+    if (ax) *ax = amp * (aX * c - aY * s);
+    if (ay) *ay = amp * (aX * s + aY * c);
+    if (h) {
+        h[0] = rho * (c * c * hXX - 2.0 * c * s * hXY + s * s * hYY);
+        h[2] = rho * (s * s * hXX + 2.0 * c * s * hXY + c * c * hYY);
+        h[1] = rho * (c * s * (hXX - hYY) + (c * c - s * s) * hXY);
+    }
+    if (psi) *psi = rho * rs * rs / q * ps;
+}
+static int enfw_valid(const double* nf) {
+    if (!(nf[0] >= 0.0)) return 0;
+    if (nf[0] == 0.0) return 1;
+    return (nf[1] > 0.0) && (nf[2] > 0.0) && (nf[2] <= 1.0);
+}
+
 /* Total deflection at image-plane position (thx, thy): lam * EPL (rotated by phi_PA
  * about the lens centre) + external shear (Eq. 49, origin = lens centre,
  * reading R-L5) + point mass alpha = thE2 * D/|D|^2 (reading R-L6) + the mass
  * sheet (rc > 0; rc <= 0 = no sheet, lam must then be 1). */
+void glad_oracle_deflection_halo(const double* p, double lam, double rc, double rt, const double* nf, double thx, double thy,
+                                 double* ax, double* ay);
 void glad_oracle_deflection_sheet(const double* p, double lam, double rc, double rt, double thx, double thy,
                                   double* ax, double* ay) {
+    glad_oracle_deflection_halo(p, lam, rc, rt, NULL, thx, thy, ax, ay);
+}
+/* ... + the eNFW halo nf = {rho_s, r_s, q, phi} about the lens centre (NULL or rho_s = 0: none) */
+void glad_oracle_deflection_halo(const double* p, double lam, double rc, double rt, const double* nf, double thx, double thy,
+                                 double* ax, double* ay) {
     double dx = thx - p[0], dy = thy - p[1];
     double c = cos(p[5]), s = sin(p[5]);
     double xl = dx * c + dy * s, yl = -dx * s + dy * c;
@@ -214,6 +299,12 @@ void glad_oracle_deflection_sheet(const double* p, double lam, double rc, double
         sheet_terms(lam, rc, rt, dx, dy, &sx, &sy, NULL, NULL, NULL);
         a_x += sx;
         a_y += sy;
+    }
+    if (nf && nf[0] != 0.0) {
+        double hx, hy;
+        glad_oracle_enfw(nf, dx, dy, NULL, &hx, &hy, NULL, NULL);
+        a_x += hx;
+        a_y += hy;
     }
     *ax = a_x;
     *ay = a_y;
@@ -288,11 +379,25 @@ int glad_oracle_lens_image_batch_kinds(const float* lens, int B, int nx, int ny,
 }
 /* same, with the internal mass sheet: lambda [B] float32 (NULL = none), rt > rc > 0 arcsec (R-S1..3);
  * a non-finite lambda invalidates the vector */
+int glad_oracle_lens_image_batch_halo(const float* lens, int B, int nx, int ny, int s, double pix,
+                                      double x0, double y0, const float* psf, int kpsf,
+                                      const float* data, const float* ivar, const int* kinds,
+                                      const float* lambda, double rc, double rt, const float* enfw,
+                                      double* images, double* chi2, int32_t* flags);
 int glad_oracle_lens_image_batch_sheet(const float* lens, int B, int nx, int ny, int s, double pix,
                                        double x0, double y0, const float* psf, int kpsf,
                                        const float* data, const float* ivar, const int* kinds,
                                        const float* lambda, double rc, double rt,
                                        double* images, double* chi2, int32_t* flags) {
+    return glad_oracle_lens_image_batch_halo(lens, B, nx, ny, s, pix, x0, y0, psf, kpsf, data, ivar, kinds, lambda, rc, rt, NULL,
+                                             images, chi2, flags);
+}
+/* same, with an eNFW halo per vector: enfw [B,4] float32 {rho_s, r_s, q, phi} or NULL (mass part) */
+int glad_oracle_lens_image_batch_halo(const float* lens, int B, int nx, int ny, int s, double pix,
+                                      double x0, double y0, const float* psf, int kpsf,
+                                      const float* data, const float* ivar, const int* kinds,
+                                      const float* lambda, double rc, double rt, const float* enfw,
+                                      double* images, double* chi2, int32_t* flags) {
     if (lambda && !(rc > 0.0 && rt > rc)) return -1;
     if (B < 0 || nx <= 0 || ny <= 0 || s <= 0 || kpsf <= 0 || (kpsf % 2) == 0) return -1;
     if (kinds) for (int c = 0; c < 3; ++c) if (kinds[c] != 0 && kinds[c] != 1) return -1;
@@ -304,7 +409,10 @@ int glad_oracle_lens_image_batch_sheet(const float* lens, int B, int nx, int ny,
         for (int i = 0; i < ORACLE_NLENS; ++i) p[i] = (double)lens[(size_t)b * ORACLE_NLENS + i];
         if (flags) flags[b] = 0;
         const double lam = lambda ? (double)lambda[b] : 1.0, src = lambda ? rc : 0.0;
-        if (!lens_params_valid_kinds(p, kinds) || !isfinite(lam)) {
+        double nfv[4] = {0.0, 1.0, 1.0, 0.0};
+        if (enfw) for (int i = 0; i < 4; ++i) nfv[i] = (double)enfw[(size_t)b * 4 + i];
+        const double* nf = enfw ? nfv : NULL;
+        if (!lens_params_valid_kinds(p, kinds) || !isfinite(lam) || !enfw_valid(nfv)) {
             if (flags) flags[b] |= FLAG_LENS_INVALID;
             if (images) for (int i = 0; i < npx; ++i) images[(size_t)b * npx + i] = NAN;
             if (chi2) chi2[b] = INFINITY;
@@ -323,7 +431,7 @@ int glad_oracle_lens_image_batch_sheet(const float* lens, int B, int nx, int ny,
                         double thx = x0 + ix * pix + ((sa + 0.5) / s - 0.5) * pix;
                         double thy = y0 + iy * pix + ((sb + 0.5) / s - 0.5) * pix;
                         double ax, ay;
-                        glad_oracle_deflection_sheet(p, lam, src, rt, thx, thy, &ax, &ay);
+                        glad_oracle_deflection_halo(p, lam, src, rt, nf, thx, thy, &ax, &ay);
                         double bx = thx - ax, by = thy - ay; /* beta = theta - alpha */
                         double v = 0.0;
                         if (p[11] != 0.0)
@@ -613,7 +721,11 @@ double glad_oracle_potential(const double* p, double thx, double thy) {
     return glad_oracle_potential_sheet(p, 1.0, 0.0, 0.0, thx, thy);
 }
 /* with the internal mass sheet: lam psi_epl + psi_sheet (+ shear, point mass), Eq. 8 with the dPIE sheet */
+double glad_oracle_potential_halo(const double* p, double lam, double rc, double rt, const double* nf, double thx, double thy);
 double glad_oracle_potential_sheet(const double* p, double lam, double rc, double rt, double thx, double thy) {
+    return glad_oracle_potential_halo(p, lam, rc, rt, NULL, thx, thy);
+}
+double glad_oracle_potential_halo(const double* p, double lam, double rc, double rt, const double* nf, double thx, double thy) {
     double dx = thx - p[0], dy = thy - p[1];
     double c = cos(p[5]), s = sin(p[5]);
     double xl = dx * c + dy * s, yl = -dx * s + dy * c;
@@ -630,6 +742,11 @@ double glad_oracle_potential_sheet(const double* p, double lam, double rc, doubl
         sheet_terms(lam, rc, rt, dx, dy, NULL, NULL, NULL, &ps, NULL);
         psi += ps;
     }
+    if (nf && nf[0] != 0.0) {
+        double ph;
+        glad_oracle_enfw(nf, dx, dy, NULL, NULL, NULL, NULL, &ph);
+        psi += ph;
+    }
     return psi;
 }
 
@@ -638,7 +755,11 @@ void glad_oracle_hessian_sheet(const double* p, double lam, double rc, double rt
 void glad_oracle_hessian(const double* p, double thx, double thy, double* h) {
     glad_oracle_hessian_sheet(p, 1.0, 0.0, 0.0, thx, thy, h);
 }
+void glad_oracle_hessian_halo(const double* p, double lam, double rc, double rt, const double* nf, double thx, double thy, double* h);
 void glad_oracle_hessian_sheet(const double* p, double lam, double rc, double rt, double thx, double thy, double* h) {
+    glad_oracle_hessian_halo(p, lam, rc, rt, NULL, thx, thy, h);
+}
+void glad_oracle_hessian_halo(const double* p, double lam, double rc, double rt, const double* nf, double thx, double thy, double* h) {
     double dx = thx - p[0], dy = thy - p[1];
     double c = cos(p[5]), s = sin(p[5]);
     double xl = dx * c + dy * s, yl = -dx * s + dy * c;
@@ -665,6 +786,11 @@ void glad_oracle_hessian_sheet(const double* p, double lam, double rc, double rt
         double hs[3];
         sheet_terms(lam, rc, rt, dx, dy, NULL, NULL, hs, NULL, NULL);
         hxx += hs[0]; hxy += hs[1]; hyy += hs[2];
+    }
+    if (nf && nf[0] != 0.0) {
+        double hh[3];
+        glad_oracle_enfw(nf, dx, dy, NULL, NULL, NULL, hh, NULL);
+        hxx += hh[0]; hxy += hh[1]; hyy += hh[2];
     }
     double c2 = cos(2.0 * p[7]), s2 = sin(2.0 * p[7]);
     hxx += p[6] * c2;
@@ -714,11 +840,23 @@ int glad_oracle_quasar_batch(const float* lens, const float* ddt, int B, int n_i
     return glad_oracle_quasar_batch_sheet(lens, ddt, NULL, 0.0, 0.0, B, n_img, theta_obs, sigma_theta, ref, dt_obs, sigma_dt,
                                           chi2_img, chi2_tmd, theta_pre, dt_pre, beta_bar, last_step);
 }
+int glad_oracle_quasar_batch_halo(const float* lens, const float* ddt, const float* lambda, double rc, double rt, const float* enfw,
+                                  int B, int n_img, const double* theta_obs, const double* sigma_theta, int ref,
+                                  const double* dt_obs, const double* sigma_dt, double* chi2_img, double* chi2_tmd,
+                                  double* theta_pre, double* dt_pre, double* beta_bar, double* last_step);
 /* same with the internal mass sheet (lambda [B] float32 or NULL; rt > rc > 0) in alpha, the Hessian and psi */
 int glad_oracle_quasar_batch_sheet(const float* lens, const float* ddt, const float* lambda, double rc, double rt, int B,
                                    int n_img, const double* theta_obs, const double* sigma_theta, int ref,
                                    const double* dt_obs, const double* sigma_dt, double* chi2_img, double* chi2_tmd,
                                    double* theta_pre, double* dt_pre, double* beta_bar, double* last_step) {
+    return glad_oracle_quasar_batch_halo(lens, ddt, lambda, rc, rt, NULL, B, n_img, theta_obs, sigma_theta, ref, dt_obs, sigma_dt,
+                                         chi2_img, chi2_tmd, theta_pre, dt_pre, beta_bar, last_step);
+}
+/* same with an eNFW halo per vector (enfw [B,4] float32 or NULL) */
+int glad_oracle_quasar_batch_halo(const float* lens, const float* ddt, const float* lambda, double rc, double rt, const float* enfw,
+                                  int B, int n_img, const double* theta_obs, const double* sigma_theta, int ref,
+                                  const double* dt_obs, const double* sigma_dt, double* chi2_img, double* chi2_tmd,
+                                  double* theta_pre, double* dt_pre, double* beta_bar, double* last_step) {
     if (lambda && !(rc > 0.0 && rt > rc)) return -1;
     if (n_img < 1 || n_img > ORACLE_MAX_QIMG || ref < 0 || ref >= n_img) return -1;
     const double K = glad_oracle_tdelay_const();
@@ -727,7 +865,11 @@ int glad_oracle_quasar_batch_sheet(const float* lens, const float* ddt, const fl
         double p[ORACLE_NLENS];
         for (int k = 0; k < ORACLE_NLENS; ++k) p[k] = (double)lens[(size_t)b * ORACLE_NLENS + k];
         const double lam = lambda ? (double)lambda[b] : 1.0, src = lambda ? rc : 0.0;
-        int ok = (p[2] >= 0.0) && (p[3] > 1.0) && (p[3] < 3.0) && (p[4] > 0.0) && (p[4] <= 1.0) && (p[8] >= 0.0) && isfinite(lam);
+        double nfv[4] = {0.0, 1.0, 1.0, 0.0};
+        if (enfw) for (int i = 0; i < 4; ++i) nfv[i] = (double)enfw[(size_t)b * 4 + i];
+        const double* nf = enfw ? nfv : NULL;
+        int ok = (p[2] >= 0.0) && (p[3] > 1.0) && (p[3] < 3.0) && (p[4] > 0.0) && (p[4] <= 1.0) && (p[8] >= 0.0) && isfinite(lam) &&
+                 enfw_valid(nfv);
         if (!ok) {
             if (chi2_img) chi2_img[b] = INFINITY;
             if (chi2_tmd) chi2_tmd[b] = INFINITY;
@@ -743,8 +885,8 @@ int glad_oracle_quasar_batch_sheet(const float* lens, const float* ddt, const fl
         double bx = 0.0, by = 0.0, wsum = 0.0;
         for (int i = 0; i < n_img; ++i) {
             double tx = theta_obs[2 * i], ty = theta_obs[2 * i + 1], ax, ay, h[3];
-            glad_oracle_deflection_sheet(p, lam, src, rt, tx, ty, &ax, &ay);
-            glad_oracle_hessian_sheet(p, lam, src, rt, tx, ty, h);
+            glad_oracle_deflection_halo(p, lam, src, rt, nf, tx, ty, &ax, &ay);
+            glad_oracle_hessian_halo(p, lam, src, rt, nf, tx, ty, h);
             double det = (1.0 - h[0]) * (1.0 - h[2]) - h[1] * h[1];
             double w = fabs(1.0 / det);
             bx += w * (tx - ax);
@@ -760,8 +902,8 @@ int glad_oracle_quasar_batch_sheet(const float* lens, const float* ddt, const fl
             double tx = theta_obs[2 * i], ty = theta_obs[2 * i + 1], step = 0.0;
             for (int it = 0; it < NEWTON_STEPS; ++it) {
                 double ax, ay, h[3];
-                glad_oracle_deflection_sheet(p, lam, src, rt, tx, ty, &ax, &ay);
-                glad_oracle_hessian_sheet(p, lam, src, rt, tx, ty, h);
+                glad_oracle_deflection_halo(p, lam, src, rt, nf, tx, ty, &ax, &ay);
+                glad_oracle_hessian_halo(p, lam, src, rt, nf, tx, ty, h);
                 double fx = tx - ax - bx, fy = ty - ay - by;          /* lens equation residual */
                 double a11 = 1.0 - h[0], a12 = -h[1], a22 = 1.0 - h[2];
                 double det = a11 * a22 - a12 * a12;
@@ -774,7 +916,7 @@ int glad_oracle_quasar_batch_sheet(const float* lens, const float* ddt, const fl
             if (last_step) last_step[(size_t)b * n_img + i] = step;
             double ex = theta_obs[2 * i] - tx, ey = theta_obs[2 * i + 1] - ty;
             c2i += (ex * ex + ey * ey) / (sigma_theta[i] * sigma_theta[i]);
-            phi[i] = 0.5 * ((tx - bx) * (tx - bx) + (ty - by) * (ty - by)) - glad_oracle_potential_sheet(p, lam, src, rt, tx, ty);
+            phi[i] = 0.5 * ((tx - bx) * (tx - bx) + (ty - by) * (ty - by)) - glad_oracle_potential_halo(p, lam, src, rt, nf, tx, ty);
         }
         double c2t = 0.0;
         for (int i = 0; i < n_img; ++i) {
@@ -835,6 +977,11 @@ static double complex mge_profile(int kind, const double* prof, double bn, doubl
         double complex w = cpow(z / prof[1], 1.0 / prof[2]);
         return prof[0] * cexp(-bn * (w - 1.0));
     }
+    if (kind == 3) {   /* eNFW through CSEs, Eq. A.2-A.4: prof = {scale, r_s, -, q}; F = scale sum A_i / (2 (s_i^2 + u^2)^(3/2)), u = z sqrt(q)/r_s */
+        double complex u2 = z * z * prof[3] / (prof[1] * prof[1]), acc = 0.0;
+        for (int i = 0; i < g_ncse; ++i) acc += g_cse_A[i] * 0.5 / cpow(g_cse_s[i] * g_cse_s[i] + u2, 1.5);
+        return prof[0] * acc;
+    }
     if (kind == 2) {   /* Chameleon, Eq. 47: prof = {I_0, w_c, w_t, q} */
         double opq = 1.0 + prof[3];
         double ac = 4.0 * prof[1] * prof[1] / (opq * opq), at = 4.0 * prof[2] * prof[2] / (opq * opq);
@@ -865,7 +1012,7 @@ double glad_oracle_mge_f_sigma(int kind, const double* prof, double sigma, int P
 
 int glad_oracle_mge1d(int kind, const double* prof, int n_gauss, double sigma_lo, double sigma_hi, int P,
                       double* mge /* [n_gauss,3] */) {
-    if ((kind != 0 && kind != 1 && kind != 2) || n_gauss < 2 || !(sigma_lo > 0.0) || !(sigma_hi > sigma_lo) || P < 1 || P > 20)
+    if ((kind != 0 && kind != 1 && kind != 2 && kind != 3) || n_gauss < 2 || !(sigma_lo > 0.0) || !(sigma_hi > sigma_lo) || P < 1 || P > 20)
         return -1;
     double dln = log(sigma_hi / sigma_lo) / (n_gauss - 1);
     for (int n = 0; n < n_gauss; ++n) {

@@ -10,4 +10,4 @@ These inputs stand in for the paper's simulated RXJ1131 HST-ACS image and
 NIRSpec-like kinematic map (section 4), which are not
 available; shapes/distributions follow BASELINE.json:configs first.
 """
-from .generate import CONFIGS, make_workload, gauss_legendre_u, quasar_data, subset, pixsrc_inputs, kronrod_composite, jam_sph_rules  # noqa: F401
+from .generate import CONFIGS, make_workload, gauss_legendre_u, quasar_data, subset, pixsrc_inputs, kronrod_composite, jam_sph_rules, cse_table, enfw_params  # noqa: F401

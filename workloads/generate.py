@@ -102,6 +102,22 @@ def jam_sph_rules(kin: dict, panels: int = 16, nr: int = 20, nth: int = 10, nz: 
                 tau=t.astype(f), wtau=w.astype(f), un=u.astype(f), uw=(L * u * w).astype(f), zeta=z.astype(f), wz=wz.astype(f))
 
 
+def cse_table():
+    """(A_i, s_i) of the CSE expansion of the NFW convergence (Eq. A.3-A.5): the table workloads/fit_cse_nfw.py wrote.  An input of
+    the method ("predetermined"): this repository's fit, not Oguri (2021)'s 44 pairs (not available, not printed)."""
+    import os
+    t = np.loadtxt(os.path.join(os.path.dirname(os.path.abspath(__file__)), "cse_nfw.txt"))
+    return t[:, 0].copy(), t[:, 1].copy()
+
+
+def enfw_params(B: int, seed: int = 11) -> np.ndarray:
+    """Per-vector halo {rho_s, r_s [arcsec], q, phi}: a dark-matter halo that carries roughly half the convergence at the Einstein
+    radius of the C2 truth (kappa_enfw(1.65") ~ 0.2-0.35), r_s ~ U(8, 20) arcsec (the RXJ1131 class), q ~ U(0.6, 1)."""
+    rng = np.random.default_rng(seed)
+    out = np.stack([rng.uniform(0.15, 0.3, B), rng.uniform(8.0, 20.0, B), rng.uniform(0.6, 1.0, B), rng.uniform(0.0, np.pi, B)], 1)
+    return out.astype(np.float32)
+
+
 def _psf(kind: str, k: int, pix: float, fwhm: float) -> np.ndarray:
     c = k // 2
     yy, xx = np.mgrid[0:k, 0:k]
