@@ -100,7 +100,7 @@ def test_rows_layout_weights_and_linearity():
     m2 = oracle.mge1d(oracle.PROFILE_SERSIC, [6.0, 1.2, 3.0, 0.7], 15, 0.05, 20.0)
     assert np.allclose(m2[:, 0], 3.0 * m[:, 0], rtol=1e-12)
     with pytest.raises(ValueError):
-        oracle.mge1d(3, prof, 15, 0.05, 20.0)
+        oracle.mge1d(4, prof, 15, 0.05, 20.0)          # kinds 0..3 exist (3 = eNFW through CSEs)
     with pytest.raises(ValueError):
         oracle.mge1d(0, prof, 15, 20.0, 0.05)
 
