@@ -301,13 +301,15 @@ def sigma_crit(Ddt_mpc, Dd_mpc, zd) -> float:
 
 
 def model_tables(lens, dyn, ddt, zd, n_lum, n_mass, lum_range, mass_range, P=MGE_EULER_P, tracer_kind=PROFILE_SERSIC,
-                 lam=None, sheet=None):
+                 lam=None, sheet=None, enfw=None, halo=None):
     """The self-consistent joint model of P:406 / Fig. 2 (reading R-M3): from the lens vector and the distances
     derive (a) the luminous MGE = Eq. 46 of lens-light component #1 (lens[16:20]; Sersic, or Chameleon with tracer_kind), (b) the mass MGE = Eq. 46 of
     Sigma_crit * kappa_epl (Eq. 13, B.1-B.3), (c) lens[8] = theta_E,BH^2 from M_BH = dyn[2] (Eq. 4).
     Returns (lens' [B,26] float32, lum [B,n_lum,3] float32, mass [B,n_mass,3] float32): tables rounded to the
     float32 the batch calls take.  lam [B] + sheet = dict(rc, rt, n, sigma_lo, sigma_hi): internal mass sheet; the mass
-    table then has n_mass + sheet["n"] rows (lam x the EPL rows, then the sheet's round Gaussians)."""
+    table then has n_mass + sheet["n"] rows (lam x the EPL rows, then the sheet's round Gaussians).  enfw [B,4] + halo =
+    dict(n, sigma_lo, sigma_hi): the eNFW halo's rows (Eq. 46 of Sigma_crit lam kappa_enfw, profile kind 3, q' = the halo's q)
+    come last (set_cse_table first); a halo with rho_s = 0 gives rows of zero amplitude."""
     lens = _f32(lens).reshape(-1, NLENS).copy()
     dyn = _f32(dyn).reshape(-1, NDYN)
     ddt = _f32(ddt).reshape(-1)
@@ -328,6 +330,12 @@ def model_tables(lens, dyn, ddt, zd, n_lum, n_mass, lum_range, mass_range, P=MGE
             sh = mge1d(PROFILE_CHAMELEON, [i0, rc, rt, 1.0], int(sheet["n"]), float(sheet["sigma_lo"]), float(sheet["sigma_hi"]), P=P)
             m[:, 0] *= lb
             m = np.concatenate([m, sh])
+        if enfw is not None:
+            nf = [float(np.float32(v)) for v in np.asarray(enfw)[b]]
+            lb = 1.0 if lam is None else float(np.float32(lam[b]))
+            hr = mge1d(3, [sc * nf[0], nf[1], 0.0, nf[2]], int(halo["n"]), float(halo["sigma_lo"]), float(halo["sigma_hi"]), P=P)
+            hr[:, 0] *= lb
+            m = np.concatenate([m, hr])
         if mass is None:
             mass = np.empty((B, m.shape[0], 3), np.float32)
         mass[b] = m

@@ -133,3 +133,23 @@ def test_mge_of_the_halo_sums_back_to_eq_a1(oracle, halo):
     for R in np.geomspace(0.1, 30.0, 25):
         got = float(np.sum(rows[:, 0] * np.exp(-R * R / (2 * rows[:, 1] ** 2))))
         assert got == pytest.approx(scale * kappa_a1(math.sqrt(q) * R / rs), rel=1e-2), R
+
+
+def test_model_tables_append_the_halo_rows(oracle, halo):
+    """Self-consistent joint model with the halo: the mass table = the EPL rows (unchanged) followed by Eq. 46 of
+    Sigma_crit kappa_enfw; summed back it gives Sigma_crit (kappa_epl + kappa_enfw) along the major axis within 2 %."""
+    wl = workloads.make_workload("C1")
+    L, D = wl["lens"], wl["dyn"]
+    nf = workloads.enfw_params(wl["B"])
+    a = oracle.model_tables(L["params"], D["params"], wl["ddt"], wl["z_d"], 8, 12, (0.05, 8.0), (0.02, 50.0))
+    b = oracle.model_tables(L["params"], D["params"], wl["ddt"], wl["z_d"], 8, 12, (0.05, 8.0), (0.02, 50.0), enfw=nf,
+                            halo=dict(n=20, sigma_lo=0.03, sigma_hi=400.0))
+    assert b[2].shape == (wl["B"], 32, 3) and np.array_equal(b[2][:, :12], a[2]) and np.array_equal(b[0], a[0])
+    for v in (0, 3):
+        sc = oracle.sigma_crit(float(wl["ddt"][v]), float(D["params"][v, 1]), wl["z_d"])
+        rows = b[2][v, 12:].astype(np.float64)
+        assert np.allclose(rows[:, 2], nf[v, 2])
+        for R in (0.3, 1.0, 4.0):
+            got = float(np.sum(rows[:, 0] * np.exp(-R * R / (2 * rows[:, 1] ** 2))))
+            want = sc * float(nf[v, 0]) * kappa_a1(math.sqrt(float(nf[v, 2])) * R / float(nf[v, 1]))
+            assert got == pytest.approx(want, rel=2e-2)
