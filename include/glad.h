@@ -193,11 +193,13 @@ glad_status glad_joint_loglike_host(glad_ctx* ctx, const float* h_lens_params, c
  *   GLAD_PROFILE_SERSIC : {I_e, R_e, n, q'}            F = I_e exp(-b_n ((R/R_e)^(1/n) - 1))        (R-L7)
  *   GLAD_PROFILE_EPL    : {scale, theta_E, gamma, q}   F = scale (3-gamma)/2 (b/R)^(gamma-1), b of Eq. B.3
  *   GLAD_PROFILE_CHAMELEON : {I_0, w_c, w_t, q'}       F of Eq. 47, the paper's I_light
+ *   GLAD_PROFILE_NFW_CSE   : {scale, r_s, -, q}        F = scale sum_i A_i / (2 (s_i^2 + u^2)^(3/2)), u = R sqrt(q)/r_s (Eq. A.2-A.4),
+ *                                                      the CSE table of glad_set_enfw (GLAD_ESTATE without it)
  * d_mge [B,n_gauss,3] rows {A_n, sigma_n, q'}: the MGE row layout glad_jam_vrms_batch reads (stride 3*n_gauss).
  * fp64 arithmetic, fp32 rows.  Enqueues on the context stream; device pointers owned by the caller.
  * GLAD_EINVAL on a bad kind / range / order, GLAD_ESHAPE if n_gauss > GLAD_MAX_GAUSS.
  */
-typedef enum { GLAD_PROFILE_SERSIC = 0, GLAD_PROFILE_EPL = 1, GLAD_PROFILE_CHAMELEON = 2 } glad_profile_kind;
+typedef enum { GLAD_PROFILE_SERSIC = 0, GLAD_PROFILE_EPL = 1, GLAD_PROFILE_CHAMELEON = 2, GLAD_PROFILE_NFW_CSE = 3 } glad_profile_kind;
 #define GLAD_NPROF 4
 glad_status glad_mge1d_batch(glad_ctx* ctx, int kind, const float* d_prof, int B, int n_gauss, float sigma_lo,
                              float sigma_hi, int euler_order, float* d_mge);
@@ -248,6 +250,29 @@ glad_status glad_profile_read(glad_ctx* ctx, double* ms_out /*[GLAD_NKERNELS]*/,
 #define GLAD_LIGHT_SERSIC 0
 #define GLAD_LIGHT_CHAMELEON 1
 glad_status glad_set_light_profiles(glad_ctx* ctx, int source_kind, int lens1_kind, int lens2_kind);
+
+/*
+ * SURVEY 8(f) rank 4, mass part: an elliptical NFW dark-matter halo through core-steep ellipsoids (Appendix A; the dark
+ * matter of the paper's composite model kappa_int,comp):
+ *   kappa_enfw(x, y) = rho_s sum_i A_i / (2 (s_i^2 + u^2)^(3/2)),  u^2 = X^2 + Y^2/q^2,  (X, Y) = (sqrt(q)/r_s) (x, y)   (Eq. A.2-A.4)
+ * in the halo frame (centre = the lens centre lens[0..1], major axis at angle phi), with the closed-form potential of a CSE
+ * (Eq. A.6) for alpha, the Hessian and psi: psi = (rho_s r_s^2/q) sum A_i psi_CSE, alpha = (rho_s r_s/sqrt(q)) sum A_i grad psi_CSE
+ * (DESIGN.md R-N2: amplitudes from Eq. 7; the prefactor printed in Eq. A.7 is off by one power of r_s).
+ *   d_enfw [n,4] DEVICE pointer, BORROWED: {rho_s (dimensionless, >= 0; 0 = no halo for that vector), r_s [arcsec] > 0, q in (0,1], phi};
+ *     NULL switches the halo off.  Vector b of a batch reads row b; B > n returns GLAD_EINVAL; invalid rows flag the vector
+ *     (GLAD_FLAG_LENS_INVALID).
+ *   h_A, h_s [n_cse <= GLAD_MAX_CSE] HOST arrays, copied: the (A_i, s_i) table of Eq. A.3.  The paper uses Oguri (2021)'s 44 pairs
+ *     and says they are "predetermined": the table is an INPUT of the method (R-N1).  workloads/cse_nfw.txt holds a table
+ *     fitted from Eq. A.5 as printed (41 positive pairs, 6.9e-6 relative on u in [1e-6, 1e3]).
+ *   n_gauss, sigma_lo, sigma_hi: the halo's rows of the mass MGE (Eq. 46 of Sigma_crit lambda kappa_enfw, q' = q), appended after the EPL
+ *     (and mass-sheet) rows by glad_joint_loglike_model_batch / _full_batch; d_mass_mge_out is then wider by n_gauss rows.
+ * While set: the lens half (every entry built on glad_lens_image_batch) adds alpha_enfw to the ray-shoot (fp32, the Chameleon /
+ * mass-sheet instantiation of the kernel), glad_quasar_chi2_batch adds alpha, the Hessian and psi (fp64).  The pixelated-source
+ * entry does not take the halo (GLAD_ESTATE while it is set).  SYNCHRONOUS setup call (copies the table).
+ */
+#define GLAD_MAX_CSE 64
+glad_status glad_set_enfw(glad_ctx* ctx, const float* d_enfw, int n_enfw, int n_cse, const double* h_A, const double* h_s, int n_gauss,
+                          float sigma_lo, float sigma_hi);
 
 /*
  * Options of the quadrature (row a6), fixed for the context until changed; 0 selects the default of each.

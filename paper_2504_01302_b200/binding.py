@@ -13,7 +13,7 @@ import torch
 from .build import LIB, build
 
 NLENS, NDYN, NPROF = 26, 4, 4
-PROFILE_SERSIC, PROFILE_EPL, PROFILE_CHAMELEON = 0, 1, 2
+PROFILE_SERSIC, PROFILE_EPL, PROFILE_CHAMELEON, PROFILE_NFW_CSE = 0, 1, 2, 3
 LIGHT_SERSIC, LIGHT_CHAMELEON = 0, 1
 FLAG_LENS_INVALID, FLAG_DYN_INVALID, FLAG_BIN_INVALID = 1, 2, 4
 FLAG_PIXSRC_NOT_PD = 8
@@ -24,7 +24,7 @@ EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "gl
            "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count", "glad_profile_enable",
            "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch", "glad_set_overlap", "glad_set_light_profiles",
            "glad_set_quasar_data", "glad_quasar_chi2_batch", "glad_joint_loglike_full_batch", "glad_set_mass_sheet",
-           "glad_pixsrc_evidence_batch", "glad_set_jam_options", "glad_set_jam_sph_rules", "glad_jam_sph_vrms_batch"]
+           "glad_pixsrc_evidence_batch", "glad_set_jam_options", "glad_set_jam_sph_rules", "glad_jam_sph_vrms_batch", "glad_set_enfw"]
 
 
 class GladError(RuntimeError):
@@ -101,6 +101,8 @@ def load(rebuild: bool = False):
     L.glad_set_jam_sph_rules.argtypes = [vp, vp, i, vp, i, vp, vp, i, vp, vp, i, vp, vp, i]
     L.glad_jam_sph_vrms_batch.restype = i
     L.glad_jam_sph_vrms_batch.argtypes = [vp, vp, i, vp, i, l, vp, i, l, vp, i, vp, vp, vp, vp, vp]
+    L.glad_set_enfw.restype = i
+    L.glad_set_enfw.argtypes = [vp, vp, i, i, C.POINTER(C.c_double), C.POINTER(C.c_double), i, C.c_float, C.c_float]
     L.glad_set_jam_options.restype = i
     L.glad_set_jam_options.argtypes = [vp, i, i, i, i]
     L.glad_launch_count.restype = l
@@ -145,6 +147,7 @@ class Glad:
         self.ctx = ctx
         if self.DEFAULT_JAM_PATH != "auto":
             self.set_jam_options(path=self.DEFAULT_JAM_PATH)
+        self.n_halo_rows = 0
         self.image_shape = None
         self.sky_shape = None
         self.nbins = 0
@@ -178,6 +181,22 @@ class Glad:
     def set_jam_options(self, path: str = "auto", terms: int = 0, flush: int = 0, slices: int = 0):
         """Row a6 options: path "auto" (tcgen05 where the grid fits) or "simt"; bf16 terms 2/3; 0 = default."""
         self._check(self.lib.glad_set_jam_options(self.ctx, {"auto": 0, "tc": 0, "simt": 1}[path], int(terms), int(flush), int(slices)))
+
+    def set_enfw(self, enfw, cse_A=None, cse_s=None, n_gauss=16, sigma_range=(0.05, 300.0)):
+        """eNFW halo per vector: enfw [n,4] = {rho_s, r_s, q, phi} (None switches it off); (cse_A, cse_s) = the CSE table."""
+        if enfw is None:
+            self._check(self.lib.glad_set_enfw(self.ctx, None, 0, 0, None, None, 0, 0.0, 0.0))
+            self._keep.pop("enfw", None)
+            self.n_halo_rows = 0
+            return
+        t = _dev(enfw, torch.float32, self.device).reshape(-1, 4)
+        A = np.ascontiguousarray(cse_A, dtype=np.float64)
+        s = np.ascontiguousarray(cse_s, dtype=np.float64)
+        dp = C.POINTER(C.c_double)
+        self._check(self.lib.glad_set_enfw(self.ctx, _p(t), int(t.shape[0]), int(A.size), A.ctypes.data_as(dp), s.ctypes.data_as(dp),
+                                           int(n_gauss), float(sigma_range[0]), float(sigma_range[1])))
+        self._keep["enfw"] = t
+        self.n_halo_rows = int(n_gauss)
 
     def set_overlap(self, on: bool):
         self._check(self.lib.glad_set_overlap(self.ctx, 1 if on else 0))
@@ -322,7 +341,7 @@ class Glad:
         mk = lambda n, ty: out.get(n) if out.get(n) is not None else torch.empty(B, dtype=ty, device=self.device)
         ll, c2l, c2d, fl = mk("loglike", torch.float32), mk("chi2_lens", torch.float32), mk("chi2_dyn", torch.float32), mk("flags", torch.int32)
         lum = torch.empty((B, int(n_lum), 3), dtype=torch.float32, device=self.device) if want_tables else None
-        n_tot = int(n_mass) + (self._n_sheet if "lambda" in self._keep else 0)
+        n_tot = int(n_mass) + (self._n_sheet if "lambda" in self._keep else 0) + (self.n_halo_rows if "enfw" in self._keep else 0)
         mass = torch.empty((B, n_tot, 3), dtype=torch.float32, device=self.device) if want_tables else None
         self._check(self.lib.glad_joint_loglike_model_batch(
             self.ctx, _p(p), _p(d), _p(dt), float(z_d), B, int(n_lum), float(lum_range[0]), float(lum_range[1]), int(n_mass),

@@ -105,7 +105,7 @@ void glad_destroy(glad_ctx* c) {
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     free_kin(c);
     void* ps[] = {c->d_psf, c->d_lens_const, c->d_jam_tab, c->d_partial, c->d_tmp, c->d_tmpflags, c->d_stage, c->d_model, c->d_qtmp, c->d_pix,
-                  c->d_sph_tab, c->d_sph_rat};
+                  c->d_sph_tab, c->d_sph_rat, c->d_cse64, c->d_cse32};
     for (void* p : ps) if (p) cudaFree(p);
     for (cudaEvent_t e : c->prof_ev) if (e) cudaEventDestroy(e);
     }
@@ -171,6 +171,33 @@ glad_status glad_set_jam_options(glad_ctx* c, int path, int bf16_terms, int flus
     c->jam_terms = bf16_terms ? bf16_terms : 2;
     c->jam_flush = flush_chunks;
     c->jam_slices = k_slices;
+    return GLAD_OK;
+}
+
+glad_status glad_set_enfw(glad_ctx* c, const float* d_enfw, int n_enfw, int n_cse, const double* h_A, const double* h_s, int n_gauss,
+                          float sigma_lo, float sigma_hi) {
+    if (!c) return GLAD_EINVAL;
+    if (!d_enfw) { c->d_enfw = nullptr; return GLAD_OK; }
+    if (n_enfw <= 0 || !h_A || !h_s) return fail(c, GLAD_EINVAL, "glad_set_enfw: n = %d / null table", n_enfw);
+    if (n_cse < 1 || n_cse > GLAD_MAX_CSE) return fail(c, GLAD_ESHAPE, "glad_set_enfw: %d core-steep ellipsoids (1..GLAD_MAX_CSE)", n_cse);
+    if (n_gauss < 2 || !(sigma_lo > 0.f) || !(sigma_hi > sigma_lo)) return fail(c, GLAD_EINVAL, "glad_set_enfw: %d Gaussians on [%g, %g]", n_gauss, sigma_lo, sigma_hi);
+    if (n_gauss > GLAD_MAX_GAUSS) return fail(c, GLAD_ESHAPE, "glad_set_enfw: more than GLAD_MAX_GAUSS Gaussians");
+    double2 t64[GLAD_MAX_CSE];
+    float2 t32[GLAD_MAX_CSE];
+    for (int i = 0; i < n_cse; ++i) {
+        if (!(h_s[i] > 0.0) || !isfinite(h_A[i])) return fail(c, GLAD_EINVAL, "glad_set_enfw: table entry %d = (%g, %g)", i, h_A[i], h_s[i]);
+        t64[i] = make_double2(h_A[i], h_s[i]);
+        t32[i] = make_float2((float)(h_A[i] / h_s[i]), (float)h_s[i]);
+    }
+    DeviceScope ds(c);
+    CU(cudaStreamSynchronize(c->stream), "sync");
+    if (c->side_stream) CU(cudaStreamSynchronize(c->side_stream), "sync");
+    if (!c->d_cse64) CU(cudaMalloc((void**)&c->d_cse64, sizeof(double2) * GLAD_MAX_CSE), "cudaMalloc CSE table");
+    if (!c->d_cse32) CU(cudaMalloc((void**)&c->d_cse32, sizeof(float2) * GLAD_MAX_CSE), "cudaMalloc CSE table");
+    CU(cudaMemcpy(c->d_cse64, t64, sizeof(double2) * n_cse, cudaMemcpyHostToDevice), "copy CSE table");
+    CU(cudaMemcpy(c->d_cse32, t32, sizeof(float2) * n_cse, cudaMemcpyHostToDevice), "copy CSE table");
+    c->d_enfw = d_enfw; c->n_enfw = n_enfw; c->ncse = n_cse;
+    c->nf_n = n_gauss; c->nf_lo = sigma_lo; c->nf_hi = sigma_hi;
     return GLAD_OK;
 }
 
@@ -332,6 +359,7 @@ glad_status glad_set_kin_data(glad_ctx* c, const glad_sky_grid* g, const int32_t
 static glad_status lens_impl(glad_ctx* c, const float* d_lens, int B, float* d_images, float* d_chi2, int32_t* d_flags) {
     if (!c->have_image) return fail(c, GLAD_ESTATE, "lens: glad_set_image_data not called");
     if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "lens: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
+    if (c->d_enfw && B > c->n_enfw) return fail(c, GLAD_EINVAL, "lens: batch of %d vectors but %d eNFW halos", B, c->n_enfw);
     if (d_chi2 && !c->d_data) return fail(c, GLAD_ESTATE, "lens: chi2 requested but no data/ivar set");
     glad_status st = grow(c, &c->d_lens_const, &c->lens_const_cap, (size_t)B * LC_SIZE);
     if (st != GLAD_OK) return st;
@@ -546,6 +574,7 @@ glad_status glad_quasar_chi2_batch(glad_ctx* c, const float* d_lens, const float
     if (B < 0 || (B > 0 && (!d_lens || !d_ddt))) return fail(c, GLAD_EINVAL, "glad_quasar_chi2_batch: B=%d / null pointer", B);
     if (!c->have_qso) return fail(c, GLAD_ESTATE, "glad_quasar_chi2_batch: glad_set_quasar_data not called");
     if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "glad_quasar_chi2_batch: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
+    if (c->d_enfw && B > c->n_enfw) return fail(c, GLAD_EINVAL, "glad_quasar_chi2_batch: batch of %d vectors but %d eNFW halos", B, c->n_enfw);
     if (B == 0) return GLAD_OK;
     DeviceScope ds(c);
     CU(launch_quasar(c, c->stream, d_lens, d_ddt, B, d_chi2_img, d_chi2_tmd, d_theta_pre, d_dt_pre, d_beta), "quasar_kernel");
@@ -558,6 +587,7 @@ glad_status glad_pixsrc_evidence_batch(glad_ctx* c, const float* d_lens, const f
     if (!c) return GLAD_EINVAL;
     if (B < 0 || (B > 0 && (!d_lens || !d_src_grid || !d_lam))) return fail(c, GLAD_EINVAL, "glad_pixsrc_evidence_batch: B=%d / null pointer", B);
     if (!c->have_image || !c->d_data || !c->d_ivar) return fail(c, GLAD_ESTATE, "glad_pixsrc_evidence_batch: glad_set_image_data (with data and ivar) not called");
+    if (c->d_enfw) return fail(c, GLAD_ESTATE, "glad_pixsrc_evidence_batch: the eNFW halo is not part of this entry; clear it with glad_set_enfw(ctx, NULL, ...)");
     if (nsx < 2 || nsy < 2 || (long)nsx * nsy > 4096) return fail(c, GLAD_ESHAPE, "glad_pixsrc_evidence_batch: source grid %d x %d (need >= 2 x 2, N_s <= 4096)", nsx, nsy);
     if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "glad_pixsrc_evidence_batch: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
     if (B == 0) return GLAD_OK;
@@ -646,7 +676,9 @@ glad_status glad_mge1d_batch(glad_ctx* c, int kind, const float* d_prof, int B, 
                              int P, float* d_mge) {
     if (!c) return GLAD_EINVAL;
     if (B < 0 || (B > 0 && (!d_prof || !d_mge))) return fail(c, GLAD_EINVAL, "glad_mge1d_batch: B=%d / null pointer", B);
-    if (kind != GLAD_PROFILE_SERSIC && kind != GLAD_PROFILE_EPL && kind != GLAD_PROFILE_CHAMELEON) return fail(c, GLAD_EINVAL, "glad_mge1d_batch: profile kind %d", kind);
+    if (kind != GLAD_PROFILE_SERSIC && kind != GLAD_PROFILE_EPL && kind != GLAD_PROFILE_CHAMELEON && kind != GLAD_PROFILE_NFW_CSE)
+        return fail(c, GLAD_EINVAL, "glad_mge1d_batch: profile kind %d", kind);
+    if (kind == GLAD_PROFILE_NFW_CSE && !c->d_cse64) return fail(c, GLAD_ESTATE, "glad_mge1d_batch: GLAD_PROFILE_NFW_CSE needs the CSE table of glad_set_enfw");
     if (P == 0) P = MGE_DEFAULT_ORDER;
     if (P < 1 || P > 15) return fail(c, GLAD_EINVAL, "glad_mge1d_batch: Euler order %d outside [1,15]", P);
     glad_status st = mge_check(c, "glad_mge1d_batch", n_gauss, sigma_lo, sigma_hi);
@@ -676,7 +708,8 @@ static glad_status model_impl(glad_ctx* c, const float* d_lens, const float* d_d
     if (B == 0) return GLAD_OK;
     DeviceScope ds(c);
     if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "joint model: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
-    const int nmt = nm + (c->d_lambda ? c->ms_n : 0);      // the mass sheet adds rows of its own
+    if (c->d_enfw && B > c->n_enfw) return fail(c, GLAD_EINVAL, "joint model: batch of %d vectors but %d eNFW halos", B, c->n_enfw);
+    const int nmt = nm + (c->d_lambda ? c->ms_n : 0) + (c->d_enfw ? c->nf_n : 0);      // the mass sheet and the halo add rows of their own
     if (nmt > GLAD_MAX_GAUSS) return fail(c, GLAD_ESHAPE, "joint model: n_mass %d + %d sheet Gaussians exceed GLAD_MAX_GAUSS", nm, nmt - nm);
     const size_t n_lens = (size_t)B * GLAD_NLENS, n_lum = (size_t)B * nl * 3, n_mass = (size_t)B * nmt * 3;
     st = grow(c, &c->d_model, &c->model_cap, n_lens + n_lum + n_mass);

@@ -23,7 +23,10 @@ enum LensConstIdx {
     LC_MS_RC, LC_MS_RT,
     LC_SERSIC0 = 16,   // 3 components x 8 floats: xc, yc, cos, sin, 1/q^2, amp = Ie e^bn, k1 = bn log2e Re^(-1/n), h = 1/(2n)
     LC_SERIES = 40,    // c_n, n = 1..GLAD_EPL_MAX_TERMS : (2n-(2-t))/(2n+(2-t))
-    LC_SIZE = 80
+    LC_NF_AMP = 80,    // eNFW halo (glad_set_enfw): rho_s r_s / sqrt(q), 0 = no halo
+    LC_NF_SC,          // sqrt(q) / r_s
+    LC_NF_Q, LC_NF_COS, LC_NF_SIN,
+    LC_SIZE = 88
 };
 #define LC_SERSIC_STRIDE 8
 
@@ -50,6 +53,14 @@ static inline __host__ __device__ int jam_table_floats(int nl, int nmx) {
 #define GLAD_PROF_MAX 2048
 enum GladKernelId { GK_LENS_PREP = 0, GK_LENS_IMAGE, GK_JAM_PREP, GK_JAM_QUAD, GK_JAM_POST, GK_JOINT, GK_MGE, GK_QUASAR,
                     GK_PIX_MAP, GK_PIX_BLUR, GK_PIX_SYRK, GK_PIX_RHS, GK_PIX_CHOL, GK_PIX_MODEL, GK_JAM_SPH, GK_JAM_SPH_LOS };
+
+// eNFW halo (glad_set_enfw), passed to the kernels by value: per-vector {rho_s, r_s, q, phi} rows and the CSE table (A_i, s_i)
+struct HaloArgs {
+    const float* nf;         // [B,4] or NULL = no halo
+    const double2* cse64;    // [ncse] for the fp64 kernels
+    const float2* cse32;     // [ncse] {A_i / s_i, s_i} for the fp32 ray-shoot
+    int ncse;
+};
 
 // quasar data (glad_set_quasar_data), passed to quasar_kernel by value
 struct glad_quasar_data {
@@ -92,6 +103,13 @@ struct glad_ctx {
     const float* d_lambda;
     double ms_rc, ms_rt, ms_lo, ms_hi;
     int ms_n, n_lambda;
+
+    // eNFW halo (glad_set_enfw): d_enfw borrowed, NULL = off; the CSE table is copied
+    const float* d_enfw;
+    int n_enfw, ncse, nf_n;
+    double nf_lo, nf_hi;
+    double2* d_cse64;
+    float2* d_cse32;
 
     // quasar static data (copied)
     bool have_qso;
@@ -176,6 +194,13 @@ struct DeviceScope {
     explicit DeviceScope(const glad_ctx* c) : prev(-1) { if (cudaGetDevice(&prev) != cudaSuccess) prev = -1; if (prev != c->device) cudaSetDevice(c->device); else prev = -1; }
     ~DeviceScope() { if (prev >= 0) cudaSetDevice(prev); }
 };
+
+static inline HaloArgs halo_args(const glad_ctx* c, size_t first_vector = 0) {
+    HaloArgs a;
+    a.nf = c->d_enfw ? c->d_enfw + 4 * first_vector : nullptr;
+    a.cse64 = c->d_cse64; a.cse32 = c->d_cse32; a.ncse = c->ncse;
+    return a;
+}
 
 // kernel launchers (return cudaGetLastError())
 cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B);

@@ -11,6 +11,11 @@ struct MassConst {
     double lam, ms_rc, ms_rt, ms_a;     // internal mass sheet (R-S1..3): ms_a = (1 - lam) rc rt, 0 = none
     int nterms;
     bool epl, sheet;
+    // eNFW halo through core-steep ellipsoids (Appendix A; DESIGN.md R-N1..3): amp = rho_s r_s / sqrt(q), sc = sqrt(q) / r_s
+    bool halo, halo_ok;
+    double nf_rho, nf_amp, nf_sc, nf_q, nf_c, nf_s, nf_psi;
+    const double2* cse;
+    int ncse;
 };
 
 struct MassEval { double ax, ay, hxx, hxy, hyy, psi; };
@@ -39,6 +44,21 @@ __device__ static inline void mass_const(const float* __restrict__ p, double lam
     m.sh_c = (double)p[6] * c2;
     m.sh_s = (double)p[6] * s2;
     m.bh = p[8];
+}
+
+// per-vector halo constants; nf = {rho_s, r_s, q, phi} (NULL = none).  halo_ok = the vector's halo parameters are valid.
+__device__ static inline void mass_const_halo(const float* __restrict__ nf, const double2* cse, int ncse, MassConst& m) {
+    m.halo = false; m.halo_ok = true; m.cse = cse; m.ncse = ncse;
+    if (!nf) return;
+    const double rho = nf[0], rs = nf[1], q = nf[2];
+    m.halo_ok = (rho >= 0.0) && (rho == 0.0 || (rs > 0.0 && q > 0.0 && q <= 1.0));
+    if (!(rho > 0.0) || !m.halo_ok) return;
+    m.halo = true;
+    m.nf_rho = rho; m.nf_q = q;
+    m.nf_amp = rho * rs / sqrt(q);
+    m.nf_sc = sqrt(q) / rs;
+    m.nf_psi = rho * rs * rs / q;
+    sincos((double)nf[3], &m.nf_s, &m.nf_c);
 }
 
 // deflection, Hessian and potential of EPL + shear + point mass at the sky position (thx, thy)
@@ -109,6 +129,38 @@ __device__ static inline void mass_eval(const MassConst& m, double thx, double t
         hxx += g + ee * dx * dx; hyy += g + ee * dy * dy; hxy += ee * dx * dy;
         const double dc = R2 / (hc + rc), dt = R2 / (ht + rt);
         psi += 2.0 * m.ms_a / (rt - rc) * ((dc - rc * log1p(dc / (2.0 * rc))) - (dt - rt * log1p(dt / (2.0 * rt))));
+    }
+    if (m.halo) {
+        // kappa = rho_s sum A_i / (2 (s_i^2 + u^2)^(3/2)) (Eq. A.3-A.4); psi_CSE = q/(2s) ln Psi - q/s ln((1+q)s) (Eq. A.6),
+        // Psi = (psi_s + s)^2 + (1-q^2) X^2, psi_s = sqrt(q^2 (s^2 + X^2) + Y^2), (X, Y) = sc x (halo-frame offset)
+        const double q = m.nf_q, q2 = q * q;
+        const double xh = dx * m.nf_c + dy * m.nf_s, yh = dy * m.nf_c - dx * m.nf_s;
+        const double X = m.nf_sc * xh, Y = m.nf_sc * yh;
+        double aX = 0.0, aY = 0.0, hXX = 0.0, hXY = 0.0, hYY = 0.0, ps = 0.0;
+        for (int i = 0; i < m.ncse; ++i) {
+            const double2 t = m.cse[i];
+            const double A = t.x, si = t.y;
+            const double pss = sqrt(q2 * (si * si + X * X) + Y * Y), ip = 1.0 / pss, a = pss + si;
+            const double Psi = a * a + (1.0 - q2) * X * X, iP = 1.0 / Psi;
+            const double sX = q2 * X * ip, sY = Y * ip;
+            const double sXX = q2 * ip - sX * sX * ip, sYY = ip - sY * sY * ip, sXY = -sX * sY * ip;
+            const double PX = 2.0 * a * sX + 2.0 * (1.0 - q2) * X, PY = 2.0 * a * sY;
+            const double PXX = 2.0 * sX * sX + 2.0 * a * sXX + 2.0 * (1.0 - q2), PYY = 2.0 * sY * sY + 2.0 * a * sYY,
+                         PXY = 2.0 * sX * sY + 2.0 * a * sXY;
+            const double f = A * q / (2.0 * si);
+            aX += f * PX * iP; aY += f * PY * iP;
+            hXX += f * (PXX * iP - PX * PX * iP * iP);
+            hYY += f * (PYY * iP - PY * PY * iP * iP);
+            hXY += f * (PXY * iP - PX * PY * iP * iP);
+            ps += A * (q / (2.0 * si) * log(Psi) - q / si * log((1.0 + q) * si));
+        }
+        const double c = m.nf_c, s = m.nf_s;
+        ax += m.nf_amp * (aX * c - aY * s);
+        ay += m.nf_amp * (aX * s + aY * c);
+        hxx += m.nf_rho * (c * c * hXX - 2.0 * c * s * hXY + s * s * hYY);
+        hyy += m.nf_rho * (s * s * hXX + 2.0 * c * s * hXY + c * c * hYY);
+        hxy += m.nf_rho * (c * s * (hXX - hYY) + (c * c - s * s) * hXY);
+        psi += m.nf_psi * ps;
     }
     e.ax = ax; e.ay = ay; e.hxx = hxx; e.hxy = hxy; e.hyy = hyy; e.psi = psi;
 }

@@ -15,7 +15,7 @@
 #define LENS_PREP_ROLES 4
 __global__ void __launch_bounds__(32 * LENS_PREP_ROLES) lens_prep_kernel(const float* __restrict__ params, int B, int kinds,
                                                                          const float* __restrict__ lambda, double ms_rc, double ms_rt,
-                                                                         float* __restrict__ consts) {
+                                                                         const float* __restrict__ enfw, float* __restrict__ consts) {
     const int b = blockIdx.x * 32 + (threadIdx.x & 31), role = threadIdx.x >> 5;
     if (b >= B) return;
     const float* p = params + (size_t)b * GLAD_NLENS;
@@ -25,6 +25,9 @@ __global__ void __launch_bounds__(32 * LENS_PREP_ROLES) lens_prep_kernel(const f
     // internal mass sheet (Eq. 6 P:85 with the dPIE profile of Eq. 50; R-S1..3): kappa_int = (1-lam) S(R) + lam kappa_epl
     const double lam = lambda ? (double)lambda[b] : 1.0;
     if (!isfinite(lam)) valid = false;
+    // eNFW halo {rho_s, r_s, q, phi} (Appendix A; R-N1..3): rho_s = 0 disables it
+    const float* nf = enfw ? enfw + (size_t)b * 4 : nullptr;
+    if (nf && !((nf[0] >= 0.f) && (nf[0] == 0.f || (nf[1] > 0.f && nf[2] > 0.f && nf[2] <= 1.f)))) valid = false;
     for (int k = 0; k < 3; ++k) {
         const float* s = p + (k == 0 ? 11 : (k == 1 ? 16 : 21));
         const bool cham = (kinds >> k) & 1;                            // Chameleon (Eq. 47): 0 < w_c < w_t
@@ -62,6 +65,14 @@ __global__ void __launch_bounds__(32 * LENS_PREP_ROLES) lens_prep_kernel(const f
     for (int i = LC_SERIES; i < LC_SIZE; ++i) c[i] = 0.f;
     c[LC_VALID] = valid ? 1.f : 0.f;
     if (!valid) return;
+    if (nf && nf[0] > 0.f) {
+        const double rho = nf[0], rs = nf[1], qh = nf[2];
+        c[LC_NF_AMP] = (float)(rho * rs / sqrt(qh));
+        c[LC_NF_SC] = (float)(sqrt(qh) / rs);
+        c[LC_NF_Q] = (float)qh;
+        c[LC_NF_COS] = (float)cos((double)nf[3]);
+        c[LC_NF_SIN] = (float)sin((double)nf[3]);
+    }
     double tt = gam - 1.0;
     double f = (1.0 - q) / (1.0 + q);
     double bTM = q * pow(2.0 / (1.0 + q), 1.0 / tt) * thE;  // b_TM = q b, b from Eq. B.3
@@ -127,7 +138,7 @@ __device__ __forceinline__ float light_eval(int kinds, int k, const float* __res
 // code of the common case is exactly the table-driven loop
 template <bool CH, bool LONG>
 __device__ __forceinline__ float shoot(const float* __restrict__ c, float thx, float thy, int nterms,
-                                       bool has_src, bool has_l1, bool has_l2, int kinds) {
+                                       bool has_src, bool has_l1, bool has_l2, int kinds, const float2* __restrict__ cse, int ncse) {
     float dx = thx - c[LC_XL], dy = thy - c[LC_YL];
     float cs = c[LC_COSPA], sn = c[LC_SINPA];
     float x = dx * cs + dy * sn, y = dy * cs - dx * sn;
@@ -176,6 +187,26 @@ __device__ __forceinline__ float shoot(const float* __restrict__ c, float thx, f
         ax = fmaf(gs, dx, ax);
         ay = fmaf(gs, dy, ay);
     }
+    if (CH && c[LC_NF_AMP] != 0.f) {
+        // eNFW halo = sum of core-steep ellipsoids (Eq. A.3-A.7): alpha_X = (q X / s) [a q^2/psi_s + 1 - q^2] / Psi,
+        // alpha_Y = (q Y / s) a / (psi_s Psi), a = psi_s + s, in the halo frame scaled by sqrt(q)/r_s; every term positive
+        const float q = c[LC_NF_Q], q2 = q * q, omq2 = 1.f - q2, hc = c[LC_NF_COS], hs = c[LC_NF_SIN];
+        const float X = c[LC_NF_SC] * (dx * hc + dy * hs), Y = c[LC_NF_SC] * (dy * hc - dx * hs);
+        const float X2 = X * X, Y2 = Y * Y;
+        float sx = 0.f, sy = 0.f;
+        for (int i = 0; i < ncse; ++i) {
+            const float2 t = __ldg(cse + i);                          // {A_i / s_i, s_i}
+            const float s2 = t.y * t.y;
+            const float pss = sqrtf(fmaf(q2, s2 + X2, Y2));
+            const float a = pss + t.y;
+            const float iden = __fdividef(t.x, pss * fmaf(a, a, omq2 * X2));
+            sx = fmaf(iden, fmaf(a, q2, omq2 * pss), sx);
+            sy = fmaf(iden, a, sy);
+        }
+        const float hx = c[LC_NF_AMP] * q * X * sx, hy = c[LC_NF_AMP] * q * Y * sy;
+        ax += hx * hc - hy * hs;
+        ay += hx * hs + hy * hc;
+    }
     float v = 0.f;
     if (has_src) v += light_eval<CH>(kinds, 0, c + LC_SERSIC0, thx - ax, thy - ay);
     if (has_l1) v += light_eval<CH>(kinds, 1, c + LC_SERSIC0 + LC_SERSIC_STRIDE, thx, thy);
@@ -198,7 +229,7 @@ static inline __host__ __device__ int lens_img_pitch(int nx, int kpsf) { return 
 // rows a1-a3 for one vector: every sub-pixel ray, averaged into the binned image in shared memory
 template <bool CH, bool LONG>
 __device__ __forceinline__ void ray_pass(const float* __restrict__ c, const glad_image_grid& g, float* __restrict__ img, int pitch,
-                                         int HL, int nterms, int kinds) {
+                                         int HL, int nterms, int kinds, const float2* __restrict__ cse, int ncse) {
     const int tid = threadIdx.x, nthr = blockDim.x, nx = g.nx, npx = g.nx * g.ny, ss = g.supersample;
     const bool has_src = c[LC_SERSIC0 + 5] != 0.f;
     const bool has_l1 = c[LC_SERSIC0 + LC_SERSIC_STRIDE + 5] != 0.f;
@@ -211,7 +242,7 @@ __device__ __forceinline__ void ray_pass(const float* __restrict__ c, const glad
             float thy = fmaf(g.pix, (float)iy + (((float)sb + 0.5f) * inv_s - 0.5f), g.y0);
             for (int sa = 0; sa < ss; ++sa) {
                 float thx = fmaf(g.pix, (float)ix + (((float)sa + 0.5f) * inv_s - 0.5f), g.x0);
-                acc += shoot<CH, LONG>(c, thx, thy, nterms, has_src, has_l1, has_l2, kinds);
+                acc += shoot<CH, LONG>(c, thx, thy, nterms, has_src, has_l1, has_l2, kinds, cse, ncse);
             }
         }
         img[iy * pitch + HL + ix] = acc * inv_s2;
@@ -221,8 +252,8 @@ __device__ __forceinline__ void ray_pass(const float* __restrict__ c, const glad
 // out of line: the rare long-series loop must not raise the register count of the kernel (2 CTAs of 512 threads per SM)
 template <bool CH>
 __device__ __noinline__ void ray_pass_long(const float* __restrict__ c, const glad_image_grid& g, float* __restrict__ img, int pitch,
-                                           int HL, int nterms, int kinds) {
-    ray_pass<CH, true>(c, g, img, pitch, HL, nterms, kinds);
+                                           int HL, int nterms, int kinds, const float2* __restrict__ cse, int ncse) {
+    ray_pass<CH, true>(c, g, img, pitch, HL, nterms, kinds, cse, ncse);
 }
 
 template <bool CH>
@@ -230,7 +261,8 @@ __global__ void __launch_bounds__(512, 2) lens_image_kernel(const float* __restr
                                                          const float* __restrict__ psf, int kpsf,
                                                          const float* __restrict__ data,
                                                          const float* __restrict__ ivar, float* __restrict__ images,
-                                                         float* __restrict__ chi2, int32_t* __restrict__ flags) {
+                                                         float* __restrict__ chi2, int32_t* __restrict__ flags,
+                                                         const float2* __restrict__ cse, int ncse) {
     extern __shared__ __align__(16) float smem[];
     const int b = blockIdx.x, tid = threadIdx.x, nthr = blockDim.x;
     const int nx = g.nx, ny = g.ny, npx = nx * ny, ss = g.supersample;
@@ -259,8 +291,8 @@ __global__ void __launch_bounds__(512, 2) lens_image_kernel(const float* __restr
     const int nterms = (int)c[LC_NTERMS];
 
     // rows a1-a3: rays -> binned pixel in shared memory
-    if (nterms > GLAD_EPL_MAX_TERMS) ray_pass_long<CH>(c, g, img, pitch, HL, nterms, kinds);        // CTA-uniform: one vector per CTA
-    else ray_pass<CH, false>(c, g, img, pitch, HL, nterms, kinds);
+    if (nterms > GLAD_EPL_MAX_TERMS) ray_pass_long<CH>(c, g, img, pitch, HL, nterms, kinds, cse, ncse);   // CTA-uniform: one vector per CTA
+    else ray_pass<CH, false>(c, g, img, pitch, HL, nterms, kinds, cse, ncse);
     __syncthreads();
 
     // row a4: PSF convolution from shared memory + chi2.  out[x] = sum_dy sum_dx psf[dy][dx] img[y+cc-dy][x+cc-dx]
@@ -324,7 +356,7 @@ __global__ void __launch_bounds__(512, 2) lens_image_kernel(const float* __restr
 cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B) {
     ProfScope ps(c, GK_LENS_PREP, c->lens_stream);
     lens_prep_kernel<<<(B + 31) / 32, 32 * LENS_PREP_ROLES, 0, c->lens_stream>>>(d_params, B, c->light_kinds, c->d_lambda, c->ms_rc,
-                                                                                 c->ms_rt, c->d_lens_const);
+                                                                                 c->ms_rt, c->d_enfw, c->d_lens_const);
     return cudaGetLastError();
 }
 
@@ -335,15 +367,15 @@ size_t lens_image_smem_bytes(int nx, int ny, int kpsf) {
 cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2, int32_t* d_flags) {
     const size_t smem = lens_image_smem_bytes(c->grid.nx, c->grid.ny, c->kpsf);
     if (smem > (size_t)glad_smem_dynamic_max(c)) return cudaErrorInvalidConfiguration;   // glad_set_image_data checks this up front
-    const int ch = c->light_kinds != 0 || c->d_lambda != nullptr;
+    const int ch = c->light_kinds != 0 || c->d_lambda != nullptr || c->d_enfw != nullptr;
     cudaError_t e = ch ? smem_optin(c, lens_image_kernel<true>) : smem_optin(c, lens_image_kernel<false>);
     if (e != cudaSuccess) return e;
     ProfScope ps(c, GK_LENS_IMAGE, c->lens_stream);
     if (ch)
         lens_image_kernel<true><<<B, 512, smem, c->lens_stream>>>(c->d_lens_const, c->light_kinds, c->grid, c->d_psf, c->kpsf,
-                                                                 c->d_data, c->d_ivar, d_images, d_chi2, d_flags);
+                                                                 c->d_data, c->d_ivar, d_images, d_chi2, d_flags, c->d_cse32, c->ncse);
     else
         lens_image_kernel<false><<<B, 512, smem, c->lens_stream>>>(c->d_lens_const, 0, c->grid, c->d_psf, c->kpsf, c->d_data,
-                                                                  c->d_ivar, d_images, d_chi2, d_flags);
+                                                                  c->d_ivar, d_images, d_chi2, d_flags, nullptr, 0);
     return cudaGetLastError();
 }

@@ -61,7 +61,8 @@ static EulerConsts euler_consts(int P) {
 // One profile of one vector: the n_gauss rows {A_n, sigma_n, q'} (Eq. 46).  Called by all warps of the CTA; warp w takes
 // Gaussians w, w + nwarps, ..; lane n = term n of the Euler sum.  bn = Sersic b_n (unused for the EPL).
 __device__ static void mge_rows(int kind, double p0, double p1, double p2, double qp, double bn, const EulerConsts& ec,
-                                int n_gauss, double sigma_lo, double dln, float* __restrict__ out_rows, double scale = 1.0) {
+                                int n_gauss, double sigma_lo, double dln, float* __restrict__ out_rows, double scale = 1.0,
+                                const double2* __restrict__ cse = nullptr, int ncse = 0) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
     const int nterm = 2 * ec.P + 1;
     const double t = p2 - 1.0;
@@ -77,6 +78,16 @@ __device__ static void mge_rows(int kind, double p0, double p1, double p2, doubl
             if (kind == GLAD_PROFILE_SERSIC) {
                 const cplx w = cpow_real({z.re / p1, z.im / p1}, 1.0 / p2);
                 re = p0 * cexp_d({-bn * (w.re - 1.0), -bn * w.im}).re;
+            } else if (kind == GLAD_PROFILE_NFW_CSE) {
+                // Eq. A.2-A.4 at complex radius: p0 sum A_i / (2 (s_i^2 + u^2)^(3/2)), u = z sqrt(q) / r_s
+                const double k2 = qp / (p1 * p1);
+                const cplx u2 = {k2 * (z.re * z.re - z.im * z.im), k2 * 2.0 * z.re * z.im};
+                double acc = 0.0;
+                for (int i = 0; i < ncse; ++i) {
+                    const double2 t = cse[i];
+                    acc += t.x * 0.5 * cpow_real({t.y * t.y + u2.re, u2.im}, -1.5).re;
+                }
+                re = p0 * acc;
             } else if (kind == GLAD_PROFILE_CHAMELEON) {
                 // Eq. 47 at complex radius: p0/(1+q) [ (z^2 + a_c)^(-1/2) - (z^2 + a_t)^(-1/2) ], a = 4 w^2/(1+q)^2
                 const double opq = 1.0 + qp, ac = 4.0 * p1 * p1 / (opq * opq), at = 4.0 * p2 * p2 / (opq * opq);
@@ -103,7 +114,7 @@ __device__ static void mge_rows(int kind, double p0, double p1, double p2, doubl
 
 __global__ void __launch_bounds__(256) mge1d_kernel(int kind, const float* __restrict__ prof, int B, int n_gauss,
                                                     double sigma_lo, double dln, const __grid_constant__ EulerConsts ec,
-                                                    float* __restrict__ mge) {
+                                                    const double2* __restrict__ cse, int ncse, float* __restrict__ mge) {
     __shared__ double s_bn;
     const int b = blockIdx.x;
     const float* p = prof + (size_t)b * GLAD_NPROF;
@@ -113,7 +124,7 @@ __global__ void __launch_bounds__(256) mge1d_kernel(int kind, const float* __res
         __syncthreads();
     }
     mge_rows(kind, p0, p1, p2, qp, kind == GLAD_PROFILE_SERSIC ? s_bn : 0.0, ec, n_gauss, sigma_lo, dln,
-             mge + (size_t)b * n_gauss * 3);
+             mge + (size_t)b * n_gauss * 3, 1.0, cse, ncse);
 }
 
 cudaError_t launch_mge1d(glad_ctx* c, int kind, const float* d_prof, int B, int n_gauss, float sigma_lo, float sigma_hi,
@@ -121,7 +132,7 @@ cudaError_t launch_mge1d(glad_ctx* c, int kind, const float* d_prof, int B, int 
     ProfScope ps(c, GK_MGE);
     const double dln = log((double)sigma_hi / (double)sigma_lo) / (n_gauss - 1);
     const int warps = n_gauss < 8 ? n_gauss : 8;
-    mge1d_kernel<<<B, 32 * warps, 0, c->stream>>>(kind, d_prof, B, n_gauss, (double)sigma_lo, dln, euler_consts(P), d_mge);
+    mge1d_kernel<<<B, 32 * warps, 0, c->stream>>>(kind, d_prof, B, n_gauss, (double)sigma_lo, dln, euler_consts(P), c->d_cse64, c->ncse, d_mge);
     return cudaGetLastError();
 }
 
@@ -135,7 +146,8 @@ __global__ void __launch_bounds__(256) model_kernel(const float* __restrict__ le
                                                     const float* __restrict__ ddt, double zd, int B, int tracer_kind, int n_lum, double lum_lo,
                                                     double lum_dln, int n_mass, double mass_lo, double mass_dln,
                                                     const float* __restrict__ lambda, double ms_rc, double ms_rt, int ms_n, double ms_lo,
-                                                    double ms_dln, const __grid_constant__ EulerConsts ec, float* __restrict__ lens_out,
+                                                    double ms_dln, const HaloArgs halo, int nf_n, double nf_lo, double nf_dln,
+                                                    const __grid_constant__ EulerConsts ec, float* __restrict__ lens_out,
                                                     float* __restrict__ lum, float* __restrict__ mass) {
     __shared__ double s_bn, s_sc;
     const int b = blockIdx.x;
@@ -156,13 +168,20 @@ __global__ void __launch_bounds__(256) model_kernel(const float* __restrict__ le
     mge_rows(tracer_kind, L[16], L[17], L[18], L[19], s_bn, ec, n_lum, lum_lo, lum_dln, lum + (size_t)b * n_lum * 3);
     // internal mass sheet (Eq. 6, 12, 50; R-S1..3): Sigma_int = Sigma_crit [lam kappa_epl + (1 - lam) S(R)].  The EPL rows carry lam;
     // the round sheet (q' = 1) gets ms_n rows of its own after them: it is Eq. 47's shape at q = 1 with I_0/2 = Sigma_crit (1-lam)/(1/rc - 1/rt)
-    const int nm_tot = n_mass + (lambda ? ms_n : 0);
+    const int nm_tot = n_mass + (lambda ? ms_n : 0) + (halo.nf ? nf_n : 0);
     const double lam = lambda ? (double)lambda[b] : 1.0;
     float* M = mass + (size_t)b * nm_tot * 3;
     mge_rows(GLAD_PROFILE_EPL, s_sc, L[2], L[3], L[4], 0.0, ec, n_mass, mass_lo, mass_dln, M, lam);
     if (lambda)
         mge_rows(GLAD_PROFILE_CHAMELEON, 2.0 * s_sc * (1.0 - lam) / (1.0 / ms_rc - 1.0 / ms_rt), ms_rc, ms_rt, 1.0, 0.0, ec, ms_n, ms_lo,
                  ms_dln, M + (size_t)n_mass * 3);
+    // eNFW halo (Appendix A): Sigma_crit lam kappa_enfw, nf_n rows with q' = the halo's q after the EPL (and sheet) rows;
+    // the halo is part of the lens mass, so it carries lam like the EPL (kappa_int,comp of P:380)
+    if (halo.nf) {
+        const float* nf = halo.nf + 4 * (size_t)b;
+        mge_rows(GLAD_PROFILE_NFW_CSE, s_sc * (double)nf[0], (double)nf[1], 0.0, (double)nf[2], 0.0, ec, nf_n, nf_lo, nf_dln,
+                 M + (size_t)(n_mass + (lambda ? ms_n : 0)) * 3, lam, halo.cse64, halo.ncse);
+    }
 }
 
 cudaError_t launch_model(glad_ctx* c, const float* d_lens, const float* d_dyn, const float* d_ddt, double zd, int B, int tracer_kind, int n_lum,
@@ -172,6 +191,7 @@ cudaError_t launch_model(glad_ctx* c, const float* d_lens, const float* d_dyn, c
     const double ldln = log((double)lum_hi / (double)lum_lo) / (n_lum - 1), mdln = log((double)mass_hi / (double)mass_lo) / (n_mass - 1);
     const double sdln = (c->d_lambda && c->ms_n > 1) ? log(c->ms_hi / c->ms_lo) / (c->ms_n - 1) : 0.0;
     model_kernel<<<B, 256, 0, c->stream>>>(d_lens, d_dyn, d_ddt, zd, B, tracer_kind, n_lum, (double)lum_lo, ldln, n_mass, (double)mass_lo, mdln,
-                                           c->d_lambda, c->ms_rc, c->ms_rt, c->ms_n, c->ms_lo, sdln, euler_consts(P), d_lens_out, d_lum, d_mass);
+                                           c->d_lambda, c->ms_rc, c->ms_rt, c->ms_n, c->ms_lo, sdln, halo_args(c), c->nf_n, c->nf_lo,
+                                           (c->d_enfw && c->nf_n > 1) ? log(c->nf_hi / c->nf_lo) / (c->nf_n - 1) : 0.0, euler_consts(P), d_lens_out, d_lum, d_mass);
     return cudaGetLastError();
 }

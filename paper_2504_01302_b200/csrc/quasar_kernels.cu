@@ -26,8 +26,8 @@ __device__ __forceinline__ double group_sum(double v) {
 }
 
 __global__ void __launch_bounds__(64) quasar_kernel(const float* __restrict__ lens, const float* __restrict__ ddt,
-                                                    const float* __restrict__ lambda, double ms_rc, double ms_rt, int B,
-                                                    const glad_quasar_data qd, float* __restrict__ chi2_img,
+                                                    const float* __restrict__ lambda, double ms_rc, double ms_rt, const HaloArgs halo,
+                                                    int B, const glad_quasar_data qd, float* __restrict__ chi2_img,
                                                     float* __restrict__ chi2_tmd, double* __restrict__ theta_pre,
                                                     double* __restrict__ dt_pre, double* __restrict__ beta_out) {
     const int gid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -37,11 +37,13 @@ __global__ void __launch_bounds__(64) quasar_kernel(const float* __restrict__ le
     if (!vec) b = B - 1;
     const float* p = lens + (size_t)b * GLAD_NLENS;
     const double lam = lambda ? (double)lambda[b] : 1.0;
-    const bool valid = (p[2] >= 0.f) && (p[3] > 1.f && p[3] < 3.f) && (p[4] > 0.f && p[4] <= 1.f) && (p[8] >= 0.f) && isfinite(lam);
+    bool valid = (p[2] >= 0.f) && (p[3] > 1.f && p[3] < 3.f) && (p[4] > 0.f && p[4] <= 1.f) && (p[8] >= 0.f) && isfinite(lam);
     const bool img = i < qd.n_img;
     const double inf = __longlong_as_double(0x7ff0000000000000LL), nan = __longlong_as_double(0x7ff8000000000000LL);
     MassConst m;
     mass_const(p, lam, ms_rc, ms_rt, lambda != nullptr, m);
+    mass_const_halo(halo.nf ? halo.nf + 4 * (size_t)b : nullptr, halo.cse64, halo.ncse, m);
+    valid = valid && m.halo_ok;
     const int ii = img ? i : 0;
     const double ox = qd.theta[2 * ii], oy = qd.theta[2 * ii + 1];
     MassEval e;
@@ -88,7 +90,7 @@ cudaError_t launch_quasar(glad_ctx* c, cudaStream_t st, const float* d_lens, con
                           float* d_chi2_tmd, double* d_theta_pre, double* d_dt_pre, double* d_beta) {
     ProfScope ps(c, GK_QUASAR, st);
     const int threads = 64, total = B * QSO_LANES;
-    quasar_kernel<<<(total + threads - 1) / threads, threads, 0, st>>>(d_lens, d_ddt, c->d_lambda, c->ms_rc, c->ms_rt, B, c->qso, d_chi2_img, d_chi2_tmd,
+    quasar_kernel<<<(total + threads - 1) / threads, threads, 0, st>>>(d_lens, d_ddt, c->d_lambda, c->ms_rc, c->ms_rt, halo_args(c), B, c->qso, d_chi2_img, d_chi2_tmd,
                                                                       d_theta_pre, d_dt_pre, d_beta);
     return cudaGetLastError();
 }
