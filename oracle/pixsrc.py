@@ -149,3 +149,21 @@ def pixsrc_batch(lens, grid, psf, data, ivar, src_grids, lam, nsx, nsy):
                            dict(nx=nsx, ny=nsy, pix=float(sg[b, 2]), x0=float(sg[b, 0]), y0=float(sg[b, 1])),
                            np.float32(-1.0) if (bad[b] or not sg[b, 2] > 0) else lam[b], Bm) for b in range(B)]
     return {k: np.array([r[k] for r in res]) for k in res[0]}
+
+
+def pixsrc_lambda_opt(params, grid, psf, data, ivar, src_grid, lam_lo, lam_hi, Bm=None):
+    """Eq. 43: the evidence "at the optimal regularisation constant" -- lambda_hat = argmax over
+    [lam_lo, lam_hi] of ln P(d | f, lambda, g), by scipy's bounded scalar minimiser on x = ln(lambda) applied to pixsrc_evidence
+    as it stands (F, D do not depend on lambda; they are rebuilt per call all the same: no reuse, no shortcut).
+    Returns dict(lam_hat, and pixsrc_evidence(lam_hat)'s fields).  lam_hat is rounded to float32 (the type the batch call takes)
+    and the evidence is evaluated at that rounded value."""
+    from scipy.optimize import minimize_scalar
+    if Bm is None:
+        Bm = blurring_matrix(psf, int(grid["nx"]), int(grid["ny"]))
+    neg = lambda x: -pixsrc_evidence(params, grid, psf, data, ivar, src_grid, np.exp(x), Bm)["logev"]
+    r = minimize_scalar(neg, bounds=(np.log(lam_lo), np.log(lam_hi)), method="bounded", options=dict(xatol=1e-9, maxiter=200))
+    lam_hat = float(np.float32(np.exp(r.x)))
+    out = pixsrc_evidence(params, grid, psf, data, ivar, src_grid, lam_hat, Bm)
+    out["lam_hat"] = lam_hat
+    return out
+

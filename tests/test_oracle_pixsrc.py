@@ -149,3 +149,36 @@ def test_noise_free_data_recovered_and_batch_wrapper():
     out = pixsrc.pixsrc_batch(lens, grid, psf, data, ivar, sg, np.array([1e-6, -1.0], np.float32), src["nx"], src["ny"])
     assert np.isclose(out["logev"][0], r["logev"], rtol=1e-12) and out["flag"][0] == 0
     assert out["flag"][1] == 1 and out["logev"][1] == -np.inf
+
+
+def test_lambda_hat_satisfies_the_stationarity_condition():
+    """lambda_hat of Eq. 43.  At the maximum of the evidence over lambda, with s_MP the minimiser of chi2/2 + lambda E_S
+    (envelope theorem): d ln P / d lambda = -E_S(s_MP) - 1/2 tr[(F + lambda g)^-1 g] + N_s / (2 lambda) = 0, i.e.
+    2 lambda_hat E_S = N_s - lambda_hat tr[(F + lambda_hat g)^-1 g]  (the condition Suyu et al. 2006 give for the optimal lambda).
+    Evaluated here from F, g and s_MP rebuilt in numpy, beside the finite-difference slope of ln P itself."""
+    grid, psf, _, ivar, src = _setup()
+    for seed, p in ((1, _lens()), (2, _lens(thetaE=0.9, gamma=2.2, q=0.7))):
+        # data = a smooth source through the operator + noise, so that the evidence has an interior maximum in lambda
+        rng = np.random.default_rng(seed)
+        Lm, _ = pixsrc.mapping_matrix(p, grid, src)
+        f = pixsrc.blurring_matrix(psf, grid["nx"], grid["ny"]) @ Lm
+        jj, ii = np.mgrid[0:src["ny"], 0:src["nx"]]
+        s_true = 3.0 * np.exp(-((ii - 3.0) ** 2 + (jj - 2.5) ** 2) / 4.0).reshape(-1)
+        data = (f @ s_true + rng.normal(0.0, 0.05, f.shape[0])).reshape(grid["ny"], grid["nx"]).astype(np.float32)
+        w = np.full(data.shape, 400.0, np.float32)
+        w[0, :3] = 0.0
+        r = pixsrc.pixsrc_lambda_opt(p, grid, psf, data, w, src, 1e-6, 1e6)
+        lam = r["lam_hat"]
+        assert 1e-5 < lam < 1e5 and r["flag"] == 0
+        wv = w.astype(np.float64).reshape(-1)
+        F = f.T @ (wv[:, None] * f)
+        g = pixsrc.curvature_g(src["nx"], src["ny"])
+        tr = np.trace(np.linalg.solve(F + lam * g, g))
+        ns = src["nx"] * src["ny"]
+        assert 2 * lam * r["reg"] == pytest.approx(ns - lam * tr, rel=1e-4)
+        ev = lambda x: pixsrc.pixsrc_evidence(p, grid, psf, data, w, src, np.exp(x))["logev"]
+        x0, h = np.log(lam), 1e-3
+        slope = (ev(x0 + h) - ev(x0 - h)) / (2 * h)
+        curv = (ev(x0 + h) - 2 * ev(x0) + ev(x0 - h)) / h**2
+        assert curv < 0 and abs(slope / curv) < 1e-4                      # distance to the stationary point in ln(lambda)
+        assert ev(x0) >= max(ev(x0 + 0.05), ev(x0 - 0.05))
