@@ -418,6 +418,22 @@ glad_status glad_jam_sph_vrms_batch(glad_ctx* ctx, const float* d_dyn_params, in
                                     int beta_per_gaussian, float* d_vrms, float* d_chi2, float* d_v2map, float* d_moments,
                                     int32_t* d_flags);
 
+/*
+ * Eq. 43: the evidence of the pixelated-source reconstruction AT THE OPTIMAL regularisation constant,
+ *   lambda_hat = argmax over [lambda_lo, lambda_hi] of ln P(d_esr | f, lambda, g).
+ * F and D do not depend on lambda, only the factorisation does: the chain of glad_pixsrc_evidence_batch is run once up to F and D,
+ * then, on the device and without a host round trip, 22 evaluations of ln P(lambda) up to lambda-independent terms,
+ *   J(ln lambda) = y^T y / 2 - ln det(F + lambda g) / 2 + N_s ln(lambda) / 2,  L L^T = F + lambda g,  L y = D
+ * (since -chi2/2 - lambda E_S = -(d^T C_d^-1 d - D^T s_MP)/2 at s_MP): the two ends, then 18 golden-section steps on ln lambda, then
+ * the vertex of the parabola through the last bracket.  lambda_hat is rounded to float32 and everything glad_pixsrc_evidence_batch
+ * returns is then evaluated at that value.  d_lam_hat [B] (required) receives lambda_hat; other arguments, outputs, flags and
+ * errors as glad_pixsrc_evidence_batch; one vector needs about 4 N_pix N_s + 16 N_s^2 bytes of scratch.  GLAD_EINVAL unless
+ * 0 < lambda_lo < lambda_hi.  An evidence that is not unimodal on the interval gives a local maximum.
+ */
+glad_status glad_pixsrc_lambda_opt_batch(glad_ctx* ctx, const float* d_lens_params, const float* d_src_grid, float lambda_lo, float lambda_hi,
+                                         int n_sx, int n_sy, int B, int scratch_mib_max, float* d_lam_hat, float* d_logev, float* d_chi2,
+                                         float* d_reg, float* d_s_mp, float* d_model, int32_t* d_flags);
+
 /* Number of kernel launches enqueued by this context since creation (for bench.py's gpu_launches). */
 long glad_launch_count(const glad_ctx* ctx);
 

@@ -24,7 +24,7 @@ EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "gl
            "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count", "glad_profile_enable",
            "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch", "glad_set_overlap", "glad_set_light_profiles",
            "glad_set_quasar_data", "glad_quasar_chi2_batch", "glad_joint_loglike_full_batch", "glad_set_mass_sheet",
-           "glad_pixsrc_evidence_batch", "glad_set_jam_options", "glad_set_jam_sph_rules", "glad_jam_sph_vrms_batch", "glad_set_enfw"]
+           "glad_pixsrc_evidence_batch", "glad_set_jam_options", "glad_set_jam_sph_rules", "glad_jam_sph_vrms_batch", "glad_set_enfw", "glad_pixsrc_lambda_opt_batch"]
 
 
 class GladError(RuntimeError):
@@ -101,6 +101,8 @@ def load(rebuild: bool = False):
     L.glad_set_jam_sph_rules.argtypes = [vp, vp, i, vp, i, vp, vp, i, vp, vp, i, vp, vp, i]
     L.glad_jam_sph_vrms_batch.restype = i
     L.glad_jam_sph_vrms_batch.argtypes = [vp, vp, i, vp, i, l, vp, i, l, vp, i, vp, vp, vp, vp, vp]
+    L.glad_pixsrc_lambda_opt_batch.restype = i
+    L.glad_pixsrc_lambda_opt_batch.argtypes = [vp, vp, vp, C.c_float, C.c_float, i, i, i, i, vp, vp, vp, vp, vp, vp, vp]
     L.glad_set_enfw.restype = i
     L.glad_set_enfw.argtypes = [vp, vp, i, i, C.POINTER(C.c_double), C.POINTER(C.c_double), i, C.c_float, C.c_float]
     L.glad_set_jam_options.restype = i
@@ -409,6 +411,24 @@ class Glad:
         self._check(self.lib.glad_pixsrc_evidence_batch(self.ctx, _p(p), _p(sg), _p(lm), int(nsx), int(nsy), B, int(scratch_mib),
                                                         _p(ev), _p(c2), _p(rg), _p(s), _p(m), _p(fl)))
         return {"logev": ev, "chi2": c2, "reg": rg, "s_mp": s, "model": m, "flags": fl}
+
+    def pixsrc_lambda_opt_batch(self, lens_params, src_grids, lam_range, nsx, nsy, want_source=True, want_model=True, scratch_mib=0):
+        """Eq. 43: lambda_hat on [lam_range] per vector and the evidence (and everything pixsrc_evidence_batch returns) at it."""
+        p = _dev(lens_params, torch.float32, self.device).reshape(-1, NLENS)
+        sg = _dev(src_grids, torch.float32, self.device).reshape(-1, 3)
+        B = p.shape[0]
+        if sg.shape[0] != B:
+            raise GladError("lens and source-grid batches differ")
+        if getattr(self, "image_shape", None) is None:
+            raise GladError("set_image_data has not been called")
+        f32 = lambda *shape: torch.empty(shape, dtype=torch.float32, device=self.device)
+        lh, ev, c2, rg = f32(B), f32(B), f32(B), f32(B)
+        fl = torch.empty(B, dtype=torch.int32, device=self.device)
+        s = f32(B, int(nsy), int(nsx)) if want_source else None
+        m = f32(B, *self.image_shape) if want_model else None
+        self._check(self.lib.glad_pixsrc_lambda_opt_batch(self.ctx, _p(p), _p(sg), float(lam_range[0]), float(lam_range[1]), int(nsx), int(nsy),
+                                                          B, int(scratch_mib), _p(lh), _p(ev), _p(c2), _p(rg), _p(s), _p(m), _p(fl)))
+        return {"lam_hat": lh, "logev": ev, "chi2": c2, "reg": rg, "s_mp": s, "model": m, "flags": fl}
 
     def joint_loglike_full_batch(self, lens_params, dyn_params, ddt, z_d, n_lum, lum_range, n_mass, mass_range, beta, out=None):
         p = _dev(lens_params, torch.float32, self.device).reshape(-1, NLENS)

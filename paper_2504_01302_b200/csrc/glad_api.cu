@@ -581,26 +581,25 @@ glad_status glad_quasar_chi2_batch(glad_ctx* c, const float* d_lens, const float
     return GLAD_OK;
 }
 
-glad_status glad_pixsrc_evidence_batch(glad_ctx* c, const float* d_lens, const float* d_src_grid, const float* d_lam, int nsx, int nsy,
-                                       int B, int scratch_mib_max, float* d_logev, float* d_chi2, float* d_reg, float* d_s_mp,
-                                       float* d_model, int32_t* d_flags) {
-    if (!c) return GLAD_EINVAL;
-    if (B < 0 || (B > 0 && (!d_lens || !d_src_grid || !d_lam))) return fail(c, GLAD_EINVAL, "glad_pixsrc_evidence_batch: B=%d / null pointer", B);
-    if (!c->have_image || !c->d_data || !c->d_ivar) return fail(c, GLAD_ESTATE, "glad_pixsrc_evidence_batch: glad_set_image_data (with data and ivar) not called");
-    if (c->d_enfw) return fail(c, GLAD_ESTATE, "glad_pixsrc_evidence_batch: the eNFW halo is not part of this entry; clear it with glad_set_enfw(ctx, NULL, ...)");
-    if (nsx < 2 || nsy < 2 || (long)nsx * nsy > 4096) return fail(c, GLAD_ESHAPE, "glad_pixsrc_evidence_batch: source grid %d x %d (need >= 2 x 2, N_s <= 4096)", nsx, nsy);
-    if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "glad_pixsrc_evidence_batch: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
+static glad_status pixsrc_impl(glad_ctx* c, const char* who, const float* d_lens, const float* d_src_grid, const float* d_lam, double lam_lo,
+                               double lam_hi, float* d_lam_hat, int nsx, int nsy, int B, int scratch_mib_max, float* d_logev, float* d_chi2,
+                               float* d_reg, float* d_s_mp, float* d_model, int32_t* d_flags) {
+    const bool search = d_lam == nullptr;
+    if (!c->have_image || !c->d_data || !c->d_ivar) return fail(c, GLAD_ESTATE, "%s: glad_set_image_data (with data and ivar) not called", who);
+    if (c->d_enfw) return fail(c, GLAD_ESTATE, "%s: the eNFW halo is not part of this entry; clear it with glad_set_enfw(ctx, NULL, ...)", who);
+    if (nsx < 2 || nsy < 2 || (long)nsx * nsy > 4096) return fail(c, GLAD_ESHAPE, "%s: source grid %d x %d (need >= 2 x 2, N_s <= 4096)", who, nsx, nsy);
+    if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "%s: batch of %d vectors but the mass sheet has %d lambdas", who, B, c->n_lambda);
     if (B == 0) return GLAD_OK;
     DeviceScope ds(c);
     const int npix = c->grid.nx * c->grid.ny, ns = nsx * nsy;
     const size_t cap = (size_t)(scratch_mib_max > 0 ? scratch_mib_max : 16384) << 20;
-    const size_t one = pixsrc_scratch_bytes(npix, ns, 1);
-    if (one > cap) return fail(c, GLAD_ESHAPE, "glad_pixsrc_evidence_batch: one vector needs %zu bytes of scratch, limit %zu", one, cap);
+    const size_t one = pixsrc_scratch_bytes(npix, ns, 1, search);
+    if (one > cap) return fail(c, GLAD_ESHAPE, "%s: one vector needs %zu bytes of scratch, limit %zu", who, one, cap);
     int Bc = (int)(cap / one);
     if (Bc > B) Bc = B;
     if (Bc > 2 * c->sm_count) Bc = 2 * c->sm_count;
-    while (Bc > 1 && pixsrc_scratch_bytes(npix, ns, Bc) > cap) --Bc;
-    glad_status st = grow(c, &c->d_pix, &c->pix_cap, pixsrc_scratch_bytes(npix, ns, Bc), true);
+    while (Bc > 1 && pixsrc_scratch_bytes(npix, ns, Bc, search) > cap) --Bc;
+    glad_status st = grow(c, &c->d_pix, &c->pix_cap, pixsrc_scratch_bytes(npix, ns, Bc, search), true);
     if (st != GLAD_OK) return st;
     // ln det g in closed form: g = kron(I, T^2) + kron(T^2, I), T the (1,-2,1) matrix with eigenvalues -2 + 2 cos(k pi/(n+1))
     double logdet_g = 0.0;
@@ -611,14 +610,33 @@ glad_status glad_pixsrc_evidence_batch(glad_ctx* c, const float* d_lens, const f
         }
     for (int b0 = 0; b0 < B; b0 += Bc) {
         const int nb = B - b0 < Bc ? B - b0 : Bc;
-        CU(launch_pixsrc_chunk(c, c->d_pix, d_lens + (size_t)b0 * GLAD_NLENS, d_src_grid + (size_t)b0 * 3, d_lam + b0,
+        CU(launch_pixsrc_chunk(c, c->d_pix, d_lens + (size_t)b0 * GLAD_NLENS, d_src_grid + (size_t)b0 * 3, d_lam ? d_lam + b0 : nullptr,
                                c->d_lambda ? c->d_lambda + b0 : nullptr, nsx, nsy, nb, logdet_g, d_logev ? d_logev + b0 : nullptr,
                                d_chi2 ? d_chi2 + b0 : nullptr, d_reg ? d_reg + b0 : nullptr,
                                d_s_mp ? d_s_mp + (size_t)b0 * ns : nullptr, d_model ? d_model + (size_t)b0 * npix : nullptr,
-                               d_flags ? d_flags + b0 : nullptr),
+                               d_flags ? d_flags + b0 : nullptr, lam_lo, lam_hi, d_lam_hat ? d_lam_hat + b0 : nullptr),
            "pixsrc kernels");
     }
     return GLAD_OK;
+}
+
+glad_status glad_pixsrc_evidence_batch(glad_ctx* c, const float* d_lens, const float* d_src_grid, const float* d_lam, int nsx, int nsy,
+                                       int B, int scratch_mib_max, float* d_logev, float* d_chi2, float* d_reg, float* d_s_mp,
+                                       float* d_model, int32_t* d_flags) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && (!d_lens || !d_src_grid || !d_lam))) return fail(c, GLAD_EINVAL, "glad_pixsrc_evidence_batch: B=%d / null pointer", B);
+    return pixsrc_impl(c, "glad_pixsrc_evidence_batch", d_lens, d_src_grid, d_lam, 0.0, 0.0, nullptr, nsx, nsy, B, scratch_mib_max, d_logev, d_chi2,
+                       d_reg, d_s_mp, d_model, d_flags);
+}
+
+glad_status glad_pixsrc_lambda_opt_batch(glad_ctx* c, const float* d_lens, const float* d_src_grid, float lam_lo, float lam_hi, int nsx, int nsy,
+                                         int B, int scratch_mib_max, float* d_lam_hat, float* d_logev, float* d_chi2, float* d_reg,
+                                         float* d_s_mp, float* d_model, int32_t* d_flags) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && (!d_lens || !d_src_grid || !d_lam_hat))) return fail(c, GLAD_EINVAL, "glad_pixsrc_lambda_opt_batch: B=%d / null pointer", B);
+    if (!(lam_lo > 0.f) || !(lam_hi > lam_lo) || !isfinite(lam_hi)) return fail(c, GLAD_EINVAL, "glad_pixsrc_lambda_opt_batch: lambda range [%g, %g]", lam_lo, lam_hi);
+    return pixsrc_impl(c, "glad_pixsrc_lambda_opt_batch", d_lens, d_src_grid, nullptr, (double)lam_lo, (double)lam_hi, d_lam_hat, nsx, nsy, B,
+                       scratch_mib_max, d_logev, d_chi2, d_reg, d_s_mp, d_model, d_flags);
 }
 
 glad_status glad_joint_loglike_host(glad_ctx* c, const float* h_lens, const float* h_dyn, int B, const float* h_lum, int nl,

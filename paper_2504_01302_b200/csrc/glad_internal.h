@@ -230,10 +230,13 @@ cudaError_t launch_model(glad_ctx* c, const float* d_lens, const float* d_dyn, c
                          float lum_lo, float lum_hi, int n_mass, float mass_lo, float mass_hi, int P, float* d_lens_out,
                          float* d_lum, float* d_mass);
 // pixelated-source evidence (pixsrc_kernels.cu): bytes of scratch for a chunk of Bc vectors; the whole chain for one chunk
-size_t pixsrc_scratch_bytes(int npix, int ns, int Bc);
+// search = the lambda_hat entry (a second N_s^2 matrix per vector + the search state)
+size_t pixsrc_scratch_bytes(int npix, int ns, int Bc, bool search);
+// d_lam != NULL: evidence at the given lambda; d_lam == NULL: lambda_hat searched on [lam_lo, lam_hi] (Eq. 43) and written to d_lam_hat
 cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens, const float* d_src_grid, const float* d_lam,
                                 const float* d_ms_lambda, int nsx, int nsy, int Bc, double logdet_g, float* d_logev, float* d_chi2,
-                                float* d_reg, float* d_s_mp, float* d_model, int32_t* d_flags);
+                                float* d_reg, float* d_s_mp, float* d_model, int32_t* d_flags, double lam_lo, double lam_hi,
+                                float* d_lam_hat);
 // tensor-core (tcgen05) form of row a6; supported when the folded grid has ny_f <= 128, N = terms * nx_f <= 256
 // and two operand stages fit in shared memory
 bool jam_quad_tc_supported(const glad_ctx* c, int nl, int nmx);

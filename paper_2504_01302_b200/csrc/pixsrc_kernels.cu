@@ -41,14 +41,17 @@ __global__ void __launch_bounds__(PX_MAP_THREADS) pixsrc_map_kernel(const float*
     const int npix = g.nx * g.ny;
     const float* p = lens + (size_t)b * GLAD_NLENS;
     __shared__ MassConst m;
-    if (threadIdx.x == 0) mass_const(p, ms_lambda ? (double)ms_lambda[b] : 1.0, ms_rc, ms_rt, ms_lambda != nullptr, m);
+    if (threadIdx.x == 0) {
+        mass_const(p, ms_lambda ? (double)ms_lambda[b] : 1.0, ms_rc, ms_rt, ms_lambda != nullptr, m);
+        mass_const_halo(nullptr, nullptr, 0, m);
+    }
     __syncthreads();
     const int q = blockIdx.x * PX_MAP_THREADS + threadIdx.x;
     if (q >= npix) return;
     const float* sg = src_grid + (size_t)b * 3;
     int id = -1;
     float2 w = make_float2(0.f, 0.f);
-    if (pixsrc_valid(p, lam_reg[b], sg[2])) {
+    if (pixsrc_valid(p, lam_reg ? lam_reg[b] : 1.f, sg[2])) {     // lam_reg == NULL: lambda is searched for (Eq. 43)
         const int iy = q / g.nx, ix = q - iy * g.nx;
         const double thx = (double)g.x0 + ix * (double)g.pix, thy = (double)g.y0 + iy * (double)g.pix;
         MassEval e;
@@ -236,7 +239,7 @@ __global__ void __launch_bounds__(256, 2) pixsrc_syrk_kernel(const float* __rest
         }
         hit_cur = hit_nxt;
     }
-    const double lam = (double)lam_reg[b];
+    const double lam = lam_reg ? (double)lam_reg[b] : 0.0;       // NULL: plain F (the lambda_hat search adds lambda g itself)
     double* Ab = A + (size_t)b * ns * ns;
 #pragma unroll
     for (int r = 0; r < 8; ++r)
@@ -267,10 +270,12 @@ __global__ void __launch_bounds__(256) pixsrc_rhs_kernel(const float* __restrict
 // ------------------------------------------------------------------------------------------------------------------
 // Cholesky, solve, regulariser: one CTA per vector, fp64
 // ------------------------------------------------------------------------------------------------------------------
-// out[b*4 + {0,1,2,3}] = {ln det A, E_S, chi2 (filled by pixsrc_model_kernel), not-positive-definite flag}
+// out[b*PX_OUT + {0,1,2,3,4}] = {ln det A, E_S, chi2 (filled by pixsrc_model_kernel), not-positive-definite flag, y^T y = D^T A^-1 D}
+// search = 1 (the lambda_hat search of Eq. 43): stop after the forward substitution -- the objective needs ln det A and y^T y only
+#define PX_OUT 6
 __global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_chol_kernel(double* __restrict__ A, const double* __restrict__ D, int ns,
                                                                       int nsx, int nsy, double* __restrict__ s_out,
-                                                                      double* __restrict__ out) {
+                                                                      double* __restrict__ out, int search) {
     extern __shared__ double px_sm[];
     double* L11 = px_sm;                         // [32][33]
     double* Pi = L11 + PX_NB * (PX_NB + 1);      // [32][PX_PP] (k-major): rows of the 64-row tile along the pitch
@@ -404,6 +409,22 @@ __global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_chol_kernel(double*
         }
         __syncthreads();
     }
+    if (search) {
+        double yy = 0.0;
+        for (int a = tid; a < ns; a += PX_CHOL_THREADS) yy += yv[a] * yv[a];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) yy += __shfl_xor_sync(0xffffffffu, yy, o);
+        if (lane == 0) red[warp] = yy;
+        __syncthreads();
+        if (tid == 0) {
+            double t = 0.0;
+            for (int w = 0; w < PX_CHOL_THREADS / 32; ++w) t += red[w];
+            out[(size_t)b * PX_OUT + 0] = logdet;
+            out[(size_t)b * PX_OUT + 3] = bad ? 1.0 : 0.0;
+            out[(size_t)b * PX_OUT + 4] = t;
+        }
+        return;
+    }
     // backward substitution L^T s = y (s overwrites yv from the end)
     const int nblk = (ns + PX_NB - 1) / PX_NB;
     for (int kb = nblk - 1; kb >= 0; --kb) {
@@ -449,9 +470,9 @@ __global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_chol_kernel(double*
     if (tid == 0) {
         double t = 0.0;
         for (int w = 0; w < PX_CHOL_THREADS / 32; ++w) t += red[w];
-        out[(size_t)b * 4 + 0] = logdet;
-        out[(size_t)b * 4 + 1] = t;
-        out[(size_t)b * 4 + 3] = bad ? 1.0 : 0.0;
+        out[(size_t)b * PX_OUT + 0] = logdet;
+        out[(size_t)b * PX_OUT + 1] = t;
+        out[(size_t)b * PX_OUT + 3] = bad ? 1.0 : 0.0;
     }
 }
 
@@ -480,7 +501,7 @@ __global__ void __launch_bounds__(256) pixsrc_model_kernel(const float* __restri
             if (w != 0.0) { const double rr = v - (double)data[p]; c2 += w * rr * rr; }
         }
     }
-    if (lane == 0 && c2 != 0.0) atomicAdd(&out[(size_t)b * 4 + 2], c2);
+    if (lane == 0 && c2 != 0.0) atomicAdd(&out[(size_t)b * PX_OUT + 2], c2);
 }
 
 // N_d and sum ln ivar over the unmasked pixels (static data; one CTA)
@@ -510,11 +531,11 @@ __global__ void pixsrc_final_kernel(const float* __restrict__ lens, const float*
     const float lam = lam_reg[b];
     bool valid = pixsrc_valid(lens + (size_t)b * GLAD_NLENS, lam, src_grid[(size_t)b * 3 + 2]);
     if (ms_lambda && !isfinite(ms_lambda[b])) valid = false;
-    const bool notpd = out[(size_t)b * 4 + 3] != 0.0;
+    const bool notpd = out[(size_t)b * PX_OUT + 3] != 0.0;
     const bool ok = valid && !notpd;
     const float inf = __int_as_float(0x7f800000), nan = __int_as_float(0x7fc00000);
     if (threadIdx.x == 0) {
-        const double c2 = out[(size_t)b * 4 + 2], es = out[(size_t)b * 4 + 1], ld = out[(size_t)b * 4 + 0];
+        const double c2 = out[(size_t)b * PX_OUT + 2], es = out[(size_t)b * PX_OUT + 1], ld = out[(size_t)b * PX_OUT + 0];
         const double ev = -0.5 * c2 - (double)lam * es - 0.5 * ld + 0.5 * ns * log((double)lam) + 0.5 * logdet_g -
                           0.5 * st[0] * 1.8378770664093454836 + 0.5 * st[1];
         if (logev) logev[b] = ok ? (float)ev : -inf;
@@ -533,15 +554,86 @@ __global__ void pixsrc_final_kernel(const float* __restrict__ lens, const float*
 // ------------------------------------------------------------------------------------------------------------------
 static inline size_t px_align(size_t n) { return (n + 255) & ~(size_t)255; }
 
-size_t pixsrc_scratch_bytes(int npix, int ns, int Bc) {
-    return px_align(sizeof(int) * (size_t)Bc * npix) + px_align(sizeof(float2) * (size_t)Bc * npix) + px_align(sizeof(int2) * (size_t)Bc * npix) +
-           px_align(sizeof(float) * (size_t)Bc * npix * ns) + px_align(sizeof(double) * (size_t)Bc * ns * ns) +
-           2 * px_align(sizeof(double) * (size_t)Bc * ns) + px_align(sizeof(double) * (size_t)Bc * 4) + px_align(sizeof(double) * 2);
+// ------------------------------------------------------------------------------------------------------------------
+// lambda_hat of Eq. 43: F and D do not depend on lambda, only the factorisation does.  With (F + lambda g) s = D,
+//   -chi2/2 - lambda E_S = -(d^T C^-1 d - D^T s)/2, so up to lambda-independent terms
+//   ln P(lambda) = J(x) = y^T y / 2 - ln det(F + e^x g) / 2 + N_s x / 2,  x = ln lambda, L y = D the forward substitution.
+// Per vector: PX_GOLD golden-section steps on [ln lam_lo, ln lam_hi] (one Cholesky each), then the vertex of the parabola through
+// the last bracket (a, better interior point, b); lambda_hat is rounded to the float32 the evidence entry takes.
+// ------------------------------------------------------------------------------------------------------------------
+#define PX_GOLD 18
+#define PX_PHI 0.6180339887498949
+struct PxSearch { double a, b, x1, x2, f1, f2, fa, fb; int which, pad; };   // which: the interior point (1 or 2) whose value is being computed
+
+// A = F + lambda g on the lower triangle
+__global__ void __launch_bounds__(256) pixsrc_shift_kernel(const double* __restrict__ F, const double* __restrict__ lam, int ns, int nsx,
+                                                           int nsy, double* __restrict__ A) {
+    const int b = blockIdx.y;
+    const size_t e = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (e >= (size_t)ns * ns) return;
+    const int i = (int)(e / ns), j = (int)(e - (size_t)i * ns);
+    if (j > i) return;
+    A[(size_t)b * ns * ns + e] = F[(size_t)b * ns * ns + e] + lam[b] * px_curv(i, j, nsx, nsy);
 }
 
+__device__ __forceinline__ double px_objective(const double* __restrict__ o, int ns, double x) {
+    if (o[3] != 0.0 || !isfinite(o[0]) || !isfinite(o[4])) return -__longlong_as_double(0x7ff0000000000000LL);   // not positive definite
+    return 0.5 * o[4] - 0.5 * o[0] + 0.5 * ns * x;
+}
+
+// step -2: set up the bracket and ask for J(a); -1: store J(a), ask J(b); 0: store J(b), ask J(x1); 1: store J(x1), ask J(x2);
+// 2..: one golden-section step per call; last: parabola vertex -> lam_hat
+__global__ void pixsrc_search_kernel(PxSearch* __restrict__ st, const double* __restrict__ out, int B, int ns, double xlo, double xhi,
+                                     int step, int last, double* __restrict__ lam_cur, float* __restrict__ lam_hat) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    PxSearch s = st[b];
+    const double* o = out + (size_t)b * PX_OUT;
+    double ask;
+    if (step == -2) {
+        s.a = xlo; s.b = xhi;
+        s.x1 = s.b - PX_PHI * (s.b - s.a); s.x2 = s.a + PX_PHI * (s.b - s.a);
+        ask = s.a;
+    } else if (step == -1) { s.fa = px_objective(o, ns, s.a); ask = s.b; }
+    else if (step == 0) { s.fb = px_objective(o, ns, s.b); ask = s.x1; }
+    else if (step == 1) { s.f1 = px_objective(o, ns, s.x1); ask = s.x2; s.which = 2; }
+    else {
+        if (s.which == 1) s.f1 = px_objective(o, ns, s.x1);
+        else s.f2 = px_objective(o, ns, s.x2);
+        if (!last) {
+            if (s.f1 > s.f2) { s.b = s.x2; s.fb = s.f2; s.x2 = s.x1; s.f2 = s.f1; s.x1 = s.b - PX_PHI * (s.b - s.a); ask = s.x1; s.which = 1; }
+            else { s.a = s.x1; s.fa = s.f1; s.x1 = s.x2; s.f1 = s.f2; s.x2 = s.a + PX_PHI * (s.b - s.a); ask = s.x2; s.which = 2; }
+        } else {
+            // vertex of the parabola through (a, fa), (m, fm), (b, fb), m = the better interior point; kept inside the bracket
+            const double m = s.f1 > s.f2 ? s.x1 : s.x2, fm = s.f1 > s.f2 ? s.f1 : s.f2;
+            double x = m;
+            const double d1 = (m - s.a) * (fm - s.fb), d2 = (m - s.b) * (fm - s.fa);
+            const double den = d1 - d2;
+            if (isfinite(s.fa) && isfinite(s.fb) && isfinite(fm) && den != 0.0) {
+                const double v = m - 0.5 * ((m - s.a) * d1 - (m - s.b) * d2) / den;
+                if (v > s.a && v < s.b) x = v;
+            }
+            lam_hat[b] = (float)exp(x);
+            ask = x;
+        }
+    }
+    lam_cur[b] = last ? (double)lam_hat[b] : exp(ask);
+    st[b] = s;
+}
+
+size_t pixsrc_scratch_bytes(int npix, int ns, int Bc, bool search) {
+    return px_align(sizeof(int) * (size_t)Bc * npix) + px_align(sizeof(float2) * (size_t)Bc * npix) + px_align(sizeof(int2) * (size_t)Bc * npix) +
+           px_align(sizeof(float) * (size_t)Bc * npix * ns) + (search ? 2 : 1) * px_align(sizeof(double) * (size_t)Bc * ns * ns) +
+           2 * px_align(sizeof(double) * (size_t)Bc * ns) + px_align(sizeof(double) * (size_t)Bc * PX_OUT) + px_align(sizeof(double) * 2) +
+           (search ? px_align(sizeof(PxSearch) * (size_t)Bc) + px_align(sizeof(double) * (size_t)Bc) + px_align(sizeof(float) * (size_t)Bc) : 0);
+}
+
+// d_lam != NULL: the evidence at the given lambda; d_lam == NULL: search lambda_hat on [lam_lo, lam_hi] first, write it to d_lam_hat
 cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens, const float* d_src_grid, const float* d_lam,
                                 const float* d_ms_lambda, int nsx, int nsy, int Bc, double logdet_g, float* d_logev, float* d_chi2,
-                                float* d_reg, float* d_s_mp, float* d_model, int32_t* d_flags) {
+                                float* d_reg, float* d_s_mp, float* d_model, int32_t* d_flags, double lam_lo, double lam_hi,
+                                float* d_lam_hat) {
+    const bool search = d_lam == nullptr;
     const int nx = c->grid.nx, ny = c->grid.ny, npix = nx * ny, ns = nsx * nsy;
     cudaStream_t st = c->stream;
     char* q = (char*)scratch;
@@ -552,11 +644,18 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
     double* A = (double*)q;        q += px_align(sizeof(double) * (size_t)Bc * ns * ns);
     double* D = (double*)q;        q += px_align(sizeof(double) * (size_t)Bc * ns);
     double* s = (double*)q;        q += px_align(sizeof(double) * (size_t)Bc * ns);
-    double* out = (double*)q;      q += px_align(sizeof(double) * (size_t)Bc * 4);
-    double* stat = (double*)q;
+    double* out = (double*)q;      q += px_align(sizeof(double) * (size_t)Bc * PX_OUT);
+    double* stat = (double*)q;     q += px_align(sizeof(double) * 2);
+    double* Fm = nullptr; PxSearch* sst = nullptr; double* lam_cur = nullptr; float* lam_f = nullptr;
+    if (search) {
+        Fm = (double*)q;           q += px_align(sizeof(double) * (size_t)Bc * ns * ns);
+        sst = (PxSearch*)q;        q += px_align(sizeof(PxSearch) * (size_t)Bc);
+        lam_cur = (double*)q;      q += px_align(sizeof(double) * (size_t)Bc);
+        lam_f = (float*)q;
+    }
     cudaError_t e;
     if ((e = cudaMemsetAsync(D, 0, sizeof(double) * (size_t)Bc * ns, st)) != cudaSuccess) return e;
-    if ((e = cudaMemsetAsync(out, 0, sizeof(double) * (size_t)Bc * 4, st)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(out, 0, sizeof(double) * (size_t)Bc * PX_OUT, st)) != cudaSuccess) return e;
 
     const int rows_per_cta = 64;
     const size_t sm_blur = sizeof(float) * (size_t)PX_BLUR_WARPS * ns;
@@ -579,23 +678,41 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
     {
         ProfScope ps(c, GK_PIX_SYRK);
         const int nt = (ns + PX_ST - 1) / PX_ST;
-        pixsrc_syrk_kernel<<<dim3(nt * (nt + 1) / 2, Bc), 256, 0, st>>>(f, c->d_ivar, rng, d_lam, npix, ns, nsx, nsy, A);
+        pixsrc_syrk_kernel<<<dim3(nt * (nt + 1) / 2, Bc), 256, 0, st>>>(f, c->d_ivar, rng, d_lam, npix, ns, nsx, nsy, search ? Fm : A);
     }
     {
         ProfScope ps(c, GK_PIX_RHS);
         const int chunks = 16;
         pixsrc_rhs_kernel<<<dim3((ns + 255) / 256, chunks, Bc), 256, 0, st>>>(f, c->d_ivar, c->d_data, npix, ns, chunks, D);
     }
+    const float* lam_use = d_lam;
+    if (search) {
+        // Eq. 43: PX_GOLD golden-section steps, each = A <- F + lambda g, Cholesky + forward substitution, bracket update; all on
+        // the stream, no host round trip
+        const dim3 gs((unsigned)(((size_t)ns * ns + 255) / 256), Bc);
+        const int last_step = 2 + PX_GOLD;
+        for (int step = -2; step <= last_step; ++step) {
+            pixsrc_search_kernel<<<(Bc + 127) / 128, 128, 0, st>>>(sst, out, Bc, ns, log(lam_lo), log(lam_hi), step, step == last_step, lam_cur, lam_f);
+            c->launches++;
+            pixsrc_shift_kernel<<<gs, 256, 0, st>>>(Fm, lam_cur, ns, nsx, nsy, A);
+            c->launches++;
+            if (step == last_step) break;
+            ProfScope ps(c, GK_PIX_CHOL);
+            pixsrc_chol_kernel<<<Bc, PX_CHOL_THREADS, sm_chol, st>>>(A, D, ns, nsx, nsy, s, out, 1);
+        }
+        lam_use = lam_f;
+        if (d_lam_hat && (e = cudaMemcpyAsync(d_lam_hat, lam_f, sizeof(float) * Bc, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return e;
+    }
     {
         ProfScope ps(c, GK_PIX_CHOL);
-        pixsrc_chol_kernel<<<Bc, PX_CHOL_THREADS, sm_chol, st>>>(A, D, ns, nsx, nsy, s, out);
+        pixsrc_chol_kernel<<<Bc, PX_CHOL_THREADS, sm_chol, st>>>(A, D, ns, nsx, nsy, s, out, 0);
     }
     {
         ProfScope ps(c, GK_PIX_MODEL);
         pixsrc_model_kernel<<<dim3((npix + 63) / 64, Bc), 256, sizeof(double) * ns, st>>>(f, s, c->d_ivar, c->d_data, npix, ns, d_model,
                                                                                           (long)npix, out);
     }
-    pixsrc_final_kernel<<<Bc, 128, 0, st>>>(d_lens, d_src_grid, d_lam, d_ms_lambda, out, stat, s, logdet_g, Bc, ns, npix, d_logev, d_chi2,
+    pixsrc_final_kernel<<<Bc, 128, 0, st>>>(d_lens, d_src_grid, lam_use, d_ms_lambda, out, stat, s, logdet_g, Bc, ns, npix, d_logev, d_chi2,
                                             d_reg, d_s_mp, d_model, d_flags);
     c->launches++;
     return cudaGetLastError();

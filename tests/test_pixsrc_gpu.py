@@ -131,3 +131,41 @@ def test_errors(glad_mod, oracle):
     g2 = glad_mod.Glad(0)
     with pytest.raises(glad_mod.GladError):
         g2.pixsrc_evidence_batch(L["params"], pin["src_grids"], pin["lam"], 8, 8)
+
+
+def test_lambda_hat_search_on_the_device(glad_mod, oracle):
+    """Eq. 43: glad_pixsrc_lambda_opt_batch against scipy's bounded maximisation of the oracle's evidence.  The optimum is flat
+    (curvature of ln P in ln lambda ~ N_s/2), so lambda_hat itself is compared at 1e-3 relative; ln P(lambda_hat) at 1e-5 (the bar of
+    a log-likelihood), and, as the strict check of the final pass, every output against the oracle evaluated AT the device's lambda_hat."""
+    from oracle import pixsrc
+    wl = workloads.make_workload("C1", oracle_data_model(oracle))
+    L = wl["lens"]
+    nsx, nsy = 12, 10
+    pin = workloads.pixsrc_inputs(wl, nsx, nsy)
+    g = glad_mod.Glad(0)
+    g.set_image_data(L["grid"], L["psf"], L["data"], L["ivar"])
+    bad = L["params"].copy(); bad[2, 3] = 3.5                          # invalid mass model: flagged, lambda_hat irrelevant
+    out = g.pixsrc_lambda_opt_batch(bad, pin["src_grids"], (1e-4, 1e4), nsx, nsy)
+    lh = out["lam_hat"].cpu().numpy()
+    ev = out["logev"].cpu().numpy().astype(np.float64)
+    fl = out["flags"].cpu().numpy()
+    assert fl[2] == glad_mod.FLAG_LENS_INVALID and np.isinf(ev[2]) and (np.delete(fl, 2) == 0).all()
+    Bm = pixsrc.blurring_matrix(L["psf"], L["grid"]["nx"], L["grid"]["ny"])
+    for b in (0, 1, 5):
+        sg = dict(nx=nsx, ny=nsy, pix=float(pin["src_grids"][b, 2]), x0=float(pin["src_grids"][b, 0]), y0=float(pin["src_grids"][b, 1]))
+        ref = pixsrc.pixsrc_lambda_opt(bad[b], L["grid"], L["psf"], L["data"], L["ivar"], sg, 1e-4, 1e4, Bm)
+        assert 1e-4 < ref["lam_hat"] < 1e4                             # an interior maximum
+        assert lh[b] == pytest.approx(ref["lam_hat"], rel=1e-3), b
+        assert ev[b] == pytest.approx(ref["logev"], rel=1e-5), b
+        at = pixsrc.pixsrc_evidence(bad[b], L["grid"], L["psf"], L["data"], L["ivar"], sg, lh[b], Bm)
+        assert ev[b] == pytest.approx(at["logev"], rel=1e-6)
+        assert out["chi2"].cpu().numpy()[b] == pytest.approx(at["chi2"], rel=1e-4)
+        assert out["reg"].cpu().numpy()[b] == pytest.approx(at["reg"], rel=1e-3)
+        s = out["s_mp"].cpu().numpy()[b]
+        assert np.max(np.abs(s - at["s_mp"])) < 2e-3 * np.abs(at["s_mp"]).max()
+    # the fixed-lambda entry at lambda_hat gives the same numbers bit for bit (same kernels after the search)
+    again = g.pixsrc_evidence_batch(bad, pin["src_grids"], lh, nsx, nsy)
+    ok = fl == 0
+    assert np.array_equal(again["logev"].cpu().numpy()[ok], out["logev"].cpu().numpy()[ok])
+    g.close()
+
