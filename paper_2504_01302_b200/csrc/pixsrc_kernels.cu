@@ -16,6 +16,7 @@
 
 #include "glad_internal.h"
 #include "glad_mass_fp64.cuh"
+#include "pixsrc_common.cuh"
 
 #define PX_MAP_THREADS 128
 #define PX_BLUR_WARPS 8
@@ -116,22 +117,6 @@ __global__ void __launch_bounds__(32 * PX_BLUR_WARPS) pixsrc_blur_kernel(const i
         for (int i = lane; i < ns; i += 32) out[i] = row[i];
         __syncwarp();
     }
-}
-
-// (T^2)[i, i'] of the (1,-2,1) second-difference matrix T with zeros outside, n points (R-P3)
-__device__ __forceinline__ double px_t2(int i, int ip, int n) {
-    const int d = i > ip ? i - ip : ip - i;
-    if (d == 0) return 4.0 + (i > 0 ? 1.0 : 0.0) + (i < n - 1 ? 1.0 : 0.0);
-    if (d == 1) return -4.0;
-    if (d == 2) return 1.0;
-    return 0.0;
-}
-__device__ __forceinline__ double px_curv(int a, int c, int nsx, int nsy) {
-    const int ja = a / nsx, ia = a - ja * nsx, jc = c / nsx, ic = c - jc * nsx;
-    double v = 0.0;
-    if (ja == jc) v += px_t2(ia, ic, nsx);
-    if (ia == ic) v += px_t2(ja, jc, nsy);
-    return v;
 }
 
 // ------------------------------------------------------------------------------------------------------------------
@@ -504,21 +489,27 @@ __global__ void __launch_bounds__(256) pixsrc_model_kernel(const float* __restri
     if (lane == 0 && c2 != 0.0) atomicAdd(&out[(size_t)b * PX_OUT + 2], c2);
 }
 
-// N_d and sum ln ivar over the unmasked pixels (static data; one CTA)
-__global__ void __launch_bounds__(256) pixsrc_static_kernel(const float* __restrict__ ivar, int npix, double* __restrict__ st) {
-    __shared__ double r1[256], r2[256];
-    double n = 0.0, sl = 0.0;
+// N_d and sum ln ivar over the unmasked pixels, max ivar and sum |psf| (the operand scales of the tensor-core contraction): static
+// data; one CTA.  st[0..3]
+__global__ void __launch_bounds__(256) pixsrc_static_kernel(const float* __restrict__ ivar, int npix, const float* __restrict__ psf,
+                                                            int ktaps, double* __restrict__ st) {
+    __shared__ double r1[256], r2[256], r3[256], r4[256];
+    double n = 0.0, sl = 0.0, wm = 0.0, ps = 0.0;
     for (int p = threadIdx.x; p < npix; p += 256) {
         const float w = ivar[p];
-        if (w > 0.f) { n += 1.0; sl += log((double)w); }
+        if (w > 0.f) { n += 1.0; sl += log((double)w); wm = fmax(wm, (double)w); }
     }
-    r1[threadIdx.x] = n; r2[threadIdx.x] = sl;
+    for (int t = threadIdx.x; t < ktaps; t += 256) ps += fabs((double)psf[t]);
+    r1[threadIdx.x] = n; r2[threadIdx.x] = sl; r3[threadIdx.x] = wm; r4[threadIdx.x] = ps;
     __syncthreads();
     for (int o = 128; o > 0; o >>= 1) {
-        if (threadIdx.x < o) { r1[threadIdx.x] += r1[threadIdx.x + o]; r2[threadIdx.x] += r2[threadIdx.x + o]; }
+        if (threadIdx.x < o) {
+            r1[threadIdx.x] += r1[threadIdx.x + o]; r2[threadIdx.x] += r2[threadIdx.x + o];
+            r3[threadIdx.x] = fmax(r3[threadIdx.x], r3[threadIdx.x + o]); r4[threadIdx.x] += r4[threadIdx.x + o];
+        }
         __syncthreads();
     }
-    if (threadIdx.x == 0) { st[0] = r1[0]; st[1] = r2[0]; }
+    if (threadIdx.x == 0) { st[0] = r1[0]; st[1] = r2[0]; st[2] = r3[0] > 0.0 ? r3[0] : 1.0; st[3] = r4[0] > 0.0 ? r4[0] : 1.0; }
 }
 
 __global__ void pixsrc_final_kernel(const float* __restrict__ lens, const float* __restrict__ src_grid, const float* __restrict__ lam_reg,
@@ -624,7 +615,7 @@ __global__ void pixsrc_search_kernel(PxSearch* __restrict__ st, const double* __
 size_t pixsrc_scratch_bytes(int npix, int ns, int Bc, bool search) {
     return px_align(sizeof(int) * (size_t)Bc * npix) + px_align(sizeof(float2) * (size_t)Bc * npix) + px_align(sizeof(int2) * (size_t)Bc * npix) +
            px_align(sizeof(float) * (size_t)Bc * npix * ns) + (search ? 2 : 1) * px_align(sizeof(double) * (size_t)Bc * ns * ns) +
-           2 * px_align(sizeof(double) * (size_t)Bc * ns) + px_align(sizeof(double) * (size_t)Bc * PX_OUT) + px_align(sizeof(double) * 2) +
+           2 * px_align(sizeof(double) * (size_t)Bc * ns) + px_align(sizeof(double) * (size_t)Bc * PX_OUT) + px_align(sizeof(double) * 4) +
            (search ? px_align(sizeof(PxSearch) * (size_t)Bc) + px_align(sizeof(double) * (size_t)Bc) + px_align(sizeof(float) * (size_t)Bc) : 0);
 }
 
@@ -645,7 +636,7 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
     double* D = (double*)q;        q += px_align(sizeof(double) * (size_t)Bc * ns);
     double* s = (double*)q;        q += px_align(sizeof(double) * (size_t)Bc * ns);
     double* out = (double*)q;      q += px_align(sizeof(double) * (size_t)Bc * PX_OUT);
-    double* stat = (double*)q;     q += px_align(sizeof(double) * 2);
+    double* stat = (double*)q;     q += px_align(sizeof(double) * 4);
     double* Fm = nullptr; PxSearch* sst = nullptr; double* lam_cur = nullptr; float* lam_f = nullptr;
     if (search) {
         Fm = (double*)q;           q += px_align(sizeof(double) * (size_t)Bc * ns * ns);
@@ -654,7 +645,6 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
         lam_f = (float*)q;
     }
     cudaError_t e;
-    if ((e = cudaMemsetAsync(D, 0, sizeof(double) * (size_t)Bc * ns, st)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(out, 0, sizeof(double) * (size_t)Bc * PX_OUT, st)) != cudaSuccess) return e;
 
     const int rows_per_cta = 64;
@@ -663,7 +653,7 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
     if (sm_blur > 227 * 1024 || sm_chol > 227 * 1024) return cudaErrorInvalidConfiguration;
     if ((e = smem_optin(c, pixsrc_blur_kernel)) != cudaSuccess) return e;
     if ((e = smem_optin(c, pixsrc_chol_kernel)) != cudaSuccess) return e;
-    pixsrc_static_kernel<<<1, 256, 0, st>>>(c->d_ivar, npix, stat);
+    pixsrc_static_kernel<<<1, 256, 0, st>>>(c->d_ivar, npix, c->d_psf, c->kpsf * c->kpsf, stat);
     c->launches++;
     {
         ProfScope ps(c, GK_PIX_MAP);
@@ -676,14 +666,9 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
             idx, wgt, c->d_psf, c->kpsf, nx, ny, nsx, ns, rows_per_cta, f, rng);
     }
     {
+        // F (+ lambda g) and D in one pass over f on the tensor cores (pixsrc_syrk_tc.cu)
         ProfScope ps(c, GK_PIX_SYRK);
-        const int nt = (ns + PX_ST - 1) / PX_ST;
-        pixsrc_syrk_kernel<<<dim3(nt * (nt + 1) / 2, Bc), 256, 0, st>>>(f, c->d_ivar, rng, d_lam, npix, ns, nsx, nsy, search ? Fm : A);
-    }
-    {
-        ProfScope ps(c, GK_PIX_RHS);
-        const int chunks = 16;
-        pixsrc_rhs_kernel<<<dim3((ns + 255) / 256, chunks, Bc), 256, 0, st>>>(f, c->d_ivar, c->d_data, npix, ns, chunks, D);
+        if ((e = launch_pixsrc_syrk_tc(c, st, f, rng, d_lam, npix, ns, nsx, nsy, Bc, stat, search ? Fm : A, D)) != cudaSuccess) return e;
     }
     const float* lam_use = d_lam;
     if (search) {
