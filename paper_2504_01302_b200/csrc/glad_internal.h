@@ -239,7 +239,7 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
                                 float* d_lam_hat);
 // F = f^T C_d^-1 f (+ lambda g, lower triangle, fp64 out) and D = f^T C_d^-1 d on tcgen05 (pixsrc_syrk_tc.cu); d_lam NULL = plain F
 cudaError_t launch_pixsrc_syrk_tc(glad_ctx* c, cudaStream_t st, const float* f, const int2* rng, const float* d_lam, int npix, int ns,
-                                  int nsx, int nsy, int Bc, const double* stat, double* A, double* D);
+                                  int nsx, int nsy, int Bc, const double* stat, unsigned short* rowlist, double* A, double* D);
 // tensor-core (tcgen05) form of row a6; supported when the folded grid has ny_f <= 128, N = terms * nx_f <= 256
 // and two operand stages fit in shared memory
 bool jam_quad_tc_supported(const glad_ctx* c, int nl, int nmx);

@@ -4,9 +4,8 @@
 //                              L is kept as its <= 4 non-zeros per row ({top-left source pixel, (fx, fy)}), never dense
 //   pixsrc_blur_kernel   f = B L (Eq. 38): a warp per image pixel scatters PSF tap x bilinear weight into a shared-memory row
 //                              of N_s floats and streams the row out (f [N_pix, N_s] fp32, the one large intermediate)
-//   pixsrc_syrk_kernel   F = f^T C_d^-1 f (Eq. 41) + lambda g  -> A (lower triangle, fp64 store): 128 x 128 output tiles,
-//                              8 x 8 register tiles, fp32 FFMA over the N_pix contraction
-//   pixsrc_rhs_kernel    D = f^T C_d^-1 d (Eq. 42), fp64 accumulation
+//   pixsrc_syrk_tc_kernel (pixsrc_syrk_tc.cu)  F = f^T C_d^-1 f (Eq. 41) + lambda g -> A (lower triangle, fp64 store) and
+//                              D = f^T C_d^-1 d (Eq. 42): tcgen05 MMAs on two-term fp16 operands, 128 x 128 output tiles
 //   pixsrc_chol_kernel   A = L L^T in fp64 (blocked right-looking, one CTA per vector), ln det A, s_MP = A^-1 D (Eq. 40),
 //                              E_S = 1/2 s^T g s from its pixel definition
 //   pixsrc_model_kernel  f s_MP (Eq. 37) and chi^2 = sum ivar (f s - d)^2, a warp per image pixel
@@ -21,7 +20,6 @@
 #define PX_MAP_THREADS 128
 #define PX_BLUR_WARPS 8
 #define PX_TILE 64
-#define PX_BK 16
 #define PX_NB 32           // Cholesky panel width
 #define PX_CHOL_THREADS 256
 #define PX_PP 65           // pitch (doubles) of the k-major panel tiles in shared memory: conflict-free transposed stores
@@ -119,138 +117,7 @@ __global__ void __launch_bounds__(32 * PX_BLUR_WARPS) pixsrc_blur_kernel(const i
     }
 }
 
-// ------------------------------------------------------------------------------------------------------------------
-// A = f^T diag(ivar) f + lambda g, lower triangle, 128 x 128 output tiles, 8 x 8 register tiles (as four 4 x 4 quadrants 64 apart,
-// so that every LDS.128 of a quarter-warp is contiguous): 4 LDS.128 per 64 FFMA
-// ------------------------------------------------------------------------------------------------------------------
-#define PX_ST 128
-__device__ __forceinline__ void px_cp_async16(void* smem, const void* gmem) {
-    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void px_cp_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-__device__ __forceinline__ void px_cp_wait1() { asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
-
-// Two shared-memory stages filled by cp.async (no staging registers): chunk c+1 streams in while chunk c is contracted.  ivar
-// stays out of the copies: row k of a chunk is scaled by Ws[k] when the a operand is read (and skipped when Ws[k] = 0).
-__global__ void __launch_bounds__(256, 2) pixsrc_syrk_kernel(const float* __restrict__ f, const float* __restrict__ ivar,
-                                                             const int2* __restrict__ rng, const float* __restrict__ lam_reg, int npix,
-                                                             int ns, int nsx, int nsy, double* __restrict__ A) {
-    __shared__ __align__(16) float As[2][PX_BK][PX_ST];
-    __shared__ __align__(16) float Bs[2][PX_BK][PX_ST];
-    __shared__ float Ws[2][PX_BK];
-    const int b = blockIdx.y;
-    // tile pair (ti >= tj) from the linear index
-    int ti = (int)((sqrtf(8.f * (float)blockIdx.x + 1.f) - 1.f) * 0.5f);
-    while ((ti + 1) * (ti + 2) / 2 <= (int)blockIdx.x) ++ti;
-    while (ti * (ti + 1) / 2 > (int)blockIdx.x) --ti;
-    const int tj = blockIdx.x - ti * (ti + 1) / 2;
-    const int i0 = ti * PX_ST, j0 = tj * PX_ST;
-    const float* fb = f + (size_t)b * npix * ns;
-    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
-    const int lr = tid >> 4, lc = (tid & 15) * 8;      // staging: row of the K-chunk, 8 consecutive columns
-    const bool vec4 = (ns & 3) == 0;
-    const int2* rb = rng + (size_t)b * npix;
-    float acc[8][8];
-#pragma unroll
-    for (int r = 0; r < 8; ++r)
-#pragma unroll
-        for (int c = 0; c < 8; ++c) acc[r][c] = 0.f;
-
-    // A row of f is non-zero only on [lo, hi] (the PSF footprint mapped into the source plane, recorded by the blur kernel): a row
-    // that misses either column tile contributes nothing to this output tile; it is stored as zeros with weight 0, and a chunk
-    // of PX_BK image pixels without any hit is skipped altogether (uniform decision).
-    auto fill = [&](int st, int p0) -> bool {
-        const int p = p0 + lr;
-        float w = 0.f;
-        bool hit = false;
-        if (p < npix) {
-            w = ivar[p];
-            const int2 r = rb[p];
-            hit = (w != 0.f) && r.x <= i0 + PX_ST - 1 && r.y >= i0 && r.x <= j0 + PX_ST - 1 && r.y >= j0;
-        }
-        if ((tid & 15) == 0) Ws[st][lr] = hit ? w : 0.f;
-        float* as = &As[st][lr][lc];
-        float* bs = &Bs[st][lr][lc];
-        const float* rowp = fb + (size_t)p * ns;
-        const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int ca = i0 + lc + 4 * h, cb = j0 + lc + 4 * h;
-            if (hit && vec4 && ca < ns) px_cp_async16(as + 4 * h, rowp + ca);
-            else if (hit && !vec4) {
-                float v[4];
-#pragma unroll
-                for (int e = 0; e < 4; ++e) v[e] = (ca + e < ns) ? rowp[ca + e] : 0.f;
-                *reinterpret_cast<float4*>(as + 4 * h) = make_float4(v[0], v[1], v[2], v[3]);
-            } else *reinterpret_cast<float4*>(as + 4 * h) = z;
-            if (hit && vec4 && cb < ns) px_cp_async16(bs + 4 * h, rowp + cb);
-            else if (hit && !vec4) {
-                float v[4];
-#pragma unroll
-                for (int e = 0; e < 4; ++e) v[e] = (cb + e < ns) ? rowp[cb + e] : 0.f;
-                *reinterpret_cast<float4*>(bs + 4 * h) = make_float4(v[0], v[1], v[2], v[3]);
-            } else *reinterpret_cast<float4*>(bs + 4 * h) = z;
-        }
-        return hit;
-    };
-
-    const int nch = (npix + PX_BK - 1) / PX_BK;
-    bool hit_cur = fill(0, 0);
-    px_cp_commit();
-    for (int ch = 0; ch < nch; ++ch) {
-        const int st = ch & 1;
-        bool hit_nxt = false;
-        if (ch + 1 < nch) hit_nxt = fill(st ^ 1, (ch + 1) * PX_BK);
-        px_cp_commit();
-        px_cp_wait1();                                   // this thread's copies of chunk ch have landed
-        if (__syncthreads_or(hit_cur)) {                 // ... and after the barrier everybody's have
-#pragma unroll 2
-            for (int k = 0; k < PX_BK; ++k) {
-                const float wk = Ws[st][k];
-                if (wk == 0.f) continue;                 // uniform: a row that does not count
-                const float4 a0 = *reinterpret_cast<const float4*>(&As[st][k][ty * 4]);
-                const float4 a1 = *reinterpret_cast<const float4*>(&As[st][k][64 + ty * 4]);
-                const float4 b0 = *reinterpret_cast<const float4*>(&Bs[st][k][tx * 4]);
-                const float4 b1 = *reinterpret_cast<const float4*>(&Bs[st][k][64 + tx * 4]);
-                const float ar[8] = {wk * a0.x, wk * a0.y, wk * a0.z, wk * a0.w, wk * a1.x, wk * a1.y, wk * a1.z, wk * a1.w};
-                const float br[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
-#pragma unroll
-                for (int r = 0; r < 8; ++r)
-#pragma unroll
-                    for (int c = 0; c < 8; ++c) acc[r][c] = fmaf(ar[r], br[c], acc[r][c]);
-            }
-            __syncthreads();                             // stage st is refilled two chunks from now
-        }
-        hit_cur = hit_nxt;
-    }
-    const double lam = lam_reg ? (double)lam_reg[b] : 0.0;       // NULL: plain F (the lambda_hat search adds lambda g itself)
-    double* Ab = A + (size_t)b * ns * ns;
-#pragma unroll
-    for (int r = 0; r < 8; ++r)
-#pragma unroll
-        for (int c = 0; c < 8; ++c) {
-            const int i = i0 + (r >> 2) * 64 + ty * 4 + (r & 3), j = j0 + (c >> 2) * 64 + tx * 4 + (c & 3);
-            if (i < ns && j <= i) Ab[(size_t)i * ns + j] = (double)acc[r][c] + lam * px_curv(i, j, nsx, nsy);
-        }
-}
-
-// D = f^T (ivar d): thread per source pixel, the image pixels split over blockIdx.y
-__global__ void __launch_bounds__(256) pixsrc_rhs_kernel(const float* __restrict__ f, const float* __restrict__ ivar,
-                                                         const float* __restrict__ data, int npix, int ns, int chunks,
-                                                         double* __restrict__ D) {
-    const int b = blockIdx.z, i = blockIdx.x * 256 + threadIdx.x;
-    if (i >= ns) return;
-    const int per = (npix + chunks - 1) / chunks;
-    const int pa = blockIdx.y * per, pb = min(npix, pa + per);
-    const float* fb = f + (size_t)b * npix * ns;
-    double acc = 0.0;
-    for (int p = pa; p < pb; ++p) {
-        const float w = ivar[p];
-        if (w != 0.f) acc += (double)(w * data[p]) * (double)fb[(size_t)p * ns + i];
-    }
-    atomicAdd(&D[(size_t)b * ns + i], acc);
-}
+// F = f^T C_d^-1 f (+ lambda g) and D = f^T C_d^-1 d: pixsrc_syrk_tc.cu (tcgen05)
 
 // ------------------------------------------------------------------------------------------------------------------
 // Cholesky, solve, regulariser: one CTA per vector, fp64
@@ -612,11 +479,13 @@ __global__ void pixsrc_search_kernel(PxSearch* __restrict__ st, const double* __
     st[b] = s;
 }
 
+static inline size_t px_ntiles(int ns) { const size_t nt = (ns + 127) / 128; return nt * (nt + 1) / 2; }   // output tiles of the contraction
 size_t pixsrc_scratch_bytes(int npix, int ns, int Bc, bool search) {
     return px_align(sizeof(int) * (size_t)Bc * npix) + px_align(sizeof(float2) * (size_t)Bc * npix) + px_align(sizeof(int2) * (size_t)Bc * npix) +
            px_align(sizeof(float) * (size_t)Bc * npix * ns) + (search ? 2 : 1) * px_align(sizeof(double) * (size_t)Bc * ns * ns) +
            2 * px_align(sizeof(double) * (size_t)Bc * ns) + px_align(sizeof(double) * (size_t)Bc * PX_OUT) + px_align(sizeof(double) * 4) +
-           (search ? px_align(sizeof(PxSearch) * (size_t)Bc) + px_align(sizeof(double) * (size_t)Bc) + px_align(sizeof(float) * (size_t)Bc) : 0);
+           (search ? px_align(sizeof(PxSearch) * (size_t)Bc) + px_align(sizeof(double) * (size_t)Bc) + px_align(sizeof(float) * (size_t)Bc) : 0) +
+           px_align(sizeof(unsigned short) * (size_t)Bc * px_ntiles(ns) * npix);
 }
 
 // d_lam != NULL: the evidence at the given lambda; d_lam == NULL: search lambda_hat on [lam_lo, lam_hi] first, write it to d_lam_hat
@@ -642,8 +511,9 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
         Fm = (double*)q;           q += px_align(sizeof(double) * (size_t)Bc * ns * ns);
         sst = (PxSearch*)q;        q += px_align(sizeof(PxSearch) * (size_t)Bc);
         lam_cur = (double*)q;      q += px_align(sizeof(double) * (size_t)Bc);
-        lam_f = (float*)q;
+        lam_f = (float*)q;         q += px_align(sizeof(float) * (size_t)Bc);
     }
+    unsigned short* rowlist = (unsigned short*)q;
     cudaError_t e;
     if ((e = cudaMemsetAsync(out, 0, sizeof(double) * (size_t)Bc * PX_OUT, st)) != cudaSuccess) return e;
 
@@ -668,7 +538,7 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
     {
         // F (+ lambda g) and D in one pass over f on the tensor cores (pixsrc_syrk_tc.cu)
         ProfScope ps(c, GK_PIX_SYRK);
-        if ((e = launch_pixsrc_syrk_tc(c, st, f, rng, d_lam, npix, ns, nsx, nsy, Bc, stat, search ? Fm : A, D)) != cudaSuccess) return e;
+        if ((e = launch_pixsrc_syrk_tc(c, st, f, rng, d_lam, npix, ns, nsx, nsy, Bc, stat, rowlist, search ? Fm : A, D)) != cudaSuccess) return e;
     }
     const float* lam_use = d_lam;
     if (search) {

@@ -12,9 +12,10 @@
 // tensor core adds into TMEM with truncation, so the K loop is cut into groups of SY_FL chunks (512 pixels) that alternate between
 // two TMEM buffers and are added into fp32 registers with ordinary round-to-nearest FADDs.
 //
-// CTA = (vector, 128 x 128 output tile of the lower triangle), 512 threads, one CTA per SM.  A pre-pass lists the chunks of 32
-// image pixels that count for the tile (some f row touches both column blocks: the PSF footprint recorded by the blur kernel; the
-// rest, about half, is skipped).  The raw fp32 columns of a listed chunk are copied into a 3-slot shared-memory ring by cp.async
+// CTA = (vector, 128 x 128 output tile of the lower triangle), 512 threads, one CTA per SM.  A pre-pass lists the image pixels that
+// count for the tile (the f row touches both column blocks: the PSF footprint recorded by the blur kernel) -- about a third of them;
+// the sum over pixels can be taken in any order, so only the listed rows are contracted, 32 at a time ("chunk"; skipping whole
+// chunks of consecutive pixels instead removes only ~45 %).  The raw fp32 columns of a chunk are gathered into a 3-slot ring by cp.async
 // two chunks ahead (the first version loaded them into registers at the point of use: 33 ms per 296 vectors, latency-bound with
 // 16 warps per SM).  All threads then convert: thread = (side A/B, column, half of the chunk's pixel octs) reads its 8 pixels of one
 // column from the ring (conflict-free), applies ivar (A side), splits, and writes one 16-byte core-matrix row per term into the
@@ -29,7 +30,6 @@
 #define SY_FL 16                 // chunks per TMEM accumulator group (512 pixels)
 #define SY_RAW 3                 // ring of raw fp32 chunks (cp.async runs two chunks ahead)
 #define SY_RAW_BYTES (2 * SY_KC * SY_T * 4)      // A-side and B-side columns of one chunk: 32 KB
-#define SY_MAXCH ((GLAD_MAX_IMAGE_PIXELS + SY_KC - 1) / SY_KC)
 #define SY_THREADS 512
 #define SY_A_BYTES (SY_T * SY_KC * 2)            // one bf16 term of the A tile: 16 KB
 #define SY_B_BYTES (2 * SY_T * SY_KC * 2)        // [B1 | B2]: 32 KB
@@ -87,15 +87,13 @@ __device__ __forceinline__ void sy_split(float (&v)[8], uint4& hi, uint4& lo) {
 __global__ void __launch_bounds__(SY_THREADS, 1) pixsrc_syrk_tc_kernel(const float* __restrict__ f, const float* __restrict__ ivar,
                                                                       const float* __restrict__ data, const int2* __restrict__ rng,
                                                                       const float* __restrict__ lam_reg, const double* __restrict__ stat,
-                                                                      int npix, int ns, int nsx, int nsy, double* __restrict__ A,
-                                                                      double* __restrict__ Dv) {
+                                                                      int npix, int ns, int nsx, int nsy, unsigned short* __restrict__ rowlist,
+                                                                      double* __restrict__ A, double* __restrict__ Dv) {
     extern __shared__ __align__(128) unsigned char sy_sm[];
     __shared__ __align__(8) uint64_t s_bar[3];           // stage 0, stage 1, done
     __shared__ uint32_t s_tmem;
-    __shared__ float s_w[SY_RAW][SY_KC], s_wd[SY_RAW][SY_KC];   // sA * ivar and ivar * data of the staged chunks' pixels
-    __shared__ unsigned char s_flag[SY_MAXCH];
-    __shared__ unsigned short s_list[SY_MAXCH];          // the chunks that count for this tile, in order
-    __shared__ int s_nrel;
+    __shared__ float s_w[SY_THREADS / 32][SY_RAW][16], s_wd[SY_THREADS / 32][SY_RAW][16];   // per warp: sA * ivar, ivar * data of its 16 rows
+    __shared__ int s_cnt[SY_THREADS / 32], s_nrows;
     __shared__ double s_d[2 * SY_T];
     const int b = blockIdx.y, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     int ti = (int)((sqrtf(8.f * (float)blockIdx.x + 1.f) - 1.f) * 0.5f);
@@ -163,59 +161,79 @@ __global__ void __launch_bounds__(SY_THREADS, 1) pixsrc_syrk_tc_kernel(const flo
     const uint32_t idesc256 = idesc_base | ((256u >> 3) << 17), idesc128 = idesc_base | ((128u >> 3) << 17);
     const uint32_t sm_base = sy_smem_u32(sy_sm);
 
-    // ---- which chunks of SY_KC pixels count for this tile?  (some pixel with ivar != 0 whose f row touches both column blocks)
-    const int nch = (npix + SY_KC - 1) / SY_KC;
-    for (int ch = tid; ch < nch; ch += SY_THREADS) s_flag[ch] = 0;
-    __syncthreads();
-    for (int p = tid; p < npix; p += SY_THREADS) {
-        const int2 r = rb[p];
-        if (ivar[p] != 0.f && r.x <= i0 + SY_T - 1 && r.y >= i0 && r.x <= j0 + SY_T - 1 && r.y >= j0) s_flag[p / SY_KC] = 1;
-    }
-    __syncthreads();
-    if (warp == 0) {
+    // ---- which image pixels count for this tile?  (ivar != 0 and the f row touches both column blocks: about a third of them.)  The
+    // contraction is a sum over pixels in any order, so the rows that count are COMPACTED: listed in ascending order (two passes per
+    // warp over its segment of the image: count, then write at the prefix offset) and consumed SY_KC at a time.
+    unsigned short* list = rowlist + ((size_t)b * gridDim.x + blockIdx.x) * npix;
+    {
+        const int seg = (((npix + SY_THREADS / 32 - 1) / (SY_THREADS / 32)) + 31) & ~31;
+        const int pa = warp * seg, pb = min(npix, pa + seg);
+        auto hits = [&](int p) -> bool {
+            if (p >= pb) return false;
+            const int2 r = rb[p];
+            return ivar[p] != 0.f && r.x <= i0 + SY_T - 1 && r.y >= i0 && r.x <= j0 + SY_T - 1 && r.y >= j0;
+        };
         int cnt = 0;
-        for (int base = 0; base < nch; base += 32) {
-            const bool fl = base + lane < nch && s_flag[base + lane];
-            const unsigned m = __ballot_sync(0xffffffffu, fl);
-            if (fl) s_list[cnt + __popc(m & ((1u << lane) - 1u))] = (unsigned short)(base + lane);
-            cnt += __popc(m);
+        for (int p = pa; p < pb; p += 32) cnt += __popc(__ballot_sync(0xffffffffu, hits(p + lane)));
+        if (lane == 0) s_cnt[warp] = cnt;
+        __syncthreads();
+        int off = 0;
+        for (int w = 0; w < warp; ++w) off += s_cnt[w];
+        for (int p = pa; p < pb; p += 32) {
+            const bool h = hits(p + lane);
+            const unsigned m = __ballot_sync(0xffffffffu, h);
+            if (h) list[off + __popc(m & ((1u << lane) - 1u))] = (unsigned short)(p + lane);
+            off += __popc(m);
         }
-        if (lane == 0) s_nrel = cnt;
+        if (tid == SY_THREADS - 1) s_nrows = off;
+        __syncthreads();                                 // also makes the list (global memory, written by this CTA) visible to the CTA
     }
-    __syncthreads();
-    const int nrel = s_nrel;
+    const int nrows = s_nrows, nrel = (nrows + SY_KC - 1) / SY_KC;
 
-    // ---- raw fp32 tiles of f: ring of SY_RAW chunks filled by cp.async two chunks ahead of the conversion
+    // ---- raw fp32 tiles of f: ring of SY_RAW chunks filled by cp.async two chunks ahead of the conversion.  Every WARP copies
+    // exactly the 16 pixel rows x 32 columns it converts (four 16-byte pieces per lane), so a __syncwarp orders copy and use and the
+    // ring needs no CTA-wide barrier.
     unsigned char* raw_base = sy_sm + 2 * (size_t)SY_STAGE_BYTES;
     const bool vec4 = (ns & 3) == 0;
-    auto stage_raw = [&](int idx) {                      // chunk s_list[idx] -> ring slot idx % SY_RAW (idx >= nrel: nothing)
-        if (idx < nrel) {
-            const int slot = idx % SY_RAW, p0 = (int)s_list[idx] * SY_KC;
-            float* rawp = reinterpret_cast<float*>(raw_base + (size_t)slot * SY_RAW_BYTES);
+    const int col0 = (side ? j0 : i0) + 32 * (warp & 3);                 // first column of this warp
+    // the lane's four pieces: fixed (row of the chunk, 4-column segment) inside the warp's block.  A chunk row past the end of the
+    // list is read from pixel 0 with A-side weight 0, so it adds nothing.
+    int prow[4], pcol[4];
+    unsigned fastmask = 0;
 #pragma unroll
-            for (int it = 0; it < (2 * SY_KC * 32) / SY_THREADS; ++it) {
-                const int q = tid + it * SY_THREADS;
-                const int sd = q / (SY_KC * 32), row = (q / 32) % SY_KC, seg = q & 31;
-                const int cc = (sd ? j0 : i0) + seg * 4, pp = p0 + row;
-                float* dst = rawp + (sd * SY_KC + row) * SY_T + seg * 4;
-                const float* src = fb + (size_t)pp * ns + cc;
-                if (pp < npix && vec4 && cc + 3 < ns) px_cp_async16(dst, src);
+    for (int it = 0; it < 4; ++it) {
+        const int piece = lane + 32 * it;
+        prow[it] = piece >> 3;                           // 0..15 within the warp's 16 rows
+        pcol[it] = col0 + (piece & 7) * 4;
+        if (vec4 && pcol[it] + 3 < ns) fastmask |= 1u << it;
+    }
+    float* const raw_warp = reinterpret_cast<float*>(raw_base) + (side * SY_KC + og * 16) * SY_T + 32 * (warp & 3);
+    auto stage_raw = [&](int idx) {                      // rows idx*SY_KC.. of the list -> ring slot idx % SY_RAW (idx >= nrel: nothing)
+        if (idx < nrel) {
+            const int slot = idx % SY_RAW;
+            const int li = idx * SY_KC + og * 16 + (lane & 15);              // lanes 0..15 (and 16..31 again): the warp's 16 rows
+            const bool have = li < nrows;
+            const int pid = have ? (int)list[li] : 0;
+            float* rawp = raw_warp + (size_t)slot * (SY_RAW_BYTES / 4);
+#pragma unroll
+            for (int it = 0; it < 4; ++it) {
+                const int pp = __shfl_sync(0xffffffffu, pid, prow[it]);
+                float* dst = rawp + prow[it] * SY_T + (pcol[it] - col0);
+                const float* src = fb + (size_t)pp * ns + pcol[it];
+                if (fastmask & (1u << it)) px_cp_async16(dst, src);
                 else {
                     float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-                    if (pp < npix) {
-                        if (cc < ns) z.x = src[0];
-                        if (cc + 1 < ns) z.y = src[1];
-                        if (cc + 2 < ns) z.z = src[2];
-                        if (cc + 3 < ns) z.w = src[3];
-                    }
+                    if (pcol[it] < ns) z.x = src[0];
+                    if (pcol[it] + 1 < ns) z.y = src[1];
+                    if (pcol[it] + 2 < ns) z.z = src[2];
+                    if (pcol[it] + 3 < ns) z.w = src[3];
                     *reinterpret_cast<float4*>(dst) = z;
                 }
             }
-            if (tid < SY_KC) {
-                const int pp = p0 + tid;
-                const float w = pp < npix ? ivar[pp] : 0.f;
-                s_w[slot][tid] = w * sA;
-                s_wd[slot][tid] = pp < npix ? w * data[pp] : 0.f;
+            if (side == 0 && lane < 16) {
+                const float w = have ? ivar[pid] : 0.f;
+                s_w[warp][slot][lane] = w * sA;
+                s_wd[warp][slot][lane] = (diag && have) ? w * data[pid] : 0.f;
             }
         }
         asm volatile("cp.async.commit_group;\n" ::: "memory");
@@ -233,20 +251,20 @@ __global__ void __launch_bounds__(SY_THREADS, 1) pixsrc_syrk_tc_kernel(const flo
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             while ((gf + 1) * SY_FL - 1 <= n - 2) flush(gf++);
         }
-        __syncthreads();                                 // everybody's copies of chunk n have landed; s_w, s_wd visible
+        __syncwarp();                                    // this warp's copies of chunk n have landed; its weights are visible
         unsigned char* stage = sy_sm + (size_t)st * SY_STAGE_BYTES;
-        const float* rawc = reinterpret_cast<const float*>(raw_base + (size_t)slot * SY_RAW_BYTES) + side * SY_KC * SY_T + c;
+        const float* rawc = raw_warp + (size_t)slot * (SY_RAW_BYTES / 4) + lane;
 #pragma unroll
         for (int oo = 0; oo < SY_KC / 16; ++oo) {
             const int o = og * (SY_KC / 16) + oo;
             float v[8];
 #pragma unroll
-            for (int k = 0; k < 8; ++k) v[k] = rawc[(o * 8 + k) * SY_T];
+            for (int k = 0; k < 8; ++k) v[k] = rawc[(oo * 8 + k) * SY_T];
             if (side == 0) {
 #pragma unroll
                 for (int k = 0; k < 8; ++k) {
-                    if (diag) dsum = fma((double)v[k], (double)s_wd[slot][o * 8 + k], dsum);
-                    v[k] *= s_w[slot][o * 8 + k];
+                    if (diag) dsum = fma((double)v[k], (double)s_wd[warp][slot][oo * 8 + k], dsum);
+                    v[k] *= s_w[warp][slot][oo * 8 + k];
                 }
             } else {
 #pragma unroll
@@ -316,11 +334,11 @@ __global__ void __launch_bounds__(SY_THREADS, 1) pixsrc_syrk_tc_kernel(const flo
 }
 
 cudaError_t launch_pixsrc_syrk_tc(glad_ctx* c, cudaStream_t st, const float* f, const int2* rng, const float* d_lam, int npix, int ns,
-                                  int nsx, int nsy, int Bc, const double* stat, double* A, double* D) {
+                                  int nsx, int nsy, int Bc, const double* stat, unsigned short* rowlist, double* A, double* D) {
     const size_t smem = 2 * (size_t)SY_STAGE_BYTES + SY_RAW * (size_t)SY_RAW_BYTES;
     cudaError_t e = smem_optin(c, pixsrc_syrk_tc_kernel);
     if (e != cudaSuccess) return e;
     const int nt = (ns + SY_T - 1) / SY_T;
-    pixsrc_syrk_tc_kernel<<<dim3(nt * (nt + 1) / 2, Bc), SY_THREADS, smem, st>>>(f, c->d_ivar, c->d_data, rng, d_lam, stat, npix, ns, nsx, nsy, A, D);
+    pixsrc_syrk_tc_kernel<<<dim3(nt * (nt + 1) / 2, Bc), SY_THREADS, smem, st>>>(f, c->d_ivar, c->d_data, rng, d_lam, stat, npix, ns, nsx, nsy, rowlist, A, D);
     return cudaGetLastError();
 }
