@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libglad.so")
-SOURCES = ["glad_api.cu", "lens_kernels.cu", "jam_prep_post.cu", "jam_quad.cu", "jam_quad_tc.cu", "jam_sph.cu", "mge_kernels.cu", "quasar_kernels.cu", "pixsrc_kernels.cu", "pixsrc_syrk_tc.cu"]
+SOURCES = ["glad_api.cu", "lens_kernels.cu", "jam_prep_post.cu", "jam_quad.cu", "jam_quad_tc.cu", "jam_sph.cu", "mge_kernels.cu", "quasar_kernels.cu", "pixsrc_kernels.cu", "pixsrc_syrk_tc.cu", "pixsrc_chol.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "shared"]
 

@@ -240,6 +240,9 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
 // F = f^T C_d^-1 f (+ lambda g, lower triangle, fp64 out) and D = f^T C_d^-1 d on tcgen05 (pixsrc_syrk_tc.cu); d_lam NULL = plain F
 cudaError_t launch_pixsrc_syrk_tc(glad_ctx* c, cudaStream_t st, const float* f, const int2* rng, const float* d_lam, int npix, int ns,
                                   int nsx, int nsy, int Bc, const double* stat, unsigned short* rowlist, double* A, double* D);
+// batched Cholesky of the Bc matrices A [ns, ns] (lower triangle, in place; pixsrc_chol.cu); out[b*6+0] = ln det, out[b*6+3] = not-PD flag
+size_t pixsrc_factor_scratch_bytes(int Bc);
+cudaError_t launch_pixsrc_factor(glad_ctx* c, cudaStream_t st, double* A, int ns, int Bc, double* out, double* Winv);
 // tensor-core (tcgen05) form of row a6; supported when the folded grid has ny_f <= 128, N = terms * nx_f <= 256
 // and two operand stages fit in shared memory
 bool jam_quad_tc_supported(const glad_ctx* c, int nl, int nmx);

@@ -265,7 +265,7 @@ __global__ void __launch_bounds__(512, 2) lens_image_kernel(const float* __restr
                                                          const float2* __restrict__ cse, int ncse) {
     extern __shared__ __align__(16) float smem[];
     const int b = blockIdx.x, tid = threadIdx.x, nthr = blockDim.x;
-    const int nx = g.nx, ny = g.ny, npx = nx * ny, ss = g.supersample;
+    const int nx = g.nx, ny = g.ny, npx = nx * ny;
     const int KP = lens_tap_pitch(kpsf), HL = lens_halo_left(kpsf), pitch = lens_img_pitch(nx, kpsf);
     float* c = smem;                       // LC_SIZE
     float* spsf = smem + LC_SIZE;          // kpsf rows x KP taps, zero padded

@@ -1,0 +1,203 @@
+// Batched Cholesky factorisation A = L L^T (fp64, lower triangle in place) of the B matrices F + lambda g of the pixelated-source
+// likelihood (Eq. 40, 43), N_s = 100 .. 4096.  Right-looking, panel width 64, THREE kernels per panel over the whole
+// batch instead of one CTA per matrix:
+//   chol_diag_kernel    CTA per matrix: the 64 x 64 diagonal block in shared memory; ln det and the not-positive-definite flag
+//                       and W = L11^-1
+//   chol_trsm_kernel    CTA per (64 rows below the block, matrix): L21 = A21 W^T as a 64 x 64 x 64 tile product
+//   chol_update_kernel  CTA per (row of 64 x 64 tiles of the trailing lower triangle, matrix): A22 -= L21 L21^T, 4 x 4 doubles per
+//                       thread, the panel tiles streamed through shared memory by cp.async
+// The version this replaces ran the whole factorisation in one CTA per matrix (profiles/r1e.md: fp64 pipe 20 % active, 12 TFLOP/s,
+// and at the paper's 64 x 64 source grid only 54 matrices fit the scratch, so 54 CTAs on 148 SMs: 2.47 s per 296 matrices).
+// Here every trailing update is a grid of (tiles x matrices) CTAs whatever the batch size.
+#include <math.h>
+
+#include "glad_internal.h"
+
+#define CH_NB 64
+#define CH_P 65            // pitch (doubles) of the shared-memory tiles
+#define CH_OUT 6           // doubles per vector in `out` (pixsrc_kernels.cu PX_OUT): [0] ln det A, [3] not-positive-definite flag
+
+__global__ void __launch_bounds__(256) chol_diag_kernel(double* __restrict__ A, int ns, int k0, double* __restrict__ out,
+                                                        double* __restrict__ Winv) {
+    __shared__ double L[CH_NB * CH_P];
+    __shared__ double s_ld;
+    __shared__ int s_bad;
+    const int b = blockIdx.x, tid = threadIdx.x;
+    double* Ab = A + (size_t)b * ns * ns;
+    const int nb = min(CH_NB, ns - k0);
+    if (tid == 0) { s_ld = 0.0; s_bad = 0; }
+    for (int e = tid; e < CH_NB * CH_NB; e += 256) {
+        const int r = e >> 6, c = e & 63;
+        L[r * CH_P + c] = (r < nb && c <= r) ? Ab[(size_t)(k0 + r) * ns + k0 + c] : (r == c ? 1.0 : 0.0);
+    }
+    __syncthreads();
+    for (int j = 0; j < nb; ++j) {
+        if (tid == 0) {
+            const double d = L[j * CH_P + j];
+            if (!(d > 0.0) || !isfinite(d)) { s_bad = 1; L[j * CH_P + j] = 1.0; }
+            else { L[j * CH_P + j] = sqrt(d); s_ld += log(d); }
+        }
+        __syncthreads();
+        const double dj = L[j * CH_P + j];
+        if (tid > j && tid < nb) L[tid * CH_P + j] /= dj;
+        __syncthreads();
+        for (int e = tid; e < CH_NB * CH_NB; e += 256) {
+            const int r = e >> 6, c = e & 63;
+            if (c > j && r >= c && r < nb) L[r * CH_P + c] -= L[r * CH_P + j] * L[c * CH_P + j];
+        }
+        __syncthreads();
+    }
+    for (int e = tid; e < CH_NB * CH_NB; e += 256) {
+        const int r = e >> 6, c = e & 63;
+        if (r < nb && c <= r) Ab[(size_t)(k0 + r) * ns + k0 + c] = L[r * CH_P + c];
+    }
+    if (tid == 0) {
+        double* o = out + (size_t)b * CH_OUT;
+        o[0] = (k0 == 0 ? 0.0 : o[0]) + s_ld;
+        o[3] = (k0 == 0 ? 0.0 : o[3]) + (s_bad ? 1.0 : 0.0);
+    }
+    // W = L11^-1 for the panel kernel (only full blocks have rows below them): thread c solves L11 x = e_c by forward substitution
+    if (nb == CH_NB && k0 + CH_NB < ns && tid < CH_NB) {
+        double* Wb = Winv + (size_t)b * CH_NB * CH_NB;
+        double x[CH_NB];
+#pragma unroll
+        for (int r = 0; r < CH_NB; ++r) {
+            double v = (r == tid) ? 1.0 : 0.0;
+#pragma unroll
+            for (int k = 0; k < r; ++k) v = fma(-L[r * CH_P + k], x[k], v);
+            x[r] = v / L[r * CH_P + r];
+        }
+#pragma unroll
+        for (int r = 0; r < CH_NB; ++r) Wb[r * CH_NB + tid] = x[r];     // W[r][c]
+    }
+}
+
+// L21 = A21 L11^-T = A21 W^T with W = L11^-1 from chol_diag_kernel: a 64-row tile of the panel times a 64 x 64 matrix, the same
+// sum_k P_i[i,k] P_j[c,k] form as the trailing update (a thread per row with its 64 doubles in registers took 3.2 of 15 ms)
+__global__ void __launch_bounds__(256, 2) chol_trsm_kernel(double* __restrict__ A, const double* __restrict__ Winv, int ns, int k0) {
+    extern __shared__ double ch_sm[];
+    double* Pi = ch_sm;                     // [k][row of the tile], pitch CH_P
+    double* Pj = ch_sm + CH_NB * CH_P;      // [k][c] = W[c][k]
+    const int b = blockIdx.y, tid = threadIdx.x;
+    const int ib = k0 + CH_NB + blockIdx.x * CH_NB;
+    double* Ab = A + (size_t)b * ns * ns;
+    const double* Wb = Winv + (size_t)b * CH_NB * CH_NB;
+    for (int e = tid; e < CH_NB * CH_NB; e += 256) {
+        const int r = e >> 6, k = e & 63;
+        Pi[k * CH_P + r] = (ib + r < ns) ? Ab[(size_t)(ib + r) * ns + k0 + k] : 0.0;
+        Pj[k * CH_P + r] = Wb[r * CH_NB + k];
+    }
+    __syncthreads();
+    const int ty = tid >> 4, tx = tid & 15;
+    double acc[4][4];
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) acc[r][c] = 0.0;
+#pragma unroll 8
+    for (int k = 0; k < CH_NB; ++k) {
+        double ar[4], br[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) { ar[r] = Pi[k * CH_P + ty * 4 + r]; br[r] = Pj[k * CH_P + tx + 16 * r]; }
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) acc[r][c] = fma(ar[r], br[c], acc[r][c]);
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const int i = ib + ty * 4 + r;
+            if (i < ns) Ab[(size_t)i * ns + k0 + tx + 16 * c] = acc[r][c];
+        }
+}
+
+__device__ __forceinline__ void ch_cp_async8(void* smem, const void* gmem) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gmem) : "memory");
+}
+
+// A[i, j] -= sum_k L21[i, k] L21[j, k] on the trailing lower triangle (rows / columns >= r0).  CTA = (row of 64 x 64 tiles ti, matrix):
+// the panel rows of ti stay in shared memory, those of tj = 0 .. ti stream through a double buffer filled by cp.async one tile
+// ahead (row-major [row][k], pitch 65 doubles: 8-byte copies, conflict-free reads), and the A tile is fetched into registers before
+// the 1024 DFMAs of a thread.  Rows of tiles are handed out longest first.  (One tile per CTA with a synchronous transposing load:
+// 32 % of the DFMA rate.)
+__global__ void __launch_bounds__(256, 2) chol_update_kernel(double* __restrict__ A, int ns, int k0, int nt) {
+    extern __shared__ double ch_sm[];
+    double* Pi = ch_sm;
+    double* Pj = ch_sm + CH_NB * CH_P;      // two buffers
+    const int b = blockIdx.y, tid = threadIdx.x;
+    const int ti = nt - 1 - (int)blockIdx.x;
+    const int r0 = k0 + CH_NB, ib = r0 + ti * CH_NB;
+    double* Ab = A + (size_t)b * ns * ns;
+    auto fill = [&](double* dst, int rb) {         // rows rb .. rb + 63, columns k0 .. k0 + 63 of the panel
+#pragma unroll
+        for (int it = 0; it < (CH_NB * CH_NB) / 256; ++it) {
+            const int e = tid + it * 256, r = e >> 6, k = e & 63;
+            if (rb + r < ns) ch_cp_async8(dst + r * CH_P + k, Ab + (size_t)(rb + r) * ns + k0 + k);
+            else dst[r * CH_P + k] = 0.0;
+        }
+        asm volatile("cp.async.commit_group;\n" ::: "memory");
+    };
+    fill(Pi, ib);
+    fill(Pj, r0);
+    const int ty = tid >> 4, tx = tid & 15;
+    for (int tj = 0; tj <= ti; ++tj) {
+        const int jb = r0 + tj * CH_NB;
+        double* Pc = Pj + (tj & 1) * CH_NB * CH_P;
+        if (tj < ti) fill(Pj + ((tj + 1) & 1) * CH_NB * CH_P, jb + CH_NB);
+        double cur[4][4], acc[4][4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int i = ib + ty * 4 + r, j = jb + tx + 16 * c;
+                cur[r][c] = (i < ns && j <= i) ? Ab[(size_t)i * ns + j] : 0.0;
+                acc[r][c] = 0.0;
+            }
+        if (tj < ti) asm volatile("cp.async.wait_group 1;\n" ::: "memory");
+        else asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+        __syncthreads();
+#pragma unroll 8
+        for (int k = 0; k < CH_NB; ++k) {
+            double ar[4], br[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) { ar[r] = Pi[(ty * 4 + r) * CH_P + k]; br[r] = Pc[(tx + 16 * r) * CH_P + k]; }
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) acc[r][c] = fma(ar[r], br[c], acc[r][c]);
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const int i = ib + ty * 4 + r, j = jb + tx + 16 * c;
+                if (i < ns && j <= i) Ab[(size_t)i * ns + j] = cur[r][c] - acc[r][c];
+            }
+        __syncthreads();                   // the buffer just read is refilled by the next iteration's prefetch
+    }
+}
+
+// the whole factorisation of Bc matrices on stream st; out[b*6 + 0] = ln det A, out[b*6 + 3] != 0 = not positive definite
+size_t pixsrc_factor_scratch_bytes(int Bc) { return sizeof(double) * (size_t)Bc * CH_NB * CH_NB; }
+
+// Winv: scratch of pixsrc_factor_scratch_bytes(Bc)
+cudaError_t launch_pixsrc_factor(glad_ctx* c, cudaStream_t st, double* A, int ns, int Bc, double* out, double* Winv) {
+    const size_t sm_trsm = sizeof(double) * 2 * CH_NB * CH_P, sm_upd = sizeof(double) * 3 * CH_NB * CH_P;
+    cudaError_t e = smem_optin(c, chol_update_kernel);
+    if (e == cudaSuccess) e = smem_optin(c, chol_trsm_kernel);
+    if (e != cudaSuccess) return e;
+    for (int k0 = 0; k0 < ns; k0 += CH_NB) {
+        chol_diag_kernel<<<Bc, 256, 0, st>>>(A, ns, k0, out, Winv);
+        c->launches++;
+        const int rest = ns - k0 - CH_NB;
+        if (rest <= 0) break;
+        const int nt = (rest + CH_NB - 1) / CH_NB;
+        chol_trsm_kernel<<<dim3(nt, Bc), 256, sm_trsm, st>>>(A, Winv, ns, k0);
+        chol_update_kernel<<<dim3(nt, Bc), 256, sm_upd, st>>>(A, ns, k0, nt);
+        c->launches += 2;
+    }
+    return cudaGetLastError();
+}

@@ -6,8 +6,8 @@
 //                              of N_s floats and streams the row out (f [N_pix, N_s] fp32, the one large intermediate)
 //   pixsrc_syrk_tc_kernel (pixsrc_syrk_tc.cu)  F = f^T C_d^-1 f (Eq. 41) + lambda g -> A (lower triangle, fp64 store) and
 //                              D = f^T C_d^-1 d (Eq. 42): tcgen05 MMAs on two-term fp16 operands, 128 x 128 output tiles
-//   pixsrc_chol_kernel   A = L L^T in fp64 (blocked right-looking, one CTA per vector), ln det A, s_MP = A^-1 D (Eq. 40),
-//                              E_S = 1/2 s^T g s from its pixel definition
+//   chol_*_kernel (pixsrc_chol.cu)  A = L L^T in fp64, ln det A: three kernels per 64-wide panel over the whole batch
+//   pixsrc_solve_kernel  s_MP = A^-1 D (Eq. 40) by forward / backward substitution, E_S = 1/2 s^T g s from its pixel definition
 //   pixsrc_model_kernel  f s_MP (Eq. 37) and chi^2 = sum ivar (f s - d)^2, a warp per image pixel
 //   pixsrc_final_kernel  the evidence of Eq. 43 (R-P5), flags
 // Readings R-P1..5 are stated in DESIGN.md section 2.
@@ -19,10 +19,8 @@
 
 #define PX_MAP_THREADS 128
 #define PX_BLUR_WARPS 8
-#define PX_TILE 64
-#define PX_NB 32           // Cholesky panel width
+#define PX_NB 32           // block length of the substitutions
 #define PX_CHOL_THREADS 256
-#define PX_PP 65           // pitch (doubles) of the k-major panel tiles in shared memory: conflict-free transposed stores
 
 __device__ __forceinline__ bool pixsrc_valid(const float* __restrict__ p, float lam, float ps) {
     return (p[2] >= 0.f) && (p[3] > 1.f && p[3] < 3.f) && (p[4] > 0.f && p[4] <= 1.f) && (p[8] >= 0.f) && (lam > 0.f) &&
@@ -120,120 +118,20 @@ __global__ void __launch_bounds__(32 * PX_BLUR_WARPS) pixsrc_blur_kernel(const i
 // F = f^T C_d^-1 f (+ lambda g) and D = f^T C_d^-1 d: pixsrc_syrk_tc.cu (tcgen05)
 
 // ------------------------------------------------------------------------------------------------------------------
-// Cholesky, solve, regulariser: one CTA per vector, fp64
+// Solve with the factor of pixsrc_chol.cu, regulariser: one CTA per vector, fp64
 // ------------------------------------------------------------------------------------------------------------------
-// out[b*PX_OUT + {0,1,2,3,4}] = {ln det A, E_S, chi2 (filled by pixsrc_model_kernel), not-positive-definite flag, y^T y = D^T A^-1 D}
+// out[b*PX_OUT + {0,1,2,3,4}] = {ln det A (chol_diag_kernel), E_S, chi2 (filled by pixsrc_model_kernel), not-positive-definite flag
+// (chol_diag_kernel), y^T y = D^T A^-1 D}
 // search = 1 (the lambda_hat search of Eq. 43): stop after the forward substitution -- the objective needs ln det A and y^T y only
 #define PX_OUT 6
-__global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_chol_kernel(double* __restrict__ A, const double* __restrict__ D, int ns,
-                                                                      int nsx, int nsy, double* __restrict__ s_out,
-                                                                      double* __restrict__ out, int search) {
+__global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_solve_kernel(const double* __restrict__ A, const double* __restrict__ D, int ns,
+                                                                       int nsx, int nsy, double* __restrict__ s_out,
+                                                                       double* __restrict__ out, int search) {
     extern __shared__ double px_sm[];
-    double* L11 = px_sm;                         // [32][33]
-    double* Pi = L11 + PX_NB * (PX_NB + 1);      // [32][PX_PP] (k-major): rows of the 64-row tile along the pitch
-    double* Pj = Pi + PX_NB * PX_PP;
-    double* yv = Pj + PX_NB * PX_PP;             // [ns]
+    double* yv = px_sm;                          // [ns]
     double* red = yv + ns;                       // [8][32]
-    __shared__ int bad;
-    __shared__ double logdet;
     const int b = blockIdx.x, tid = threadIdx.x;
-    double* Ab = A + (size_t)b * ns * ns;
-    if (tid == 0) { bad = 0; logdet = 0.0; }
-    __syncthreads();
-
-    for (int k0 = 0; k0 < ns; k0 += PX_NB) {
-        const int nb = min(PX_NB, ns - k0);
-        // diagonal block -> shared
-        for (int e = tid; e < PX_NB * PX_NB; e += PX_CHOL_THREADS) {
-            const int r = e >> 5, c = e & 31;
-            L11[r * (PX_NB + 1) + c] = (r < nb && c <= r) ? Ab[(size_t)(k0 + r) * ns + k0 + c] : (r == c ? 1.0 : 0.0);
-        }
-        __syncthreads();
-        for (int j = 0; j < nb; ++j) {
-            if (tid == 0) {
-                const double d = L11[j * (PX_NB + 1) + j];
-                if (!(d > 0.0) || !isfinite(d)) { bad = 1; L11[j * (PX_NB + 1) + j] = 1.0; }
-                else { L11[j * (PX_NB + 1) + j] = sqrt(d); logdet += log(d); }
-            }
-            __syncthreads();
-            const double dj = L11[j * (PX_NB + 1) + j];
-            if (tid > j && tid < nb) L11[tid * (PX_NB + 1) + j] /= dj;
-            __syncthreads();
-            for (int e = tid; e < PX_NB * PX_NB; e += PX_CHOL_THREADS) {
-                const int r = e >> 5, c = e & 31;
-                if (c > j && r >= c && r < nb) L11[r * (PX_NB + 1) + c] -= L11[r * (PX_NB + 1) + j] * L11[c * (PX_NB + 1) + j];
-            }
-            __syncthreads();
-        }
-        // write the factored diagonal block back
-        for (int e = tid; e < PX_NB * PX_NB; e += PX_CHOL_THREADS) {
-            const int r = e >> 5, c = e & 31;
-            if (r < nb && c <= r) Ab[(size_t)(k0 + r) * ns + k0 + c] = L11[r * (PX_NB + 1) + c];
-        }
-        const int r0 = k0 + nb;
-        if (r0 >= ns) break;
-        // panel: L21[i, :] = A[i, k0:k0+nb] L11^-T, a thread per row (nb == PX_NB here: only the last block is ragged)
-        for (int i = r0 + tid; i < ns; i += PX_CHOL_THREADS) {
-            double x[PX_NB];
-            double* arow = Ab + (size_t)i * ns + k0;
-#pragma unroll
-            for (int c = 0; c < PX_NB; ++c) x[c] = arow[c];
-#pragma unroll
-            for (int c = 0; c < PX_NB; ++c) {
-                double v = x[c];
-#pragma unroll
-                for (int k = 0; k < c; ++k) v -= x[k] * L11[c * (PX_NB + 1) + k];
-                x[c] = v / L11[c * (PX_NB + 1) + c];
-            }
-#pragma unroll
-            for (int c = 0; c < PX_NB; ++c) arow[c] = x[c];
-        }
-        __syncthreads();
-        // trailing update: A[i, j] -= sum_k L21[i, k] L21[j, k], i >= j >= r0, 64 x 64 tiles
-        const int nt = (ns - r0 + PX_TILE - 1) / PX_TILE;
-        const int ty = tid >> 4, tx = tid & 15;
-        for (int ti = 0; ti < nt; ++ti)
-            for (int tj = 0; tj <= ti; ++tj) {
-                const int ib = r0 + ti * PX_TILE, jb = r0 + tj * PX_TILE;
-                for (int e = tid; e < PX_NB * PX_TILE; e += PX_CHOL_THREADS) {
-                    const int r = e >> 5, k = e & 31;          // consecutive threads read consecutive k of one row
-                    Pi[k * PX_PP + r] = (ib + r < ns) ? Ab[(size_t)(ib + r) * ns + k0 + k] : 0.0;
-                    Pj[k * PX_PP + r] = (jb + r < ns) ? Ab[(size_t)(jb + r) * ns + k0 + k] : 0.0;
-                }
-                __syncthreads();
-                // thread (ty, tx): rows ib + 4 ty + r, columns jb + tx + 16 c (consecutive lanes on consecutive columns: the Pj reads
-                // are conflict-free and the read-modify-write of A is coalesced); A is fetched before the k loop so that its latency
-                // hides behind the 512 DFMAs
-                double cur[4][4], acc[4][4];
-#pragma unroll
-                for (int r = 0; r < 4; ++r)
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        const int i = ib + ty * 4 + r, j = jb + tx + 16 * c;
-                        cur[r][c] = (i < ns && j <= i) ? Ab[(size_t)i * ns + j] : 0.0;
-                        acc[r][c] = 0.0;
-                    }
-#pragma unroll 8
-                for (int k = 0; k < PX_NB; ++k) {
-                    double ar[4], br[4];
-#pragma unroll
-                    for (int r = 0; r < 4; ++r) { ar[r] = Pi[k * PX_PP + ty * 4 + r]; br[r] = Pj[k * PX_PP + tx + 16 * r]; }
-#pragma unroll
-                    for (int r = 0; r < 4; ++r)
-#pragma unroll
-                        for (int c = 0; c < 4; ++c) acc[r][c] = fma(ar[r], br[c], acc[r][c]);
-                }
-#pragma unroll
-                for (int r = 0; r < 4; ++r)
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) {
-                        const int i = ib + ty * 4 + r, j = jb + tx + 16 * c;
-                        if (i < ns && j <= i) Ab[(size_t)i * ns + j] = cur[r][c] - acc[r][c];
-                    }
-                __syncthreads();
-            }
-    }
-    __syncthreads();
+    const double* Ab = A + (size_t)b * ns * ns;
 
     // forward substitution L y = D
     const int warp = tid >> 5, lane = tid & 31;
@@ -271,8 +169,6 @@ __global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_chol_kernel(double*
         if (tid == 0) {
             double t = 0.0;
             for (int w = 0; w < PX_CHOL_THREADS / 32; ++w) t += red[w];
-            out[(size_t)b * PX_OUT + 0] = logdet;
-            out[(size_t)b * PX_OUT + 3] = bad ? 1.0 : 0.0;
             out[(size_t)b * PX_OUT + 4] = t;
         }
         return;
@@ -322,9 +218,7 @@ __global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_chol_kernel(double*
     if (tid == 0) {
         double t = 0.0;
         for (int w = 0; w < PX_CHOL_THREADS / 32; ++w) t += red[w];
-        out[(size_t)b * PX_OUT + 0] = logdet;
         out[(size_t)b * PX_OUT + 1] = t;
-        out[(size_t)b * PX_OUT + 3] = bad ? 1.0 : 0.0;
     }
 }
 
@@ -485,7 +379,7 @@ size_t pixsrc_scratch_bytes(int npix, int ns, int Bc, bool search) {
            px_align(sizeof(float) * (size_t)Bc * npix * ns) + (search ? 2 : 1) * px_align(sizeof(double) * (size_t)Bc * ns * ns) +
            2 * px_align(sizeof(double) * (size_t)Bc * ns) + px_align(sizeof(double) * (size_t)Bc * PX_OUT) + px_align(sizeof(double) * 4) +
            (search ? px_align(sizeof(PxSearch) * (size_t)Bc) + px_align(sizeof(double) * (size_t)Bc) + px_align(sizeof(float) * (size_t)Bc) : 0) +
-           px_align(sizeof(unsigned short) * (size_t)Bc * px_ntiles(ns) * npix);
+           px_align(sizeof(unsigned short) * (size_t)Bc * px_ntiles(ns) * npix) + px_align(pixsrc_factor_scratch_bytes(Bc));
 }
 
 // d_lam != NULL: the evidence at the given lambda; d_lam == NULL: search lambda_hat on [lam_lo, lam_hi] first, write it to d_lam_hat
@@ -513,16 +407,17 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
         lam_cur = (double*)q;      q += px_align(sizeof(double) * (size_t)Bc);
         lam_f = (float*)q;         q += px_align(sizeof(float) * (size_t)Bc);
     }
-    unsigned short* rowlist = (unsigned short*)q;
+    unsigned short* rowlist = (unsigned short*)q;   q += px_align(sizeof(unsigned short) * (size_t)Bc * px_ntiles(ns) * npix);
+    double* Winv = (double*)q;
     cudaError_t e;
     if ((e = cudaMemsetAsync(out, 0, sizeof(double) * (size_t)Bc * PX_OUT, st)) != cudaSuccess) return e;
 
     const int rows_per_cta = 64;
     const size_t sm_blur = sizeof(float) * (size_t)PX_BLUR_WARPS * ns;
-    const size_t sm_chol = sizeof(double) * ((size_t)PX_NB * (PX_NB + 1) + 2 * PX_NB * PX_PP + ns + 8 * 32);
+    const size_t sm_chol = sizeof(double) * ((size_t)ns + 8 * 32);
     if (sm_blur > 227 * 1024 || sm_chol > 227 * 1024) return cudaErrorInvalidConfiguration;
     if ((e = smem_optin(c, pixsrc_blur_kernel)) != cudaSuccess) return e;
-    if ((e = smem_optin(c, pixsrc_chol_kernel)) != cudaSuccess) return e;
+    if ((e = smem_optin(c, pixsrc_solve_kernel)) != cudaSuccess) return e;
     pixsrc_static_kernel<<<1, 256, 0, st>>>(c->d_ivar, npix, c->d_psf, c->kpsf * c->kpsf, stat);
     c->launches++;
     {
@@ -553,14 +448,16 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
             c->launches++;
             if (step == last_step) break;
             ProfScope ps(c, GK_PIX_CHOL);
-            pixsrc_chol_kernel<<<Bc, PX_CHOL_THREADS, sm_chol, st>>>(A, D, ns, nsx, nsy, s, out, 1);
+            if ((e = launch_pixsrc_factor(c, st, A, ns, Bc, out, Winv)) != cudaSuccess) return e;
+            pixsrc_solve_kernel<<<Bc, PX_CHOL_THREADS, sm_chol, st>>>(A, D, ns, nsx, nsy, s, out, 1);
         }
         lam_use = lam_f;
         if (d_lam_hat && (e = cudaMemcpyAsync(d_lam_hat, lam_f, sizeof(float) * Bc, cudaMemcpyDeviceToDevice, st)) != cudaSuccess) return e;
     }
     {
         ProfScope ps(c, GK_PIX_CHOL);
-        pixsrc_chol_kernel<<<Bc, PX_CHOL_THREADS, sm_chol, st>>>(A, D, ns, nsx, nsy, s, out, 0);
+        if ((e = launch_pixsrc_factor(c, st, A, ns, Bc, out, Winv)) != cudaSuccess) return e;
+        pixsrc_solve_kernel<<<Bc, PX_CHOL_THREADS, sm_chol, st>>>(A, D, ns, nsx, nsy, s, out, 0);
     }
     {
         ProfScope ps(c, GK_PIX_MODEL);
