@@ -547,17 +547,33 @@ def run_ours(args, rank, world, local_rank):
         syrk_ms = pp["pixsrc_syrk"][0] / p_steps
         chol_ms = pp["pixsrc_chol"][0] / p_steps
         syrk_flops = Bp * float(npx) * nsrc * (nsrc + 1)             # dense lower triangle of F = f^T C_d^-1 f, 2 flops per term
-        chol_flops = Bp * 2.0 * nsrc ** 3 / 3.0                       # fp64
+        chol_flops = Bp * nsrc ** 3 / 3.0                             # fp64: N^3/3 (multiplies and adds) per factorisation
         model["pixsrc_entry"] = {
             "api": "glad_pixsrc_evidence_batch", "value": Bp / (p_ms * 1e-3), "unit": "evidences/s", "ms_per_step": p_ms, "batch": Bp,
             "sizes": f"N_d = {npx} image pixels, PSF {L['psf'].shape[0]} x {L['psf'].shape[0]}, N_s = {nsx} x {nsy} source pixels",
             "kernel_ms": {k[7:]: pp[k][0] / p_steps for k in pp if k.startswith("pixsrc_")},
             "finite": int(torch.isfinite(po["logev"]).sum().item()),
-            "contraction": {"kernel": "pixsrc_syrk_kernel", "ms_per_launch": syrk_ms, "dense_flops_per_launch": syrk_flops,
-                            "dense_equivalent_tflops": syrk_flops / (syrk_ms * 1e-3) / 1e12, "fp32_peak_tflops": torch.cuda.get_device_properties(dev).multi_processor_count * FP32_LANES_PER_SM * 2 * float(clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12,
-                            "note": "fp32 FFMA; chunks of 16 image pixels whose f rows miss either 64-column tile are skipped, so the dense-equivalent rate can exceed the executed one"},
-            "cholesky": {"kernel": "pixsrc_chol_kernel", "ms_per_launch": chol_ms, "fp64_gflops": chol_flops / (chol_ms * 1e-3) / 1e9},
+            "contraction": {"kernel": "pixsrc_syrk_tc_kernel", "ms_per_launch": syrk_ms, "dense_flops_per_launch": syrk_flops,
+                            "dense_equivalent_tflops": syrk_flops / (syrk_ms * 1e-3) / 1e12,
+                            "note": "tcgen05.mma on two-term fp16 operands (22 mantissa bits), three products per K-step, fp32 accumulation in TMEM "
+                                    "flushed into registers every 512 pixels; D = f^T C_d^-1 d accumulated in fp64 on the diagonal tiles in the same pass; "
+                                    "only the pixel rows whose f row touches both column blocks of a tile are contracted (about a third), so the "
+                                    "dense-equivalent rate exceeds the executed one"},
+            "cholesky": {"kernels": "chol_diag / chol_trsm / chol_update (three per 64-wide panel over the batch) + pixsrc_solve", "ms_per_factorisation_and_solve": chol_ms,
+                         "fp64_gflops": chol_flops / (chol_ms * 1e-3) / 1e9},
             "paper_context": "extended-image step, one vector, 64 x 64 source grid, N_d ~ 1e4: 0.21 s on one A100 in fp64, 2 s with GLEE on one CPU core (Table 2 P:453-458); other hardware, context only"}
+        # Eq. 43: the same chain with lambda_hat searched on the device (22 extra factorisations per vector)
+        for _ in range(1):
+            lo = g.pixsrc_lambda_opt_batch(pa[0], pa[1], (1e-3, 1e3), nsx, nsy, want_source=False, want_model=False)
+        torch.cuda.synchronize()
+        l0, l1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0.record()
+        lo = g.pixsrc_lambda_opt_batch(pa[0], pa[1], (1e-3, 1e3), nsx, nsy, want_source=False, want_model=False)
+        l1.record()
+        torch.cuda.synchronize()
+        model["pixsrc_entry"]["lambda_opt"] = {"api": "glad_pixsrc_lambda_opt_batch", "ms_per_step": l0.elapsed_time(l1), "batch": Bp,
+                                               "value": Bp / (l0.elapsed_time(l1) * 1e-3), "unit": "optimised evidences/s",
+                                               "lambda_range": [1e-3, 1e3], "finite": int(torch.isfinite(lo["logev"]).sum().item())}
 
     if rank == 0:
         # JAM_sph, the paper's own dynamics, on the same dynamics inputs with the paper's mesh (P:358-362:
