@@ -97,6 +97,7 @@ struct glad_ctx {
     const float* d_data;
     const float* d_ivar;
     float* d_psf;  // ctx-owned copy [kpsf*kpsf]
+    const float* d_lens_params_cur;   // the lens vectors of the batch call in flight (launch_lens_prep -> launch_lens_image)
     int kpsf;
 
     // internal mass sheet (glad_set_mass_sheet): d_lambda borrowed, NULL = off

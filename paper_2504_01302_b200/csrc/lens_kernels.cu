@@ -9,6 +9,7 @@
 
 #include "glad_internal.h"
 #include "glad_special.cuh"
+#include "glad_mass_fp64.cuh"
 
 // 4 warps per 32 parameter vectors (lane = vector): warp role 0 = EPL / shear / point mass / validity, roles 1..3 =
 // one Sersic component each (the b_n root is the only long serial chain of the kernel; a warp never mixes roles).
@@ -115,6 +116,21 @@ __device__ __forceinline__ float sersic_eval(const float* __restrict__ o, float 
     return o[5] * ex2f(-o[6] * pw);
 }
 
+// Cusp guard: an fp32 ray carries ~5e-7" of absolute error in beta (|alpha| ~ 1.7").  Where the source
+// profile is steep, |d ln I / dR| = ln2 k1 2h (R^2)^h / R, that error is amplified: above LENS_CUSP_SLOPE per arcsec (2e-5 per ray) the
+// pixel is recomputed with fp64 rays (src_pixel_fp64).  Happens within ~0.05" of the centre of an n ~ 4 source: a few hundred of the
+// 40 000 rays of a C2 vector; one C2 vector in 1024 had a peak pixel 1.09e-4 off without it.
+#define LENS_CUSP_SLOPE 30.f
+__device__ __forceinline__ float sersic_at(const float* __restrict__ o, float dx, float dy, bool& cusp) {
+    float x = dx * o[2] + dy * o[3];
+    float y = dy * o[2] - dx * o[3];
+    float R2 = fmaf(y * y, o[4], x * x);
+    float pw = ex2f(o[7] * lg2f(R2));      // (R^2)^(1/2n); R2 = 0 -> 0
+    const float gl = 1.3862944f * o[6] * o[7] * pw;                  // |d ln I / d ln R| = ln2 k1 2h pw
+    cusp = gl * gl > (LENS_CUSP_SLOPE * LENS_CUSP_SLOPE) * R2;
+    return o[5] * ex2f(-o[6] * pw);
+}
+
 __device__ __forceinline__ float chameleon_eval(const float* __restrict__ o, float px, float py) {
     float dx = px - o[0], dy = py - o[1];
     float x = dx * o[2] + dy * o[3];
@@ -138,7 +154,8 @@ __device__ __forceinline__ float light_eval(int kinds, int k, const float* __res
 // code of the common case is exactly the table-driven loop
 template <bool CH, bool LONG>
 __device__ __forceinline__ float shoot(const float* __restrict__ c, float thx, float thy, int nterms,
-                                       bool has_src, bool has_l1, bool has_l2, int kinds, const float2* __restrict__ cse, int ncse) {
+                                       bool has_src, bool has_l1, bool has_l2, int kinds, const float2* __restrict__ cse, int ncse,
+                                       float& src, bool& cusp) {
     float dx = thx - c[LC_XL], dy = thy - c[LC_YL];
     float cs = c[LC_COSPA], sn = c[LC_SINPA];
     float x = dx * cs + dy * sn, y = dy * cs - dx * sn;
@@ -208,7 +225,13 @@ __device__ __forceinline__ float shoot(const float* __restrict__ c, float thx, f
         ay += hx * hs + hy * hc;
     }
     float v = 0.f;
-    if (has_src) v += light_eval<CH>(kinds, 0, c + LC_SERSIC0, thx - ax, thy - ay);
+    src = 0.f;
+    cusp = false;
+    if (has_src) {
+        const float* o = c + LC_SERSIC0;
+        if (CH && (kinds & 1)) src = chameleon_eval(o, thx - ax, thy - ay);          // cored: no cusp
+        else src = sersic_at(o, (thx - ax) - o[0], (thy - ay) - o[1], cusp);
+    }
     if (has_l1) v += light_eval<CH>(kinds, 1, c + LC_SERSIC0 + LC_SERSIC_STRIDE, thx, thy);
     if (has_l2) v += light_eval<CH>(kinds, 2, c + LC_SERSIC0 + 2 * LC_SERSIC_STRIDE, thx, thy);
     return v;
@@ -226,10 +249,21 @@ static inline __host__ __device__ int lens_tap_pitch(int kpsf) { return (kpsf + 
 static inline __host__ __device__ int lens_halo_left(int kpsf) { return kpsf / 2 + LENS_TAPS; }
 static inline __host__ __device__ int lens_img_pitch(int nx, int kpsf) { return (nx + 2 * (kpsf / 2) + LENS_TAPS + LENS_STRIP - 1) | 1; }
 
-// rows a1-a3 for one vector: every sub-pixel ray, averaged into the binned image in shared memory
+#define LENS_CUSP_LIST 2048
+__device__ __noinline__ void cusp_mass_const(const float* __restrict__ p, double lam, double rc, double rt, bool sheet, const float* nf,
+                                             const double2* cse, int ncse, MassConst& m) {
+    mass_const(p, lam, rc, rt, sheet, m);
+    mass_const_halo(nf, cse, ncse, m);
+}
+// rows a1-a3 for one vector: every sub-pixel ray, averaged into the binned image in shared memory.  A pixel one of whose rays trips
+// the cusp guard keeps only its lens light here and is put on the list for src_pixel_fp64 (or, if the list is full, done at once).
+template <bool CH>
+__device__ __noinline__ float src_pixel_fp64(const float* __restrict__ c, const glad_image_grid& g, const MassConst& m, int ix, int iy);
+
 template <bool CH, bool LONG>
 __device__ __forceinline__ void ray_pass(const float* __restrict__ c, const glad_image_grid& g, float* __restrict__ img, int pitch,
-                                         int HL, int nterms, int kinds, const float2* __restrict__ cse, int ncse) {
+                                         int HL, int nterms, int kinds, const float2* __restrict__ cse, int ncse,
+                                         unsigned short* __restrict__ cusp_list, int* __restrict__ cusp_count, const MassConst& m) {
     const int tid = threadIdx.x, nthr = blockDim.x, nx = g.nx, npx = g.nx * g.ny, ss = g.supersample;
     const bool has_src = c[LC_SERSIC0 + 5] != 0.f;
     const bool has_l1 = c[LC_SERSIC0 + LC_SERSIC_STRIDE + 5] != 0.f;
@@ -237,23 +271,54 @@ __device__ __forceinline__ void ray_pass(const float* __restrict__ c, const glad
     const float inv_s = 1.f / (float)ss, inv_s2 = 1.f / (float)(ss * ss);
     for (int p = tid; p < npx; p += nthr) {
         int iy = p / nx, ix = p - iy * nx;
-        float acc = 0.f;
+        float acc = 0.f, acc_s = 0.f;
+        bool any = false;
         for (int sb = 0; sb < ss; ++sb) {
             float thy = fmaf(g.pix, (float)iy + (((float)sb + 0.5f) * inv_s - 0.5f), g.y0);
             for (int sa = 0; sa < ss; ++sa) {
                 float thx = fmaf(g.pix, (float)ix + (((float)sa + 0.5f) * inv_s - 0.5f), g.x0);
-                acc += shoot<CH, LONG>(c, thx, thy, nterms, has_src, has_l1, has_l2, kinds, cse, ncse);
+                float src;
+                bool cusp;
+                acc += shoot<CH, LONG>(c, thx, thy, nterms, has_src, has_l1, has_l2, kinds, cse, ncse, src, cusp);
+                acc_s += src;
+                any |= cusp;
             }
         }
-        img[iy * pitch + HL + ix] = acc * inv_s2;
+        if (any) {
+            const int slot = atomicAdd(cusp_count, 1);
+            if (slot < LENS_CUSP_LIST) { cusp_list[slot] = (unsigned short)p; acc_s = 0.f; }
+            else acc_s = src_pixel_fp64<CH>(c, g, m, ix, iy);
+        }
+        img[iy * pitch + HL + ix] = (acc + acc_s) * inv_s2;
     }
 }
 
 // out of line: the rare long-series loop must not raise the register count of the kernel (2 CTAs of 512 threads per SM)
 template <bool CH>
 __device__ __noinline__ void ray_pass_long(const float* __restrict__ c, const glad_image_grid& g, float* __restrict__ img, int pitch,
-                                           int HL, int nterms, int kinds, const float2* __restrict__ cse, int ncse) {
-    ray_pass<CH, true>(c, g, img, pitch, HL, nterms, kinds, cse, ncse);
+                                           int HL, int nterms, int kinds, const float2* __restrict__ cse, int ncse,
+                                           unsigned short* __restrict__ cusp_list, int* __restrict__ cusp_count, const MassConst& m) {
+    ray_pass<CH, true>(c, g, img, pitch, HL, nterms, kinds, cse, ncse, cusp_list, cusp_count, m);
+}
+
+// Sum over the s x s rays of pixel (ix, iy) of the SOURCE brightness with the deflection in fp64 (the mass model of the quasar terms,
+// glad_mass_fp64.cuh, from the raw parameters: the same arithmetic type as the definition), beta - source centre formed in fp64, the
+// profile itself in fp32.  Only the Sersic source reaches this (a Chameleon source has a core).
+template <bool CH>
+__device__ __noinline__ float src_pixel_fp64(const float* __restrict__ c, const glad_image_grid& g, const MassConst& m, int ix, int iy) {
+    const float* o = c + LC_SERSIC0;
+    const int ss = g.supersample;
+    float sum = 0.f;
+    for (int sb = 0; sb < ss; ++sb)
+        for (int sa = 0; sa < ss; ++sa) {
+            const double thx = (double)g.x0 + (double)g.pix * ((double)ix + (((double)sa + 0.5) / ss - 0.5));
+            const double thy = (double)g.y0 + (double)g.pix * ((double)iy + (((double)sb + 0.5) / ss - 0.5));
+            MassEval e;
+            mass_eval(m, thx, thy, e);
+            bool dummy;
+            sum += sersic_at(o, (float)(thx - e.ax - (double)o[0]), (float)(thy - e.ay - (double)o[1]), dummy);
+        }
+    return sum;
 }
 
 template <bool CH>
@@ -262,8 +327,12 @@ __global__ void __launch_bounds__(512, 2) lens_image_kernel(const float* __restr
                                                          const float* __restrict__ data,
                                                          const float* __restrict__ ivar, float* __restrict__ images,
                                                          float* __restrict__ chi2, int32_t* __restrict__ flags,
-                                                         const float2* __restrict__ cse, int ncse) {
+                                                         const float2* __restrict__ cse, int ncse, const float* __restrict__ params,
+                                                         const float* __restrict__ lambda, double ms_rc, double ms_rt, const HaloArgs halo) {
     extern __shared__ __align__(16) float smem[];
+    __shared__ MassConst s_mc;                           // fp64 mass model of this vector, for the cusp guard's rays
+    __shared__ unsigned short s_cusp[LENS_CUSP_LIST];
+    __shared__ int s_ncusp;
     const int b = blockIdx.x, tid = threadIdx.x, nthr = blockDim.x;
     const int nx = g.nx, ny = g.ny, npx = nx * ny;
     const int KP = lens_tap_pitch(kpsf), HL = lens_halo_left(kpsf), pitch = lens_img_pitch(nx, kpsf);
@@ -278,6 +347,11 @@ __global__ void __launch_bounds__(512, 2) lens_image_kernel(const float* __restr
         spsf[i] = k < kpsf ? psf[r * kpsf + k] : 0.f;
     }
     for (int i = tid; i < (ny + 1) * pitch; i += nthr) img[i] = 0.f;
+    if (tid == nthr - 1) {
+        s_ncusp = 0;
+        cusp_mass_const(params + (size_t)b * GLAD_NLENS, (CH && lambda) ? (double)lambda[b] : 1.0, ms_rc, ms_rt, CH && lambda != nullptr,
+                        (CH && halo.nf) ? halo.nf + 4 * (size_t)b : nullptr, halo.cse64, halo.ncse, s_mc);
+    }
     __syncthreads();
     const bool valid = c[LC_VALID] != 0.f;
     if (!valid) {
@@ -291,9 +365,20 @@ __global__ void __launch_bounds__(512, 2) lens_image_kernel(const float* __restr
     const int nterms = (int)c[LC_NTERMS];
 
     // rows a1-a3: rays -> binned pixel in shared memory
-    if (nterms > GLAD_EPL_MAX_TERMS) ray_pass_long<CH>(c, g, img, pitch, HL, nterms, kinds, cse, ncse);   // CTA-uniform: one vector per CTA
-    else ray_pass<CH, false>(c, g, img, pitch, HL, nterms, kinds, cse, ncse);
+    if (nterms > GLAD_EPL_MAX_TERMS) ray_pass_long<CH>(c, g, img, pitch, HL, nterms, kinds, cse, ncse, s_cusp, &s_ncusp, s_mc);   // CTA-uniform
+    else ray_pass<CH, false>(c, g, img, pitch, HL, nterms, kinds, cse, ncse, s_cusp, &s_ncusp, s_mc);
     __syncthreads();
+    {
+        // cusp guard: the listed pixels get their source light from fp64 rays; one thread per pixel, so no atomics and a result that
+        // does not depend on the order of the list
+        const int nc = min(s_ncusp, LENS_CUSP_LIST);
+        const float inv_s2 = 1.f / (float)(g.supersample * g.supersample);
+        for (int i = tid; i < nc; i += nthr) {
+            const int p = s_cusp[i], iy = p / nx, ix = p - iy * nx;
+            img[iy * pitch + HL + ix] += src_pixel_fp64<CH>(c, g, s_mc, ix, iy) * inv_s2;
+        }
+        __syncthreads();
+    }
 
     // row a4: PSF convolution from shared memory + chi2.  out[x] = sum_dy sum_dx psf[dy][dx] img[y+cc-dy][x+cc-dx]
     const int cc = kpsf / 2;
@@ -354,6 +439,7 @@ __global__ void __launch_bounds__(512, 2) lens_image_kernel(const float* __restr
 }
 
 cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B) {
+    c->d_lens_params_cur = d_params;                 // lens_image_kernel's cusp guard re-reads the raw vectors (launched right after this)
     ProfScope ps(c, GK_LENS_PREP, c->lens_stream);
     lens_prep_kernel<<<(B + 31) / 32, 32 * LENS_PREP_ROLES, 0, c->lens_stream>>>(d_params, B, c->light_kinds, c->d_lambda, c->ms_rc,
                                                                                  c->ms_rt, c->d_enfw, c->d_lens_const);
@@ -373,9 +459,10 @@ cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2
     ProfScope ps(c, GK_LENS_IMAGE, c->lens_stream);
     if (ch)
         lens_image_kernel<true><<<B, 512, smem, c->lens_stream>>>(c->d_lens_const, c->light_kinds, c->grid, c->d_psf, c->kpsf,
-                                                                 c->d_data, c->d_ivar, d_images, d_chi2, d_flags, c->d_cse32, c->ncse);
+                                                                 c->d_data, c->d_ivar, d_images, d_chi2, d_flags, c->d_cse32, c->ncse, c->d_lens_params_cur,
+                                                                 c->d_lambda, c->ms_rc, c->ms_rt, halo_args(c));
     else
         lens_image_kernel<false><<<B, 512, smem, c->lens_stream>>>(c->d_lens_const, 0, c->grid, c->d_psf, c->kpsf, c->d_data,
-                                                                  c->d_ivar, d_images, d_chi2, d_flags, nullptr, 0);
+                                                                  c->d_ivar, d_images, d_chi2, d_flags, nullptr, 0, c->d_lens_params_cur, nullptr, 0.0, 0.0, HaloArgs{nullptr, nullptr, nullptr, 0});
     return cudaGetLastError();
 }
