@@ -151,9 +151,10 @@ def gpu_data_model(device):
 def oracle_joint(wl):
     import oracle
     L, D = wl["lens"], wl["dyn"]
-    c2l = oracle.lens_image_batch(L["params"], L["grid"], L["psf"], L["data"], L["ivar"], want_images=False)["chi2"]
-    c2d = oracle.jam_vrms_batch(D["params"], D["lum_mge"], D["mass_mge"], D["beta"], D["kin"])["chi2"]
-    return oracle.joint_loglike(c2l, c2d)
+    B = wl["B"]
+    c2l = oracle.lens_image_batch(L["params"], L["grid"], L["psf"], L["data"], L["ivar"], want_images=False)["chi2"] if L else np.zeros(B)
+    c2d = oracle.jam_vrms_batch(D["params"], D["lum_mge"], D["mass_mge"], D["beta"], D["kin"])["chi2"] if D else np.zeros(B)
+    return oracle.joint_loglike(c2l, c2d)            # a lens-only / dynamics-only config: the half that exists
 
 
 def workload_terms(wl):
@@ -184,7 +185,7 @@ def run_reference(args, rank):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{args.config} (BASELINE.json configs[1], RXJ1131-shaped joint model), bounded sample"},
+            "config": {"workload": f"{args.config} ({'BASELINE.json configs[1], RXJ1131-shaped joint model' if args.config == 'C2' else 'BASELINE.json config'}), bounded sample"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -303,6 +304,35 @@ def ncu_summary(args):
     lines.append(f"{args.capture_key} {args.out} {args.capture_source} {sha}")
     open(CAPTURE_INDEX, "w").write("\n".join(lines) + "\n")
     print(f"wrote {args.out}; {args.capture_key} -> sha {sha}")
+
+
+SASS_OPS = ["UTCHMMA", "LDTM", "UTMALDG", "UBLKCP", "LDGSTS", "MUFU.EX2", "MUFU.LG2", "MUFU.RCP", "MUFU.RSQ", "FFMA", "FMUL2", "FFMA2", "FHFMA",
+            "F2FP", "DFMA", "HMMA", "SYNCS", "BAR"]
+
+
+def sass_counts():
+    """--sass-counts: `cuobjdump -sass paper_2504_01302_b200/libglad.so | python bench.py --sass-counts` prints a markdown table of opcode
+    counts per kernel (UTCHMMA = tcgen05.mma, LDTM = tcgen05.ld, UTMALDG / UBLKCP = TMA, LDGSTS = cp.async; B200_PROFILING.md)."""
+    import collections
+    import re
+    cur, cnt, total = None, collections.defaultdict(collections.Counter), collections.Counter()
+    for line in sys.stdin:
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            cur = m.group(1)
+            continue
+        m = re.search(r"/\*[0-9a-f]{4,8}\*/\s+(?:@!?U?P\d+\s+)?([A-Z0-9_.]+)", line)
+        if m and cur:
+            op = m.group(1)
+            total[cur] += 1
+            for o in SASS_OPS:
+                if op == o or op.startswith(o + "."):
+                    cnt[cur][o] += 1
+    names = {k: subprocess.run(["c++filt", k], capture_output=True, text=True).stdout.strip().split("(")[0] for k in total}
+    print("| kernel | SASS instructions | " + " | ".join(SASS_OPS) + " |")
+    print("|---|---|" + "---|" * len(SASS_OPS))
+    for k in sorted(total, key=lambda k: names[k]):
+        print(f"| `{names[k]}` | {total[k]} | " + " | ".join(str(cnt[k].get(o, 0)) for o in SASS_OPS) + " |")
 
 
 def peak_tf_of(dev, clocks):
@@ -801,7 +831,11 @@ def main():
     ap.add_argument("--capture-source", default="paper_2504_01302_b200/csrc/jam_quad_tc.cu")
     ap.add_argument("--capture-row", type=int, default=0, help="which profiled launch of the report")
     ap.add_argument("--out", default=None)
+    ap.add_argument("--sass-counts", action="store_true", help="opcode counts per kernel from `cuobjdump -sass` on stdin")
     args = ap.parse_args()
+    if args.sass_counts:
+        sass_counts()
+        return
     if args.ncu_summary:
         ncu_summary(args)
         return

@@ -599,6 +599,7 @@ static glad_status pixsrc_impl(glad_ctx* c, const char* who, const float* d_lens
     if (Bc > B) Bc = B;
     if (Bc > 2 * c->sm_count) Bc = 2 * c->sm_count;
     while (Bc > 1 && pixsrc_scratch_bytes(npix, ns, Bc, search) > cap) --Bc;
+    Bc = (B + (B + Bc - 1) / Bc - 1) / ((B + Bc - 1) / Bc);   // equal chunks: a short tail chunk pays every launch latency again
     glad_status st = grow(c, &c->d_pix, &c->pix_cap, pixsrc_scratch_bytes(npix, ns, Bc, search), true);
     if (st != GLAD_OK) return st;
     // ln det g in closed form: g = kron(I, T^2) + kron(T^2, I), T the (1,-2,1) matrix with eigenvalues -2 + 2 cos(k pi/(n+1))
