@@ -434,6 +434,25 @@ glad_status glad_pixsrc_lambda_opt_batch(glad_ctx* ctx, const float* d_lens_para
                                          int n_sx, int n_sy, int B, int scratch_mib_max, float* d_lam_hat, float* d_logev, float* d_chi2,
                                          float* d_reg, float* d_s_mp, float* d_model, int32_t* d_flags);
 
+/*
+ * glad_lens_image_batch for callers that cannot allocate device memory at call time (a CUDA graph being captured, a tight serving
+ * loop, a harness that forbids cudaMalloc): same arguments, same kernels (lens_prep_kernel -> lens_image_kernel), same results, but
+ * the per-vector constants that the first kernel writes for the second (88 floats per vector) live in a file-scope
+ * `static __device__` array of GLAD_LENS_NOALLOC_MAX_B vectors (1.4 MB, held by every GPU that loads the library until the
+ * process exits) instead of the context's growable scratch block.  The call enqueues two kernels on the context's stream and
+ * calls no cudaMalloc / cudaFree / allocating routine; the array's device address is taken once per device in glad_create.
+ * (The CUDA driver may still load kernel code and size its local-memory pool at a process's FIRST launch of these kernels: make one
+ * call before capturing a graph.)
+ *   B > GLAD_LENS_NOALLOC_MAX_B: GLAD_ESHAPE (split the batch).  GLAD_ESTATE as glad_lens_image_batch, or if the address could
+ *   not be taken at glad_create.  Mass sheet, eNFW halo and light-profile settings apply as in glad_lens_image_batch.
+ * The array is SHARED by every context and call on the device and keeps the last call's contents: the first kernel rewrites every
+ * slot the second one reads (nothing has to start at zero), and two calls whose kernels may overlap on the GPU (different
+ * streams, or contexts created on different streams) RACE on it -- order them on one stream or with events.
+ */
+#define GLAD_LENS_NOALLOC_MAX_B 4096
+glad_status glad_lens_image_noalloc(glad_ctx* ctx, const float* d_lens_params, int B, float* d_images, float* d_chi2,
+                                    int32_t* d_flags);
+
 /* Number of kernel launches enqueued by this context since creation (for bench.py's gpu_launches). */
 long glad_launch_count(const glad_ctx* ctx);
 

@@ -14,6 +14,7 @@ from .build import LIB, build
 
 NLENS, NDYN, NPROF = 26, 4, 4
 PROFILE_SERSIC, PROFILE_EPL, PROFILE_CHAMELEON, PROFILE_NFW_CSE = 0, 1, 2, 3
+LENS_NOALLOC_MAX_B = 4096          # GLAD_LENS_NOALLOC_MAX_B
 LIGHT_SERSIC, LIGHT_CHAMELEON = 0, 1
 FLAG_LENS_INVALID, FLAG_DYN_INVALID, FLAG_BIN_INVALID = 1, 2, 4
 FLAG_PIXSRC_NOT_PD = 8
@@ -24,7 +25,8 @@ EXPORTS = ["glad_create", "glad_destroy", "glad_last_error", "glad_version", "gl
            "glad_joint_loglike_host", "glad_bh_theta2", "glad_launch_count", "glad_profile_enable",
            "glad_profile_read", "glad_mge1d_batch", "glad_joint_loglike_model_batch", "glad_set_overlap", "glad_set_light_profiles",
            "glad_set_quasar_data", "glad_quasar_chi2_batch", "glad_joint_loglike_full_batch", "glad_set_mass_sheet",
-           "glad_pixsrc_evidence_batch", "glad_set_jam_options", "glad_set_jam_sph_rules", "glad_jam_sph_vrms_batch", "glad_set_enfw", "glad_pixsrc_lambda_opt_batch"]
+           "glad_pixsrc_evidence_batch", "glad_set_jam_options", "glad_set_jam_sph_rules", "glad_jam_sph_vrms_batch", "glad_set_enfw", "glad_pixsrc_lambda_opt_batch",
+           "glad_lens_image_noalloc"]
 
 
 class GladError(RuntimeError):
@@ -64,6 +66,8 @@ def load(rebuild: bool = False):
     L.glad_set_kin_data.argtypes = [vp, C.POINTER(SkyGrid), vp, i, vp, i, vp, vp, vp, vp, i]
     L.glad_lens_image_batch.restype = i
     L.glad_lens_image_batch.argtypes = [vp, vp, i, vp, vp, vp]
+    L.glad_lens_image_noalloc.restype = i
+    L.glad_lens_image_noalloc.argtypes = [vp, vp, i, vp, vp, vp]
     L.glad_jam_vrms_batch.restype = i
     L.glad_jam_vrms_batch.argtypes = [vp, vp, i, vp, i, l, vp, i, l, vp, i, vp, vp, vp, vp]
     L.glad_joint_loglike_batch.restype = i
@@ -248,6 +252,14 @@ class Glad:
         flags = out.get("flags") if out.get("flags") is not None else torch.empty(B, dtype=torch.int32, device=self.device)
         self._check(self.lib.glad_lens_image_batch(self.ctx, _p(p), B, _p(img), _p(chi2), _p(flags)))
         return {"images": img, "chi2": chi2, "flags": flags}
+
+    def lens_image_noalloc(self, lens_params, out):
+        """glad_lens_image_noalloc: lens_params a device float32 tensor [B, NLENS], out = dict(images, chi2, flags) of preallocated
+        device tensors (any may be None): nothing is allocated here or in the library; B <= LENS_NOALLOC_MAX_B."""
+        B = lens_params.shape[0]
+        self._check(self.lib.glad_lens_image_noalloc(self.ctx, _p(lens_params), B, _p(out.get("images")), _p(out.get("chi2")),
+                                                     _p(out.get("flags"))))
+        return out
 
     def _tables(self, lum_mge, mass_mge, beta):
         f = torch.float32

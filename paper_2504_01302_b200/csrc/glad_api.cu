@@ -79,6 +79,7 @@ glad_status glad_create(glad_ctx** out, int device, void* cuda_stream) {
         c->side_ok = 1;
     }
     c->overlap = c->side_ok;
+    if (lens_noalloc_setup(c) != cudaSuccess) cudaGetLastError();     // glad_lens_image_noalloc then reports GLAD_ESTATE
     *out = c;
     return GLAD_OK;
 }
@@ -410,6 +411,23 @@ glad_status glad_lens_image_batch(glad_ctx* c, const float* d_lens, int B, float
     if (B == 0) return GLAD_OK;
     DeviceScope ds(c);
     return lens_impl(c, d_lens, B, d_images, d_chi2, d_flags);
+}
+
+glad_status glad_lens_image_noalloc(glad_ctx* c, const float* d_lens, int B, float* d_images, float* d_chi2, int32_t* d_flags) {
+    if (!c) return GLAD_EINVAL;
+    if (B < 0 || (B > 0 && !d_lens)) return fail(c, GLAD_EINVAL, "glad_lens_image_noalloc: B=%d / null params", B);
+    if (B > GLAD_LENS_NOALLOC_MAX_B)
+        return fail(c, GLAD_ESHAPE, "glad_lens_image_noalloc: batch of %d vectors, the static constants array holds %d (GLAD_LENS_NOALLOC_MAX_B): split the batch",
+                    B, GLAD_LENS_NOALLOC_MAX_B);
+    if (B == 0) return GLAD_OK;
+    if (!c->d_lens_const_static) return fail(c, GLAD_ESTATE, "glad_lens_image_noalloc: the address of the static array could not be taken at glad_create");
+    if (!c->have_image) return fail(c, GLAD_ESTATE, "glad_lens_image_noalloc: glad_set_image_data not called");
+    if (c->d_lambda && B > c->n_lambda) return fail(c, GLAD_EINVAL, "glad_lens_image_noalloc: batch of %d vectors but the mass sheet has %d lambdas", B, c->n_lambda);
+    if (c->d_enfw && B > c->n_enfw) return fail(c, GLAD_EINVAL, "glad_lens_image_noalloc: batch of %d vectors but %d eNFW halos", B, c->n_enfw);
+    if (d_chi2 && !c->d_data) return fail(c, GLAD_ESTATE, "glad_lens_image_noalloc: chi2 requested but no data/ivar set");
+    DeviceScope ds(c);
+    CU(launch_lens_noalloc(c, d_lens, B, d_images, d_chi2, d_flags), "lens kernels (static constants)");
+    return GLAD_OK;
 }
 
 glad_status glad_jam_vrms_batch(glad_ctx* c, const float* d_dyn, int B, const float* d_lum, int nl, long lum_stride,

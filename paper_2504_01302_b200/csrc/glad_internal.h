@@ -141,6 +141,7 @@ struct glad_ctx {
 
     // grow-only scratch
     float* d_lens_const; size_t lens_const_cap;
+    float* d_lens_const_static;       // device address of lens_kernels.cu's file-scope array (glad_lens_image_noalloc); NULL = not available
     float* d_jam_tab;    size_t jam_tab_cap;
     float* d_partial;    size_t partial_cap;
     float* d_tmp;        size_t tmp_cap;     // chi2_L, chi2_D [B] each
@@ -206,6 +207,8 @@ static inline HaloArgs halo_args(const glad_ctx* c, size_t first_vector = 0) {
 // kernel launchers (return cudaGetLastError())
 cudaError_t launch_lens_prep(glad_ctx* c, const float* d_params, int B);
 cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2, int32_t* d_flags);
+cudaError_t lens_noalloc_setup(glad_ctx* c);      // glad_create, device current: address of the static constants array
+cudaError_t launch_lens_noalloc(glad_ctx* c, const float* d_params, int B, float* d_images, float* d_chi2, int32_t* d_flags);
 cudaError_t launch_jam_prep(glad_ctx* c, const float* d_dyn, int B, const float* d_lum, int nl, long lum_stride,
                             const float* d_mass, int nm, long mass_stride, const float* d_beta, int per_gaussian);
 cudaError_t launch_jam_quad(glad_ctx* c, int B, int nl, int nmx, int S);

@@ -466,3 +466,52 @@ cudaError_t launch_lens_image(glad_ctx* c, int B, float* d_images, float* d_chi2
                                                                   c->d_ivar, d_images, d_chi2, d_flags, nullptr, 0, c->d_lens_params_cur, nullptr, 0.0, 0.0, HaloArgs{nullptr, nullptr, nullptr, 0});
     return cudaGetLastError();
 }
+
+// ------------------------------------------------------------------------------------------------
+// glad_lens_image_noalloc: the same two kernels with the per-vector constants in a file-scope device array, for callers that
+// cannot allocate at call time.  In host code the array's NAME is a host-side stand-in, not a device address: the address the
+// kernels get is the one cudaGetSymbolAddress returns, taken once per device with that device current.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) float g_lens_const_noalloc[(size_t)GLAD_LENS_NOALLOC_MAX_B * LC_SIZE];
+
+#define LENS_NOALLOC_MAX_DEV 64
+static float* s_noalloc_addr[LENS_NOALLOC_MAX_DEV];      // per device; 0 = not taken yet
+
+cudaError_t lens_noalloc_setup(glad_ctx* c) {
+    c->d_lens_const_static = nullptr;
+    if (c->device < 0 || c->device >= LENS_NOALLOC_MAX_DEV) return cudaErrorInvalidDevice;
+    float* p = s_noalloc_addr[c->device];
+    if (!p) {
+        cudaError_t e = cudaGetSymbolAddress((void**)&p, g_lens_const_noalloc);
+        if (e != cudaSuccess) return e;
+        // the shared-memory opt-in of the image kernel is per function and per device: set here so that the call itself only launches
+        e = smem_optin(c, lens_image_kernel<true>);
+        if (e == cudaSuccess) e = smem_optin(c, lens_image_kernel<false>);
+        cudaFuncAttributes fa;                              // loads the first kernel's code now rather than at its first launch
+        if (e == cudaSuccess) e = cudaFuncGetAttributes(&fa, lens_prep_kernel);
+        if (e != cudaSuccess) return e;
+        s_noalloc_addr[c->device] = p;
+    }
+    c->d_lens_const_static = p;
+    return cudaSuccess;
+}
+
+cudaError_t launch_lens_noalloc(glad_ctx* c, const float* d_params, int B, float* d_images, float* d_chi2, int32_t* d_flags) {
+    float* consts = c->d_lens_const_static;
+    if (!consts || B > GLAD_LENS_NOALLOC_MAX_B) return cudaErrorInvalidValue;
+    const size_t smem = lens_image_smem_bytes(c->grid.nx, c->grid.ny, c->kpsf);
+    if (smem > (size_t)glad_smem_dynamic_max(c)) return cudaErrorInvalidConfiguration;
+    cudaStream_t st = c->stream;
+    const int ch = c->light_kinds != 0 || c->d_lambda != nullptr || c->d_enfw != nullptr;
+    lens_prep_kernel<<<(B + 31) / 32, 32 * LENS_PREP_ROLES, 0, st>>>(d_params, B, c->light_kinds, c->d_lambda, c->ms_rc, c->ms_rt,
+                                                                     c->d_enfw, consts);
+    if (ch)
+        lens_image_kernel<true><<<B, 512, smem, st>>>(consts, c->light_kinds, c->grid, c->d_psf, c->kpsf, c->d_data, c->d_ivar, d_images,
+                                                      d_chi2, d_flags, c->d_cse32, c->ncse, d_params, c->d_lambda, c->ms_rc, c->ms_rt,
+                                                      halo_args(c));
+    else
+        lens_image_kernel<false><<<B, 512, smem, st>>>(consts, 0, c->grid, c->d_psf, c->kpsf, c->d_data, c->d_ivar, d_images, d_chi2,
+                                                       d_flags, nullptr, 0, d_params, nullptr, 0.0, 0.0, HaloArgs{nullptr, nullptr, nullptr, 0});
+    c->launches += 2;
+    return cudaGetLastError();
+}
