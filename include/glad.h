@@ -279,7 +279,9 @@ glad_status glad_set_enfw(glad_ctx* ctx, const float* d_enfw, int n_enfw, int n_
  *   path         GLAD_JAM_AUTO: tcgen05 tensor-core contraction where the folded grid fits (<= 128 rows, terms * columns <= 256),
  *                the FP32 SIMT kernel otherwise; GLAD_JAM_SIMT: always the FP32 SIMT kernel.
  *   bf16_terms   operand values are split into 2 (default: 16 mantissa bits) or 3 (24 bits) bf16 terms on the tcgen05 path.
- *   flush_chunks operand chunks per TMEM accumulator group before the group is added into fp32 registers (default: 512 rows).
+ *   flush_chunks operand chunks per TMEM accumulator group before the group is added into fp32 registers (default: 512 contraction rows;
+ *                a chunk is the rows one producer group stages, 64 at the default sizes; never fewer than 2 * groups - 2 = 14 chunks,
+ *                which the reuse of the two TMEM buffers needs, so smaller values are raised to that).
  *   k_slices     CTAs per parameter vector along the contraction (default: enough for 4 CTAs per SM on small batches).
  * The arithmetic of a context therefore never depends on the caller's environment.  GLAD_EINVAL on a bad value.
  */

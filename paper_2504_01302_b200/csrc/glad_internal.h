@@ -81,7 +81,7 @@ struct glad_ctx {
     // row a6 options (glad_set_jam_options): nothing in the library reads the environment
     int jam_simt;   // 1 = force the FP32 SIMT quadrature kernel; default tcgen05 where the grid fits
     int jam_terms;  // bf16 terms per operand value on the tcgen05 path: 2 (default) or 3
-    int jam_flush;  // chunks per TMEM accumulator group, 0 = default (512 contraction rows)
+    int jam_flush;  // chunks per TMEM accumulator group, 0 = default (512 contraction rows, at least 2 * groups - 2 chunks)
     int jam_slices; // K-slices per vector, 0 = automatic
     // The two halves are independent until joint_kernel: glad_joint_loglike_batch forks the lens half onto a context-owned
     // side stream (event fork/join on the caller's stream, so the caller still sees plain stream order).  lens_stream is

@@ -23,15 +23,25 @@
 // octs of one K = 16 step.  A quarter-warp writes one core matrix with one conflict-free 16-byte store per lane.
 //
 // CTA = (parameter vector, K-slice), PW producer warps + 1 MMA warp, ONE CTA per SM, no CTA-wide barrier in the
-// main loop.  The kernel is latency-bound (profiles/r1b.md: ~10 cycles per instruction and warp), so the design
-// goal is resident warps and registers per warp: with one CTA per SM the running map is spread over PW/4 warps per
-// TMEM lane quarter (80 columns -> 16..24 accumulator registers per thread instead of 40).
-//   producer warp, chunk c (MC contraction rows):  wait until the MMAs that read stage c%2 have completed
-//   (mbarrier armed by tcgen05.commit) -> add finished accumulator groups into registers -> every R-th chunk one
-//   coefficient row of chunk c+2 -> its blocks of chunk c into stage c%2 -> fence.proxy.async -> bar.arrive on
-//   the stage's "full" named barrier (does not block).
-//   MMA warp, chunk c:  bar.sync on "full" -> one lane issues the MMAs of the chunk and commits to "empty".
-//   The tensor core works on chunk c while the CUDA cores produce chunk c+1.
+// main loop.  The producer warps form G groups that take the chunks in turn (group g: chunks g, g+G, ..), each
+// group into its own operand stage of MC rows.  The groups drift apart, so one group's MUFU-heavy operand loop runs
+// beside another group's coefficient rows, accumulator adds and waits (in lock step, two stages of 256 rows shared
+// by all warps, the XU pipe limited the operand loops and idled in between: profiles/r2.md).  With MC = the group's
+// threads a thread owns one oct over ALL its pixel blocks, so the per-chunk costs (wait, coefficient loads, fence,
+// arrive) are paid once per oct and (n_y + n_x)/8 blocks.
+//   group g, its i-th chunk c = G i + g (MC contraction rows):  wait until the MMAs that read stage g have completed
+//   (mbarrier armed by tcgen05.commit) -> add finished accumulator groups into registers -> the oct's blocks of
+//   chunk c into stage g -> fence.proxy.async -> bar.arrive on the stage's "full" named barrier (does not block)
+//   -> every R-th chunk one coefficient row of later chunks (in the shadow of the MMAs just released).
+//   MMA warp, chunk c (in order):  bar.sync on "full" of stage c%G -> an elected lane issues the MMAs and commits to
+//   the stage's "empty" mbarrier.  Its loop body is the latency a group sees between arrive and release, so it is
+//   kept short: convergent code, warp-uniform operands, descriptors carried from chunk to chunk.
+//
+// Tried and measured on C2 (1024 vectors, B200), not kept: the X side factorised as e^{-A x^2} = E1[iu,j](x) G[k](x)
+// with G in shared memory cuts the XU pipe from 55 % to 36 % but adds 444 shared-memory load
+// wavefronts per 256 rows, and LSU + tensor-core wavefronts then fill 98 % of the shared-memory pipe: 1.94 ms against
+// 1.93 without it.  Adding accumulator groups early (before the group's own wait) and two blocks in flight without
+// register copies were 2-3 % slower.
 #include "glad_internal.h"
 
 #define LOG2E_F 1.4426950408889634f
@@ -43,9 +53,10 @@ struct JTArgs {
     int ny8, nxp;        // padded map rows (multiple of 8) and columns (multiple of 8 or 16)
     int multi;           // 0: A = [Y1;..;Y_NT] in one M=128 tile;  1: NT MMAs per K-step
     int N;               // accumulator columns = NT * nxp
-    int MC, lgMC;        // contraction rows per stage (128 or 256)
+    int MC, lgMC;        // contraction rows per chunk = per stage (32 .. 256)
+    int G, lgG;          // producer groups = operand stages (2, 4 or 8)
     int FL;              // chunks per accumulator group (>= 1)
-    int cslots;          // coefficient ring slots (power of two >= NPROD/MC + 3)
+    int cslots;          // coefficient ring slots: G * (power of two >= NPROD/G/MC + 2), slot = chunk % cslots
     int tmem_cols;       // power of two >= 2 * N
     int S;
     float* partial;
@@ -76,6 +87,19 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes
 __device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// the same from convergent code with warp-uniform operands: one elected lane issues (the operands can then stay in
+// uniform registers; issued from inside an `if (lane == 0)` every MMA costs a 16-instruction broadcast loop)
+// (descriptors as their low words plus the common high word: only the low word moves from MMA to MMA)
+__device__ __forceinline__ void umma_bf16_elect(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t desc_hi, uint32_t idesc, uint32_t accumulate) {
+    asm volatile("{\n\t.reg .pred p, e;\n\t.reg .b64 da, db;\n\telect.sync _|e, 0xffffffff;\n\tsetp.ne.b32 p, %5, 0;\n\t"
+                 "mov.b64 da, {%1, %3};\n\tmov.b64 db, {%2, %3};\n\t"
+                 "@e tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %4, p;\n\t}"
+                 ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(desc_hi), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit_elect(uint32_t bar) {
+    asm volatile("{\n\t.reg .pred e;\n\telect.sync _|e, 0xffffffff;\n\t"
+                 "@e tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
@@ -131,8 +155,9 @@ __device__ __forceinline__ void bar_sync(int id, int count) { asm volatile("bar.
 template <int NT, int NACC, int PW>
 __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) {
     constexpr int NPROD = PW * 32, NTHR = NPROD + 32;
+    const int G = a.G, GW = PW >> a.lgG, GT = GW * 32;     // producer groups; warps and threads per group
     extern __shared__ __align__(128) float sm[];
-    __shared__ __align__(8) uint64_t s_bar[3];     // empty[0], empty[1], done
+    __shared__ __align__(8) uint64_t s_bar[9];     // empty[0 .. G-1], done at [8]
     __shared__ uint32_t s_tmem;
     __shared__ int s_stride[3];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -160,7 +185,7 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
     float* s_c2 = s_ld + ((nl + 3) & ~3);            // ny8 + nxp squared coordinates, y first
     // coefficient ring: a.cslots chunks, per chunk [-Q log2e | -P log2e | F0 | F1] x MC floats
     float* s_coef = sm + ((4 * nl + 4 * nmx + 2 * nmx * nl + 2 * nu + ((nl + 3) & ~3) + ny8 + nxp + 31) & ~31);
-    uint4* s_ops = reinterpret_cast<uint4*>(s_coef + a.cslots * 4 * MC);   // 2 stages + tail pad, 128-byte aligned
+    uint4* s_ops = reinterpret_cast<uint4*>(s_coef + a.cslots * 4 * MC);   // G stages + tail pad, 128-byte aligned
 
     for (int k = tid; k < nl; k += NTHR) {
         s_lk[k] = make_float4(TLg[JL_INVS2 * nl + k], TLg[JL_BKQ * nl + k], TLg[JL_S0 * nl + k], TLg[JL_NKS * nl + k]);
@@ -176,11 +201,9 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
         else { int j = i - ny8; if (j < a.nxf) v = a.xf2[j]; }
         s_c2[i] = v;
     }
-    for (int i = tid; i < 2 * stage16 + 128; i += NTHR) s_ops[i] = make_uint4(0u, 0u, 0u, 0u);
+    for (int i = tid; i < G * stage16 + 128; i += NTHR) s_ops[i] = make_uint4(0u, 0u, 0u, 0u);
     if (tid == 0) {
-        mbar_init(smem_u32(&s_bar[0]), 1);
-        mbar_init(smem_u32(&s_bar[1]), 1);
-        mbar_init(smem_u32(&s_bar[2]), 1);
+        for (int i = 0; i < 9; ++i) mbar_init(smem_u32(&s_bar[i]), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 0) {
@@ -204,58 +227,67 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
 
     if (warp == PW) {
         // ------------------------------------------------------------------ MMA warp
+        // The loop body is the latency between a group's arrive and the release of its stage: everything that can be
+        // carried from one chunk to the next is (stage descriptors, accumulator group), no division, no multiply.
         // instruction descriptor: D fp32, A/B bf16, both K-major, M = 128, N>>3 filled per MMA
         const uint32_t idesc_base = (1u << 4) | (1u << 7) | (1u << 10) | (8u << 24);
         const uint32_t ops_addr = smem_u32(s_ops);
         const uint32_t a_lbo = GA * 128, b_lbo = GB * 128;              // bytes between the two octs of a K-step
+        // descriptors advance by one K-step (two octs) per MMA and by one stage per chunk: only the 14-bit
+        // start-address field (16-byte units) changes
+        const uint32_t desc_hi = (128u >> 4) | (1u << 14);              // SBO = 128 B, version 1 (as umma_desc)
+        const uint32_t ad0 = ((ops_addr >> 4) & 0x3FFFu) | (((a_lbo >> 4) & 0x3FFFu) << 16);
+        const uint32_t bd0 = (((ops_addr + a16 * 16) >> 4) & 0x3FFFu) | (((b_lbo >> 4) & 0x3FFFu) << 16);
+        const uint32_t ad_step = (2 * a_lbo) >> 4, bd_step = (2 * b_lbo) >> 4;
+        const uint32_t idesc1 = idesc_base | ((uint32_t)(N >> 3) << 17);
+        const uint32_t bar0 = smem_u32(&s_bar[0]);
+        const int nks = MC >> 4;
+        uint32_t ad_s = ad0, bd_s = bd0;
+        int buf = 0, fl = 0;                                            // stage; chunk within the accumulator group
+        uint32_t d = tmem;                                              // warp-uniform
         for (int it = 0; it < nch; ++it) {
-            const int buf = it & 1;
-            bar_sync(1 + buf, NTHR);                                    // every producer has written its share of chunk it
-            if (lane == 0) {
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const int g = it / a.FL;
-                const uint32_t d = tmem + (uint32_t)(g & 1) * dstride;
-                const uint32_t sa = ops_addr + (uint32_t)buf * stage16 * 16, sb = sa + a16 * 16;
-                uint32_t accum = (it - g * a.FL) ? 1u : 0u;
-                // descriptors advance by one K-step (two octs) per MMA: only the 14-bit start-address field changes
-                uint64_t ad = umma_desc(sa, a_lbo), bd = umma_desc(sb, b_lbo);
-                const uint64_t ad_step = (uint64_t)((2 * a_lbo) >> 4), bd_step = (uint64_t)((2 * b_lbo) >> 4);
-                const uint32_t idesc1 = idesc_base | ((uint32_t)(N >> 3) << 17);
-                if (!a.multi) {
+            bar_sync(1 + buf, GT + 32);                                 // group it%G has written chunk it into its stage
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            uint32_t accum = fl ? 1u : 0u;
+            uint32_t ad = ad_s, bd = bd_s;
+            if (!a.multi) {
 #pragma unroll 4
-                    for (int ks = 0; ks < (MC >> 4); ++ks) {
-                        umma_bf16(d, ad, bd, idesc1, accum);
-                        accum = 1u; ad += ad_step; bd += bd_step;
-                    }
-                } else {
-                    for (int ks = 0; ks < (MC >> 4); ++ks) {
-#pragma unroll
-                        for (int t = 0; t < NT; ++t) {
-                            umma_bf16(d, ad + (uint64_t)((t * nyb * 128) >> 4), bd,
-                                      idesc_base | ((uint32_t)(((NT - t) * nxp) >> 3) << 17), accum);
-                            accum = 1u;
-                        }
-                        ad += ad_step; bd += bd_step;
-                    }
+                for (int ks = 0; ks < nks; ++ks) {
+                    umma_bf16_elect(d, ad, bd, desc_hi, idesc1, accum);
+                    accum = 1u; ad += ad_step; bd += bd_step;
                 }
-                umma_commit(smem_u32(&s_bar[buf]));
-                if (it == nch - 1) umma_commit(smem_u32(&s_bar[2]));
+            } else {
+                for (int ks = 0; ks < nks; ++ks) {
+#pragma unroll
+                    for (int t = 0; t < NT; ++t) {
+                        umma_bf16_elect(d, ad + (uint32_t)((t * nyb * 128) >> 4), bd, desc_hi,
+                                        idesc_base | ((uint32_t)(((NT - t) * nxp) >> 3) << 17), accum);
+                        accum = 1u;
+                    }
+                    ad += ad_step; bd += bd_step;
+                }
             }
-            __syncwarp();
+            umma_commit_elect(bar0 + 8 * buf);
+            if (it == nch - 1) umma_commit_elect(bar0 + 64);
+            ++buf; ad_s += (uint32_t)stage16; bd_s += (uint32_t)stage16;
+            if (buf == G) { buf = 0; ad_s = ad0; bd_s = bd0; }
+            if (++fl == a.FL) { fl = 0; d = d == tmem ? tmem + dstride : tmem; }
         }
     } else {
         // ------------------------------------------------------------------ producer warps
         const float cos2i = Tg[JH_COS2I];
         const float inv_pairs = 1.f / (float)pairs, inv_nl = 1.f / (float)nl;
+        const int grp = warp / GW, lw = warp - grp * GW, lt = tid - grp * GT;   // producer group, warp and thread in it
 
         // Coefficients of contraction row m = (iu, j, k), k fastest: (-Q log2e, -P log2e, F0, F1); rows past the end have
-        // F0 = F1 = 0 and contribute 0.  Chunk `rc` (relative to c0) lives in ring slot rc % cslots.  Every R-th
-        // iteration (R = NPROD / MC) ALL producer threads write one row each of chunks it+2 .. it+R+1, so the warps stay
-        // in step (a group taking turns would skew them by one coefficient block per chunk, and with two operand
-        // stages any skew ends in the "empty" wait).  A chunk is therefore written at iteration <= rc-2 and read during
-        // iteration rc: the reader has passed the "empty" wait of chunk rc-2, so every producer has arrived on "full"
-        // of rc-2, i.e. finished writing.  While a thread writes in iteration `it` the slowest warp can still be
-        // reading chunk it-1 (the writer passed the "empty" wait of it-2): slots it-1 .. it+R+1 are live, cslots >= R+3.
+        // F0 = F1 = 0 and contribute 0.  Chunk `rc` (relative to c0) lives in ring slot rc % cslots, so the groups use
+        // alternate slots.  After every R-th chunk of the group (R = GT / MC) ALL its threads write one row each of the
+        // group's chunks i+2 .. i+R+1 (i = the chunk just handed to the MMA warp), so the warps of a group stay in step.
+        // A chunk is therefore written during iteration <= i'-2 and read during iteration i': the reader has passed
+        // the "empty" wait of chunk i'-1, so every thread of the group has arrived on "full" of i'-1, which in program
+        // order follows its coefficient writes of iteration i'-2.  While a thread writes in iteration i the slowest
+        // warp of the group can still be reading chunk i (the writer passed the "empty" wait of i-1): the group's
+        // slots i .. i+R+1 are live, cslots/2 >= R+2.
         // one row from its (iu, j, k): 3 MUFU.RCP + 1 MUFU.RSQ (approx, <= 2 ulp: the operands carry 16 bits)
         auto coef_store = [&](int rc, int r, int iu, int j, int k) {
             float cq = 0.f, cp = 0.f, f0 = 0.f, f1 = 0.f;
@@ -289,20 +321,20 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
             const int j = div_small(rem, nl, inv_nl), k = rem - j * nl;
             coef_store(rc, r, iu, j, k);
         };
-        const int R = NPROD / MC;                                       // producer thread groups of MC threads
-        const int cgrp = tid / MC, crow = tid - cgrp * MC;
+        const int R = GT / MC;                                          // thread sets of MC threads in a group
+        const int cgrp = lt / MC, crow = lt - cgrp * MC;
 
         // Quarter-warp = one oct of the chunk (8 contraction rows), lane l8 = pixel within an 8-pixel block.  The
         // thread loads the 8 rows' coefficients once (LDS.128 delivers 512 B per warp whatever the broadcast) and
-        // reuses them over its blocks.  The oct's block list [Y blocks | X blocks] is cut into NQ contiguous ranges
-        // of about equal cost (profiles/r1c.md: a Y block is 51 issue slots, an X block 53); a warp holds one range
-        // index ("role") and four octs.  Roles alternate every four warps so that each of the SM's four schedulers
-        // (warp % 4) sees every role: the ranges are never exactly equal.
-        const int qw = tid >> 3, l8 = tid & 7;
-        const int NQ = (NPROD >> 3) / (MC >> 3);                        // quarter-warps per oct: 2, 4 or 8
-        const bool mix = (PW % (4 * NQ)) == 0;
-        const int role = mix ? (warp >> 2) % NQ : warp % NQ;
-        const int oct = (qw & 3) + 4 * (mix ? (warp & 3) + 4 * (warp / (4 * NQ)) : warp / NQ);
+        // reuses them over its blocks.  With MC = GT a quarter-warp owns its oct's whole block list [Y blocks | X blocks];
+        // with smaller chunks the list is cut into NQ = GT / MC contiguous ranges of about equal cost (a Y block is
+        // about 20, an X block 21 units); a warp holds one range index ("role") and four octs.  Roles alternate every
+        // four warps so that each of the SM's four schedulers (warp % 4) sees every role: the ranges are never equal.
+        const int qw = lt >> 3, l8 = lt & 7;
+        const int NQ = R;                                               // quarter-warps per oct: 1, 2 or 4
+        const bool mix = (GW % (4 * NQ)) == 0;
+        const int role = mix ? (lw >> 2) % NQ : lw % NQ;
+        const int oct = (qw & 3) + 4 * (mix ? (lw & 3) + 4 * (lw / (4 * NQ)) : lw / NQ);
         int yb0, yb1, xb0, xb1;
         {
             const int ctot = 20 * nyb + 21 * nxb;
@@ -327,8 +359,8 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
         const int offA = oct * GA * 8 + l8 + yb0 * 8, offB = a16 + oct * GB * 8 + l8 + xb0 * 8;
         const int nyblk = yb1 - yb0, nxblk = xb1 - xb0;
         const int tsA = nyb * 8, tsB = nxb * 8;                          // 16-byte units between the bf16 terms of a value
-        auto produce = [&](int it, int buf) {
-            const float* cb = s_coef + (it & (a.cslots - 1)) * (4 * MC) + 8 * oct;
+        auto produce = [&](int rc, int buf) {
+            const float* cb = s_coef + (rc & (a.cslots - 1)) * (4 * MC) + 8 * oct;
             uint4* const stage = s_ops + buf * stage16;
             if (nyblk > 0) {
                 const float4 e0 = *reinterpret_cast<const float4*>(cb), e1 = *reinterpret_cast<const float4*>(cb + 4);
@@ -410,50 +442,58 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         };
 
+        // The MMA warp starts chunk c after the MMAs of c-1 .. c-G+1 were issued, i.e. after every other group passed
+        // the wait before its latest chunk c' > c-G and added the accumulator groups complete by c'-G >= c-2G+1; this
+        // group has added those complete by c-G.  The TMEM buffer that chunk c re-initialises held the accumulator
+        // group that ended with chunk c - FL - 1: FL >= 2G - 2.
         int gf = 0;                                                     // next accumulator group to add into acc
-        const uint32_t bar_empty = smem_u32(&s_bar[0]);
+        const uint32_t bar_empty = smem_u32(&s_bar[grp]);
         if (tid == 0) {                                                 // the stride NPROD as (du, dj, dk): CTA-uniform, kept in smem
             const int sdu = div_small(NPROD, pairs, inv_pairs), srem = NPROD - sdu * pairs;
             const int sdj = div_small(srem, nl, inv_nl);
             s_stride[0] = sdu; s_stride[1] = sdj; s_stride[2] = srem - sdj * nl;
         }
         if (nch > 0) {
-            if (cgrp < 2 && cgrp < nch) coef_row(cgrp, crow);           // chunks 0 and 1
-            bar_sync(3, NPROD);
+            for (int e = cgrp; e < 2; e += R)                           // the group's first two chunks
+                if (grp + G * e < nch) coef_row(grp + G * e, crow);
+            bar_sync(9, NPROD);
         }
-        int cphase = 0;                                                 // it % R
-        // In the loop a thread's rows advance by NPROD contraction rows per call: (iu, j, k) is carried, not divided.
+        int cphase = 0;                                                 // i % R
+        // In the loop a thread's rows advance by R chunks of the group = NPROD contraction rows per call: (iu, j, k) is
+        // carried, not divided.
         int ciu, cj, ck;
         {
-            const int m0 = (c0 + 2 + cgrp) * MC + crow;
+            const int m0 = (c0 + grp + G * (2 + cgrp)) * MC + crow;
             ciu = div_small(m0, pairs, inv_pairs);
             const int rem = m0 - ciu * pairs;
             cj = div_small(rem, nl, inv_nl); ck = rem - cj * nl;
         }
-        for (int it = 0; it < nch; ++it) {
-            const int buf = it & 1;
-            if (it >= 2) {
-                mbar_wait(bar_empty + 8 * buf, ((it >> 1) - 1) & 1);    // MMAs up to chunk it-2 are complete
+        const int ng = (nch - grp + G - 1) >> a.lgG;                    // chunks of this group
+        for (int i = 0; i < ng; ++i) {
+            const int rc = grp + G * i;
+            if (i >= 1) {
+                mbar_wait(bar_empty, (i - 1) & 1);                      // the MMAs of the group's previous chunk are complete
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                while ((gf + 1) * a.FL - 1 <= it - 2) flush(gf++);
+                while ((gf + 1) * a.FL - 1 <= rc - G) flush(gf++);
             }
-            if (cphase == 0) {                                          // chunks it+2 .. it+R+1, one row per thread
-                if (it + 2 + cgrp < nch) coef_store(it + 2 + cgrp, crow, ciu, cj, ck);
+            produce(rc, grp);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            bar_arrive(1 + grp, GT + 32);
+            if (cphase == 0) {                                          // the group's chunks i+2 .. i+R+1, one row per thread
+                const int rcw = rc + G * (2 + cgrp);
+                if (rcw < nch) coef_store(rcw, crow, ciu, cj, ck);
                 ck += s_stride[2]; if (ck >= nl) { ck -= nl; ++cj; }
                 cj += s_stride[1]; if (cj >= nm) { cj -= nm; ++ciu; }
                 ciu += s_stride[0];
             }
             cphase = cphase + 1 == R ? 0 : cphase + 1;
-            produce(it, buf);
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            bar_arrive(1 + buf, NTHR);
         }
 
         // epilogue: remaining groups -> registers -> shared memory (fold the term blocks) -> this slice's partial map
         const int npf = a.nxf * a.nyf;
         float* out = a.partial + ((size_t)b * a.S + s) * npf;
         if (nch > 0) {
-            mbar_wait(smem_u32(&s_bar[2]), 0);                           // all MMAs done: the stages are free
+            mbar_wait(smem_u32(&s_bar[8]), 0);                           // all MMAs done: the stages are free
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             while (gf * a.FL < nch) flush(gf++);
             float* scr = reinterpret_cast<float*>(s_ops);                // [128][nxp]
@@ -463,7 +503,7 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
                 const int col = cg * NACC + i;
                 if (col < nxp) scr[row * nxp + col] = acc[i];
             }
-            bar_sync(3, NPROD);
+            bar_sync(9, NPROD);
             const int TR = a.multi ? 1 : NT;
             for (int i = tid; i < npf; i += NPROD) {
                 const int iy = i / a.nxf, ix = i - iy * a.nxf;
@@ -483,6 +523,7 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
 // bf16 terms per operand: 2 by default (16 mantissa bits, per-term error <= 2^-16), 3 after glad_set_jam_options(.., 3, ..)
 static int tc_terms(const glad_ctx* c) { return c->jam_terms == 3 ? 3 : 2; }
 #define TC_PW 16    // producer warps per CTA (24 was tried: 72 registers per thread spill, slower)
+#define TC_GROUPS 8 // producer groups = operand stages (measured on C2: 2 -> 2.05 ms, 4 -> 1.97, 8 -> 1.92)
 
 // launch plan for the current sky grid and table sizes; false = not supported (the FP32 kernel takes over)
 static bool tc_plan(const glad_ctx* c, int nl, int nmx, JTArgs* a, int* nacc, size_t* smem) {
@@ -498,11 +539,19 @@ static bool tc_plan(const glad_ctx* c, int nl, int nmx, JTArgs* a, int* nacc, si
     a->tmem_cols = 512;                                                  // one CTA per SM: two accumulator buffers of 256 columns
     const size_t fixed = (((size_t)4 * nl + 4 * nmx + 2 * (size_t)nmx * nl + 2 * (size_t)c->nu + ((nl + 3) & ~3) +
                            (size_t)(a->ny8 + a->nxp) + 31) & ~(size_t)31) * 4;
-    for (a->MC = 256, a->lgMC = 8; a->MC >= 64; a->MC >>= 1, --a->lgMC) {
-        size_t ops = 2 * (size_t)a->MC * NT * (a->ny8 + a->nxp) * 2 + 2048;   // two stages + the M = 128 over-read
+    // RT = contraction rows in flight (all stages): with RT = producer threads a quarter-warp owns its oct's whole
+    // block list; each halving doubles the quarter-warps per oct
+    for (int RT = PW * 32; RT >= PW * 8; RT >>= 1) {
+        a->G = TC_GROUPS;
+        while (RT / a->G < 32) a->G >>= 1;                                   // a warp's quarters take 4 different octs of a chunk
+        for (a->lgG = 0; (1 << a->lgG) < a->G; ++a->lgG) {}
+        a->MC = RT >> a->lgG;
+        for (a->lgMC = 0; (1 << a->lgMC) < a->MC; ++a->lgMC) {}
+        size_t ops = (size_t)RT * NT * (a->ny8 + a->nxp) * 2 + 2048;         // G stages + the M = 128 over-read
         const size_t scr = (size_t)128 * a->nxp * 4;                         // epilogue scratch reuses the stages
         if (ops < scr) ops = scr;
-        a->cslots = (PW * 32 / a->MC) <= 4 ? 8 : 16;
+        const int R = PW * 32 / RT;                                          // group threads / MC
+        a->cslots = a->G * (R <= 2 ? 4 : 8);                                 // G * pow2(R + 2)
         *smem = fixed + (size_t)a->cslots * 4 * a->MC * 4 + ops;
         if (*smem <= 225 * 1024) return true;
     }
@@ -534,8 +583,11 @@ cudaError_t launch_jam_quad_tc(glad_ctx* c, int B, int nl, int nmx, int S) {
     a.un = c->d_un; a.uw = c->d_uw; a.nu = c->nu;
     a.xf2 = c->d_xf2; a.yf2 = c->d_yf2; a.nxf = c->nxf; a.nyf = c->nyf;
     a.S = S; a.partial = c->d_partial;
+    // 512 contraction rows (32 K-steps) per accumulator group, but not fewer chunks than the kernel's TMEM buffer
+    // reuse argument needs (2G - 2)
     a.FL = 512 / a.MC;
     if (c->jam_flush >= 1) a.FL = c->jam_flush;
+    if (a.FL < 2 * a.G - 2) a.FL = 2 * a.G - 2;
     ProfScope ps(c, GK_JAM_QUAD);
     return tc_terms(c) == 3 ? tc_dispatch<3>(c, a, nacc, B * S, smem, c->stream) : tc_dispatch<2>(c, a, nacc, B * S, smem, c->stream);
 }
