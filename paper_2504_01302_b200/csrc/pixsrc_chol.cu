@@ -118,15 +118,25 @@ __device__ __forceinline__ void ch_cp_async8(void* smem, const void* gmem) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gmem) : "memory");
 }
 
+// D (8 x 8) = A (8 x 4, row-major) B (4 x 8, column-major) + C on the fp64 tensor-core path: a thread holds A[lane/4][lane%4],
+// B[lane%4][lane/4] and C[lane/4][2 (lane%4) + {0, 1}]
+__device__ __forceinline__ void ch_dmma(double& d0, double& d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+#define CH_PU 68           // pitch (doubles) of the update kernel's tiles: 2 * 68 mod 32 = 8, so the 16 lanes of a half-warp
+                           // (4 rows x 4 consecutive k) read 16 different bank pairs
+
 // A[i, j] -= sum_k L21[i, k] L21[j, k] on the trailing lower triangle (rows / columns >= r0).  CTA = (row of 64 x 64 tiles ti, matrix):
 // the panel rows of ti stay in shared memory, those of tj = 0 .. ti stream through a double buffer filled by cp.async one tile
-// ahead (row-major [row][k], pitch 65 doubles: 8-byte copies, conflict-free reads), and the A tile is fetched into registers before
-// the 1024 DFMAs of a thread.  Rows of tiles are handed out longest first.  (One tile per CTA with a synchronous transposing load:
-// 32 % of the DFMA rate.)
+// ahead (row-major [row][k]: 8-byte copies), and the A tile is fetched into registers before the tile product.  The product runs
+// as DMMA m8n8k4 (warp = 16 x 32 outputs = 2 x 4 fragments: 6 shared-memory loads per 8 DMMAs = 64 multiply-adds per thread; the
+// 4 x 4 DFMA form it replaces needed 8 loads per 16 and stopped at 45 % of the fp64 pipe: profiles/r2.md).  Rows of tiles are
+// handed out longest first.
 __global__ void __launch_bounds__(256, 2) chol_update_kernel(double* __restrict__ A, int ns, int k0, int nt) {
     extern __shared__ double ch_sm[];
     double* Pi = ch_sm;
-    double* Pj = ch_sm + CH_NB * CH_P;      // two buffers
+    double* Pj = ch_sm + CH_NB * CH_PU;     // two buffers
     const int b = blockIdx.y, tid = threadIdx.x;
     const int ti = nt - 1 - (int)blockIdx.x;
     const int r0 = k0 + CH_NB, ib = r0 + ti * CH_NB;
@@ -135,47 +145,56 @@ __global__ void __launch_bounds__(256, 2) chol_update_kernel(double* __restrict_
 #pragma unroll
         for (int it = 0; it < (CH_NB * CH_NB) / 256; ++it) {
             const int e = tid + it * 256, r = e >> 6, k = e & 63;
-            if (rb + r < ns) ch_cp_async8(dst + r * CH_P + k, Ab + (size_t)(rb + r) * ns + k0 + k);
-            else dst[r * CH_P + k] = 0.0;
+            if (rb + r < ns) ch_cp_async8(dst + r * CH_PU + k, Ab + (size_t)(rb + r) * ns + k0 + k);
+            else dst[r * CH_PU + k] = 0.0;
         }
         asm volatile("cp.async.commit_group;\n" ::: "memory");
     };
     fill(Pi, ib);
     fill(Pj, r0);
-    const int ty = tid >> 4, tx = tid & 15;
+    const int warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
+    const int wr = (warp >> 1) * 16, wc = (warp & 1) * 32;      // the warp's 16 rows and 32 columns of the tile
+    const double* pa = Pi + (wr + g) * CH_PU + q;
     for (int tj = 0; tj <= ti; ++tj) {
         const int jb = r0 + tj * CH_NB;
-        double* Pc = Pj + (tj & 1) * CH_NB * CH_P;
-        if (tj < ti) fill(Pj + ((tj + 1) & 1) * CH_NB * CH_P, jb + CH_NB);
-        double cur[4][4], acc[4][4];
+        const double* Pc = Pj + (tj & 1) * CH_NB * CH_PU;
+        if (tj < ti) fill(Pj + ((tj + 1) & 1) * CH_NB * CH_PU, jb + CH_NB);
+        double cur[2][4][2], acc[2][4][2];
 #pragma unroll
-        for (int r = 0; r < 4; ++r)
+        for (int m = 0; m < 2; ++m)
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const int i = ib + ty * 4 + r, j = jb + tx + 16 * c;
-                cur[r][c] = (i < ns && j <= i) ? Ab[(size_t)i * ns + j] : 0.0;
-                acc[r][c] = 0.0;
-            }
+            for (int n = 0; n < 4; ++n)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int i = ib + wr + 8 * m + g, j = jb + wc + 8 * n + 2 * q + e;
+                    cur[m][n][e] = (i < ns && j <= i) ? Ab[(size_t)i * ns + j] : 0.0;
+                    acc[m][n][e] = 0.0;
+                }
         if (tj < ti) asm volatile("cp.async.wait_group 1;\n" ::: "memory");
         else asm volatile("cp.async.wait_group 0;\n" ::: "memory");
         __syncthreads();
-#pragma unroll 8
-        for (int k = 0; k < CH_NB; ++k) {
-            double ar[4], br[4];
+        const double* pb = Pc + (wc + g) * CH_PU + q;
+#pragma unroll 4
+        for (int k = 0; k < CH_NB; k += 4) {
+            double ar[2], br[4];
 #pragma unroll
-            for (int r = 0; r < 4; ++r) { ar[r] = Pi[(ty * 4 + r) * CH_P + k]; br[r] = Pc[(tx + 16 * r) * CH_P + k]; }
+            for (int m = 0; m < 2; ++m) ar[m] = pa[m * 8 * CH_PU + k];
 #pragma unroll
-            for (int r = 0; r < 4; ++r)
+            for (int n = 0; n < 4; ++n) br[n] = pb[n * 8 * CH_PU + k];
 #pragma unroll
-                for (int c = 0; c < 4; ++c) acc[r][c] = fma(ar[r], br[c], acc[r][c]);
+            for (int m = 0; m < 2; ++m)
+#pragma unroll
+                for (int n = 0; n < 4; ++n) ch_dmma(acc[m][n][0], acc[m][n][1], ar[m], br[n]);
         }
 #pragma unroll
-        for (int r = 0; r < 4; ++r)
+        for (int m = 0; m < 2; ++m)
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                const int i = ib + ty * 4 + r, j = jb + tx + 16 * c;
-                if (i < ns && j <= i) Ab[(size_t)i * ns + j] = cur[r][c] - acc[r][c];
-            }
+            for (int n = 0; n < 4; ++n)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int i = ib + wr + 8 * m + g, j = jb + wc + 8 * n + 2 * q + e;
+                    if (i < ns && j <= i) Ab[(size_t)i * ns + j] = cur[m][n][e] - acc[m][n][e];
+                }
         __syncthreads();                   // the buffer just read is refilled by the next iteration's prefetch
     }
 }
@@ -185,7 +204,7 @@ size_t pixsrc_factor_scratch_bytes(int Bc) { return sizeof(double) * (size_t)Bc 
 
 // Winv: scratch of pixsrc_factor_scratch_bytes(Bc)
 cudaError_t launch_pixsrc_factor(glad_ctx* c, cudaStream_t st, double* A, int ns, int Bc, double* out, double* Winv) {
-    const size_t sm_trsm = sizeof(double) * 2 * CH_NB * CH_P, sm_upd = sizeof(double) * 3 * CH_NB * CH_P;
+    const size_t sm_trsm = sizeof(double) * 2 * CH_NB * CH_P, sm_upd = sizeof(double) * 3 * CH_NB * CH_PU;
     cudaError_t e = smem_optin(c, chol_update_kernel);
     if (e == cudaSuccess) e = smem_optin(c, chol_trsm_kernel);
     if (e != cudaSuccess) return e;
