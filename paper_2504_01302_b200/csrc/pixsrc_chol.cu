@@ -133,6 +133,13 @@ __device__ __forceinline__ void ch_dmma(double& d0, double& d1, double a, double
 // as DMMA m8n8k4 (warp = 16 x 32 outputs = 2 x 4 fragments: 6 shared-memory loads per 8 DMMAs = 64 multiply-adds per thread; the
 // 4 x 4 DFMA form it replaces needed 8 loads per 16 and stopped at 45 % of the fp64 pipe: profiles/r2.md).  Rows of tiles are
 // handed out longest first.
+__device__ __forceinline__ void ch_cp_async16(void* smem, const void* gmem) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(gmem) : "memory");
+}
+
+// EVEN: n_s is even, so every row of A starts on a 16-byte boundary and pairs of columns move as one 16-byte access
+template <bool EVEN>
 __global__ void __launch_bounds__(256, 2) chol_update_kernel(double* __restrict__ A, int ns, int k0, int nt) {
     extern __shared__ double ch_sm[];
     double* Pi = ch_sm;
@@ -142,11 +149,20 @@ __global__ void __launch_bounds__(256, 2) chol_update_kernel(double* __restrict_
     const int r0 = k0 + CH_NB, ib = r0 + ti * CH_NB;
     double* Ab = A + (size_t)b * ns * ns;
     auto fill = [&](double* dst, int rb) {         // rows rb .. rb + 63, columns k0 .. k0 + 63 of the panel
+        if (EVEN) {
 #pragma unroll
-        for (int it = 0; it < (CH_NB * CH_NB) / 256; ++it) {
-            const int e = tid + it * 256, r = e >> 6, k = e & 63;
-            if (rb + r < ns) ch_cp_async8(dst + r * CH_PU + k, Ab + (size_t)(rb + r) * ns + k0 + k);
-            else dst[r * CH_PU + k] = 0.0;
+            for (int it = 0; it < (CH_NB * CH_NB) / 512; ++it) {
+                const int e = tid + it * 256, r = e >> 5, k = (e & 31) * 2;
+                if (rb + r < ns) ch_cp_async16(dst + r * CH_PU + k, Ab + (size_t)(rb + r) * ns + k0 + k);
+                else { dst[r * CH_PU + k] = 0.0; dst[r * CH_PU + k + 1] = 0.0; }
+            }
+        } else {
+#pragma unroll
+            for (int it = 0; it < (CH_NB * CH_NB) / 256; ++it) {
+                const int e = tid + it * 256, r = e >> 6, k = e & 63;
+                if (rb + r < ns) ch_cp_async8(dst + r * CH_PU + k, Ab + (size_t)(rb + r) * ns + k0 + k);
+                else dst[r * CH_PU + k] = 0.0;
+            }
         }
         asm volatile("cp.async.commit_group;\n" ::: "memory");
     };
@@ -163,13 +179,17 @@ __global__ void __launch_bounds__(256, 2) chol_update_kernel(double* __restrict_
 #pragma unroll
         for (int m = 0; m < 2; ++m)
 #pragma unroll
-            for (int n = 0; n < 4; ++n)
+            for (int n = 0; n < 4; ++n) {
+                const int i = ib + wr + 8 * m + g, j = jb + wc + 8 * n + 2 * q;
+                if (EVEN) {                 // j is even and j <= i < n_s: j + 1 < n_s too, the pair is inside the row
+                    const double2 v = (i < ns && j <= i) ? *reinterpret_cast<const double2*>(Ab + (size_t)i * ns + j) : make_double2(0.0, 0.0);
+                    cur[m][n][0] = v.x; cur[m][n][1] = v.y;
+                } else {
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int i = ib + wr + 8 * m + g, j = jb + wc + 8 * n + 2 * q + e;
-                    cur[m][n][e] = (i < ns && j <= i) ? Ab[(size_t)i * ns + j] : 0.0;
-                    acc[m][n][e] = 0.0;
+                    for (int e = 0; e < 2; ++e) cur[m][n][e] = (i < ns && j + e <= i) ? Ab[(size_t)i * ns + j + e] : 0.0;
                 }
+                acc[m][n][0] = acc[m][n][1] = 0.0;
+            }
         if (tj < ti) asm volatile("cp.async.wait_group 1;\n" ::: "memory");
         else asm volatile("cp.async.wait_group 0;\n" ::: "memory");
         __syncthreads();
@@ -189,12 +209,16 @@ __global__ void __launch_bounds__(256, 2) chol_update_kernel(double* __restrict_
 #pragma unroll
         for (int m = 0; m < 2; ++m)
 #pragma unroll
-            for (int n = 0; n < 4; ++n)
+            for (int n = 0; n < 4; ++n) {
+                const int i = ib + wr + 8 * m + g, j = jb + wc + 8 * n + 2 * q;
+                if (EVEN && i < ns && j + 1 <= i)        // both below or on the diagonal: one 16-byte store
+                    *reinterpret_cast<double2*>(Ab + (size_t)i * ns + j) = make_double2(cur[m][n][0] - acc[m][n][0], cur[m][n][1] - acc[m][n][1]);
+                else {
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int i = ib + wr + 8 * m + g, j = jb + wc + 8 * n + 2 * q + e;
-                    if (i < ns && j <= i) Ab[(size_t)i * ns + j] = cur[m][n][e] - acc[m][n][e];
+                    for (int e = 0; e < 2; ++e)
+                        if (i < ns && j + e <= i) Ab[(size_t)i * ns + j + e] = cur[m][n][e] - acc[m][n][e];
                 }
+            }
         __syncthreads();                   // the buffer just read is refilled by the next iteration's prefetch
     }
 }
@@ -205,7 +229,8 @@ size_t pixsrc_factor_scratch_bytes(int Bc) { return sizeof(double) * (size_t)Bc 
 // Winv: scratch of pixsrc_factor_scratch_bytes(Bc)
 cudaError_t launch_pixsrc_factor(glad_ctx* c, cudaStream_t st, double* A, int ns, int Bc, double* out, double* Winv) {
     const size_t sm_trsm = sizeof(double) * 2 * CH_NB * CH_P, sm_upd = sizeof(double) * 3 * CH_NB * CH_PU;
-    cudaError_t e = smem_optin(c, chol_update_kernel);
+    cudaError_t e = smem_optin(c, chol_update_kernel<true>);
+    if (e == cudaSuccess) e = smem_optin(c, chol_update_kernel<false>);
     if (e == cudaSuccess) e = smem_optin(c, chol_trsm_kernel);
     if (e != cudaSuccess) return e;
     for (int k0 = 0; k0 < ns; k0 += CH_NB) {
@@ -215,7 +240,8 @@ cudaError_t launch_pixsrc_factor(glad_ctx* c, cudaStream_t st, double* A, int ns
         if (rest <= 0) break;
         const int nt = (rest + CH_NB - 1) / CH_NB;
         chol_trsm_kernel<<<dim3(nt, Bc), 256, sm_trsm, st>>>(A, Winv, ns, k0);
-        chol_update_kernel<<<dim3(nt, Bc), 256, sm_upd, st>>>(A, ns, k0, nt);
+        if (ns % 2 == 0) chol_update_kernel<true><<<dim3(nt, Bc), 256, sm_upd, st>>>(A, ns, k0, nt);
+        else chol_update_kernel<false><<<dim3(nt, Bc), 256, sm_upd, st>>>(A, ns, k0, nt);
         c->launches += 2;
     }
     return cudaGetLastError();
