@@ -46,10 +46,11 @@ def _setup(glad_mod, oracle, name, B):
     return wl, L, g
 
 
-@pytest.mark.parametrize("nsx,nsy", [(12, 12), (9, 14), (32, 20)])
+@pytest.mark.parametrize("nsx,nsy", [(12, 12), (9, 14), (32, 20), (15, 13)])
 def test_c1_parity_ragged_source_grids(glad_mod, oracle, nsx, nsy):
-    """C1 image (40 x 40, 5 x 5 PSF); N_s = 144, 126, 640: ragged 64-tiles and Cholesky panels, n_sx != n_sy; masked pixels;
-    one invalid mass model, one lambda <= 0, one pixel size <= 0."""
+    """C1 image (40 x 40, 5 x 5 PSF); N_s = 144, 126, 640, 195: ragged 64-tiles and Cholesky panels, n_sx != n_sy; masked pixels;
+    one invalid mass model, one lambda <= 0, one pixel size <= 0.  N_s = 195 is odd: the trailing update of the Cholesky then runs
+    its 8-byte instantiation (rows of A do not start on 16-byte boundaries), every other size the 16-byte one."""
     from oracle import pixsrc
     wl, L, g = _setup(glad_mod, oracle, "C1", 8)
     ivar = L["ivar"].copy()
