@@ -77,20 +77,12 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
                      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     } while (!ok);
 }
-// UMMA shared-memory descriptor: K-major, no swizzle, version 1 (sm_100).  SBO = 128 B between 8-row groups
-// along M/N, LBO = byte distance between the two 16-byte K halves of a K = 16 (bf16) step.
-__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes) {
-    uint32_t lo = ((saddr >> 4) & 0x3FFFu) | (((lbo_bytes >> 4) & 0x3FFFu) << 16);
-    uint32_t hi = (128u >> 4) | (1u << 14);
-    return ((uint64_t)hi << 32) | lo;
-}
-__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-                 ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
-}
-// the same from convergent code with warp-uniform operands: one elected lane issues (the operands can then stay in
-// uniform registers; issued from inside an `if (lane == 0)` every MMA costs a 16-instruction broadcast loop)
-// (descriptors as their low words plus the common high word: only the low word moves from MMA to MMA)
+// UMMA shared-memory descriptors are K-major, no swizzle, version 1 (sm_100): SBO = 128 B between 8-row groups along M/N,
+// LBO = byte distance between the two 16-byte K halves of a K = 16 (bf16) step; low word = (address >> 4) | (LBO >> 4) << 16,
+// high word = (SBO >> 4) | 1 << 14.
+// tcgen05.mma from convergent code with warp-uniform operands: one elected lane issues (issued from inside an `if (lane == 0)`
+// every MMA costs a 16-instruction broadcast loop).  Descriptors come as their low words plus the common high word: only the
+// low word moves from MMA to MMA.
 __device__ __forceinline__ void umma_bf16_elect(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t desc_hi, uint32_t idesc, uint32_t accumulate) {
     asm volatile("{\n\t.reg .pred p, e;\n\t.reg .b64 da, db;\n\telect.sync _|e, 0xffffffff;\n\tsetp.ne.b32 p, %5, 0;\n\t"
                  "mov.b64 da, {%1, %3};\n\tmov.b64 db, {%2, %3};\n\t"
@@ -100,9 +92,6 @@ __device__ __forceinline__ void umma_bf16_elect(uint32_t d_tmem, uint32_t a_lo, 
 __device__ __forceinline__ void umma_commit_elect(uint32_t bar) {
     asm volatile("{\n\t.reg .pred e;\n\telect.sync _|e, 0xffffffff;\n\t"
                  "@e tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
 // {hi: bf16_rn(b), lo: bf16_rn(a)}: element a sits at the lower address
 __device__ __forceinline__ uint32_t pack_bf16(float a, float b) {
@@ -114,7 +103,6 @@ __device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64
 __device__ __forceinline__ void unpk2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
 __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ f32x2 ex2_2(f32x2 x) { float a, b; unpk2(x, a, b); return pk2(ex2_tc(a), ex2_tc(b)); }
 // a -= bf16 low half of w, b -= bf16 high half of w, exactly (mixed-precision FHFMA.BF16: one issue slot per value,
 // no unpacking of the bf16 pair into fp32 registers)
@@ -235,7 +223,7 @@ __global__ void __launch_bounds__(PW * 32 + 32, 1) jam_quad_tc_kernel(JTArgs a) 
         const uint32_t a_lbo = GA * 128, b_lbo = GB * 128;              // bytes between the two octs of a K-step
         // descriptors advance by one K-step (two octs) per MMA and by one stage per chunk: only the 14-bit
         // start-address field (16-byte units) changes
-        const uint32_t desc_hi = (128u >> 4) | (1u << 14);              // SBO = 128 B, version 1 (as umma_desc)
+        const uint32_t desc_hi = (128u >> 4) | (1u << 14);              // SBO = 128 B, version 1 (see above)
         const uint32_t ad0 = ((ops_addr >> 4) & 0x3FFFu) | (((a_lbo >> 4) & 0x3FFFu) << 16);
         const uint32_t bd0 = (((ops_addr + a16 * 16) >> 4) & 0x3FFFu) | (((b_lbo >> 4) & 0x3FFFu) << 16);
         const uint32_t ad_step = (2 * a_lbo) >> 4, bd_step = (2 * b_lbo) >> 4;
