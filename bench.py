@@ -757,6 +757,9 @@ def run_ours(args, rank, world, local_rank):
                                   "algorithmic_flops_per_launch": alg, "achieved_algorithmic": alg / (l_avg * 1e-3) / 1e12,
                                   "frac_algorithmic": alg / (l_avg * 1e-3) / 1e12 / peak_tf}
         k3 = ["smsp__sass_thread_inst_executed_op_%s_pred_on.sum" % o for o in ("ffma", "fmul", "fadd")]
+        if not all(k in m for k in k3) and "sm__cycles_elapsed.avg" in m and all(k + ".per_cycle_elapsed" in m for k in k3):
+            for k in k3:                         # the raw page lists these counters per elapsed cycle only
+                m[k] = m[k + ".per_cycle_elapsed"] * m["sm__cycles_elapsed.avg"]
         if cap_l["fresh"] and args.config == "C2" and all(k in m for k in k3) and m.get("launch__grid_size") == B:
             lf = 2.0 * m[k3[0]] + m[k3[1]] + m[k3[2]]
             roofline["lens_image"].update({"flops_per_launch": lf, "achieved": lf / (l_avg * 1e-3) / 1e12, "frac": lf / (l_avg * 1e-3) / 1e12 / peak_tf,
