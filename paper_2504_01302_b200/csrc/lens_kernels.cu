@@ -117,7 +117,9 @@ __device__ __forceinline__ float sersic_eval(const float* __restrict__ o, float 
 }
 
 // Cusp guard: an fp32 ray carries ~5e-7" of absolute error in beta (|alpha| ~ 1.7").  Where the source
-// profile is steep, |d ln I / dR| = ln2 k1 2h (R^2)^h / R, that error is amplified: above LENS_CUSP_SLOPE per arcsec (2e-5 per ray) the
+// profile is steep, |grad ln I| <= ln2 k1 2h (R^2)^h / R x max(1, 1/q_s) (the elliptical radius R stretches the minor axis by 1/q_s: a
+// q_s = 0.15, n = 3.8 source of the C2 batch was 1.4e-4 off at its peak with the bound in R alone), that error is amplified: above
+// LENS_CUSP_SLOPE per arcsec (2e-5 per ray) the
 // pixel is recomputed with fp64 rays (src_pixel_fp64).  Happens within ~0.05" of the centre of an n ~ 4 source: a few hundred of the
 // 40 000 rays of a C2 vector; one C2 vector in 1024 had a peak pixel 1.09e-4 off without it.
 #define LENS_CUSP_SLOPE 30.f
@@ -127,7 +129,7 @@ __device__ __forceinline__ float sersic_at(const float* __restrict__ o, float dx
     float R2 = fmaf(y * y, o[4], x * x);
     float pw = ex2f(o[7] * lg2f(R2));      // (R^2)^(1/2n); R2 = 0 -> 0
     const float gl = 1.3862944f * o[6] * o[7] * pw;                  // |d ln I / d ln R| = ln2 k1 2h pw
-    cusp = gl * gl > (LENS_CUSP_SLOPE * LENS_CUSP_SLOPE) * R2;
+    cusp = gl * gl * fmaxf(o[4], 1.f) > (LENS_CUSP_SLOPE * LENS_CUSP_SLOPE) * R2;   // |grad ln I| <= (gl / R) max(1, 1/q_s): o[4] = 1/q_s^2
     return o[5] * ex2f(-o[6] * pw);
 }
 

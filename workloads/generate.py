@@ -242,8 +242,11 @@ def make_workload(name: str, data_model=None, B: int | None = None) -> dict:
             p[:, 16:21] = np.stack([Ie_1, Re_1, n_1, q_1, pa], axis=1)
         if L["n_lens_light"] >= 2:
             p[:, 21:26] = np.stack([Ie_2, Re_2, n_2, q_2, pa], axis=1)
-        n, pix = L["n"], L["pix"]
-        grid = dict(nx=n, ny=n, supersample=L["s"], pix=pix, x0=-(n - 1) / 2 * pix, y0=-(n - 1) / 2 * pix)
+        # the C ABI takes the grid as fp32: the numbers are made fp32-representable HERE so that the fp64 oracle and the library get
+        # the same grid (0.05 and -2.475 are not: rays 1e-7 arcsec apart move the peak of a magnified n = 3.8 source by 1.4e-4)
+        n, pix = L["n"], float(np.float32(L["pix"]))
+        x0 = float(np.float32(-(n - 1) / 2 * pix))
+        grid = dict(nx=n, ny=n, supersample=L["s"], pix=pix, x0=x0, y0=x0)
         wl["lens"] = dict(params=p.astype(np.float32), grid=grid,
                           psf=_psf(L["psf"][0], L["psf"][1], pix, IMG_FWHM), noise=L["noise"],
                           data=np.zeros((n, n), np.float32), ivar=np.ones((n, n), np.float32))
