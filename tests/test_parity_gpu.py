@@ -177,7 +177,8 @@ def test_c2_rxj1131_full_batch_every_vector(glad_mod, oracle):
 def test_c3_dynamics_sweep_cells(glad_mod, oracle):
     dm = oracle_data_model(oracle)
     for name, idx in (("C3-10-40-256", [0, 1, 2, 3, 4, 5, 6, 255]), ("C3-40-80-256", [0, 200]), ("C3-20-160-256", [0, 77]),
-                      ("C3-10-40-4096", [0, 1, 2047, 4095]), ("C3-20-80-4096", [0, 4095])):   # the last two: BASELINE's large batch
+                      ("C3-10-40-4096", np.linspace(0, 4095, 256).astype(int)),           # BASELINE's large batch: 256 spread vectors (6 s
+                      ("C3-20-80-4096", np.linspace(0, 4095, 32).astype(int))):           # of oracle) and 32 (10 s)
         wl = workloads.make_workload(name, dm)
         run_jam(glad_mod, oracle, wl, np.array(idx), maps=True)
 
