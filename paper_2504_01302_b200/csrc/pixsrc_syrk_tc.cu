@@ -285,7 +285,10 @@ __global__ void __launch_bounds__(SY_THREADS, 1) pixsrc_syrk_tc_kernel(const flo
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        __syncthreads();
+        // only warp 0 waits for the chunk to be complete (named barrier 1 + st: 480 arrives + its own 32); the other warps go on
+        // to the next chunk, held back by the "empty" mbarrier of their stage alone
+        if (warp != 0) asm volatile("bar.arrive %0, %1;" ::"r"(1 + st), "r"(SY_THREADS) : "memory");
+        else asm volatile("bar.sync %0, %1;" ::"r"(1 + st), "r"(SY_THREADS) : "memory");
         if (tid == 0) {
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             const int g = n / SY_FL;
