@@ -65,7 +65,11 @@ __global__ void __launch_bounds__(PX_MAP_THREADS) pixsrc_map_kernel(const float*
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// f = B L: a warp per image pixel, row in shared memory
+// f = B L: a warp per image pixel, row in shared memory.  A row is non-zero only between the first and the last source pixel that the
+// PSF footprint of its image pixel maps to (about a third of the row at the paper's sizes); the range goes to rng, which
+// pixsrc_model_kernel uses to read only that part and pixsrc_syrk_tc_kernel to list the rows that count for a tile.  (Writing only
+// the range and letting the contraction zero-fill the rest while it stages was measured: the kernel is bound by its shared-memory
+// atomics, not by its stores -- 10.6 -> 10.1 ms -- and the range test cost the contraction 1.6 ms.)
 // ------------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(32 * PX_BLUR_WARPS) pixsrc_blur_kernel(const int* __restrict__ idx, const float2* __restrict__ wgt,
                                                                          const float* __restrict__ psf, int kpsf, int nx, int ny,
@@ -78,11 +82,11 @@ __global__ void __launch_bounds__(32 * PX_BLUR_WARPS) pixsrc_blur_kernel(const i
     const int* ib = idx + (size_t)b * npix;
     const float2* wb = wgt + (size_t)b * npix;
     const int p0 = blockIdx.x * rows_per_cta;
+    for (int i = lane; i < ns; i += 32) row[i] = 0.f;      // the row is all zero between pixels: the written range is cleared after use
+    __syncwarp();
     for (int r = warp; r < rows_per_cta; r += PX_BLUR_WARPS) {
         const int p = p0 + r;
         if (p >= npix) break;
-        for (int i = lane; i < ns; i += 32) row[i] = 0.f;
-        __syncwarp();
         const int iy = p / nx, ix = p - iy * nx;
         int lo = 0x7fffffff, hi = -1;             // first and last source pixel this row touches (row-major index)
         for (int t = lane; t < k2; t += 32) {
@@ -111,6 +115,8 @@ __global__ void __launch_bounds__(32 * PX_BLUR_WARPS) pixsrc_blur_kernel(const i
         __syncwarp();
         float* out = f + ((size_t)b * npix + p) * ns;
         for (int i = lane; i < ns; i += 32) out[i] = row[i];
+        if (hi >= 0)
+            for (int i = lo + lane; i <= hi; i += 32) row[i] = 0.f;
         __syncwarp();
     }
 }
@@ -226,7 +232,7 @@ __global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_solve_kernel(const 
 __global__ void __launch_bounds__(256) pixsrc_model_kernel(const float* __restrict__ f, const double* __restrict__ s,
                                                            const float* __restrict__ ivar, const float* __restrict__ data, int npix,
                                                            int ns, float* __restrict__ model, long model_stride,
-                                                           double* __restrict__ out) {
+                                                           double* __restrict__ out, const int2* __restrict__ rng) {
     extern __shared__ double px_s[];
     const int b = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int i = threadIdx.x; i < ns; i += 256) px_s[i] = s[(size_t)b * ns + i];
@@ -238,7 +244,9 @@ __global__ void __launch_bounds__(256) pixsrc_model_kernel(const float* __restri
         if (p >= npix) break;
         const float* row = f + ((size_t)b * npix + p) * ns;
         double v = 0.0;
-        for (int i = lane; i < ns; i += 32) v += (double)row[i] * px_s[i];
+        const int2 rg = rng[(size_t)b * npix + p];                     // the row is zero outside its range
+        if (rg.y >= 0)
+            for (int i = (rg.x & ~3) + lane, i1 = min(rg.y | 3, ns - 1); i <= i1; i += 32) v += (double)row[i] * px_s[i];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
         if (lane == 0) {
@@ -462,7 +470,7 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
     {
         ProfScope ps(c, GK_PIX_MODEL);
         pixsrc_model_kernel<<<dim3((npix + 63) / 64, Bc), 256, sizeof(double) * ns, st>>>(f, s, c->d_ivar, c->d_data, npix, ns, d_model,
-                                                                                          (long)npix, out);
+                                                                                          (long)npix, out, rng);
     }
     pixsrc_final_kernel<<<Bc, 128, 0, st>>>(d_lens, d_src_grid, lam_use, d_ms_lambda, out, stat, s, logdet_g, Bc, ns, npix, d_logev, d_chi2,
                                             d_reg, d_s_mp, d_model, d_flags);
