@@ -41,9 +41,14 @@ __global__ void __launch_bounds__(256) chol_diag_kernel(double* __restrict__ A, 
         const double dj = L[j * CH_P + j];
         if (tid > j && tid < nb) L[tid * CH_P + j] /= dj;
         __syncthreads();
-        for (int e = tid; e < CH_NB * CH_NB; e += 256) {
-            const int r = e >> 6, c = e & 63;
-            if (c > j && r >= c && r < nb) L[r * CH_P + c] -= L[r * CH_P + j] * L[c * CH_P + j];
+        // rank-1 update of the trailing lower triangle only: thread (tr, tc) of a 16 x 16 arrangement takes rows j+1+tr, +16, ..
+        // and columns j+1+tc, +16, .. <= row (a loop over all 4096 elements with the test inside was two thirds of this kernel)
+        {
+            const int tr = tid >> 4, tc = tid & 15;
+            for (int r = j + 1 + tr; r < nb; r += 16) {
+                const double lrj = L[r * CH_P + j];
+                for (int c = j + 1 + tc; c <= r; c += 16) L[r * CH_P + c] = fma(-lrj, L[c * CH_P + j], L[r * CH_P + c]);
+            }
         }
         __syncthreads();
     }
