@@ -20,7 +20,7 @@
 __global__ void __launch_bounds__(256) chol_diag_kernel(double* __restrict__ A, int ns, int k0, double* __restrict__ out,
                                                         double* __restrict__ Winv) {
     __shared__ double L[CH_NB * CH_P];
-    __shared__ double s_ld;
+    __shared__ double s_ld, s_isq[CH_NB], s_lg[CH_NB];
     __shared__ int s_bad;
     const int b = blockIdx.x, tid = threadIdx.x;
     double* Ab = A + (size_t)b * ns * ns;
@@ -31,27 +31,41 @@ __global__ void __launch_bounds__(256) chol_diag_kernel(double* __restrict__ A, 
         L[r * CH_P + c] = (r < nb && c <= r) ? Ab[(size_t)(k0 + r) * ns + k0 + c] : (r == c ? 1.0 : 0.0);
     }
     __syncthreads();
-    for (int j = 0; j < nb; ++j) {
-        if (tid == 0) {
+    // Elimination with UNSCALED columns and one barrier per step: column j and the pivot d_j = L[j][j] are final after step j - 1
+    // and are not written again, so step j reads them and updates the trailing lower triangle with L[r][j] L[c][j] / d_j; the
+    // scaling L[r][j] /= sqrt(d_j) of every column, the square roots and the logarithms wait until the elimination is over.  (Pivot,
+    // barrier, column scaling, barrier, update, barrier per step: the barriers and thread 0's sqrt / log were most of the kernel.)
+    // Thread (tr, tc) of a 16 x 16 arrangement takes rows j+1+tr, +16, .. and columns j+1+tc, +16, .. <= row.
+    {
+        const int tr = tid >> 4, tc = tid & 15;
+        for (int j = 0; j < nb; ++j) {
             const double d = L[j * CH_P + j];
-            if (!(d > 0.0) || !isfinite(d)) { s_bad = 1; L[j * CH_P + j] = 1.0; }
-            else { L[j * CH_P + j] = sqrt(d); s_ld += log(d); }
-        }
-        __syncthreads();
-        const double dj = L[j * CH_P + j];
-        if (tid > j && tid < nb) L[tid * CH_P + j] /= dj;
-        __syncthreads();
-        // rank-1 update of the trailing lower triangle only: thread (tr, tc) of a 16 x 16 arrangement takes rows j+1+tr, +16, ..
-        // and columns j+1+tc, +16, .. <= row (a loop over all 4096 elements with the test inside was two thirds of this kernel)
-        {
-            const int tr = tid >> 4, tc = tid & 15;
+            const bool okd = (d > 0.0) && isfinite(d);
+            const double invd = okd ? 1.0 / d : 1.0;               // a pivot that is not positive is flagged and taken as 1
             for (int r = j + 1 + tr; r < nb; r += 16) {
-                const double lrj = L[r * CH_P + j];
+                const double lrj = L[r * CH_P + j] * invd;
                 for (int c = j + 1 + tc; c <= r; c += 16) L[r * CH_P + c] = fma(-lrj, L[c * CH_P + j], L[r * CH_P + c]);
             }
+            __syncthreads();
         }
-        __syncthreads();
     }
+    if (tid < nb) {                                                // thread j: pivot j -> ln det, flag, 1 / sqrt(d_j)
+        const double d = L[tid * CH_P + tid];
+        const bool okd = (d > 0.0) && isfinite(d);
+        if (!okd) s_bad = 1;
+        s_isq[tid] = okd ? rsqrt(d) : 1.0;
+        s_lg[tid] = okd ? log(d) : 0.0;
+    }
+    __syncthreads();
+    for (int e = tid; e < CH_NB * CH_NB; e += 256) {
+        const int r = e >> 6, c = e & 63;
+        if (r < nb && c <= r) {                                     // (only thread (c, c) touches the pivot itself)
+            const double v = L[r * CH_P + c];
+            L[r * CH_P + c] = (r == c) ? (((v > 0.0) && isfinite(v)) ? sqrt(v) : 1.0) : v * s_isq[c];
+        }
+    }
+    if (tid == 0) { double t = 0.0; for (int j = 0; j < nb; ++j) t += s_lg[j]; s_ld = t; }
+    __syncthreads();
     for (int e = tid; e < CH_NB * CH_NB; e += 256) {
         const int r = e >> 6, c = e & 63;
         if (r < nb && c <= r) Ab[(size_t)(k0 + r) * ns + k0 + c] = L[r * CH_P + c];
