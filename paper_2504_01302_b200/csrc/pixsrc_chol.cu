@@ -3,9 +3,9 @@
 // batch instead of one CTA per matrix:
 //   chol_diag_kernel    CTA per matrix: the 64 x 64 diagonal block in shared memory; ln det and the not-positive-definite flag
 //                       and W = L11^-1
-//   chol_trsm_kernel    CTA per (64 rows below the block, matrix): L21 = A21 W^T as a 64 x 64 x 64 tile product
-//   chol_update_kernel  CTA per (row of 64 x 64 tiles of the trailing lower triangle, matrix): A22 -= L21 L21^T, 4 x 4 doubles per
-//                       thread, the panel tiles streamed through shared memory by cp.async
+//   chol_trsm_kernel    CTA per (64 rows below the block, matrix): L21 = A21 W^T as a 64 x 64 x 64 tile product (DMMA)
+//   chol_update_kernel  CTA per (row of 64 x 64 tiles of the trailing lower triangle, matrix): A22 -= L21 L21^T on the fp64
+//                       tensor-core path (DMMA m8n8k4), the panel tiles streamed through shared memory by cp.async
 // The version this replaces ran the whole factorisation in one CTA per matrix (profiles/r1e.md: fp64 pipe 20 % active, 12 TFLOP/s,
 // and at the paper's 64 x 64 source grid only 54 matrices fit the scratch, so 54 CTAs on 148 SMs: 2.47 s per 296 matrices).
 // Here every trailing update is a grid of (tiles x matrices) CTAs whatever the batch size.
@@ -16,6 +16,16 @@
 #define CH_NB 64
 #define CH_P 65            // pitch (doubles) of the shared-memory tiles
 #define CH_OUT 6           // doubles per vector in `out` (pixsrc_kernels.cu PX_OUT): [0] ln det A, [3] not-positive-definite flag
+
+// D (8 x 8) = A (8 x 4, row-major) B (4 x 8, column-major) + C on the fp64 tensor-core path: a thread holds A[lane/4][lane%4],
+// B[lane%4][lane/4] and C[lane/4][2 (lane%4) + {0, 1}]
+__device__ __forceinline__ void ch_dmma(double& d0, double& d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+#define CH_PU 68           // pitch (doubles) of the update kernel's tiles: 2 * 68 mod 32 = 8, so the 16 lanes of a half-warp
+                           // (4 rows x 4 consecutive k) read 16 different bank pairs
+
 
 __global__ void __launch_bounds__(256) chol_diag_kernel(double* __restrict__ A, int ns, int k0, double* __restrict__ out,
                                                         double* __restrict__ Winv) {
@@ -95,59 +105,58 @@ __global__ void __launch_bounds__(256) chol_diag_kernel(double* __restrict__ A, 
 }
 
 // L21 = A21 L11^-T = A21 W^T with W = L11^-1 from chol_diag_kernel: a 64-row tile of the panel times a 64 x 64 matrix, the same
-// sum_k P_i[i,k] P_j[c,k] form as the trailing update (a thread per row with its 64 doubles in registers took 3.2 of 15 ms)
+// sum_k P_i[i,k] P_j[c,k] form as the trailing update and, like it, on the DMMA path (a thread per row with its 64 doubles in
+// registers took 3.2 of 15 ms; 4 x 4 doubles per thread with DFMA 1.7 of 10.6)
 __global__ void __launch_bounds__(256, 2) chol_trsm_kernel(double* __restrict__ A, const double* __restrict__ Winv, int ns, int k0) {
     extern __shared__ double ch_sm[];
-    double* Pi = ch_sm;                     // [k][row of the tile], pitch CH_P
-    double* Pj = ch_sm + CH_NB * CH_P;      // [k][c] = W[c][k]
+    double* Pi = ch_sm;                     // [row of the tile][k], pitch CH_PU
+    double* Pj = ch_sm + CH_NB * CH_PU;     // [c][k] = W[c][k]
     const int b = blockIdx.y, tid = threadIdx.x;
     const int ib = k0 + CH_NB + blockIdx.x * CH_NB;
     double* Ab = A + (size_t)b * ns * ns;
     const double* Wb = Winv + (size_t)b * CH_NB * CH_NB;
     for (int e = tid; e < CH_NB * CH_NB; e += 256) {
         const int r = e >> 6, k = e & 63;
-        Pi[k * CH_P + r] = (ib + r < ns) ? Ab[(size_t)(ib + r) * ns + k0 + k] : 0.0;
-        Pj[k * CH_P + r] = Wb[r * CH_NB + k];
+        Pi[r * CH_PU + k] = (ib + r < ns) ? Ab[(size_t)(ib + r) * ns + k0 + k] : 0.0;
+        Pj[r * CH_PU + k] = Wb[r * CH_NB + k];
     }
     __syncthreads();
-    const int ty = tid >> 4, tx = tid & 15;
-    double acc[4][4];
+    const int warp = tid >> 5, lane = tid & 31, g = lane >> 2, q = lane & 3;
+    const int wr = (warp >> 1) * 16, wc = (warp & 1) * 32;      // the warp's 16 rows and 32 columns of the tile
+    const double* pa = Pi + (wr + g) * CH_PU + q;
+    const double* pb = Pj + (wc + g) * CH_PU + q;
+    double acc[2][4][2];
 #pragma unroll
-    for (int r = 0; r < 4; ++r)
+    for (int m = 0; m < 2; ++m)
 #pragma unroll
-        for (int c = 0; c < 4; ++c) acc[r][c] = 0.0;
-#pragma unroll 8
-    for (int k = 0; k < CH_NB; ++k) {
-        double ar[4], br[4];
+        for (int n = 0; n < 4; ++n) acc[m][n][0] = acc[m][n][1] = 0.0;
+#pragma unroll 4
+    for (int k = 0; k < CH_NB; k += 4) {
+        double ar[2], br[4];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) { ar[r] = Pi[k * CH_P + ty * 4 + r]; br[r] = Pj[k * CH_P + tx + 16 * r]; }
+        for (int m = 0; m < 2; ++m) ar[m] = pa[m * 8 * CH_PU + k];
 #pragma unroll
-        for (int r = 0; r < 4; ++r)
+        for (int n = 0; n < 4; ++n) br[n] = pb[n * 8 * CH_PU + k];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) acc[r][c] = fma(ar[r], br[c], acc[r][c]);
+        for (int m = 0; m < 2; ++m)
+#pragma unroll
+            for (int n = 0; n < 4; ++n) ch_dmma(acc[m][n][0], acc[m][n][1], ar[m], br[n]);
     }
 #pragma unroll
-    for (int r = 0; r < 4; ++r)
+    for (int m = 0; m < 2; ++m)
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            const int i = ib + ty * 4 + r;
-            if (i < ns) Ab[(size_t)i * ns + k0 + tx + 16 * c] = acc[r][c];
-        }
+        for (int n = 0; n < 4; ++n)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int i = ib + wr + 8 * m + g;
+                if (i < ns) Ab[(size_t)i * ns + k0 + wc + 8 * n + 2 * q + e] = acc[m][n][e];
+            }
 }
 
 __device__ __forceinline__ void ch_cp_async8(void* smem, const void* gmem) {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gmem) : "memory");
 }
-
-// D (8 x 8) = A (8 x 4, row-major) B (4 x 8, column-major) + C on the fp64 tensor-core path: a thread holds A[lane/4][lane%4],
-// B[lane%4][lane/4] and C[lane/4][2 (lane%4) + {0, 1}]
-__device__ __forceinline__ void ch_dmma(double& d0, double& d1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
-}
-
-#define CH_PU 68           // pitch (doubles) of the update kernel's tiles: 2 * 68 mod 32 = 8, so the 16 lanes of a half-warp
-                           // (4 rows x 4 consecutive k) read 16 different bank pairs
 
 // A[i, j] -= sum_k L21[i, k] L21[j, k] on the trailing lower triangle (rows / columns >= r0).  CTA = (row of 64 x 64 tiles ti, matrix):
 // the panel rows of ti stay in shared memory, those of tj = 0 .. ti stream through a double buffer filled by cp.async one tile
@@ -250,7 +259,7 @@ size_t pixsrc_factor_scratch_bytes(int Bc) { return sizeof(double) * (size_t)Bc 
 
 // Winv: scratch of pixsrc_factor_scratch_bytes(Bc)
 cudaError_t launch_pixsrc_factor(glad_ctx* c, cudaStream_t st, double* A, int ns, int Bc, double* out, double* Winv) {
-    const size_t sm_trsm = sizeof(double) * 2 * CH_NB * CH_P, sm_upd = sizeof(double) * 3 * CH_NB * CH_PU;
+    const size_t sm_trsm = sizeof(double) * 2 * CH_NB * CH_PU, sm_upd = sizeof(double) * 3 * CH_NB * CH_PU;
     cudaError_t e = smem_optin(c, chol_update_kernel<true>);
     if (e == cudaSuccess) e = smem_optin(c, chol_update_kernel<false>);
     if (e == cudaSuccess) e = smem_optin(c, chol_trsm_kernel);
