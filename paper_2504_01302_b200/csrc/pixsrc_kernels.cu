@@ -136,6 +136,7 @@ __global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_solve_kernel(const 
     extern __shared__ double px_sm[];
     double* yv = px_sm;                          // [ns]
     double* red = yv + ns;                       // [8][32]
+    double* blk = red + (PX_CHOL_THREADS / 32) * 32;   // [32][33]: the diagonal block of the step (its serial part reads shared memory)
     const int b = blockIdx.x, tid = threadIdx.x;
     const double* Ab = A + (size_t)b * ns * ns;
 
@@ -152,10 +153,14 @@ __global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_solve_kernel(const 
             for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
             if (lane == 0) yv[k0 + r] = Db[k0 + r] - v;
         }
+        for (int e = tid; e < PX_NB * PX_NB; e += PX_CHOL_THREADS) {
+            const int r = e >> 5, cc = e & 31;
+            blk[r * (PX_NB + 1) + cc] = (r < nb && cc <= r) ? Ab[(size_t)(k0 + r) * ns + k0 + cc] : 0.0;
+        }
         __syncthreads();
         if (warp == 0) {
             for (int r = 0; r < nb; ++r) {
-                const double* lrow = Ab + (size_t)(k0 + r) * ns + k0;
+                const double* lrow = blk + r * (PX_NB + 1);
                 double v = (lane < r) ? lrow[lane] * yv[k0 + lane] : 0.0;
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
@@ -188,6 +193,10 @@ __global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_solve_kernel(const 
         if (lane < nb)
             for (int r = k0 + nb + warp; r < ns; r += PX_CHOL_THREADS / 32) v += Ab[(size_t)r * ns + k0 + lane] * yv[r];
         red[warp * 32 + lane] = v;
+        for (int e = tid; e < PX_NB * PX_NB; e += PX_CHOL_THREADS) {
+            const int r = e >> 5, cc = e & 31;
+            blk[r * (PX_NB + 1) + cc] = (r < nb && cc <= r) ? Ab[(size_t)(k0 + r) * ns + k0 + cc] : 0.0;
+        }
         __syncthreads();
         if (warp == 0) {
             double t = 0.0;
@@ -197,10 +206,10 @@ __global__ void __launch_bounds__(PX_CHOL_THREADS, 2) pixsrc_solve_kernel(const 
             __syncwarp();
             for (int c = nb - 1; c >= 0; --c) {
                 // s_c = (y_c - sum_{r in block, r > c} L[k0 + r, k0 + c] s_r) / L[c, c]
-                double u = (lane > c && lane < nb) ? Ab[(size_t)(k0 + lane) * ns + k0 + c] * yv[k0 + lane] : 0.0;
+                double u = (lane > c && lane < nb) ? blk[lane * (PX_NB + 1) + c] * yv[k0 + lane] : 0.0;
 #pragma unroll
                 for (int o = 16; o > 0; o >>= 1) u += __shfl_xor_sync(0xffffffffu, u, o);
-                if (lane == 0) yv[k0 + c] = (yv[k0 + c] - u) / Ab[(size_t)(k0 + c) * ns + k0 + c];
+                if (lane == 0) yv[k0 + c] = (yv[k0 + c] - u) / blk[c * (PX_NB + 1) + c];
                 __syncwarp();
             }
         }
@@ -422,7 +431,7 @@ cudaError_t launch_pixsrc_chunk(glad_ctx* c, void* scratch, const float* d_lens,
 
     const int rows_per_cta = 64;
     const size_t sm_blur = sizeof(float) * (size_t)PX_BLUR_WARPS * ns;
-    const size_t sm_chol = sizeof(double) * ((size_t)ns + 8 * 32);
+    const size_t sm_chol = sizeof(double) * ((size_t)ns + 8 * 32 + PX_NB * (PX_NB + 1));
     if (sm_blur > 227 * 1024 || sm_chol > 227 * 1024) return cudaErrorInvalidConfiguration;
     if ((e = smem_optin(c, pixsrc_blur_kernel)) != cudaSuccess) return e;
     if ((e = smem_optin(c, pixsrc_solve_kernel)) != cudaSuccess) return e;
