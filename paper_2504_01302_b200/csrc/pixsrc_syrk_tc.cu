@@ -61,6 +61,21 @@ __device__ __forceinline__ void sy_mma(uint32_t d_tmem, uint64_t adesc, uint64_t
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
                  ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
+// One lane of converged warp 0 issues: behind an elect.sync branch ptxas moves the operands into uniform registers with plain R2URs
+// (under `if (tid == 0)` every tcgen05.mma is wrapped in a 16-instruction broadcast loop), and descriptors go in as low words plus
+// the common high word.  With the CTA-wide barrier still in place this was slower (16.7 against 16.1 ms); now that warp 0 alone
+// waits and issues, its own time per chunk is what counts: 14.4 -> 14.0 ms.
+__device__ __forceinline__ bool sy_elect_one() {
+    uint32_t e;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(e));
+    return e != 0;
+}
+__device__ __forceinline__ void sy_mma_lo(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t desc_hi, uint32_t idesc, uint32_t accumulate) {
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\tsetp.ne.b32 p, %5, 0;\n\t"
+                 "mov.b64 da, {%1, %3};\n\tmov.b64 db, {%2, %3};\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %4, p;\n\t}"
+                 ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(desc_hi), "r"(idesc), "r"(accumulate) : "memory");
+}
 __device__ __forceinline__ void sy_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
@@ -289,22 +304,27 @@ __global__ void __launch_bounds__(SY_THREADS, 1) pixsrc_syrk_tc_kernel(const flo
         // to the next chunk, held back by the "empty" mbarrier of their stage alone
         if (warp != 0) asm volatile("bar.arrive %0, %1;" ::"r"(1 + st), "r"(SY_THREADS) : "memory");
         else asm volatile("bar.sync %0, %1;" ::"r"(1 + st), "r"(SY_THREADS) : "memory");
-        if (tid == 0) {
+        if (warp == 0) {
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const int g = n / SY_FL;
-            const uint32_t d = tmem + (uint32_t)(g & 1) * 256u;
-            uint32_t accum = (n - g * SY_FL) ? 1u : 0u;
-            const uint32_t sa = sm_base + (uint32_t)st * SY_STAGE_BYTES;
-            const uint64_t a1 = sy_desc(sa, SY_T * 16), a2 = sy_desc(sa + SY_A_BYTES, SY_T * 16);
-            const uint64_t bd = sy_desc(sa + 2 * SY_A_BYTES, 2 * SY_T * 16);
+            if (sy_elect_one()) {
+                const int g = n / SY_FL;
+                const uint32_t d = tmem + (uint32_t)(g & 1) * 256u;
+                uint32_t accum = (n - g * SY_FL) ? 1u : 0u;
+                const uint32_t sa = sm_base + (uint32_t)st * SY_STAGE_BYTES;
+                const uint32_t desc_hi = (128u >> 4) | (1u << 14);
+                const uint32_t a1 = ((sa >> 4) & 0x3FFFu) | ((((uint32_t)(SY_T * 16) >> 4) & 0x3FFFu) << 16);
+                const uint32_t a2 = (((sa + SY_A_BYTES) >> 4) & 0x3FFFu) | ((((uint32_t)(SY_T * 16) >> 4) & 0x3FFFu) << 16);
+                const uint32_t bd = (((sa + 2 * SY_A_BYTES) >> 4) & 0x3FFFu) | ((((uint32_t)(2 * SY_T * 16) >> 4) & 0x3FFFu) << 16);
 #pragma unroll
-            for (int ks = 0; ks < SY_KC / 16; ++ks) {
-                const uint64_t astep = (uint64_t)((ks * 2 * SY_T * 16) >> 4), bstep = (uint64_t)((ks * 4 * SY_T * 16) >> 4);
-                sy_mma(d, a1 + astep, bd + bstep, idesc256, accum);        // hi.hi | hi.lo
-                sy_mma(d, a2 + astep, bd + bstep, idesc128, 1u);           // lo.hi into columns 0..127
-                accum = 1u;
+                for (int ks = 0; ks < SY_KC / 16; ++ks) {
+                    const uint32_t astep = (uint32_t)((ks * 2 * SY_T * 16) >> 4), bstep = (uint32_t)((ks * 4 * SY_T * 16) >> 4);
+                    sy_mma_lo(d, a1 + astep, bd + bstep, desc_hi, idesc256, accum);     // hi.hi | hi.lo
+                    sy_mma_lo(d, a2 + astep, bd + bstep, desc_hi, idesc128, 1u);        // lo.hi into columns 0..127
+                    accum = 1u;
+                }
+                sy_commit(sy_smem_u32(&s_bar[st]));
             }
-            sy_commit(sy_smem_u32(&s_bar[st]));
+            __syncwarp();
         }
     }
     asm volatile("cp.async.wait_group 0;\n" ::: "memory");
