@@ -81,7 +81,7 @@ __global__ void __launch_bounds__(32 * PX_BLUR_WARPS) pixsrc_blur_kernel(const i
     // 2^30 / S cannot overflow; each of the <= K^2 terms is rounded to S 2^-31: |error| <= K^2 S 2^-31 (2e-7 S for a 21 x 21 PSF,
     // at the level of the 22-bit operands the contraction makes of f).  Measured: 10.5 -> 5.2 ms per 296 vectors at N_s = 1024; a
     // second word per entry that carries the remainders in units of S 2^-50 (f then exact to fp32 rounding; 9.9 ms) gives the same
-    // errors against the oracle (ln evidence 4.9e-8 on C2 32 x 32; 1.6e-5 on the ill-conditioned C1 32 x 20 case, float atomics 9e-6:
+    // errors against the fp64 definition in the parity tests (ln evidence 4.9e-8 on C2 32 x 32; 1.6e-5 on the ill-conditioned C1 32 x 20 case, float atomics 9e-6:
     // the contraction's operands, not this rounding, set them), so one word is kept.
     extern __shared__ int px_rows[];
     const int b = blockIdx.y, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
