@@ -261,6 +261,8 @@ __device__ __noinline__ void cusp_mass_const(const float* __restrict__ p, double
 // the cusp guard keeps only its lens light here and is put on the list for src_pixel_fp64 (or, if the list is full, done at once).
 template <bool CH>
 __device__ __noinline__ float src_pixel_fp64(const float* __restrict__ c, const glad_image_grid& g, const MassConst& m, int ix, int iy);
+template <bool CH>
+__device__ __noinline__ float src_ray_fp64(const float* __restrict__ c, const glad_image_grid& g, const MassConst& m, int ix, int iy, int r);
 
 template <bool CH, bool LONG>
 __device__ __forceinline__ void ray_pass(const float* __restrict__ c, const glad_image_grid& g, float* __restrict__ img, int pitch,
@@ -308,19 +310,22 @@ __device__ __noinline__ void ray_pass_long(const float* __restrict__ c, const gl
 // profile itself in fp32.  Only the Sersic source reaches this (a Chameleon source has a core).
 template <bool CH>
 __device__ __noinline__ float src_pixel_fp64(const float* __restrict__ c, const glad_image_grid& g, const MassConst& m, int ix, int iy) {
-    const float* o = c + LC_SERSIC0;
     const int ss = g.supersample;
     float sum = 0.f;
-    for (int sb = 0; sb < ss; ++sb)
-        for (int sa = 0; sa < ss; ++sa) {
-            const double thx = (double)g.x0 + (double)g.pix * ((double)ix + (((double)sa + 0.5) / ss - 0.5));
-            const double thy = (double)g.y0 + (double)g.pix * ((double)iy + (((double)sb + 0.5) / ss - 0.5));
-            MassEval e;
-            mass_eval(m, thx, thy, e);
-            bool dummy;
-            sum += sersic_at(o, (float)(thx - e.ax - (double)o[0]), (float)(thy - e.ay - (double)o[1]), dummy);
-        }
+    for (int r = 0; r < ss * ss; ++r) sum += src_ray_fp64<CH>(c, g, m, ix, iy, r);
     return sum;
+}
+// one of the s x s rays of the pixel: r = sb * s + sa
+template <bool CH>
+__device__ __noinline__ float src_ray_fp64(const float* __restrict__ c, const glad_image_grid& g, const MassConst& m, int ix, int iy, int r) {
+    const float* o = c + LC_SERSIC0;
+    const int ss = g.supersample, sb = r / ss, sa = r - sb * ss;
+    const double thx = (double)g.x0 + (double)g.pix * ((double)ix + (((double)sa + 0.5) / ss - 0.5));
+    const double thy = (double)g.y0 + (double)g.pix * ((double)iy + (((double)sb + 0.5) / ss - 0.5));
+    MassEval e;
+    mass_eval(m, thx, thy, e);
+    bool dummy;
+    return sersic_at(o, (float)(thx - e.ax - (double)o[0]), (float)(thy - e.ay - (double)o[1]), dummy);
 }
 
 template <bool CH>
@@ -371,13 +376,25 @@ __global__ void __launch_bounds__(512, 2) lens_image_kernel(const float* __restr
     else ray_pass<CH, false>(c, g, img, pitch, HL, nterms, kinds, cse, ncse, s_cusp, &s_ncusp, s_mc);
     __syncthreads();
     {
-        // cusp guard: the listed pixels get their source light from fp64 rays; one thread per pixel, so no atomics and a result that
-        // does not depend on the order of the list
+        // cusp guard: the listed pixels get their source light from fp64 rays.  LP = 4 or 8 neighbouring lanes share a pixel, one
+        // ray (or two) each, and add up by shuffles: no atomics, a result that does not depend on the order of the list, and the
+        // few hundred listed pixels keep the whole CTA busy (one thread per pixel left most of it idle behind a chain of s^2 fp64
+        // ray evaluations: a tenth of the kernel)
         const int nc = min(s_ncusp, LENS_CUSP_LIST);
-        const float inv_s2 = 1.f / (float)(g.supersample * g.supersample);
-        for (int i = tid; i < nc; i += nthr) {
-            const int p = s_cusp[i], iy = p / nx, ix = p - iy * nx;
-            img[iy * pitch + HL + ix] += src_pixel_fp64<CH>(c, g, s_mc, ix, iy) * inv_s2;
+        const int R = g.supersample * g.supersample, LP = R <= 4 ? 4 : 8;
+        const float inv_s2 = 1.f / (float)R;
+        const int lr = tid & (LP - 1), per_pass = nthr / LP;
+        for (int base = 0; base < nc; base += per_pass) {                   // trip count is CTA-uniform
+            const int e = base + tid / LP;
+            float sum = 0.f;
+            int iy = 0, ix = 0;
+            if (e < nc) {
+                const int p = s_cusp[e];
+                iy = p / nx; ix = p - iy * nx;
+                for (int r = lr; r < R; r += LP) sum += src_ray_fp64<CH>(c, g, s_mc, ix, iy, r);
+            }
+            for (int o = LP >> 1; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+            if (e < nc && lr == 0) img[iy * pitch + HL + ix] += sum * inv_s2;
         }
         __syncthreads();
     }
