@@ -94,13 +94,16 @@ __global__ void __launch_bounds__(32 * PX_BLUR_WARPS) pixsrc_blur_kernel(const i
     const int p0 = blockIdx.x * rows_per_cta;
     for (int i = lane; i < ns; i += 32) row[i] = 0;        // the row is all zero between pixels: the written range is cleared after use
     __syncwarp();
+    const int sdy = 32 / kpsf, sdx = 32 - sdy * kpsf;
     for (int r = warp; r < rows_per_cta; r += PX_BLUR_WARPS) {
         const int p = p0 + r;
         if (p >= npix) break;
         const int iy = p / nx, ix = p - iy * nx;
         int lo = 0x7fffffff, hi = -1;             // first and last source pixel this row touches (row-major index)
-        for (int t = lane; t < k2; t += 32) {
-            const int dy = t / kpsf, dx = t - dy * kpsf;
+        // tap t = lane, lane + 32, ..: (dy, dx) is carried, not divided (32 = sdy * kpsf + sdx)
+        int dy = lane / kpsf, dx = lane - dy * kpsf;
+        for (int t = lane; t < k2; t += 32, dy += sdy, dx += sdx) {
+            if (dx >= kpsf) { dx -= kpsf; ++dy; }
             const int sy = iy - (dy - cc), sx = ix - (dx - cc);
             if (sy < 0 || sy >= ny || sx < 0 || sx >= nx) continue;
             const int q = sy * nx + sx;
